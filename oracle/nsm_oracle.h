@@ -1,0 +1,152 @@
+/*
+ * nsm_oracle.h — float64 CPU ORACLE of the NeRF-SLAM mapping step (arxiv 2210.13641).
+ *
+ * TEST INFRASTRUCTURE ONLY.  Only tests/, __graft_entry__.smoke() and bench.py's
+ * cpu_baseline / --impl reference legs may build, load or call this.  It shares no code,
+ * header, table or constant generator with the CUDA path (paper_2210_13641_b200/csrc); the
+ * product never links or imports it.
+ *
+ * What it computes (PAPER.md = /root/reference/PAPER.md, DESIGN.md "Readings" = R-numbers):
+ *   S0  level tables                      DESIGN.md R11 (PAPER.md:65,167 delegate to [17])
+ *   S1  candidate samples t, delta, x     PAPER.md:139,143 (Eq. 5 text), R6, R14
+ *   S2  occupancy test                    R17 (paper silent)
+ *   S3  compaction in (ray,k) order       BASELINE.json north_star
+ *   S4  multiresolution hash encoding     PAPER.md:65,143,167 -> [17]; R11
+ *   S5  density MLP, sigma = exp(g0)      PAPER.md:143; R10
+ *   S6  spherical-harmonics direction enc R9
+ *   S7  colour MLP, sigmoid               PAPER.md:151; R8, R10
+ *   S8  transmittance + compositing       PAPER.md:141 (Eq. 5), 145 (Eq. 6), 151
+ *   S9  loss L_M = L_rgb + lambda_D L_D   PAPER.md:130 (Eq. 3), 137 (Eq. 4), 149 (Eq. 7); R2, R4, R13
+ *   S10-S12 backward (analytic derivative of the above, written out)
+ *   S13 Adam                              R16 (paper names no optimiser)
+ *   S14 occupancy from field              R17
+ *   S15 render with transmittance cut     PAPER.md:163; R15
+ *
+ * Precision: the INDEX PATH (everything that decides an integer, and the fp32 quantities
+ * t, delta, x, w) is a fixed sequence of IEEE binary32 operations (compile with
+ * -ffp-contract=off; fmaf where an fma is specified).  The VALUE PATH is float64.
+ *
+ * Pins (tests/test_oracle_*.py): level tables printed in SURVEY.md section 8, hand-computed hash
+ * slots, partition of unity / affine reproduction of the trilinear interpolation, SH
+ * orthonormality by quadrature and the addition theorem, compositing closed forms
+ * (constant-density slab, opaque shell), loss special cases, central finite differences on
+ * every parameter of a tiny field, an independent float64 torch-autograd restatement, and
+ * torch.optim.Adam.  Parity unpinned: none of the paper's printed numbers (Table 1, fps)
+ * concern this path; the jitter hash's statistical quality and the Adam hyper-parameters are
+ * conventions fixed in DESIGN.md.
+ */
+#ifndef NSM_ORACLE_H
+#define NSM_ORACLE_H
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct {
+  float    aabb_min[3];
+  float    aabb_extent;
+  uint32_t n_levels, n_features, log2_table_size, n_min, n_max;
+  uint32_t occ_res;
+  uint32_t density_hidden, density_out;
+  uint32_t geo_offset, geo_count;
+  uint32_t sh_degree;
+  uint32_t color_hidden, color_hidden_layers;
+  float    bg[3];
+  float    occ_sigma_threshold;
+  float    lr, beta1, beta2, eps;
+  uint32_t sparse_table_adam;
+  uint64_t seed;
+} orc_config;
+
+typedef struct {
+  uint32_t     n_rays;
+  const float *origins, *dirs;      /* [R,3] */
+  const float *rgb;                 /* [R,3] */
+  const float *depth, *depth_var;   /* [R] */
+  float        t_min, t_max;
+  uint32_t     n_candidates;        /* K */
+} orc_batch;
+
+typedef struct {
+  double   loss, loss_rgb, loss_depth;
+  uint64_t n_samples;
+  uint32_t n_rays, step;
+} orc_stats;
+
+/* Optional outputs of one step; any pointer may be NULL.  Capacities are the caller's duty:
+ * per-sample arrays hold R*K entries, per-ray arrays R. */
+typedef struct {
+  uint32_t *counts;      /* [R]    n_r */
+  uint32_t *offsets;     /* [R+1]  exclusive scan */
+  uint32_t *s_ray, *s_k; /* [S] */
+  float    *s_t, *s_delta, *s_x; /* [S], [S], [S,3]  index-path fp32 outputs */
+  uint32_t *slots;       /* [S, L, 8]  table slot of every corner (corner bit0=x, bit1=y, bit2=z) */
+  float    *w;           /* [S, L, 3]  trilinear fractions */
+  double   *e;           /* [S, L*F] */
+  double   *sigma;       /* [S] */
+  double   *rgb;         /* [S,3] */
+  double   *C, *D_hat, *O; /* [R,3], [R], [R] */
+  double   *dsigma, *drgb; /* [S], [S,3]  dL/dsigma_i, dL/dc_i */
+  double   *grad;        /* [P]  canonical flat layout: tables then MLP matrices */
+  uint8_t  *touched;     /* [n_entries]  1 if the (level,slot) entry was referenced this step */
+} orc_trace;
+
+/* S0.  res[L], offset[L+1] (in entries).  Returns 0, or -1 on a bad config. */
+int orc_level_table(const orc_config *cfg, uint32_t *res, uint64_t *offset);
+/* Parameter counts: table floats (= F * sum E_l) and MLP floats. */
+int orc_param_count(const orc_config *cfg, uint64_t *n_table, uint64_t *n_mlp);
+/* Offsets (in floats, relative to the start of the MLP block) of W_d1, W_d2, W_c1, [W_c2,] W_c3
+ * and the end; out has color_hidden_layers + 4 entries. */
+int orc_mlp_offsets(const orc_config *cfg, uint64_t *out);
+
+/* S1.1: jitter hash -> 24-bit uniform in [0,1). */
+uint32_t orc_hash32(uint64_t seed, uint32_t step, uint32_t r, uint32_t k);
+float    orc_jitter_u(uint64_t seed, uint32_t step, uint32_t r, uint32_t k);
+
+/* S1-S3.  jitter=0 => u == 0.5.  step = the 1-based step about to be taken.  Returns S (or -1). */
+int64_t orc_march(const orc_config *cfg, const uint8_t *bits, const orc_batch *b, int jitter,
+                  uint32_t step, uint32_t *counts, uint32_t *offsets, uint32_t *s_ray,
+                  uint32_t *s_k, float *s_t, float *s_delta, float *s_x);
+
+/* S4 for S points x[S,3] in [0,1)^3.  slots/w may be NULL. */
+int orc_encode(const orc_config *cfg, const double *theta, uint64_t S, const float *x,
+               uint32_t *slots, float *w, double *e);
+
+/* S6: n*n real orthonormal SH of the unit vector d. */
+void orc_sh(uint32_t n, const double d[3], double *Y);
+
+/* S5+S7 for one sample: e[L*F], Y[n*n] -> sigma, rgb[3] (theta_mlp = start of the MLP block). */
+int orc_field_eval(const orc_config *cfg, const double *theta_mlp, const double *e, const double *Y,
+                   double *sigma, double *rgb);
+
+/* S8 for one ray: n samples (sigma, rgb[n,3], t, delta) -> C[3], D_hat, O.  cut<=0: none (S15). */
+void orc_composite(uint32_t n, const double *sigma, const double *rgb, const float *t,
+                   const float *delta, const float bg[3], double cut, double *C, double *D_hat,
+                   double *O);
+
+/* S1-S13: one training step.  theta/m/v: [P] float64 state, updated in place iff apply_adam.
+ * *step_inout is the number of steps already taken; incremented iff apply_adam. */
+int orc_train_step(const orc_config *cfg, double *theta, double *m, double *v, uint32_t *step_inout,
+                   const uint8_t *bits, const orc_batch *b, double lambda_d, int jitter,
+                   int apply_adam, orc_stats *stats, orc_trace *trace);
+
+/* S13 alone: one Adam step on n parameters given gradient g; mask (may be NULL) selects entries. */
+void orc_adam(uint64_t n, double *theta, double *m, double *v, const double *g, const uint8_t *mask,
+              uint32_t mask_group, uint32_t step, double lr, double beta1, double beta2, double eps);
+
+/* S14 FROM_FIELD: bits_out has G^3/8 bytes.  sigma_out (may be NULL) gets G^3 densities. */
+int orc_occupancy_from_field(const orc_config *cfg, const double *theta, uint8_t *bits_out,
+                             double *sigma_out);
+
+/* S15. */
+int orc_render(const orc_config *cfg, const double *theta, const uint8_t *bits, const orc_batch *b,
+               double cut, double *rgb, double *depth, double *opacity, uint64_t *n_samples);
+
+/* Threads the library will use (1 unless built with -fopenmp). */
+int orc_num_threads(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif
