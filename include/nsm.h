@@ -1,0 +1,184 @@
+/*
+ * nsm.h — C-ABI boundary of the B200-native NeRF-SLAM mapping step ("nsm").
+ *
+ * One thing is behind this header: the radiance-field training step of NeRF-SLAM's mapping
+ * thread (arxiv 2210.13641; PAPER.md = the paper text) and its forward-only render, as
+ * hand-written CUDA for sm_100a.  PAPER.md section 3.2 defines what is minimised:
+ *
+ *     L_M(T, Theta) = L_rgb + lambda_D * L_D                      (Eq. 3)
+ *     L_D   = || D - D*(T,Theta) ||^2_{Sigma_D}                    (Eq. 4)
+ *     d*    = sum_i T_i (1 - exp(-sigma_i delta_i)) d_i            (Eq. 5)
+ *     T_i   = exp(- sum_{j<i} sigma_j delta_j)                     (Eq. 6)
+ *     L_rgb = || I - I*(T,Theta) ||^2                              (Eq. 7)
+ *
+ * with the field (hash-grid encoding + density MLP + colour MLP) delegated to Instant-NGP
+ * (PAPER.md:143, 167).  The readings of everything the paper leaves open are in DESIGN.md
+ * ("Readings", R1..R22) and the step-by-step algorithm S0..S15 in DESIGN.md "Algorithm".
+ *
+ * Conventions
+ *   - Plain C types only.  Every pointer in nsm_ray_batch and every d_* argument is a DEVICE
+ *     pointer owned by the caller (e.g. torch.Tensor.data_ptr()); the *_host entry points take
+ *     HOST pointers instead and perform the copies themselves.  The library never retains a
+ *     caller pointer past the call.
+ *   - The field owns parameters, Adam state, occupancy bits and workspace.
+ *   - All work is enqueued on the CUDA stream given at creation; calls return without
+ *     synchronising unless a host stats pointer is passed (one sync to fill it) or the entry
+ *     point takes host buffers.
+ *   - Every entry point returns an nsm_status; nsm_last_error() gives a thread-local message.
+ *     Arguments are validated before anything is launched: a failed call leaves the field
+ *     unchanged.  There is no CPU fallback: without a CUDA device nsm_create_field fails with
+ *     NSM_ERR_CUDA.
+ *   - Canonical layouts (what getters, setters and the oracle agree on):
+ *       table parameter   theta[(offset_l + slot) * F + f]
+ *       MLP matrices      row-major [out][in], in the order W_d1, W_d2, W_c1, (W_c2,) W_c3,
+ *                         appended after the tables
+ *       occupancy bit     i = gx + G*(gy + G*gz) is bit (i & 7) of byte (i >> 3)
+ *       samples           ordered by (ray, candidate k)
+ */
+#ifndef NSM_H
+#define NSM_H
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct nsm_field nsm_field; /* opaque */
+
+typedef enum {
+  NSM_OK = 0,
+  NSM_ERR_INVALID_ARG = 1,
+  NSM_ERR_OOM = 2,
+  NSM_ERR_CUDA = 3,
+  NSM_ERR_CAPACITY = 4,
+  NSM_ERR_UNIMPLEMENTED = 5
+} nsm_status;
+
+/* Arithmetic of the two MLPs (S5, S7, S11).  FP32: CUDA-core fp32 throughout.  FP16 / BF16:
+ * 16-bit operands on the tcgen05 tensor cores with fp32 accumulation. */
+typedef enum { NSM_MLP_FP32 = 0, NSM_MLP_FP16 = 1, NSM_MLP_BF16 = 2 } nsm_precision;
+
+/* S14. */
+typedef enum { NSM_OCC_FULL = 0, NSM_OCC_SET = 1, NSM_OCC_FROM_FIELD = 2 } nsm_occ_mode;
+
+typedef struct {
+  uint32_t struct_size;              /* sizeof(nsm_field_config), ABI check */
+  float    aabb_min[3], aabb_extent; /* cube: x = (p - aabb_min) / aabb_extent in [0,1)^3 */
+  uint32_t n_levels, n_features;     /* L <= 32, F in {1,2,4,8} */
+  uint32_t log2_table_size;          /* T = 2^log2_table_size entries per hashed level */
+  uint32_t n_min, n_max;             /* coarsest / finest resolution (S0) */
+  uint32_t occ_res;                  /* G, power of two, G^3 bits */
+  uint32_t density_hidden, density_out;   /* one hidden layer; density_out <= 16 */
+  uint32_t geo_offset, geo_count;    /* slice of the density output fed to the colour MLP */
+  uint32_t sh_degree;                /* n -> n*n real SH coefficients, n <= 4 */
+  uint32_t color_hidden, color_hidden_layers; /* 1 or 2 hidden layers */
+  uint32_t mlp_precision;            /* nsm_precision */
+  float    bg[3];                    /* background colour (R12) */
+  float    occ_sigma_threshold;      /* FROM_FIELD: bit = sigma > threshold */
+  float    lr, beta1, beta2, eps;    /* Adam (S13) */
+  uint32_t sparse_table_adam;        /* 1: only table entries touched this step are updated */
+  uint32_t jitter;                   /* 1: per-(ray,bin) stratified jitter in training (S1) */
+  uint64_t seed;                     /* jitter stream */
+  uint32_t max_rays, max_candidates; /* workspace capacity per call / per render chunk */
+} nsm_field_config;
+
+typedef struct {
+  uint32_t     n_rays;               /* R */
+  const float *origins, *dirs;       /* [R,3] row-major fp32; dirs unit length (R5) */
+  const float *rgb;                  /* [R,3] target colour in [0,1]; NULL for render */
+  const float *depth;                /* [R] SLAM depth as range along the ray; <= 0: no depth term */
+  const float *depth_var;            /* [R] variance Sigma_D; <= 0 or non-finite: no depth term */
+  float        t_min, t_max;         /* candidate lattice: dt = (t_max - t_min) / K */
+  uint32_t     n_candidates;         /* K */
+} nsm_ray_batch;
+
+typedef struct {
+  double   loss, loss_rgb, loss_depth; /* L_M, L_rgb, L_D of Eqs. 3, 7, 4 (means over the batch) */
+  uint64_t n_samples;                  /* S, live samples this step */
+  uint32_t n_rays, step;               /* step = number of Adam steps taken so far */
+} nsm_step_stats;
+
+/* Items nsm_debug_last_step can copy out (state left by the last backward / train / render). */
+typedef enum {
+  NSM_DBG_COUNTS = 0,    /* u32 [R]        n_r */
+  NSM_DBG_OFFSETS = 1,   /* u32 [R+1]      exclusive scan; [R] = S */
+  NSM_DBG_SAMPLE_RAY = 2,/* u32 [S] */
+  NSM_DBG_SAMPLE_K = 3,  /* u32 [S] */
+  NSM_DBG_SAMPLE_T = 4,  /* f32 [S] */
+  NSM_DBG_SAMPLE_DELTA = 5, /* f32 [S] */
+  NSM_DBG_SAMPLE_X = 6,  /* f32 [S,3] */
+  NSM_DBG_SLOTS = 7,     /* u32 [S,L,8]    corner bit0=x, bit1=y, bit2=z */
+  NSM_DBG_W = 8,         /* f32 [S,L,3] */
+  NSM_DBG_E = 9,         /* f32 [S,L*F] */
+  NSM_DBG_SIGMA = 10,    /* f32 [S] */
+  NSM_DBG_RGB = 11,      /* f32 [S,3] */
+  NSM_DBG_C = 12,        /* f32 [R,3] */
+  NSM_DBG_D_HAT = 13,    /* f32 [R] */
+  NSM_DBG_O = 14,        /* f32 [R] */
+  NSM_DBG_DSIGMA = 15,   /* f32 [S] */
+  NSM_DBG_DRGB = 16,     /* f32 [S,3] */
+  NSM_DBG_GRAD = 17,     /* f32 [P]        canonical layout; valid after nsm_backward */
+  NSM_DBG_TOUCHED = 18   /* u8  [n_entries] valid after nsm_backward */
+} nsm_debug_item;
+
+/* Create a field on the current CUDA device.  cuda_stream: a cudaStream_t (NULL = default
+ * stream).  Parameters start at zero (tables) / zero (MLPs): upload theta_0 with
+ * nsm_set_params.  Occupancy starts FULL.  Fails with NSM_ERR_INVALID_ARG on a bad config,
+ * NSM_ERR_UNIMPLEMENTED on an unsupported shape, NSM_ERR_OOM / NSM_ERR_CUDA otherwise. */
+nsm_status nsm_create_field(const nsm_field_config *cfg, void *cuda_stream, nsm_field **out);
+void       nsm_destroy_field(nsm_field *f);
+
+/* S14.  SET: d_bits = G^3/8 bytes (device) in the canonical layout.  FULL: all ones.
+ * FROM_FIELD: bit = sigma(cell centre) > occ_sigma_threshold from the current parameters. */
+nsm_status nsm_update_occupancy(nsm_field *f, nsm_occ_mode mode, const uint8_t *d_bits);
+/* Copy the current G^3/8 occupancy bytes to d_bits (device). */
+nsm_status nsm_get_occupancy(nsm_field *f, uint8_t *d_bits);
+
+/* S1-S13: one training step of L_M (Eq. 3) on a ray batch: march, encode, MLPs, composite
+ * (Eqs. 5, 6), loss (Eqs. 3, 4, 7), backward, Adam.  host_stats may be NULL (no sync). */
+nsm_status nsm_train_step(nsm_field *f, const nsm_ray_batch *batch, float lambda_d,
+                          nsm_step_stats *host_stats);
+/* The same with HOST pointers in *batch: inputs are copied host->device inside the call. */
+nsm_status nsm_train_step_host(nsm_field *f, const nsm_ray_batch *host_batch, float lambda_d,
+                               nsm_step_stats *host_stats);
+
+/* S1-S12 only: forward + backward, gradients left in place for nsm_debug_last_step; and S13
+ * alone on the gradients in place.  nsm_train_step == nsm_backward + nsm_apply_adam. */
+nsm_status nsm_backward(nsm_field *f, const nsm_ray_batch *batch, float lambda_d,
+                        nsm_step_stats *host_stats);
+nsm_status nsm_apply_adam(nsm_field *f);
+/* Overwrite the gradient buffer / touched flags (device pointers, canonical layouts). */
+nsm_status nsm_debug_set_grad(nsm_field *f, const float *d_grad, const uint8_t *d_touched);
+
+/* S15: forward-only render, u == 0.5, a ray stops after T < transmittance_cut (0 = never).
+ * d_rgb [R,3], d_depth [R], d_opacity [R] or NULL.  R may exceed max_rays (chunked). */
+nsm_status nsm_render(nsm_field *f, const nsm_ray_batch *batch, float transmittance_cut,
+                      float *d_rgb, float *d_depth, float *d_opacity);
+nsm_status nsm_render_host(nsm_field *f, const nsm_ray_batch *host_batch, float transmittance_cut,
+                           float *h_rgb, float *h_depth, float *h_opacity);
+
+/* Parameter access (canonical flat layout; device pointers; any of d_theta/d_m/d_v/step may
+ * be NULL). */
+nsm_status nsm_param_count(const nsm_field *f, uint64_t *n_table, uint64_t *n_mlp);
+nsm_status nsm_get_params(nsm_field *f, float *d_theta, float *d_m, float *d_v, uint32_t *step);
+nsm_status nsm_set_params(nsm_field *f, const float *d_theta, const float *d_m, const float *d_v,
+                          uint32_t step);
+/* S0 tables: res[L] resolutions, offset[L+1] entry offsets (host pointers). */
+nsm_status nsm_get_level_table(const nsm_field *f, uint32_t *res, uint64_t *offset);
+
+/* Copy a debug item of the last step to d_out (device); fails with NSM_ERR_CAPACITY if
+ * capacity_bytes is too small.  *n_bytes_out (may be NULL) receives the item's size. */
+nsm_status nsm_debug_last_step(nsm_field *f, int item, void *d_out, uint64_t capacity_bytes,
+                               uint64_t *n_bytes_out);
+
+/* Number of this library's kernels launched by this field so far (bench.py's gpu_launches). */
+uint64_t    nsm_launch_count(const nsm_field *f);
+/* Which MLP path the field runs: "simt_fp32", "tcgen05_f16", "tcgen05_bf16". */
+const char *nsm_mlp_path(const nsm_field *f);
+const char *nsm_last_error(void);
+const char *nsm_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif

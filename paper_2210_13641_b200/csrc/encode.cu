@@ -1,0 +1,214 @@
+// encode.cu — S4 (multiresolution hash-grid encoding, forward gather) and S12 (table-gradient
+// scatter) of DESIGN.md "Algorithm".  PAPER.md:65,143,167 delegate the encoding to [17]; the
+// vertex grid, dense-vs-hashed rule and XOR-of-products hash are readings R11.
+//
+// Work decomposition: one thread per (level, sample), level-major, so that a warp holds 32
+// consecutive samples (neighbours along a ray) of ONE level: their corners share cache lines at
+// coarse levels, the whole chip works on one level's table slice at a time (L2/L1 locality), and
+// the feature planes e[l*F+f][s] are written / read fully coalesced.
+#include "nsm_internal.cuh"
+
+namespace {
+
+struct CornerIndex {
+  uint32_t slot[8];
+  float w[3];
+};
+
+// Index path of S4 (fp32 ops explicit; integers bit-exact against the oracle).
+__device__ __forceinline__ CornerIndex corner_index(const LevelTable &lv, uint32_t l, float x0,
+                                                    float x1, float x2) {
+  CornerIndex ci;
+  const uint32_t N = lv.res[l];
+  const float Nf = __uint2float_rn(N);
+  uint32_t c0[3];
+  const float x[3] = {x0, x1, x2};
+#pragma unroll
+  for (int a = 0; a < 3; ++a) {
+    float pos = __fmul_rn(x[a], Nf);
+    int c = min(__float2int_rd(pos), (int)N - 1);
+    c = max(c, 0);
+    c0[a] = (uint32_t)c;
+    ci.w[a] = __fsub_rn(pos, __int2float_rn(c));
+  }
+  if (lv.dense[l]) {
+    const uint32_t side = N + 1;
+#pragma unroll
+    for (uint32_t k = 0; k < 8; ++k)
+      ci.slot[k] = (c0[0] + (k & 1u)) + side * ((c0[1] + ((k >> 1) & 1u)) + side * (c0[2] + ((k >> 2) & 1u)));
+  } else {
+#pragma unroll
+    for (uint32_t k = 0; k < 8; ++k)
+      ci.slot[k] = ((c0[0] + (k & 1u)) ^ ((c0[1] + ((k >> 1) & 1u)) * 2654435761u) ^
+                    ((c0[2] + ((k >> 2) & 1u)) * 805459861u)) & lv.t_mask;
+  }
+  return ci;
+}
+
+__device__ __forceinline__ float corner_weight(uint32_t k, const float w[3]) {
+  float a = (k & 1u) ? w[0] : 1.0f - w[0];
+  float b = (k & 2u) ? w[1] : 1.0f - w[1];
+  float c = (k & 4u) ? w[2] : 1.0f - w[2];
+  return a * b * c;
+}
+
+template <int F> struct Vec;
+template <> struct Vec<1> { using T = float; };
+template <> struct Vec<2> { using T = float2; };
+template <> struct Vec<4> { using T = float4; };
+
+template <int F>
+__device__ __forceinline__ void load_entry(const float *p, float out[F]) {
+  if constexpr (F == 8) {
+    float4 a = __ldg(reinterpret_cast<const float4 *>(p)), b = __ldg(reinterpret_cast<const float4 *>(p) + 1);
+    out[0] = a.x; out[1] = a.y; out[2] = a.z; out[3] = a.w;
+    out[4] = b.x; out[5] = b.y; out[6] = b.z; out[7] = b.w;
+  } else if constexpr (F == 4) {
+    float4 a = __ldg(reinterpret_cast<const float4 *>(p));
+    out[0] = a.x; out[1] = a.y; out[2] = a.z; out[3] = a.w;
+  } else if constexpr (F == 2) {
+    float2 a = __ldg(reinterpret_cast<const float2 *>(p));
+    out[0] = a.x; out[1] = a.y;
+  } else {
+    out[0] = __ldg(p);
+  }
+}
+
+template <int F>
+__global__ void __launch_bounds__(256) encode_forward_kernel(LevelTable lv, const float *__restrict__ theta,
+                                                             Workspace ws, const uint32_t *__restrict__ d_S) {
+  const uint64_t S = *d_S;
+  const uint64_t total = S * lv.n_levels;
+  for (uint64_t wi = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; wi < total;
+       wi += (uint64_t)gridDim.x * blockDim.x) {
+    const uint32_t l = (uint32_t)(wi / S);
+    const uint64_t s = wi - (uint64_t)l * S;
+    CornerIndex ci = corner_index(lv, l, ws.s_x[s], ws.s_x[ws.cap + s], ws.s_x[2 * ws.cap + s]);
+    const float *tab = theta + lv.offset[l] * F;
+    float v[8][F];
+#pragma unroll
+    for (int k = 0; k < 8; ++k) load_entry<F>(tab + (size_t)ci.slot[k] * F, v[k]);  // 8 gathers in flight
+    float acc[F];
+#pragma unroll
+    for (int f = 0; f < F; ++f) acc[f] = 0.0f;
+#pragma unroll
+    for (int k = 0; k < 8; ++k) {
+      float om = corner_weight(k, ci.w);
+#pragma unroll
+      for (int f = 0; f < F; ++f) acc[f] = fmaf(om, v[k][f], acc[f]);
+    }
+#pragma unroll
+    for (int f = 0; f < F; ++f) ws.e[(size_t)(l * F + f) * ws.cap + s] = acc[f];
+  }
+}
+
+template <int F>
+__device__ __forceinline__ void red_add_entry(float *p, const float g[F]) {
+  // vectorised no-return reductions (red.global.add.v2/v4.f32, sm_90+)
+  if constexpr (F == 8) {
+    atomicAdd(reinterpret_cast<float4 *>(p), make_float4(g[0], g[1], g[2], g[3]));
+    atomicAdd(reinterpret_cast<float4 *>(p) + 1, make_float4(g[4], g[5], g[6], g[7]));
+  } else if constexpr (F == 4) {
+    atomicAdd(reinterpret_cast<float4 *>(p), make_float4(g[0], g[1], g[2], g[3]));
+  } else if constexpr (F == 2) {
+    atomicAdd(reinterpret_cast<float2 *>(p), make_float2(g[0], g[1]));
+  } else {
+    atomicAdd(p, g[0]);
+  }
+}
+
+// S12: d theta[(offset_l + slot) F + f] += omega * dL/de[l F + f]; the touched set U is marked
+// structurally (every referenced entry), independent of the gradient's value.
+template <int F>
+__global__ void __launch_bounds__(256) scatter_backward_kernel(LevelTable lv, float *__restrict__ grad,
+                                                               uint8_t *__restrict__ touched, Workspace ws,
+                                                               const uint32_t *__restrict__ d_S) {
+  const uint64_t S = *d_S;
+  const uint64_t total = S * lv.n_levels;
+  for (uint64_t wi = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; wi < total;
+       wi += (uint64_t)gridDim.x * blockDim.x) {
+    const uint32_t l = (uint32_t)(wi / S);
+    const uint64_t s = wi - (uint64_t)l * S;
+    CornerIndex ci = corner_index(lv, l, ws.s_x[s], ws.s_x[ws.cap + s], ws.s_x[2 * ws.cap + s]);
+    float de[F];
+#pragma unroll
+    for (int f = 0; f < F; ++f) de[f] = ws.de[(size_t)(l * F + f) * ws.cap + s];
+    float *tab = grad + lv.offset[l] * F;
+    uint8_t *tch = touched + lv.offset[l];
+#pragma unroll
+    for (int k = 0; k < 8; ++k) {
+      float om = corner_weight(k, ci.w);
+      float g[F];
+#pragma unroll
+      for (int f = 0; f < F; ++f) g[f] = om * de[f];
+      red_add_entry<F>(tab + (size_t)ci.slot[k] * F, g);
+      tch[ci.slot[k]] = 1;
+    }
+  }
+}
+
+__global__ void debug_slots_kernel(LevelTable lv, Workspace ws, const uint32_t *__restrict__ d_S,
+                                   uint32_t *slots, float *w) {
+  const uint64_t S = *d_S;
+  const uint64_t total = S * lv.n_levels;
+  for (uint64_t wi = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; wi < total;
+       wi += (uint64_t)gridDim.x * blockDim.x) {
+    const uint32_t l = (uint32_t)(wi / S);
+    const uint64_t s = wi - (uint64_t)l * S;
+    CornerIndex ci = corner_index(lv, l, ws.s_x[s], ws.s_x[ws.cap + s], ws.s_x[2 * ws.cap + s]);
+    if (slots)
+      for (int k = 0; k < 8; ++k) slots[(s * lv.n_levels + l) * 8 + k] = ci.slot[k];
+    if (w)
+      for (int a = 0; a < 3; ++a) w[(s * lv.n_levels + l) * 3 + a] = ci.w[a];
+  }
+}
+
+__global__ void planes_to_rows_kernel(const float *__restrict__ planes, uint64_t cap, uint32_t n_planes,
+                                      const uint32_t *__restrict__ d_S, float *__restrict__ rows) {
+  const uint64_t S = *d_S;
+  const uint64_t total = S * n_planes;
+  for (uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; i < total;
+       i += (uint64_t)gridDim.x * blockDim.x) {
+    uint64_t s = i / n_planes;
+    uint32_t p = (uint32_t)(i - s * n_planes);
+    rows[i] = planes[(size_t)p * cap + s];
+  }
+}
+
+}  // namespace
+
+int launch_encode(const LevelTable &lv, const float *theta, const Workspace &ws, const uint32_t *d_S,
+                  int n_sms, cudaStream_t st) {
+  dim3 grid(n_sms * 8), block(256);
+  switch (lv.n_features) {
+    case 1: encode_forward_kernel<1><<<grid, block, 0, st>>>(lv, theta, ws, d_S); break;
+    case 2: encode_forward_kernel<2><<<grid, block, 0, st>>>(lv, theta, ws, d_S); break;
+    case 4: encode_forward_kernel<4><<<grid, block, 0, st>>>(lv, theta, ws, d_S); break;
+    default: encode_forward_kernel<8><<<grid, block, 0, st>>>(lv, theta, ws, d_S); break;
+  }
+  return 1;
+}
+
+int launch_scatter(const LevelTable &lv, float *grad, uint8_t *touched, const Workspace &ws,
+                   const uint32_t *d_S, int n_sms, cudaStream_t st) {
+  dim3 grid(n_sms * 8), block(256);
+  switch (lv.n_features) {
+    case 1: scatter_backward_kernel<1><<<grid, block, 0, st>>>(lv, grad, touched, ws, d_S); break;
+    case 2: scatter_backward_kernel<2><<<grid, block, 0, st>>>(lv, grad, touched, ws, d_S); break;
+    case 4: scatter_backward_kernel<4><<<grid, block, 0, st>>>(lv, grad, touched, ws, d_S); break;
+    default: scatter_backward_kernel<8><<<grid, block, 0, st>>>(lv, grad, touched, ws, d_S); break;
+  }
+  return 1;
+}
+
+int launch_debug_slots(const LevelTable &lv, const Workspace &ws, const uint32_t *d_S, uint32_t *slots,
+                       float *w, cudaStream_t st) {
+  debug_slots_kernel<<<1024, 256, 0, st>>>(lv, ws, d_S, slots, w);
+  return 1;
+}
+
+int launch_planes_to_rows(const float *planes, uint64_t cap, uint32_t n_planes, const uint32_t *d_S,
+                          float *rows, cudaStream_t st) {
+  planes_to_rows_kernel<<<1024, 256, 0, st>>>(planes, cap, n_planes, d_S, rows);
+  return 1;
+}

@@ -1,0 +1,559 @@
+// nsm_api.cu — the C-ABI boundary (include/nsm.h): argument validation, the field object
+// (parameters, Adam state, occupancy bits, workspace arena) and the host-side step scheduler
+// that enqueues the kernels of S1..S15 on the field's stream.  No arithmetic of the method is
+// done on the host except S0's integer level table and Adam's scalar bias corrections.
+#include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <cstdlib>
+#include <cstring>
+#include <new>
+#include <string>
+#include <vector>
+
+#include "nsm_internal.cuh"
+
+namespace {
+
+thread_local std::string g_err;
+
+nsm_status fail(nsm_status st, const char *fmt, ...) {
+  char buf[512];
+  va_list ap;
+  va_start(ap, fmt);
+  vsnprintf(buf, sizeof buf, fmt, ap);
+  va_end(ap);
+  g_err = buf;
+  return st;
+}
+
+#define CUDA_TRY(expr)                                                                         \
+  do {                                                                                         \
+    cudaError_t e_ = (expr);                                                                   \
+    if (e_ != cudaSuccess)                                                                     \
+      return fail(e_ == cudaErrorMemoryAllocation ? NSM_ERR_OOM : NSM_ERR_CUDA, "%s: %s", #expr, \
+                  cudaGetErrorString(e_));                                                     \
+  } while (0)
+
+}  // namespace
+
+struct nsm_field {
+  nsm_field_config cfg;
+  cudaStream_t stream = nullptr;
+  int n_sms = 148;
+  LevelTable lv;
+  MlpShape ms;
+  FieldParams fp;
+  Workspace ws;
+  std::vector<void *> allocs;
+  uint32_t step = 0;
+  uint64_t launches = 0;
+  bool occ_full = true;
+  bool grads_dirty = false;
+  // state of the last step, for the debug getter
+  uint32_t last_R = 0, last_K = 0;
+  bool last_was_render = false;
+  // staging for the *_host entry points
+  float *stage_dev = nullptr;     // [max_rays * 11]
+  float *stage_out = nullptr;     // render outputs [max_rays * 5]
+  struct HostStats { double acc[2]; uint32_t S; } *pinned = nullptr;
+  const char *mlp_path = "simt_fp32";
+
+  template <typename T>
+  cudaError_t alloc(T **p, size_t n, bool zero = true) {
+    void *q = nullptr;
+    size_t bytes = (n * sizeof(T) + 255) & ~size_t(255);
+    cudaError_t e = cudaMalloc(&q, bytes ? bytes : 256);
+    if (e != cudaSuccess) return e;
+    allocs.push_back(q);
+    *p = (T *)q;
+    if (zero) return cudaMemsetAsync(q, 0, bytes ? bytes : 256, stream);
+    return cudaSuccess;
+  }
+};
+
+namespace {
+
+// S0 — integer level table: N_l = floor(N_min * exp(l ln(N_max/N_min)/(L-1)) + 1e-6) in float64,
+// ends forced; E_l = min((N_l+1)^3, T); dense iff (N_l+1)^3 <= T.
+nsm_status build_levels(const nsm_field_config &c, LevelTable &lv) {
+  const uint32_t L = c.n_levels;
+  const uint64_t T = 1ull << c.log2_table_size;
+  lv.n_levels = L;
+  lv.n_features = c.n_features;
+  lv.t_mask = (uint32_t)(T - 1);
+  lv.offset[0] = 0;
+  for (uint32_t l = 0; l < L; ++l) {
+    uint32_t N;
+    if (l == 0) N = c.n_min;
+    else if (l == L - 1) N = c.n_max;
+    else {
+      double step = std::log((double)c.n_max / (double)c.n_min) / (double)(L - 1);
+      N = (uint32_t)std::floor((double)c.n_min * std::exp(step * (double)l) + 1e-6);
+    }
+    lv.res[l] = N;
+    const uint64_t side = (uint64_t)N + 1, cube = side * side * side;
+    lv.dense[l] = cube <= T;
+    lv.offset[l + 1] = lv.offset[l] + (cube <= T ? cube : T);
+  }
+  return NSM_OK;
+}
+
+nsm_status validate_config(const nsm_field_config *c) {
+  if (!c) return fail(NSM_ERR_INVALID_ARG, "config is NULL");
+  if (c->struct_size != sizeof(nsm_field_config))
+    return fail(NSM_ERR_INVALID_ARG, "struct_size %u != %zu (ABI mismatch)", c->struct_size, sizeof(nsm_field_config));
+  if (!(c->aabb_extent > 0.f) || !std::isfinite(c->aabb_extent)) return fail(NSM_ERR_INVALID_ARG, "aabb_extent must be > 0");
+  if (c->n_levels < 1 || c->n_levels > NSM_MAX_LEVELS) return fail(NSM_ERR_INVALID_ARG, "n_levels out of [1,32]");
+  if (c->n_features != 1 && c->n_features != 2 && c->n_features != 4 && c->n_features != 8)
+    return fail(NSM_ERR_INVALID_ARG, "n_features must be 1, 2, 4 or 8");
+  if (c->log2_table_size < 4 || c->log2_table_size > 28) return fail(NSM_ERR_INVALID_ARG, "log2_table_size out of [4,28]");
+  if (c->n_min < 1 || c->n_max < c->n_min || c->n_max > (1u << 20)) return fail(NSM_ERR_INVALID_ARG, "bad n_min/n_max");
+  if (c->occ_res < 1 || (c->occ_res & (c->occ_res - 1)) || c->occ_res > 1024)
+    return fail(NSM_ERR_INVALID_ARG, "occ_res must be a power of two <= 1024");
+  if (c->density_hidden < 1 || c->density_hidden > 128 || c->density_out < 1 || c->density_out > 16)
+    return fail(NSM_ERR_INVALID_ARG, "density MLP widths out of range");
+  if (c->geo_offset + c->geo_count > c->density_out) return fail(NSM_ERR_INVALID_ARG, "geo slice exceeds density_out");
+  if (c->sh_degree < 1 || c->sh_degree > 4) return fail(NSM_ERR_UNIMPLEMENTED, "sh_degree must be in [1,4]");
+  if (c->color_hidden < 1 || c->color_hidden > 128) return fail(NSM_ERR_INVALID_ARG, "color_hidden out of range");
+  if (c->color_hidden_layers < 1 || c->color_hidden_layers > 2) return fail(NSM_ERR_INVALID_ARG, "color_hidden_layers must be 1 or 2");
+  if (c->n_levels * c->n_features > 128) return fail(NSM_ERR_UNIMPLEMENTED, "L*F > 128 not supported");
+  if (c->mlp_precision > NSM_MLP_BF16) return fail(NSM_ERR_INVALID_ARG, "bad mlp_precision");
+  if (!(c->lr > 0.f) || !(c->beta1 >= 0.f && c->beta1 < 1.f) || !(c->beta2 >= 0.f && c->beta2 < 1.f) || !(c->eps >= 0.f))
+    return fail(NSM_ERR_INVALID_ARG, "bad Adam hyper-parameters");
+  if (c->max_rays < 1 || c->max_candidates < 1 || c->max_candidates > 4096)
+    return fail(NSM_ERR_INVALID_ARG, "bad workspace capacity");
+  if ((uint64_t)c->max_rays * c->max_candidates > (1ull << 31))
+    return fail(NSM_ERR_INVALID_ARG, "max_rays * max_candidates exceeds 2^31");
+  return NSM_OK;
+}
+
+nsm_status validate_batch(const nsm_field *f, const nsm_ray_batch *b, bool train, bool chunked) {
+  if (!f) return fail(NSM_ERR_INVALID_ARG, "field is NULL");
+  if (!b) return fail(NSM_ERR_INVALID_ARG, "batch is NULL");
+  if (!b->origins || !b->dirs) return fail(NSM_ERR_INVALID_ARG, "origins/dirs are NULL");
+  if (train && (!b->rgb || !b->depth || !b->depth_var)) return fail(NSM_ERR_INVALID_ARG, "rgb/depth/depth_var are NULL");
+  if (b->n_rays == 0) return fail(NSM_ERR_INVALID_ARG, "n_rays is 0");
+  if (b->n_candidates == 0) return fail(NSM_ERR_INVALID_ARG, "n_candidates is 0");
+  if (!(b->t_max > b->t_min) || !std::isfinite(b->t_min) || !std::isfinite(b->t_max))
+    return fail(NSM_ERR_INVALID_ARG, "need finite t_min < t_max");
+  if (!chunked && b->n_rays > f->cfg.max_rays) return fail(NSM_ERR_CAPACITY, "n_rays %u > max_rays %u", b->n_rays, f->cfg.max_rays);
+  if (b->n_candidates > f->cfg.max_candidates)
+    return fail(NSM_ERR_CAPACITY, "n_candidates %u > max_candidates %u", b->n_candidates, f->cfg.max_candidates);
+  return NSM_OK;
+}
+
+MarchParams make_march(const nsm_field *f, const nsm_ray_batch *b, uint32_t R, bool jitter, uint32_t step) {
+  MarchParams mp;
+  for (int a = 0; a < 3; ++a) mp.aabb_min[a] = f->cfg.aabb_min[a];
+  mp.inv_extent = 1.0f / f->cfg.aabb_extent;                     // S0 host constant, one fp32 divide
+  mp.t_min = b->t_min;
+  mp.dt = (b->t_max - b->t_min) / (float)b->n_candidates;        // one fp32 subtract, one fp32 divide
+  mp.K = b->n_candidates;
+  mp.G = f->cfg.occ_res;
+  mp.jitter = jitter ? 1u : 0u;
+  mp.step = step;
+  mp.seed = f->cfg.seed;
+  mp.R = R;
+  return mp;
+}
+
+// S1-S8 forward (+ S9-S12 when train): everything up to, but excluding, Adam.
+void enqueue_forward(nsm_field *f, const nsm_ray_batch *b, uint32_t R, bool jitter, uint32_t step) {
+  const uint32_t *d_S = f->ws.offsets + R;
+  MarchParams mp = make_march(f, b, R, jitter, step);
+  f->launches += launch_march(mp, f->occ_full ? nullptr : f->fp.occ_bits, b->origins, b->dirs, f->ws, f->stream);
+  f->launches += launch_encode(f->lv, f->fp.theta, f->ws, d_S, f->n_sms, f->stream);
+  f->launches += launch_mlp_forward_simt(f->ms, f->fp.theta + f->fp.n_table, b->dirs, f->ws, d_S, 0, f->n_sms, f->stream);
+}
+
+nsm_status clear_grads_if_dirty(nsm_field *f) {
+  if (f->grads_dirty) {
+    CUDA_TRY(cudaMemsetAsync(f->fp.grad, 0, sizeof(float) * (f->fp.n_table + f->fp.n_mlp), f->stream));
+    CUDA_TRY(cudaMemsetAsync(f->fp.touched, 0, f->fp.n_entries, f->stream));
+    f->grads_dirty = false;
+  }
+  return NSM_OK;
+}
+
+nsm_status enqueue_backward(nsm_field *f, const nsm_ray_batch *b, float lambda_d) {
+  const uint32_t R = b->n_rays;
+  const uint32_t *d_S = f->ws.offsets + R;
+  nsm_status st = clear_grads_if_dirty(f);
+  if (st != NSM_OK) return st;
+  enqueue_forward(f, b, R, f->cfg.jitter != 0, f->step + 1);
+  f->launches += launch_composite_train(f->ws, R, b->rgb, b->depth, b->depth_var, lambda_d, f->cfg.bg, f->stream);
+  f->launches += launch_mlp_backward_simt(f->ms, f->fp.theta + f->fp.n_table, f->fp.grad + f->fp.n_table, b->dirs,
+                                          f->ws, d_S, f->n_sms, f->stream);
+  f->launches += launch_scatter(f->lv, f->fp.grad, f->fp.touched, f->ws, d_S, f->n_sms, f->stream);
+  f->grads_dirty = true;
+  f->last_R = R;
+  f->last_K = b->n_candidates;
+  f->last_was_render = false;
+  CUDA_TRY(cudaGetLastError());
+  return NSM_OK;
+}
+
+nsm_status enqueue_adam(nsm_field *f) {
+  const uint32_t t = f->step + 1;
+  const double bc1 = 1.0 - std::pow((double)f->cfg.beta1, (double)t);
+  const double bc2 = 1.0 - std::pow((double)f->cfg.beta2, (double)t);
+  f->launches += launch_adam(f->fp, f->cfg.n_features, f->cfg.sparse_table_adam != 0, f->cfg.lr, f->cfg.beta1,
+                             f->cfg.beta2, f->cfg.eps, (float)(1.0 / bc1), (float)(1.0 / bc2), f->n_sms, f->stream);
+  f->step = t;
+  f->grads_dirty = false;   // the Adam kernels clear what they consume
+  CUDA_TRY(cudaGetLastError());
+  return NSM_OK;
+}
+
+nsm_status read_stats(nsm_field *f, uint32_t R, nsm_step_stats *out) {
+  if (!out) return NSM_OK;
+  CUDA_TRY(cudaMemcpyAsync(f->pinned->acc, f->ws.loss_acc, 2 * sizeof(double), cudaMemcpyDeviceToHost, f->stream));
+  CUDA_TRY(cudaMemcpyAsync(&f->pinned->S, f->ws.offsets + R, sizeof(uint32_t), cudaMemcpyDeviceToHost, f->stream));
+  CUDA_TRY(cudaStreamSynchronize(f->stream));
+  out->loss_rgb = f->pinned->acc[0] / (double)R;
+  out->loss_depth = f->pinned->acc[1] / (double)R;
+  out->n_samples = f->pinned->S;
+  out->n_rays = R;
+  out->step = f->step;
+  return NSM_OK;
+}
+
+// copy a host batch into the device staging area; returns a batch of device pointers
+nsm_status stage_batch(nsm_field *f, const nsm_ray_batch *hb, uint32_t first, uint32_t R, bool train, nsm_ray_batch *db) {
+  float *p = f->stage_dev;
+  const uint32_t M = f->cfg.max_rays;
+  *db = *hb;
+  db->n_rays = R;
+  CUDA_TRY(cudaMemcpyAsync(p, hb->origins + 3 * (size_t)first, sizeof(float) * 3 * R, cudaMemcpyHostToDevice, f->stream));
+  db->origins = p;
+  CUDA_TRY(cudaMemcpyAsync(p + 3 * M, hb->dirs + 3 * (size_t)first, sizeof(float) * 3 * R, cudaMemcpyHostToDevice, f->stream));
+  db->dirs = p + 3 * M;
+  if (train) {
+    CUDA_TRY(cudaMemcpyAsync(p + 6 * M, hb->rgb + 3 * (size_t)first, sizeof(float) * 3 * R, cudaMemcpyHostToDevice, f->stream));
+    CUDA_TRY(cudaMemcpyAsync(p + 9 * M, hb->depth + first, sizeof(float) * R, cudaMemcpyHostToDevice, f->stream));
+    CUDA_TRY(cudaMemcpyAsync(p + 10 * M, hb->depth_var + first, sizeof(float) * R, cudaMemcpyHostToDevice, f->stream));
+    db->rgb = p + 6 * M;
+    db->depth = p + 9 * M;
+    db->depth_var = p + 10 * M;
+  }
+  return NSM_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+const char *nsm_last_error(void) { return g_err.c_str(); }
+const char *nsm_version(void) { return "nsm 0.1 (sm_100a)"; }
+uint64_t nsm_launch_count(const nsm_field *f) { return f ? f->launches : 0; }
+const char *nsm_mlp_path(const nsm_field *f) { return f ? f->mlp_path : ""; }
+
+nsm_status nsm_create_field(const nsm_field_config *cfg, void *cuda_stream, nsm_field **out) {
+  if (!out) return fail(NSM_ERR_INVALID_ARG, "out is NULL");
+  *out = nullptr;
+  nsm_status st = validate_config(cfg);
+  if (st != NSM_OK) return st;
+  int dev = 0, n_dev = 0;
+  if (cudaGetDeviceCount(&n_dev) != cudaSuccess || n_dev == 0) {
+    cudaGetLastError();
+    return fail(NSM_ERR_CUDA, "no CUDA device: this library has no CPU fallback");
+  }
+  CUDA_TRY(cudaGetDevice(&dev));
+  cudaDeviceProp prop;
+  CUDA_TRY(cudaGetDeviceProperties(&prop, dev));
+  if (prop.major < 10) return fail(NSM_ERR_CUDA, "device sm_%d%d is not sm_100: built for B200 only", prop.major, prop.minor);
+
+  nsm_field *f = new (std::nothrow) nsm_field();
+  if (!f) return fail(NSM_ERR_OOM, "host allocation failed");
+  f->cfg = *cfg;
+  f->stream = (cudaStream_t)cuda_stream;
+  f->n_sms = prop.multiProcessorCount;
+  build_levels(*cfg, f->lv);
+  MlpShape &ms = f->ms;
+  ms.LF = cfg->n_levels * cfg->n_features;
+  ms.Hd = cfg->density_hidden; ms.Do = cfg->density_out;
+  ms.sh_degree = cfg->sh_degree; ms.n_sh = cfg->sh_degree * cfg->sh_degree;
+  ms.geo_off = cfg->geo_offset; ms.geo_cnt = cfg->geo_count;
+  ms.Ci = ms.geo_cnt + ms.n_sh; ms.Hc = cfg->color_hidden; ms.n_color_layers = cfg->color_hidden_layers;
+  uint32_t o = 0;
+  ms.o_d1 = o; o += ms.Hd * ms.LF;
+  ms.o_d2 = o; o += ms.Do * ms.Hd;
+  ms.o_c1 = o; o += ms.Hc * ms.Ci;
+  ms.o_c2 = o; o += (ms.n_color_layers == 2 ? ms.Hc * ms.Hc : 0);
+  ms.o_c3 = o; o += 3 * ms.Hc;
+  ms.n_mlp = o;
+  if (ms.Ci > 128) { delete f; return fail(NSM_ERR_UNIMPLEMENTED, "colour input width > 128"); }
+  if (mlp_simt_smem_bytes(ms, 1) > (size_t)prop.sharedMemPerBlockOptin) {
+    delete f;
+    return fail(NSM_ERR_UNIMPLEMENTED, "MLP shape needs %zu B shared memory (> %zu)", mlp_simt_smem_bytes(ms, 1),
+                (size_t)prop.sharedMemPerBlockOptin);
+  }
+
+  FieldParams &fp = f->fp;
+  fp.n_entries = f->lv.offset[cfg->n_levels];
+  fp.n_table = fp.n_entries * cfg->n_features;
+  fp.n_mlp = ms.n_mlp;
+  const uint64_t P = fp.n_table + fp.n_mlp;
+  Workspace &ws = f->ws;
+  const uint64_t cap = (((uint64_t)cfg->max_rays * cfg->max_candidates + NSM_TILE - 1) / NSM_TILE) * NSM_TILE;
+  ws.cap = cap;
+  ws.max_rays = cfg->max_rays;
+  const uint64_t G3 = (uint64_t)cfg->occ_res * cfg->occ_res * cfg->occ_res;
+  const uint32_t R = cfg->max_rays, words = (cfg->max_candidates + 31) / 32;
+  cudaError_t e = cudaSuccess;
+  auto A = [&](cudaError_t r) { if (e == cudaSuccess) e = r; };
+  A(f->alloc(&fp.theta, P)); A(f->alloc(&fp.m, P)); A(f->alloc(&fp.v, P)); A(f->alloc(&fp.grad, P));
+  A(f->alloc(&fp.touched, fp.n_entries)); A(f->alloc(&fp.occ_bits, (G3 + 7) / 8 + 4));
+  A(f->alloc(&ws.counts, R)); A(f->alloc(&ws.offsets, R + 1)); A(f->alloc(&ws.live_mask, (size_t)R * words));
+  A(f->alloc(&ws.C, 3 * (size_t)R)); A(f->alloc(&ws.D_hat, R)); A(f->alloc(&ws.O, R));
+  A(f->alloc(&ws.s_ray, cap)); A(f->alloc(&ws.s_k, cap)); A(f->alloc(&ws.s_t, cap)); A(f->alloc(&ws.s_delta, cap));
+  A(f->alloc(&ws.s_x, 3 * cap)); A(f->alloc(&ws.e, ms.LF * cap)); A(f->alloc(&ws.hd, ms.Hd * cap));
+  A(f->alloc(&ws.g, ms.Do * cap)); A(f->alloc(&ws.h1, ms.Hc * cap));
+  A(f->alloc(&ws.h2, (ms.n_color_layers == 2 ? ms.Hc : 1) * cap));
+  A(f->alloc(&ws.sigma, cap)); A(f->alloc(&ws.rgb, 3 * cap)); A(f->alloc(&ws.T_excl, cap));
+  A(f->alloc(&ws.dsigma, cap)); A(f->alloc(&ws.drgb, 3 * cap)); A(f->alloc(&ws.de, ms.LF * cap));
+  A(f->alloc(&ws.loss_acc, 2));
+  A(f->alloc(&f->stage_dev, 11 * (size_t)R)); A(f->alloc(&f->stage_out, 5 * (size_t)R));
+  if (e == cudaSuccess) e = cudaMallocHost((void **)&f->pinned, sizeof(*f->pinned));
+  if (e != cudaSuccess) {
+    nsm_destroy_field(f);
+    cudaGetLastError();
+    return fail(e == cudaErrorMemoryAllocation ? NSM_ERR_OOM : NSM_ERR_CUDA, "allocation failed: %s", cudaGetErrorString(e));
+  }
+  *out = f;
+  return NSM_OK;
+}
+
+void nsm_destroy_field(nsm_field *f) {
+  if (!f) return;
+  cudaStreamSynchronize(f->stream);
+  for (void *p : f->allocs) cudaFree(p);
+  if (f->pinned) cudaFreeHost(f->pinned);
+  delete f;
+}
+
+nsm_status nsm_param_count(const nsm_field *f, uint64_t *n_table, uint64_t *n_mlp) {
+  if (!f) return fail(NSM_ERR_INVALID_ARG, "field is NULL");
+  if (n_table) *n_table = f->fp.n_table;
+  if (n_mlp) *n_mlp = f->fp.n_mlp;
+  return NSM_OK;
+}
+
+nsm_status nsm_get_level_table(const nsm_field *f, uint32_t *res, uint64_t *offset) {
+  if (!f) return fail(NSM_ERR_INVALID_ARG, "field is NULL");
+  for (uint32_t l = 0; l < f->lv.n_levels; ++l) {
+    if (res) res[l] = f->lv.res[l];
+    if (offset) offset[l] = f->lv.offset[l];
+  }
+  if (offset) offset[f->lv.n_levels] = f->lv.offset[f->lv.n_levels];
+  return NSM_OK;
+}
+
+nsm_status nsm_get_params(nsm_field *f, float *d_theta, float *d_m, float *d_v, uint32_t *step) {
+  if (!f) return fail(NSM_ERR_INVALID_ARG, "field is NULL");
+  const size_t bytes = sizeof(float) * (f->fp.n_table + f->fp.n_mlp);
+  if (d_theta) CUDA_TRY(cudaMemcpyAsync(d_theta, f->fp.theta, bytes, cudaMemcpyDeviceToDevice, f->stream));
+  if (d_m) CUDA_TRY(cudaMemcpyAsync(d_m, f->fp.m, bytes, cudaMemcpyDeviceToDevice, f->stream));
+  if (d_v) CUDA_TRY(cudaMemcpyAsync(d_v, f->fp.v, bytes, cudaMemcpyDeviceToDevice, f->stream));
+  if (step) *step = f->step;
+  return NSM_OK;
+}
+
+nsm_status nsm_set_params(nsm_field *f, const float *d_theta, const float *d_m, const float *d_v, uint32_t step) {
+  if (!f) return fail(NSM_ERR_INVALID_ARG, "field is NULL");
+  const size_t bytes = sizeof(float) * (f->fp.n_table + f->fp.n_mlp);
+  if (d_theta) CUDA_TRY(cudaMemcpyAsync(f->fp.theta, d_theta, bytes, cudaMemcpyDeviceToDevice, f->stream));
+  if (d_m) CUDA_TRY(cudaMemcpyAsync(f->fp.m, d_m, bytes, cudaMemcpyDeviceToDevice, f->stream));
+  if (d_v) CUDA_TRY(cudaMemcpyAsync(f->fp.v, d_v, bytes, cudaMemcpyDeviceToDevice, f->stream));
+  f->step = step;
+  return NSM_OK;
+}
+
+nsm_status nsm_get_occupancy(nsm_field *f, uint8_t *d_bits) {
+  if (!f || !d_bits) return fail(NSM_ERR_INVALID_ARG, "NULL argument");
+  const uint64_t G3 = (uint64_t)f->cfg.occ_res * f->cfg.occ_res * f->cfg.occ_res;
+  if (f->occ_full) CUDA_TRY(cudaMemsetAsync(d_bits, 0xff, (G3 + 7) / 8, f->stream));
+  else CUDA_TRY(cudaMemcpyAsync(d_bits, f->fp.occ_bits, (G3 + 7) / 8, cudaMemcpyDeviceToDevice, f->stream));
+  return NSM_OK;
+}
+
+nsm_status nsm_update_occupancy(nsm_field *f, nsm_occ_mode mode, const uint8_t *d_bits) {
+  if (!f) return fail(NSM_ERR_INVALID_ARG, "field is NULL");
+  const uint64_t G3 = (uint64_t)f->cfg.occ_res * f->cfg.occ_res * f->cfg.occ_res;
+  switch (mode) {
+    case NSM_OCC_FULL:
+      f->occ_full = true;
+      return NSM_OK;
+    case NSM_OCC_SET:
+      if (!d_bits) return fail(NSM_ERR_INVALID_ARG, "d_bits is NULL");
+      CUDA_TRY(cudaMemcpyAsync(f->fp.occ_bits, d_bits, (G3 + 7) / 8, cudaMemcpyDeviceToDevice, f->stream));
+      f->occ_full = false;
+      return NSM_OK;
+    case NSM_OCC_FROM_FIELD: {
+      // the cell centres go through S4 + S5 in chunks of the workspace capacity (multiples of 32)
+      const uint64_t chunk = f->ws.cap & ~uint64_t(31);
+      uint32_t *d_S = f->ws.offsets;  // offsets[0] doubles as the chunk's sample count
+      for (uint64_t first = 0; first < G3; first += chunk) {
+        const uint64_t n = (G3 - first < chunk) ? G3 - first : chunk;
+        f->launches += launch_occ_cells(f->cfg.occ_res, first, n, f->ws, d_S, f->stream);
+        f->launches += launch_encode(f->lv, f->fp.theta, f->ws, d_S, f->n_sms, f->stream);
+        f->launches += launch_mlp_forward_simt(f->ms, f->fp.theta + f->fp.n_table, nullptr, f->ws, d_S, 1, f->n_sms, f->stream);
+        f->launches += launch_occ_threshold(f->cfg.occ_res, first, n, f->ws.sigma, f->cfg.occ_sigma_threshold,
+                                            f->fp.occ_bits, f->stream);
+      }
+      f->occ_full = false;
+      CUDA_TRY(cudaGetLastError());
+      return NSM_OK;
+    }
+  }
+  return fail(NSM_ERR_INVALID_ARG, "bad occupancy mode %d", (int)mode);
+}
+
+nsm_status nsm_backward(nsm_field *f, const nsm_ray_batch *batch, float lambda_d, nsm_step_stats *host_stats) {
+  nsm_status st = validate_batch(f, batch, true, false);
+  if (st != NSM_OK) return st;
+  st = enqueue_backward(f, batch, lambda_d);
+  if (st != NSM_OK) return st;
+  st = read_stats(f, batch->n_rays, host_stats);
+  if (st == NSM_OK && host_stats) host_stats->loss = host_stats->loss_rgb + (double)lambda_d * host_stats->loss_depth;
+  return st;
+}
+
+nsm_status nsm_apply_adam(nsm_field *f) {
+  if (!f) return fail(NSM_ERR_INVALID_ARG, "field is NULL");
+  return enqueue_adam(f);
+}
+
+nsm_status nsm_train_step(nsm_field *f, const nsm_ray_batch *batch, float lambda_d, nsm_step_stats *host_stats) {
+  nsm_status st = validate_batch(f, batch, true, false);
+  if (st != NSM_OK) return st;
+  st = enqueue_backward(f, batch, lambda_d);
+  if (st != NSM_OK) return st;
+  st = enqueue_adam(f);
+  if (st != NSM_OK) return st;
+  st = read_stats(f, batch->n_rays, host_stats);
+  if (st == NSM_OK && host_stats) host_stats->loss = host_stats->loss_rgb + (double)lambda_d * host_stats->loss_depth;
+  return st;
+}
+
+nsm_status nsm_train_step_host(nsm_field *f, const nsm_ray_batch *hb, float lambda_d, nsm_step_stats *host_stats) {
+  nsm_status st = validate_batch(f, hb, true, false);
+  if (st != NSM_OK) return st;
+  nsm_ray_batch db;
+  st = stage_batch(f, hb, 0, hb->n_rays, true, &db);
+  if (st != NSM_OK) return st;
+  nsm_step_stats local;
+  st = nsm_train_step(f, &db, lambda_d, host_stats ? host_stats : &local);  // always syncs: host buffers may be reused
+  return st;
+}
+
+nsm_status nsm_debug_set_grad(nsm_field *f, const float *d_grad, const uint8_t *d_touched) {
+  if (!f) return fail(NSM_ERR_INVALID_ARG, "field is NULL");
+  if (d_grad) CUDA_TRY(cudaMemcpyAsync(f->fp.grad, d_grad, sizeof(float) * (f->fp.n_table + f->fp.n_mlp), cudaMemcpyDeviceToDevice, f->stream));
+  if (d_touched) CUDA_TRY(cudaMemcpyAsync(f->fp.touched, d_touched, f->fp.n_entries, cudaMemcpyDeviceToDevice, f->stream));
+  f->grads_dirty = true;
+  return NSM_OK;
+}
+
+static nsm_status render_chunks(nsm_field *f, const nsm_ray_batch *b, float cut, float *rgb, float *depth, float *opacity,
+                                bool host) {
+  nsm_status st = validate_batch(f, b, false, true);
+  if (st != NSM_OK) return st;
+  if (!rgb || !depth) return fail(NSM_ERR_INVALID_ARG, "output pointers are NULL");
+  if (!(cut >= 0.f)) return fail(NSM_ERR_INVALID_ARG, "transmittance_cut must be >= 0");
+  const uint32_t M = f->cfg.max_rays;
+  for (uint32_t first = 0; first < b->n_rays; first += M) {
+    const uint32_t R = (b->n_rays - first < M) ? b->n_rays - first : M;
+    nsm_ray_batch cb = *b;
+    cb.n_rays = R;
+    float *o_rgb = rgb + 3 * (size_t)first, *o_d = depth + first, *o_op = opacity ? opacity + first : nullptr;
+    if (host) {
+      st = stage_batch(f, b, first, R, false, &cb);
+      if (st != NSM_OK) return st;
+      o_rgb = f->stage_out; o_d = f->stage_out + 3 * (size_t)M; o_op = f->stage_out + 4 * (size_t)M;
+    } else {
+      cb.origins = b->origins + 3 * (size_t)first;
+      cb.dirs = b->dirs + 3 * (size_t)first;
+    }
+    enqueue_forward(f, &cb, R, false, 0);
+    f->launches += launch_composite_render(f->ws, R, cut, f->cfg.bg, o_rgb, o_d, o_op, f->stream);
+    if (host) {
+      CUDA_TRY(cudaMemcpyAsync(rgb + 3 * (size_t)first, o_rgb, sizeof(float) * 3 * R, cudaMemcpyDeviceToHost, f->stream));
+      CUDA_TRY(cudaMemcpyAsync(depth + first, o_d, sizeof(float) * R, cudaMemcpyDeviceToHost, f->stream));
+      if (opacity) CUDA_TRY(cudaMemcpyAsync(opacity + first, o_op, sizeof(float) * R, cudaMemcpyDeviceToHost, f->stream));
+      CUDA_TRY(cudaStreamSynchronize(f->stream));  // staging buffers are reused by the next chunk
+    }
+    f->last_R = R;
+    f->last_K = b->n_candidates;
+    f->last_was_render = true;
+  }
+  CUDA_TRY(cudaGetLastError());
+  return NSM_OK;
+}
+
+nsm_status nsm_render(nsm_field *f, const nsm_ray_batch *batch, float cut, float *d_rgb, float *d_depth, float *d_opacity) {
+  return render_chunks(f, batch, cut, d_rgb, d_depth, d_opacity, false);
+}
+
+nsm_status nsm_render_host(nsm_field *f, const nsm_ray_batch *hb, float cut, float *h_rgb, float *h_depth, float *h_opacity) {
+  return render_chunks(f, hb, cut, h_rgb, h_depth, h_opacity, true);
+}
+
+nsm_status nsm_debug_last_step(nsm_field *f, int item, void *d_out, uint64_t capacity_bytes, uint64_t *n_bytes_out) {
+  if (!f) return fail(NSM_ERR_INVALID_ARG, "field is NULL");
+  if (f->last_R == 0) return fail(NSM_ERR_INVALID_ARG, "no step has been run yet");
+  const uint32_t R = f->last_R;
+  const uint32_t *d_S = f->ws.offsets + R;
+  uint32_t S = 0;
+  CUDA_TRY(cudaMemcpyAsync(&f->pinned->S, d_S, sizeof(uint32_t), cudaMemcpyDeviceToHost, f->stream));
+  CUDA_TRY(cudaStreamSynchronize(f->stream));
+  S = f->pinned->S;
+  const uint32_t L = f->lv.n_levels;
+  const Workspace &ws = f->ws;
+  const void *src = nullptr;
+  uint64_t bytes = 0;
+  switch (item) {
+    case NSM_DBG_COUNTS: src = ws.counts; bytes = 4ull * R; break;
+    case NSM_DBG_OFFSETS: src = ws.offsets; bytes = 4ull * (R + 1); break;
+    case NSM_DBG_SAMPLE_RAY: src = ws.s_ray; bytes = 4ull * S; break;
+    case NSM_DBG_SAMPLE_K: src = ws.s_k; bytes = 4ull * S; break;
+    case NSM_DBG_SAMPLE_T: src = ws.s_t; bytes = 4ull * S; break;
+    case NSM_DBG_SAMPLE_DELTA: src = ws.s_delta; bytes = 4ull * S; break;
+    case NSM_DBG_SIGMA: src = ws.sigma; bytes = 4ull * S; break;
+    case NSM_DBG_RGB: src = ws.rgb; bytes = 12ull * S; break;
+    case NSM_DBG_C: src = ws.C; bytes = 12ull * R; break;
+    case NSM_DBG_D_HAT: src = ws.D_hat; bytes = 4ull * R; break;
+    case NSM_DBG_O: src = ws.O; bytes = 4ull * R; break;
+    case NSM_DBG_DSIGMA: src = ws.dsigma; bytes = 4ull * S; break;
+    case NSM_DBG_DRGB: src = ws.drgb; bytes = 12ull * S; break;
+    case NSM_DBG_GRAD: src = f->fp.grad; bytes = 4ull * (f->fp.n_table + f->fp.n_mlp); break;
+    case NSM_DBG_TOUCHED: src = f->fp.touched; bytes = f->fp.n_entries; break;
+    case NSM_DBG_SAMPLE_X: bytes = 12ull * S; break;
+    case NSM_DBG_E: bytes = 4ull * S * f->ms.LF; break;
+    case NSM_DBG_SLOTS: bytes = 4ull * S * L * 8; break;
+    case NSM_DBG_W: bytes = 4ull * S * L * 3; break;
+    default: return fail(NSM_ERR_INVALID_ARG, "unknown debug item %d", item);
+  }
+  if (n_bytes_out) *n_bytes_out = bytes;
+  if (!d_out) return NSM_OK;  // size query
+  if (bytes > capacity_bytes) return fail(NSM_ERR_CAPACITY, "debug item needs %llu bytes, capacity %llu", (unsigned long long)bytes, (unsigned long long)capacity_bytes);
+  if (f->last_was_render && (item == NSM_DBG_C || item == NSM_DBG_D_HAT || item == NSM_DBG_O || item >= NSM_DBG_DSIGMA))
+    return fail(NSM_ERR_INVALID_ARG, "item %d is not produced by nsm_render", item);
+  if (bytes == 0) return NSM_OK;
+  if (src) {
+    CUDA_TRY(cudaMemcpyAsync(d_out, src, bytes, cudaMemcpyDeviceToDevice, f->stream));
+  } else if (item == NSM_DBG_SAMPLE_X) {
+    f->launches += launch_planes_to_rows(ws.s_x, ws.cap, 3, d_S, (float *)d_out, f->stream);
+  } else if (item == NSM_DBG_E) {
+    f->launches += launch_planes_to_rows(ws.e, ws.cap, f->ms.LF, d_S, (float *)d_out, f->stream);
+  } else if (item == NSM_DBG_SLOTS) {
+    f->launches += launch_debug_slots(f->lv, ws, d_S, (uint32_t *)d_out, nullptr, f->stream);
+  } else {
+    f->launches += launch_debug_slots(f->lv, ws, d_S, nullptr, (float *)d_out, f->stream);
+  }
+  CUDA_TRY(cudaGetLastError());
+  return NSM_OK;
+}
+
+}  // extern "C"

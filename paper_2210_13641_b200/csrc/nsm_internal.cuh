@@ -1,0 +1,99 @@
+// nsm_internal.cuh — device-side data layout and kernel launchers shared by the .cu files of
+// the CUDA path.  Nothing here is shared with oracle/.  See DESIGN.md "Data layout in HBM".
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "nsm.h"
+
+#define NSM_MAX_LEVELS 32
+#define NSM_TILE 128          // samples per MLP tile
+#define NSM_LD 132            // smem row stride (floats) of a [feature][sample] activation buffer
+
+// Per-level constants (S0), passed by value to kernels.
+struct LevelTable {
+  uint32_t n_levels, n_features, t_mask;
+  uint32_t res[NSM_MAX_LEVELS];
+  uint32_t dense[NSM_MAX_LEVELS];      // 1: slot = vx + (N+1)(vy + (N+1) vz); 0: hashed
+  uint64_t offset[NSM_MAX_LEVELS + 1]; // in entries
+};
+
+// Offsets (floats) of the MLP matrices inside the MLP block (canonical order) and their shapes.
+struct MlpShape {
+  uint32_t LF, Hd, Do, Ci, Hc, n_color_layers, n_sh, sh_degree, geo_off, geo_cnt;
+  uint32_t o_d1, o_d2, o_c1, o_c2, o_c3, n_mlp;
+};
+
+// Candidate lattice + field cube, by value to the march kernels.
+struct MarchParams {
+  float aabb_min[3], inv_extent;
+  float t_min, dt;
+  uint32_t K, G, jitter, step;
+  uint64_t seed;
+  uint32_t R;
+};
+
+// Per-step device workspace.  All per-sample arrays are planes of `cap` floats (cap = capacity,
+// a multiple of NSM_TILE), feature-major, so a warp reading 32 consecutive samples is coalesced.
+struct Workspace {
+  uint64_t cap;          // samples
+  uint32_t max_rays;
+  // rays
+  uint32_t *counts;      // [R]
+  uint32_t *offsets;     // [R+1]; offsets[R] = S
+  uint32_t *live_mask;   // [R, ceil(K/32)]
+  float *C, *D_hat, *O;  // [R,3], [R], [R]
+  // samples
+  uint32_t *s_ray, *s_k; // [cap]
+  float *s_t, *s_delta;  // [cap]
+  float *s_x;            // [3][cap] planes
+  float *e;              // [LF][cap]
+  float *hd;             // [Hd][cap]
+  float *g;              // [Do][cap]
+  float *h1, *h2;        // [Hc][cap]
+  float *sigma;          // [cap]
+  float *rgb;            // [cap,3]
+  float *T_excl;         // [cap] transmittance before the sample (T_i of Eq. 6)
+  float *dsigma;         // [cap]
+  float *drgb;           // [cap,3]
+  float *de;             // [LF][cap]
+  // loss accumulators: [0]=sum rgb, [1]=sum depth (doubles); device
+  double *loss_acc;
+};
+
+struct FieldParams {
+  float *theta, *m, *v, *grad; // [P] canonical: tables then MLP
+  uint8_t *touched;            // [n_entries]
+  uint8_t *occ_bits;           // [G^3/8]
+  uint64_t n_entries, n_table, n_mlp;
+};
+
+// ---- launchers (each enqueues on `st`, returns the number of kernels launched) ----
+int launch_march(const MarchParams &mp, const uint8_t *bits, const float *origins, const float *dirs,
+                 const Workspace &ws, cudaStream_t st);
+int launch_encode(const LevelTable &lv, const float *theta, const Workspace &ws,
+                  const uint32_t *d_S, int n_sms, cudaStream_t st);
+int launch_scatter(const LevelTable &lv, float *grad, uint8_t *touched, const Workspace &ws,
+                   const uint32_t *d_S, int n_sms, cudaStream_t st);
+int launch_mlp_forward_simt(const MlpShape &ms, const float *theta_mlp, const float *dirs,
+                            const Workspace &ws, const uint32_t *d_S, int density_only, int n_sms,
+                            cudaStream_t st);
+int launch_mlp_backward_simt(const MlpShape &ms, const float *theta_mlp, float *grad_mlp,
+                             const float *dirs, const Workspace &ws, const uint32_t *d_S, int n_sms,
+                             cudaStream_t st);
+size_t mlp_simt_smem_bytes(const MlpShape &ms, int backward);
+int launch_composite_train(const Workspace &ws, uint32_t R, const float *rgb, const float *depth,
+                           const float *depth_var, float lambda_d, const float bg[3],
+                           cudaStream_t st);
+int launch_composite_render(const Workspace &ws, uint32_t R, float cut, const float bg[3],
+                            float *out_rgb, float *out_depth, float *out_opacity, cudaStream_t st);
+int launch_adam(const FieldParams &fp, uint32_t F, int sparse, float lr, float beta1, float beta2,
+                float eps, float inv_bc1, float inv_bc2, int n_sms, cudaStream_t st);
+int launch_occ_cells(uint32_t G, uint64_t first_cell, uint64_t n_cells, const Workspace &ws,
+                     uint32_t *d_S, cudaStream_t st);
+int launch_occ_threshold(uint32_t G, uint64_t first_cell, uint64_t n_cells, const float *sigma,
+                         float thr, uint8_t *bits, cudaStream_t st);
+int launch_debug_slots(const LevelTable &lv, const Workspace &ws, const uint32_t *d_S,
+                       uint32_t *slots, float *w, cudaStream_t st);
+int launch_planes_to_rows(const float *planes, uint64_t cap, uint32_t n_planes, const uint32_t *d_S,
+                          float *rows, cudaStream_t st);
