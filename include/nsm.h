@@ -171,6 +171,19 @@ nsm_status nsm_get_level_table(const nsm_field *f, uint32_t *res, uint64_t *offs
 nsm_status nsm_debug_last_step(nsm_field *f, int item, void *d_out, uint64_t capacity_bytes,
                                uint64_t *n_bytes_out);
 
+/* Live samples processed by all training / backward steps since creation (a device counter
+ * updated by the compaction kernel; this call synchronises the stream). */
+nsm_status nsm_total_samples(nsm_field *f, uint64_t *out);
+
+/* Per-kernel timing for roofline reports: when enabled, every kernel launch is bracketed by CUDA
+ * events on the field's stream and each step ends with a synchronise (so do not enable it for
+ * whole-step timing).  nsm_profile_read fills up to `capacity` entries: kernel-class names
+ * (static strings), summed milliseconds and launch counts since enabling; *n_out = number of
+ * kernel classes. */
+nsm_status nsm_profile(nsm_field *f, int enable);
+nsm_status nsm_profile_read(nsm_field *f, uint32_t capacity, const char **names, double *total_ms,
+                            uint64_t *launches, uint32_t *n_out);
+
 /* Number of this library's kernels launched by this field so far (bench.py's gpu_launches). */
 uint64_t    nsm_launch_count(const nsm_field *f);
 /* Which MLP path the field runs: "simt_fp32", "tcgen05_f16", "tcgen05_bf16". */

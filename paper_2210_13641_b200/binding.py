@@ -26,7 +26,8 @@ DEBUG_ITEMS = dict(counts=(0, np.uint32), offsets=(1, np.uint32), s_ray=(2, np.u
 EXPORTS = ["nsm_create_field", "nsm_destroy_field", "nsm_update_occupancy", "nsm_get_occupancy",
            "nsm_train_step", "nsm_train_step_host", "nsm_backward", "nsm_apply_adam", "nsm_debug_set_grad",
            "nsm_render", "nsm_render_host", "nsm_param_count", "nsm_get_params", "nsm_set_params",
-           "nsm_get_level_table", "nsm_debug_last_step", "nsm_launch_count", "nsm_mlp_path",
+           "nsm_get_level_table", "nsm_debug_last_step", "nsm_total_samples", "nsm_profile",
+           "nsm_profile_read", "nsm_launch_count", "nsm_mlp_path",
            "nsm_last_error", "nsm_version"]
 
 
@@ -88,6 +89,9 @@ def load_library():
         L.nsm_set_params.argtypes = [vp, vp, vp, vp, C.c_uint32]
         L.nsm_get_level_table.argtypes = [vp, u32p, u64p]
         L.nsm_debug_last_step.argtypes = [vp, C.c_int, vp, C.c_uint64, u64p]
+        L.nsm_total_samples.argtypes = [vp, u64p]
+        L.nsm_profile.argtypes = [vp, C.c_int]
+        L.nsm_profile_read.argtypes = [vp, C.c_uint32, C.POINTER(C.c_char_p), C.POINTER(C.c_double), u64p, u32p]
         L.nsm_launch_count.argtypes = [vp]
         L.nsm_launch_count.restype = C.c_uint64
         for name in ("nsm_mlp_path", "nsm_last_error", "nsm_version"):
@@ -317,6 +321,24 @@ class Field:
         L, F = self.fc.n_levels, self.fc.n_features
         shape = dict(s_x=(-1, 3), slots=(-1, L, 8), w=(-1, L, 3), e=(-1, L * F), rgb=(-1, 3), C=(-1, 3), drgb=(-1, 3))
         return a.reshape(shape[name]) if name in shape else a
+
+    def nsm_total_samples(self):
+        n = C.c_uint64()
+        _check(self.lib.nsm_total_samples(self.h, C.byref(n)))
+        return int(n.value)
+
+    def nsm_profile(self, enable):
+        _check(self.lib.nsm_profile(self.h, int(bool(enable))))
+
+    def nsm_profile_read(self):
+        """{kernel class: (total ms, launches)} since nsm_profile(True)."""
+        cap = 32
+        names = (C.c_char_p * cap)()
+        ms = (C.c_double * cap)()
+        cnt = (C.c_uint64 * cap)()
+        n = C.c_uint32()
+        _check(self.lib.nsm_profile_read(self.h, cap, names, ms, cnt, C.byref(n)))
+        return {names[i].decode(): (ms[i], int(cnt[i])) for i in range(n.value)}
 
     def nsm_launch_count(self):
         return int(self.lib.nsm_launch_count(self.h))

@@ -54,8 +54,8 @@ __global__ void adam_dense_kernel(float *__restrict__ theta, float *__restrict__
 
 }  // namespace
 
-int launch_adam(const FieldParams &fp, uint32_t F, int sparse, float lr, float beta1, float beta2, float eps,
-                float inv_bc1, float inv_bc2, int n_sms, cudaStream_t st) {
+int launch_adam_table(const FieldParams &fp, uint32_t F, int sparse, float lr, float beta1, float beta2, float eps,
+                      float inv_bc1, float inv_bc2, int n_sms, cudaStream_t st) {
   AdamConst c{lr, beta1, beta2, eps, inv_bc1, inv_bc2};
   dim3 grid(n_sms * 8), block(256);
   switch (F) {
@@ -64,8 +64,14 @@ int launch_adam(const FieldParams &fp, uint32_t F, int sparse, float lr, float b
     case 4: adam_table_kernel<4><<<grid, block, 0, st>>>(fp.theta, fp.m, fp.v, fp.grad, fp.touched, fp.n_entries, sparse, c); break;
     default: adam_table_kernel<8><<<grid, block, 0, st>>>(fp.theta, fp.m, fp.v, fp.grad, fp.touched, fp.n_entries, sparse, c); break;
   }
+  return 1;
+}
+
+int launch_adam_mlp(const FieldParams &fp, float lr, float beta1, float beta2, float eps, float inv_bc1, float inv_bc2,
+                    cudaStream_t st) {
+  AdamConst c{lr, beta1, beta2, eps, inv_bc1, inv_bc2};
   adam_dense_kernel<<<(unsigned)((fp.n_mlp + 255) / 256), 256, 0, st>>>(fp.theta + fp.n_table, fp.m + fp.n_table,
                                                                        fp.v + fp.n_table, fp.grad + fp.n_table,
                                                                        fp.n_mlp, c);
-  return 2;
+  return 1;
 }

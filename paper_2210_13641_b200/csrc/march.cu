@@ -106,7 +106,7 @@ __global__ void __launch_bounds__(256) march_count_kernel(MarchParams mp, const 
 // reset of the loss accumulators.  Deterministic.
 __global__ void __launch_bounds__(1024) scan_counts_kernel(const uint32_t *__restrict__ counts,
                                                            uint32_t *__restrict__ offsets, uint32_t R,
-                                                           double *loss_acc) {
+                                                           double *loss_acc, unsigned long long *total) {
   __shared__ uint32_t warp_sums[32];
   __shared__ uint32_t carry_s;
   const uint32_t tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
@@ -143,7 +143,10 @@ __global__ void __launch_bounds__(1024) scan_counts_kernel(const uint32_t *__res
     if (tid == 1023) carry_s = excl + v;
     __syncthreads();
   }
-  if (tid == 0) offsets[R] = carry_s;
+  if (tid == 0) {
+    offsets[R] = carry_s;
+    if (total) *total += carry_s;
+  }
 }
 
 // Second pass: each live candidate is written at offsets[r] + its rank among the ray's live ones.
@@ -208,14 +211,24 @@ __global__ void occ_threshold_kernel(uint64_t first_cell, uint64_t n_cells,
 
 }  // namespace
 
-int launch_march(const MarchParams &mp, const uint8_t *bits, const float *origins, const float *dirs,
-                 const Workspace &ws, cudaStream_t st) {
-  const uint32_t warps_per_block = 8;
-  dim3 grid((mp.R + warps_per_block - 1) / warps_per_block), block(32 * warps_per_block);
+int launch_march_count(const MarchParams &mp, const uint8_t *bits, const float *origins, const float *dirs,
+                       const Workspace &ws, cudaStream_t st) {
+  dim3 grid((mp.R + 7) / 8), block(256);
   march_count_kernel<<<grid, block, 0, st>>>(mp, bits, origins, dirs, ws.counts, ws.live_mask);
-  scan_counts_kernel<<<1, 1024, 0, st>>>(ws.counts, ws.offsets, mp.R, ws.loss_acc);
-  march_write_kernel<<<grid, block, 0, st>>>(mp, bits, origins, dirs, ws.offsets, ws.live_mask, ws);
-  return 3;
+  return 1;
+}
+
+int launch_scan(const MarchParams &mp, const Workspace &ws, int count_total, cudaStream_t st) {
+  scan_counts_kernel<<<1, 1024, 0, st>>>(ws.counts, ws.offsets, mp.R, ws.loss_acc,
+                                         count_total ? ws.total_samples : nullptr);
+  return 1;
+}
+
+int launch_march_write(const MarchParams &mp, const float *origins, const float *dirs, const Workspace &ws,
+                       cudaStream_t st) {
+  dim3 grid((mp.R + 7) / 8), block(256);
+  march_write_kernel<<<grid, block, 0, st>>>(mp, nullptr, origins, dirs, ws.offsets, ws.live_mask, ws);
+  return 1;
 }
 
 int launch_occ_cells(uint32_t G, uint64_t first_cell, uint64_t n_cells, const Workspace &ws,

@@ -37,8 +37,39 @@ nsm_status fail(nsm_status st, const char *fmt, ...) {
 
 }  // namespace
 
+static const char *kKernelNames[K_COUNT] = {"march_count", "scan", "march_write", "encode", "mlp_fwd", "composite",
+                                            "mlp_bwd", "scatter", "adam_table", "adam_mlp", "occupancy", "debug"};
+
+// Optional per-kernel CUDA-event timing (bench.py's roofline leg).  When enabled every launch is
+// bracketed by two events on the field's stream and each step ends with a synchronise.
+struct Profiler {
+  bool on = false;
+  double ms[K_COUNT] = {0};
+  uint64_t n[K_COUNT] = {0};
+  struct Rec { int id; cudaEvent_t a, b; };
+  std::vector<Rec> pending;
+  std::vector<cudaEvent_t> pool;
+  cudaEvent_t get() {
+    if (!pool.empty()) { cudaEvent_t e = pool.back(); pool.pop_back(); return e; }
+    cudaEvent_t e; cudaEventCreate(&e); return e;
+  }
+  void collect() {
+    for (auto &r : pending) {
+      float t = 0.f;
+      cudaEventSynchronize(r.b);
+      cudaEventElapsedTime(&t, r.a, r.b);
+      ms[r.id] += t; n[r.id] += 1;
+      pool.push_back(r.a); pool.push_back(r.b);
+    }
+    pending.clear();
+  }
+  void destroy() { collect(); for (auto e : pool) cudaEventDestroy(e); pool.clear(); }
+};
+
 struct nsm_field {
   nsm_field_config cfg;
+  Profiler prof;
+  uint64_t launches_by[K_COUNT] = {0};
   cudaStream_t stream = nullptr;
   int n_sms = 148;
   LevelTable lv;
@@ -143,6 +174,22 @@ nsm_status validate_batch(const nsm_field *f, const nsm_ray_batch *b, bool train
   return NSM_OK;
 }
 
+// launch one kernel class, counted and (optionally) timed
+#define RUN(f, id, call)                                                    \
+  do {                                                                      \
+    if ((f)->prof.on) {                                                     \
+      Profiler::Rec r_{id, (f)->prof.get(), (f)->prof.get()};               \
+      cudaEventRecord(r_.a, (f)->stream);                                   \
+      int n_ = (call);                                                      \
+      cudaEventRecord(r_.b, (f)->stream);                                   \
+      (f)->prof.pending.push_back(r_);                                      \
+      (f)->launches += n_; (f)->launches_by[id] += n_;                      \
+    } else {                                                                \
+      int n_ = (call);                                                      \
+      (f)->launches += n_; (f)->launches_by[id] += n_;                      \
+    }                                                                       \
+  } while (0)
+
 MarchParams make_march(const nsm_field *f, const nsm_ray_batch *b, uint32_t R, bool jitter, uint32_t step) {
   MarchParams mp;
   for (int a = 0; a < 3; ++a) mp.aabb_min[a] = f->cfg.aabb_min[a];
@@ -159,12 +206,14 @@ MarchParams make_march(const nsm_field *f, const nsm_ray_batch *b, uint32_t R, b
 }
 
 // S1-S8 forward (+ S9-S12 when train): everything up to, but excluding, Adam.
-void enqueue_forward(nsm_field *f, const nsm_ray_batch *b, uint32_t R, bool jitter, uint32_t step) {
+void enqueue_forward(nsm_field *f, const nsm_ray_batch *b, uint32_t R, bool jitter, uint32_t step, bool train) {
   const uint32_t *d_S = f->ws.offsets + R;
   MarchParams mp = make_march(f, b, R, jitter, step);
-  f->launches += launch_march(mp, f->occ_full ? nullptr : f->fp.occ_bits, b->origins, b->dirs, f->ws, f->stream);
-  f->launches += launch_encode(f->lv, f->fp.theta, f->ws, d_S, f->n_sms, f->stream);
-  f->launches += launch_mlp_forward_simt(f->ms, f->fp.theta + f->fp.n_table, b->dirs, f->ws, d_S, 0, f->n_sms, f->stream);
+  RUN(f, K_MARCH_COUNT, launch_march_count(mp, f->occ_full ? nullptr : f->fp.occ_bits, b->origins, b->dirs, f->ws, f->stream));
+  RUN(f, K_SCAN, launch_scan(mp, f->ws, train ? 1 : 0, f->stream));
+  RUN(f, K_MARCH_WRITE, launch_march_write(mp, b->origins, b->dirs, f->ws, f->stream));
+  RUN(f, K_ENCODE, launch_encode(f->lv, f->fp.theta, f->ws, d_S, f->n_sms, f->stream));
+  RUN(f, K_MLP_FWD, launch_mlp_forward_simt(f->ms, f->fp.theta + f->fp.n_table, b->dirs, f->ws, d_S, 0, f->n_sms, f->stream));
 }
 
 nsm_status clear_grads_if_dirty(nsm_field *f) {
@@ -181,11 +230,11 @@ nsm_status enqueue_backward(nsm_field *f, const nsm_ray_batch *b, float lambda_d
   const uint32_t *d_S = f->ws.offsets + R;
   nsm_status st = clear_grads_if_dirty(f);
   if (st != NSM_OK) return st;
-  enqueue_forward(f, b, R, f->cfg.jitter != 0, f->step + 1);
-  f->launches += launch_composite_train(f->ws, R, b->rgb, b->depth, b->depth_var, lambda_d, f->cfg.bg, f->stream);
-  f->launches += launch_mlp_backward_simt(f->ms, f->fp.theta + f->fp.n_table, f->fp.grad + f->fp.n_table, b->dirs,
-                                          f->ws, d_S, f->n_sms, f->stream);
-  f->launches += launch_scatter(f->lv, f->fp.grad, f->fp.touched, f->ws, d_S, f->n_sms, f->stream);
+  enqueue_forward(f, b, R, f->cfg.jitter != 0, f->step + 1, true);
+  RUN(f, K_COMPOSITE, launch_composite_train(f->ws, R, b->rgb, b->depth, b->depth_var, lambda_d, f->cfg.bg, f->stream));
+  RUN(f, K_MLP_BWD, launch_mlp_backward_simt(f->ms, f->fp.theta + f->fp.n_table, f->fp.grad + f->fp.n_table, b->dirs,
+                                             f->ws, d_S, f->n_sms, f->stream));
+  RUN(f, K_SCATTER, launch_scatter(f->lv, f->fp.grad, f->fp.touched, f->ws, d_S, f->n_sms, f->stream));
   f->grads_dirty = true;
   f->last_R = R;
   f->last_K = b->n_candidates;
@@ -198,9 +247,12 @@ nsm_status enqueue_adam(nsm_field *f) {
   const uint32_t t = f->step + 1;
   const double bc1 = 1.0 - std::pow((double)f->cfg.beta1, (double)t);
   const double bc2 = 1.0 - std::pow((double)f->cfg.beta2, (double)t);
-  f->launches += launch_adam(f->fp, f->cfg.n_features, f->cfg.sparse_table_adam != 0, f->cfg.lr, f->cfg.beta1,
-                             f->cfg.beta2, f->cfg.eps, (float)(1.0 / bc1), (float)(1.0 / bc2), f->n_sms, f->stream);
+  RUN(f, K_ADAM_TABLE, launch_adam_table(f->fp, f->cfg.n_features, f->cfg.sparse_table_adam != 0, f->cfg.lr, f->cfg.beta1,
+                                         f->cfg.beta2, f->cfg.eps, (float)(1.0 / bc1), (float)(1.0 / bc2), f->n_sms, f->stream));
+  RUN(f, K_ADAM_MLP, launch_adam_mlp(f->fp, f->cfg.lr, f->cfg.beta1, f->cfg.beta2, f->cfg.eps, (float)(1.0 / bc1),
+                                     (float)(1.0 / bc2), f->stream));
   f->step = t;
+  if (f->prof.on) f->prof.collect();
   f->grads_dirty = false;   // the Adam kernels clear what they consume
   CUDA_TRY(cudaGetLastError());
   return NSM_OK;
@@ -313,7 +365,7 @@ nsm_status nsm_create_field(const nsm_field_config *cfg, void *cuda_stream, nsm_
   A(f->alloc(&ws.h2, (ms.n_color_layers == 2 ? ms.Hc : 1) * cap));
   A(f->alloc(&ws.sigma, cap)); A(f->alloc(&ws.rgb, 3 * cap)); A(f->alloc(&ws.T_excl, cap));
   A(f->alloc(&ws.dsigma, cap)); A(f->alloc(&ws.drgb, 3 * cap)); A(f->alloc(&ws.de, ms.LF * cap));
-  A(f->alloc(&ws.loss_acc, 2));
+  A(f->alloc(&ws.loss_acc, 2)); A(f->alloc(&ws.total_samples, 1));
   A(f->alloc(&f->stage_dev, 11 * (size_t)R)); A(f->alloc(&f->stage_out, 5 * (size_t)R));
   if (e == cudaSuccess) e = cudaMallocHost((void **)&f->pinned, sizeof(*f->pinned));
   if (e != cudaSuccess) {
@@ -328,9 +380,41 @@ nsm_status nsm_create_field(const nsm_field_config *cfg, void *cuda_stream, nsm_
 void nsm_destroy_field(nsm_field *f) {
   if (!f) return;
   cudaStreamSynchronize(f->stream);
+  f->prof.destroy();
   for (void *p : f->allocs) cudaFree(p);
   if (f->pinned) cudaFreeHost(f->pinned);
   delete f;
+}
+
+nsm_status nsm_total_samples(nsm_field *f, uint64_t *out) {
+  if (!f || !out) return fail(NSM_ERR_INVALID_ARG, "NULL argument");
+  unsigned long long v = 0;
+  CUDA_TRY(cudaMemcpyAsync(&v, f->ws.total_samples, sizeof v, cudaMemcpyDeviceToHost, f->stream));
+  CUDA_TRY(cudaStreamSynchronize(f->stream));
+  *out = v;
+  return NSM_OK;
+}
+
+nsm_status nsm_profile(nsm_field *f, int enable) {
+  if (!f) return fail(NSM_ERR_INVALID_ARG, "field is NULL");
+  CUDA_TRY(cudaStreamSynchronize(f->stream));
+  f->prof.collect();
+  f->prof.on = enable != 0;
+  if (enable) for (int i = 0; i < K_COUNT; ++i) { f->prof.ms[i] = 0.0; f->prof.n[i] = 0; }
+  return NSM_OK;
+}
+
+nsm_status nsm_profile_read(nsm_field *f, uint32_t capacity, const char **names, double *total_ms, uint64_t *launches,
+                            uint32_t *n_out) {
+  if (!f || !n_out) return fail(NSM_ERR_INVALID_ARG, "NULL argument");
+  f->prof.collect();
+  *n_out = K_COUNT;
+  for (uint32_t i = 0; i < capacity && i < K_COUNT; ++i) {
+    if (names) names[i] = kKernelNames[i];
+    if (total_ms) total_ms[i] = f->prof.ms[i];
+    if (launches) launches[i] = f->prof.on ? f->prof.n[i] : f->launches_by[i];
+  }
+  return NSM_OK;
 }
 
 nsm_status nsm_param_count(const nsm_field *f, uint64_t *n_table, uint64_t *n_mlp) {
@@ -396,11 +480,11 @@ nsm_status nsm_update_occupancy(nsm_field *f, nsm_occ_mode mode, const uint8_t *
       uint32_t *d_S = f->ws.offsets;  // offsets[0] doubles as the chunk's sample count
       for (uint64_t first = 0; first < G3; first += chunk) {
         const uint64_t n = (G3 - first < chunk) ? G3 - first : chunk;
-        f->launches += launch_occ_cells(f->cfg.occ_res, first, n, f->ws, d_S, f->stream);
-        f->launches += launch_encode(f->lv, f->fp.theta, f->ws, d_S, f->n_sms, f->stream);
-        f->launches += launch_mlp_forward_simt(f->ms, f->fp.theta + f->fp.n_table, nullptr, f->ws, d_S, 1, f->n_sms, f->stream);
-        f->launches += launch_occ_threshold(f->cfg.occ_res, first, n, f->ws.sigma, f->cfg.occ_sigma_threshold,
-                                            f->fp.occ_bits, f->stream);
+        RUN(f, K_OCC, launch_occ_cells(f->cfg.occ_res, first, n, f->ws, d_S, f->stream));
+        RUN(f, K_ENCODE, launch_encode(f->lv, f->fp.theta, f->ws, d_S, f->n_sms, f->stream));
+        RUN(f, K_MLP_FWD, launch_mlp_forward_simt(f->ms, f->fp.theta + f->fp.n_table, nullptr, f->ws, d_S, 1, f->n_sms, f->stream));
+        RUN(f, K_OCC, launch_occ_threshold(f->cfg.occ_res, first, n, f->ws.sigma, f->cfg.occ_sigma_threshold,
+                                           f->fp.occ_bits, f->stream));
       }
       f->occ_full = false;
       CUDA_TRY(cudaGetLastError());
@@ -476,8 +560,9 @@ static nsm_status render_chunks(nsm_field *f, const nsm_ray_batch *b, float cut,
       cb.origins = b->origins + 3 * (size_t)first;
       cb.dirs = b->dirs + 3 * (size_t)first;
     }
-    enqueue_forward(f, &cb, R, false, 0);
-    f->launches += launch_composite_render(f->ws, R, cut, f->cfg.bg, o_rgb, o_d, o_op, f->stream);
+    enqueue_forward(f, &cb, R, false, 0, false);
+    RUN(f, K_COMPOSITE, launch_composite_render(f->ws, R, cut, f->cfg.bg, o_rgb, o_d, o_op, f->stream));
+    if (f->prof.on) f->prof.collect();
     if (host) {
       CUDA_TRY(cudaMemcpyAsync(rgb + 3 * (size_t)first, o_rgb, sizeof(float) * 3 * R, cudaMemcpyDeviceToHost, f->stream));
       CUDA_TRY(cudaMemcpyAsync(depth + first, o_d, sizeof(float) * R, cudaMemcpyDeviceToHost, f->stream));
@@ -544,13 +629,13 @@ nsm_status nsm_debug_last_step(nsm_field *f, int item, void *d_out, uint64_t cap
   if (src) {
     CUDA_TRY(cudaMemcpyAsync(d_out, src, bytes, cudaMemcpyDeviceToDevice, f->stream));
   } else if (item == NSM_DBG_SAMPLE_X) {
-    f->launches += launch_planes_to_rows(ws.s_x, ws.cap, 3, d_S, (float *)d_out, f->stream);
+    RUN(f, K_DEBUG, launch_planes_to_rows(ws.s_x, ws.cap, 3, d_S, (float *)d_out, f->stream));
   } else if (item == NSM_DBG_E) {
-    f->launches += launch_planes_to_rows(ws.e, ws.cap, f->ms.LF, d_S, (float *)d_out, f->stream);
+    RUN(f, K_DEBUG, launch_planes_to_rows(ws.e, ws.cap, f->ms.LF, d_S, (float *)d_out, f->stream));
   } else if (item == NSM_DBG_SLOTS) {
-    f->launches += launch_debug_slots(f->lv, ws, d_S, (uint32_t *)d_out, nullptr, f->stream);
+    RUN(f, K_DEBUG, launch_debug_slots(f->lv, ws, d_S, (uint32_t *)d_out, nullptr, f->stream));
   } else {
-    f->launches += launch_debug_slots(f->lv, ws, d_S, nullptr, (float *)d_out, f->stream);
+    RUN(f, K_DEBUG, launch_debug_slots(f->lv, ws, d_S, nullptr, (float *)d_out, f->stream));
   }
   CUDA_TRY(cudaGetLastError());
   return NSM_OK;

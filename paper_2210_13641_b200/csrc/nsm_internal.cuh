@@ -59,6 +59,13 @@ struct Workspace {
   float *de;             // [LF][cap]
   // loss accumulators: [0]=sum rgb, [1]=sum depth (doubles); device
   double *loss_acc;
+  unsigned long long *total_samples;  // running sum of S over training steps (device)
+};
+
+// Kernel classes, for launch counting and the optional per-kernel event timing.
+enum KernelId {
+  K_MARCH_COUNT = 0, K_SCAN, K_MARCH_WRITE, K_ENCODE, K_MLP_FWD, K_COMPOSITE, K_MLP_BWD, K_SCATTER,
+  K_ADAM_TABLE, K_ADAM_MLP, K_OCC, K_DEBUG, K_COUNT
 };
 
 struct FieldParams {
@@ -69,8 +76,11 @@ struct FieldParams {
 };
 
 // ---- launchers (each enqueues on `st`, returns the number of kernels launched) ----
-int launch_march(const MarchParams &mp, const uint8_t *bits, const float *origins, const float *dirs,
-                 const Workspace &ws, cudaStream_t st);
+int launch_march_count(const MarchParams &mp, const uint8_t *bits, const float *origins, const float *dirs,
+                       const Workspace &ws, cudaStream_t st);
+int launch_scan(const MarchParams &mp, const Workspace &ws, int count_total, cudaStream_t st);
+int launch_march_write(const MarchParams &mp, const float *origins, const float *dirs, const Workspace &ws,
+                       cudaStream_t st);
 int launch_encode(const LevelTable &lv, const float *theta, const Workspace &ws,
                   const uint32_t *d_S, int n_sms, cudaStream_t st);
 int launch_scatter(const LevelTable &lv, float *grad, uint8_t *touched, const Workspace &ws,
@@ -87,8 +97,10 @@ int launch_composite_train(const Workspace &ws, uint32_t R, const float *rgb, co
                            cudaStream_t st);
 int launch_composite_render(const Workspace &ws, uint32_t R, float cut, const float bg[3],
                             float *out_rgb, float *out_depth, float *out_opacity, cudaStream_t st);
-int launch_adam(const FieldParams &fp, uint32_t F, int sparse, float lr, float beta1, float beta2,
-                float eps, float inv_bc1, float inv_bc2, int n_sms, cudaStream_t st);
+int launch_adam_table(const FieldParams &fp, uint32_t F, int sparse, float lr, float beta1, float beta2,
+                      float eps, float inv_bc1, float inv_bc2, int n_sms, cudaStream_t st);
+int launch_adam_mlp(const FieldParams &fp, float lr, float beta1, float beta2, float eps, float inv_bc1,
+                    float inv_bc2, cudaStream_t st);
 int launch_occ_cells(uint32_t G, uint64_t first_cell, uint64_t n_cells, const Workspace &ws,
                      uint32_t *d_S, cudaStream_t st);
 int launch_occ_threshold(uint32_t G, uint64_t first_cell, uint64_t n_cells, const float *sigma,
