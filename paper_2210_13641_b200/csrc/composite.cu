@@ -44,6 +44,7 @@ __global__ void __launch_bounds__(256) composite_kernel(Workspace ws, uint32_t R
                                                         float *__restrict__ out_opacity) {
   const uint32_t r = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
   float l_rgb = 0.0f, l_d = 0.0f;  // lane 0 holds the ray's loss terms
+  float gmax = 0.0f;               // max |gradient entering the MLP backward| seen by this thread
   if (r < R) {
     const uint32_t off = ws.offsets[r], n = ws.offsets[r + 1] - off;
     // ---- forward (S8) ----
@@ -121,8 +122,12 @@ __global__ void __launch_bounds__(256) composite_kernel(Workspace ws, uint32_t R
         float sfx_incl = warp_suffix_scan(wq, lane);
         float sfx = suffix_carry + (sfx_incl - wq);                            // sum_{j>i} w_j q_j
         if (ok) {
-          ws.dsigma[s] = dl * (Tn * q - sfx - T_end * bgdot);
+          const float ds = dl * (Tn * q - sfx - T_end * bgdot);
+          ws.dsigma[s] = ds;
           ws.drgb[3 * s] = w * gC0; ws.drgb[3 * s + 1] = w * gC1; ws.drgb[3 * s + 2] = w * gC2;
+          // what S11 starts from: dL/dg0 = dsigma*sigma and dL/d(pre-sigmoid) = dc * c(1-c)
+          gmax = fmaxf(gmax, fabsf(ds * sg));
+          gmax = fmaxf(gmax, 0.25f * w * fmaxf(fabsf(gC0), fmaxf(fabsf(gC1), fabsf(gC2))));
         }
         suffix_carry += __shfl_sync(0xffffffffu, sfx_incl, 0);
       }
@@ -139,6 +144,9 @@ __global__ void __launch_bounds__(256) composite_kernel(Workspace ws, uint32_t R
       for (uint32_t w = 0; w < (blockDim.x >> 5); ++w) acc += (double)red[threadIdx.x][w];
       atomicAdd(ws.loss_acc + threadIdx.x, acc);
     }
+#pragma unroll
+    for (int sft = 16; sft > 0; sft >>= 1) gmax = fmaxf(gmax, __shfl_xor_sync(0xffffffffu, gmax, sft));
+    if (lane == 0 && gmax > 0.f && isfinite(gmax)) atomicMax(ws.grad_absmax, __float_as_uint(gmax));
   }
 }
 

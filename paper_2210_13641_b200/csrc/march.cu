@@ -106,13 +106,14 @@ __global__ void __launch_bounds__(256) march_count_kernel(MarchParams mp, const 
 // reset of the loss accumulators.  Deterministic.
 __global__ void __launch_bounds__(1024) scan_counts_kernel(const uint32_t *__restrict__ counts,
                                                            uint32_t *__restrict__ offsets, uint32_t R,
-                                                           double *loss_acc, unsigned long long *total) {
+                                                           double *loss_acc, unsigned long long *total, uint32_t *absmax) {
   __shared__ uint32_t warp_sums[32];
   __shared__ uint32_t carry_s;
   const uint32_t tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
   if (tid == 0) {
     carry_s = 0;
     if (loss_acc) { loss_acc[0] = 0.0; loss_acc[1] = 0.0; }
+    if (absmax) *absmax = 0u;
   }
   __syncthreads();
   for (uint32_t base = 0; base < R; base += 1024) {
@@ -220,7 +221,7 @@ int launch_march_count(const MarchParams &mp, const uint8_t *bits, const float *
 
 int launch_scan(const MarchParams &mp, const Workspace &ws, int count_total, cudaStream_t st) {
   scan_counts_kernel<<<1, 1024, 0, st>>>(ws.counts, ws.offsets, mp.R, ws.loss_acc,
-                                         count_total ? ws.total_samples : nullptr);
+                                         count_total ? ws.total_samples : nullptr, ws.grad_absmax);
   return 1;
 }
 

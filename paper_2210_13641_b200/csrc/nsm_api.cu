@@ -89,6 +89,8 @@ struct nsm_field {
   float *stage_out = nullptr;     // render outputs [max_rays * 5]
   struct HostStats { double acc[2]; uint32_t S; } *pinned = nullptr;
   const char *mlp_path = "simt_fp32";
+  bool use_tc = false;   // tcgen05 MLP kernels (16-bit configurations with supported shapes)
+  bool tc_fwd = true, tc_bwd = true;  // debugging: NSM_TC_MODE=1 forward only, 2 backward only
 
   template <typename T>
   cudaError_t alloc(T **p, size_t n, bool zero = true) {
@@ -213,7 +215,11 @@ void enqueue_forward(nsm_field *f, const nsm_ray_batch *b, uint32_t R, bool jitt
   RUN(f, K_SCAN, launch_scan(mp, f->ws, train ? 1 : 0, f->stream));
   RUN(f, K_MARCH_WRITE, launch_march_write(mp, b->origins, b->dirs, f->ws, f->stream));
   RUN(f, K_ENCODE, launch_encode(f->lv, f->fp.theta, f->ws, d_S, f->n_sms, f->stream));
-  RUN(f, K_MLP_FWD, launch_mlp_forward_simt(f->ms, f->fp.theta + f->fp.n_table, b->dirs, f->ws, d_S, 0, f->n_sms, f->stream));
+  if (f->use_tc && f->tc_fwd)
+    RUN(f, K_MLP_FWD, launch_mlp_forward_tc(f->ms, f->cfg.mlp_precision == NSM_MLP_BF16, f->fp.theta + f->fp.n_table, b->dirs,
+                                            f->ws, d_S, 0, 1, f->n_sms, f->stream));
+  else
+    RUN(f, K_MLP_FWD, launch_mlp_forward_simt(f->ms, f->fp.theta + f->fp.n_table, b->dirs, f->ws, d_S, 0, f->n_sms, f->stream));
 }
 
 nsm_status clear_grads_if_dirty(nsm_field *f) {
@@ -232,8 +238,12 @@ nsm_status enqueue_backward(nsm_field *f, const nsm_ray_batch *b, float lambda_d
   if (st != NSM_OK) return st;
   enqueue_forward(f, b, R, f->cfg.jitter != 0, f->step + 1, true);
   RUN(f, K_COMPOSITE, launch_composite_train(f->ws, R, b->rgb, b->depth, b->depth_var, lambda_d, f->cfg.bg, f->stream));
-  RUN(f, K_MLP_BWD, launch_mlp_backward_simt(f->ms, f->fp.theta + f->fp.n_table, f->fp.grad + f->fp.n_table, b->dirs,
-                                             f->ws, d_S, f->n_sms, f->stream));
+  if (f->use_tc && f->tc_bwd)
+    RUN(f, K_MLP_BWD, launch_mlp_backward_tc(f->ms, f->cfg.mlp_precision == NSM_MLP_BF16, f->fp.theta + f->fp.n_table,
+                                             f->fp.grad + f->fp.n_table, b->dirs, f->ws, d_S, f->n_sms, f->stream));
+  else
+    RUN(f, K_MLP_BWD, launch_mlp_backward_simt(f->ms, f->fp.theta + f->fp.n_table, f->fp.grad + f->fp.n_table, b->dirs,
+                                               f->ws, d_S, f->n_sms, f->stream));
   RUN(f, K_SCATTER, launch_scatter(f->lv, f->fp.grad, f->fp.touched, f->ws, d_S, f->n_sms, f->stream));
   f->grads_dirty = true;
   f->last_R = R;
@@ -342,6 +352,14 @@ nsm_status nsm_create_field(const nsm_field_config *cfg, void *cuda_stream, nsm_
                 (size_t)prop.sharedMemPerBlockOptin);
   }
 
+  // 16-bit configurations run the MLPs on tcgen05 when the shapes fit its tiles (NSM_FORCE_SIMT=1
+  // keeps the fp32 CUDA-core kernels, for A/B debugging)
+  const char *force = std::getenv("NSM_FORCE_SIMT");
+  if (cfg->mlp_precision != NSM_MLP_FP32 && mlp_tc_supported(ms) && !(force && force[0] == '1')) {
+    f->use_tc = true;
+    if (const char *mode = std::getenv("NSM_TC_MODE")) { f->tc_fwd = (atoi(mode) & 1) != 0; f->tc_bwd = (atoi(mode) & 2) != 0; }
+    f->mlp_path = cfg->mlp_precision == NSM_MLP_BF16 ? "tcgen05_bf16" : "tcgen05_f16";
+  }
   FieldParams &fp = f->fp;
   fp.n_entries = f->lv.offset[cfg->n_levels];
   fp.n_table = fp.n_entries * cfg->n_features;
@@ -365,7 +383,7 @@ nsm_status nsm_create_field(const nsm_field_config *cfg, void *cuda_stream, nsm_
   A(f->alloc(&ws.h2, (ms.n_color_layers == 2 ? ms.Hc : 1) * cap));
   A(f->alloc(&ws.sigma, cap)); A(f->alloc(&ws.rgb, 3 * cap)); A(f->alloc(&ws.T_excl, cap));
   A(f->alloc(&ws.dsigma, cap)); A(f->alloc(&ws.drgb, 3 * cap)); A(f->alloc(&ws.de, ms.LF * cap));
-  A(f->alloc(&ws.loss_acc, 2)); A(f->alloc(&ws.total_samples, 1));
+  A(f->alloc(&ws.loss_acc, 2)); A(f->alloc(&ws.total_samples, 1)); A(f->alloc(&ws.grad_absmax, 1));
   A(f->alloc(&f->stage_dev, 11 * (size_t)R)); A(f->alloc(&f->stage_out, 5 * (size_t)R));
   if (e == cudaSuccess) e = cudaMallocHost((void **)&f->pinned, sizeof(*f->pinned));
   if (e != cudaSuccess) {
@@ -482,7 +500,11 @@ nsm_status nsm_update_occupancy(nsm_field *f, nsm_occ_mode mode, const uint8_t *
         const uint64_t n = (G3 - first < chunk) ? G3 - first : chunk;
         RUN(f, K_OCC, launch_occ_cells(f->cfg.occ_res, first, n, f->ws, d_S, f->stream));
         RUN(f, K_ENCODE, launch_encode(f->lv, f->fp.theta, f->ws, d_S, f->n_sms, f->stream));
-        RUN(f, K_MLP_FWD, launch_mlp_forward_simt(f->ms, f->fp.theta + f->fp.n_table, nullptr, f->ws, d_S, 1, f->n_sms, f->stream));
+        if (f->use_tc)
+          RUN(f, K_MLP_FWD, launch_mlp_forward_tc(f->ms, f->cfg.mlp_precision == NSM_MLP_BF16, f->fp.theta + f->fp.n_table, nullptr,
+                                                  f->ws, d_S, 1, 0, f->n_sms, f->stream));
+        else
+          RUN(f, K_MLP_FWD, launch_mlp_forward_simt(f->ms, f->fp.theta + f->fp.n_table, nullptr, f->ws, d_S, 1, f->n_sms, f->stream));
         RUN(f, K_OCC, launch_occ_threshold(f->cfg.occ_res, first, n, f->ws.sigma, f->cfg.occ_sigma_threshold,
                                            f->fp.occ_bits, f->stream));
       }

@@ -60,6 +60,7 @@ struct Workspace {
   // loss accumulators: [0]=sum rgb, [1]=sum depth (doubles); device
   double *loss_acc;
   unsigned long long *total_samples;  // running sum of S over training steps (device)
+  uint32_t *grad_absmax;              // bits of max |dL/d(pre-activation)| entering S11 this step (loss scale)
 };
 
 // Kernel classes, for launch counting and the optional per-kernel event timing.
@@ -92,6 +93,11 @@ int launch_mlp_backward_simt(const MlpShape &ms, const float *theta_mlp, float *
                              const float *dirs, const Workspace &ws, const uint32_t *d_S, int n_sms,
                              cudaStream_t st);
 size_t mlp_simt_smem_bytes(const MlpShape &ms, int backward);
+bool mlp_tc_supported(const MlpShape &ms);
+int launch_mlp_backward_tc(const MlpShape &ms, int bf16, const float *theta_mlp, float *grad_mlp, const float *dirs,
+                           const Workspace &ws, const uint32_t *d_S, int n_sms, cudaStream_t st);
+int launch_mlp_forward_tc(const MlpShape &ms, int bf16, const float *theta_mlp, const float *dirs, const Workspace &ws,
+                          const uint32_t *d_S, int density_only, int write_planes, int n_sms, cudaStream_t st);
 int launch_composite_train(const Workspace &ws, uint32_t R, const float *rgb, const float *depth,
                            const float *depth_var, float lambda_d, const float bg[3],
                            cudaStream_t st);
