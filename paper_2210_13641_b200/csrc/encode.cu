@@ -6,6 +6,9 @@
 // consecutive samples (neighbours along a ray) of ONE level: their corners share cache lines at
 // coarse levels, the whole chip works on one level's table slice at a time (L2/L1 locality), and
 // the feature planes e[l*F+f][s] are written / read fully coalesced.
+#include <cuda_bf16.h>
+#include <cuda_fp16.h>
+
 #include "nsm_internal.cuh"
 
 namespace {
@@ -74,31 +77,48 @@ __device__ __forceinline__ void load_entry(const float *p, float out[F]) {
   }
 }
 
-template <int F>
+// MODE 0: e -> fp32 planes [l*F+f][cap].  MODE 1 / 2: e -> fp16 / bf16 operand-tile blob of the
+// tensor-core MLP kernels ([tile][8-column panel][128 rows][8 x 16 bit], mlp_tc.cu); the rows of
+// the last tile beyond S are zero-filled so the MMA never reads stale data.
+template <int F, int MODE>
 __global__ void __launch_bounds__(256) encode_forward_kernel(LevelTable lv, const float *__restrict__ theta,
                                                              Workspace ws, const uint32_t *__restrict__ d_S) {
   const uint64_t S = *d_S;
-  const uint64_t total = S * lv.n_levels;
+  const uint64_t S_it = MODE == 0 ? S : ((S + NSM_TILE - 1) / NSM_TILE) * NSM_TILE;
+  const uint64_t total = S_it * lv.n_levels;
+  const uint32_t LF = lv.n_levels * F;
   for (uint64_t wi = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; wi < total;
        wi += (uint64_t)gridDim.x * blockDim.x) {
-    const uint32_t l = (uint32_t)(wi / S);
-    const uint64_t s = wi - (uint64_t)l * S;
-    CornerIndex ci = corner_index(lv, l, ws.s_x[s], ws.s_x[ws.cap + s], ws.s_x[2 * ws.cap + s]);
-    const float *tab = theta + lv.offset[l] * F;
-    float v[8][F];
-#pragma unroll
-    for (int k = 0; k < 8; ++k) load_entry<F>(tab + (size_t)ci.slot[k] * F, v[k]);  // 8 gathers in flight
+    const uint32_t l = (uint32_t)(wi / S_it);
+    const uint64_t s = wi - (uint64_t)l * S_it;
     float acc[F];
 #pragma unroll
     for (int f = 0; f < F; ++f) acc[f] = 0.0f;
+    if (s < S) {
+      CornerIndex ci = corner_index(lv, l, ws.s_x[s], ws.s_x[ws.cap + s], ws.s_x[2 * ws.cap + s]);
+      const float *tab = theta + lv.offset[l] * F;
+      float v[8][F];
 #pragma unroll
-    for (int k = 0; k < 8; ++k) {
-      float om = corner_weight(k, ci.w);
+      for (int k = 0; k < 8; ++k) load_entry<F>(tab + (size_t)ci.slot[k] * F, v[k]);  // 8 gathers in flight
 #pragma unroll
-      for (int f = 0; f < F; ++f) acc[f] = fmaf(om, v[k][f], acc[f]);
+      for (int k = 0; k < 8; ++k) {
+        float om = corner_weight(k, ci.w);
+#pragma unroll
+        for (int f = 0; f < F; ++f) acc[f] = fmaf(om, v[k][f], acc[f]);
+      }
     }
+    if (MODE == 0) {
 #pragma unroll
-    for (int f = 0; f < F; ++f) ws.e[(size_t)(l * F + f) * ws.cap + s] = acc[f];
+      for (int f = 0; f < F; ++f) ws.e[(size_t)(l * F + f) * ws.cap + s] = acc[f];
+    } else {
+      const uint32_t c = l * F;   // F consecutive columns never straddle an 8-column panel (F | 8)
+      uint8_t *dst = ws.blob_e + (s >> 7) * ((size_t)LF * NSM_TILE * 2) + (c >> 3) * (NSM_TILE * 16) + (s & 127) * 16 + (c & 7) * 2;
+#pragma unroll
+      for (int f = 0; f < F; ++f) {
+        if (MODE == 1) reinterpret_cast<__half *>(dst)[f] = __float2half_rn(acc[f]);
+        else reinterpret_cast<__nv_bfloat16 *>(dst)[f] = __float2bfloat16_rn(acc[f]);
+      }
+    }
   }
 }
 
@@ -177,14 +197,22 @@ __global__ void planes_to_rows_kernel(const float *__restrict__ planes, uint64_t
 
 }  // namespace
 
-int launch_encode(const LevelTable &lv, const float *theta, const Workspace &ws, const uint32_t *d_S,
+template <int F>
+static void launch_encode_f(const LevelTable &lv, const float *theta, const Workspace &ws, const uint32_t *d_S, int out_mode,
+                            dim3 grid, dim3 block, cudaStream_t st) {
+  if (out_mode == 0) encode_forward_kernel<F, 0><<<grid, block, 0, st>>>(lv, theta, ws, d_S);
+  else if (out_mode == 1) encode_forward_kernel<F, 1><<<grid, block, 0, st>>>(lv, theta, ws, d_S);
+  else encode_forward_kernel<F, 2><<<grid, block, 0, st>>>(lv, theta, ws, d_S);
+}
+
+int launch_encode(const LevelTable &lv, const float *theta, const Workspace &ws, const uint32_t *d_S, int out_mode,
                   int n_sms, cudaStream_t st) {
   dim3 grid(n_sms * 8), block(256);
   switch (lv.n_features) {
-    case 1: encode_forward_kernel<1><<<grid, block, 0, st>>>(lv, theta, ws, d_S); break;
-    case 2: encode_forward_kernel<2><<<grid, block, 0, st>>>(lv, theta, ws, d_S); break;
-    case 4: encode_forward_kernel<4><<<grid, block, 0, st>>>(lv, theta, ws, d_S); break;
-    default: encode_forward_kernel<8><<<grid, block, 0, st>>>(lv, theta, ws, d_S); break;
+    case 1: launch_encode_f<1>(lv, theta, ws, d_S, out_mode, grid, block, st); break;
+    case 2: launch_encode_f<2>(lv, theta, ws, d_S, out_mode, grid, block, st); break;
+    case 4: launch_encode_f<4>(lv, theta, ws, d_S, out_mode, grid, block, st); break;
+    default: launch_encode_f<8>(lv, theta, ws, d_S, out_mode, grid, block, st); break;
   }
   return 1;
 }

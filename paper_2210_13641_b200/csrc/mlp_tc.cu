@@ -1,14 +1,18 @@
-// mlp_tc.cu — S5/S6/S7 (and S11) on the 5th-generation tensor cores: the density and colour MLPs
-// of PAPER.md:143,151 as 128-sample tcgen05.mma tiles (M = 128 samples, N = layer width, K = input
+// mlp_tc.cu — S5/S6/S7 and S11 on the 5th-generation tensor cores: the density and colour MLPs of
+// PAPER.md:143,151 as 128-sample tcgen05.mma tiles (M = 128 samples, N = layer width, K = input
 // width; 16-bit operands in shared memory, fp32 accumulators in TMEM).
 //
-// One CTA (4 warps) owns a 128-sample tile; thread r owns sample row r: it builds its row of the
-// layer input in shared memory (UMMA canonical no-swizzle K-major layout, 16-byte chunks at a 16 B
-// stride across threads: conflict-free), ONE thread issues the layer's tcgen05.mma k-steps and a
-// tcgen05.commit onto an mbarrier, everyone waits on it, reads its accumulator row back with
-// tcgen05.ld (TMEM lane = sample row), applies the activation and writes the next layer's input.
-// Weights are converted fp32 -> 16-bit and staged in shared memory once per CTA (persistent over
-// tiles).  Activations never leave the SM between layers.
+// One CTA (4 warps) owns a 128-sample tile; thread r owns sample row r: it writes its row of the
+// next layer's input into shared memory (UMMA canonical no-swizzle layout: 16-byte chunks at a 16 B
+// stride across threads, conflict-free), ONE thread issues the layer's tcgen05.mma k-steps and a
+// tcgen05.commit onto an mbarrier, everyone waits on it and reads its accumulator row back with
+// tcgen05.ld (TMEM lane = sample row).  Activations never leave the SM between layers.
+//
+// Everything that crosses HBM is stored as the exact byte image of the shared-memory operand tile
+// ("blob": [tile][8-column panel][128 rows][8 x 16 bit]), so it comes back with ONE TMA bulk copy
+// (cp.async.bulk, no tensor map needed) straight into the MMA operand buffer: the encoder's output
+// e, the activations saved for the backward pass, and the 16-bit weight images (packed once per
+// step by pack_weights_kernel, not converted per CTA).
 #include "nsm_internal.cuh"
 #include "tc_common.cuh"
 
@@ -22,30 +26,46 @@ constexpr uint32_t CIP = 32;    // colour-MLP input width padded to a k-step mul
 constexpr uint32_t ROWS = NSM_TILE;
 constexpr uint32_t PANEL = ROWS * 16;  // bytes of one 8-column panel of a 128-row tile
 
-// TMEM column map (fp32 accumulators, 128 lanes = sample rows)
-constexpr uint32_t COL_D1 = 0, COL_D2 = 64, COL_C1 = 96, COL_C2 = 160, COL_C3 = 224, FWD_COLS = 256;
-
-struct FwdSmem {
-  static constexpr uint32_t wd1 = 0;                         // [64][LF<=64]
-  static constexpr uint32_t wd2 = wd1 + H * 64 * 2;          // [16][64]
-  static constexpr uint32_t wc1 = wd2 + DO * H * 2;          // [64][32]
-  static constexpr uint32_t wc2 = wc1 + H * CIP * 2;         // [64][64]
-  static constexpr uint32_t wc3 = wc2 + H * H * 2;           // [16][64]
-  static constexpr uint32_t bufA = wc3 + 16 * H * 2;         // [128][64]
-  static constexpr uint32_t bufB = bufA + ROWS * H * 2;      // [128][64]
-  static constexpr uint32_t bar = bufB + ROWS * H * 2;       // mbarrier
-  static constexpr uint32_t tmem = bar + 8;
-  static constexpr uint32_t total = tmem + 8;
+// ---- weight images (byte images of the shared-memory weight regions) ---------------------------
+// forward: B tiles [N = n_out pad][K = n_in pad] (K-major);  backward: transposed tiles [n_in pad][n_out pad]
+struct WImg {
+  // forward region
+  static constexpr uint32_t f_d1 = 0;                       // [64][64 max]  (LF <= 64 columns used)
+  static constexpr uint32_t f_d2 = f_d1 + H * 64 * 2;       // [16][64]
+  static constexpr uint32_t f_c1 = f_d2 + DO * H * 2;       // [64][32]
+  static constexpr uint32_t f_c2 = f_c1 + H * CIP * 2;      // [64][64]
+  static constexpr uint32_t f_c3 = f_c2 + H * H * 2;        // [16][64]
+  static constexpr uint32_t f_total = f_c3 + 16 * H * 2;    // 24576
+  // backward region
+  static constexpr uint32_t b_c3 = 0;                       // [64][16]
+  static constexpr uint32_t b_c2 = b_c3 + H * 16 * 2;       // [64][64]
+  static constexpr uint32_t b_c1 = b_c2 + H * H * 2;        // [32][64]
+  static constexpr uint32_t b_d2 = b_c1 + CIP * H * 2;      // [64][16]
+  static constexpr uint32_t b_d1 = b_d2 + H * 16 * 2;       // [64 max][64]
+  static constexpr uint32_t b_total = b_d1 + 64 * H * 2;    // 24576
 };
 
-// fp32 canonical W[n_out][n_in] (global) -> 16-bit operand tile [NP][KP] in shared memory, zero padded
+// fp32 master weights -> both 16-bit images.  Padding elements are written as zero.
 template <typename T>
-__device__ void stage_weight(uint8_t *tile, const float *__restrict__ W, uint32_t n_out, uint32_t n_in, uint32_t NP,
-                             uint32_t KP) {
-  for (uint32_t i = threadIdx.x; i < NP * KP; i += blockDim.x) {
-    const uint32_t n = i / KP, k = i - n * KP;
-    const float v = (n < n_out && k < n_in) ? __ldg(W + n * n_in + k) : 0.f;
-    *reinterpret_cast<T *>(tile + tile_off(NP, n, k)) = T(v);
+__global__ void pack_weights_kernel(MlpShape ms, const float *__restrict__ Wm, uint8_t *__restrict__ img_f,
+                                    uint8_t *__restrict__ img_b) {
+  struct M { uint32_t off, n_out, n_in, f_off, f_NP, f_KP, b_off, b_NP, b_KP; };
+  const M mats[5] = {{ms.o_d1, H, ms.LF, WImg::f_d1, H, ms.LF, WImg::b_d1, ms.LF, H},
+                     {ms.o_d2, DO, H, WImg::f_d2, DO, H, WImg::b_d2, H, 16},
+                     {ms.o_c1, H, ms.Ci, WImg::f_c1, H, CIP, WImg::b_c1, CIP, H},
+                     {ms.o_c2, ms.n_color_layers == 2 ? H : 0, H, WImg::f_c2, H, H, WImg::b_c2, H, H},
+                     {ms.o_c3, 3, H, WImg::f_c3, 16, H, WImg::b_c3, H, 16}};
+  const M m = mats[blockIdx.x];
+  // forward tile: element (n, k) = W[n][k];  backward tile: element (i, o) = W[o][i]
+  for (uint32_t idx = threadIdx.x; idx < m.f_NP * m.f_KP; idx += blockDim.x) {
+    const uint32_t n = idx / m.f_KP, k = idx - n * m.f_KP;
+    const float v = (n < m.n_out && k < m.n_in) ? Wm[m.off + n * m.n_in + k] : 0.f;
+    *reinterpret_cast<T *>(img_f + m.f_off + tile_off(m.f_NP, n, k)) = T(v);
+  }
+  for (uint32_t idx = threadIdx.x; idx < m.b_NP * m.b_KP; idx += blockDim.x) {
+    const uint32_t i = idx / m.b_KP, o = idx - i * m.b_KP;
+    const float v = (i < m.n_in && o < m.n_out) ? Wm[m.off + o * m.n_in + i] : 0.f;
+    *reinterpret_cast<T *>(img_b + m.b_off + tile_off(m.b_NP, i, o)) = T(v);
   }
 }
 
@@ -78,75 +98,108 @@ __device__ __forceinline__ void sh_row(uint32_t n, float x, float y, float z, fl
   Y[15] = 0.5900435899266435f * x * (xx - 3.f * yy);
 }
 
+// 16 accumulator columns -> (optional ReLU) -> this thread's row of a shared tile and of a global blob tile
+template <typename T, bool RELU>
+__device__ __forceinline__ void emit16(float *v, uint8_t *smem_tile, uint8_t *blob_tile, uint32_t c0, bool valid) {
+  if (RELU) {
+#pragma unroll
+    for (int j = 0; j < 16; ++j) v[j] = fmaxf(v[j], 0.f);
+  }
+  uint4 q0, q1;
+  q0.x = pack2<T>(v[0], v[1]); q0.y = pack2<T>(v[2], v[3]); q0.z = pack2<T>(v[4], v[5]); q0.w = pack2<T>(v[6], v[7]);
+  q1.x = pack2<T>(v[8], v[9]); q1.y = pack2<T>(v[10], v[11]); q1.z = pack2<T>(v[12], v[13]); q1.w = pack2<T>(v[14], v[15]);
+  const uint32_t o0 = tile_off(ROWS, threadIdx.x, c0), o1 = tile_off(ROWS, threadIdx.x, c0 + 8);
+  *reinterpret_cast<uint4 *>(smem_tile + o0) = q0;
+  *reinterpret_cast<uint4 *>(smem_tile + o1) = q1;
+  if (blob_tile) {   // rows of invalid samples are stored as zeros so the backward wgrad never sees garbage
+    const uint4 z = make_uint4(0, 0, 0, 0);
+    *reinterpret_cast<uint4 *>(blob_tile + o0) = valid ? q0 : z;
+    *reinterpret_cast<uint4 *>(blob_tile + o1) = valid ? q1 : z;
+  }
+}
+
+// ------------------------------------------------------------------------------------- forward
+constexpr uint32_t COL_D1 = 0, COL_D2 = 64, COL_C1 = 96, COL_C2 = 160, COL_C3 = 224, FWD_COLS = 256;
+
+struct FwdSmem {
+  static constexpr uint32_t w = 0;                                // weight image (WImg forward region)
+  static constexpr uint32_t bufE = w + WImg::f_total;             // [128][64] encoder output tile (TMA destination)
+  static constexpr uint32_t bufA = bufE + ROWS * H * 2;           // [128][64]
+  static constexpr uint32_t bufB = bufA + ROWS * H * 2;           // [128][64]
+  static constexpr uint32_t bar_mma = bufB + ROWS * H * 2;
+  static constexpr uint32_t bar_w = bar_mma + 8;
+  static constexpr uint32_t bar_e = bar_w + 8;
+  static constexpr uint32_t tmem = bar_e + 8;
+  static constexpr uint32_t total = tmem + 8;
+};
+
 template <typename T>
-__global__ void __launch_bounds__(128) mlp_forward_tc_kernel(MlpShape ms, const float *__restrict__ Wm,
-                                                             const float *__restrict__ dirs, Workspace ws,
+__global__ void __launch_bounds__(128) mlp_forward_tc_kernel(MlpShape ms, const float *__restrict__ dirs, Workspace ws,
                                                              const uint32_t *__restrict__ d_S, int density_only,
-                                                             int write_planes) {
+                                                             int save_blobs) {
   extern __shared__ __align__(1024) uint8_t smem[];
   const uint32_t tid = threadIdx.x, warp = tid >> 5;
   const uint32_t sbase = smem_u32(smem);
-  const uint32_t bar = sbase + FwdSmem::bar;
+  const uint32_t bar_mma = sbase + FwdSmem::bar_mma, bar_w = sbase + FwdSmem::bar_w, bar_e = sbase + FwdSmem::bar_e;
   const uint32_t LF = ms.LF;
+  const uint32_t e_bytes = LF * ROWS * 2;
+  const uint64_t S = *d_S;
+  if ((uint64_t)blockIdx.x * ROWS >= S) return;
 
-  stage_weight<T>(smem + FwdSmem::wd1, Wm + ms.o_d1, H, LF, H, LF);
-  stage_weight<T>(smem + FwdSmem::wd2, Wm + ms.o_d2, DO, H, DO, H);
-  if (!density_only) {
-    stage_weight<T>(smem + FwdSmem::wc1, Wm + ms.o_c1, H, ms.Ci, H, CIP);
-    if (ms.n_color_layers == 2) stage_weight<T>(smem + FwdSmem::wc2, Wm + ms.o_c2, H, H, H, H);
-    stage_weight<T>(smem + FwdSmem::wc3, Wm + ms.o_c3, 3, H, 16, H);
+  if (tid == 0) {
+    mbar_init(bar_mma, 1); mbar_init(bar_w, 1); mbar_init(bar_e, 1);
+    fence_async_smem();
+    mbar_expect_tx(bar_w, WImg::f_total);
+    bulk_g2s(sbase + FwdSmem::w, ws.wimg_fwd, WImg::f_total, bar_w);
+    mbar_expect_tx(bar_e, e_bytes);
+    bulk_g2s(sbase + FwdSmem::bufE, ws.blob_e + (size_t)blockIdx.x * e_bytes, e_bytes, bar_e);
   }
-  if (tid == 0) mbar_init(bar, 1);
   if (warp == 0) tmem_alloc<FWD_COLS>(sbase + FwdSmem::tmem);
-  fence_async_smem();
   fence_before();
   __syncthreads();
   fence_after();
   const uint32_t tmem_base = *reinterpret_cast<volatile uint32_t *>(smem + FwdSmem::tmem);
   const uint32_t tlane = tmem_base + ((warp * 32u) << 16);
-  uint32_t phase = 0;
+  uint32_t ph_mma = 0, ph_e = 0;
   const uint32_t fmt = Fmt<T>::id;
   uint8_t *bufA = smem + FwdSmem::bufA, *bufB = smem + FwdSmem::bufB;
-  const uint32_t sA = sbase + FwdSmem::bufA, sB = sbase + FwdSmem::bufB;
+  const uint32_t sE = sbase + FwdSmem::bufE, sA = sbase + FwdSmem::bufA, sB = sbase + FwdSmem::bufB, sW = sbase + FwdSmem::w;
+  if (tid == 0) mbar_wait(bar_w, 0);
 
-  const uint64_t S = *d_S;
-  for (uint64_t base = (uint64_t)blockIdx.x * ROWS; base < S; base += (uint64_t)gridDim.x * ROWS) {
-    const uint64_t s = base + tid;
+  for (uint64_t tile = blockIdx.x; tile * ROWS < S; tile += gridDim.x) {
+    const uint64_t s = tile * ROWS + tid;
     const bool valid = s < S;
     float v[16];
-    // ---- layer input: e row -> bufA
-    for (uint32_t c0 = 0; c0 < LF; c0 += 8) {
-#pragma unroll
-      for (int j = 0; j < 8; ++j) v[j] = valid ? ws.e[(size_t)(c0 + j) * ws.cap + s] : 0.f;
-      store8<T>(bufA, ROWS, tid, c0, v);
+    // ---- density hidden layer: A = encoder tile (already in shared memory via TMA)
+    if (tid == 0) {
+      mbar_wait(bar_e, ph_e);
+      fence_after();
+      issue_layer(tmem_base + COL_D1, sE, sW + WImg::f_d1, LF, H, H, fmt, bar_mma);
     }
-    fence_async_smem(); fence_before(); __syncthreads();
-    if (tid == 0) { fence_after(); issue_layer(tmem_base + COL_D1, sA, sbase + FwdSmem::wd1, LF, H, H, fmt, bar); }
-    mbar_wait(bar, phase); phase ^= 1; fence_after();
-    // ---- h = ReLU(.) -> bufB
+    ph_e ^= 1;
+    mbar_wait(bar_mma, ph_mma); ph_mma ^= 1; fence_after();
+    if (tid == 0) {   // bufE is free again: prefetch the CTA's next encoder tile
+      const uint64_t nxt = tile + gridDim.x;
+      if (nxt * ROWS < S) {
+        mbar_expect_tx(bar_e, e_bytes);
+        bulk_g2s(sE, ws.blob_e + (size_t)nxt * e_bytes, e_bytes, bar_e);
+      }
+    }
+    uint8_t *blob_hd = (save_blobs && !density_only) ? ws.blob_hd + (size_t)tile * (H * ROWS * 2) : nullptr;
 #pragma unroll
     for (uint32_t c0 = 0; c0 < H; c0 += 16) {
       tmem_ld16(tlane + COL_D1 + c0, v);
       tmem_ld_wait();
-#pragma unroll
-      for (int j = 0; j < 16; ++j) v[j] = fmaxf(v[j], 0.f);
-      store8<T>(bufB, ROWS, tid, c0, v);
-      store8<T>(bufB, ROWS, tid, c0 + 8, v + 8);
-      if (write_planes && valid && !density_only)
-#pragma unroll
-        for (int j = 0; j < 16; ++j) ws.hd[(size_t)(c0 + j) * ws.cap + s] = v[j];
+      emit16<T, true>(v, bufB, blob_hd, c0, valid);
     }
     fence_async_smem(); fence_before(); __syncthreads();
-    if (tid == 0) { fence_after(); issue_layer(tmem_base + COL_D2, sB, sbase + FwdSmem::wd2, H, DO, DO, fmt, bar); }
-    mbar_wait(bar, phase); phase ^= 1; fence_after();
+    if (tid == 0) { fence_after(); issue_layer(tmem_base + COL_D2, sB, sW + WImg::f_d2, H, DO, DO, fmt, bar_mma); }
+    mbar_wait(bar_mma, ph_mma); ph_mma ^= 1; fence_after();
     float g[16];
     tmem_ld16(tlane + COL_D2, g);
     tmem_ld_wait();
     if (valid) ws.sigma[s] = expf(fminf(fmaxf(g[0], -15.f), 15.f));
-    if (density_only) { fence_before(); __syncthreads(); continue; }
-    if (write_planes && valid)
-#pragma unroll
-      for (int j = 0; j < 16; ++j) ws.g[(size_t)j * ws.cap + s] = g[j];
+    if (density_only) { fence_before(); continue; }
     // ---- colour input [g slice, Y(d), 0 pad] -> bufA (K = 32)
     {
       float ci[CIP];
@@ -161,46 +214,37 @@ __global__ void __launch_bounds__(128) mlp_forward_tc_kernel(MlpShape ms, const 
       float Y[16];
       sh_row(ms.sh_degree, dx, dy, dz, Y);
       for (uint32_t j = 0; j < ms.n_sh; ++j) ci[ms.geo_cnt + j] = Y[j];
-#pragma unroll
-      for (uint32_t c0 = 0; c0 < CIP; c0 += 8) store8<T>(bufA, ROWS, tid, c0, ci + c0);
+      uint8_t *blob_ci = save_blobs ? ws.blob_ci + (size_t)tile * (CIP * ROWS * 2) : nullptr;
+      emit16<T, false>(ci, bufA, blob_ci, 0, valid);
+      emit16<T, false>(ci + 16, bufA, blob_ci, 16, valid);
     }
     fence_async_smem(); fence_before(); __syncthreads();
-    if (tid == 0) { fence_after(); issue_layer(tmem_base + COL_C1, sA, sbase + FwdSmem::wc1, CIP, H, H, fmt, bar); }
-    mbar_wait(bar, phase); phase ^= 1; fence_after();
+    if (tid == 0) { fence_after(); issue_layer(tmem_base + COL_C1, sA, sW + WImg::f_c1, CIP, H, H, fmt, bar_mma); }
+    mbar_wait(bar_mma, ph_mma); ph_mma ^= 1; fence_after();
+    uint8_t *blob_h1 = save_blobs ? ws.blob_h1 + (size_t)tile * (H * ROWS * 2) : nullptr;
 #pragma unroll
     for (uint32_t c0 = 0; c0 < H; c0 += 16) {
       tmem_ld16(tlane + COL_C1 + c0, v);
       tmem_ld_wait();
-#pragma unroll
-      for (int j = 0; j < 16; ++j) v[j] = fmaxf(v[j], 0.f);
-      store8<T>(bufB, ROWS, tid, c0, v);
-      store8<T>(bufB, ROWS, tid, c0 + 8, v + 8);
-      if (write_planes && valid)
-#pragma unroll
-        for (int j = 0; j < 16; ++j) ws.h1[(size_t)(c0 + j) * ws.cap + s] = v[j];
+      emit16<T, true>(v, bufB, blob_h1, c0, valid);
     }
     uint32_t sLast = sB;
     if (ms.n_color_layers == 2) {
       fence_async_smem(); fence_before(); __syncthreads();
-      if (tid == 0) { fence_after(); issue_layer(tmem_base + COL_C2, sB, sbase + FwdSmem::wc2, H, H, H, fmt, bar); }
-      mbar_wait(bar, phase); phase ^= 1; fence_after();
+      if (tid == 0) { fence_after(); issue_layer(tmem_base + COL_C2, sB, sW + WImg::f_c2, H, H, H, fmt, bar_mma); }
+      mbar_wait(bar_mma, ph_mma); ph_mma ^= 1; fence_after();
+      uint8_t *blob_h2 = save_blobs ? ws.blob_h2 + (size_t)tile * (H * ROWS * 2) : nullptr;
 #pragma unroll
       for (uint32_t c0 = 0; c0 < H; c0 += 16) {
         tmem_ld16(tlane + COL_C2 + c0, v);
         tmem_ld_wait();
-#pragma unroll
-        for (int j = 0; j < 16; ++j) v[j] = fmaxf(v[j], 0.f);
-        store8<T>(bufA, ROWS, tid, c0, v);
-        store8<T>(bufA, ROWS, tid, c0 + 8, v + 8);
-        if (write_planes && valid)
-#pragma unroll
-          for (int j = 0; j < 16; ++j) ws.h2[(size_t)(c0 + j) * ws.cap + s] = v[j];
+        emit16<T, true>(v, bufA, blob_h2, c0, valid);
       }
       sLast = sA;
     }
     fence_async_smem(); fence_before(); __syncthreads();
-    if (tid == 0) { fence_after(); issue_layer(tmem_base + COL_C3, sLast, sbase + FwdSmem::wc3, H, 16, 16, fmt, bar); }
-    mbar_wait(bar, phase); phase ^= 1; fence_after();
+    if (tid == 0) { fence_after(); issue_layer(tmem_base + COL_C3, sLast, sW + WImg::f_c3, H, 16, 16, fmt, bar_mma); }
+    mbar_wait(bar_mma, ph_mma); ph_mma ^= 1; fence_after();
     tmem_ld16(tlane + COL_C3, v);
     tmem_ld_wait();
     if (valid) {
@@ -208,46 +252,35 @@ __global__ void __launch_bounds__(128) mlp_forward_tc_kernel(MlpShape ms, const 
       for (int c = 0; c < 3; ++c) ws.rgb[3 * s + c] = 1.f / (1.f + expf(-v[c]));
     }
     fence_before();
-    __syncthreads();
   }
   fence_before();
   __syncthreads();
   if (warp == 0) tmem_free<FWD_COLS>(tmem_base);
 }
 
-
 // ------------------------------------------------------------------------------------- backward
-// S11 on tcgen05.  Per layer and tile, two kinds of MMA read the same two shared-memory tiles:
-//   dgrad  dX[128 x n_in]   = dY[128 x n_out] * W          A = dY (K-major), B = W^T tile (K-major)
-//   wgrad  G [n_in x n_out] += X^T * dY over the 128 samples  A = X, B = dY, both viewed MN-major
-// The wgrad accumulators stay in TMEM across ALL tiles of the persistent CTA (one flush of ~11 K
-// atomics per CTA at the end); thread r owns sample row r for dgrad and feature row r for wgrad.
+// Per layer and tile, two kinds of MMA read the same two shared-memory tiles:
+//   dgrad  dX[128 x n_in]   = dY[128 x n_out] * W           A = dY (K-major), B = W^T tile (K-major)
+//   wgrad  G [n_in x n_out] += X^T * dY over the 128 samples   A = X, B = dY, both viewed MN-major
+// The wgrad accumulators stay in TMEM across ALL tiles of the persistent CTA (one flush per CTA at
+// the end); thread r owns sample row r for dgrad and feature row r for wgrad.  The saved
+// activations X of the five layers arrive by TMA into two ping-pong buffers, one layer ahead.
 constexpr uint32_t COL_G = 0;                                   // dgrad result, reused per layer (<= 64 cols)
 constexpr uint32_t GW_C3 = 64, GW_C2 = 80, GW_C1 = 144, GW_D2 = 208, GW_D1 = 224, BWD_COLS = 512;
 
 struct BwdSmem {
-  static constexpr uint32_t wt_c3 = 0;                          // [N=64][K=16]
-  static constexpr uint32_t wt_c2 = wt_c3 + H * 16 * 2;         // [64][64]
-  static constexpr uint32_t wt_c1 = wt_c2 + H * H * 2;          // [32][64]
-  static constexpr uint32_t wt_d2 = wt_c1 + CIP * H * 2;        // [64][16]
-  static constexpr uint32_t wt_d1 = wt_d2 + H * 16 * 2;         // [LF<=64][64]
-  static constexpr uint32_t bufX = wt_d1 + 64 * H * 2;          // [128][128] (features >= 64 stay zero)
-  static constexpr uint32_t bufY = bufX + ROWS * 128 * 2;       // [128][64]
-  static constexpr uint32_t bar = bufY + ROWS * H * 2;
-  static constexpr uint32_t tmem = bar + 8;
+  static constexpr uint32_t w = 0;                                // weight image (WImg backward region)
+  static constexpr uint32_t bufX0 = w + WImg::b_total;            // [128][64]; the M=128 wgrad also reads the 16 KB after it
+  static constexpr uint32_t bufX1 = bufX0 + ROWS * H * 2;         // [128][64]
+  static constexpr uint32_t bufY = bufX1 + ROWS * H * 2;          // [128][64]
+  static constexpr uint32_t pad = bufY + ROWS * H * 2;            // 16 KB readable slack behind bufY's role as "after X1"
+  static constexpr uint32_t bar_mma = pad + ROWS * H * 2;
+  static constexpr uint32_t bar_w = bar_mma + 8;
+  static constexpr uint32_t bar_x0 = bar_w + 8;
+  static constexpr uint32_t bar_x1 = bar_x0 + 8;
+  static constexpr uint32_t tmem = bar_x1 + 8;
   static constexpr uint32_t total = tmem + 8;
 };
-
-// transposed operand tile for dgrad: element (i, o) = W[o][i], tile [NP = n_in pad][KP = n_out pad]
-template <typename T>
-__device__ void stage_weight_t(uint8_t *tile, const float *__restrict__ W, uint32_t n_out, uint32_t n_in, uint32_t NP,
-                               uint32_t KP) {
-  for (uint32_t idx = threadIdx.x; idx < NP * KP; idx += blockDim.x) {
-    const uint32_t i = idx / KP, o = idx - i * KP;
-    const float v = (i < n_in && o < n_out) ? __ldg(W + o * n_in + i) : 0.f;
-    *reinterpret_cast<T *>(tile + tile_off(NP, i, o)) = T(v);
-  }
-}
 
 // wgrad k-steps over the 128 samples: G[128 (feature i) x N (output o)] (+)= X^T dY
 __device__ __forceinline__ void issue_wgrad(uint32_t tmem_d, uint32_t x_saddr, uint32_t y_saddr, uint32_t N, uint32_t fmt,
@@ -260,56 +293,87 @@ __device__ __forceinline__ void issue_wgrad(uint32_t tmem_d, uint32_t x_saddr, u
   }
 }
 
-// this thread's sample row of a [n_cols][cap] fp32 plane array -> 16-bit row of `buf`; returns the
-// ReLU mask (bit c set iff x_c > 0)
+// ReLU mask of this thread's row of a [128][64] activation tile in shared memory
 template <typename T>
-__device__ __forceinline__ uint64_t row_from_planes(uint8_t *buf, const float *__restrict__ planes, uint64_t cap,
-                                                    uint32_t n_cols, uint64_t s, bool valid) {
+__device__ __forceinline__ uint64_t row_mask(const uint8_t *tile) {
   uint64_t mask = 0;
-  float v[8];
-  for (uint32_t c0 = 0; c0 < n_cols; c0 += 8) {
 #pragma unroll
-    for (int j = 0; j < 8; ++j) {
-      v[j] = valid ? planes[(size_t)(c0 + j) * cap + s] : 0.f;
-      if (v[j] > 0.f) mask |= 1ull << (c0 + j);
+  for (uint32_t p = 0; p < H / 8; ++p) {
+    const uint4 q = *reinterpret_cast<const uint4 *>(tile + p * PANEL + threadIdx.x * 16);
+    const uint32_t w[4] = {q.x, q.y, q.z, q.w};
+#pragma unroll
+    for (int j = 0; j < 4; ++j) {
+      const float2 f = unpack2<T>(w[j]);
+      if (f.x > 0.f) mask |= 1ull << (p * 8 + 2 * j);
+      if (f.y > 0.f) mask |= 1ull << (p * 8 + 2 * j + 1);
     }
-    store8<T>(buf, ROWS, threadIdx.x, c0, v);
   }
   return mask;
 }
 
 template <typename T>
-__global__ void __launch_bounds__(128, 1) mlp_backward_tc_kernel(MlpShape ms, const float *__restrict__ Wm,
-                                                                 float *__restrict__ gradW, const float *__restrict__ dirs,
-                                                                 Workspace ws, const uint32_t *__restrict__ d_S) {
+__device__ __forceinline__ void masked_to_Y(uint32_t tlane, uint64_t mask, uint8_t *bufY) {
+  float v[16];
+#pragma unroll
+  for (uint32_t c0 = 0; c0 < H; c0 += 16) {
+    tmem_ld16(tlane + COL_G + c0, v);
+    tmem_ld_wait();
+#pragma unroll
+    for (int j = 0; j < 16; ++j) v[j] = ((mask >> (c0 + j)) & 1ull) ? v[j] : 0.f;
+    emit16<T, false>(v, bufY, nullptr, c0, true);
+  }
+}
+
+template <typename T>
+__global__ void __launch_bounds__(128, 1) mlp_backward_tc_kernel(MlpShape ms, float *__restrict__ gradW, Workspace ws,
+                                                                 const uint32_t *__restrict__ d_S) {
   extern __shared__ __align__(1024) uint8_t smem[];
   const uint32_t tid = threadIdx.x, warp = tid >> 5;
   const uint32_t sbase = smem_u32(smem);
-  const uint32_t bar = sbase + BwdSmem::bar;
+  const uint32_t bar_mma = sbase + BwdSmem::bar_mma, bar_w = sbase + BwdSmem::bar_w;
+  const uint32_t bar_x[2] = {sbase + BwdSmem::bar_x0, sbase + BwdSmem::bar_x1};
+  const uint32_t sX[2] = {sbase + BwdSmem::bufX0, sbase + BwdSmem::bufX1};
+  uint8_t *bufX[2] = {smem + BwdSmem::bufX0, smem + BwdSmem::bufX1};
+  uint8_t *bufY = smem + BwdSmem::bufY;
+  const uint32_t sY = sbase + BwdSmem::bufY, sW = sbase + BwdSmem::w;
   const uint32_t LF = ms.LF;
   const uint64_t S = *d_S;
-  if ((uint64_t)blockIdx.x * ROWS >= S) return;   // CTA without tiles: nothing allocated yet
+  if ((uint64_t)blockIdx.x * ROWS >= S) return;   // CTA without tiles
+  const bool two = ms.n_color_layers == 2;
+  const uint32_t hbytes = H * ROWS * 2, cbytes = CIP * ROWS * 2, ebytes = LF * ROWS * 2;
 
-  stage_weight_t<T>(smem + BwdSmem::wt_c3, Wm + ms.o_c3, 3, H, H, 16);
-  if (ms.n_color_layers == 2) stage_weight_t<T>(smem + BwdSmem::wt_c2, Wm + ms.o_c2, H, H, H, H);
-  stage_weight_t<T>(smem + BwdSmem::wt_c1, Wm + ms.o_c1, H, ms.Ci, CIP, H);
-  stage_weight_t<T>(smem + BwdSmem::wt_d2, Wm + ms.o_d2, DO, H, H, 16);
-  stage_weight_t<T>(smem + BwdSmem::wt_d1, Wm + ms.o_d1, H, LF, LF, H);
-  for (uint32_t i = tid; i < ROWS * 128 * 2 / 16; i += blockDim.x) reinterpret_cast<uint4 *>(smem + BwdSmem::bufX)[i] = make_uint4(0, 0, 0, 0);
-  if (tid == 0) mbar_init(bar, 1);
+  // the activation tiles of one 128-sample tile, in the order the layers consume them
+  auto load_x = [&](uint32_t which, uint32_t buf, uint64_t tile) {   // one thread
+    const uint8_t *src; uint32_t bytes;
+    switch (which) {
+      case 0: src = (two ? ws.blob_h2 : ws.blob_h1) + tile * hbytes; bytes = hbytes; break;
+      case 1: src = ws.blob_h1 + tile * hbytes; bytes = hbytes; break;
+      case 2: src = ws.blob_ci + tile * cbytes; bytes = cbytes; break;
+      case 3: src = ws.blob_hd + tile * hbytes; bytes = hbytes; break;
+      default: src = ws.blob_e + tile * ebytes; bytes = ebytes; break;
+    }
+    mbar_expect_tx(bar_x[buf], bytes);
+    bulk_g2s(sX[buf], src, bytes, bar_x[buf]);
+  };
+
+  if (tid == 0) {
+    mbar_init(bar_mma, 1); mbar_init(bar_w, 1); mbar_init(bar_x[0], 1); mbar_init(bar_x[1], 1);
+    fence_async_smem();
+    mbar_expect_tx(bar_w, WImg::b_total);
+    bulk_g2s(sW, ws.wimg_bwd, WImg::b_total, bar_w);
+    load_x(0, 0, blockIdx.x);
+    load_x(two ? 1 : 2, 1, blockIdx.x);
+  }
   if (warp == 0) tmem_alloc<BWD_COLS>(sbase + BwdSmem::tmem);
-  fence_async_smem();
   fence_before();
   __syncthreads();
   fence_after();
   const uint32_t tmem_base = *reinterpret_cast<volatile uint32_t *>(smem + BwdSmem::tmem);
   const uint32_t tlane = tmem_base + ((warp * 32u) << 16);
-  uint32_t phase = 0;
+  uint32_t ph_mma = 0, ph_x[2] = {0, 0};
   const uint32_t fmt = Fmt<T>::id;
-  uint8_t *bufX = smem + BwdSmem::bufX, *bufY = smem + BwdSmem::bufY;
-  const uint32_t sX = sbase + BwdSmem::bufX, sY = sbase + BwdSmem::bufY;
 
-  // loss scale (fp16 only): one power of two per step from the largest input gradient magnitude
+  // loss scale (fp16 only): one power of two per step from the largest gradient entering S11
   float scale = 1.f;
   if (Fmt<T>::id == 0) {
     const float mx = __uint_as_float(*ws.grad_absmax);
@@ -317,88 +381,67 @@ __global__ void __launch_bounds__(128, 1) mlp_backward_tc_kernel(MlpShape ms, co
   }
   const float inv_scale = 1.f / scale;
   uint32_t acc = 0;   // wgrad accumulate flag (0 on the CTA's first tile)
+  if (tid == 0) mbar_wait(bar_w, 0);
 
-  for (uint64_t base = (uint64_t)blockIdx.x * ROWS; base < S; base += (uint64_t)gridDim.x * ROWS) {
-    const uint64_t s = base + tid;
+  for (uint64_t tile = blockIdx.x; tile * ROWS < S; tile += gridDim.x) {
+    const uint64_t s = tile * ROWS + tid;
     const bool valid = s < S;
+    const uint64_t next_tile = tile + gridDim.x;
+    const bool has_next = next_tile * ROWS < S;
     float v[16];
-    // ---- colour output layer: dY = dL/dc * c (1 - c)
+    uint32_t cur = 0;   // X buffer of the current layer; tiles always start with buffer 0
+    // ---- colour output layer: dY = dL/dc * c (1 - c); X = last hidden activations
 #pragma unroll
     for (int j = 0; j < 16; ++j) v[j] = 0.f;
+    float sig = 0.f, dsig = 0.f;
     if (valid) {
 #pragma unroll
       for (int c = 0; c < 3; ++c) {
         const float col = ws.rgb[3 * s + c];
         v[c] = ws.drgb[3 * s + c] * col * (1.f - col) * scale;
       }
+      sig = ws.sigma[s];
+      dsig = ws.dsigma[s];
     }
-    store8<T>(bufY, ROWS, tid, 0, v);
-    store8<T>(bufY, ROWS, tid, 8, v + 8);
-    uint64_t mask = row_from_planes<T>(bufX, ms.n_color_layers == 2 ? ws.h2 : ws.h1, ws.cap, H, s, valid);
+    emit16<T, false>(v, bufY, nullptr, 0, true);
+    mbar_wait(bar_x[cur], ph_x[cur]); ph_x[cur] ^= 1;
+    uint64_t mask = row_mask<T>(bufX[cur]);
     fence_async_smem(); fence_before(); __syncthreads();
     if (tid == 0) {
       fence_after();
-      issue_wgrad(tmem_base + GW_C3, sX, sY, 16, fmt, acc);
-      issue_layer(tmem_base + COL_G, sY, sbase + BwdSmem::wt_c3, 16, H, H, fmt, bar);
+      issue_wgrad(tmem_base + GW_C3, sX[cur], sY, 16, fmt, acc);
+      issue_layer(tmem_base + COL_G, sY, sW + WImg::b_c3, 16, H, H, fmt, bar_mma);
     }
-    mbar_wait(bar, phase); phase ^= 1; fence_after();
+    mbar_wait(bar_mma, ph_mma); ph_mma ^= 1; fence_after();
+    if (tid == 0) load_x(two ? 2 : 3, cur, tile);    // buffer free: fetch the layer after next
+    cur ^= 1;
     // ---- second colour hidden layer
-    if (ms.n_color_layers == 2) {
-#pragma unroll
-      for (uint32_t c0 = 0; c0 < H; c0 += 16) {
-        tmem_ld16(tlane + COL_G + c0, v);
-        tmem_ld_wait();
-#pragma unroll
-        for (int j = 0; j < 16; ++j) v[j] = ((mask >> (c0 + j)) & 1ull) ? v[j] : 0.f;
-        store8<T>(bufY, ROWS, tid, c0, v);
-        store8<T>(bufY, ROWS, tid, c0 + 8, v + 8);
-      }
-      fence_before(); __syncthreads();          // everyone has read its accumulator row; bufX may be replaced
-      mask = row_from_planes<T>(bufX, ws.h1, ws.cap, H, s, valid);
+    if (two) {
+      masked_to_Y<T>(tlane, mask, bufY);
+      mbar_wait(bar_x[cur], ph_x[cur]); ph_x[cur] ^= 1;
+      mask = row_mask<T>(bufX[cur]);
       fence_async_smem(); fence_before(); __syncthreads();
       if (tid == 0) {
         fence_after();
-        issue_wgrad(tmem_base + GW_C2, sX, sY, H, fmt, acc);
-        issue_layer(tmem_base + COL_G, sY, sbase + BwdSmem::wt_c2, H, H, H, fmt, bar);
+        issue_wgrad(tmem_base + GW_C2, sX[cur], sY, H, fmt, acc);
+        issue_layer(tmem_base + COL_G, sY, sW + WImg::b_c2, H, H, H, fmt, bar_mma);
       }
-      mbar_wait(bar, phase); phase ^= 1; fence_after();
+      mbar_wait(bar_mma, ph_mma); ph_mma ^= 1; fence_after();
+      if (tid == 0) load_x(3, cur, tile);
+      cur ^= 1;
     }
     // ---- first colour layer: dY = d h1 (masked); X = [g slice, Y(d), 0]
-#pragma unroll
-    for (uint32_t c0 = 0; c0 < H; c0 += 16) {
-      tmem_ld16(tlane + COL_G + c0, v);
-      tmem_ld_wait();
-#pragma unroll
-      for (int j = 0; j < 16; ++j) v[j] = ((mask >> (c0 + j)) & 1ull) ? v[j] : 0.f;
-      store8<T>(bufY, ROWS, tid, c0, v);
-      store8<T>(bufY, ROWS, tid, c0 + 8, v + 8);
-    }
-    fence_before(); __syncthreads();
-    float g0 = 0.f;
-    {
-      float ci[CIP];
-#pragma unroll
-      for (int j = 0; j < (int)CIP; ++j) ci[j] = 0.f;
-      float dx = 0.f, dy = 0.f, dz = 1.f;
-      if (valid) {
-        g0 = ws.g[s];
-        for (uint32_t j = 0; j < ms.geo_cnt; ++j) ci[j] = ws.g[(size_t)(ms.geo_off + j) * ws.cap + s];
-        const uint32_t ray = ws.s_ray[s];
-        dx = __ldg(dirs + 3 * (size_t)ray); dy = __ldg(dirs + 3 * (size_t)ray + 1); dz = __ldg(dirs + 3 * (size_t)ray + 2);
-        float Y[16];
-        sh_row(ms.sh_degree, dx, dy, dz, Y);
-        for (uint32_t j = 0; j < ms.n_sh; ++j) ci[ms.geo_cnt + j] = Y[j];
-      }
-#pragma unroll
-      for (uint32_t c0 = 0; c0 < CIP; c0 += 8) store8<T>(bufX, ROWS, tid, c0, ci + c0);
-    }
+    masked_to_Y<T>(tlane, mask, bufY);
+    mbar_wait(bar_x[cur], ph_x[cur]); ph_x[cur] ^= 1;
     fence_async_smem(); fence_before(); __syncthreads();
     if (tid == 0) {
       fence_after();
-      issue_wgrad(tmem_base + GW_C1, sX, sY, H, fmt, acc);
-      issue_layer(tmem_base + COL_G, sY, sbase + BwdSmem::wt_c1, H, CIP, CIP, fmt, bar);
+      issue_wgrad(tmem_base + GW_C1, sX[cur], sY, H, fmt, acc);
+      issue_layer(tmem_base + COL_G, sY, sW + WImg::b_c1, H, CIP, CIP, fmt, bar_mma);
     }
-    mbar_wait(bar, phase); phase ^= 1; fence_after();
+    mbar_wait(bar_mma, ph_mma); ph_mma ^= 1; fence_after();
+    if (tid == 0) load_x(4, cur, tile);
+    cur ^= 1;
     // ---- density output layer: dg = [geo slice of d ci] + e_0 * dL/dsigma * sigma (0 where clamped)
     {
       float dci[CIP], dg[16];
@@ -408,38 +451,38 @@ __global__ void __launch_bounds__(128, 1) mlp_backward_tc_kernel(MlpShape ms, co
 #pragma unroll
       for (int j = 0; j < 16; ++j) dg[j] = 0.f;
       for (uint32_t j = 0; j < ms.geo_cnt; ++j) dg[ms.geo_off + j] = dci[j];
-      if (valid && g0 > -15.f && g0 < 15.f) dg[0] += ws.dsigma[s] * ws.sigma[s] * scale;
-      store8<T>(bufY, ROWS, tid, 0, dg);
-      store8<T>(bufY, ROWS, tid, 8, dg + 8);
+      // sigma = exp(clamp(g0, -15, 15)): the clamp is active iff sigma sits on a bound
+      if (valid && sig > 3.0590232e-07f * 1.0001f && sig < 3269017.4f * 0.9999f) dg[0] += dsig * sig * scale;
+      emit16<T, false>(dg, bufY, nullptr, 0, true);
     }
-    fence_before(); __syncthreads();
-    mask = row_from_planes<T>(bufX, ws.hd, ws.cap, H, s, valid);
+    mbar_wait(bar_x[cur], ph_x[cur]); ph_x[cur] ^= 1;
+    mask = row_mask<T>(bufX[cur]);
     fence_async_smem(); fence_before(); __syncthreads();
     if (tid == 0) {
       fence_after();
-      issue_wgrad(tmem_base + GW_D2, sX, sY, 16, fmt, acc);
-      issue_layer(tmem_base + COL_G, sY, sbase + BwdSmem::wt_d2, 16, H, H, fmt, bar);
+      issue_wgrad(tmem_base + GW_D2, sX[cur], sY, 16, fmt, acc);
+      issue_layer(tmem_base + COL_G, sY, sW + WImg::b_d2, 16, H, H, fmt, bar_mma);
     }
-    mbar_wait(bar, phase); phase ^= 1; fence_after();
+    mbar_wait(bar_mma, ph_mma); ph_mma ^= 1; fence_after();
+    const uint32_t buf_hd = cur;
+    cur ^= 1;
     // ---- density hidden layer: dY = d hd (masked); X = e
-#pragma unroll
-    for (uint32_t c0 = 0; c0 < H; c0 += 16) {
-      tmem_ld16(tlane + COL_G + c0, v);
-      tmem_ld_wait();
-#pragma unroll
-      for (int j = 0; j < 16; ++j) v[j] = ((mask >> (c0 + j)) & 1ull) ? v[j] : 0.f;
-      store8<T>(bufY, ROWS, tid, c0, v);
-      store8<T>(bufY, ROWS, tid, c0 + 8, v + 8);
-    }
-    fence_before(); __syncthreads();
-    row_from_planes<T>(bufX, ws.e, ws.cap, LF, s, valid);
+    masked_to_Y<T>(tlane, mask, bufY);
+    mbar_wait(bar_x[cur], ph_x[cur]); ph_x[cur] ^= 1;
     fence_async_smem(); fence_before(); __syncthreads();
     if (tid == 0) {
       fence_after();
-      issue_wgrad(tmem_base + GW_D1, sX, sY, H, fmt, acc);
-      issue_layer(tmem_base + COL_G, sY, sbase + BwdSmem::wt_d1, H, LF, LF, fmt, bar);
+      issue_wgrad(tmem_base + GW_D1, sX[cur], sY, H, fmt, acc);
+      issue_layer(tmem_base + COL_G, sY, sW + WImg::b_d1, H, LF, LF, fmt, bar_mma);
     }
-    mbar_wait(bar, phase); phase ^= 1; fence_after();
+    mbar_wait(bar_mma, ph_mma); ph_mma ^= 1; fence_after();
+    // both X buffers are free: the next tile's first two layers.  The layer order leaves the
+    // buffers in the roles (cur = e, buf_hd = hd); the next tile starts again at buffer 0.
+    if (tid == 0 && has_next) {
+      load_x(0, 0, next_tile);
+      load_x(two ? 1 : 2, 1, next_tile);
+    }
+    (void)buf_hd;
     // ---- dL/de -> planes
     for (uint32_t c0 = 0; c0 < LF; c0 += 16) {
       tmem_ld16(tlane + COL_G + c0, v);
@@ -448,10 +491,12 @@ __global__ void __launch_bounds__(128, 1) mlp_backward_tc_kernel(MlpShape ms, co
 #pragma unroll
         for (int j = 0; j < 16; ++j) ws.de[(size_t)(c0 + j) * ws.cap + s] = v[j] * inv_scale;
     }
-    fence_before(); __syncthreads();
+    fence_before();
     acc = 1;
   }
   // ---- flush the CTA's weight gradients: thread i holds feature row i of every G = X^T dY
+  fence_before();
+  __syncthreads();
   fence_after();
   auto flush = [&](uint32_t col, uint32_t g_off, uint32_t n_out, uint32_t n_in, uint32_t ncols) {
     float v[16];
@@ -467,13 +512,26 @@ __global__ void __launch_bounds__(128, 1) mlp_backward_tc_kernel(MlpShape ms, co
     }
   };
   flush(GW_C3, ms.o_c3, 3, H, 16);
-  if (ms.n_color_layers == 2) flush(GW_C2, ms.o_c2, H, H, H);
+  if (two) flush(GW_C2, ms.o_c2, H, H, H);
   flush(GW_C1, ms.o_c1, H, ms.Ci, H);
   flush(GW_D2, ms.o_d2, DO, H, 16);
   flush(GW_D1, ms.o_d1, H, LF, H);
   fence_before();
   __syncthreads();
   if (warp == 0) tmem_free<BWD_COLS>(tmem_base);
+}
+
+// blob tile image -> fp32 rows [S][n_cols] (debug getter)
+template <typename T>
+__global__ void blob_to_rows_kernel(const uint8_t *__restrict__ blob, uint32_t n_cols, const uint32_t *__restrict__ d_S,
+                                    float *__restrict__ rows) {
+  const uint64_t S = *d_S, total = S * n_cols;
+  for (uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; i < total; i += (uint64_t)gridDim.x * blockDim.x) {
+    const uint64_t s = i / n_cols;
+    const uint32_t c = (uint32_t)(i - s * n_cols);
+    const uint8_t *p = blob + (s >> 7) * ((size_t)n_cols * ROWS * 2) + tile_off(ROWS, (uint32_t)(s & 127), c);
+    rows[i] = (float)(*reinterpret_cast<const T *>(p));
+  }
 }
 
 }  // namespace
@@ -483,28 +541,42 @@ bool mlp_tc_supported(const MlpShape &ms) {
          ms.n_sh <= 16 && ms.geo_off + ms.geo_cnt <= DO;
 }
 
-int launch_mlp_forward_tc(const MlpShape &ms, int bf16, const float *theta_mlp, const float *dirs, const Workspace &ws,
-                          const uint32_t *d_S, int density_only, int write_planes, int n_sms, cudaStream_t st) {
+size_t mlp_tc_wimg_bytes(int backward) { return backward ? WImg::b_total : WImg::f_total; }
+
+int launch_pack_weights(const MlpShape &ms, int bf16, const float *theta_mlp, const Workspace &ws, cudaStream_t st) {
+  if (bf16) pack_weights_kernel<__nv_bfloat16><<<5, 256, 0, st>>>(ms, theta_mlp, ws.wimg_fwd, ws.wimg_bwd);
+  else pack_weights_kernel<__half><<<5, 256, 0, st>>>(ms, theta_mlp, ws.wimg_fwd, ws.wimg_bwd);
+  return 1;
+}
+
+int launch_mlp_forward_tc(const MlpShape &ms, int bf16, const float *dirs, const Workspace &ws, const uint32_t *d_S,
+                          int density_only, int save_blobs, int n_sms, cudaStream_t st) {
   const size_t smem = FwdSmem::total;
   if (bf16) {
     cudaFuncSetAttribute(mlp_forward_tc_kernel<__nv_bfloat16>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    mlp_forward_tc_kernel<__nv_bfloat16><<<2 * n_sms, 128, smem, st>>>(ms, theta_mlp, dirs, ws, d_S, density_only, write_planes);
+    mlp_forward_tc_kernel<__nv_bfloat16><<<2 * n_sms, 128, smem, st>>>(ms, dirs, ws, d_S, density_only, save_blobs);
   } else {
     cudaFuncSetAttribute(mlp_forward_tc_kernel<__half>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    mlp_forward_tc_kernel<__half><<<2 * n_sms, 128, smem, st>>>(ms, theta_mlp, dirs, ws, d_S, density_only, write_planes);
+    mlp_forward_tc_kernel<__half><<<2 * n_sms, 128, smem, st>>>(ms, dirs, ws, d_S, density_only, save_blobs);
   }
   return 1;
 }
 
-int launch_mlp_backward_tc(const MlpShape &ms, int bf16, const float *theta_mlp, float *grad_mlp, const float *dirs,
-                           const Workspace &ws, const uint32_t *d_S, int n_sms, cudaStream_t st) {
+int launch_mlp_backward_tc(const MlpShape &ms, int bf16, float *grad_mlp, const Workspace &ws, const uint32_t *d_S,
+                           int n_sms, cudaStream_t st) {
   const size_t smem = BwdSmem::total;
   if (bf16) {
     cudaFuncSetAttribute(mlp_backward_tc_kernel<__nv_bfloat16>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    mlp_backward_tc_kernel<__nv_bfloat16><<<n_sms, 128, smem, st>>>(ms, theta_mlp, grad_mlp, dirs, ws, d_S);
+    mlp_backward_tc_kernel<__nv_bfloat16><<<n_sms, 128, smem, st>>>(ms, grad_mlp, ws, d_S);
   } else {
     cudaFuncSetAttribute(mlp_backward_tc_kernel<__half>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    mlp_backward_tc_kernel<__half><<<n_sms, 128, smem, st>>>(ms, theta_mlp, grad_mlp, dirs, ws, d_S);
+    mlp_backward_tc_kernel<__half><<<n_sms, 128, smem, st>>>(ms, grad_mlp, ws, d_S);
   }
+  return 1;
+}
+
+int launch_blob_to_rows(int bf16, const uint8_t *blob, uint32_t n_cols, const uint32_t *d_S, float *rows, cudaStream_t st) {
+  if (bf16) blob_to_rows_kernel<__nv_bfloat16><<<1024, 256, 0, st>>>(blob, n_cols, d_S, rows);
+  else blob_to_rows_kernel<__half><<<1024, 256, 0, st>>>(blob, n_cols, d_S, rows);
   return 1;
 }

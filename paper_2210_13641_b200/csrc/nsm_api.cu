@@ -90,7 +90,6 @@ struct nsm_field {
   struct HostStats { double acc[2]; uint32_t S; } *pinned = nullptr;
   const char *mlp_path = "simt_fp32";
   bool use_tc = false;   // tcgen05 MLP kernels (16-bit configurations with supported shapes)
-  bool tc_fwd = true, tc_bwd = true;  // debugging: NSM_TC_MODE=1 forward only, 2 backward only
 
   template <typename T>
   cudaError_t alloc(T **p, size_t n, bool zero = true) {
@@ -214,12 +213,18 @@ void enqueue_forward(nsm_field *f, const nsm_ray_batch *b, uint32_t R, bool jitt
   RUN(f, K_MARCH_COUNT, launch_march_count(mp, f->occ_full ? nullptr : f->fp.occ_bits, b->origins, b->dirs, f->ws, f->stream));
   RUN(f, K_SCAN, launch_scan(mp, f->ws, train ? 1 : 0, f->stream));
   RUN(f, K_MARCH_WRITE, launch_march_write(mp, b->origins, b->dirs, f->ws, f->stream));
-  RUN(f, K_ENCODE, launch_encode(f->lv, f->fp.theta, f->ws, d_S, f->n_sms, f->stream));
-  if (f->use_tc && f->tc_fwd)
-    RUN(f, K_MLP_FWD, launch_mlp_forward_tc(f->ms, f->cfg.mlp_precision == NSM_MLP_BF16, f->fp.theta + f->fp.n_table, b->dirs,
-                                            f->ws, d_S, 0, 1, f->n_sms, f->stream));
+  const int bf16 = f->cfg.mlp_precision == NSM_MLP_BF16;
+  RUN(f, K_ENCODE, launch_encode(f->lv, f->fp.theta, f->ws, d_S, f->use_tc ? 1 + bf16 : 0, f->n_sms, f->stream));
+  if (f->use_tc)
+    RUN(f, K_MLP_FWD, launch_mlp_forward_tc(f->ms, bf16, b->dirs, f->ws, d_S, 0, train ? 1 : 0, f->n_sms, f->stream));
   else
     RUN(f, K_MLP_FWD, launch_mlp_forward_simt(f->ms, f->fp.theta + f->fp.n_table, b->dirs, f->ws, d_S, 0, f->n_sms, f->stream));
+}
+
+// the tensor-core kernels read 16-bit weight images: repack after every change of the MLP weights
+void repack_weights(nsm_field *f) {
+  if (f->use_tc)
+    RUN(f, K_ADAM_MLP, launch_pack_weights(f->ms, f->cfg.mlp_precision == NSM_MLP_BF16, f->fp.theta + f->fp.n_table, f->ws, f->stream));
 }
 
 nsm_status clear_grads_if_dirty(nsm_field *f) {
@@ -238,9 +243,9 @@ nsm_status enqueue_backward(nsm_field *f, const nsm_ray_batch *b, float lambda_d
   if (st != NSM_OK) return st;
   enqueue_forward(f, b, R, f->cfg.jitter != 0, f->step + 1, true);
   RUN(f, K_COMPOSITE, launch_composite_train(f->ws, R, b->rgb, b->depth, b->depth_var, lambda_d, f->cfg.bg, f->stream));
-  if (f->use_tc && f->tc_bwd)
-    RUN(f, K_MLP_BWD, launch_mlp_backward_tc(f->ms, f->cfg.mlp_precision == NSM_MLP_BF16, f->fp.theta + f->fp.n_table,
-                                             f->fp.grad + f->fp.n_table, b->dirs, f->ws, d_S, f->n_sms, f->stream));
+  if (f->use_tc)
+    RUN(f, K_MLP_BWD, launch_mlp_backward_tc(f->ms, f->cfg.mlp_precision == NSM_MLP_BF16, f->fp.grad + f->fp.n_table, f->ws, d_S,
+                                             f->n_sms, f->stream));
   else
     RUN(f, K_MLP_BWD, launch_mlp_backward_simt(f->ms, f->fp.theta + f->fp.n_table, f->fp.grad + f->fp.n_table, b->dirs,
                                                f->ws, d_S, f->n_sms, f->stream));
@@ -261,6 +266,7 @@ nsm_status enqueue_adam(nsm_field *f) {
                                          f->cfg.beta2, f->cfg.eps, (float)(1.0 / bc1), (float)(1.0 / bc2), f->n_sms, f->stream));
   RUN(f, K_ADAM_MLP, launch_adam_mlp(f->fp, f->cfg.lr, f->cfg.beta1, f->cfg.beta2, f->cfg.eps, (float)(1.0 / bc1),
                                      (float)(1.0 / bc2), f->stream));
+  repack_weights(f);
   f->step = t;
   if (f->prof.on) f->prof.collect();
   f->grads_dirty = false;   // the Adam kernels clear what they consume
@@ -357,7 +363,6 @@ nsm_status nsm_create_field(const nsm_field_config *cfg, void *cuda_stream, nsm_
   const char *force = std::getenv("NSM_FORCE_SIMT");
   if (cfg->mlp_precision != NSM_MLP_FP32 && mlp_tc_supported(ms) && !(force && force[0] == '1')) {
     f->use_tc = true;
-    if (const char *mode = std::getenv("NSM_TC_MODE")) { f->tc_fwd = (atoi(mode) & 1) != 0; f->tc_bwd = (atoi(mode) & 2) != 0; }
     f->mlp_path = cfg->mlp_precision == NSM_MLP_BF16 ? "tcgen05_bf16" : "tcgen05_f16";
   }
   FieldParams &fp = f->fp;
@@ -378,9 +383,17 @@ nsm_status nsm_create_field(const nsm_field_config *cfg, void *cuda_stream, nsm_
   A(f->alloc(&ws.counts, R)); A(f->alloc(&ws.offsets, R + 1)); A(f->alloc(&ws.live_mask, (size_t)R * words));
   A(f->alloc(&ws.C, 3 * (size_t)R)); A(f->alloc(&ws.D_hat, R)); A(f->alloc(&ws.O, R));
   A(f->alloc(&ws.s_ray, cap)); A(f->alloc(&ws.s_k, cap)); A(f->alloc(&ws.s_t, cap)); A(f->alloc(&ws.s_delta, cap));
-  A(f->alloc(&ws.s_x, 3 * cap)); A(f->alloc(&ws.e, ms.LF * cap)); A(f->alloc(&ws.hd, ms.Hd * cap));
-  A(f->alloc(&ws.g, ms.Do * cap)); A(f->alloc(&ws.h1, ms.Hc * cap));
-  A(f->alloc(&ws.h2, (ms.n_color_layers == 2 ? ms.Hc : 1) * cap));
+  A(f->alloc(&ws.s_x, 3 * cap));
+  ws.e = ws.hd = ws.g = ws.h1 = ws.h2 = nullptr;
+  ws.blob_e = ws.blob_hd = ws.blob_ci = ws.blob_h1 = ws.blob_h2 = ws.wimg_fwd = ws.wimg_bwd = nullptr;
+  if (f->use_tc) {   // 16-bit operand-tile blobs: 2 bytes per value, 128-row tiles
+    A(f->alloc(&ws.blob_e, 2 * ms.LF * cap)); A(f->alloc(&ws.blob_hd, 2 * ms.Hd * cap)); A(f->alloc(&ws.blob_ci, 2 * 32 * cap));
+    A(f->alloc(&ws.blob_h1, 2 * ms.Hc * cap)); A(f->alloc(&ws.blob_h2, 2 * (ms.n_color_layers == 2 ? ms.Hc : 1) * cap));
+    A(f->alloc(&ws.wimg_fwd, mlp_tc_wimg_bytes(0))); A(f->alloc(&ws.wimg_bwd, mlp_tc_wimg_bytes(1)));
+  } else {
+    A(f->alloc(&ws.e, ms.LF * cap)); A(f->alloc(&ws.hd, ms.Hd * cap)); A(f->alloc(&ws.g, ms.Do * cap));
+    A(f->alloc(&ws.h1, ms.Hc * cap)); A(f->alloc(&ws.h2, (ms.n_color_layers == 2 ? ms.Hc : 1) * cap));
+  }
   A(f->alloc(&ws.sigma, cap)); A(f->alloc(&ws.rgb, 3 * cap)); A(f->alloc(&ws.T_excl, cap));
   A(f->alloc(&ws.dsigma, cap)); A(f->alloc(&ws.drgb, 3 * cap)); A(f->alloc(&ws.de, ms.LF * cap));
   A(f->alloc(&ws.loss_acc, 2)); A(f->alloc(&ws.total_samples, 1)); A(f->alloc(&ws.grad_absmax, 1));
@@ -391,6 +404,7 @@ nsm_status nsm_create_field(const nsm_field_config *cfg, void *cuda_stream, nsm_
     cudaGetLastError();
     return fail(e == cudaErrorMemoryAllocation ? NSM_ERR_OOM : NSM_ERR_CUDA, "allocation failed: %s", cudaGetErrorString(e));
   }
+  repack_weights(f);
   *out = f;
   return NSM_OK;
 }
@@ -468,6 +482,7 @@ nsm_status nsm_set_params(nsm_field *f, const float *d_theta, const float *d_m, 
   if (d_theta) CUDA_TRY(cudaMemcpyAsync(f->fp.theta, d_theta, bytes, cudaMemcpyDeviceToDevice, f->stream));
   if (d_m) CUDA_TRY(cudaMemcpyAsync(f->fp.m, d_m, bytes, cudaMemcpyDeviceToDevice, f->stream));
   if (d_v) CUDA_TRY(cudaMemcpyAsync(f->fp.v, d_v, bytes, cudaMemcpyDeviceToDevice, f->stream));
+  if (d_theta) repack_weights(f);
   f->step = step;
   return NSM_OK;
 }
@@ -499,10 +514,11 @@ nsm_status nsm_update_occupancy(nsm_field *f, nsm_occ_mode mode, const uint8_t *
       for (uint64_t first = 0; first < G3; first += chunk) {
         const uint64_t n = (G3 - first < chunk) ? G3 - first : chunk;
         RUN(f, K_OCC, launch_occ_cells(f->cfg.occ_res, first, n, f->ws, d_S, f->stream));
-        RUN(f, K_ENCODE, launch_encode(f->lv, f->fp.theta, f->ws, d_S, f->n_sms, f->stream));
+        RUN(f, K_ENCODE, launch_encode(f->lv, f->fp.theta, f->ws, d_S, f->use_tc ? 1 + (f->cfg.mlp_precision == NSM_MLP_BF16) : 0,
+                                       f->n_sms, f->stream));
         if (f->use_tc)
-          RUN(f, K_MLP_FWD, launch_mlp_forward_tc(f->ms, f->cfg.mlp_precision == NSM_MLP_BF16, f->fp.theta + f->fp.n_table, nullptr,
-                                                  f->ws, d_S, 1, 0, f->n_sms, f->stream));
+          RUN(f, K_MLP_FWD, launch_mlp_forward_tc(f->ms, f->cfg.mlp_precision == NSM_MLP_BF16, nullptr, f->ws, d_S, 1, 0, f->n_sms,
+                                                  f->stream));
         else
           RUN(f, K_MLP_FWD, launch_mlp_forward_simt(f->ms, f->fp.theta + f->fp.n_table, nullptr, f->ws, d_S, 1, f->n_sms, f->stream));
         RUN(f, K_OCC, launch_occ_threshold(f->cfg.occ_res, first, n, f->ws.sigma, f->cfg.occ_sigma_threshold,
@@ -653,7 +669,10 @@ nsm_status nsm_debug_last_step(nsm_field *f, int item, void *d_out, uint64_t cap
   } else if (item == NSM_DBG_SAMPLE_X) {
     RUN(f, K_DEBUG, launch_planes_to_rows(ws.s_x, ws.cap, 3, d_S, (float *)d_out, f->stream));
   } else if (item == NSM_DBG_E) {
-    RUN(f, K_DEBUG, launch_planes_to_rows(ws.e, ws.cap, f->ms.LF, d_S, (float *)d_out, f->stream));
+    if (f->use_tc)
+      RUN(f, K_DEBUG, launch_blob_to_rows(f->cfg.mlp_precision == NSM_MLP_BF16, ws.blob_e, f->ms.LF, d_S, (float *)d_out, f->stream));
+    else
+      RUN(f, K_DEBUG, launch_planes_to_rows(ws.e, ws.cap, f->ms.LF, d_S, (float *)d_out, f->stream));
   } else if (item == NSM_DBG_SLOTS) {
     RUN(f, K_DEBUG, launch_debug_slots(f->lv, ws, d_S, (uint32_t *)d_out, nullptr, f->stream));
   } else {

@@ -60,6 +60,9 @@ struct Workspace {
   // loss accumulators: [0]=sum rgb, [1]=sum depth (doubles); device
   double *loss_acc;
   unsigned long long *total_samples;  // running sum of S over training steps (device)
+  // tensor-core path: 16-bit operand-tile images ("blobs", see mlp_tc.cu) instead of the fp32 planes e/hd/g/h1/h2
+  uint8_t *blob_e, *blob_hd, *blob_ci, *blob_h1, *blob_h2;
+  uint8_t *wimg_fwd, *wimg_bwd;       // 16-bit weight images, repacked whenever the MLP weights change
   uint32_t *grad_absmax;              // bits of max |dL/d(pre-activation)| entering S11 this step (loss scale)
 };
 
@@ -82,8 +85,9 @@ int launch_march_count(const MarchParams &mp, const uint8_t *bits, const float *
 int launch_scan(const MarchParams &mp, const Workspace &ws, int count_total, cudaStream_t st);
 int launch_march_write(const MarchParams &mp, const float *origins, const float *dirs, const Workspace &ws,
                        cudaStream_t st);
+// out_mode: 0 = fp32 planes ws.e, 1 = fp16 blob ws.blob_e, 2 = bf16 blob ws.blob_e
 int launch_encode(const LevelTable &lv, const float *theta, const Workspace &ws,
-                  const uint32_t *d_S, int n_sms, cudaStream_t st);
+                  const uint32_t *d_S, int out_mode, int n_sms, cudaStream_t st);
 int launch_scatter(const LevelTable &lv, float *grad, uint8_t *touched, const Workspace &ws,
                    const uint32_t *d_S, int n_sms, cudaStream_t st);
 int launch_mlp_forward_simt(const MlpShape &ms, const float *theta_mlp, const float *dirs,
@@ -94,10 +98,13 @@ int launch_mlp_backward_simt(const MlpShape &ms, const float *theta_mlp, float *
                              cudaStream_t st);
 size_t mlp_simt_smem_bytes(const MlpShape &ms, int backward);
 bool mlp_tc_supported(const MlpShape &ms);
-int launch_mlp_backward_tc(const MlpShape &ms, int bf16, const float *theta_mlp, float *grad_mlp, const float *dirs,
-                           const Workspace &ws, const uint32_t *d_S, int n_sms, cudaStream_t st);
-int launch_mlp_forward_tc(const MlpShape &ms, int bf16, const float *theta_mlp, const float *dirs, const Workspace &ws,
-                          const uint32_t *d_S, int density_only, int write_planes, int n_sms, cudaStream_t st);
+size_t mlp_tc_wimg_bytes(int backward);
+int launch_pack_weights(const MlpShape &ms, int bf16, const float *theta_mlp, const Workspace &ws, cudaStream_t st);
+int launch_mlp_forward_tc(const MlpShape &ms, int bf16, const float *dirs, const Workspace &ws, const uint32_t *d_S,
+                          int density_only, int save_blobs, int n_sms, cudaStream_t st);
+int launch_mlp_backward_tc(const MlpShape &ms, int bf16, float *grad_mlp, const Workspace &ws, const uint32_t *d_S,
+                           int n_sms, cudaStream_t st);
+int launch_blob_to_rows(int bf16, const uint8_t *blob, uint32_t n_cols, const uint32_t *d_S, float *rows, cudaStream_t st);
 int launch_composite_train(const Workspace &ws, uint32_t R, const float *rgb, const float *depth,
                            const float *depth_var, float lambda_d, const float bg[3],
                            cudaStream_t st);

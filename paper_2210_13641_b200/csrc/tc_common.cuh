@@ -89,6 +89,16 @@ __device__ __forceinline__ void mbar_wait(uint32_t bar_saddr, uint32_t parity) {
   }
 }
 
+// ---- TMA 1-D bulk copies (cp.async.bulk, SASS UBLKCP): global -> shared, completion on an mbarrier ----
+__device__ __forceinline__ void mbar_expect_tx(uint32_t bar_saddr, uint32_t bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar_saddr), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void bulk_g2s(uint32_t dst_saddr, const void *src, uint32_t bytes, uint32_t bar_saddr) {
+  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(dst_saddr),
+               "l"(src), "r"(bytes), "r"(bar_saddr)
+               : "memory");
+}
+
 // ---- TMEM ------------------------------------------------------------------------------------
 template <uint32_t NCOLS>
 __device__ __forceinline__ void tmem_alloc(uint32_t dst_saddr) {  // one full warp
