@@ -18,28 +18,46 @@ __device__ __forceinline__ void adam_one(float &th, float &m, float &v, float g,
   th = th - c.lr * mhat / (sqrtf(vhat) + c.eps);
 }
 
+// One thread per 4 consecutive entries: the four flag bytes come in one coalesced 4-byte load; a
+// touched entry's record (4F floats; one 32 B sector for F = 2) is read and written with float4s.
 template <int F>
-__global__ void __launch_bounds__(256) adam_table_kernel(float *__restrict__ theta, float *__restrict__ m,
-                                                         float *__restrict__ v, float *__restrict__ grad,
-                                                         uint8_t *__restrict__ touched, uint64_t n_entries,
-                                                         int sparse, AdamConst c) {
-  for (uint64_t e = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; e < n_entries;
-       e += (uint64_t)gridDim.x * blockDim.x) {
-    const uint8_t t = touched[e];
-    if (sparse && !t) continue;
-    float th[F], mm[F], vv[F], gg[F];
-#pragma unroll
-    for (int f = 0; f < F; ++f) {
-      th[f] = theta[e * F + f]; mm[f] = m[e * F + f]; vv[f] = v[e * F + f]; gg[f] = grad[e * F + f];
+__global__ void __launch_bounds__(256) adam_table_kernel(float *__restrict__ rec, uint8_t *__restrict__ touched,
+                                                         uint64_t n_entries, int sparse, AdamConst c) {
+  const uint64_t n_quads = (n_entries + 3) / 4;
+  for (uint64_t q = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; q < n_quads; q += (uint64_t)gridDim.x * blockDim.x) {
+    const uint64_t e0 = q * 4;
+    uint32_t flags;
+    if (e0 + 4 <= n_entries) {
+      flags = *reinterpret_cast<const uint32_t *>(touched + e0);
+    } else {
+      flags = 0;
+      for (uint64_t e = e0; e < n_entries; ++e) flags |= (uint32_t)touched[e] << (8 * (e - e0));
     }
+    if (sparse && flags == 0) continue;
 #pragma unroll
-    for (int f = 0; f < F; ++f) adam_one(th[f], mm[f], vv[f], gg[f], c);
+    for (int j = 0; j < 4; ++j) {
+      const uint64_t e = e0 + j;
+      const bool t = (flags >> (8 * j)) & 0xffu;
+      if (e >= n_entries || (sparse && !t)) continue;
+      float4 *r4 = reinterpret_cast<float4 *>(rec + e * 4 * F);
+      float vals[4 * F];
 #pragma unroll
-    for (int f = 0; f < F; ++f) {
-      theta[e * F + f] = th[f]; m[e * F + f] = mm[f]; v[e * F + f] = vv[f];
-      if (t) grad[e * F + f] = 0.f;
+      for (int i = 0; i < F; ++i) {
+        const float4 x = r4[i];
+        vals[4 * i] = x.x; vals[4 * i + 1] = x.y; vals[4 * i + 2] = x.z; vals[4 * i + 3] = x.w;
+      }
+#pragma unroll
+      for (int f = 0; f < F; ++f) {
+        adam_one(vals[f], vals[2 * F + f], vals[3 * F + f], vals[F + f], c);
+        vals[F + f] = 0.f;   // the gradient is consumed
+      }
+#pragma unroll
+      for (int i = 0; i < F; ++i) r4[i] = make_float4(vals[4 * i], vals[4 * i + 1], vals[4 * i + 2], vals[4 * i + 3]);
     }
-    if (t) touched[e] = 0;
+    if (flags) {
+      if (e0 + 4 <= n_entries) *reinterpret_cast<uint32_t *>(touched + e0) = 0u;
+      else for (uint64_t e = e0; e < n_entries; ++e) touched[e] = 0;
+    }
   }
 }
 
@@ -59,10 +77,10 @@ int launch_adam_table(const FieldParams &fp, uint32_t F, int sparse, float lr, f
   AdamConst c{lr, beta1, beta2, eps, inv_bc1, inv_bc2};
   dim3 grid(n_sms * 8), block(256);
   switch (F) {
-    case 1: adam_table_kernel<1><<<grid, block, 0, st>>>(fp.theta, fp.m, fp.v, fp.grad, fp.touched, fp.n_entries, sparse, c); break;
-    case 2: adam_table_kernel<2><<<grid, block, 0, st>>>(fp.theta, fp.m, fp.v, fp.grad, fp.touched, fp.n_entries, sparse, c); break;
-    case 4: adam_table_kernel<4><<<grid, block, 0, st>>>(fp.theta, fp.m, fp.v, fp.grad, fp.touched, fp.n_entries, sparse, c); break;
-    default: adam_table_kernel<8><<<grid, block, 0, st>>>(fp.theta, fp.m, fp.v, fp.grad, fp.touched, fp.n_entries, sparse, c); break;
+    case 1: adam_table_kernel<1><<<grid, block, 0, st>>>(fp.rec, fp.touched, fp.n_entries, sparse, c); break;
+    case 2: adam_table_kernel<2><<<grid, block, 0, st>>>(fp.rec, fp.touched, fp.n_entries, sparse, c); break;
+    case 4: adam_table_kernel<4><<<grid, block, 0, st>>>(fp.rec, fp.touched, fp.n_entries, sparse, c); break;
+    default: adam_table_kernel<8><<<grid, block, 0, st>>>(fp.rec, fp.touched, fp.n_entries, sparse, c); break;
   }
   return 1;
 }
@@ -70,8 +88,6 @@ int launch_adam_table(const FieldParams &fp, uint32_t F, int sparse, float lr, f
 int launch_adam_mlp(const FieldParams &fp, float lr, float beta1, float beta2, float eps, float inv_bc1, float inv_bc2,
                     cudaStream_t st) {
   AdamConst c{lr, beta1, beta2, eps, inv_bc1, inv_bc2};
-  adam_dense_kernel<<<(unsigned)((fp.n_mlp + 255) / 256), 256, 0, st>>>(fp.theta + fp.n_table, fp.m + fp.n_table,
-                                                                       fp.v + fp.n_table, fp.grad + fp.n_table,
-                                                                       fp.n_mlp, c);
+  adam_dense_kernel<<<(unsigned)((fp.n_mlp + 255) / 256), 256, 0, st>>>(fp.mlp_theta, fp.mlp_m, fp.mlp_v, fp.mlp_grad, fp.n_mlp, c);
   return 1;
 }

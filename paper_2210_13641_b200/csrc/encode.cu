@@ -81,7 +81,7 @@ __device__ __forceinline__ void load_entry(const float *p, float out[F]) {
 // tensor-core MLP kernels ([tile][8-column panel][128 rows][8 x 16 bit], mlp_tc.cu); the rows of
 // the last tile beyond S are zero-filled so the MMA never reads stale data.
 template <int F, int MODE>
-__global__ void __launch_bounds__(256) encode_forward_kernel(LevelTable lv, const float *__restrict__ theta,
+__global__ void __launch_bounds__(256) encode_forward_kernel(LevelTable lv, const float *__restrict__ rec,
                                                              Workspace ws, const uint32_t *__restrict__ d_S) {
   const uint64_t S = *d_S;
   const uint64_t S_it = MODE == 0 ? S : ((S + NSM_TILE - 1) / NSM_TILE) * NSM_TILE;
@@ -96,10 +96,10 @@ __global__ void __launch_bounds__(256) encode_forward_kernel(LevelTable lv, cons
     for (int f = 0; f < F; ++f) acc[f] = 0.0f;
     if (s < S) {
       CornerIndex ci = corner_index(lv, l, ws.s_x[s], ws.s_x[ws.cap + s], ws.s_x[2 * ws.cap + s]);
-      const float *tab = theta + lv.offset[l] * F;
+      const float *tab = rec + lv.offset[l] * (4 * F);   // theta = the first F floats of a 4F-float record
       float v[8][F];
 #pragma unroll
-      for (int k = 0; k < 8; ++k) load_entry<F>(tab + (size_t)ci.slot[k] * F, v[k]);  // 8 gathers in flight
+      for (int k = 0; k < 8; ++k) load_entry<F>(tab + (size_t)ci.slot[k] * (4 * F), v[k]);  // 8 gathers in flight
 #pragma unroll
       for (int k = 0; k < 8; ++k) {
         float om = corner_weight(k, ci.w);
@@ -140,7 +140,7 @@ __device__ __forceinline__ void red_add_entry(float *p, const float g[F]) {
 // S12: d theta[(offset_l + slot) F + f] += omega * dL/de[l F + f]; the touched set U is marked
 // structurally (every referenced entry), independent of the gradient's value.
 template <int F>
-__global__ void __launch_bounds__(256) scatter_backward_kernel(LevelTable lv, float *__restrict__ grad,
+__global__ void __launch_bounds__(256) scatter_backward_kernel(LevelTable lv, float *__restrict__ rec,
                                                                uint8_t *__restrict__ touched, Workspace ws,
                                                                const uint32_t *__restrict__ d_S) {
   const uint64_t S = *d_S;
@@ -153,7 +153,7 @@ __global__ void __launch_bounds__(256) scatter_backward_kernel(LevelTable lv, fl
     float de[F];
 #pragma unroll
     for (int f = 0; f < F; ++f) de[f] = ws.de[(size_t)(l * F + f) * ws.cap + s];
-    float *tab = grad + lv.offset[l] * F;
+    float *tab = rec + lv.offset[l] * (4 * F) + F;   // the gradient field of the records
     uint8_t *tch = touched + lv.offset[l];
 #pragma unroll
     for (int k = 0; k < 8; ++k) {
@@ -161,7 +161,7 @@ __global__ void __launch_bounds__(256) scatter_backward_kernel(LevelTable lv, fl
       float g[F];
 #pragma unroll
       for (int f = 0; f < F; ++f) g[f] = om * de[f];
-      red_add_entry<F>(tab + (size_t)ci.slot[k] * F, g);
+      red_add_entry<F>(tab + (size_t)ci.slot[k] * (4 * F), g);
       tch[ci.slot[k]] = 1;
     }
   }
@@ -195,7 +195,37 @@ __global__ void planes_to_rows_kernel(const float *__restrict__ planes, uint64_t
   }
 }
 
+__global__ void pack_records_kernel(float *__restrict__ rec, uint32_t F, uint64_t n_entries, int which,
+                                    const float *__restrict__ src) {
+  const uint64_t total = n_entries * F;
+  for (uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; i < total; i += (uint64_t)gridDim.x * blockDim.x) {
+    const uint64_t e = i / F;
+    const uint32_t f = (uint32_t)(i - e * F);
+    rec[e * 4 * F + (uint64_t)which * F + f] = src ? src[i] : 0.f;
+  }
+}
+
+__global__ void unpack_records_kernel(const float *__restrict__ rec, uint32_t F, uint64_t n_entries, int which,
+                                      float *__restrict__ dst) {
+  const uint64_t total = n_entries * F;
+  for (uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; i < total; i += (uint64_t)gridDim.x * blockDim.x) {
+    const uint64_t e = i / F;
+    const uint32_t f = (uint32_t)(i - e * F);
+    dst[i] = rec[e * 4 * F + (uint64_t)which * F + f];
+  }
+}
+
 }  // namespace
+
+int launch_pack_records(const FieldParams &fp, int which, const float *src, cudaStream_t st) {
+  pack_records_kernel<<<2048, 256, 0, st>>>(fp.rec, fp.F, fp.n_entries, which, src);
+  return 1;
+}
+
+int launch_unpack_records(const FieldParams &fp, int which, float *dst, cudaStream_t st) {
+  unpack_records_kernel<<<2048, 256, 0, st>>>(fp.rec, fp.F, fp.n_entries, which, dst);
+  return 1;
+}
 
 template <int F>
 static void launch_encode_f(const LevelTable &lv, const float *theta, const Workspace &ws, const uint32_t *d_S, int out_mode,

@@ -214,22 +214,23 @@ void enqueue_forward(nsm_field *f, const nsm_ray_batch *b, uint32_t R, bool jitt
   RUN(f, K_SCAN, launch_scan(mp, f->ws, train ? 1 : 0, f->stream));
   RUN(f, K_MARCH_WRITE, launch_march_write(mp, b->origins, b->dirs, f->ws, f->stream));
   const int bf16 = f->cfg.mlp_precision == NSM_MLP_BF16;
-  RUN(f, K_ENCODE, launch_encode(f->lv, f->fp.theta, f->ws, d_S, f->use_tc ? 1 + bf16 : 0, f->n_sms, f->stream));
+  RUN(f, K_ENCODE, launch_encode(f->lv, f->fp.rec, f->ws, d_S, f->use_tc ? 1 + bf16 : 0, f->n_sms, f->stream));
   if (f->use_tc)
     RUN(f, K_MLP_FWD, launch_mlp_forward_tc(f->ms, bf16, b->dirs, f->ws, d_S, 0, train ? 1 : 0, f->n_sms, f->stream));
   else
-    RUN(f, K_MLP_FWD, launch_mlp_forward_simt(f->ms, f->fp.theta + f->fp.n_table, b->dirs, f->ws, d_S, 0, f->n_sms, f->stream));
+    RUN(f, K_MLP_FWD, launch_mlp_forward_simt(f->ms, f->fp.mlp_theta, b->dirs, f->ws, d_S, 0, f->n_sms, f->stream));
 }
 
 // the tensor-core kernels read 16-bit weight images: repack after every change of the MLP weights
 void repack_weights(nsm_field *f) {
   if (f->use_tc)
-    RUN(f, K_ADAM_MLP, launch_pack_weights(f->ms, f->cfg.mlp_precision == NSM_MLP_BF16, f->fp.theta + f->fp.n_table, f->ws, f->stream));
+    RUN(f, K_ADAM_MLP, launch_pack_weights(f->ms, f->cfg.mlp_precision == NSM_MLP_BF16, f->fp.mlp_theta, f->ws, f->stream));
 }
 
 nsm_status clear_grads_if_dirty(nsm_field *f) {
   if (f->grads_dirty) {
-    CUDA_TRY(cudaMemsetAsync(f->fp.grad, 0, sizeof(float) * (f->fp.n_table + f->fp.n_mlp), f->stream));
+    RUN(f, K_DEBUG, launch_pack_records(f->fp, 1, nullptr, f->stream));
+    CUDA_TRY(cudaMemsetAsync(f->fp.mlp_grad, 0, sizeof(float) * f->fp.n_mlp, f->stream));
     CUDA_TRY(cudaMemsetAsync(f->fp.touched, 0, f->fp.n_entries, f->stream));
     f->grads_dirty = false;
   }
@@ -244,12 +245,12 @@ nsm_status enqueue_backward(nsm_field *f, const nsm_ray_batch *b, float lambda_d
   enqueue_forward(f, b, R, f->cfg.jitter != 0, f->step + 1, true);
   RUN(f, K_COMPOSITE, launch_composite_train(f->ws, R, b->rgb, b->depth, b->depth_var, lambda_d, f->cfg.bg, f->stream));
   if (f->use_tc)
-    RUN(f, K_MLP_BWD, launch_mlp_backward_tc(f->ms, f->cfg.mlp_precision == NSM_MLP_BF16, f->fp.grad + f->fp.n_table, f->ws, d_S,
+    RUN(f, K_MLP_BWD, launch_mlp_backward_tc(f->ms, f->cfg.mlp_precision == NSM_MLP_BF16, f->fp.mlp_grad, f->ws, d_S,
                                              f->n_sms, f->stream));
   else
-    RUN(f, K_MLP_BWD, launch_mlp_backward_simt(f->ms, f->fp.theta + f->fp.n_table, f->fp.grad + f->fp.n_table, b->dirs,
+    RUN(f, K_MLP_BWD, launch_mlp_backward_simt(f->ms, f->fp.mlp_theta, f->fp.mlp_grad, b->dirs,
                                                f->ws, d_S, f->n_sms, f->stream));
-  RUN(f, K_SCATTER, launch_scatter(f->lv, f->fp.grad, f->fp.touched, f->ws, d_S, f->n_sms, f->stream));
+  RUN(f, K_SCATTER, launch_scatter(f->lv, f->fp.rec, f->fp.touched, f->ws, d_S, f->n_sms, f->stream));
   f->grads_dirty = true;
   f->last_R = R;
   f->last_K = b->n_candidates;
@@ -369,7 +370,7 @@ nsm_status nsm_create_field(const nsm_field_config *cfg, void *cuda_stream, nsm_
   fp.n_entries = f->lv.offset[cfg->n_levels];
   fp.n_table = fp.n_entries * cfg->n_features;
   fp.n_mlp = ms.n_mlp;
-  const uint64_t P = fp.n_table + fp.n_mlp;
+  fp.F = cfg->n_features;
   Workspace &ws = f->ws;
   const uint64_t cap = (((uint64_t)cfg->max_rays * cfg->max_candidates + NSM_TILE - 1) / NSM_TILE) * NSM_TILE;
   ws.cap = cap;
@@ -378,7 +379,8 @@ nsm_status nsm_create_field(const nsm_field_config *cfg, void *cuda_stream, nsm_
   const uint32_t R = cfg->max_rays, words = (cfg->max_candidates + 31) / 32;
   cudaError_t e = cudaSuccess;
   auto A = [&](cudaError_t r) { if (e == cudaSuccess) e = r; };
-  A(f->alloc(&fp.theta, P)); A(f->alloc(&fp.m, P)); A(f->alloc(&fp.v, P)); A(f->alloc(&fp.grad, P));
+  A(f->alloc(&fp.rec, 4 * fp.n_table));
+  A(f->alloc(&fp.mlp_theta, fp.n_mlp)); A(f->alloc(&fp.mlp_m, fp.n_mlp)); A(f->alloc(&fp.mlp_v, fp.n_mlp)); A(f->alloc(&fp.mlp_grad, fp.n_mlp));
   A(f->alloc(&fp.touched, fp.n_entries)); A(f->alloc(&fp.occ_bits, (G3 + 7) / 8 + 4));
   A(f->alloc(&ws.counts, R)); A(f->alloc(&ws.offsets, R + 1)); A(f->alloc(&ws.live_mask, (size_t)R * words));
   A(f->alloc(&ws.C, 3 * (size_t)R)); A(f->alloc(&ws.D_hat, R)); A(f->alloc(&ws.O, R));
@@ -468,22 +470,34 @@ nsm_status nsm_get_level_table(const nsm_field *f, uint32_t *res, uint64_t *offs
 
 nsm_status nsm_get_params(nsm_field *f, float *d_theta, float *d_m, float *d_v, uint32_t *step) {
   if (!f) return fail(NSM_ERR_INVALID_ARG, "field is NULL");
-  const size_t bytes = sizeof(float) * (f->fp.n_table + f->fp.n_mlp);
-  if (d_theta) CUDA_TRY(cudaMemcpyAsync(d_theta, f->fp.theta, bytes, cudaMemcpyDeviceToDevice, f->stream));
-  if (d_m) CUDA_TRY(cudaMemcpyAsync(d_m, f->fp.m, bytes, cudaMemcpyDeviceToDevice, f->stream));
-  if (d_v) CUDA_TRY(cudaMemcpyAsync(d_v, f->fp.v, bytes, cudaMemcpyDeviceToDevice, f->stream));
+  const size_t mb = sizeof(float) * f->fp.n_mlp;
+  float *dst[3] = {d_theta, d_m, d_v};
+  const float *mlp[3] = {f->fp.mlp_theta, f->fp.mlp_m, f->fp.mlp_v};
+  const int which[3] = {0, 2, 3};
+  for (int i = 0; i < 3; ++i) {
+    if (!dst[i]) continue;
+    RUN(f, K_DEBUG, launch_unpack_records(f->fp, which[i], dst[i], f->stream));
+    CUDA_TRY(cudaMemcpyAsync(dst[i] + f->fp.n_table, mlp[i], mb, cudaMemcpyDeviceToDevice, f->stream));
+  }
   if (step) *step = f->step;
+  CUDA_TRY(cudaGetLastError());
   return NSM_OK;
 }
 
 nsm_status nsm_set_params(nsm_field *f, const float *d_theta, const float *d_m, const float *d_v, uint32_t step) {
   if (!f) return fail(NSM_ERR_INVALID_ARG, "field is NULL");
-  const size_t bytes = sizeof(float) * (f->fp.n_table + f->fp.n_mlp);
-  if (d_theta) CUDA_TRY(cudaMemcpyAsync(f->fp.theta, d_theta, bytes, cudaMemcpyDeviceToDevice, f->stream));
-  if (d_m) CUDA_TRY(cudaMemcpyAsync(f->fp.m, d_m, bytes, cudaMemcpyDeviceToDevice, f->stream));
-  if (d_v) CUDA_TRY(cudaMemcpyAsync(f->fp.v, d_v, bytes, cudaMemcpyDeviceToDevice, f->stream));
+  const size_t mb = sizeof(float) * f->fp.n_mlp;
+  const float *src[3] = {d_theta, d_m, d_v};
+  float *mlp[3] = {f->fp.mlp_theta, f->fp.mlp_m, f->fp.mlp_v};
+  const int which[3] = {0, 2, 3};
+  for (int i = 0; i < 3; ++i) {
+    if (!src[i]) continue;
+    RUN(f, K_DEBUG, launch_pack_records(f->fp, which[i], src[i], f->stream));
+    CUDA_TRY(cudaMemcpyAsync(mlp[i], src[i] + f->fp.n_table, mb, cudaMemcpyDeviceToDevice, f->stream));
+  }
   if (d_theta) repack_weights(f);
   f->step = step;
+  CUDA_TRY(cudaGetLastError());
   return NSM_OK;
 }
 
@@ -514,13 +528,13 @@ nsm_status nsm_update_occupancy(nsm_field *f, nsm_occ_mode mode, const uint8_t *
       for (uint64_t first = 0; first < G3; first += chunk) {
         const uint64_t n = (G3 - first < chunk) ? G3 - first : chunk;
         RUN(f, K_OCC, launch_occ_cells(f->cfg.occ_res, first, n, f->ws, d_S, f->stream));
-        RUN(f, K_ENCODE, launch_encode(f->lv, f->fp.theta, f->ws, d_S, f->use_tc ? 1 + (f->cfg.mlp_precision == NSM_MLP_BF16) : 0,
+        RUN(f, K_ENCODE, launch_encode(f->lv, f->fp.rec, f->ws, d_S, f->use_tc ? 1 + (f->cfg.mlp_precision == NSM_MLP_BF16) : 0,
                                        f->n_sms, f->stream));
         if (f->use_tc)
           RUN(f, K_MLP_FWD, launch_mlp_forward_tc(f->ms, f->cfg.mlp_precision == NSM_MLP_BF16, nullptr, f->ws, d_S, 1, 0, f->n_sms,
                                                   f->stream));
         else
-          RUN(f, K_MLP_FWD, launch_mlp_forward_simt(f->ms, f->fp.theta + f->fp.n_table, nullptr, f->ws, d_S, 1, f->n_sms, f->stream));
+          RUN(f, K_MLP_FWD, launch_mlp_forward_simt(f->ms, f->fp.mlp_theta, nullptr, f->ws, d_S, 1, f->n_sms, f->stream));
         RUN(f, K_OCC, launch_occ_threshold(f->cfg.occ_res, first, n, f->ws.sigma, f->cfg.occ_sigma_threshold,
                                            f->fp.occ_bits, f->stream));
       }
@@ -572,7 +586,10 @@ nsm_status nsm_train_step_host(nsm_field *f, const nsm_ray_batch *hb, float lamb
 
 nsm_status nsm_debug_set_grad(nsm_field *f, const float *d_grad, const uint8_t *d_touched) {
   if (!f) return fail(NSM_ERR_INVALID_ARG, "field is NULL");
-  if (d_grad) CUDA_TRY(cudaMemcpyAsync(f->fp.grad, d_grad, sizeof(float) * (f->fp.n_table + f->fp.n_mlp), cudaMemcpyDeviceToDevice, f->stream));
+  if (d_grad) {
+    RUN(f, K_DEBUG, launch_pack_records(f->fp, 1, d_grad, f->stream));
+    CUDA_TRY(cudaMemcpyAsync(f->fp.mlp_grad, d_grad + f->fp.n_table, sizeof(float) * f->fp.n_mlp, cudaMemcpyDeviceToDevice, f->stream));
+  }
   if (d_touched) CUDA_TRY(cudaMemcpyAsync(f->fp.touched, d_touched, f->fp.n_entries, cudaMemcpyDeviceToDevice, f->stream));
   f->grads_dirty = true;
   return NSM_OK;
@@ -650,7 +667,7 @@ nsm_status nsm_debug_last_step(nsm_field *f, int item, void *d_out, uint64_t cap
     case NSM_DBG_O: src = ws.O; bytes = 4ull * R; break;
     case NSM_DBG_DSIGMA: src = ws.dsigma; bytes = 4ull * S; break;
     case NSM_DBG_DRGB: src = ws.drgb; bytes = 12ull * S; break;
-    case NSM_DBG_GRAD: src = f->fp.grad; bytes = 4ull * (f->fp.n_table + f->fp.n_mlp); break;
+    case NSM_DBG_GRAD: bytes = 4ull * (f->fp.n_table + f->fp.n_mlp); break;
     case NSM_DBG_TOUCHED: src = f->fp.touched; bytes = f->fp.n_entries; break;
     case NSM_DBG_SAMPLE_X: bytes = 12ull * S; break;
     case NSM_DBG_E: bytes = 4ull * S * f->ms.LF; break;
@@ -666,6 +683,9 @@ nsm_status nsm_debug_last_step(nsm_field *f, int item, void *d_out, uint64_t cap
   if (bytes == 0) return NSM_OK;
   if (src) {
     CUDA_TRY(cudaMemcpyAsync(d_out, src, bytes, cudaMemcpyDeviceToDevice, f->stream));
+  } else if (item == NSM_DBG_GRAD) {
+    RUN(f, K_DEBUG, launch_unpack_records(f->fp, 1, (float *)d_out, f->stream));
+    CUDA_TRY(cudaMemcpyAsync((float *)d_out + f->fp.n_table, f->fp.mlp_grad, sizeof(float) * f->fp.n_mlp, cudaMemcpyDeviceToDevice, f->stream));
   } else if (item == NSM_DBG_SAMPLE_X) {
     RUN(f, K_DEBUG, launch_planes_to_rows(ws.s_x, ws.cap, 3, d_S, (float *)d_out, f->stream));
   } else if (item == NSM_DBG_E) {

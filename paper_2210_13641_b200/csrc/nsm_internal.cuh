@@ -72,11 +72,19 @@ enum KernelId {
   K_ADAM_TABLE, K_ADAM_MLP, K_OCC, K_DEBUG, K_COUNT
 };
 
+// Parameters.  Hash-table entries are stored as RECORDS: entry e owns 4F consecutive floats
+//   rec[e*4F + 0F .. 1F) = theta   rec[.. 1F..2F) = gradient   rec[.. 2F..3F) = Adam m   rec[.. 3F..4F) = Adam v
+// so that with F = 2 an entry is exactly one 32-byte DRAM/L2 sector: the gather (theta), the
+// scatter (gradient) and the touched-only Adam update (all four) of one entry hit the SAME sector,
+// which the step's first access brings into the 126 MB L2 and the later ones find there.  The
+// canonical flat layout of include/nsm.h exists only at the boundary (pack/unpack kernels).
 struct FieldParams {
-  float *theta, *m, *v, *grad; // [P] canonical: tables then MLP
-  uint8_t *touched;            // [n_entries]
-  uint8_t *occ_bits;           // [G^3/8]
+  float *rec;                                       // [n_entries][4F]
+  float *mlp_theta, *mlp_m, *mlp_v, *mlp_grad;      // [n_mlp] each, canonical order
+  uint8_t *touched;                                 // [n_entries]
+  uint8_t *occ_bits;                                // [G^3/8]
   uint64_t n_entries, n_table, n_mlp;
+  uint32_t F;
 };
 
 // ---- launchers (each enqueues on `st`, returns the number of kernels launched) ----
@@ -86,10 +94,13 @@ int launch_scan(const MarchParams &mp, const Workspace &ws, int count_total, cud
 int launch_march_write(const MarchParams &mp, const float *origins, const float *dirs, const Workspace &ws,
                        cudaStream_t st);
 // out_mode: 0 = fp32 planes ws.e, 1 = fp16 blob ws.blob_e, 2 = bf16 blob ws.blob_e
-int launch_encode(const LevelTable &lv, const float *theta, const Workspace &ws,
+int launch_encode(const LevelTable &lv, const float *rec, const Workspace &ws,
                   const uint32_t *d_S, int out_mode, int n_sms, cudaStream_t st);
-int launch_scatter(const LevelTable &lv, float *grad, uint8_t *touched, const Workspace &ws,
+int launch_scatter(const LevelTable &lv, float *rec, uint8_t *touched, const Workspace &ws,
                    const uint32_t *d_S, int n_sms, cudaStream_t st);
+// canonical [n_entries][F] <-> field `which` (0 theta, 1 grad, 2 m, 3 v) of the records; src == nullptr packs zeros
+int launch_pack_records(const FieldParams &fp, int which, const float *src, cudaStream_t st);
+int launch_unpack_records(const FieldParams &fp, int which, float *dst, cudaStream_t st);
 int launch_mlp_forward_simt(const MlpShape &ms, const float *theta_mlp, const float *dirs,
                             const Workspace &ws, const uint32_t *d_S, int density_only, int n_sms,
                             cudaStream_t st);
