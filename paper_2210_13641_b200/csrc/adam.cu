@@ -18,45 +18,60 @@ __device__ __forceinline__ void adam_one(float &th, float &m, float &v, float g,
   th = th - c.lr * mhat / (sqrtf(vhat) + c.eps);
 }
 
-// One thread per 4 consecutive entries: the four flag bytes come in one coalesced 4-byte load; a
-// touched entry's record (4F floats; one 32 B sector for F = 2) is read and written with float4s.
+// One thread per B consecutive entries: their flag bytes come in one coalesced load; the records
+// of the touched ones (4F floats each; one 32 B sector for F = 2) are ALL requested before any is
+// used, so a thread keeps up to B record loads in flight (the kernel is latency-, not
+// bandwidth-limited at 25 % touched).
 template <int F>
 __global__ void __launch_bounds__(256) adam_table_kernel(float *__restrict__ rec, uint8_t *__restrict__ touched,
                                                          uint64_t n_entries, int sparse, AdamConst c) {
-  const uint64_t n_quads = (n_entries + 3) / 4;
-  for (uint64_t q = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; q < n_quads; q += (uint64_t)gridDim.x * blockDim.x) {
-    const uint64_t e0 = q * 4;
-    uint32_t flags;
-    if (e0 + 4 <= n_entries) {
-      flags = *reinterpret_cast<const uint32_t *>(touched + e0);
+  constexpr int B = (F <= 2) ? 8 : 4;
+  const uint64_t n_groups = (n_entries + B - 1) / B;
+  for (uint64_t q = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; q < n_groups; q += (uint64_t)gridDim.x * blockDim.x) {
+    const uint64_t e0 = q * B;
+    uint64_t flags = 0;
+    if (e0 + B <= n_entries) {
+      if (B == 8) flags = *reinterpret_cast<const uint64_t *>(touched + e0);
+      else flags = *reinterpret_cast<const uint32_t *>(touched + e0);
     } else {
-      flags = 0;
-      for (uint64_t e = e0; e < n_entries; ++e) flags |= (uint32_t)touched[e] << (8 * (e - e0));
+      for (uint64_t e = e0; e < n_entries; ++e) flags |= (uint64_t)touched[e] << (8 * (e - e0));
     }
     if (sparse && flags == 0) continue;
+    float4 x[B][F];
+    bool act[B];
 #pragma unroll
-    for (int j = 0; j < 4; ++j) {
-      const uint64_t e = e0 + j;
-      const bool t = (flags >> (8 * j)) & 0xffu;
-      if (e >= n_entries || (sparse && !t)) continue;
-      float4 *r4 = reinterpret_cast<float4 *>(rec + e * 4 * F);
+    for (int j = 0; j < B; ++j) {
+      act[j] = (e0 + j < n_entries) && (!sparse || ((flags >> (8 * j)) & 0xffu));
+      if (act[j]) {
+        const float4 *r4 = reinterpret_cast<const float4 *>(rec + (e0 + j) * 4 * F);
+#pragma unroll
+        for (int i = 0; i < F; ++i) x[j][i] = r4[i];
+      }
+    }
+#pragma unroll
+    for (int j = 0; j < B; ++j) {
+      if (!act[j]) continue;
       float vals[4 * F];
 #pragma unroll
       for (int i = 0; i < F; ++i) {
-        const float4 x = r4[i];
-        vals[4 * i] = x.x; vals[4 * i + 1] = x.y; vals[4 * i + 2] = x.z; vals[4 * i + 3] = x.w;
+        vals[4 * i] = x[j][i].x; vals[4 * i + 1] = x[j][i].y; vals[4 * i + 2] = x[j][i].z; vals[4 * i + 3] = x[j][i].w;
       }
 #pragma unroll
       for (int f = 0; f < F; ++f) {
         adam_one(vals[f], vals[2 * F + f], vals[3 * F + f], vals[F + f], c);
         vals[F + f] = 0.f;   // the gradient is consumed
       }
+      float4 *r4 = reinterpret_cast<float4 *>(rec + (e0 + j) * 4 * F);
 #pragma unroll
       for (int i = 0; i < F; ++i) r4[i] = make_float4(vals[4 * i], vals[4 * i + 1], vals[4 * i + 2], vals[4 * i + 3]);
     }
     if (flags) {
-      if (e0 + 4 <= n_entries) *reinterpret_cast<uint32_t *>(touched + e0) = 0u;
-      else for (uint64_t e = e0; e < n_entries; ++e) touched[e] = 0;
+      if (e0 + B <= n_entries) {
+        if (B == 8) *reinterpret_cast<uint64_t *>(touched + e0) = 0ull;
+        else *reinterpret_cast<uint32_t *>(touched + e0) = 0u;
+      } else {
+        for (uint64_t e = e0; e < n_entries; ++e) touched[e] = 0;
+      }
     }
   }
 }

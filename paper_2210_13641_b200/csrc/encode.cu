@@ -112,11 +112,20 @@ __global__ void __launch_bounds__(256) encode_forward_kernel(LevelTable lv, cons
       for (int f = 0; f < F; ++f) ws.e[(size_t)(l * F + f) * ws.cap + s] = acc[f];
     } else {
       const uint32_t c = l * F;   // F consecutive columns never straddle an 8-column panel (F | 8)
-      uint8_t *dst = ws.blob_e + (s >> 7) * ((size_t)LF * NSM_TILE * 2) + (c >> 3) * (NSM_TILE * 16) + (s & 127) * 16 + (c & 7) * 2;
+      // two-term tile: [hi: LF*256 bytes][lo: LF*256 bytes] per 128-sample tile (e = hi + lo)
+      const size_t half = (size_t)LF * NSM_TILE * 2;
+      uint8_t *dst = ws.blob_e + (s >> 7) * (2 * half) + (c >> 3) * (NSM_TILE * 16) + (s & 127) * 16 + (c & 7) * 2;
 #pragma unroll
       for (int f = 0; f < F; ++f) {
-        if (MODE == 1) reinterpret_cast<__half *>(dst)[f] = __float2half_rn(acc[f]);
-        else reinterpret_cast<__nv_bfloat16 *>(dst)[f] = __float2bfloat16_rn(acc[f]);
+        if (MODE == 1) {
+          const __half hi = __float2half_rn(acc[f]);
+          reinterpret_cast<__half *>(dst)[f] = hi;
+          reinterpret_cast<__half *>(dst + half)[f] = __float2half_rn(acc[f] - __half2float(hi));
+        } else {
+          const __nv_bfloat16 hi = __float2bfloat16_rn(acc[f]);
+          reinterpret_cast<__nv_bfloat16 *>(dst)[f] = hi;
+          reinterpret_cast<__nv_bfloat16 *>(dst + half)[f] = __float2bfloat16_rn(acc[f] - __bfloat162float(hi));
+        }
       }
     }
   }

@@ -13,6 +13,13 @@
 // (cp.async.bulk, no tensor map needed) straight into the MMA operand buffer: the encoder's output
 // e, the activations saved for the backward pass, and the 16-bit weight images (packed once per
 // step by pack_weights_kernel, not converted per CTA).
+//
+// Forward precision: every forward operand is carried as a two-term 16-bit expansion x = hi + lo
+// (hi = round16(x), lo = round16(x - hi)) and each layer issues three MMA groups into the same fp32
+// accumulator, hi*hi + lo*hi + hi*lo.  The tensor-core time is negligible here, and the forward
+// pre-activations become accurate to ~2^-16 or better, so the ReLU masks the backward pass uses agree with the
+// float64 oracle (a plain 16-bit forward flips masks of near-zero pre-activations, which alone
+// costs 1-3 % of relative L2 error on the fine-level table gradients).
 #include "nsm_internal.cuh"
 #include "tc_common.cuh"
 
@@ -60,7 +67,9 @@ __global__ void pack_weights_kernel(MlpShape ms, const float *__restrict__ Wm, u
   for (uint32_t idx = threadIdx.x; idx < m.f_NP * m.f_KP; idx += blockDim.x) {
     const uint32_t n = idx / m.f_KP, k = idx - n * m.f_KP;
     const float v = (n < m.n_out && k < m.n_in) ? Wm[m.off + n * m.n_in + k] : 0.f;
-    *reinterpret_cast<T *>(img_f + m.f_off + tile_off(m.f_NP, n, k)) = T(v);
+    const T hi = T(v);
+    *reinterpret_cast<T *>(img_f + m.f_off + tile_off(m.f_NP, n, k)) = hi;
+    *reinterpret_cast<T *>(img_f + WImg::f_total + m.f_off + tile_off(m.f_NP, n, k)) = T(v - (float)hi);   // lo image
   }
   for (uint32_t idx = threadIdx.x; idx < m.b_NP * m.b_KP; idx += blockDim.x) {
     const uint32_t i = idx / m.b_KP, o = idx - i * m.b_KP;
@@ -77,6 +86,23 @@ __device__ __forceinline__ void issue_layer(uint32_t tmem_d, uint32_t a_saddr, u
     const uint64_t da = make_desc(a_saddr + k * 2 * PANEL, PANEL, 128);
     const uint64_t db = make_desc(b_saddr + k * 2 * NP * 16, NP * 16, 128);
     mma_ss(tmem_d, da, db, idesc, k > 0);
+  }
+  mma_commit(bar_saddr);
+}
+
+// the same with two-term operands: D = A_hi B_hi + A_lo B_hi + A_hi B_lo (lo tiles sit a_lo / b_lo bytes behind)
+__device__ __forceinline__ void issue_layer_split(uint32_t tmem_d, uint32_t a_saddr, uint32_t a_lo, uint32_t b_saddr,
+                                                  uint32_t b_lo, uint32_t K, uint32_t N, uint32_t NP, uint32_t fmt,
+                                                  uint32_t bar_saddr) {
+  const uint32_t idesc = make_idesc(fmt, 128, N, 0, 0);
+#pragma unroll 1
+  for (uint32_t term = 0; term < 3; ++term) {
+    const uint32_t a = a_saddr + (term == 1 ? a_lo : 0u), b = b_saddr + (term == 2 ? b_lo : 0u);
+    for (uint32_t k = 0; k < K / 16; ++k) {
+      const uint64_t da = make_desc(a + k * 2 * PANEL, PANEL, 128);
+      const uint64_t db = make_desc(b + k * 2 * NP * 16, NP * 16, 128);
+      mma_ss(tmem_d, da, db, idesc, (term | k) > 0);
+    }
   }
   mma_commit(bar_saddr);
 }
@@ -118,15 +144,43 @@ __device__ __forceinline__ void emit16(float *v, uint8_t *smem_tile, uint8_t *bl
   }
 }
 
+// two-term version: hi -> smem_tile and blob, lo -> smem_tile + lo_off
+template <typename T, bool RELU>
+__device__ __forceinline__ void emit16s(float *v, uint8_t *smem_tile, uint32_t lo_off, uint8_t *blob_tile, uint32_t c0,
+                                        bool valid) {
+  if (RELU) {
+#pragma unroll
+    for (int j = 0; j < 16; ++j) v[j] = fmaxf(v[j], 0.f);
+  }
+  uint32_t hi[8], lo[8];
+#pragma unroll
+  for (int j = 0; j < 8; ++j) {
+    hi[j] = pack2<T>(v[2 * j], v[2 * j + 1]);
+    const float2 h = unpack2<T>(hi[j]);
+    lo[j] = pack2<T>(v[2 * j] - h.x, v[2 * j + 1] - h.y);
+  }
+  const uint32_t o0 = tile_off(ROWS, threadIdx.x, c0), o1 = tile_off(ROWS, threadIdx.x, c0 + 8);
+  *reinterpret_cast<uint4 *>(smem_tile + o0) = make_uint4(hi[0], hi[1], hi[2], hi[3]);
+  *reinterpret_cast<uint4 *>(smem_tile + o1) = make_uint4(hi[4], hi[5], hi[6], hi[7]);
+  *reinterpret_cast<uint4 *>(smem_tile + lo_off + o0) = make_uint4(lo[0], lo[1], lo[2], lo[3]);
+  *reinterpret_cast<uint4 *>(smem_tile + lo_off + o1) = make_uint4(lo[4], lo[5], lo[6], lo[7]);
+  if (blob_tile) {
+    const uint4 z = make_uint4(0, 0, 0, 0);
+    *reinterpret_cast<uint4 *>(blob_tile + o0) = valid ? make_uint4(hi[0], hi[1], hi[2], hi[3]) : z;
+    *reinterpret_cast<uint4 *>(blob_tile + o1) = valid ? make_uint4(hi[4], hi[5], hi[6], hi[7]) : z;
+  }
+}
+
 // ------------------------------------------------------------------------------------- forward
 constexpr uint32_t COL_D1 = 0, COL_D2 = 64, COL_C1 = 96, COL_C2 = 160, COL_C3 = 224, FWD_COLS = 256;
 
+constexpr uint32_t TILE_BYTES = ROWS * H * 2;   // one [128][64] 16-bit tile
 struct FwdSmem {
-  static constexpr uint32_t w = 0;                                // weight image (WImg forward region)
-  static constexpr uint32_t bufE = w + WImg::f_total;             // [128][64] encoder output tile (TMA destination)
-  static constexpr uint32_t bufA = bufE + ROWS * H * 2;           // [128][64]
-  static constexpr uint32_t bufB = bufA + ROWS * H * 2;           // [128][64]
-  static constexpr uint32_t bar_mma = bufB + ROWS * H * 2;
+  static constexpr uint32_t w = 0;                                // weight images: hi (WImg forward region) then lo
+  static constexpr uint32_t bufE = w + 2 * WImg::f_total;         // encoder tile hi | lo (TMA destination, 2 x LF*256 bytes)
+  static constexpr uint32_t bufA = bufE + 2 * TILE_BYTES;         // hi | lo
+  static constexpr uint32_t bufB = bufA + 2 * TILE_BYTES;         // hi | lo
+  static constexpr uint32_t bar_mma = bufB + 2 * TILE_BYTES;
   static constexpr uint32_t bar_w = bar_mma + 8;
   static constexpr uint32_t bar_e = bar_w + 8;
   static constexpr uint32_t tmem = bar_e + 8;
@@ -142,15 +196,15 @@ __global__ void __launch_bounds__(128) mlp_forward_tc_kernel(MlpShape ms, const 
   const uint32_t sbase = smem_u32(smem);
   const uint32_t bar_mma = sbase + FwdSmem::bar_mma, bar_w = sbase + FwdSmem::bar_w, bar_e = sbase + FwdSmem::bar_e;
   const uint32_t LF = ms.LF;
-  const uint32_t e_bytes = LF * ROWS * 2;
+  const uint32_t e_half = LF * ROWS * 2, e_bytes = 2 * e_half;   // hi | lo
   const uint64_t S = *d_S;
   if ((uint64_t)blockIdx.x * ROWS >= S) return;
 
   if (tid == 0) {
     mbar_init(bar_mma, 1); mbar_init(bar_w, 1); mbar_init(bar_e, 1);
     fence_async_smem();
-    mbar_expect_tx(bar_w, WImg::f_total);
-    bulk_g2s(sbase + FwdSmem::w, ws.wimg_fwd, WImg::f_total, bar_w);
+    mbar_expect_tx(bar_w, 2 * WImg::f_total);
+    bulk_g2s(sbase + FwdSmem::w, ws.wimg_fwd, 2 * WImg::f_total, bar_w);
     mbar_expect_tx(bar_e, e_bytes);
     bulk_g2s(sbase + FwdSmem::bufE, ws.blob_e + (size_t)blockIdx.x * e_bytes, e_bytes, bar_e);
   }
@@ -174,7 +228,7 @@ __global__ void __launch_bounds__(128) mlp_forward_tc_kernel(MlpShape ms, const 
     if (tid == 0) {
       mbar_wait(bar_e, ph_e);
       fence_after();
-      issue_layer(tmem_base + COL_D1, sE, sW + WImg::f_d1, LF, H, H, fmt, bar_mma);
+      issue_layer_split(tmem_base + COL_D1, sE, e_half, sW + WImg::f_d1, WImg::f_total, LF, H, H, fmt, bar_mma);
     }
     ph_e ^= 1;
     mbar_wait(bar_mma, ph_mma); ph_mma ^= 1; fence_after();
@@ -190,10 +244,10 @@ __global__ void __launch_bounds__(128) mlp_forward_tc_kernel(MlpShape ms, const 
     for (uint32_t c0 = 0; c0 < H; c0 += 16) {
       tmem_ld16(tlane + COL_D1 + c0, v);
       tmem_ld_wait();
-      emit16<T, true>(v, bufB, blob_hd, c0, valid);
+      emit16s<T, true>(v, bufB, TILE_BYTES, blob_hd, c0, valid);
     }
     fence_async_smem(); fence_before(); __syncthreads();
-    if (tid == 0) { fence_after(); issue_layer(tmem_base + COL_D2, sB, sW + WImg::f_d2, H, DO, DO, fmt, bar_mma); }
+    if (tid == 0) { fence_after(); issue_layer_split(tmem_base + COL_D2, sB, TILE_BYTES, sW + WImg::f_d2, WImg::f_total, H, DO, DO, fmt, bar_mma); }
     mbar_wait(bar_mma, ph_mma); ph_mma ^= 1; fence_after();
     float g[16];
     tmem_ld16(tlane + COL_D2, g);
@@ -215,35 +269,35 @@ __global__ void __launch_bounds__(128) mlp_forward_tc_kernel(MlpShape ms, const 
       sh_row(ms.sh_degree, dx, dy, dz, Y);
       for (uint32_t j = 0; j < ms.n_sh; ++j) ci[ms.geo_cnt + j] = Y[j];
       uint8_t *blob_ci = save_blobs ? ws.blob_ci + (size_t)tile * (CIP * ROWS * 2) : nullptr;
-      emit16<T, false>(ci, bufA, blob_ci, 0, valid);
-      emit16<T, false>(ci + 16, bufA, blob_ci, 16, valid);
+      emit16s<T, false>(ci, bufA, TILE_BYTES, blob_ci, 0, valid);
+      emit16s<T, false>(ci + 16, bufA, TILE_BYTES, blob_ci, 16, valid);
     }
     fence_async_smem(); fence_before(); __syncthreads();
-    if (tid == 0) { fence_after(); issue_layer(tmem_base + COL_C1, sA, sW + WImg::f_c1, CIP, H, H, fmt, bar_mma); }
+    if (tid == 0) { fence_after(); issue_layer_split(tmem_base + COL_C1, sA, TILE_BYTES, sW + WImg::f_c1, WImg::f_total, CIP, H, H, fmt, bar_mma); }
     mbar_wait(bar_mma, ph_mma); ph_mma ^= 1; fence_after();
     uint8_t *blob_h1 = save_blobs ? ws.blob_h1 + (size_t)tile * (H * ROWS * 2) : nullptr;
 #pragma unroll
     for (uint32_t c0 = 0; c0 < H; c0 += 16) {
       tmem_ld16(tlane + COL_C1 + c0, v);
       tmem_ld_wait();
-      emit16<T, true>(v, bufB, blob_h1, c0, valid);
+      emit16s<T, true>(v, bufB, TILE_BYTES, blob_h1, c0, valid);
     }
     uint32_t sLast = sB;
     if (ms.n_color_layers == 2) {
       fence_async_smem(); fence_before(); __syncthreads();
-      if (tid == 0) { fence_after(); issue_layer(tmem_base + COL_C2, sB, sW + WImg::f_c2, H, H, H, fmt, bar_mma); }
+      if (tid == 0) { fence_after(); issue_layer_split(tmem_base + COL_C2, sB, TILE_BYTES, sW + WImg::f_c2, WImg::f_total, H, H, H, fmt, bar_mma); }
       mbar_wait(bar_mma, ph_mma); ph_mma ^= 1; fence_after();
       uint8_t *blob_h2 = save_blobs ? ws.blob_h2 + (size_t)tile * (H * ROWS * 2) : nullptr;
 #pragma unroll
       for (uint32_t c0 = 0; c0 < H; c0 += 16) {
         tmem_ld16(tlane + COL_C2 + c0, v);
         tmem_ld_wait();
-        emit16<T, true>(v, bufA, blob_h2, c0, valid);
+        emit16s<T, true>(v, bufA, TILE_BYTES, blob_h2, c0, valid);
       }
       sLast = sA;
     }
     fence_async_smem(); fence_before(); __syncthreads();
-    if (tid == 0) { fence_after(); issue_layer(tmem_base + COL_C3, sLast, sW + WImg::f_c3, H, 16, 16, fmt, bar_mma); }
+    if (tid == 0) { fence_after(); issue_layer_split(tmem_base + COL_C3, sLast, TILE_BYTES, sW + WImg::f_c3, WImg::f_total, H, 16, 16, fmt, bar_mma); }
     mbar_wait(bar_mma, ph_mma); ph_mma ^= 1; fence_after();
     tmem_ld16(tlane + COL_C3, v);
     tmem_ld_wait();
@@ -350,7 +404,7 @@ __global__ void __launch_bounds__(128, 1) mlp_backward_tc_kernel(MlpShape ms, fl
       case 1: src = ws.blob_h1 + tile * hbytes; bytes = hbytes; break;
       case 2: src = ws.blob_ci + tile * cbytes; bytes = cbytes; break;
       case 3: src = ws.blob_hd + tile * hbytes; bytes = hbytes; break;
-      default: src = ws.blob_e + tile * ebytes; bytes = ebytes; break;
+      default: src = ws.blob_e + tile * (2 * (size_t)ebytes); bytes = ebytes; break;   // the hi half of the two-term tile
     }
     mbar_expect_tx(bar_x[buf], bytes);
     bulk_g2s(sX[buf], src, bytes, bar_x[buf]);
@@ -523,14 +577,17 @@ __global__ void __launch_bounds__(128, 1) mlp_backward_tc_kernel(MlpShape ms, fl
 
 // blob tile image -> fp32 rows [S][n_cols] (debug getter)
 template <typename T>
-__global__ void blob_to_rows_kernel(const uint8_t *__restrict__ blob, uint32_t n_cols, const uint32_t *__restrict__ d_S,
-                                    float *__restrict__ rows) {
+__global__ void blob_to_rows_kernel(const uint8_t *__restrict__ blob, uint32_t n_cols, int two_term,
+                                    const uint32_t *__restrict__ d_S, float *__restrict__ rows) {
   const uint64_t S = *d_S, total = S * n_cols;
   for (uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; i < total; i += (uint64_t)gridDim.x * blockDim.x) {
     const uint64_t s = i / n_cols;
     const uint32_t c = (uint32_t)(i - s * n_cols);
-    const uint8_t *p = blob + (s >> 7) * ((size_t)n_cols * ROWS * 2) + tile_off(ROWS, (uint32_t)(s & 127), c);
-    rows[i] = (float)(*reinterpret_cast<const T *>(p));
+    const size_t half = (size_t)n_cols * ROWS * 2;
+    const uint8_t *p = blob + (s >> 7) * (two_term ? 2 * half : half) + tile_off(ROWS, (uint32_t)(s & 127), c);
+    float v = (float)(*reinterpret_cast<const T *>(p));
+    if (two_term) v += (float)(*reinterpret_cast<const T *>(p + half));
+    rows[i] = v;
   }
 }
 
@@ -541,7 +598,7 @@ bool mlp_tc_supported(const MlpShape &ms) {
          ms.n_sh <= 16 && ms.geo_off + ms.geo_cnt <= DO;
 }
 
-size_t mlp_tc_wimg_bytes(int backward) { return backward ? WImg::b_total : WImg::f_total; }
+size_t mlp_tc_wimg_bytes(int backward) { return backward ? WImg::b_total : 2 * WImg::f_total; }
 
 int launch_pack_weights(const MlpShape &ms, int bf16, const float *theta_mlp, const Workspace &ws, cudaStream_t st) {
   if (bf16) pack_weights_kernel<__nv_bfloat16><<<5, 256, 0, st>>>(ms, theta_mlp, ws.wimg_fwd, ws.wimg_bwd);
@@ -575,8 +632,9 @@ int launch_mlp_backward_tc(const MlpShape &ms, int bf16, float *grad_mlp, const 
   return 1;
 }
 
-int launch_blob_to_rows(int bf16, const uint8_t *blob, uint32_t n_cols, const uint32_t *d_S, float *rows, cudaStream_t st) {
-  if (bf16) blob_to_rows_kernel<__nv_bfloat16><<<1024, 256, 0, st>>>(blob, n_cols, d_S, rows);
-  else blob_to_rows_kernel<__half><<<1024, 256, 0, st>>>(blob, n_cols, d_S, rows);
+int launch_blob_to_rows(int bf16, const uint8_t *blob, uint32_t n_cols, int two_term, const uint32_t *d_S, float *rows,
+                        cudaStream_t st) {
+  if (bf16) blob_to_rows_kernel<__nv_bfloat16><<<1024, 256, 0, st>>>(blob, n_cols, two_term, d_S, rows);
+  else blob_to_rows_kernel<__half><<<1024, 256, 0, st>>>(blob, n_cols, two_term, d_S, rows);
   return 1;
 }

@@ -389,7 +389,7 @@ nsm_status nsm_create_field(const nsm_field_config *cfg, void *cuda_stream, nsm_
   ws.e = ws.hd = ws.g = ws.h1 = ws.h2 = nullptr;
   ws.blob_e = ws.blob_hd = ws.blob_ci = ws.blob_h1 = ws.blob_h2 = ws.wimg_fwd = ws.wimg_bwd = nullptr;
   if (f->use_tc) {   // 16-bit operand-tile blobs: 2 bytes per value, 128-row tiles
-    A(f->alloc(&ws.blob_e, 2 * ms.LF * cap)); A(f->alloc(&ws.blob_hd, 2 * ms.Hd * cap)); A(f->alloc(&ws.blob_ci, 2 * 32 * cap));
+    A(f->alloc(&ws.blob_e, 4 * ms.LF * cap));   /* two-term (hi | lo) tiles */ A(f->alloc(&ws.blob_hd, 2 * ms.Hd * cap)); A(f->alloc(&ws.blob_ci, 2 * 32 * cap));
     A(f->alloc(&ws.blob_h1, 2 * ms.Hc * cap)); A(f->alloc(&ws.blob_h2, 2 * (ms.n_color_layers == 2 ? ms.Hc : 1) * cap));
     A(f->alloc(&ws.wimg_fwd, mlp_tc_wimg_bytes(0))); A(f->alloc(&ws.wimg_bwd, mlp_tc_wimg_bytes(1)));
   } else {
@@ -690,7 +690,7 @@ nsm_status nsm_debug_last_step(nsm_field *f, int item, void *d_out, uint64_t cap
     RUN(f, K_DEBUG, launch_planes_to_rows(ws.s_x, ws.cap, 3, d_S, (float *)d_out, f->stream));
   } else if (item == NSM_DBG_E) {
     if (f->use_tc)
-      RUN(f, K_DEBUG, launch_blob_to_rows(f->cfg.mlp_precision == NSM_MLP_BF16, ws.blob_e, f->ms.LF, d_S, (float *)d_out, f->stream));
+      RUN(f, K_DEBUG, launch_blob_to_rows(f->cfg.mlp_precision == NSM_MLP_BF16, ws.blob_e, f->ms.LF, 1, d_S, (float *)d_out, f->stream));
     else
       RUN(f, K_DEBUG, launch_planes_to_rows(ws.e, ws.cap, f->ms.LF, d_S, (float *)d_out, f->stream));
   } else if (item == NSM_DBG_SLOTS) {

@@ -115,7 +115,8 @@ int launch_mlp_forward_tc(const MlpShape &ms, int bf16, const float *dirs, const
                           int density_only, int save_blobs, int n_sms, cudaStream_t st);
 int launch_mlp_backward_tc(const MlpShape &ms, int bf16, float *grad_mlp, const Workspace &ws, const uint32_t *d_S,
                            int n_sms, cudaStream_t st);
-int launch_blob_to_rows(int bf16, const uint8_t *blob, uint32_t n_cols, const uint32_t *d_S, float *rows, cudaStream_t st);
+int launch_blob_to_rows(int bf16, const uint8_t *blob, uint32_t n_cols, int two_term, const uint32_t *d_S, float *rows,
+                        cudaStream_t st);
 int launch_composite_train(const Workspace &ws, uint32_t R, const float *rgb, const float *depth,
                            const float *depth_var, float lambda_d, const float bg[3],
                            cudaStream_t st);

@@ -27,8 +27,8 @@ def nsm():
     return mod
 
 
-# the encoder output is fp32 on the CUDA-core path; the tensor-core path stores it as the 16-bit MMA operand
-E_TOL = {"simt_fp32": 1e-4, "tcgen05_f16": 1e-3, "tcgen05_bf16": 8e-3}
+# the encoder output is fp32 on the CUDA-core path and a two-term 16-bit expansion on the tensor-core path
+E_TOL = {"simt_fp32": 1e-4, "tcgen05_f16": 1e-4, "tcgen05_bf16": 1e-4}   # two-term (hi + lo) tiles
 
 
 def tol_for(fc, path):
