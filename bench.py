@@ -85,20 +85,40 @@ class ClockSampler:
         return out
 
 
-def make_workload(n_batches):
+WORKLOADS = {
+    1: "BASELINE.json configs[0]: tiny fp32 case, 256 rays x 32 samples, full occupancy, L=4 F=2 T=2^10, 16-wide MLPs",
+    2: "BASELINE.json configs[1]: Instant-NGP-default field, 4096 rays x 128 candidates, 128^3 sphere-union occupancy, "
+       "L=16 F=2 T=2^19, MLPs 32->64->16 / 31->64->64->3",
+    3: "BASELINE.json configs[2]: keyframe-window mapping, 10 synthetic 1200x680 keyframes of the 8x6x3 m room, 2^14 rays x 128 "
+       "candidates per step, occupancy FULL then FROM_FIELD every 16 steps, field as config 2",
+    4: "BASELINE.json configs[3]: large-table stress, 2^12 rays x 512 candidates, L=16 F=4 T=2^22 N_max=8192 (719 MB of tables), "
+       "256^3 occupancy at ~10 %, bf16 MLPs",
+    5: "BASELINE.json configs[4]: full-frame render of 4 held-out 1200x680 views, 256 candidates/ray, cut 1e-4, field trained on "
+       "config 3's data",
+}
+
+
+def make_workload(n_batches, cfg=2):
     from workloads import configs
-    return configs.config2(n_batches=n_batches)
+    if cfg == 1:
+        return configs.config1()
+    if cfg == 2:
+        return configs.config2(n_batches=n_batches)
+    if cfg == 3:
+        return configs.config3(n_batches=n_batches)
+    if cfg == 4:
+        return configs.config4(n_batches=min(n_batches, 8))
+    raise ValueError(cfg)
 
 
-def workload_config(w, extra=None):
+def workload_config(w, extra=None, cfg=2):
     fc = w.field
-    c = dict(workload="BASELINE.json configs[1]: Instant-NGP-default field, 4096 rays x 128 candidates, 128^3 sphere-union "
-                      "occupancy, L=16 F=2 T=2^19, MLPs 32->64->16 / 31->64->64->3",
+    c = dict(workload=WORKLOADS[cfg],
              rays_per_step=w.batches[0].n_rays, candidates_per_ray=w.batches[0].n_candidates,
-             occupancy_fraction=round(w.extra["occupancy_fraction"], 4), lambda_d=w.lambda_d,
-             table_params=None, mlp_precision=["fp32", "fp16", "bf16"][fc.mlp_precision],
-             l2="not flushed: a step's working set (48.8 MB tables + 48.8 MB gradients + 97.6 MB Adam moments + per-sample "
-                "workspace) exceeds the 126 MB L2, and every step gets a fresh ray batch",
+             occupancy_fraction=round(w.extra["occupancy_fraction"], 4) if "occupancy_fraction" in w.extra else None,
+             lambda_d=w.lambda_d, table_params=None, mlp_precision=["fp32", "fp16", "bf16"][fc.mlp_precision],
+             l2="not flushed: the table records (theta, gradient, Adam m and v: 16 B per parameter, 195 MB at config 2) plus the "
+                "per-sample workspace exceed the 126 MB L2, and every step gets a fresh ray batch",
              batches=f"{len(w.batches)} distinct pre-generated batches, cycled")
     if extra:
         c.update(extra)
@@ -145,7 +165,7 @@ def run_reference(args):
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return 0
-    w = make_workload(N_BATCHES)
+    w = make_workload(N_BATCHES, 2)
     r = time_oracle(w, args.steps, args.warmup, budget_s=150.0)   # stops early past 150 s; steps actually done are reported
     sample = f"{r['steps']} oracle steps, each on the first {REF_RAYS} of the 4096 rays of a config-2 batch ({r['samples']} live samples in {r['seconds']:.1f} s)"
     line = dict(impl="reference", metric=METRIC, value=r["value"], unit=UNIT, n_gpus=args.gpus, steps=r["steps"], warmup=args.warmup,
@@ -181,6 +201,72 @@ def kernel_model(name, S, R, K, L, F, LF, U, E, mac, n_mlp):
     return dict(bound="hbm", bytes=0)
 
 
+def run_render(args, nsm, replicas, dev, rank, world, peaks):
+    """Config 5: forward-only full-frame render (rays/s, samples/s) of a field trained on config 3's data."""
+    import torch
+    from workloads import configs
+    w = configs.config3(n_batches=100)
+    fc = w.field
+    from dataclasses import replace
+    fc = replace(fc, max_candidates=256, max_rays=1 << 16)
+    f = nsm.Field(fc, dev)
+    f.nsm_set_params(configs.init_params(fc.seed, f.n_table, f.mlp_shapes()))
+    train_steps = 500
+    for i in range(train_steps):
+        if i > 0 and i % 16 == 0:
+            f.nsm_update_occupancy(nsm.NSM_OCC_FROM_FIELD, sync=False)
+        f.nsm_train_step(nsm.DeviceBatch(w.batches[i % len(w.batches)], dev), w.lambda_d, want_stats=False)
+    f.nsm_update_occupancy(nsm.NSM_OCC_FROM_FIELD)
+    occ = float(np.unpackbits(f.nsm_get_occupancy()).mean())
+    views = [nsm.DeviceBatch(v, dev) for v in configs.config5_views()]
+    hviews = [nsm.HostBatch(v) for v in configs.config5_views()]
+    K, W = args.steps, max(args.warmup, 3)
+    stream = torch.cuda.current_stream(dev)
+    n_rays = views[0].n_rays
+
+    def timed(fn, n):
+        ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize(dev)
+        ev0.record(stream)
+        for i in range(n):
+            fn(i)
+        ev1.record(stream)
+        torch.cuda.synchronize(dev)
+        return ev0.elapsed_time(ev1) * 1e-3
+
+    step = lambda i: f.nsm_render(views[i % 4], 1e-4)
+    for i in range(W):
+        step(i)
+    l0 = f.nsm_launch_count()
+    sampler = ClockSampler(dev.index)
+    t = timed(step, K)
+    clocks = sampler.stop()
+    launches = f.nsm_launch_count() - l0
+    outs = (torch.empty((n_rays, 3), dtype=torch.float32).pin_memory(), torch.empty(n_rays, dtype=torch.float32).pin_memory(),
+            torch.empty(n_rays, dtype=torch.float32).pin_memory())
+    e2e = lambda i: f.nsm_render_host(hviews[i % 4], 1e-4, outs)
+    e2e(0)
+    t_e2e = timed(e2e, K)
+    f.nsm_profile(True)
+    for i in range(min(K, 4)):
+        step(i)
+    torch.cuda.synchronize(dev)
+    prof = f.nsm_profile_read()
+    f.nsm_profile(False)
+    total_ms = sum(ms for ms, n in prof.values())
+    kernels = sorted([dict(kernel=k, total_ms=ms, launches=n, share=ms / total_ms) for k, (ms, n) in prof.items() if n], key=lambda k: -k["share"])
+    line = dict(metric="render rays/sec (forward only) on 1 B200", value=K * n_rays / t, unit="rays/s", n_gpus=world, steps=K, warmup=W,
+                ms_per_step=1e3 * t / K, higher_is_better=True, scaling="weak", vs_baseline=None,
+                dtype="f16", data="synthetic", config=dict(workload=WORKLOADS[5], rays_per_view=n_rays, train_steps=train_steps,
+                                                           occupancy_fraction_after_training=occ, mlp_path=f.nsm_mlp_path()),
+                clocks=clocks, e2e=dict(value=K * n_rays / t_e2e, unit="rays/s", h2d_bytes_per_step=hviews[0].bytes_in(),
+                                        d2h_bytes_per_step=n_rays * 20, ms_per_step=1e3 * t_e2e / K),
+                gpu_launches=launches, kernels=kernels)
+    f.close()
+    print(json.dumps(line))
+    return 0
+
+
 def run_cuda(args):
     import torch
     import paper_2210_13641_b200 as nsm
@@ -195,12 +281,17 @@ def run_cuda(args):
     torch.cuda.set_device(dev)
     peaks = measured_peaks()
 
-    w = make_workload(N_BATCHES)
+    cfg = args.config
+    if cfg == 5:
+        return run_render(args, nsm, replicas, dev, rank, world, peaks)
+    w = make_workload(N_BATCHES if cfg != 3 else 100, cfg)
     fc = w.field
     f = nsm.Field(fc, dev)
     theta0 = configs.init_params(fc.seed + rank, f.n_table, f.mlp_shapes())
     f.nsm_set_params(theta0)
-    f.nsm_update_occupancy(nsm.NSM_OCC_SET, w.bits)
+    if w.bits is not None:
+        f.nsm_update_occupancy(nsm.NSM_OCC_SET, w.bits)
+    refresh = 16 if cfg == 3 else 0          # config 3: occupancy FROM_FIELD every 16 steps (inside the timed region)
     dbatches = [nsm.DeviceBatch(b, dev) for b in w.batches]
     hbatches = [nsm.HostBatch(b) for b in w.batches]
     K, W = args.steps, max(args.warmup, 3)
@@ -220,7 +311,10 @@ def run_cuda(args):
         return ev0.elapsed_time(ev1) * 1e-3
 
     # ---- device-resident leg: inputs already in HBM, no host sync inside the timed region
-    dev_step = lambda i: f.nsm_train_step(dbatches[i % len(dbatches)], lam, want_stats=False)
+    def dev_step(i):
+        if refresh and i > 0 and i % refresh == 0:
+            f.nsm_update_occupancy(nsm.NSM_OCC_FROM_FIELD, sync=False)
+        f.nsm_train_step(dbatches[i % len(dbatches)], lam, want_stats=False)
     for i in range(W):
         dev_step(i)
     s0, l0 = f.nsm_total_samples(), f.nsm_launch_count()
@@ -232,7 +326,10 @@ def run_cuda(args):
     value, total_samples, t_max = replicas.aggregate_throughput(samples_dev, t_dev)
 
     # ---- end-to-end leg: HOST buffers through the C-ABI, H2D of the batch and D2H of the stats every step
-    e2e_step = lambda i: f.nsm_train_step_host(hbatches[i % len(hbatches)], lam, want_stats=True)
+    def e2e_step(i):
+        if refresh and i > 0 and i % refresh == 0:
+            f.nsm_update_occupancy(nsm.NSM_OCC_FROM_FIELD, sync=False)
+        f.nsm_train_step_host(hbatches[i % len(hbatches)], lam, want_stats=True)
     for i in range(W):
         e2e_step(i)
     s1 = f.nsm_total_samples()
@@ -297,7 +394,7 @@ def run_cuda(args):
         line = dict(metric=METRIC, value=value, unit=UNIT, n_gpus=world, steps=K, warmup=W, ms_per_step=1e3 * t_max / K,
                     higher_is_better=True, scaling="weak", vs_baseline=None, dtype="f32" if f.nsm_mlp_path() == "simt_fp32" else
                     ("f16" if fc.mlp_precision == 1 else "bf16"), data="synthetic",
-                    config=workload_config(w, dict(table_params=f.n_table, mlp_params=f.n_mlp, mlp_path=f.nsm_mlp_path(),
+                    config=workload_config(w, cfg=cfg, extra=dict(table_params=f.n_table, mlp_params=f.n_mlp, mlp_path=f.nsm_mlp_path(),
                                                    parallelism=f"{world} independent replica(s)",
                                                    samples_per_step=total_samples / K / world)),
                     rays_per_s=world * K * b0.n_rays / t_max, clocks=clocks,
@@ -318,9 +415,11 @@ def main():
     ap.add_argument("--steps", type=int, default=None, help="timed steps (default 2000; 40 for --impl reference)")
     ap.add_argument("--warmup", type=int, default=None, help="untimed warm-up steps (default 20; 2 for --impl reference)")
     ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
+    ap.add_argument("--config", type=int, default=2, choices=[1, 2, 3, 4, 5],
+                    help="BASELINE.json config to run (default 2 = configs[1], the one the metric is quoted on)")
     args = ap.parse_args()
     if args.steps is None:
-        args.steps = 40 if args.impl == "reference" else 2000
+        args.steps = 40 if args.impl == "reference" else {1: 2000, 2: 2000, 3: 100, 4: 200, 5: 3}[args.config]
     if args.warmup is None:
         args.warmup = 2 if args.impl == "reference" else 20
     if args.impl == "reference":

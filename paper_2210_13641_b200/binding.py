@@ -252,13 +252,15 @@ class Field:
         return th.cpu().numpy(), m.cpu().numpy(), v.cpu().numpy(), step.value
 
     # ---- occupancy
-    def nsm_update_occupancy(self, mode, bits=None):
+    def nsm_update_occupancy(self, mode, bits=None, sync=True):
         d = None
         if bits is not None:
             d = torch.as_tensor(np.ascontiguousarray(bits, np.uint8)).to(self.device)
             assert d.numel() == (self.fc.occ_res ** 3 + 7) // 8
+            sync = True     # the staging tensor must outlive the copy
         _check(self.lib.nsm_update_occupancy(self.h, int(mode), _dev_ptr(d, torch.uint8)))
-        torch.cuda.synchronize(self.device)
+        if sync:
+            torch.cuda.synchronize(self.device)
 
     def nsm_get_occupancy(self):
         d = torch.empty((self.fc.occ_res ** 3 + 7) // 8, dtype=torch.uint8, device=self.device)
