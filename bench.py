@@ -185,19 +185,17 @@ def kernel_model(name, S, R, K, L, F, LF, U, E, mac, n_mlp):
     if name == "encode":
         return dict(bound="hbm", bytes=gather + 12 * S + 4 * LF * S)
     if name == "scatter":
-        return dict(bound="hbm", bytes=2 * gather + 4 * LF * S + 12 * S + 8 * L * S)
+        return dict(bound="hbm", bytes=2 * gather + 4 * LF * S + 12 * S)
     if name == "adam_table":
-        return dict(bound="hbm", bytes=32 * F * U + E + U)
+        return dict(bound="hbm", bytes=32 * F * U)
     if name == "mlp_fwd":
         return dict(bound="alu", flops=2 * mac * S)
     if name == "mlp_bwd":
         return dict(bound="alu", flops=4 * mac * S)
     if name == "composite":
         return dict(bound="hbm", bytes=S * (4 + 4 + 4 + 12) * 2 + S * (4 + 4 + 12) + R * 40)
-    if name == "march_count":
+    if name == "march":
         return dict(bound="alu", flops=40 * R * K)
-    if name == "march_write":
-        return dict(bound="hbm", bytes=28 * S + R * 4 * ((K + 31) // 32))
     return dict(bound="hbm", bytes=0)
 
 

@@ -147,7 +147,8 @@ nsm_status nsm_train_step_host(nsm_field *f, const nsm_ray_batch *host_batch, fl
 nsm_status nsm_backward(nsm_field *f, const nsm_ray_batch *batch, float lambda_d,
                         nsm_step_stats *host_stats);
 nsm_status nsm_apply_adam(nsm_field *f);
-/* Overwrite the gradient buffer / touched flags (device pointers, canonical layouts). */
+/* Overwrite the gradient buffer (d_grad: [n_table + n_mlp], canonical layout, required) and the
+ * touched set (d_touched: one byte per table entry, or NULL = every entry touched). */
 nsm_status nsm_debug_set_grad(nsm_field *f, const float *d_grad, const uint8_t *d_touched);
 
 /* S15: forward-only render, u == 0.5, a ray stops after T < transmittance_cut (0 = never).

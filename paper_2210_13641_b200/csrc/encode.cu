@@ -146,11 +146,11 @@ __device__ __forceinline__ void red_add_entry(float *p, const float g[F]) {
   }
 }
 
-// S12: d theta[(offset_l + slot) F + f] += omega * dL/de[l F + f]; the touched set U is marked
-// structurally (every referenced entry), independent of the gradient's value.
+// S12: d theta[(offset_l + slot) F + f] += omega * dL/de[l F + f].  The touched set U is structural
+// (every referenced entry, independent of the gradient's value): it is carried by the gradient words
+// themselves, see FieldParams in nsm_internal.cuh.
 template <int F>
-__global__ void __launch_bounds__(256) scatter_backward_kernel(LevelTable lv, float *__restrict__ rec,
-                                                               uint8_t *__restrict__ touched, Workspace ws,
+__global__ void __launch_bounds__(256) scatter_backward_kernel(LevelTable lv, float *__restrict__ grad, Workspace ws,
                                                                const uint32_t *__restrict__ d_S) {
   const uint64_t S = *d_S;
   const uint64_t total = S * lv.n_levels;
@@ -162,18 +162,36 @@ __global__ void __launch_bounds__(256) scatter_backward_kernel(LevelTable lv, fl
     float de[F];
 #pragma unroll
     for (int f = 0; f < F; ++f) de[f] = ws.de[(size_t)(l * F + f) * ws.cap + s];
-    float *tab = rec + lv.offset[l] * (4 * F) + F;   // the gradient field of the records
-    uint8_t *tch = touched + lv.offset[l];
+    float *tab = grad + lv.offset[l] * F;
 #pragma unroll
     for (int k = 0; k < 8; ++k) {
       float om = corner_weight(k, ci.w);
       float g[F];
 #pragma unroll
-      for (int f = 0; f < F; ++f) g[f] = om * de[f];
-      red_add_entry<F>(tab + (size_t)ci.slot[k] * (4 * F), g);
-      tch[ci.slot[k]] = 1;
+      for (int f = 0; f < F; ++f) {
+        const float v = om * de[f];
+        g[f] = fabsf(v) < NSM_GRAD_MIN_ADDEND ? 0.0f : v;   // never -0.0, never near-subnormal; NaN stays NaN
+      }
+      red_add_entry<F>(tab + (size_t)ci.slot[k] * F, g);
     }
   }
+}
+
+// gradient array <- canonical gradient and flags (debug / test entry point)
+__global__ void set_grad_kernel(float *__restrict__ grad, uint32_t F, uint64_t n_entries, const float *__restrict__ src,
+                                const uint8_t *__restrict__ touched) {
+  const uint64_t total = n_entries * F;
+  for (uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; i < total; i += (uint64_t)gridDim.x * blockDim.x) {
+    const uint64_t e = i / F;
+    const bool t = src && (!touched || touched[e]);
+    const float v = t ? src[i] : 0.f;
+    grad[i] = t ? (fabsf(v) < NSM_GRAD_MIN_ADDEND ? 0.0f : v) : __uint_as_float(NSM_GRAD_UNTOUCHED);
+  }
+}
+
+__global__ void get_touched_kernel(const float *__restrict__ grad, uint32_t F, uint64_t n_entries, uint8_t *__restrict__ dst) {
+  for (uint64_t e = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; e < n_entries; e += (uint64_t)gridDim.x * blockDim.x)
+    dst[e] = __float_as_uint(grad[e * F]) != NSM_GRAD_UNTOUCHED;
 }
 
 __global__ void debug_slots_kernel(LevelTable lv, Workspace ws, const uint32_t *__restrict__ d_S,
@@ -256,14 +274,24 @@ int launch_encode(const LevelTable &lv, const float *theta, const Workspace &ws,
   return 1;
 }
 
-int launch_scatter(const LevelTable &lv, float *grad, uint8_t *touched, const Workspace &ws,
+int launch_set_grad(const FieldParams &fp, const float *src, const uint8_t *touched, cudaStream_t st) {
+  set_grad_kernel<<<2048, 256, 0, st>>>(fp.grad, fp.F, fp.n_entries, src, touched);
+  return 1;
+}
+
+int launch_get_touched(const FieldParams &fp, uint8_t *dst, cudaStream_t st) {
+  get_touched_kernel<<<2048, 256, 0, st>>>(fp.grad, fp.F, fp.n_entries, dst);
+  return 1;
+}
+
+int launch_scatter(const LevelTable &lv, float *grad, const Workspace &ws,
                    const uint32_t *d_S, int n_sms, cudaStream_t st) {
   dim3 grid(n_sms * 8), block(256);
   switch (lv.n_features) {
-    case 1: scatter_backward_kernel<1><<<grid, block, 0, st>>>(lv, grad, touched, ws, d_S); break;
-    case 2: scatter_backward_kernel<2><<<grid, block, 0, st>>>(lv, grad, touched, ws, d_S); break;
-    case 4: scatter_backward_kernel<4><<<grid, block, 0, st>>>(lv, grad, touched, ws, d_S); break;
-    default: scatter_backward_kernel<8><<<grid, block, 0, st>>>(lv, grad, touched, ws, d_S); break;
+    case 1: scatter_backward_kernel<1><<<grid, block, 0, st>>>(lv, grad, ws, d_S); break;
+    case 2: scatter_backward_kernel<2><<<grid, block, 0, st>>>(lv, grad, ws, d_S); break;
+    case 4: scatter_backward_kernel<4><<<grid, block, 0, st>>>(lv, grad, ws, d_S); break;
+    default: scatter_backward_kernel<8><<<grid, block, 0, st>>>(lv, grad, ws, d_S); break;
   }
   return 1;
 }

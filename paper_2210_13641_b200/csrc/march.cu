@@ -74,115 +74,124 @@ __device__ __forceinline__ Candidate make_candidate(const MarchParams &mp, const
   return c;
 }
 
-// One warp per ray: lanes stride over the K candidates; ballot gives the live mask words.
-__global__ void __launch_bounds__(256) march_count_kernel(MarchParams mp, const uint8_t *bits,
-                                                          const float *__restrict__ origins,
-                                                          const float *__restrict__ dirs,
-                                                          uint32_t *__restrict__ counts,
-                                                          uint32_t *__restrict__ live_mask) {
-  const uint32_t warp = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
-  if (warp >= mp.R) return;
-  const uint32_t r = warp, words = (mp.K + 31) >> 5;
-  float o[3], d[3];
-#pragma unroll
-  for (int a = 0; a < 3; ++a) {
-    o[a] = __ldg(origins + 3 * (size_t)r + a);
-    d[a] = __ldg(dirs + 3 * (size_t)r + a);
-  }
-  const uint32_t hpre = ray_hash_prefix(mp.seed, mp.step, r);
-  uint32_t n = 0;
-  for (uint32_t wd = 0; wd < words; ++wd) {
-    uint32_t k = wd * 32 + lane;
-    bool live = false;
-    if (k < mp.K) live = make_candidate(mp, bits, hpre, o, d, k).live;
-    uint32_t m = __ballot_sync(0xffffffffu, live);
-    if (lane == 0) live_mask[(size_t)r * words + wd] = m;
-    n += __popc(m);
-  }
-  if (lane == 0) counts[r] = n;
-}
+// S1-S3 in ONE launch.  One warp per ray, MARCH_WARPS rays per block.  Pass 1: lanes stride over the
+// K candidates, ballot gives the live-mask words (kept in shared memory) and the ray's count n_r.
+// The exclusive scan over rays is a single-pass chained scan with decoupled look-back: blocks take a
+// ticket (so block order = ray order whatever the hardware's dispatch order is), publish their
+// aggregate, and sum their predecessors' aggregates back to the nearest published inclusive prefix.
+// Pass 2: each live candidate is written at offsets[r] + its rank among the ray's live ones, so the
+// compacted list is in (ray, k) order and bit-identical from run to run.  The last block to finish
+// resets the scan state for the next launch.
+constexpr uint32_t MARCH_WARPS = 16;
+constexpr uint32_t MARCH_MAX_WORDS = 128;        // K <= 4096 (validate_config)
+constexpr uint64_t SCAN_AGG = 1ull << 32, SCAN_INCL = 2ull << 32;
 
-// Exclusive scan of counts[R] -> offsets[R+1] by one block (R <= a few 100 K per call), and
-// reset of the loss accumulators.  Deterministic.
-__global__ void __launch_bounds__(1024) scan_counts_kernel(const uint32_t *__restrict__ counts,
-                                                           uint32_t *__restrict__ offsets, uint32_t R,
-                                                           double *loss_acc, unsigned long long *total, uint32_t *absmax) {
-  __shared__ uint32_t warp_sums[32];
-  __shared__ uint32_t carry_s;
-  const uint32_t tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
-  if (tid == 0) {
-    carry_s = 0;
-    if (loss_acc) { loss_acc[0] = 0.0; loss_acc[1] = 0.0; }
-    if (absmax) *absmax = 0u;
-  }
+__global__ void __launch_bounds__(MARCH_WARPS * 32) march_fused_kernel(MarchParams mp, const uint8_t *bits,
+                                                                       const float *__restrict__ origins,
+                                                                       const float *__restrict__ dirs, Workspace ws,
+                                                                       int count_total) {
+  __shared__ uint32_t masks[MARCH_WARPS][MARCH_MAX_WORDS];
+  __shared__ uint32_t warp_n[MARCH_WARPS];
+  __shared__ uint32_t ticket_s, block_base_s;
+  const uint32_t tid = threadIdx.x, wid = tid >> 5, lane = tid & 31;
+  uint32_t *ticket_ctr = ws.scan_ctr, *done_ctr = ws.scan_ctr + 1;
+  volatile unsigned long long *state = ws.scan_state;
+  if (tid == 0) ticket_s = atomicAdd(ticket_ctr, 1u);
   __syncthreads();
-  for (uint32_t base = 0; base < R; base += 1024) {
-    uint32_t i = base + tid;
-    uint32_t v = i < R ? counts[i] : 0u;
+  const uint32_t ticket = ticket_s;
+  const uint32_t r = ticket * MARCH_WARPS + wid, words = (mp.K + 31) >> 5;
+  float o[3] = {0.f, 0.f, 0.f}, d[3] = {0.f, 0.f, 0.f};
+  uint32_t hpre = 0, n = 0;
+  if (r < mp.R) {
+#pragma unroll
+    for (int a = 0; a < 3; ++a) {
+      o[a] = __ldg(origins + 3 * (size_t)r + a);
+      d[a] = __ldg(dirs + 3 * (size_t)r + a);
+    }
+    hpre = ray_hash_prefix(mp.seed, mp.step, r);
+    for (uint32_t wd = 0; wd < words; ++wd) {
+      const uint32_t k = wd * 32 + lane;
+      bool live = false;
+      if (k < mp.K) live = make_candidate(mp, bits, hpre, o, d, k).live;
+      const uint32_t m = __ballot_sync(0xffffffffu, live);
+      if (lane == 0) masks[wid][wd] = m;
+      n += __popc(m);
+    }
+  }
+  if (lane == 0) warp_n[wid] = n;
+  __syncthreads();
+  if (wid == 0) {
+    // block-local exclusive scan of the MARCH_WARPS counts
+    const uint32_t v = lane < MARCH_WARPS ? warp_n[lane] : 0u;
     uint32_t incl = v;
 #pragma unroll
     for (int s = 1; s < 32; s <<= 1) {
-      uint32_t y = __shfl_up_sync(0xffffffffu, incl, s);
-      if (lane >= s) incl += y;
+      const uint32_t y = __shfl_up_sync(0xffffffffu, incl, s);
+      if (lane >= (uint32_t)s) incl += y;
     }
-    if (lane == 31) warp_sums[wid] = incl;
-    __syncthreads();
-    if (wid == 0) {
-      uint32_t ws = warp_sums[lane], wi = ws;
+    if (lane < MARCH_WARPS) warp_n[lane] = incl - v;
+    const uint32_t total = __shfl_sync(0xffffffffu, incl, 31);
+    // publish, then look back
+    if (lane == 0) atomicExch((unsigned long long *)&state[ticket], (ticket == 0 ? SCAN_INCL : SCAN_AGG) | total);
+    uint32_t excl = 0;
+    int64_t top = (int64_t)ticket - 1;       // nearest predecessor not yet summed
+    while (top >= 0) {
+      const int64_t idx = top - lane;
+      unsigned long long st = SCAN_INCL;     // lanes before ticket 0 count as "inclusive prefix 0"
+      if (idx >= 0) do { st = state[idx]; } while ((st >> 32) == 0);
+      const uint32_t is_incl = __ballot_sync(0xffffffffu, (st >> 32) == 2);
+      const uint32_t first = is_incl ? (uint32_t)__ffs(is_incl) - 1 : 31u;
+      uint32_t val = lane <= first ? (uint32_t)st : 0u;
 #pragma unroll
-      for (int s = 1; s < 32; s <<= 1) {
-        uint32_t y = __shfl_up_sync(0xffffffffu, wi, s);
-        if (lane >= s) wi += y;
+      for (int s = 16; s > 0; s >>= 1) val += __shfl_xor_sync(0xffffffffu, val, s);
+      excl += val;
+      if (is_incl) break;
+      top -= 32;
+    }
+    if (lane == 0) {
+      if (ticket != 0) atomicExch((unsigned long long *)&state[ticket], SCAN_INCL | (unsigned long long)(excl + total));
+      block_base_s = excl;
+      if (ticket == gridDim.x - 1) {
+        ws.offsets[mp.R] = excl + total;
+        if (count_total) *ws.total_samples += excl + total;
       }
-      warp_sums[lane] = wi - ws;  // exclusive warp offsets
+      if (ticket == 0) {
+        ws.loss_acc[0] = 0.0; ws.loss_acc[1] = 0.0;
+        *ws.grad_absmax = 0u;
+      }
     }
-    __syncthreads();
-    uint32_t carry = carry_s;
-    uint32_t excl = carry + warp_sums[wid] + incl - v;
-    if (i < R) offsets[i] = excl;
-    __syncthreads();
-    if (tid == 1023) carry_s = excl + v;
-    __syncthreads();
   }
+  __syncthreads();
+  if (r < mp.R) {
+    uint32_t base = block_base_s + warp_n[wid];
+    if (lane == 0) { ws.offsets[r] = base; ws.counts[r] = n; }
+    for (uint32_t wd = 0; wd < words; ++wd) {
+      const uint32_t m = masks[wid][wd];
+      if ((m >> lane) & 1u) {
+        const uint32_t k = wd * 32 + lane;
+        const Candidate c = make_candidate(mp, nullptr, hpre, o, d, k);
+        const uint64_t s = (uint64_t)base + __popc(m & ((1u << lane) - 1u));
+        ws.s_ray[s] = r;
+        ws.s_k[s] = k;
+        ws.s_t[s] = c.t;
+        ws.s_delta[s] = c.delta;
+        ws.s_x[s] = c.x[0];
+        ws.s_x[ws.cap + s] = c.x[1];
+        ws.s_x[2 * ws.cap + s] = c.x[2];
+      }
+      base += __popc(m);
+    }
+  }
+  // the last block to get here has seen every look-back finish: reset the scan state
+  __syncthreads();
   if (tid == 0) {
-    offsets[R] = carry_s;
-    if (total) *total += carry_s;
-  }
-}
-
-// Second pass: each live candidate is written at offsets[r] + its rank among the ray's live ones.
-__global__ void __launch_bounds__(256) march_write_kernel(MarchParams mp, const uint8_t *bits,
-                                                          const float *__restrict__ origins,
-                                                          const float *__restrict__ dirs,
-                                                          const uint32_t *__restrict__ offsets,
-                                                          const uint32_t *__restrict__ live_mask,
-                                                          Workspace ws) {
-  const uint32_t warp = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
-  if (warp >= mp.R) return;
-  const uint32_t r = warp, words = (mp.K + 31) >> 5;
-  float o[3], d[3];
-#pragma unroll
-  for (int a = 0; a < 3; ++a) {
-    o[a] = __ldg(origins + 3 * (size_t)r + a);
-    d[a] = __ldg(dirs + 3 * (size_t)r + a);
-  }
-  const uint32_t hpre = ray_hash_prefix(mp.seed, mp.step, r);
-  uint32_t base = offsets[r];
-  for (uint32_t wd = 0; wd < words; ++wd) {
-    uint32_t m = live_mask[(size_t)r * words + wd];
-    if ((m >> lane) & 1u) {
-      uint32_t k = wd * 32 + lane;
-      Candidate c = make_candidate(mp, nullptr, hpre, o, d, k);
-      uint64_t s = (uint64_t)base + __popc(m & ((1u << lane) - 1u));
-      ws.s_ray[s] = r;
-      ws.s_k[s] = k;
-      ws.s_t[s] = c.t;
-      ws.s_delta[s] = c.delta;
-      ws.s_x[s] = c.x[0];
-      ws.s_x[ws.cap + s] = c.x[1];
-      ws.s_x[2 * ws.cap + s] = c.x[2];
+    __threadfence();
+    if (atomicAdd(done_ctr, 1u) == gridDim.x - 1) {
+      for (uint32_t i = 0; i < gridDim.x; ++i) state[i] = 0ull;
+      *ticket_ctr = 0u;
+      *done_ctr = 0u;
+      __threadfence();
     }
-    base += __popc(m);
   }
 }
 
@@ -212,25 +221,14 @@ __global__ void occ_threshold_kernel(uint64_t first_cell, uint64_t n_cells,
 
 }  // namespace
 
-int launch_march_count(const MarchParams &mp, const uint8_t *bits, const float *origins, const float *dirs,
-                       const Workspace &ws, cudaStream_t st) {
-  dim3 grid((mp.R + 7) / 8), block(256);
-  march_count_kernel<<<grid, block, 0, st>>>(mp, bits, origins, dirs, ws.counts, ws.live_mask);
+int launch_march(const MarchParams &mp, const uint8_t *bits, const float *origins, const float *dirs,
+                 const Workspace &ws, int count_total, cudaStream_t st) {
+  dim3 grid((mp.R + MARCH_WARPS - 1) / MARCH_WARPS), block(MARCH_WARPS * 32);
+  march_fused_kernel<<<grid, block, 0, st>>>(mp, bits, origins, dirs, ws, count_total);
   return 1;
 }
 
-int launch_scan(const MarchParams &mp, const Workspace &ws, int count_total, cudaStream_t st) {
-  scan_counts_kernel<<<1, 1024, 0, st>>>(ws.counts, ws.offsets, mp.R, ws.loss_acc,
-                                         count_total ? ws.total_samples : nullptr, ws.grad_absmax);
-  return 1;
-}
-
-int launch_march_write(const MarchParams &mp, const float *origins, const float *dirs, const Workspace &ws,
-                       cudaStream_t st) {
-  dim3 grid((mp.R + 7) / 8), block(256);
-  march_write_kernel<<<grid, block, 0, st>>>(mp, nullptr, origins, dirs, ws.offsets, ws.live_mask, ws);
-  return 1;
-}
+uint32_t march_scan_state_entries(uint32_t max_rays) { return (max_rays + MARCH_WARPS - 1) / MARCH_WARPS; }
 
 int launch_occ_cells(uint32_t G, uint64_t first_cell, uint64_t n_cells, const Workspace &ws,
                      uint32_t *d_S, cudaStream_t st) {

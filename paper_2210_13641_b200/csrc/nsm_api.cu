@@ -37,7 +37,7 @@ nsm_status fail(nsm_status st, const char *fmt, ...) {
 
 }  // namespace
 
-static const char *kKernelNames[K_COUNT] = {"march_count", "scan", "march_write", "encode", "mlp_fwd", "composite",
+static const char *kKernelNames[K_COUNT] = {"march", "encode", "mlp_fwd", "composite",
                                             "mlp_bwd", "scatter", "adam_table", "adam_mlp", "occupancy", "debug"};
 
 // Optional per-kernel CUDA-event timing (bench.py's roofline leg).  When enabled every launch is
@@ -210,9 +210,7 @@ MarchParams make_march(const nsm_field *f, const nsm_ray_batch *b, uint32_t R, b
 void enqueue_forward(nsm_field *f, const nsm_ray_batch *b, uint32_t R, bool jitter, uint32_t step, bool train) {
   const uint32_t *d_S = f->ws.offsets + R;
   MarchParams mp = make_march(f, b, R, jitter, step);
-  RUN(f, K_MARCH_COUNT, launch_march_count(mp, f->occ_full ? nullptr : f->fp.occ_bits, b->origins, b->dirs, f->ws, f->stream));
-  RUN(f, K_SCAN, launch_scan(mp, f->ws, train ? 1 : 0, f->stream));
-  RUN(f, K_MARCH_WRITE, launch_march_write(mp, b->origins, b->dirs, f->ws, f->stream));
+  RUN(f, K_MARCH, launch_march(mp, f->occ_full ? nullptr : f->fp.occ_bits, b->origins, b->dirs, f->ws, train ? 1 : 0, f->stream));
   const int bf16 = f->cfg.mlp_precision == NSM_MLP_BF16;
   RUN(f, K_ENCODE, launch_encode(f->lv, f->fp.rec, f->ws, d_S, f->use_tc ? 1 + bf16 : 0, f->n_sms, f->stream));
   if (f->use_tc)
@@ -229,9 +227,8 @@ void repack_weights(nsm_field *f) {
 
 nsm_status clear_grads_if_dirty(nsm_field *f) {
   if (f->grads_dirty) {
-    RUN(f, K_DEBUG, launch_pack_records(f->fp, 1, nullptr, f->stream));
+    RUN(f, K_DEBUG, launch_set_grad(f->fp, nullptr, nullptr, f->stream));
     CUDA_TRY(cudaMemsetAsync(f->fp.mlp_grad, 0, sizeof(float) * f->fp.n_mlp, f->stream));
-    CUDA_TRY(cudaMemsetAsync(f->fp.touched, 0, f->fp.n_entries, f->stream));
     f->grads_dirty = false;
   }
   return NSM_OK;
@@ -250,7 +247,7 @@ nsm_status enqueue_backward(nsm_field *f, const nsm_ray_batch *b, float lambda_d
   else
     RUN(f, K_MLP_BWD, launch_mlp_backward_simt(f->ms, f->fp.mlp_theta, f->fp.mlp_grad, b->dirs,
                                                f->ws, d_S, f->n_sms, f->stream));
-  RUN(f, K_SCATTER, launch_scatter(f->lv, f->fp.rec, f->fp.touched, f->ws, d_S, f->n_sms, f->stream));
+  RUN(f, K_SCATTER, launch_scatter(f->lv, f->fp.grad, f->ws, d_S, f->n_sms, f->stream));
   f->grads_dirty = true;
   f->last_R = R;
   f->last_K = b->n_candidates;
@@ -376,13 +373,13 @@ nsm_status nsm_create_field(const nsm_field_config *cfg, void *cuda_stream, nsm_
   ws.cap = cap;
   ws.max_rays = cfg->max_rays;
   const uint64_t G3 = (uint64_t)cfg->occ_res * cfg->occ_res * cfg->occ_res;
-  const uint32_t R = cfg->max_rays, words = (cfg->max_candidates + 31) / 32;
+  const uint32_t R = cfg->max_rays;
   cudaError_t e = cudaSuccess;
   auto A = [&](cudaError_t r) { if (e == cudaSuccess) e = r; };
   A(f->alloc(&fp.rec, 4 * fp.n_table));
   A(f->alloc(&fp.mlp_theta, fp.n_mlp)); A(f->alloc(&fp.mlp_m, fp.n_mlp)); A(f->alloc(&fp.mlp_v, fp.n_mlp)); A(f->alloc(&fp.mlp_grad, fp.n_mlp));
-  A(f->alloc(&fp.touched, fp.n_entries)); A(f->alloc(&fp.occ_bits, (G3 + 7) / 8 + 4));
-  A(f->alloc(&ws.counts, R)); A(f->alloc(&ws.offsets, R + 1)); A(f->alloc(&ws.live_mask, (size_t)R * words));
+  A(f->alloc(&fp.grad, fp.n_table, false)); A(f->alloc(&fp.occ_bits, (G3 + 7) / 8 + 4));
+  A(f->alloc(&ws.counts, R)); A(f->alloc(&ws.offsets, R + 1)); A(f->alloc(&ws.scan_state, march_scan_state_entries(R) + 1)); A(f->alloc(&ws.scan_ctr, 2));
   A(f->alloc(&ws.C, 3 * (size_t)R)); A(f->alloc(&ws.D_hat, R)); A(f->alloc(&ws.O, R));
   A(f->alloc(&ws.s_ray, cap)); A(f->alloc(&ws.s_k, cap)); A(f->alloc(&ws.s_t, cap)); A(f->alloc(&ws.s_delta, cap));
   A(f->alloc(&ws.s_x, 3 * cap));
@@ -406,6 +403,7 @@ nsm_status nsm_create_field(const nsm_field_config *cfg, void *cuda_stream, nsm_
     cudaGetLastError();
     return fail(e == cudaErrorMemoryAllocation ? NSM_ERR_OOM : NSM_ERR_CUDA, "allocation failed: %s", cudaGetErrorString(e));
   }
+  RUN(f, K_DEBUG, launch_set_grad(f->fp, nullptr, nullptr, f->stream));   // every gradient word = "untouched"
   repack_weights(f);
   *out = f;
   return NSM_OK;
@@ -586,11 +584,9 @@ nsm_status nsm_train_step_host(nsm_field *f, const nsm_ray_batch *hb, float lamb
 
 nsm_status nsm_debug_set_grad(nsm_field *f, const float *d_grad, const uint8_t *d_touched) {
   if (!f) return fail(NSM_ERR_INVALID_ARG, "field is NULL");
-  if (d_grad) {
-    RUN(f, K_DEBUG, launch_pack_records(f->fp, 1, d_grad, f->stream));
-    CUDA_TRY(cudaMemcpyAsync(f->fp.mlp_grad, d_grad + f->fp.n_table, sizeof(float) * f->fp.n_mlp, cudaMemcpyDeviceToDevice, f->stream));
-  }
-  if (d_touched) CUDA_TRY(cudaMemcpyAsync(f->fp.touched, d_touched, f->fp.n_entries, cudaMemcpyDeviceToDevice, f->stream));
+  if (!d_grad) return fail(NSM_ERR_INVALID_ARG, "d_grad is NULL");
+  RUN(f, K_DEBUG, launch_set_grad(f->fp, d_grad, d_touched, f->stream));
+  CUDA_TRY(cudaMemcpyAsync(f->fp.mlp_grad, d_grad + f->fp.n_table, sizeof(float) * f->fp.n_mlp, cudaMemcpyDeviceToDevice, f->stream));
   f->grads_dirty = true;
   return NSM_OK;
 }
@@ -668,7 +664,7 @@ nsm_status nsm_debug_last_step(nsm_field *f, int item, void *d_out, uint64_t cap
     case NSM_DBG_DSIGMA: src = ws.dsigma; bytes = 4ull * S; break;
     case NSM_DBG_DRGB: src = ws.drgb; bytes = 12ull * S; break;
     case NSM_DBG_GRAD: bytes = 4ull * (f->fp.n_table + f->fp.n_mlp); break;
-    case NSM_DBG_TOUCHED: src = f->fp.touched; bytes = f->fp.n_entries; break;
+    case NSM_DBG_TOUCHED: bytes = f->fp.n_entries; break;
     case NSM_DBG_SAMPLE_X: bytes = 12ull * S; break;
     case NSM_DBG_E: bytes = 4ull * S * f->ms.LF; break;
     case NSM_DBG_SLOTS: bytes = 4ull * S * L * 8; break;
@@ -683,8 +679,10 @@ nsm_status nsm_debug_last_step(nsm_field *f, int item, void *d_out, uint64_t cap
   if (bytes == 0) return NSM_OK;
   if (src) {
     CUDA_TRY(cudaMemcpyAsync(d_out, src, bytes, cudaMemcpyDeviceToDevice, f->stream));
+  } else if (item == NSM_DBG_TOUCHED) {
+    RUN(f, K_DEBUG, launch_get_touched(f->fp, (uint8_t *)d_out, f->stream));
   } else if (item == NSM_DBG_GRAD) {
-    RUN(f, K_DEBUG, launch_unpack_records(f->fp, 1, (float *)d_out, f->stream));
+    CUDA_TRY(cudaMemcpyAsync(d_out, f->fp.grad, sizeof(float) * f->fp.n_table, cudaMemcpyDeviceToDevice, f->stream));
     CUDA_TRY(cudaMemcpyAsync((float *)d_out + f->fp.n_table, f->fp.mlp_grad, sizeof(float) * f->fp.n_mlp, cudaMemcpyDeviceToDevice, f->stream));
   } else if (item == NSM_DBG_SAMPLE_X) {
     RUN(f, K_DEBUG, launch_planes_to_rows(ws.s_x, ws.cap, 3, d_S, (float *)d_out, f->stream));

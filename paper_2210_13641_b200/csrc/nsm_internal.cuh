@@ -41,7 +41,8 @@ struct Workspace {
   // rays
   uint32_t *counts;      // [R]
   uint32_t *offsets;     // [R+1]; offsets[R] = S
-  uint32_t *live_mask;   // [R, ceil(K/32)]
+  unsigned long long *scan_state;  // chained-scan status words of the fused marcher, one per block; zero between launches
+  uint32_t *scan_ctr;    // [0] ticket counter, [1] finished-block counter; zero between launches
   float *C, *D_hat, *O;  // [R,3], [R], [R]
   // samples
   uint32_t *s_ray, *s_k; // [cap]
@@ -68,37 +69,50 @@ struct Workspace {
 
 // Kernel classes, for launch counting and the optional per-kernel event timing.
 enum KernelId {
-  K_MARCH_COUNT = 0, K_SCAN, K_MARCH_WRITE, K_ENCODE, K_MLP_FWD, K_COMPOSITE, K_MLP_BWD, K_SCATTER,
+  K_MARCH = 0, K_ENCODE, K_MLP_FWD, K_COMPOSITE, K_MLP_BWD, K_SCATTER,
   K_ADAM_TABLE, K_ADAM_MLP, K_OCC, K_DEBUG, K_COUNT
 };
 
-// Parameters.  Hash-table entries are stored as RECORDS: entry e owns 4F consecutive floats
-//   rec[e*4F + 0F .. 1F) = theta   rec[.. 1F..2F) = gradient   rec[.. 2F..3F) = Adam m   rec[.. 3F..4F) = Adam v
-// so that with F = 2 an entry is exactly one 32-byte DRAM/L2 sector: the gather (theta), the
-// scatter (gradient) and the touched-only Adam update (all four) of one entry hit the SAME sector,
-// which the step's first access brings into the 126 MB L2 and the later ones find there.  The
-// canonical flat layout of include/nsm.h exists only at the boundary (pack/unpack kernels).
+// Parameters.  Hash-table entries are stored as RECORDS of 4F floats,
+//   rec[e*4F + 0F .. 1F) = theta   rec[.. 1F..2F) = spare   rec[.. 2F..3F) = Adam m   rec[.. 3F..4F) = Adam v
+// so that with F = 2 an entry is exactly one 32-byte DRAM/L2 sector: the touched-only Adam update
+// (a random 25 % of the entries per step at config 2) moves one sector per entry.  The GRADIENT is
+// a separate, compact array grad[e*F + f] (48.8 MB at config 2, L2-sized): the scatter's vector
+// reductions land in a table that fits the cache instead of one four times its size, and Adam
+// reads it as a dense coalesced stream.
+//
+// Touched set without flags: between steps every gradient word holds -0.0f (bits 0x80000000).
+// The scatter never adds -0.0 or a magnitude below 2^-96 (those addends become +0.0), and under
+// round-to-nearest a sum of such addends is +0.0, or a multiple of 2^-119 >= FLT_MIN in magnitude;
+// it is never -0.0 (x + (-x) = +0.0) and never a subnormal that the reduction unit could flush to
+// -0.0.  Hence "entry e was referenced this step"  <=>  bits(grad[e*F]) != 0x80000000, whatever the
+// gradient's value (the touched set is structural, S12); Adam writes -0.0f back.
+// The canonical flat layout of include/nsm.h exists only at the boundary (pack/unpack kernels).
+#define NSM_GRAD_UNTOUCHED 0x80000000u
+#define NSM_GRAD_MIN_ADDEND 1.262177448e-29f   /* 2^-96 */
 struct FieldParams {
   float *rec;                                       // [n_entries][4F]
+  float *grad;                                      // [n_entries][F]
   float *mlp_theta, *mlp_m, *mlp_v, *mlp_grad;      // [n_mlp] each, canonical order
-  uint8_t *touched;                                 // [n_entries]
   uint8_t *occ_bits;                                // [G^3/8]
   uint64_t n_entries, n_table, n_mlp;
   uint32_t F;
 };
 
 // ---- launchers (each enqueues on `st`, returns the number of kernels launched) ----
-int launch_march_count(const MarchParams &mp, const uint8_t *bits, const float *origins, const float *dirs,
-                       const Workspace &ws, cudaStream_t st);
-int launch_scan(const MarchParams &mp, const Workspace &ws, int count_total, cudaStream_t st);
-int launch_march_write(const MarchParams &mp, const float *origins, const float *dirs, const Workspace &ws,
-                       cudaStream_t st);
+// S1-S3 in one launch; also resets the loss accumulators and (count_total) adds S to the running sample count
+int launch_march(const MarchParams &mp, const uint8_t *bits, const float *origins, const float *dirs,
+                 const Workspace &ws, int count_total, cudaStream_t st);
+uint32_t march_scan_state_entries(uint32_t max_rays);
 // out_mode: 0 = fp32 planes ws.e, 1 = fp16 blob ws.blob_e, 2 = bf16 blob ws.blob_e
 int launch_encode(const LevelTable &lv, const float *rec, const Workspace &ws,
                   const uint32_t *d_S, int out_mode, int n_sms, cudaStream_t st);
-int launch_scatter(const LevelTable &lv, float *rec, uint8_t *touched, const Workspace &ws,
+int launch_scatter(const LevelTable &lv, float *grad, const Workspace &ws,
                    const uint32_t *d_S, int n_sms, cudaStream_t st);
-// canonical [n_entries][F] <-> field `which` (0 theta, 1 grad, 2 m, 3 v) of the records; src == nullptr packs zeros
+// gradient array <- canonical gradient + touched flags (NULL: every entry touched); src == nullptr: all untouched
+int launch_set_grad(const FieldParams &fp, const float *src, const uint8_t *touched, cudaStream_t st);
+int launch_get_touched(const FieldParams &fp, uint8_t *dst, cudaStream_t st);
+// canonical [n_entries][F] <-> field `which` (0 theta, 2 m, 3 v) of the records; src == nullptr packs zeros
 int launch_pack_records(const FieldParams &fp, int which, const float *src, cudaStream_t st);
 int launch_unpack_records(const FieldParams &fp, int which, float *dst, cudaStream_t st);
 int launch_mlp_forward_simt(const MlpShape &ms, const float *theta_mlp, const float *dirs,
