@@ -7,103 +7,134 @@
 
 namespace {
 
-struct AdamConst {
-  float lr, b1, b2, eps, inv_bc1, inv_bc2;
-};
+// One block per chunk of ADAM_CHUNK_FLOATS / F consecutive entries, two phases.
+//  1. The chunk's gradient words are read densely (coalesced 16-byte loads, four independent ones
+//     per thread; the array is L2-hot, the scatter has just written it).  Entries whose first word
+//     is not -0.0f (FieldParams: "referenced this step") are compacted into shared memory
+//     (index + gradient), warp-aggregated.
+//  2. The block walks the compact list: every thread has a touched entry, loads its record
+//     (theta | spare | m | v; one 32-byte sector for F = 2; two entries in flight per thread),
+//     updates and stores it.  The whole gradient chunk is then reset to -0.0f with coalesced
+//     stores, so the next step's scatter starts from "untouched" without a separate pass.
+// sparse = 0 (dense Adam, textbook): every entry goes through phase 2.
+constexpr int ADAM_CHUNK_FLOATS = 4096;
+constexpr int ADAM_THREADS = 256;
 
-__device__ __forceinline__ void adam_one(float &th, float &m, float &v, float g, const AdamConst &c) {
-  m = c.b1 * m + (1.f - c.b1) * g;
-  v = c.b2 * v + (1.f - c.b2) * g * g;
-  float mhat = m * c.inv_bc1, vhat = v * c.inv_bc2;
-  th = th - c.lr * mhat / (sqrtf(vhat) + c.eps);
-}
-
-// One thread per B consecutive entries (B*F = 4 gradient floats = one coalesced 16-byte load, two
-// for F = 8).  The gradient array is read densely (it is L2-hot: the scatter has just written it);
-// only the records of touched entries (bits(g) != -0.0f, see FieldParams) are loaded, updated and
-// stored, and their gradient words are reset to -0.0f, so the next step's scatter starts from
-// "untouched" without a separate clearing pass.
 template <int F>
-__global__ void __launch_bounds__(256) adam_table_kernel(float *__restrict__ rec, float *__restrict__ grad,
-                                                         uint64_t n_entries, int sparse, AdamConst c) {
-  constexpr int B = F >= 4 ? 1 : 4 / F;
-  constexpr int NV = B * F / 4;        // float4 loads of gradient per thread
-  const uint64_t q = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
-  const uint64_t e0 = q * B;
-  if (e0 >= n_entries) return;
-  float g[B * F];
-  if (e0 + B <= n_entries) {
-    const float4 *g4 = reinterpret_cast<const float4 *>(grad + e0 * F);
-#pragma unroll
-    for (int i = 0; i < NV; ++i) {
-      const float4 t = g4[i];
-      g[4 * i] = t.x; g[4 * i + 1] = t.y; g[4 * i + 2] = t.z; g[4 * i + 3] = t.w;
-    }
+__device__ __forceinline__ void adam_record(float *__restrict__ r, const float *g, const AdamConst &c) {
+  float th[F], m[F], v[F];
+  if constexpr (F == 1) {
+    const float4 t = *reinterpret_cast<const float4 *>(r);
+    th[0] = t.x; m[0] = t.z; v[0] = t.w;
+  } else if constexpr (F == 2) {
+    const float4 a = *reinterpret_cast<const float4 *>(r), b = *reinterpret_cast<const float4 *>(r + 4);
+    th[0] = a.x; th[1] = a.y; m[0] = b.x; m[1] = b.y; v[0] = b.z; v[1] = b.w;
   } else {
 #pragma unroll
-    for (int i = 0; i < B * F; ++i) g[i] = (e0 * F + i < n_entries * F) ? grad[e0 * F + i] : __uint_as_float(NSM_GRAD_UNTOUCHED);
+    for (int i = 0; i < F / 4; ++i) {
+      const float4 a = *reinterpret_cast<const float4 *>(r + 4 * i), b = *reinterpret_cast<const float4 *>(r + 2 * F + 4 * i),
+                   d = *reinterpret_cast<const float4 *>(r + 3 * F + 4 * i);
+      th[4 * i] = a.x; th[4 * i + 1] = a.y; th[4 * i + 2] = a.z; th[4 * i + 3] = a.w;
+      m[4 * i] = b.x; m[4 * i + 1] = b.y; m[4 * i + 2] = b.z; m[4 * i + 3] = b.w;
+      v[4 * i] = d.x; v[4 * i + 1] = d.y; v[4 * i + 2] = d.z; v[4 * i + 3] = d.w;
+    }
   }
-  bool act[B];
-  float th[B][F], m[B][F], v[B][F];
 #pragma unroll
-  for (int j = 0; j < B; ++j) {
-    act[j] = (e0 + j < n_entries) && (!sparse || __float_as_uint(g[j * F]) != NSM_GRAD_UNTOUCHED);
-    if (act[j]) {
-      const float *r = rec + (e0 + j) * 4 * F;
-      if constexpr (F == 1) {
-        const float4 t = *reinterpret_cast<const float4 *>(r);
-        th[j][0] = t.x; m[j][0] = t.z; v[j][0] = t.w;
-      } else if constexpr (F == 2) {
-        const float4 a = *reinterpret_cast<const float4 *>(r), b = *reinterpret_cast<const float4 *>(r + 4);
-        th[j][0] = a.x; th[j][1] = a.y; m[j][0] = b.x; m[j][1] = b.y; v[j][0] = b.z; v[j][1] = b.w;
-      } else {
+  for (int f = 0; f < F; ++f) adam_one(th[f], m[f], v[f], g[f], c);
+  if constexpr (F == 1) {
+    r[0] = th[0];
+    *reinterpret_cast<float2 *>(r + 2) = make_float2(m[0], v[0]);
+  } else if constexpr (F == 2) {
+    *reinterpret_cast<float2 *>(r) = make_float2(th[0], th[1]);
+    *reinterpret_cast<float4 *>(r + 4) = make_float4(m[0], m[1], v[0], v[1]);
+  } else {
 #pragma unroll
-        for (int i = 0; i < F / 4; ++i) {
-          const float4 a = *reinterpret_cast<const float4 *>(r + 4 * i), b = *reinterpret_cast<const float4 *>(r + 2 * F + 4 * i),
-                       d = *reinterpret_cast<const float4 *>(r + 3 * F + 4 * i);
-          th[j][4 * i] = a.x; th[j][4 * i + 1] = a.y; th[j][4 * i + 2] = a.z; th[j][4 * i + 3] = a.w;
-          m[j][4 * i] = b.x; m[j][4 * i + 1] = b.y; m[j][4 * i + 2] = b.z; m[j][4 * i + 3] = b.w;
-          v[j][4 * i] = d.x; v[j][4 * i + 1] = d.y; v[j][4 * i + 2] = d.z; v[j][4 * i + 3] = d.w;
+    for (int i = 0; i < F / 4; ++i) {
+      *reinterpret_cast<float4 *>(r + 4 * i) = make_float4(th[4 * i], th[4 * i + 1], th[4 * i + 2], th[4 * i + 3]);
+      *reinterpret_cast<float4 *>(r + 2 * F + 4 * i) = make_float4(m[4 * i], m[4 * i + 1], m[4 * i + 2], m[4 * i + 3]);
+      *reinterpret_cast<float4 *>(r + 3 * F + 4 * i) = make_float4(v[4 * i], v[4 * i + 1], v[4 * i + 2], v[4 * i + 3]);
+    }
+  }
+}
+
+template <int F>
+__global__ void __launch_bounds__(ADAM_THREADS) adam_table_kernel(float *__restrict__ rec, float *__restrict__ grad,
+                                                                  uint64_t n_entries, int sparse, AdamConst c) {
+  constexpr int CH = ADAM_CHUNK_FLOATS / F;            // entries per chunk
+  constexpr int NV = ADAM_CHUNK_FLOATS / 4 / ADAM_THREADS;   // float4 loads per thread
+  __shared__ float list_g[ADAM_CHUNK_FLOATS];          // compacted gradients, F floats per touched entry
+  __shared__ uint16_t list_e[CH];                      // compacted local entry indices
+  __shared__ uint32_t cnt;
+  const uint32_t tid = threadIdx.x, lane = tid & 31;
+  const uint64_t e_base = (uint64_t)blockIdx.x * CH;
+  const uint64_t n_float = n_entries * F;
+  const float4 *g4 = reinterpret_cast<const float4 *>(grad + e_base * F);
+  if (tid == 0) cnt = 0;
+  float4 gv[NV];
+#pragma unroll
+  for (int j = 0; j < NV; ++j) {
+    const uint32_t q = j * ADAM_THREADS + tid;         // float4 index inside the chunk
+    gv[j] = (e_base * F + 4ull * q < n_float) ? g4[q] : make_float4(0.f, 0.f, 0.f, 0.f);   // the array is padded to 256 B
+  }
+  __syncthreads();
+#pragma unroll
+  for (int j = 0; j < NV; ++j) {
+    const uint32_t q = j * ADAM_THREADS + tid;
+    const float w[4] = {gv[j].x, gv[j].y, gv[j].z, gv[j].w};
+    if constexpr (F <= 4) {
+      constexpr int EPV = 4 / F;                       // entries per float4
+#pragma unroll
+      for (int i = 0; i < EPV; ++i) {
+        const uint32_t le = q * EPV + i;               // local entry index
+        const bool t = (e_base + le < n_entries) && (!sparse || __float_as_uint(w[i * F]) != NSM_GRAD_UNTOUCHED);
+        const uint32_t mk = __ballot_sync(0xffffffffu, t);
+        uint32_t base = 0;
+        if (lane == 0 && mk) base = atomicAdd(&cnt, (uint32_t)__popc(mk));
+        base = __shfl_sync(0xffffffffu, base, 0);
+        if (t) {
+          const uint32_t pos = base + __popc(mk & ((1u << lane) - 1u));
+          list_e[pos] = (uint16_t)le;
+#pragma unroll
+          for (int f = 0; f < F; ++f) list_g[pos * F + f] = w[i * F + f];
         }
       }
-    }
-  }
-  bool any = false;
+    } else {                                           // F = 8: an entry spans two float4 (q even: first half)
+      const uint32_t le = q >> 1;
+      const uint32_t first_word = __float_as_uint(__shfl_sync(0xffffffffu, w[0], lane & ~1u));
+      const bool t = (e_base + le < n_entries) && (!sparse || first_word != NSM_GRAD_UNTOUCHED);
+      const uint32_t mk = __ballot_sync(0xffffffffu, t && !(lane & 1u));
+      uint32_t base = 0;
+      if (lane == 0 && mk) base = atomicAdd(&cnt, (uint32_t)__popc(mk));
+      base = __shfl_sync(0xffffffffu, base, 0);
+      if (t) {
+        const uint32_t pos = base + __popc(mk & ((1u << (lane & ~1u)) - 1u));
+        if (!(lane & 1u)) list_e[pos] = (uint16_t)le;
 #pragma unroll
-  for (int j = 0; j < B; ++j) {
-    if (!act[j]) continue;
-    any = true;
-#pragma unroll
-    for (int f = 0; f < F; ++f) {
-      adam_one(th[j][f], m[j][f], v[j][f], g[j * F + f], c);
-      g[j * F + f] = __uint_as_float(NSM_GRAD_UNTOUCHED);   // the gradient is consumed
-    }
-    float *r = rec + (e0 + j) * 4 * F;
-    if constexpr (F == 1) {
-      r[0] = th[j][0];
-      *reinterpret_cast<float2 *>(r + 2) = make_float2(m[j][0], v[j][0]);
-    } else if constexpr (F == 2) {
-      *reinterpret_cast<float2 *>(r) = make_float2(th[j][0], th[j][1]);
-      *reinterpret_cast<float4 *>(r + 4) = make_float4(m[j][0], m[j][1], v[j][0], v[j][1]);
-    } else {
-#pragma unroll
-      for (int i = 0; i < F / 4; ++i) {
-        *reinterpret_cast<float4 *>(r + 4 * i) = make_float4(th[j][4 * i], th[j][4 * i + 1], th[j][4 * i + 2], th[j][4 * i + 3]);
-        *reinterpret_cast<float4 *>(r + 2 * F + 4 * i) = make_float4(m[j][4 * i], m[j][4 * i + 1], m[j][4 * i + 2], m[j][4 * i + 3]);
-        *reinterpret_cast<float4 *>(r + 3 * F + 4 * i) = make_float4(v[j][4 * i], v[j][4 * i + 1], v[j][4 * i + 2], v[j][4 * i + 3]);
+        for (int f = 0; f < 4; ++f) list_g[pos * F + (lane & 1u) * 4 + f] = w[f];
       }
     }
   }
-  if (any) {
-    if (e0 + B <= n_entries) {
-      float4 *g4 = reinterpret_cast<float4 *>(grad + e0 * F);
-#pragma unroll
-      for (int i = 0; i < NV; ++i) g4[i] = make_float4(g[4 * i], g[4 * i + 1], g[4 * i + 2], g[4 * i + 3]);
-    } else {
-#pragma unroll
-      for (int i = 0; i < B * F; ++i)
-        if (e0 * F + i < n_entries * F) grad[e0 * F + i] = g[i];
+  __syncthreads();
+  const uint32_t n = cnt;
+  if (n == 0) return;
+  // phase 2: two records in flight per thread
+  for (uint32_t i0 = tid; i0 < n; i0 += 2 * ADAM_THREADS) {
+    const uint32_t i1 = i0 + ADAM_THREADS;
+    float *r0 = rec + (e_base + list_e[i0]) * 4 * F;
+    float *r1 = rec + (e_base + list_e[i1 < n ? i1 : i0]) * 4 * F;
+    if constexpr (F == 2) {   // touch the second record's sector early
+      asm volatile("prefetch.global.L2 [%0];" ::"l"(r1));
     }
+    adam_record<F>(r0, list_g + i0 * F, c);
+    if (i1 < n) adam_record<F>(r1, list_g + i1 * F, c);
+  }
+  // reset the chunk's gradient words
+  float4 *o4 = reinterpret_cast<float4 *>(grad + e_base * F);
+  const float nz = __uint_as_float(NSM_GRAD_UNTOUCHED);
+#pragma unroll
+  for (int j = 0; j < NV; ++j) {
+    const uint32_t q = j * ADAM_THREADS + tid;
+    if (e_base * F + 4ull * q < n_float) o4[q] = make_float4(nz, nz, nz, nz);
   }
 }
 
@@ -122,9 +153,8 @@ int launch_adam_table(const FieldParams &fp, uint32_t F, int sparse, float lr, f
                       float inv_bc1, float inv_bc2, int n_sms, cudaStream_t st) {
   (void)n_sms;
   AdamConst c{lr, beta1, beta2, eps, inv_bc1, inv_bc2};
-  const uint64_t per_thread = F >= 4 ? 1 : 4 / F;
-  const uint64_t n_threads = (fp.n_entries + per_thread - 1) / per_thread;
-  dim3 grid((unsigned)((n_threads + 255) / 256)), block(256);
+  const uint64_t chunk = ADAM_CHUNK_FLOATS / F;
+  dim3 grid((unsigned)((fp.n_entries + chunk - 1) / chunk)), block(ADAM_THREADS);
   switch (F) {
     case 1: adam_table_kernel<1><<<grid, block, 0, st>>>(fp.rec, fp.grad, fp.n_entries, sparse, c); break;
     case 2: adam_table_kernel<2><<<grid, block, 0, st>>>(fp.rec, fp.grad, fp.n_entries, sparse, c); break;

@@ -92,7 +92,8 @@ __global__ void __launch_bounds__(MARCH_WARPS * 32) march_fused_kernel(MarchPara
                                                                        int count_total) {
   __shared__ uint32_t masks[MARCH_WARPS][MARCH_MAX_WORDS];
   __shared__ uint32_t warp_n[MARCH_WARPS];
-  __shared__ uint32_t ticket_s, block_base_s;
+  __shared__ uint32_t look_first[MARCH_WARPS], look_sum[MARCH_WARPS];
+  __shared__ uint32_t ticket_s, block_base_s, total_s;
   const uint32_t tid = threadIdx.x, wid = tid >> 5, lane = tid & 31;
   uint32_t *ticket_ctr = ws.scan_ctr, *done_ctr = ws.scan_ctr + 1;
   volatile unsigned long long *state = ws.scan_state;
@@ -109,19 +110,26 @@ __global__ void __launch_bounds__(MARCH_WARPS * 32) march_fused_kernel(MarchPara
       d[a] = __ldg(dirs + 3 * (size_t)r + a);
     }
     hpre = ray_hash_prefix(mp.seed, mp.step, r);
-    for (uint32_t wd = 0; wd < words; ++wd) {
-      const uint32_t k = wd * 32 + lane;
-      bool live = false;
-      if (k < mp.K) live = make_candidate(mp, bits, hpre, o, d, k).live;
-      const uint32_t m = __ballot_sync(0xffffffffu, live);
-      if (lane == 0) masks[wid][wd] = m;
-      n += __popc(m);
+    for (uint32_t wd0 = 0; wd0 < words; wd0 += 4) {   // four words at a time: their occupancy loads are independent
+      bool live[4];
+#pragma unroll
+      for (uint32_t j = 0; j < 4; ++j) {
+        const uint32_t k = (wd0 + j) * 32 + lane;
+        live[j] = (k < mp.K) && make_candidate(mp, bits, hpre, o, d, k).live;
+      }
+#pragma unroll
+      for (uint32_t j = 0; j < 4; ++j) {
+        const uint32_t m = __ballot_sync(0xffffffffu, live[j]);
+        if (lane == 0 && wd0 + j < words) masks[wid][wd0 + j] = m;
+        n += __popc(m);
+      }
     }
   }
   if (lane == 0) warp_n[wid] = n;
   __syncthreads();
+  uint32_t total = 0;
   if (wid == 0) {
-    // block-local exclusive scan of the MARCH_WARPS counts
+    // block-local exclusive scan of the MARCH_WARPS counts, then publish the block's aggregate
     const uint32_t v = lane < MARCH_WARPS ? warp_n[lane] : 0u;
     uint32_t incl = v;
 #pragma unroll
@@ -130,35 +138,48 @@ __global__ void __launch_bounds__(MARCH_WARPS * 32) march_fused_kernel(MarchPara
       if (lane >= (uint32_t)s) incl += y;
     }
     if (lane < MARCH_WARPS) warp_n[lane] = incl - v;
-    const uint32_t total = __shfl_sync(0xffffffffu, incl, 31);
-    // publish, then look back
-    if (lane == 0) atomicExch((unsigned long long *)&state[ticket], (ticket == 0 ? SCAN_INCL : SCAN_AGG) | total);
-    uint32_t excl = 0;
-    int64_t top = (int64_t)ticket - 1;       // nearest predecessor not yet summed
-    while (top >= 0) {
-      const int64_t idx = top - lane;
-      unsigned long long st = SCAN_INCL;     // lanes before ticket 0 count as "inclusive prefix 0"
-      if (idx >= 0) do { st = state[idx]; } while ((st >> 32) == 0);
-      const uint32_t is_incl = __ballot_sync(0xffffffffu, (st >> 32) == 2);
-      const uint32_t first = is_incl ? (uint32_t)__ffs(is_incl) - 1 : 31u;
-      uint32_t val = lane <= first ? (uint32_t)st : 0u;
-#pragma unroll
-      for (int s = 16; s > 0; s >>= 1) val += __shfl_xor_sync(0xffffffffu, val, s);
-      excl += val;
-      if (is_incl) break;
-      top -= 32;
-    }
+    total = __shfl_sync(0xffffffffu, incl, 31);
     if (lane == 0) {
-      if (ticket != 0) atomicExch((unsigned long long *)&state[ticket], SCAN_INCL | (unsigned long long)(excl + total));
-      block_base_s = excl;
-      if (ticket == gridDim.x - 1) {
-        ws.offsets[mp.R] = excl + total;
-        if (count_total) *ws.total_samples += excl + total;
-      }
-      if (ticket == 0) {
-        ws.loss_acc[0] = 0.0; ws.loss_acc[1] = 0.0;
-        *ws.grad_absmax = 0u;
-      }
+      atomicExch((unsigned long long *)&state[ticket], (ticket == 0 ? SCAN_INCL : SCAN_AGG) | total);
+      total_s = total;
+    }
+  }
+  // look-back by the whole block: thread i reads predecessor ticket-1-i (spinning until it is
+  // published); the sum runs back to the nearest inclusive prefix.  One L2 round trip covers
+  // MARCH_WARPS*32 predecessors.
+  uint32_t excl = 0;
+  for (int64_t top = (int64_t)ticket - 1; top >= 0; top -= MARCH_WARPS * 32) {
+    const int64_t idx = top - tid;
+    unsigned long long st = SCAN_INCL;       // positions before ticket 0 count as "inclusive prefix 0"
+    if (idx >= 0) do { st = state[idx]; } while ((st >> 32) == 0);
+    const uint32_t incl_lanes = __ballot_sync(0xffffffffu, (st >> 32) == 2);
+    if (lane == 0) look_first[wid] = incl_lanes ? (uint32_t)__ffs(incl_lanes) - 1 : 32u;
+    __syncthreads();
+    uint32_t first = MARCH_WARPS * 32;       // block-wide position of the nearest inclusive prefix
+#pragma unroll
+    for (uint32_t w = 0; w < MARCH_WARPS; ++w)
+      if (first == MARCH_WARPS * 32 && look_first[w] < 32) first = w * 32 + look_first[w];
+    uint32_t val = tid <= first ? (uint32_t)st : 0u;
+#pragma unroll
+    for (int s = 16; s > 0; s >>= 1) val += __shfl_xor_sync(0xffffffffu, val, s);
+    if (lane == 0) look_sum[wid] = val;
+    __syncthreads();
+#pragma unroll
+    for (uint32_t w = 0; w < MARCH_WARPS; ++w) excl += look_sum[w];
+    __syncthreads();
+    if (first < MARCH_WARPS * 32) break;
+  }
+  if (tid == 0) {
+    total = total_s;
+    if (ticket != 0) atomicExch((unsigned long long *)&state[ticket], SCAN_INCL | (unsigned long long)(excl + total));
+    block_base_s = excl;
+    if (ticket == gridDim.x - 1) {
+      ws.offsets[mp.R] = excl + total;
+      if (count_total) *ws.total_samples += excl + total;
+    }
+    if (ticket == 0) {
+      ws.loss_acc[0] = 0.0; ws.loss_acc[1] = 0.0;
+      *ws.grad_absmax = 0u;
     }
   }
   __syncthreads();
@@ -186,12 +207,12 @@ __global__ void __launch_bounds__(MARCH_WARPS * 32) march_fused_kernel(MarchPara
   __syncthreads();
   if (tid == 0) {
     __threadfence();
-    if (atomicAdd(done_ctr, 1u) == gridDim.x - 1) {
-      for (uint32_t i = 0; i < gridDim.x; ++i) state[i] = 0ull;
-      *ticket_ctr = 0u;
-      *done_ctr = 0u;
-      __threadfence();
-    }
+    total_s = atomicAdd(done_ctr, 1u);
+  }
+  __syncthreads();
+  if (total_s == gridDim.x - 1) {
+    for (uint32_t i = tid; i < gridDim.x; i += MARCH_WARPS * 32) state[i] = 0ull;
+    if (tid == 0) { *ticket_ctr = 0u; *done_ctr = 0u; }
   }
 }
 

@@ -52,17 +52,32 @@ struct WImg {
   static constexpr uint32_t b_total = b_d1 + 64 * H * 2;    // 24576
 };
 
-// fp32 master weights -> both 16-bit images.  Padding elements are written as zero.
+// where the five weight matrices live in the canonical fp32 block and in the two images
+struct MatImg { uint32_t off, n_out, n_in, f_off, f_NP, f_KP, b_off, b_NP, b_KP; };
+__device__ __forceinline__ MatImg mat_img(const MlpShape &ms, uint32_t i) {
+  switch (i) {
+    case 0: return {ms.o_d1, H, ms.LF, WImg::f_d1, H, ms.LF, WImg::b_d1, ms.LF, H};
+    case 1: return {ms.o_d2, DO, H, WImg::f_d2, DO, H, WImg::b_d2, H, 16};
+    case 2: return {ms.o_c1, H, ms.Ci, WImg::f_c1, H, CIP, WImg::b_c1, CIP, H};
+    case 3: return {ms.o_c2, ms.n_color_layers == 2 ? H : 0, H, WImg::f_c2, H, H, WImg::b_c2, H, H};
+    default: return {ms.o_c3, 3, H, WImg::f_c3, 16, H, WImg::b_c3, H, 16};
+  }
+}
+
+// one weight W[n][k] = v -> forward image (hi and lo terms, element (n, k)) and backward image (element (k, n))
+template <typename T>
+__device__ __forceinline__ void put_weight(const MatImg &m, uint32_t n, uint32_t k, float v, uint8_t *img_f, uint8_t *img_b) {
+  const T hi = T(v);
+  *reinterpret_cast<T *>(img_f + m.f_off + tile_off(m.f_NP, n, k)) = hi;
+  *reinterpret_cast<T *>(img_f + WImg::f_total + m.f_off + tile_off(m.f_NP, n, k)) = T(v - (float)hi);
+  *reinterpret_cast<T *>(img_b + m.b_off + tile_off(m.b_NP, k, n)) = T(v);
+}
+
+// fp32 master weights -> both 16-bit images, padding included (after nsm_set_params / at creation).
 template <typename T>
 __global__ void pack_weights_kernel(MlpShape ms, const float *__restrict__ Wm, uint8_t *__restrict__ img_f,
                                     uint8_t *__restrict__ img_b) {
-  struct M { uint32_t off, n_out, n_in, f_off, f_NP, f_KP, b_off, b_NP, b_KP; };
-  const M mats[5] = {{ms.o_d1, H, ms.LF, WImg::f_d1, H, ms.LF, WImg::b_d1, ms.LF, H},
-                     {ms.o_d2, DO, H, WImg::f_d2, DO, H, WImg::b_d2, H, 16},
-                     {ms.o_c1, H, ms.Ci, WImg::f_c1, H, CIP, WImg::b_c1, CIP, H},
-                     {ms.o_c2, ms.n_color_layers == 2 ? H : 0, H, WImg::f_c2, H, H, WImg::b_c2, H, H},
-                     {ms.o_c3, 3, H, WImg::f_c3, 16, H, WImg::b_c3, H, 16}};
-  const M m = mats[blockIdx.x];
+  const MatImg m = mat_img(ms, blockIdx.x);
   // forward tile: element (n, k) = W[n][k];  backward tile: element (i, o) = W[o][i]
   for (uint32_t idx = threadIdx.x; idx < m.f_NP * m.f_KP; idx += blockDim.x) {
     const uint32_t n = idx / m.f_KP, k = idx - n * m.f_KP;
@@ -76,6 +91,24 @@ __global__ void pack_weights_kernel(MlpShape ms, const float *__restrict__ Wm, u
     const float v = (i < m.n_in && o < m.n_out) ? Wm[m.off + o * m.n_in + i] : 0.f;
     *reinterpret_cast<T *>(img_b + m.b_off + tile_off(m.b_NP, i, o)) = T(v);
   }
+}
+
+// S13 on the MLP weights (all of them, every step) fused with the image refresh: one thread per
+// weight updates theta, m, v, clears the gradient and writes the weight's three 16-bit image
+// elements.  Padding elements of the images stay zero from pack_weights_kernel.
+template <typename T>
+__global__ void __launch_bounds__(128) adam_pack_kernel(MlpShape ms, float *__restrict__ theta, float *__restrict__ m_,
+                                                        float *__restrict__ v_, float *__restrict__ grad, uint8_t *__restrict__ img_f,
+                                                        uint8_t *__restrict__ img_b, AdamConst c) {
+  const uint32_t p = blockIdx.x * blockDim.x + threadIdx.x;
+  if (p >= ms.n_mlp) return;
+  float th = theta[p], mm = m_[p], vv = v_[p];
+  adam_one(th, mm, vv, grad[p], c);
+  theta[p] = th; m_[p] = mm; v_[p] = vv; grad[p] = 0.f;
+  const uint32_t mi = p >= ms.o_c3 ? 4u : (p >= ms.o_c2 && ms.n_color_layers == 2) ? 3u : p >= ms.o_c1 ? 2u : p >= ms.o_d2 ? 1u : 0u;
+  const MatImg mt = mat_img(ms, mi);
+  const uint32_t q = p - mt.off, n = q / mt.n_in, k = q - n * mt.n_in;
+  put_weight<T>(mt, n, k, th, img_f, img_b);
 }
 
 // issue the k-steps of one layer: D[128 x N] = A[128 x K] * B[N x K]^T, both K-major
@@ -603,6 +636,14 @@ size_t mlp_tc_wimg_bytes(int backward) { return backward ? WImg::b_total : 2 * W
 int launch_pack_weights(const MlpShape &ms, int bf16, const float *theta_mlp, const Workspace &ws, cudaStream_t st) {
   if (bf16) pack_weights_kernel<__nv_bfloat16><<<5, 256, 0, st>>>(ms, theta_mlp, ws.wimg_fwd, ws.wimg_bwd);
   else pack_weights_kernel<__half><<<5, 256, 0, st>>>(ms, theta_mlp, ws.wimg_fwd, ws.wimg_bwd);
+  return 1;
+}
+
+int launch_adam_mlp_pack(const MlpShape &ms, int bf16, const FieldParams &fp, const Workspace &ws, const AdamConst &c,
+                         cudaStream_t st) {
+  const unsigned grid = (ms.n_mlp + 127) / 128;
+  if (bf16) adam_pack_kernel<__nv_bfloat16><<<grid, 128, 0, st>>>(ms, fp.mlp_theta, fp.mlp_m, fp.mlp_v, fp.mlp_grad, ws.wimg_fwd, ws.wimg_bwd, c);
+  else adam_pack_kernel<__half><<<grid, 128, 0, st>>>(ms, fp.mlp_theta, fp.mlp_m, fp.mlp_v, fp.mlp_grad, ws.wimg_fwd, ws.wimg_bwd, c);
   return 1;
 }
 

@@ -262,9 +262,13 @@ nsm_status enqueue_adam(nsm_field *f) {
   const double bc2 = 1.0 - std::pow((double)f->cfg.beta2, (double)t);
   RUN(f, K_ADAM_TABLE, launch_adam_table(f->fp, f->cfg.n_features, f->cfg.sparse_table_adam != 0, f->cfg.lr, f->cfg.beta1,
                                          f->cfg.beta2, f->cfg.eps, (float)(1.0 / bc1), (float)(1.0 / bc2), f->n_sms, f->stream));
-  RUN(f, K_ADAM_MLP, launch_adam_mlp(f->fp, f->cfg.lr, f->cfg.beta1, f->cfg.beta2, f->cfg.eps, (float)(1.0 / bc1),
-                                     (float)(1.0 / bc2), f->stream));
-  repack_weights(f);
+  if (f->use_tc) {
+    const AdamConst c{f->cfg.lr, f->cfg.beta1, f->cfg.beta2, f->cfg.eps, (float)(1.0 / bc1), (float)(1.0 / bc2)};
+    RUN(f, K_ADAM_MLP, launch_adam_mlp_pack(f->ms, f->cfg.mlp_precision == NSM_MLP_BF16, f->fp, f->ws, c, f->stream));
+  } else {
+    RUN(f, K_ADAM_MLP, launch_adam_mlp(f->fp, f->cfg.lr, f->cfg.beta1, f->cfg.beta2, f->cfg.eps, (float)(1.0 / bc1),
+                                       (float)(1.0 / bc2), f->stream));
+  }
   f->step = t;
   if (f->prof.on) f->prof.collect();
   f->grads_dirty = false;   // the Adam kernels clear what they consume

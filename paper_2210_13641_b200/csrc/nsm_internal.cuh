@@ -99,6 +99,18 @@ struct FieldParams {
   uint32_t F;
 };
 
+// S13: one Adam update with bias correction (inv_bc = 1 / (1 - beta^t), computed on the host in float64)
+struct AdamConst {
+  float lr, b1, b2, eps, inv_bc1, inv_bc2;
+};
+
+__device__ __forceinline__ void adam_one(float &th, float &m, float &v, float g, const AdamConst &c) {
+  m = c.b1 * m + (1.f - c.b1) * g;
+  v = c.b2 * v + (1.f - c.b2) * g * g;
+  float mhat = m * c.inv_bc1, vhat = v * c.inv_bc2;
+  th = th - c.lr * mhat / (sqrtf(vhat) + c.eps);
+}
+
 // ---- launchers (each enqueues on `st`, returns the number of kernels launched) ----
 // S1-S3 in one launch; also resets the loss accumulators and (count_total) adds S to the running sample count
 int launch_march(const MarchParams &mp, const uint8_t *bits, const float *origins, const float *dirs,
@@ -140,6 +152,9 @@ int launch_adam_table(const FieldParams &fp, uint32_t F, int sparse, float lr, f
                       float eps, float inv_bc1, float inv_bc2, int n_sms, cudaStream_t st);
 int launch_adam_mlp(const FieldParams &fp, float lr, float beta1, float beta2, float eps, float inv_bc1,
                     float inv_bc2, cudaStream_t st);
+// tensor-core path: Adam on the MLP weights and, in the same launch, the refreshed 16-bit weight images
+int launch_adam_mlp_pack(const MlpShape &ms, int bf16, const FieldParams &fp, const Workspace &ws, const AdamConst &c,
+                         cudaStream_t st);
 int launch_occ_cells(uint32_t G, uint64_t first_cell, uint64_t n_cells, const Workspace &ws,
                      uint32_t *d_S, cudaStream_t st);
 int launch_occ_threshold(uint32_t G, uint64_t first_cell, uint64_t n_cells, const float *sigma,
