@@ -21,19 +21,18 @@ constexpr int ADAM_CHUNK_FLOATS = 4096;
 constexpr int ADAM_THREADS = 256;
 
 template <int F>
-__device__ __forceinline__ void adam_record(float *__restrict__ r, const float *g, const AdamConst &c) {
+__device__ __forceinline__ void adam_record(float *__restrict__ r, const float *g, const AdamConst &c, uint64_t pol_ld, uint64_t pol) {
   float th[F], m[F], v[F];
   if constexpr (F == 1) {
-    const float4 t = *reinterpret_cast<const float4 *>(r);
+    const float4 t = ld_hint_f4(r, pol_ld);
     th[0] = t.x; m[0] = t.z; v[0] = t.w;
   } else if constexpr (F == 2) {
-    const float4 a = *reinterpret_cast<const float4 *>(r), b = *reinterpret_cast<const float4 *>(r + 4);
+    const float4 a = ld_hint_f4(r, pol_ld), b = ld_hint_f4(r + 4, pol_ld);
     th[0] = a.x; th[1] = a.y; m[0] = b.x; m[1] = b.y; v[0] = b.z; v[1] = b.w;
   } else {
 #pragma unroll
     for (int i = 0; i < F / 4; ++i) {
-      const float4 a = *reinterpret_cast<const float4 *>(r + 4 * i), b = *reinterpret_cast<const float4 *>(r + 2 * F + 4 * i),
-                   d = *reinterpret_cast<const float4 *>(r + 3 * F + 4 * i);
+      const float4 a = ld_hint_f4(r + 4 * i, pol_ld), b = ld_hint_f4(r + 2 * F + 4 * i, pol_ld), d = ld_hint_f4(r + 3 * F + 4 * i, pol_ld);
       th[4 * i] = a.x; th[4 * i + 1] = a.y; th[4 * i + 2] = a.z; th[4 * i + 3] = a.w;
       m[4 * i] = b.x; m[4 * i + 1] = b.y; m[4 * i + 2] = b.z; m[4 * i + 3] = b.w;
       v[4 * i] = d.x; v[4 * i + 1] = d.y; v[4 * i + 2] = d.z; v[4 * i + 3] = d.w;
@@ -42,17 +41,17 @@ __device__ __forceinline__ void adam_record(float *__restrict__ r, const float *
 #pragma unroll
   for (int f = 0; f < F; ++f) adam_one(th[f], m[f], v[f], g[f], c);
   if constexpr (F == 1) {
-    r[0] = th[0];
-    *reinterpret_cast<float2 *>(r + 2) = make_float2(m[0], v[0]);
+    st_hint_f1(r, th[0], pol);
+    st_hint_f2(r + 2, make_float2(m[0], v[0]), pol);
   } else if constexpr (F == 2) {
-    *reinterpret_cast<float2 *>(r) = make_float2(th[0], th[1]);
-    *reinterpret_cast<float4 *>(r + 4) = make_float4(m[0], m[1], v[0], v[1]);
+    st_hint_f2(r, make_float2(th[0], th[1]), pol);
+    st_hint_f4(r + 4, make_float4(m[0], m[1], v[0], v[1]), pol);
   } else {
 #pragma unroll
     for (int i = 0; i < F / 4; ++i) {
-      *reinterpret_cast<float4 *>(r + 4 * i) = make_float4(th[4 * i], th[4 * i + 1], th[4 * i + 2], th[4 * i + 3]);
-      *reinterpret_cast<float4 *>(r + 2 * F + 4 * i) = make_float4(m[4 * i], m[4 * i + 1], m[4 * i + 2], m[4 * i + 3]);
-      *reinterpret_cast<float4 *>(r + 3 * F + 4 * i) = make_float4(v[4 * i], v[4 * i + 1], v[4 * i + 2], v[4 * i + 3]);
+      st_hint_f4(r + 4 * i, make_float4(th[4 * i], th[4 * i + 1], th[4 * i + 2], th[4 * i + 3]), pol);
+      st_hint_f4(r + 2 * F + 4 * i, make_float4(m[4 * i], m[4 * i + 1], m[4 * i + 2], m[4 * i + 3]), pol);
+      st_hint_f4(r + 3 * F + 4 * i, make_float4(v[4 * i], v[4 * i + 1], v[4 * i + 2], v[4 * i + 3]), pol);
     }
   }
 }
@@ -66,15 +65,18 @@ __global__ void __launch_bounds__(ADAM_THREADS) adam_table_kernel(float *__restr
   __shared__ uint16_t list_e[CH];                      // compacted local entry indices
   __shared__ uint32_t cnt;
   const uint32_t tid = threadIdx.x, lane = tid & 31;
+  pdl_wait();
+  pdl_trigger();
   const uint64_t e_base = (uint64_t)blockIdx.x * CH;
   const uint64_t n_float = n_entries * F;
-  const float4 *g4 = reinterpret_cast<const float4 *>(grad + e_base * F);
+  const float *g4 = grad + e_base * F;
+  const uint64_t pol_first = l2_evict_first(), pol_last = l2_evict_last(), pol_ld = l2_evict_normal();
   if (tid == 0) cnt = 0;
   float4 gv[NV];
 #pragma unroll
   for (int j = 0; j < NV; ++j) {
     const uint32_t q = j * ADAM_THREADS + tid;         // float4 index inside the chunk
-    gv[j] = (e_base * F + 4ull * q < n_float) ? g4[q] : make_float4(0.f, 0.f, 0.f, 0.f);   // the array is padded to 256 B
+    gv[j] = (e_base * F + 4ull * q < n_float) ? ld_hint_f4(g4 + 4 * q, pol_last) : make_float4(0.f, 0.f, 0.f, 0.f);   // the array is padded to 256 B
   }
   __syncthreads();
 #pragma unroll
@@ -125,21 +127,23 @@ __global__ void __launch_bounds__(ADAM_THREADS) adam_table_kernel(float *__restr
     if constexpr (F == 2) {   // touch the second record's sector early
       asm volatile("prefetch.global.L2 [%0];" ::"l"(r1));
     }
-    adam_record<F>(r0, list_g + i0 * F, c);
-    if (i1 < n) adam_record<F>(r1, list_g + i1 * F, c);
+    adam_record<F>(r0, list_g + i0 * F, c, pol_ld, pol_first);
+    if (i1 < n) adam_record<F>(r1, list_g + i1 * F, c, pol_ld, pol_first);
   }
   // reset the chunk's gradient words
-  float4 *o4 = reinterpret_cast<float4 *>(grad + e_base * F);
+  float *o4 = grad + e_base * F;
   const float nz = __uint_as_float(NSM_GRAD_UNTOUCHED);
 #pragma unroll
   for (int j = 0; j < NV; ++j) {
     const uint32_t q = j * ADAM_THREADS + tid;
-    if (e_base * F + 4ull * q < n_float) o4[q] = make_float4(nz, nz, nz, nz);
+    if (e_base * F + 4ull * q < n_float) st_hint_f4(o4 + 4 * q, make_float4(nz, nz, nz, nz), pol_last);
   }
 }
 
 __global__ void adam_dense_kernel(float *__restrict__ theta, float *__restrict__ m, float *__restrict__ v,
                                   float *__restrict__ grad, uint64_t n, AdamConst c) {
+  pdl_wait();
+  pdl_trigger();
   for (uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (uint64_t)gridDim.x * blockDim.x) {
     float th = theta[i], mm = m[i], vv = v[i];
     adam_one(th, mm, vv, grad[i], c);
@@ -156,10 +160,10 @@ int launch_adam_table(const FieldParams &fp, uint32_t F, int sparse, float lr, f
   const uint64_t chunk = ADAM_CHUNK_FLOATS / F;
   dim3 grid((unsigned)((fp.n_entries + chunk - 1) / chunk)), block(ADAM_THREADS);
   switch (F) {
-    case 1: adam_table_kernel<1><<<grid, block, 0, st>>>(fp.rec, fp.grad, fp.n_entries, sparse, c); break;
-    case 2: adam_table_kernel<2><<<grid, block, 0, st>>>(fp.rec, fp.grad, fp.n_entries, sparse, c); break;
-    case 4: adam_table_kernel<4><<<grid, block, 0, st>>>(fp.rec, fp.grad, fp.n_entries, sparse, c); break;
-    default: adam_table_kernel<8><<<grid, block, 0, st>>>(fp.rec, fp.grad, fp.n_entries, sparse, c); break;
+    case 1: launch_pdl(adam_table_kernel<1>, grid, block, 0, st, fp.rec, fp.grad, fp.n_entries, sparse, c); break;
+    case 2: launch_pdl(adam_table_kernel<2>, grid, block, 0, st, fp.rec, fp.grad, fp.n_entries, sparse, c); break;
+    case 4: launch_pdl(adam_table_kernel<4>, grid, block, 0, st, fp.rec, fp.grad, fp.n_entries, sparse, c); break;
+    default: launch_pdl(adam_table_kernel<8>, grid, block, 0, st, fp.rec, fp.grad, fp.n_entries, sparse, c); break;
   }
   return 1;
 }
@@ -167,6 +171,7 @@ int launch_adam_table(const FieldParams &fp, uint32_t F, int sparse, float lr, f
 int launch_adam_mlp(const FieldParams &fp, float lr, float beta1, float beta2, float eps, float inv_bc1, float inv_bc2,
                     cudaStream_t st) {
   AdamConst c{lr, beta1, beta2, eps, inv_bc1, inv_bc2};
-  adam_dense_kernel<<<(unsigned)((fp.n_mlp + 255) / 256), 256, 0, st>>>(fp.mlp_theta, fp.mlp_m, fp.mlp_v, fp.mlp_grad, fp.n_mlp, c);
+  launch_pdl(adam_dense_kernel, dim3((unsigned)((fp.n_mlp + 255) / 256)), dim3(256), 0, st, fp.mlp_theta, fp.mlp_m, fp.mlp_v, fp.mlp_grad,
+             fp.n_mlp, c);
   return 1;
 }

@@ -42,6 +42,8 @@ __global__ void __launch_bounds__(256) composite_kernel(Workspace ws, uint32_t R
                                                         float bg0, float bg1, float bg2, float cut,
                                                         float *__restrict__ out_rgb, float *__restrict__ out_depth,
                                                         float *__restrict__ out_opacity) {
+  pdl_wait();
+  pdl_trigger();
   const uint32_t r = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
   float l_rgb = 0.0f, l_d = 0.0f;  // lane 0 holds the ray's loss terms
   float gmax = 0.0f;               // max |gradient entering the MLP backward| seen by this thread
@@ -155,15 +157,15 @@ __global__ void __launch_bounds__(256) composite_kernel(Workspace ws, uint32_t R
 int launch_composite_train(const Workspace &ws, uint32_t R, const float *rgb, const float *depth,
                            const float *depth_var, float lambda_d, const float bg[3], cudaStream_t st) {
   dim3 grid((R + 7) / 8), block(256);
-  composite_kernel<true><<<grid, block, 0, st>>>(ws, R, rgb, depth, depth_var, lambda_d, bg[0], bg[1], bg[2],
-                                                 0.f, nullptr, nullptr, nullptr);
+  launch_pdl(composite_kernel<true>, grid, block, 0, st, ws, R, rgb, depth, depth_var, lambda_d, bg[0], bg[1], bg[2], 0.f,
+             (float *)nullptr, (float *)nullptr, (float *)nullptr);
   return 1;
 }
 
 int launch_composite_render(const Workspace &ws, uint32_t R, float cut, const float bg[3], float *out_rgb,
                             float *out_depth, float *out_opacity, cudaStream_t st) {
   dim3 grid((R + 7) / 8), block(256);
-  composite_kernel<false><<<grid, block, 0, st>>>(ws, R, nullptr, nullptr, nullptr, 0.f, bg[0], bg[1], bg[2], cut,
-                                                  out_rgb, out_depth, out_opacity);
+  launch_pdl(composite_kernel<false>, grid, block, 0, st, ws, R, (const float *)nullptr, (const float *)nullptr,
+             (const float *)nullptr, 0.f, bg[0], bg[1], bg[2], cut, out_rgb, out_depth, out_opacity);
   return 1;
 }

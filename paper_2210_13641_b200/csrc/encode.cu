@@ -60,6 +60,24 @@ template <> struct Vec<1> { using T = float; };
 template <> struct Vec<2> { using T = float2; };
 template <> struct Vec<4> { using T = float4; };
 
+// the same through an L2 cache-policy (hashed levels: stream, evict first)
+template <int F>
+__device__ __forceinline__ void load_entry_hint(const float *p, float out[F], uint64_t pol) {
+  if constexpr (F == 8) {
+    float4 a = ld_hint_f4(p, pol), b = ld_hint_f4(p + 4, pol);
+    out[0] = a.x; out[1] = a.y; out[2] = a.z; out[3] = a.w;
+    out[4] = b.x; out[5] = b.y; out[6] = b.z; out[7] = b.w;
+  } else if constexpr (F == 4) {
+    float4 a = ld_hint_f4(p, pol);
+    out[0] = a.x; out[1] = a.y; out[2] = a.z; out[3] = a.w;
+  } else if constexpr (F == 2) {
+    float2 a = ld_hint_f2(p, pol);
+    out[0] = a.x; out[1] = a.y;
+  } else {
+    out[0] = ld_hint_f1(p, pol);
+  }
+}
+
 template <int F>
 __device__ __forceinline__ void load_entry(const float *p, float out[F]) {
   if constexpr (F == 8) {
@@ -83,10 +101,13 @@ __device__ __forceinline__ void load_entry(const float *p, float out[F]) {
 template <int F, int MODE>
 __global__ void __launch_bounds__(256) encode_forward_kernel(LevelTable lv, const float *__restrict__ rec,
                                                              Workspace ws, const uint32_t *__restrict__ d_S) {
+  pdl_wait();
+  pdl_trigger();
   const uint64_t S = *d_S;
   const uint64_t S_it = MODE == 0 ? S : ((S + NSM_TILE - 1) / NSM_TILE) * NSM_TILE;
   const uint64_t total = S_it * lv.n_levels;
   const uint32_t LF = lv.n_levels * F;
+  const uint64_t pol_first = l2_evict_first();
   for (uint64_t wi = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; wi < total;
        wi += (uint64_t)gridDim.x * blockDim.x) {
     const uint32_t l = (uint32_t)(wi / S_it);
@@ -99,7 +120,13 @@ __global__ void __launch_bounds__(256) encode_forward_kernel(LevelTable lv, cons
       const float *tab = rec + lv.offset[l] * (4 * F);   // theta = the first F floats of a 4F-float record
       float v[8][F];
 #pragma unroll
-      for (int k = 0; k < 8; ++k) load_entry<F>(tab + (size_t)ci.slot[k] * (4 * F), v[k]);  // 8 gathers in flight
+      if (lv.dense[l]) {   // coarse levels are re-read every step: normal policy; hashed levels stream through L2
+#pragma unroll
+        for (int k = 0; k < 8; ++k) load_entry<F>(tab + (size_t)ci.slot[k] * (4 * F), v[k]);  // 8 gathers in flight
+      } else {
+#pragma unroll
+        for (int k = 0; k < 8; ++k) load_entry_hint<F>(tab + (size_t)ci.slot[k] * (4 * F), v[k], pol_first);
+      }
 #pragma unroll
       for (int k = 0; k < 8; ++k) {
         float om = corner_weight(k, ci.w);
@@ -132,17 +159,17 @@ __global__ void __launch_bounds__(256) encode_forward_kernel(LevelTable lv, cons
 }
 
 template <int F>
-__device__ __forceinline__ void red_add_entry(float *p, const float g[F]) {
-  // vectorised no-return reductions (red.global.add.v2/v4.f32, sm_90+)
+__device__ __forceinline__ void red_add_entry(float *p, const float g[F], uint64_t pol) {
+  // vectorised no-return reductions (red.global.add.v2/v4.f32, sm_90+); the gradient array stays in L2
   if constexpr (F == 8) {
-    atomicAdd(reinterpret_cast<float4 *>(p), make_float4(g[0], g[1], g[2], g[3]));
-    atomicAdd(reinterpret_cast<float4 *>(p) + 1, make_float4(g[4], g[5], g[6], g[7]));
+    red_hint_f4(p, make_float4(g[0], g[1], g[2], g[3]), pol);
+    red_hint_f4(p + 4, make_float4(g[4], g[5], g[6], g[7]), pol);
   } else if constexpr (F == 4) {
-    atomicAdd(reinterpret_cast<float4 *>(p), make_float4(g[0], g[1], g[2], g[3]));
+    red_hint_f4(p, make_float4(g[0], g[1], g[2], g[3]), pol);
   } else if constexpr (F == 2) {
-    atomicAdd(reinterpret_cast<float2 *>(p), make_float2(g[0], g[1]));
+    red_hint_f2(p, make_float2(g[0], g[1]), pol);
   } else {
-    atomicAdd(p, g[0]);
+    red_hint_f1(p, g[0], pol);
   }
 }
 
@@ -152,8 +179,11 @@ __device__ __forceinline__ void red_add_entry(float *p, const float g[F]) {
 template <int F>
 __global__ void __launch_bounds__(256) scatter_backward_kernel(LevelTable lv, float *__restrict__ grad, Workspace ws,
                                                                const uint32_t *__restrict__ d_S) {
+  pdl_wait();
+  pdl_trigger();
   const uint64_t S = *d_S;
   const uint64_t total = S * lv.n_levels;
+  const uint64_t pol_last = l2_evict_last();
   for (uint64_t wi = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; wi < total;
        wi += (uint64_t)gridDim.x * blockDim.x) {
     const uint32_t l = (uint32_t)(wi / S);
@@ -172,7 +202,7 @@ __global__ void __launch_bounds__(256) scatter_backward_kernel(LevelTable lv, fl
         const float v = om * de[f];
         g[f] = fabsf(v) < NSM_GRAD_MIN_ADDEND ? 0.0f : v;   // never -0.0, never near-subnormal; NaN stays NaN
       }
-      red_add_entry<F>(tab + (size_t)ci.slot[k] * F, g);
+      red_add_entry<F>(tab + (size_t)ci.slot[k] * F, g, pol_last);
     }
   }
 }
@@ -257,9 +287,9 @@ int launch_unpack_records(const FieldParams &fp, int which, float *dst, cudaStre
 template <int F>
 static void launch_encode_f(const LevelTable &lv, const float *theta, const Workspace &ws, const uint32_t *d_S, int out_mode,
                             dim3 grid, dim3 block, cudaStream_t st) {
-  if (out_mode == 0) encode_forward_kernel<F, 0><<<grid, block, 0, st>>>(lv, theta, ws, d_S);
-  else if (out_mode == 1) encode_forward_kernel<F, 1><<<grid, block, 0, st>>>(lv, theta, ws, d_S);
-  else encode_forward_kernel<F, 2><<<grid, block, 0, st>>>(lv, theta, ws, d_S);
+  if (out_mode == 0) launch_pdl(encode_forward_kernel<F, 0>, grid, block, 0, st, lv, theta, ws, d_S);
+  else if (out_mode == 1) launch_pdl(encode_forward_kernel<F, 1>, grid, block, 0, st, lv, theta, ws, d_S);
+  else launch_pdl(encode_forward_kernel<F, 2>, grid, block, 0, st, lv, theta, ws, d_S);
 }
 
 int launch_encode(const LevelTable &lv, const float *theta, const Workspace &ws, const uint32_t *d_S, int out_mode,
@@ -288,10 +318,10 @@ int launch_scatter(const LevelTable &lv, float *grad, const Workspace &ws,
                    const uint32_t *d_S, int n_sms, cudaStream_t st) {
   dim3 grid(n_sms * 8), block(256);
   switch (lv.n_features) {
-    case 1: scatter_backward_kernel<1><<<grid, block, 0, st>>>(lv, grad, ws, d_S); break;
-    case 2: scatter_backward_kernel<2><<<grid, block, 0, st>>>(lv, grad, ws, d_S); break;
-    case 4: scatter_backward_kernel<4><<<grid, block, 0, st>>>(lv, grad, ws, d_S); break;
-    default: scatter_backward_kernel<8><<<grid, block, 0, st>>>(lv, grad, ws, d_S); break;
+    case 1: launch_pdl(scatter_backward_kernel<1>, grid, block, 0, st, lv, grad, ws, d_S); break;
+    case 2: launch_pdl(scatter_backward_kernel<2>, grid, block, 0, st, lv, grad, ws, d_S); break;
+    case 4: launch_pdl(scatter_backward_kernel<4>, grid, block, 0, st, lv, grad, ws, d_S); break;
+    default: launch_pdl(scatter_backward_kernel<8>, grid, block, 0, st, lv, grad, ws, d_S); break;
   }
   return 1;
 }

@@ -97,6 +97,8 @@ __global__ void __launch_bounds__(MARCH_WARPS * 32) march_fused_kernel(MarchPara
   const uint32_t tid = threadIdx.x, wid = tid >> 5, lane = tid & 31;
   uint32_t *ticket_ctr = ws.scan_ctr, *done_ctr = ws.scan_ctr + 1;
   volatile unsigned long long *state = ws.scan_state;
+  pdl_wait();
+  pdl_trigger();
   if (tid == 0) ticket_s = atomicAdd(ticket_ctr, 1u);
   __syncthreads();
   const uint32_t ticket = ticket_s;
@@ -245,7 +247,7 @@ __global__ void occ_threshold_kernel(uint64_t first_cell, uint64_t n_cells,
 int launch_march(const MarchParams &mp, const uint8_t *bits, const float *origins, const float *dirs,
                  const Workspace &ws, int count_total, cudaStream_t st) {
   dim3 grid((mp.R + MARCH_WARPS - 1) / MARCH_WARPS), block(MARCH_WARPS * 32);
-  march_fused_kernel<<<grid, block, 0, st>>>(mp, bits, origins, dirs, ws, count_total);
+  launch_pdl(march_fused_kernel, grid, block, 0, st, mp, bits, origins, dirs, ws, count_total);
   return 1;
 }
 

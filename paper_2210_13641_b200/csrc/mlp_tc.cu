@@ -100,6 +100,8 @@ template <typename T>
 __global__ void __launch_bounds__(128) adam_pack_kernel(MlpShape ms, float *__restrict__ theta, float *__restrict__ m_,
                                                         float *__restrict__ v_, float *__restrict__ grad, uint8_t *__restrict__ img_f,
                                                         uint8_t *__restrict__ img_b, AdamConst c) {
+  pdl_wait();
+  pdl_trigger();
   const uint32_t p = blockIdx.x * blockDim.x + threadIdx.x;
   if (p >= ms.n_mlp) return;
   float th = theta[p], mm = m_[p], vv = v_[p];
@@ -159,7 +161,7 @@ __device__ __forceinline__ void sh_row(uint32_t n, float x, float y, float z, fl
 
 // 16 accumulator columns -> (optional ReLU) -> this thread's row of a shared tile and of a global blob tile
 template <typename T, bool RELU>
-__device__ __forceinline__ void emit16(float *v, uint8_t *smem_tile, uint8_t *blob_tile, uint32_t c0, bool valid) {
+__device__ __forceinline__ void emit16(float *v, uint8_t *smem_tile, uint8_t *blob_tile, uint32_t row, uint32_t c0, bool valid) {
   if (RELU) {
 #pragma unroll
     for (int j = 0; j < 16; ++j) v[j] = fmaxf(v[j], 0.f);
@@ -167,7 +169,7 @@ __device__ __forceinline__ void emit16(float *v, uint8_t *smem_tile, uint8_t *bl
   uint4 q0, q1;
   q0.x = pack2<T>(v[0], v[1]); q0.y = pack2<T>(v[2], v[3]); q0.z = pack2<T>(v[4], v[5]); q0.w = pack2<T>(v[6], v[7]);
   q1.x = pack2<T>(v[8], v[9]); q1.y = pack2<T>(v[10], v[11]); q1.z = pack2<T>(v[12], v[13]); q1.w = pack2<T>(v[14], v[15]);
-  const uint32_t o0 = tile_off(ROWS, threadIdx.x, c0), o1 = tile_off(ROWS, threadIdx.x, c0 + 8);
+  const uint32_t o0 = tile_off(ROWS, row, c0), o1 = tile_off(ROWS, row, c0 + 8);
   *reinterpret_cast<uint4 *>(smem_tile + o0) = q0;
   *reinterpret_cast<uint4 *>(smem_tile + o1) = q1;
   if (blob_tile) {   // rows of invalid samples are stored as zeros so the backward wgrad never sees garbage
@@ -179,8 +181,8 @@ __device__ __forceinline__ void emit16(float *v, uint8_t *smem_tile, uint8_t *bl
 
 // two-term version: hi -> smem_tile and blob, lo -> smem_tile + lo_off
 template <typename T, bool RELU>
-__device__ __forceinline__ void emit16s(float *v, uint8_t *smem_tile, uint32_t lo_off, uint8_t *blob_tile, uint32_t c0,
-                                        bool valid) {
+__device__ __forceinline__ void emit16s(float *v, uint8_t *smem_tile, uint32_t lo_off, uint8_t *blob_tile, uint32_t row,
+                                        uint32_t c0, bool valid) {
   if (RELU) {
 #pragma unroll
     for (int j = 0; j < 16; ++j) v[j] = fmaxf(v[j], 0.f);
@@ -192,7 +194,7 @@ __device__ __forceinline__ void emit16s(float *v, uint8_t *smem_tile, uint32_t l
     const float2 h = unpack2<T>(hi[j]);
     lo[j] = pack2<T>(v[2 * j] - h.x, v[2 * j + 1] - h.y);
   }
-  const uint32_t o0 = tile_off(ROWS, threadIdx.x, c0), o1 = tile_off(ROWS, threadIdx.x, c0 + 8);
+  const uint32_t o0 = tile_off(ROWS, row, c0), o1 = tile_off(ROWS, row, c0 + 8);
   *reinterpret_cast<uint4 *>(smem_tile + o0) = make_uint4(hi[0], hi[1], hi[2], hi[3]);
   *reinterpret_cast<uint4 *>(smem_tile + o1) = make_uint4(hi[4], hi[5], hi[6], hi[7]);
   *reinterpret_cast<uint4 *>(smem_tile + lo_off + o0) = make_uint4(lo[0], lo[1], lo[2], lo[3]);
@@ -208,10 +210,13 @@ __device__ __forceinline__ void emit16s(float *v, uint8_t *smem_tile, uint32_t l
 constexpr uint32_t COL_D1 = 0, COL_D2 = 64, COL_C1 = 96, COL_C2 = 160, COL_C3 = 224, FWD_COLS = 256;
 
 constexpr uint32_t TILE_BYTES = ROWS * H * 2;   // one [128][64] 16-bit tile
+constexpr uint32_t FWD_THREADS = 256;
+// Two activation buffers (each hi | lo) ping-pong through the layer chain; the encoder tile arrives
+// by TMA into buffer A, which is dead again by the time the colour input is built.  With the
+// two-term weight images that is 48 + 64 KB, so TWO CTAs fit an SM (and 2 x 256 TMEM columns).
 struct FwdSmem {
   static constexpr uint32_t w = 0;                                // weight images: hi (WImg forward region) then lo
-  static constexpr uint32_t bufE = w + 2 * WImg::f_total;         // encoder tile hi | lo (TMA destination, 2 x LF*256 bytes)
-  static constexpr uint32_t bufA = bufE + 2 * TILE_BYTES;         // hi | lo
+  static constexpr uint32_t bufA = w + 2 * WImg::f_total;         // hi | lo; also the TMA destination of the encoder tile
   static constexpr uint32_t bufB = bufA + 2 * TILE_BYTES;         // hi | lo
   static constexpr uint32_t bar_mma = bufB + 2 * TILE_BYTES;
   static constexpr uint32_t bar_w = bar_mma + 8;
@@ -220,64 +225,70 @@ struct FwdSmem {
   static constexpr uint32_t total = tmem + 8;
 };
 
+// 8 warps per 128-sample tile: warp w owns TMEM lanes (= sample rows) 32 (w & 3) .. +31 -- the
+// hardware's lane-quarter rule -- and the column half (w >> 2) of every 64-wide layer, so the
+// accumulator read-back / two-term split / store of a layer is shared by two warps per SM
+// sub-partition (four with the second resident CTA).
 template <typename T>
-__global__ void __launch_bounds__(128) mlp_forward_tc_kernel(MlpShape ms, const float *__restrict__ dirs, Workspace ws,
-                                                             const uint32_t *__restrict__ d_S, int density_only,
-                                                             int save_blobs) {
+__global__ void __launch_bounds__(FWD_THREADS, 2) mlp_forward_tc_kernel(MlpShape ms, const float *__restrict__ dirs, Workspace ws,
+                                                                       const uint32_t *__restrict__ d_S, int density_only,
+                                                                       int save_blobs) {
   extern __shared__ __align__(1024) uint8_t smem[];
-  const uint32_t tid = threadIdx.x, warp = tid >> 5;
+  const uint32_t tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+  const uint32_t row = (warp & 3u) * 32u + lane, half = warp >> 2;
   const uint32_t sbase = smem_u32(smem);
   const uint32_t bar_mma = sbase + FwdSmem::bar_mma, bar_w = sbase + FwdSmem::bar_w, bar_e = sbase + FwdSmem::bar_e;
   const uint32_t LF = ms.LF;
   const uint32_t e_half = LF * ROWS * 2, e_bytes = 2 * e_half;   // hi | lo
+  // Before pdl_wait(): only data produced at least two kernels back (S from the marcher, the weight images).
   const uint64_t S = *d_S;
-  if ((uint64_t)blockIdx.x * ROWS >= S) return;
-
-  if (tid == 0) {
-    mbar_init(bar_mma, 1); mbar_init(bar_w, 1); mbar_init(bar_e, 1);
-    fence_async_smem();
-    mbar_expect_tx(bar_w, 2 * WImg::f_total);
-    bulk_g2s(sbase + FwdSmem::w, ws.wimg_fwd, 2 * WImg::f_total, bar_w);
-    mbar_expect_tx(bar_e, e_bytes);
-    bulk_g2s(sbase + FwdSmem::bufE, ws.blob_e + (size_t)blockIdx.x * e_bytes, e_bytes, bar_e);
+  const bool has_tiles = (uint64_t)blockIdx.x * ROWS < S;
+  if (has_tiles) {
+    if (tid == 0) {
+      mbar_init(bar_mma, 1); mbar_init(bar_w, 1); mbar_init(bar_e, 1);
+      fence_async_smem();
+      mbar_expect_tx(bar_w, 2 * WImg::f_total);
+      bulk_g2s(sbase + FwdSmem::w, ws.wimg_fwd, 2 * WImg::f_total, bar_w);
+    }
+    if (warp == 0) tmem_alloc<FWD_COLS>(sbase + FwdSmem::tmem);
   }
-  if (warp == 0) tmem_alloc<FWD_COLS>(sbase + FwdSmem::tmem);
+  pdl_wait();
+  pdl_trigger();
+  if (!has_tiles) return;
+  if (tid == 0) {   // the encoder's output: after the wait
+    mbar_expect_tx(bar_e, e_bytes);
+    bulk_g2s(sbase + FwdSmem::bufA, ws.blob_e + (size_t)blockIdx.x * e_bytes, e_bytes, bar_e);
+  }
   fence_before();
   __syncthreads();
   fence_after();
   const uint32_t tmem_base = *reinterpret_cast<volatile uint32_t *>(smem + FwdSmem::tmem);
-  const uint32_t tlane = tmem_base + ((warp * 32u) << 16);
+  const uint32_t tlane = tmem_base + (((warp & 3u) * 32u) << 16);
   uint32_t ph_mma = 0, ph_e = 0;
   const uint32_t fmt = Fmt<T>::id;
   uint8_t *bufA = smem + FwdSmem::bufA, *bufB = smem + FwdSmem::bufB;
-  const uint32_t sE = sbase + FwdSmem::bufE, sA = sbase + FwdSmem::bufA, sB = sbase + FwdSmem::bufB, sW = sbase + FwdSmem::w;
+  const uint32_t sA = sbase + FwdSmem::bufA, sB = sbase + FwdSmem::bufB, sW = sbase + FwdSmem::w;
+  const uint32_t cb = half * 32u;    // this thread's column half of a 64-wide layer
   if (tid == 0) mbar_wait(bar_w, 0);
 
   for (uint64_t tile = blockIdx.x; tile * ROWS < S; tile += gridDim.x) {
-    const uint64_t s = tile * ROWS + tid;
+    const uint64_t s = tile * ROWS + row;
     const bool valid = s < S;
     float v[16];
-    // ---- density hidden layer: A = encoder tile (already in shared memory via TMA)
+    // ---- density hidden layer: A = encoder tile (in buffer A via TMA)
     if (tid == 0) {
       mbar_wait(bar_e, ph_e);
       fence_after();
-      issue_layer_split(tmem_base + COL_D1, sE, e_half, sW + WImg::f_d1, WImg::f_total, LF, H, H, fmt, bar_mma);
+      issue_layer_split(tmem_base + COL_D1, sA, e_half, sW + WImg::f_d1, WImg::f_total, LF, H, H, fmt, bar_mma);
     }
     ph_e ^= 1;
     mbar_wait(bar_mma, ph_mma); ph_mma ^= 1; fence_after();
-    if (tid == 0) {   // bufE is free again: prefetch the CTA's next encoder tile
-      const uint64_t nxt = tile + gridDim.x;
-      if (nxt * ROWS < S) {
-        mbar_expect_tx(bar_e, e_bytes);
-        bulk_g2s(sE, ws.blob_e + (size_t)nxt * e_bytes, e_bytes, bar_e);
-      }
-    }
     uint8_t *blob_hd = (save_blobs && !density_only) ? ws.blob_hd + (size_t)tile * (H * ROWS * 2) : nullptr;
 #pragma unroll
-    for (uint32_t c0 = 0; c0 < H; c0 += 16) {
-      tmem_ld16(tlane + COL_D1 + c0, v);
+    for (uint32_t c0 = 0; c0 < 32; c0 += 16) {
+      tmem_ld16(tlane + COL_D1 + cb + c0, v);
       tmem_ld_wait();
-      emit16s<T, true>(v, bufB, TILE_BYTES, blob_hd, c0, valid);
+      emit16s<T, true>(v, bufB, TILE_BYTES, blob_hd, row, cb + c0, valid);
     }
     fence_async_smem(); fence_before(); __syncthreads();
     if (tid == 0) { fence_after(); issue_layer_split(tmem_base + COL_D2, sB, TILE_BYTES, sW + WImg::f_d2, WImg::f_total, H, DO, DO, fmt, bar_mma); }
@@ -285,35 +296,46 @@ __global__ void __launch_bounds__(128) mlp_forward_tc_kernel(MlpShape ms, const 
     float g[16];
     tmem_ld16(tlane + COL_D2, g);
     tmem_ld_wait();
-    if (valid) ws.sigma[s] = expf(fminf(fmaxf(g[0], -15.f), 15.f));
-    if (density_only) { fence_before(); continue; }
-    // ---- colour input [g slice, Y(d), 0 pad] -> bufA (K = 32)
+    if (valid && half == 0) ws.sigma[s] = expf(fminf(fmaxf(g[0], -15.f), 15.f));
+    if (density_only) {
+      fence_before(); __syncthreads();
+      if (tid == 0) {   // buffer A is free: the CTA's next encoder tile
+        const uint64_t nxt = tile + gridDim.x;
+        if (nxt * ROWS < S) { mbar_expect_tx(bar_e, e_bytes); bulk_g2s(sA, ws.blob_e + (size_t)nxt * e_bytes, e_bytes, bar_e); }
+      }
+      continue;
+    }
+    // ---- colour input [g slice, Y(d), 0 pad] -> buffer A (K = 32); each column half emits its 16 columns
     {
       float ci[CIP];
 #pragma unroll
       for (int j = 0; j < (int)CIP; ++j) ci[j] = 0.f;
-      for (uint32_t j = 0; j < ms.geo_cnt; ++j) ci[j] = g[ms.geo_off + j];
+      // mlp_tc_supported() admits only the slice (geo_offset, geo_count) = (1, 15) with 16 SH terms (configs 2-5):
+      // static register indexing, no local memory
+#pragma unroll
+      for (int j = 0; j < 15; ++j) ci[j] = g[1 + j];
       float dx = 0.f, dy = 0.f, dz = 1.f;
       if (valid) {
         const uint32_t ray = ws.s_ray[s];
         dx = __ldg(dirs + 3 * (size_t)ray); dy = __ldg(dirs + 3 * (size_t)ray + 1); dz = __ldg(dirs + 3 * (size_t)ray + 2);
       }
       float Y[16];
-      sh_row(ms.sh_degree, dx, dy, dz, Y);
-      for (uint32_t j = 0; j < ms.n_sh; ++j) ci[ms.geo_cnt + j] = Y[j];
+      sh_row(4, dx, dy, dz, Y);
+#pragma unroll
+      for (int j = 0; j < 16; ++j) ci[15 + j] = Y[j];
       uint8_t *blob_ci = save_blobs ? ws.blob_ci + (size_t)tile * (CIP * ROWS * 2) : nullptr;
-      emit16s<T, false>(ci, bufA, TILE_BYTES, blob_ci, 0, valid);
-      emit16s<T, false>(ci + 16, bufA, TILE_BYTES, blob_ci, 16, valid);
+      if (half == 0) emit16s<T, false>(ci, bufA, TILE_BYTES, blob_ci, row, 0, valid);
+      else emit16s<T, false>(ci + 16, bufA, TILE_BYTES, blob_ci, row, 16, valid);
     }
     fence_async_smem(); fence_before(); __syncthreads();
     if (tid == 0) { fence_after(); issue_layer_split(tmem_base + COL_C1, sA, TILE_BYTES, sW + WImg::f_c1, WImg::f_total, CIP, H, H, fmt, bar_mma); }
     mbar_wait(bar_mma, ph_mma); ph_mma ^= 1; fence_after();
     uint8_t *blob_h1 = save_blobs ? ws.blob_h1 + (size_t)tile * (H * ROWS * 2) : nullptr;
 #pragma unroll
-    for (uint32_t c0 = 0; c0 < H; c0 += 16) {
-      tmem_ld16(tlane + COL_C1 + c0, v);
+    for (uint32_t c0 = 0; c0 < 32; c0 += 16) {
+      tmem_ld16(tlane + COL_C1 + cb + c0, v);
       tmem_ld_wait();
-      emit16s<T, true>(v, bufB, TILE_BYTES, blob_h1, c0, valid);
+      emit16s<T, true>(v, bufB, TILE_BYTES, blob_h1, row, cb + c0, valid);
     }
     uint32_t sLast = sB;
     if (ms.n_color_layers == 2) {
@@ -322,23 +344,30 @@ __global__ void __launch_bounds__(128) mlp_forward_tc_kernel(MlpShape ms, const 
       mbar_wait(bar_mma, ph_mma); ph_mma ^= 1; fence_after();
       uint8_t *blob_h2 = save_blobs ? ws.blob_h2 + (size_t)tile * (H * ROWS * 2) : nullptr;
 #pragma unroll
-      for (uint32_t c0 = 0; c0 < H; c0 += 16) {
-        tmem_ld16(tlane + COL_C2 + c0, v);
+      for (uint32_t c0 = 0; c0 < 32; c0 += 16) {
+        tmem_ld16(tlane + COL_C2 + cb + c0, v);
         tmem_ld_wait();
-        emit16s<T, true>(v, bufA, TILE_BYTES, blob_h2, c0, valid);
+        emit16s<T, true>(v, bufA, TILE_BYTES, blob_h2, row, cb + c0, valid);
       }
       sLast = sA;
     }
     fence_async_smem(); fence_before(); __syncthreads();
     if (tid == 0) { fence_after(); issue_layer_split(tmem_base + COL_C3, sLast, TILE_BYTES, sW + WImg::f_c3, WImg::f_total, H, 16, 16, fmt, bar_mma); }
     mbar_wait(bar_mma, ph_mma); ph_mma ^= 1; fence_after();
-    tmem_ld16(tlane + COL_C3, v);
-    tmem_ld_wait();
-    if (valid) {
+    if (tid == 0) {   // every buffer is free: the CTA's next encoder tile
+      const uint64_t nxt = tile + gridDim.x;
+      if (nxt * ROWS < S) { mbar_expect_tx(bar_e, e_bytes); bulk_g2s(sA, ws.blob_e + (size_t)nxt * e_bytes, e_bytes, bar_e); }
+    }
+    if (half == 0) {
+      tmem_ld16(tlane + COL_C3, v);
+      tmem_ld_wait();
+      if (valid) {
 #pragma unroll
-      for (int c = 0; c < 3; ++c) ws.rgb[3 * s + c] = 1.f / (1.f + expf(-v[c]));
+        for (int c = 0; c < 3; ++c) ws.rgb[3 * s + c] = 1.f / (1.f + expf(-v[c]));
+      }
     }
     fence_before();
+    __syncthreads();   // nobody may still be reading TMEM / writing buffers when the next tile's first MMA is issued
   }
   fence_before();
   __syncthreads();
@@ -353,14 +382,17 @@ __global__ void __launch_bounds__(128) mlp_forward_tc_kernel(MlpShape ms, const 
 // the end); thread r owns sample row r for dgrad and feature row r for wgrad.  The saved
 // activations X of the five layers arrive by TMA into two ping-pong buffers, one layer ahead.
 constexpr uint32_t COL_G = 0;                                   // dgrad result, reused per layer (<= 64 cols)
-constexpr uint32_t GW_C3 = 64, GW_C2 = 80, GW_C1 = 144, GW_D2 = 208, GW_D1 = 224, BWD_COLS = 512;
+// wgrad accumulators.  The first colour layer's is kept TRANSPOSED (rows = 64 outputs, 32 input columns), which
+// brings the total to 256 columns: two CTAs per SM.
+constexpr uint32_t GW_C3 = 64, GW_C2 = 80, GW_C1T = 144, GW_D2 = 176, GW_D1 = 192, BWD_COLS = 256;
+constexpr uint32_t BWD_THREADS = 256;
 
 struct BwdSmem {
   static constexpr uint32_t w = 0;                                // weight image (WImg backward region)
   static constexpr uint32_t bufX0 = w + WImg::b_total;            // [128][64]; the M=128 wgrad also reads the 16 KB after it
   static constexpr uint32_t bufX1 = bufX0 + ROWS * H * 2;         // [128][64]
   static constexpr uint32_t bufY = bufX1 + ROWS * H * 2;          // [128][64]
-  static constexpr uint32_t pad = bufY + ROWS * H * 2;            // 16 KB readable slack behind bufY's role as "after X1"
+  static constexpr uint32_t pad = bufY + ROWS * H * 2;            // 16 KB readable slack behind bufY (M=128 reads of a 64-column tile)
   static constexpr uint32_t bar_mma = pad + ROWS * H * 2;
   static constexpr uint32_t bar_w = bar_mma + 8;
   static constexpr uint32_t bar_x0 = bar_w + 8;
@@ -369,7 +401,7 @@ struct BwdSmem {
   static constexpr uint32_t total = tmem + 8;
 };
 
-// wgrad k-steps over the 128 samples: G[128 (feature i) x N (output o)] (+)= X^T dY
+// wgrad k-steps over the 128 samples: G[128 (columns of tile A) x N (columns of tile B)] (+)= A^T B
 __device__ __forceinline__ void issue_wgrad(uint32_t tmem_d, uint32_t x_saddr, uint32_t y_saddr, uint32_t N, uint32_t fmt,
                                             uint32_t accumulate) {
   const uint32_t idesc = make_idesc(fmt, 128, N, 1, 1);
@@ -380,52 +412,61 @@ __device__ __forceinline__ void issue_wgrad(uint32_t tmem_d, uint32_t x_saddr, u
   }
 }
 
-// ReLU mask of this thread's row of a [128][64] activation tile in shared memory
+// ReLU mask of columns [cb, cb+32) of this thread's row of a [128][64] activation tile in shared memory
 template <typename T>
-__device__ __forceinline__ uint64_t row_mask(const uint8_t *tile) {
-  uint64_t mask = 0;
+__device__ __forceinline__ uint32_t row_mask32(const uint8_t *tile, uint32_t row, uint32_t cb) {
+  uint32_t mask = 0;
 #pragma unroll
-  for (uint32_t p = 0; p < H / 8; ++p) {
-    const uint4 q = *reinterpret_cast<const uint4 *>(tile + p * PANEL + threadIdx.x * 16);
+  for (uint32_t p = 0; p < 4; ++p) {
+    const uint4 q = *reinterpret_cast<const uint4 *>(tile + (cb / 8 + p) * PANEL + row * 16);
     const uint32_t w[4] = {q.x, q.y, q.z, q.w};
 #pragma unroll
     for (int j = 0; j < 4; ++j) {
       const float2 f = unpack2<T>(w[j]);
-      if (f.x > 0.f) mask |= 1ull << (p * 8 + 2 * j);
-      if (f.y > 0.f) mask |= 1ull << (p * 8 + 2 * j + 1);
+      if (f.x > 0.f) mask |= 1u << (p * 8 + 2 * j);
+      if (f.y > 0.f) mask |= 1u << (p * 8 + 2 * j + 1);
     }
   }
   return mask;
 }
 
+// dgrad columns [cb, cb+32) of this thread's row -> ReLU-masked -> bufY
 template <typename T>
-__device__ __forceinline__ void masked_to_Y(uint32_t tlane, uint64_t mask, uint8_t *bufY) {
+__device__ __forceinline__ void masked_to_Y(uint32_t tlane, uint32_t mask, uint8_t *bufY, uint32_t row, uint32_t cb) {
   float v[16];
 #pragma unroll
-  for (uint32_t c0 = 0; c0 < H; c0 += 16) {
-    tmem_ld16(tlane + COL_G + c0, v);
+  for (uint32_t c0 = 0; c0 < 32; c0 += 16) {
+    tmem_ld16(tlane + COL_G + cb + c0, v);
     tmem_ld_wait();
 #pragma unroll
-    for (int j = 0; j < 16; ++j) v[j] = ((mask >> (c0 + j)) & 1ull) ? v[j] : 0.f;
-    emit16<T, false>(v, bufY, nullptr, c0, true);
+    for (int j = 0; j < 16; ++j) v[j] = ((mask >> (c0 + j)) & 1u) ? v[j] : 0.f;
+    emit16<T, false>(v, bufY, nullptr, row, cb + c0, true);
   }
 }
 
+// 8 warps per tile as in the forward kernel: warp w owns sample rows 32 (w & 3) .. +31 (TMEM lane quarter) and the
+// column half (w >> 2) of every 64-wide dgrad.
 template <typename T>
-__global__ void __launch_bounds__(128, 1) mlp_backward_tc_kernel(MlpShape ms, float *__restrict__ gradW, Workspace ws,
-                                                                 const uint32_t *__restrict__ d_S) {
+__global__ void __launch_bounds__(BWD_THREADS, 2) mlp_backward_tc_kernel(MlpShape ms, float *__restrict__ gradW, Workspace ws,
+                                                                        const uint32_t *__restrict__ d_S) {
   extern __shared__ __align__(1024) uint8_t smem[];
-  const uint32_t tid = threadIdx.x, warp = tid >> 5;
+  const uint32_t tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+  const uint32_t row = (warp & 3u) * 32u + lane, half = warp >> 2, cb = half * 32u;
   const uint32_t sbase = smem_u32(smem);
   const uint32_t bar_mma = sbase + BwdSmem::bar_mma, bar_w = sbase + BwdSmem::bar_w;
-  const uint32_t bar_x[2] = {sbase + BwdSmem::bar_x0, sbase + BwdSmem::bar_x1};
-  const uint32_t sX[2] = {sbase + BwdSmem::bufX0, sbase + BwdSmem::bufX1};
-  uint8_t *bufX[2] = {smem + BwdSmem::bufX0, smem + BwdSmem::bufX1};
+  // the two X buffers, selected arithmetically (indexing a two-element array by a runtime value goes to local memory)
+  auto bar_x = [&](uint32_t b) { return sbase + BwdSmem::bar_x0 + 8u * b; };
+  auto sX = [&](uint32_t b) { return sbase + BwdSmem::bufX0 + (ROWS * H * 2) * b; };
+  auto bufX = [&](uint32_t b) { return smem + BwdSmem::bufX0 + (ROWS * H * 2) * b; };
+  uint32_t ph_x0 = 0, ph_x1 = 0;
+  auto wait_x = [&](uint32_t b) {
+    if (b) { mbar_wait(bar_x(1), ph_x1); ph_x1 ^= 1; } else { mbar_wait(bar_x(0), ph_x0); ph_x0 ^= 1; }
+  };
   uint8_t *bufY = smem + BwdSmem::bufY;
   const uint32_t sY = sbase + BwdSmem::bufY, sW = sbase + BwdSmem::w;
   const uint32_t LF = ms.LF;
-  const uint64_t S = *d_S;
-  if ((uint64_t)blockIdx.x * ROWS >= S) return;   // CTA without tiles
+  const uint64_t S = *d_S;                         // from the marcher, several kernels back: safe before pdl_wait()
+  const bool has_tiles = (uint64_t)blockIdx.x * ROWS < S;
   const bool two = ms.n_color_layers == 2;
   const uint32_t hbytes = H * ROWS * 2, cbytes = CIP * ROWS * 2, ebytes = LF * ROWS * 2;
 
@@ -439,25 +480,34 @@ __global__ void __launch_bounds__(128, 1) mlp_backward_tc_kernel(MlpShape ms, fl
       case 3: src = ws.blob_hd + tile * hbytes; bytes = hbytes; break;
       default: src = ws.blob_e + tile * (2 * (size_t)ebytes); bytes = ebytes; break;   // the hi half of the two-term tile
     }
-    mbar_expect_tx(bar_x[buf], bytes);
-    bulk_g2s(sX[buf], src, bytes, bar_x[buf]);
+    mbar_expect_tx(bar_x(buf), bytes);
+    bulk_g2s(sX(buf), src, bytes, bar_x(buf));
   };
 
-  if (tid == 0) {
-    mbar_init(bar_mma, 1); mbar_init(bar_w, 1); mbar_init(bar_x[0], 1); mbar_init(bar_x[1], 1);
-    fence_async_smem();
-    mbar_expect_tx(bar_w, WImg::b_total);
-    bulk_g2s(sW, ws.wimg_bwd, WImg::b_total, bar_w);
-    load_x(0, 0, blockIdx.x);
-    load_x(two ? 1 : 2, 1, blockIdx.x);
+  if (has_tiles) {   // prologue on data that is at least two kernels old (weight image, the forward pass's saved activations)
+    if (tid == 0) {
+      mbar_init(bar_mma, 1); mbar_init(bar_w, 1); mbar_init(bar_x(0), 1); mbar_init(bar_x(1), 1);
+      fence_async_smem();
+      mbar_expect_tx(bar_w, WImg::b_total);
+      bulk_g2s(sW, ws.wimg_bwd, WImg::b_total, bar_w);
+      load_x(0, 0, blockIdx.x);
+      load_x(two ? 1 : 2, 1, blockIdx.x);
+    }
+    // the slack behind bufY is read as rows 64..127 of an M = 128 operand: keep it finite
+    for (uint32_t i = tid; i < ROWS * H * 2 / 16; i += BWD_THREADS)
+      reinterpret_cast<uint4 *>(smem + BwdSmem::pad)[i] = make_uint4(0, 0, 0, 0);
+    if (warp == 0) tmem_alloc<BWD_COLS>(sbase + BwdSmem::tmem);
   }
-  if (warp == 0) tmem_alloc<BWD_COLS>(sbase + BwdSmem::tmem);
+  pdl_wait();     // the compositor's dL/dsigma, dL/dc and gradient maximum
+  pdl_trigger();
+  if (!has_tiles) return;
+  fence_async_smem();
   fence_before();
   __syncthreads();
   fence_after();
   const uint32_t tmem_base = *reinterpret_cast<volatile uint32_t *>(smem + BwdSmem::tmem);
-  const uint32_t tlane = tmem_base + ((warp * 32u) << 16);
-  uint32_t ph_mma = 0, ph_x[2] = {0, 0};
+  const uint32_t tlane = tmem_base + (((warp & 3u) * 32u) << 16);
+  uint32_t ph_mma = 0;
   const uint32_t fmt = Fmt<T>::id;
 
   // loss scale (fp16 only): one power of two per step from the largest gradient entering S11
@@ -471,32 +521,34 @@ __global__ void __launch_bounds__(128, 1) mlp_backward_tc_kernel(MlpShape ms, fl
   if (tid == 0) mbar_wait(bar_w, 0);
 
   for (uint64_t tile = blockIdx.x; tile * ROWS < S; tile += gridDim.x) {
-    const uint64_t s = tile * ROWS + tid;
+    const uint64_t s = tile * ROWS + row;
     const bool valid = s < S;
     const uint64_t next_tile = tile + gridDim.x;
     const bool has_next = next_tile * ROWS < S;
     float v[16];
     uint32_t cur = 0;   // X buffer of the current layer; tiles always start with buffer 0
     // ---- colour output layer: dY = dL/dc * c (1 - c); X = last hidden activations
-#pragma unroll
-    for (int j = 0; j < 16; ++j) v[j] = 0.f;
     float sig = 0.f, dsig = 0.f;
-    if (valid) {
+    if (half == 0) {
 #pragma unroll
-      for (int c = 0; c < 3; ++c) {
-        const float col = ws.rgb[3 * s + c];
-        v[c] = ws.drgb[3 * s + c] * col * (1.f - col) * scale;
+      for (int j = 0; j < 16; ++j) v[j] = 0.f;
+      if (valid) {
+#pragma unroll
+        for (int c = 0; c < 3; ++c) {
+          const float col = ws.rgb[3 * s + c];
+          v[c] = ws.drgb[3 * s + c] * col * (1.f - col) * scale;
+        }
+        sig = ws.sigma[s];
+        dsig = ws.dsigma[s];
       }
-      sig = ws.sigma[s];
-      dsig = ws.dsigma[s];
+      emit16<T, false>(v, bufY, nullptr, row, 0, true);
     }
-    emit16<T, false>(v, bufY, nullptr, 0, true);
-    mbar_wait(bar_x[cur], ph_x[cur]); ph_x[cur] ^= 1;
-    uint64_t mask = row_mask<T>(bufX[cur]);
+    wait_x(cur);
+    uint32_t mask = row_mask32<T>(bufX(cur), row, cb);
     fence_async_smem(); fence_before(); __syncthreads();
     if (tid == 0) {
       fence_after();
-      issue_wgrad(tmem_base + GW_C3, sX[cur], sY, 16, fmt, acc);
+      issue_wgrad(tmem_base + GW_C3, sX(cur), sY, 16, fmt, acc);
       issue_layer(tmem_base + COL_G, sY, sW + WImg::b_c3, 16, H, H, fmt, bar_mma);
     }
     mbar_wait(bar_mma, ph_mma); ph_mma ^= 1; fence_after();
@@ -504,74 +556,73 @@ __global__ void __launch_bounds__(128, 1) mlp_backward_tc_kernel(MlpShape ms, fl
     cur ^= 1;
     // ---- second colour hidden layer
     if (two) {
-      masked_to_Y<T>(tlane, mask, bufY);
-      mbar_wait(bar_x[cur], ph_x[cur]); ph_x[cur] ^= 1;
-      mask = row_mask<T>(bufX[cur]);
+      masked_to_Y<T>(tlane, mask, bufY, row, cb);
+      wait_x(cur);
+      mask = row_mask32<T>(bufX(cur), row, cb);
       fence_async_smem(); fence_before(); __syncthreads();
       if (tid == 0) {
         fence_after();
-        issue_wgrad(tmem_base + GW_C2, sX[cur], sY, H, fmt, acc);
+        issue_wgrad(tmem_base + GW_C2, sX(cur), sY, H, fmt, acc);
         issue_layer(tmem_base + COL_G, sY, sW + WImg::b_c2, H, H, H, fmt, bar_mma);
       }
       mbar_wait(bar_mma, ph_mma); ph_mma ^= 1; fence_after();
       if (tid == 0) load_x(3, cur, tile);
       cur ^= 1;
     }
-    // ---- first colour layer: dY = d h1 (masked); X = [g slice, Y(d), 0]
-    masked_to_Y<T>(tlane, mask, bufY);
-    mbar_wait(bar_x[cur], ph_x[cur]); ph_x[cur] ^= 1;
+    // ---- first colour layer: dY = d h1 (masked); X = [g slice, Y(d), 0]; wgrad transposed: G^T = dY^T X
+    masked_to_Y<T>(tlane, mask, bufY, row, cb);
+    wait_x(cur);
     fence_async_smem(); fence_before(); __syncthreads();
     if (tid == 0) {
       fence_after();
-      issue_wgrad(tmem_base + GW_C1, sX[cur], sY, H, fmt, acc);
+      issue_wgrad(tmem_base + GW_C1T, sY, sX(cur), CIP, fmt, acc);
       issue_layer(tmem_base + COL_G, sY, sW + WImg::b_c1, H, CIP, CIP, fmt, bar_mma);
     }
     mbar_wait(bar_mma, ph_mma); ph_mma ^= 1; fence_after();
     if (tid == 0) load_x(4, cur, tile);
     cur ^= 1;
     // ---- density output layer: dg = [geo slice of d ci] + e_0 * dL/dsigma * sigma (0 where clamped)
-    {
+    if (half == 0) {
       float dci[CIP], dg[16];
       tmem_ld16(tlane + COL_G, dci);
       tmem_ld16(tlane + COL_G + 16, dci + 16);
       tmem_ld_wait();
 #pragma unroll
       for (int j = 0; j < 16; ++j) dg[j] = 0.f;
-      for (uint32_t j = 0; j < ms.geo_cnt; ++j) dg[ms.geo_off + j] = dci[j];
+#pragma unroll
+      for (int j = 0; j < 15; ++j) dg[1 + j] = dci[j];   // geo slice (1, 15), see mlp_tc_supported()
       // sigma = exp(clamp(g0, -15, 15)): the clamp is active iff sigma sits on a bound
       if (valid && sig > 3.0590232e-07f * 1.0001f && sig < 3269017.4f * 0.9999f) dg[0] += dsig * sig * scale;
-      emit16<T, false>(dg, bufY, nullptr, 0, true);
+      emit16<T, false>(dg, bufY, nullptr, row, 0, true);
     }
-    mbar_wait(bar_x[cur], ph_x[cur]); ph_x[cur] ^= 1;
-    mask = row_mask<T>(bufX[cur]);
+    wait_x(cur);
+    mask = row_mask32<T>(bufX(cur), row, cb);
     fence_async_smem(); fence_before(); __syncthreads();
     if (tid == 0) {
       fence_after();
-      issue_wgrad(tmem_base + GW_D2, sX[cur], sY, 16, fmt, acc);
+      issue_wgrad(tmem_base + GW_D2, sX(cur), sY, 16, fmt, acc);
       issue_layer(tmem_base + COL_G, sY, sW + WImg::b_d2, 16, H, H, fmt, bar_mma);
     }
     mbar_wait(bar_mma, ph_mma); ph_mma ^= 1; fence_after();
-    const uint32_t buf_hd = cur;
     cur ^= 1;
     // ---- density hidden layer: dY = d hd (masked); X = e
-    masked_to_Y<T>(tlane, mask, bufY);
-    mbar_wait(bar_x[cur], ph_x[cur]); ph_x[cur] ^= 1;
+    masked_to_Y<T>(tlane, mask, bufY, row, cb);
+    wait_x(cur);
     fence_async_smem(); fence_before(); __syncthreads();
     if (tid == 0) {
       fence_after();
-      issue_wgrad(tmem_base + GW_D1, sX[cur], sY, H, fmt, acc);
+      issue_wgrad(tmem_base + GW_D1, sX(cur), sY, H, fmt, acc);
       issue_layer(tmem_base + COL_G, sY, sW + WImg::b_d1, H, LF, LF, fmt, bar_mma);
     }
     mbar_wait(bar_mma, ph_mma); ph_mma ^= 1; fence_after();
-    // both X buffers are free: the next tile's first two layers.  The layer order leaves the
-    // buffers in the roles (cur = e, buf_hd = hd); the next tile starts again at buffer 0.
+    // both X buffers are free: the next tile's first two layers (tiles always start at buffer 0)
     if (tid == 0 && has_next) {
       load_x(0, 0, next_tile);
       load_x(two ? 1 : 2, 1, next_tile);
     }
-    (void)buf_hd;
-    // ---- dL/de -> planes
-    for (uint32_t c0 = 0; c0 < LF; c0 += 16) {
+    // ---- dL/de -> planes; each column half writes its LF/2 columns
+    const uint32_t ncol = LF / 2;
+    for (uint32_t c0 = half * ncol; c0 < (half + 1) * ncol; c0 += 16) {
       tmem_ld16(tlane + COL_G + c0, v);
       tmem_ld_wait();
       if (valid)
@@ -579,28 +630,40 @@ __global__ void __launch_bounds__(128, 1) mlp_backward_tc_kernel(MlpShape ms, fl
         for (int j = 0; j < 16; ++j) ws.de[(size_t)(c0 + j) * ws.cap + s] = v[j] * inv_scale;
     }
     fence_before();
+    __syncthreads();   // all reads of COL_G and writes of bufY are done before the next tile reuses them
     acc = 1;
   }
-  // ---- flush the CTA's weight gradients: thread i holds feature row i of every G = X^T dY
+  // ---- flush the CTA's weight gradients: thread (row i, column half) holds row i of every G
   fence_before();
   __syncthreads();
   fence_after();
+  // G[i][o] = dW[o][i]: rows = input features, ncols output columns
   auto flush = [&](uint32_t col, uint32_t g_off, uint32_t n_out, uint32_t n_in, uint32_t ncols) {
     float v[16];
-    for (uint32_t c0 = 0; c0 < ncols; c0 += 16) {
+    for (uint32_t c0 = half * 16; c0 < ncols; c0 += 32) {
       tmem_ld16(tlane + col + c0, v);
       tmem_ld_wait();
-      if (tid < n_in)
+      if (row < n_in)
 #pragma unroll
         for (int j = 0; j < 16; ++j) {
           const uint32_t o = c0 + j;
-          if (o < n_out && v[j] != 0.f) atomicAdd(gradW + g_off + o * n_in + tid, v[j] * inv_scale);
+          if (o < n_out && v[j] != 0.f) atomicAdd(gradW + g_off + o * n_in + row, v[j] * inv_scale);
         }
     }
   };
   flush(GW_C3, ms.o_c3, 3, H, 16);
   if (two) flush(GW_C2, ms.o_c2, H, H, H);
-  flush(GW_C1, ms.o_c1, H, ms.Ci, H);
+  {   // transposed accumulator: rows = outputs, columns = inputs
+    float v[16];
+    tmem_ld16(tlane + GW_C1T + half * 16, v);
+    tmem_ld_wait();
+    if (row < H)
+#pragma unroll
+      for (int j = 0; j < 16; ++j) {
+        const uint32_t i = half * 16 + j;
+        if (i < ms.Ci && v[j] != 0.f) atomicAdd(gradW + ms.o_c1 + row * ms.Ci + i, v[j] * inv_scale);
+      }
+  }
   flush(GW_D2, ms.o_d2, DO, H, 16);
   flush(GW_D1, ms.o_d1, H, LF, H);
   fence_before();
@@ -627,8 +690,9 @@ __global__ void blob_to_rows_kernel(const uint8_t *__restrict__ blob, uint32_t n
 }  // namespace
 
 bool mlp_tc_supported(const MlpShape &ms) {
-  return ms.Hd == H && ms.Hc == H && ms.Do == DO && ms.LF % 16 == 0 && ms.LF >= 16 && ms.LF <= 64 && ms.Ci <= CIP &&
-         ms.n_sh <= 16 && ms.geo_off + ms.geo_cnt <= DO;
+  // the widths of configs 2-5; other shapes run on the fp32 CUDA-core kernels (mlp_simt.cu)
+  return ms.Hd == H && ms.Hc == H && ms.Do == DO && ms.LF % 16 == 0 && ms.LF >= 16 && ms.LF <= 64 && ms.n_sh == 16 &&
+         ms.geo_off == 1 && ms.geo_cnt == 15;
 }
 
 size_t mlp_tc_wimg_bytes(int backward) { return backward ? WImg::b_total : 2 * WImg::f_total; }
@@ -642,8 +706,8 @@ int launch_pack_weights(const MlpShape &ms, int bf16, const float *theta_mlp, co
 int launch_adam_mlp_pack(const MlpShape &ms, int bf16, const FieldParams &fp, const Workspace &ws, const AdamConst &c,
                          cudaStream_t st) {
   const unsigned grid = (ms.n_mlp + 127) / 128;
-  if (bf16) adam_pack_kernel<__nv_bfloat16><<<grid, 128, 0, st>>>(ms, fp.mlp_theta, fp.mlp_m, fp.mlp_v, fp.mlp_grad, ws.wimg_fwd, ws.wimg_bwd, c);
-  else adam_pack_kernel<__half><<<grid, 128, 0, st>>>(ms, fp.mlp_theta, fp.mlp_m, fp.mlp_v, fp.mlp_grad, ws.wimg_fwd, ws.wimg_bwd, c);
+  if (bf16) launch_pdl(adam_pack_kernel<__nv_bfloat16>, dim3(grid), dim3(128), 0, st, ms, fp.mlp_theta, fp.mlp_m, fp.mlp_v, fp.mlp_grad, ws.wimg_fwd, ws.wimg_bwd, c);
+  else launch_pdl(adam_pack_kernel<__half>, dim3(grid), dim3(128), 0, st, ms, fp.mlp_theta, fp.mlp_m, fp.mlp_v, fp.mlp_grad, ws.wimg_fwd, ws.wimg_bwd, c);
   return 1;
 }
 
@@ -651,11 +715,13 @@ int launch_mlp_forward_tc(const MlpShape &ms, int bf16, const float *dirs, const
                           int density_only, int save_blobs, int n_sms, cudaStream_t st) {
   const size_t smem = FwdSmem::total;
   if (bf16) {
-    cudaFuncSetAttribute(mlp_forward_tc_kernel<__nv_bfloat16>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    mlp_forward_tc_kernel<__nv_bfloat16><<<2 * n_sms, 128, smem, st>>>(ms, dirs, ws, d_S, density_only, save_blobs);
+    static const cudaError_t once = cudaFuncSetAttribute(mlp_forward_tc_kernel<__nv_bfloat16>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    (void)once;
+    launch_pdl(mlp_forward_tc_kernel<__nv_bfloat16>, dim3(2 * n_sms), dim3(FWD_THREADS), smem, st, ms, dirs, ws, d_S, density_only, save_blobs);
   } else {
-    cudaFuncSetAttribute(mlp_forward_tc_kernel<__half>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    mlp_forward_tc_kernel<__half><<<2 * n_sms, 128, smem, st>>>(ms, dirs, ws, d_S, density_only, save_blobs);
+    static const cudaError_t once = cudaFuncSetAttribute(mlp_forward_tc_kernel<__half>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    (void)once;
+    launch_pdl(mlp_forward_tc_kernel<__half>, dim3(2 * n_sms), dim3(FWD_THREADS), smem, st, ms, dirs, ws, d_S, density_only, save_blobs);
   }
   return 1;
 }
@@ -664,11 +730,13 @@ int launch_mlp_backward_tc(const MlpShape &ms, int bf16, float *grad_mlp, const 
                            int n_sms, cudaStream_t st) {
   const size_t smem = BwdSmem::total;
   if (bf16) {
-    cudaFuncSetAttribute(mlp_backward_tc_kernel<__nv_bfloat16>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    mlp_backward_tc_kernel<__nv_bfloat16><<<n_sms, 128, smem, st>>>(ms, grad_mlp, ws, d_S);
+    static const cudaError_t once = cudaFuncSetAttribute(mlp_backward_tc_kernel<__nv_bfloat16>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    (void)once;
+    launch_pdl(mlp_backward_tc_kernel<__nv_bfloat16>, dim3(2 * n_sms), dim3(BWD_THREADS), smem, st, ms, grad_mlp, ws, d_S);
   } else {
-    cudaFuncSetAttribute(mlp_backward_tc_kernel<__half>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    mlp_backward_tc_kernel<__half><<<n_sms, 128, smem, st>>>(ms, grad_mlp, ws, d_S);
+    static const cudaError_t once = cudaFuncSetAttribute(mlp_backward_tc_kernel<__half>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    (void)once;
+    launch_pdl(mlp_backward_tc_kernel<__half>, dim3(2 * n_sms), dim3(BWD_THREADS), smem, st, ms, grad_mlp, ws, d_S);
   }
   return 1;
 }

@@ -37,6 +37,16 @@ nsm_status fail(nsm_status st, const char *fmt, ...) {
 
 }  // namespace
 
+// Default: every hot-path kernel except the marcher (bit 0) and the scatter (bit 5).  Measured on B200 at
+// config 2 (profiles/r1g_pdl_sweep.md): 148.7 us/step without PDL, 135.5 us with this mask; letting the
+// table Adam's blocks become resident under the scatter, or the marcher's under the MLP Adam, costs
+// more than the launch gap it hides (149 us / 184 us).
+uint32_t g_pdl_mask = [] {
+  const char *e = std::getenv("NSM_PDL_MASK");
+  return e ? (uint32_t)std::strtoul(e, nullptr, 0) : 0xdeu;
+}();
+int g_cur_kernel = 0;
+
 static const char *kKernelNames[K_COUNT] = {"march", "encode", "mlp_fwd", "composite",
                                             "mlp_bwd", "scatter", "adam_table", "adam_mlp", "occupancy", "debug"};
 
@@ -178,6 +188,7 @@ nsm_status validate_batch(const nsm_field *f, const nsm_ray_batch *b, bool train
 // launch one kernel class, counted and (optionally) timed
 #define RUN(f, id, call)                                                    \
   do {                                                                      \
+    g_cur_kernel = (id);                                                    \
     if ((f)->prof.on) {                                                     \
       Profiler::Rec r_{id, (f)->prof.get(), (f)->prof.get()};               \
       cudaEventRecord(r_.a, (f)->stream);                                   \
