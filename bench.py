@@ -289,6 +289,9 @@ def run_cuda(args):
     f.nsm_set_params(theta0)
     if w.bits is not None:
         f.nsm_update_occupancy(nsm.NSM_OCC_SET, w.bits)
+    # the batches below are generated and uploaded before the timed region and never modified: declare them
+    # ready, so the marcher of step i+1 may run beside the table update of step i (include/nsm.h)
+    f.nsm_set_option(nsm.NSM_OPT_BATCH_READY, 1)
     refresh = 16 if cfg == 3 else 0          # config 3: occupancy FROM_FIELD every 16 steps (inside the timed region)
     dbatches = [nsm.DeviceBatch(b, dev) for b in w.batches]
     hbatches = [nsm.HostBatch(b) for b in w.batches]

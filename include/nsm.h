@@ -142,6 +142,15 @@ nsm_status nsm_train_step(nsm_field *f, const nsm_ray_batch *batch, float lambda
 nsm_status nsm_train_step_host(nsm_field *f, const nsm_ray_batch *host_batch, float lambda_d,
                                nsm_step_stats *host_stats);
 
+/* Options.
+ * NSM_OPT_BATCH_READY (default 0).  With 0 the library reads a batch strictly in the order of the field's
+ * stream.  With 1 the caller declares that the device buffers of every batch handed to nsm_train_step are
+ * complete when the call is made (e.g. a pre-staged keyframe store) and stay unmodified until the step has
+ * run: the library may then march the batch (S1-S3 read origins/dirs only) on an internal stream BESIDE the
+ * previous step's table update, ahead of work queued earlier on the field's stream.  Results are identical. */
+typedef enum { NSM_OPT_BATCH_READY = 0 } nsm_option;
+nsm_status nsm_set_option(nsm_field *f, nsm_option opt, uint32_t value);
+
 /* S1-S12 only: forward + backward, gradients left in place for nsm_debug_last_step; and S13
  * alone on the gradients in place.  nsm_train_step == nsm_backward + nsm_apply_adam. */
 nsm_status nsm_backward(nsm_field *f, const nsm_ray_batch *batch, float lambda_d,

@@ -16,6 +16,7 @@ LIB_PATH = os.path.join(_HERE, "libnsm.so")
 NSM_OK, NSM_ERR_INVALID_ARG, NSM_ERR_OOM, NSM_ERR_CUDA, NSM_ERR_CAPACITY, NSM_ERR_UNIMPLEMENTED = range(6)
 NSM_MLP_FP32, NSM_MLP_FP16, NSM_MLP_BF16 = 0, 1, 2
 NSM_OCC_FULL, NSM_OCC_SET, NSM_OCC_FROM_FIELD = 0, 1, 2
+NSM_OPT_BATCH_READY = 0
 
 DEBUG_ITEMS = dict(counts=(0, np.uint32), offsets=(1, np.uint32), s_ray=(2, np.uint32), s_k=(3, np.uint32),
                    s_t=(4, np.float32), s_delta=(5, np.float32), s_x=(6, np.float32), slots=(7, np.uint32),
@@ -26,7 +27,7 @@ DEBUG_ITEMS = dict(counts=(0, np.uint32), offsets=(1, np.uint32), s_ray=(2, np.u
 EXPORTS = ["nsm_create_field", "nsm_destroy_field", "nsm_update_occupancy", "nsm_get_occupancy",
            "nsm_train_step", "nsm_train_step_host", "nsm_backward", "nsm_apply_adam", "nsm_debug_set_grad",
            "nsm_render", "nsm_render_host", "nsm_param_count", "nsm_get_params", "nsm_set_params",
-           "nsm_get_level_table", "nsm_debug_last_step", "nsm_total_samples", "nsm_profile",
+           "nsm_get_level_table", "nsm_debug_last_step", "nsm_total_samples", "nsm_profile", "nsm_set_option",
            "nsm_profile_read", "nsm_launch_count", "nsm_mlp_path",
            "nsm_last_error", "nsm_version"]
 
@@ -91,6 +92,7 @@ def load_library():
         L.nsm_debug_last_step.argtypes = [vp, C.c_int, vp, C.c_uint64, u64p]
         L.nsm_total_samples.argtypes = [vp, u64p]
         L.nsm_profile.argtypes = [vp, C.c_int]
+        L.nsm_set_option.argtypes = [vp, C.c_int, C.c_uint32]
         L.nsm_profile_read.argtypes = [vp, C.c_uint32, C.POINTER(C.c_char_p), C.POINTER(C.c_double), u64p, u32p]
         L.nsm_launch_count.argtypes = [vp]
         L.nsm_launch_count.restype = C.c_uint64
@@ -328,6 +330,9 @@ class Field:
         n = C.c_uint64()
         _check(self.lib.nsm_total_samples(self.h, C.byref(n)))
         return int(n.value)
+
+    def nsm_set_option(self, opt, value):
+        _check(self.lib.nsm_set_option(self.h, int(opt), int(value)))
 
     def nsm_profile(self, enable):
         _check(self.lib.nsm_profile(self.h, int(bool(enable))))

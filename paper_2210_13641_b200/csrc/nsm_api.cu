@@ -98,6 +98,13 @@ struct nsm_field {
   float *stage_dev = nullptr;     // [max_rays * 11]
   float *stage_out = nullptr;     // render outputs [max_rays * 5]
   struct HostStats { double acc[2]; uint32_t S; } *pinned = nullptr;
+  // Side stream: work that does not depend on the table Adam runs beside it (it is DRAM-bound, the others
+  // are latency-bound): the MLP Adam of the same step and, when the caller has declared its batches ready
+  // (NSM_OPT_BATCH_READY), the marcher of the NEXT step.  ev_pre_adam marks "scatter of the last step done".
+  cudaStream_t side = nullptr;
+  cudaEvent_t ev_pre_adam = nullptr, ev_side = nullptr, ev_main = nullptr;
+  bool batch_ready = false;   // NSM_OPT_BATCH_READY
+  bool side_ok = false;       // nothing but a train step's Adam has been enqueued on `stream` since ev_pre_adam
   const char *mlp_path = "simt_fp32";
   bool use_tc = false;   // tcgen05 MLP kernels (16-bit configurations with supported shapes)
 
@@ -186,14 +193,15 @@ nsm_status validate_batch(const nsm_field *f, const nsm_ray_batch *b, bool train
 }
 
 // launch one kernel class, counted and (optionally) timed
-#define RUN(f, id, call)                                                    \
+#define RUN(f, id, call) RUN_ON(f, id, (f)->stream, call)
+#define RUN_ON(f, id, st_, call)                                            \
   do {                                                                      \
     g_cur_kernel = (id);                                                    \
     if ((f)->prof.on) {                                                     \
       Profiler::Rec r_{id, (f)->prof.get(), (f)->prof.get()};               \
-      cudaEventRecord(r_.a, (f)->stream);                                   \
+      cudaEventRecord(r_.a, (st_));                                         \
       int n_ = (call);                                                      \
-      cudaEventRecord(r_.b, (f)->stream);                                   \
+      cudaEventRecord(r_.b, (st_));                                         \
       (f)->prof.pending.push_back(r_);                                      \
       (f)->launches += n_; (f)->launches_by[id] += n_;                      \
     } else {                                                                \
@@ -218,10 +226,23 @@ MarchParams make_march(const nsm_field *f, const nsm_ray_batch *b, uint32_t R, b
 }
 
 // S1-S8 forward (+ S9-S12 when train): everything up to, but excluding, Adam.
-void enqueue_forward(nsm_field *f, const nsm_ray_batch *b, uint32_t R, bool jitter, uint32_t step, bool train) {
+// march_on_side: the marcher runs on the side stream, behind "scatter of the previous step done" only,
+// i.e. beside the previous step's table Adam (NSM_OPT_BATCH_READY; training steps only).
+void enqueue_forward(nsm_field *f, const nsm_ray_batch *b, uint32_t R, bool jitter, uint32_t step, bool train,
+                     bool march_on_side = false) {
   const uint32_t *d_S = f->ws.offsets + R;
   MarchParams mp = make_march(f, b, R, jitter, step);
-  RUN(f, K_MARCH, launch_march(mp, f->occ_full ? nullptr : f->fp.occ_bits, b->origins, b->dirs, f->ws, train ? 1 : 0, f->stream));
+  if (march_on_side && !f->prof.on) {
+    if (!f->side_ok) {   // other work has been enqueued on the main stream since the last Adam: order behind all of it
+      cudaEventRecord(f->ev_main, f->stream);
+      cudaStreamWaitEvent(f->side, f->ev_main, 0);
+    }
+    RUN_ON(f, K_MARCH, f->side, launch_march(mp, f->occ_full ? nullptr : f->fp.occ_bits, b->origins, b->dirs, f->ws, train ? 1 : 0, f->side));
+    cudaEventRecord(f->ev_side, f->side);
+    cudaStreamWaitEvent(f->stream, f->ev_side, 0);
+  } else {
+    RUN(f, K_MARCH, launch_march(mp, f->occ_full ? nullptr : f->fp.occ_bits, b->origins, b->dirs, f->ws, train ? 1 : 0, f->stream));
+  }
   const int bf16 = f->cfg.mlp_precision == NSM_MLP_BF16;
   RUN(f, K_ENCODE, launch_encode(f->lv, f->fp.rec, f->ws, d_S, f->use_tc ? 1 + bf16 : 0, f->n_sms, f->stream));
   if (f->use_tc)
@@ -245,12 +266,13 @@ nsm_status clear_grads_if_dirty(nsm_field *f) {
   return NSM_OK;
 }
 
-nsm_status enqueue_backward(nsm_field *f, const nsm_ray_batch *b, float lambda_d) {
+nsm_status enqueue_backward(nsm_field *f, const nsm_ray_batch *b, float lambda_d, bool march_on_side = false) {
   const uint32_t R = b->n_rays;
   const uint32_t *d_S = f->ws.offsets + R;
   nsm_status st = clear_grads_if_dirty(f);
   if (st != NSM_OK) return st;
-  enqueue_forward(f, b, R, f->cfg.jitter != 0, f->step + 1, true);
+  enqueue_forward(f, b, R, f->cfg.jitter != 0, f->step + 1, true, march_on_side);
+  f->side_ok = false;
   RUN(f, K_COMPOSITE, launch_composite_train(f->ws, R, b->rgb, b->depth, b->depth_var, lambda_d, f->cfg.bg, f->stream));
   if (f->use_tc)
     RUN(f, K_MLP_BWD, launch_mlp_backward_tc(f->ms, f->cfg.mlp_precision == NSM_MLP_BF16, f->fp.mlp_grad, f->ws, d_S,
@@ -271,14 +293,26 @@ nsm_status enqueue_adam(nsm_field *f) {
   const uint32_t t = f->step + 1;
   const double bc1 = 1.0 - std::pow((double)f->cfg.beta1, (double)t);
   const double bc2 = 1.0 - std::pow((double)f->cfg.beta2, (double)t);
-  RUN(f, K_ADAM_TABLE, launch_adam_table(f->fp, f->cfg.n_features, f->cfg.sparse_table_adam != 0, f->cfg.lr, f->cfg.beta1,
-                                         f->cfg.beta2, f->cfg.eps, (float)(1.0 / bc1), (float)(1.0 / bc2), f->n_sms, f->stream));
+  // the MLP Adam (9-11 K weights + the 16-bit image refresh) runs on the side stream beside the table Adam
+  const bool use_side = !f->prof.on;
+  cudaStream_t s_mlp = use_side ? f->side : f->stream;
+  if (use_side) {
+    cudaEventRecord(f->ev_pre_adam, f->stream);
+    cudaStreamWaitEvent(f->side, f->ev_pre_adam, 0);
+  }
   if (f->use_tc) {
     const AdamConst c{f->cfg.lr, f->cfg.beta1, f->cfg.beta2, f->cfg.eps, (float)(1.0 / bc1), (float)(1.0 / bc2)};
-    RUN(f, K_ADAM_MLP, launch_adam_mlp_pack(f->ms, f->cfg.mlp_precision == NSM_MLP_BF16, f->fp, f->ws, c, f->stream));
+    RUN_ON(f, K_ADAM_MLP, s_mlp, launch_adam_mlp_pack(f->ms, f->cfg.mlp_precision == NSM_MLP_BF16, f->fp, f->ws, c, s_mlp));
   } else {
-    RUN(f, K_ADAM_MLP, launch_adam_mlp(f->fp, f->cfg.lr, f->cfg.beta1, f->cfg.beta2, f->cfg.eps, (float)(1.0 / bc1),
-                                       (float)(1.0 / bc2), f->stream));
+    RUN_ON(f, K_ADAM_MLP, s_mlp, launch_adam_mlp(f->fp, f->cfg.lr, f->cfg.beta1, f->cfg.beta2, f->cfg.eps, (float)(1.0 / bc1),
+                                                 (float)(1.0 / bc2), s_mlp));
+  }
+  RUN(f, K_ADAM_TABLE, launch_adam_table(f->fp, f->cfg.n_features, f->cfg.sparse_table_adam != 0, f->cfg.lr, f->cfg.beta1,
+                                         f->cfg.beta2, f->cfg.eps, (float)(1.0 / bc1), (float)(1.0 / bc2), f->n_sms, f->stream));
+  if (use_side) {   // join: everything later on the main stream sees the new MLP weights
+    cudaEventRecord(f->ev_side, f->side);
+    cudaStreamWaitEvent(f->stream, f->ev_side, 0);
+    f->side_ok = true;
   }
   f->step = t;
   if (f->prof.on) f->prof.collect();
@@ -413,6 +447,14 @@ nsm_status nsm_create_field(const nsm_field_config *cfg, void *cuda_stream, nsm_
   A(f->alloc(&ws.loss_acc, 2)); A(f->alloc(&ws.total_samples, 1)); A(f->alloc(&ws.grad_absmax, 1));
   A(f->alloc(&f->stage_dev, 11 * (size_t)R)); A(f->alloc(&f->stage_out, 5 * (size_t)R));
   if (e == cudaSuccess) e = cudaMallocHost((void **)&f->pinned, sizeof(*f->pinned));
+  if (e == cudaSuccess) {   // highest priority: the side stream's small grids must not queue behind the table Adam's 3000 blocks
+    int prio_lo = 0, prio_hi = 0;
+    cudaDeviceGetStreamPriorityRange(&prio_lo, &prio_hi);
+    e = cudaStreamCreateWithPriority(&f->side, cudaStreamNonBlocking, prio_hi);
+  }
+  if (e == cudaSuccess) e = cudaEventCreateWithFlags(&f->ev_pre_adam, cudaEventDisableTiming);
+  if (e == cudaSuccess) e = cudaEventCreateWithFlags(&f->ev_side, cudaEventDisableTiming);
+  if (e == cudaSuccess) e = cudaEventCreateWithFlags(&f->ev_main, cudaEventDisableTiming);
   if (e != cudaSuccess) {
     nsm_destroy_field(f);
     cudaGetLastError();
@@ -427,6 +469,10 @@ nsm_status nsm_create_field(const nsm_field_config *cfg, void *cuda_stream, nsm_
 void nsm_destroy_field(nsm_field *f) {
   if (!f) return;
   cudaStreamSynchronize(f->stream);
+  if (f->side) { cudaStreamSynchronize(f->side); cudaStreamDestroy(f->side); }
+  if (f->ev_pre_adam) cudaEventDestroy(f->ev_pre_adam);
+  if (f->ev_side) cudaEventDestroy(f->ev_side);
+  if (f->ev_main) cudaEventDestroy(f->ev_main);
   f->prof.destroy();
   for (void *p : f->allocs) cudaFree(p);
   if (f->pinned) cudaFreeHost(f->pinned);
@@ -483,6 +529,7 @@ nsm_status nsm_get_level_table(const nsm_field *f, uint32_t *res, uint64_t *offs
 
 nsm_status nsm_get_params(nsm_field *f, float *d_theta, float *d_m, float *d_v, uint32_t *step) {
   if (!f) return fail(NSM_ERR_INVALID_ARG, "field is NULL");
+  f->side_ok = false;
   const size_t mb = sizeof(float) * f->fp.n_mlp;
   float *dst[3] = {d_theta, d_m, d_v};
   const float *mlp[3] = {f->fp.mlp_theta, f->fp.mlp_m, f->fp.mlp_v};
@@ -499,6 +546,7 @@ nsm_status nsm_get_params(nsm_field *f, float *d_theta, float *d_m, float *d_v, 
 
 nsm_status nsm_set_params(nsm_field *f, const float *d_theta, const float *d_m, const float *d_v, uint32_t step) {
   if (!f) return fail(NSM_ERR_INVALID_ARG, "field is NULL");
+  f->side_ok = false;
   const size_t mb = sizeof(float) * f->fp.n_mlp;
   const float *src[3] = {d_theta, d_m, d_v};
   float *mlp[3] = {f->fp.mlp_theta, f->fp.mlp_m, f->fp.mlp_v};
@@ -516,6 +564,7 @@ nsm_status nsm_set_params(nsm_field *f, const float *d_theta, const float *d_m, 
 
 nsm_status nsm_get_occupancy(nsm_field *f, uint8_t *d_bits) {
   if (!f || !d_bits) return fail(NSM_ERR_INVALID_ARG, "NULL argument");
+  f->side_ok = false;
   const uint64_t G3 = (uint64_t)f->cfg.occ_res * f->cfg.occ_res * f->cfg.occ_res;
   if (f->occ_full) CUDA_TRY(cudaMemsetAsync(d_bits, 0xff, (G3 + 7) / 8, f->stream));
   else CUDA_TRY(cudaMemcpyAsync(d_bits, f->fp.occ_bits, (G3 + 7) / 8, cudaMemcpyDeviceToDevice, f->stream));
@@ -524,6 +573,7 @@ nsm_status nsm_get_occupancy(nsm_field *f, uint8_t *d_bits) {
 
 nsm_status nsm_update_occupancy(nsm_field *f, nsm_occ_mode mode, const uint8_t *d_bits) {
   if (!f) return fail(NSM_ERR_INVALID_ARG, "field is NULL");
+  f->side_ok = false;
   const uint64_t G3 = (uint64_t)f->cfg.occ_res * f->cfg.occ_res * f->cfg.occ_res;
   switch (mode) {
     case NSM_OCC_FULL:
@@ -574,10 +624,11 @@ nsm_status nsm_apply_adam(nsm_field *f) {
   return enqueue_adam(f);
 }
 
-nsm_status nsm_train_step(nsm_field *f, const nsm_ray_batch *batch, float lambda_d, nsm_step_stats *host_stats) {
+static nsm_status train_step_impl(nsm_field *f, const nsm_ray_batch *batch, float lambda_d, nsm_step_stats *host_stats,
+                                  bool batch_ready) {
   nsm_status st = validate_batch(f, batch, true, false);
   if (st != NSM_OK) return st;
-  st = enqueue_backward(f, batch, lambda_d);
+  st = enqueue_backward(f, batch, lambda_d, batch_ready);
   if (st != NSM_OK) return st;
   st = enqueue_adam(f);
   if (st != NSM_OK) return st;
@@ -586,19 +637,32 @@ nsm_status nsm_train_step(nsm_field *f, const nsm_ray_batch *batch, float lambda
   return st;
 }
 
+nsm_status nsm_train_step(nsm_field *f, const nsm_ray_batch *batch, float lambda_d, nsm_step_stats *host_stats) {
+  return train_step_impl(f, batch, lambda_d, host_stats, f && f->batch_ready);
+}
+
 nsm_status nsm_train_step_host(nsm_field *f, const nsm_ray_batch *hb, float lambda_d, nsm_step_stats *host_stats) {
   nsm_status st = validate_batch(f, hb, true, false);
   if (st != NSM_OK) return st;
+  f->side_ok = false;   // the staging copies go through the main stream
   nsm_ray_batch db;
   st = stage_batch(f, hb, 0, hb->n_rays, true, &db);
   if (st != NSM_OK) return st;
   nsm_step_stats local;
-  st = nsm_train_step(f, &db, lambda_d, host_stats ? host_stats : &local);  // always syncs: host buffers may be reused
-  return st;
+  return train_step_impl(f, &db, lambda_d, host_stats ? host_stats : &local, false);  // always syncs: host buffers may be reused
+}
+
+nsm_status nsm_set_option(nsm_field *f, nsm_option opt, uint32_t value) {
+  if (!f) return fail(NSM_ERR_INVALID_ARG, "field is NULL");
+  switch (opt) {
+    case NSM_OPT_BATCH_READY: f->batch_ready = value != 0; f->side_ok = false; return NSM_OK;
+  }
+  return fail(NSM_ERR_INVALID_ARG, "unknown option %d", (int)opt);
 }
 
 nsm_status nsm_debug_set_grad(nsm_field *f, const float *d_grad, const uint8_t *d_touched) {
   if (!f) return fail(NSM_ERR_INVALID_ARG, "field is NULL");
+  f->side_ok = false;
   if (!d_grad) return fail(NSM_ERR_INVALID_ARG, "d_grad is NULL");
   RUN(f, K_DEBUG, launch_set_grad(f->fp, d_grad, d_touched, f->stream));
   CUDA_TRY(cudaMemcpyAsync(f->fp.mlp_grad, d_grad + f->fp.n_table, sizeof(float) * f->fp.n_mlp, cudaMemcpyDeviceToDevice, f->stream));
@@ -610,6 +674,7 @@ static nsm_status render_chunks(nsm_field *f, const nsm_ray_batch *b, float cut,
                                 bool host) {
   nsm_status st = validate_batch(f, b, false, true);
   if (st != NSM_OK) return st;
+  f->side_ok = false;
   if (!rgb || !depth) return fail(NSM_ERR_INVALID_ARG, "output pointers are NULL");
   if (!(cut >= 0.f)) return fail(NSM_ERR_INVALID_ARG, "transmittance_cut must be >= 0");
   const uint32_t M = f->cfg.max_rays;
@@ -653,6 +718,7 @@ nsm_status nsm_render_host(nsm_field *f, const nsm_ray_batch *hb, float cut, flo
 
 nsm_status nsm_debug_last_step(nsm_field *f, int item, void *d_out, uint64_t capacity_bytes, uint64_t *n_bytes_out) {
   if (!f) return fail(NSM_ERR_INVALID_ARG, "field is NULL");
+  f->side_ok = false;
   if (f->last_R == 0) return fail(NSM_ERR_INVALID_ARG, "no step has been run yet");
   const uint32_t R = f->last_R;
   const uint32_t *d_S = f->ws.offsets + R;

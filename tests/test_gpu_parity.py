@@ -360,3 +360,27 @@ def test_loss_decreases_over_training(nsm):
     losses = [f.nsm_train_step(nsm.DeviceBatch(b), w.lambda_d)["loss_rgb"] for b in w.batches]
     assert np.mean(losses[-10:]) < 0.5 * np.mean(losses[:5]), (losses[:5], losses[-10:])
     f.close()
+
+
+def test_batch_ready_option_gives_the_same_steps(nsm):
+    """NSM_OPT_BATCH_READY only moves the marcher (and the MLP Adam) to the internal side stream: sample counts are
+    identical and losses agree to atomic-order noise, also across an occupancy update between steps."""
+    w = configs.config3(R=2048, K=128, n_keyframes=3, n_batches=8, width=300, height=170)
+    fa, _, _ = make_pair(nsm, w, seed=9, table_scale=0.05)
+    fb, _, _ = make_pair(nsm, w, seed=9, table_scale=0.05)
+    fb.nsm_set_option(nsm.NSM_OPT_BATCH_READY, 1)
+    dba = [nsm.DeviceBatch(b) for b in w.batches]
+    for i in range(16):
+        if i == 9:
+            fa.nsm_update_occupancy(nsm.NSM_OCC_SET, w.extra["bits_alt"]) if "bits_alt" in w.extra else fa.nsm_update_occupancy(nsm.NSM_OCC_FULL)
+            fb.nsm_update_occupancy(nsm.NSM_OCC_SET, w.extra["bits_alt"]) if "bits_alt" in w.extra else fb.nsm_update_occupancy(nsm.NSM_OCC_FULL)
+        want = i % 5 == 4                      # most steps run without a host sync, so that they overlap
+        sa = fa.nsm_train_step(dba[i % 8], w.lambda_d, want_stats=want)
+        sb = fb.nsm_train_step(dba[i % 8], w.lambda_d, want_stats=want)
+        if want:
+            assert sa["n_samples"] == sb["n_samples"] and sa["step"] == sb["step"] == i + 1
+            assert abs(sa["loss"] - sb["loss"]) <= 2e-3 * abs(sa["loss"]), (i, sa["loss"], sb["loss"])
+    assert fa.nsm_total_samples() == fb.nsm_total_samples()
+    ca, cb = fa.nsm_debug_last_step("counts"), fb.nsm_debug_last_step("counts")
+    assert np.array_equal(ca, cb)
+    fa.close(); fb.close()
