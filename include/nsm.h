@@ -21,9 +21,12 @@
  *     HOST pointers instead and perform the copies themselves.  The library never retains a
  *     caller pointer past the call.
  *   - The field owns parameters, Adam state, occupancy bits and workspace.
- *   - All work is enqueued on the CUDA stream given at creation; calls return without
- *     synchronising unless a host stats pointer is passed (one sync to fill it) or the entry
- *     point takes host buffers.
+ *   - All work is enqueued on the CUDA stream given at creation (plus an internal side stream that
+ *     is joined back into it before the call returns); calls return without waiting unless a host
+ *     stats pointer is passed or the entry point takes host buffers.  Such a call waits until the
+ *     step's statistics are final and its inputs have been consumed (end of S9, the loss) -- NOT
+ *     until the backward pass and Adam (S10-S13) have run: those stay queued on the stream, and every
+ *     later call is ordered behind them.
  *   - Every entry point returns an nsm_status; nsm_last_error() gives a thread-local message.
  *     Arguments are validated before anything is launched: a failed call leaves the field
  *     unchanged.  There is no CPU fallback: without a CUDA device nsm_create_field fails with
@@ -138,7 +141,9 @@ nsm_status nsm_get_occupancy(nsm_field *f, uint8_t *d_bits);
  * (Eqs. 5, 6), loss (Eqs. 3, 4, 7), backward, Adam.  host_stats may be NULL (no sync). */
 nsm_status nsm_train_step(nsm_field *f, const nsm_ray_batch *batch, float lambda_d,
                           nsm_step_stats *host_stats);
-/* The same with HOST pointers in *batch: inputs are copied host->device inside the call. */
+/* The same with HOST pointers in *batch.  Pinned (page-locked) buffers are read in place by the kernels over
+ * the host link -- each input is needed once per ray -- and pageable ones are staged with host-to-device
+ * copies.  Always waits for the end of S9 (host_stats may still be NULL): the host buffers are free on return. */
 nsm_status nsm_train_step_host(nsm_field *f, const nsm_ray_batch *host_batch, float lambda_d,
                                nsm_step_stats *host_stats);
 

@@ -162,14 +162,15 @@ class DeviceBatch:
 
 
 class HostBatch:
-    """A ray batch in pinned host memory, for the *_host entry points."""
+    """A ray batch in host memory for the *_host entry points: pinned (read in place by the kernels) or, with
+    pinned=False, pageable (the library stages it with host-to-device copies)."""
 
-    def __init__(self, batch):
+    def __init__(self, batch, pinned=True):
         def pin(a):
             if a is None:
                 return None
             t = torch.as_tensor(np.ascontiguousarray(a, np.float32))
-            return t.pin_memory() if torch.cuda.is_available() else t
+            return t.pin_memory() if (pinned and torch.cuda.is_available()) else t
         self.origins, self.dirs = pin(batch.origins), pin(batch.dirs)
         self.rgb, self.depth, self.depth_var = pin(batch.rgb), pin(batch.depth), pin(batch.depth_var)
         self.t_min, self.t_max, self.n_candidates = float(batch.t_min), float(batch.t_max), int(batch.n_candidates)

@@ -89,7 +89,7 @@ constexpr uint64_t SCAN_AGG = 1ull << 32, SCAN_INCL = 2ull << 32;
 __global__ void __launch_bounds__(MARCH_WARPS * 32) march_fused_kernel(MarchParams mp, const uint8_t *bits,
                                                                        const float *__restrict__ origins,
                                                                        const float *__restrict__ dirs, Workspace ws,
-                                                                       int count_total) {
+                                                                       int count_total, float *__restrict__ dirs_copy) {
   __shared__ uint32_t masks[MARCH_WARPS][MARCH_MAX_WORDS];
   __shared__ uint32_t warp_n[MARCH_WARPS];
   __shared__ uint32_t look_first[MARCH_WARPS], look_sum[MARCH_WARPS];
@@ -111,6 +111,7 @@ __global__ void __launch_bounds__(MARCH_WARPS * 32) march_fused_kernel(MarchPara
       o[a] = __ldg(origins + 3 * (size_t)r + a);
       d[a] = __ldg(dirs + 3 * (size_t)r + a);
     }
+    if (dirs_copy && lane < 3) dirs_copy[3 * (size_t)r + lane] = lane == 0 ? d[0] : (lane == 1 ? d[1] : d[2]);
     hpre = ray_hash_prefix(mp.seed, mp.step, r);
     for (uint32_t wd0 = 0; wd0 < words; wd0 += 4) {   // four words at a time: their occupancy loads are independent
       bool live[4];
@@ -177,6 +178,7 @@ __global__ void __launch_bounds__(MARCH_WARPS * 32) march_fused_kernel(MarchPara
     block_base_s = excl;
     if (ticket == gridDim.x - 1) {
       ws.offsets[mp.R] = excl + total;
+      ws.loss_acc[2] = (double)(excl + total);   // S beside the loss sums: the stats come back in one copy
       if (count_total) *ws.total_samples += excl + total;
     }
     if (ticket == 0) {
@@ -245,9 +247,9 @@ __global__ void occ_threshold_kernel(uint64_t first_cell, uint64_t n_cells,
 }  // namespace
 
 int launch_march(const MarchParams &mp, const uint8_t *bits, const float *origins, const float *dirs,
-                 const Workspace &ws, int count_total, cudaStream_t st) {
+                 const Workspace &ws, int count_total, cudaStream_t st, float *dirs_copy) {
   dim3 grid((mp.R + MARCH_WARPS - 1) / MARCH_WARPS), block(MARCH_WARPS * 32);
-  launch_pdl(march_fused_kernel, grid, block, 0, st, mp, bits, origins, dirs, ws, count_total);
+  launch_pdl(march_fused_kernel, grid, block, 0, st, mp, bits, origins, dirs, ws, count_total, dirs_copy);
   return 1;
 }
 

@@ -97,12 +97,16 @@ struct nsm_field {
   // staging for the *_host entry points
   float *stage_dev = nullptr;     // [max_rays * 11]
   float *stage_out = nullptr;     // render outputs [max_rays * 5]
-  struct HostStats { double acc[2]; uint32_t S; } *pinned = nullptr;
+  struct HostStats { double acc[3]; uint32_t S; } *pinned = nullptr;   // acc[2] = S of the step, as a double
   // Side stream: work that does not depend on the table Adam runs beside it (it is DRAM-bound, the others
   // are latency-bound): the MLP Adam of the same step and, when the caller has declared its batches ready
   // (NSM_OPT_BATCH_READY), the marcher of the NEXT step.  ev_pre_adam marks "scatter of the last step done".
   cudaStream_t side = nullptr;
   cudaEvent_t ev_pre_adam = nullptr, ev_side = nullptr, ev_main = nullptr;
+  // the step's statistics (loss sums, S) are final after the compositor: they are copied out on the side stream right
+  // behind it, and a call that wants them waits for that copy only, not for the backward pass and Adam
+  cudaEvent_t ev_comp = nullptr, ev_stats = nullptr;
+  bool stats_pending = false;
   bool batch_ready = false;   // NSM_OPT_BATCH_READY
   bool side_ok = false;       // nothing but a train step's Adam has been enqueued on `stream` since ev_pre_adam
   const char *mlp_path = "simt_fp32";
@@ -228,27 +232,29 @@ MarchParams make_march(const nsm_field *f, const nsm_ray_batch *b, uint32_t R, b
 // S1-S8 forward (+ S9-S12 when train): everything up to, but excluding, Adam.
 // march_on_side: the marcher runs on the side stream, behind "scatter of the previous step done" only,
 // i.e. beside the previous step's table Adam (NSM_OPT_BATCH_READY; training steps only).
+// dirs_copy: see launch_march (zero-copy host batches); the MLP kernels then read the copy.
 void enqueue_forward(nsm_field *f, const nsm_ray_batch *b, uint32_t R, bool jitter, uint32_t step, bool train,
-                     bool march_on_side = false) {
+                     bool march_on_side = false, float *dirs_copy = nullptr) {
   const uint32_t *d_S = f->ws.offsets + R;
+  const float *mlp_dirs = dirs_copy ? dirs_copy : b->dirs;
   MarchParams mp = make_march(f, b, R, jitter, step);
   if (march_on_side && !f->prof.on) {
     if (!f->side_ok) {   // other work has been enqueued on the main stream since the last Adam: order behind all of it
       cudaEventRecord(f->ev_main, f->stream);
       cudaStreamWaitEvent(f->side, f->ev_main, 0);
     }
-    RUN_ON(f, K_MARCH, f->side, launch_march(mp, f->occ_full ? nullptr : f->fp.occ_bits, b->origins, b->dirs, f->ws, train ? 1 : 0, f->side));
+    RUN_ON(f, K_MARCH, f->side, launch_march(mp, f->occ_full ? nullptr : f->fp.occ_bits, b->origins, b->dirs, f->ws, train ? 1 : 0, f->side, dirs_copy));
     cudaEventRecord(f->ev_side, f->side);
     cudaStreamWaitEvent(f->stream, f->ev_side, 0);
   } else {
-    RUN(f, K_MARCH, launch_march(mp, f->occ_full ? nullptr : f->fp.occ_bits, b->origins, b->dirs, f->ws, train ? 1 : 0, f->stream));
+    RUN(f, K_MARCH, launch_march(mp, f->occ_full ? nullptr : f->fp.occ_bits, b->origins, b->dirs, f->ws, train ? 1 : 0, f->stream, dirs_copy));
   }
   const int bf16 = f->cfg.mlp_precision == NSM_MLP_BF16;
   RUN(f, K_ENCODE, launch_encode(f->lv, f->fp.rec, f->ws, d_S, f->use_tc ? 1 + bf16 : 0, f->n_sms, f->stream));
   if (f->use_tc)
-    RUN(f, K_MLP_FWD, launch_mlp_forward_tc(f->ms, bf16, b->dirs, f->ws, d_S, 0, train ? 1 : 0, f->n_sms, f->stream));
+    RUN(f, K_MLP_FWD, launch_mlp_forward_tc(f->ms, bf16, mlp_dirs, f->ws, d_S, 0, train ? 1 : 0, f->n_sms, f->stream));
   else
-    RUN(f, K_MLP_FWD, launch_mlp_forward_simt(f->ms, f->fp.mlp_theta, b->dirs, f->ws, d_S, 0, f->n_sms, f->stream));
+    RUN(f, K_MLP_FWD, launch_mlp_forward_simt(f->ms, f->fp.mlp_theta, mlp_dirs, f->ws, d_S, 0, f->n_sms, f->stream));
 }
 
 // the tensor-core kernels read 16-bit weight images: repack after every change of the MLP weights
@@ -266,19 +272,27 @@ nsm_status clear_grads_if_dirty(nsm_field *f) {
   return NSM_OK;
 }
 
-nsm_status enqueue_backward(nsm_field *f, const nsm_ray_batch *b, float lambda_d, bool march_on_side = false) {
+nsm_status enqueue_backward(nsm_field *f, const nsm_ray_batch *b, float lambda_d, bool march_on_side = false,
+                            float *dirs_copy = nullptr, bool want_stats = false) {
   const uint32_t R = b->n_rays;
   const uint32_t *d_S = f->ws.offsets + R;
   nsm_status st = clear_grads_if_dirty(f);
   if (st != NSM_OK) return st;
-  enqueue_forward(f, b, R, f->cfg.jitter != 0, f->step + 1, true, march_on_side);
+  enqueue_forward(f, b, R, f->cfg.jitter != 0, f->step + 1, true, march_on_side, dirs_copy);
   f->side_ok = false;
   RUN(f, K_COMPOSITE, launch_composite_train(f->ws, R, b->rgb, b->depth, b->depth_var, lambda_d, f->cfg.bg, f->stream));
+  if (want_stats) {
+    CUDA_TRY(cudaEventRecord(f->ev_comp, f->stream));
+    CUDA_TRY(cudaStreamWaitEvent(f->side, f->ev_comp, 0));
+    CUDA_TRY(cudaMemcpyAsync(f->pinned->acc, f->ws.loss_acc, 3 * sizeof(double), cudaMemcpyDeviceToHost, f->side));
+    CUDA_TRY(cudaEventRecord(f->ev_stats, f->side));
+    f->stats_pending = true;
+  }
   if (f->use_tc)
     RUN(f, K_MLP_BWD, launch_mlp_backward_tc(f->ms, f->cfg.mlp_precision == NSM_MLP_BF16, f->fp.mlp_grad, f->ws, d_S,
                                              f->n_sms, f->stream));
   else
-    RUN(f, K_MLP_BWD, launch_mlp_backward_simt(f->ms, f->fp.mlp_theta, f->fp.mlp_grad, b->dirs,
+    RUN(f, K_MLP_BWD, launch_mlp_backward_simt(f->ms, f->fp.mlp_theta, f->fp.mlp_grad, dirs_copy ? dirs_copy : b->dirs,
                                                f->ws, d_S, f->n_sms, f->stream));
   RUN(f, K_SCATTER, launch_scatter(f->lv, f->fp.grad, f->ws, d_S, f->n_sms, f->stream));
   f->grads_dirty = true;
@@ -323,9 +337,10 @@ nsm_status enqueue_adam(nsm_field *f) {
 
 nsm_status read_stats(nsm_field *f, uint32_t R, nsm_step_stats *out) {
   if (!out) return NSM_OK;
-  CUDA_TRY(cudaMemcpyAsync(f->pinned->acc, f->ws.loss_acc, 2 * sizeof(double), cudaMemcpyDeviceToHost, f->stream));
-  CUDA_TRY(cudaMemcpyAsync(&f->pinned->S, f->ws.offsets + R, sizeof(uint32_t), cudaMemcpyDeviceToHost, f->stream));
-  CUDA_TRY(cudaStreamSynchronize(f->stream));
+  if (!f->stats_pending) return fail(NSM_ERR_INVALID_ARG, "internal: statistics were not requested for this step");
+  CUDA_TRY(cudaEventSynchronize(f->ev_stats));   // S1-S9 of this step are done; S10-S13 may still be running
+  f->stats_pending = false;
+  f->pinned->S = (uint32_t)f->pinned->acc[2];
   out->loss_rgb = f->pinned->acc[0] / (double)R;
   out->loss_depth = f->pinned->acc[1] / (double)R;
   out->n_samples = f->pinned->S;
@@ -444,7 +459,7 @@ nsm_status nsm_create_field(const nsm_field_config *cfg, void *cuda_stream, nsm_
   }
   A(f->alloc(&ws.sigma, cap)); A(f->alloc(&ws.rgb, 3 * cap)); A(f->alloc(&ws.T_excl, cap));
   A(f->alloc(&ws.dsigma, cap)); A(f->alloc(&ws.drgb, 3 * cap)); A(f->alloc(&ws.de, ms.LF * cap));
-  A(f->alloc(&ws.loss_acc, 2)); A(f->alloc(&ws.total_samples, 1)); A(f->alloc(&ws.grad_absmax, 1));
+  A(f->alloc(&ws.loss_acc, 3)); A(f->alloc(&ws.total_samples, 1)); A(f->alloc(&ws.grad_absmax, 1));
   A(f->alloc(&f->stage_dev, 11 * (size_t)R)); A(f->alloc(&f->stage_out, 5 * (size_t)R));
   if (e == cudaSuccess) e = cudaMallocHost((void **)&f->pinned, sizeof(*f->pinned));
   if (e == cudaSuccess) {   // highest priority: the side stream's small grids must not queue behind the table Adam's 3000 blocks
@@ -455,6 +470,8 @@ nsm_status nsm_create_field(const nsm_field_config *cfg, void *cuda_stream, nsm_
   if (e == cudaSuccess) e = cudaEventCreateWithFlags(&f->ev_pre_adam, cudaEventDisableTiming);
   if (e == cudaSuccess) e = cudaEventCreateWithFlags(&f->ev_side, cudaEventDisableTiming);
   if (e == cudaSuccess) e = cudaEventCreateWithFlags(&f->ev_main, cudaEventDisableTiming);
+  if (e == cudaSuccess) e = cudaEventCreateWithFlags(&f->ev_comp, cudaEventDisableTiming);
+  if (e == cudaSuccess) e = cudaEventCreateWithFlags(&f->ev_stats, cudaEventDisableTiming);
   if (e != cudaSuccess) {
     nsm_destroy_field(f);
     cudaGetLastError();
@@ -473,6 +490,8 @@ void nsm_destroy_field(nsm_field *f) {
   if (f->ev_pre_adam) cudaEventDestroy(f->ev_pre_adam);
   if (f->ev_side) cudaEventDestroy(f->ev_side);
   if (f->ev_main) cudaEventDestroy(f->ev_main);
+  if (f->ev_comp) cudaEventDestroy(f->ev_comp);
+  if (f->ev_stats) cudaEventDestroy(f->ev_stats);
   f->prof.destroy();
   for (void *p : f->allocs) cudaFree(p);
   if (f->pinned) cudaFreeHost(f->pinned);
@@ -612,7 +631,8 @@ nsm_status nsm_update_occupancy(nsm_field *f, nsm_occ_mode mode, const uint8_t *
 nsm_status nsm_backward(nsm_field *f, const nsm_ray_batch *batch, float lambda_d, nsm_step_stats *host_stats) {
   nsm_status st = validate_batch(f, batch, true, false);
   if (st != NSM_OK) return st;
-  st = enqueue_backward(f, batch, lambda_d);
+  f->side_ok = false;
+  st = enqueue_backward(f, batch, lambda_d, false, nullptr, host_stats != nullptr);
   if (st != NSM_OK) return st;
   st = read_stats(f, batch->n_rays, host_stats);
   if (st == NSM_OK && host_stats) host_stats->loss = host_stats->loss_rgb + (double)lambda_d * host_stats->loss_depth;
@@ -625,10 +645,10 @@ nsm_status nsm_apply_adam(nsm_field *f) {
 }
 
 static nsm_status train_step_impl(nsm_field *f, const nsm_ray_batch *batch, float lambda_d, nsm_step_stats *host_stats,
-                                  bool batch_ready) {
+                                  bool batch_ready, float *dirs_copy = nullptr) {
   nsm_status st = validate_batch(f, batch, true, false);
   if (st != NSM_OK) return st;
-  st = enqueue_backward(f, batch, lambda_d, batch_ready);
+  st = enqueue_backward(f, batch, lambda_d, batch_ready, dirs_copy, host_stats != nullptr);
   if (st != NSM_OK) return st;
   st = enqueue_adam(f);
   if (st != NSM_OK) return st;
@@ -641,14 +661,28 @@ nsm_status nsm_train_step(nsm_field *f, const nsm_ray_batch *batch, float lambda
   return train_step_impl(f, batch, lambda_d, host_stats, f && f->batch_ready);
 }
 
+// device alias of a pinned (page-locked, device-mapped) host pointer, or NULL for pageable memory
+static const float *host_mapped(const float *p) {
+  cudaPointerAttributes a;
+  if (cudaPointerGetAttributes(&a, p) != cudaSuccess) { cudaGetLastError(); return nullptr; }
+  return a.type == cudaMemoryTypeHost ? (const float *)a.devicePointer : nullptr;
+}
+
 nsm_status nsm_train_step_host(nsm_field *f, const nsm_ray_batch *hb, float lambda_d, nsm_step_stats *host_stats) {
   nsm_status st = validate_batch(f, hb, true, false);
   if (st != NSM_OK) return st;
-  f->side_ok = false;   // the staging copies go through the main stream
-  nsm_ray_batch db;
+  nsm_step_stats local;
+  nsm_ray_batch db = *hb;
+  // Pinned host buffers are read IN PLACE over the host link: every input is needed exactly once per ray (origins and
+  // directions by the marcher, which leaves a device copy of the directions for the MLPs; colour, depth and variance
+  // by the compositor), so there is nothing a staging copy would save -- and five small DMA launches to lose.
+  db.origins = host_mapped(hb->origins); db.dirs = host_mapped(hb->dirs); db.rgb = host_mapped(hb->rgb);
+  db.depth = host_mapped(hb->depth); db.depth_var = host_mapped(hb->depth_var);
+  if (db.origins && db.dirs && db.rgb && db.depth && db.depth_var)   // the call syncs: the host buffers are free on return
+    return train_step_impl(f, &db, lambda_d, host_stats ? host_stats : &local, true, f->stage_dev + 3 * (size_t)f->cfg.max_rays);
+  f->side_ok = false;   // pageable memory: staging copies through the main stream
   st = stage_batch(f, hb, 0, hb->n_rays, true, &db);
   if (st != NSM_OK) return st;
-  nsm_step_stats local;
   return train_step_impl(f, &db, lambda_d, host_stats ? host_stats : &local, false);  // always syncs: host buffers may be reused
 }
 

@@ -58,7 +58,7 @@ struct Workspace {
   float *dsigma;         // [cap]
   float *drgb;           // [cap,3]
   float *de;             // [LF][cap]
-  // loss accumulators: [0]=sum rgb, [1]=sum depth (doubles); device
+  // loss accumulators: [0]=sum rgb, [1]=sum depth, [2]=S of the step (doubles); device
   double *loss_acc;
   unsigned long long *total_samples;  // running sum of S over training steps (device)
   // tensor-core path: 16-bit operand-tile images ("blobs", see mlp_tc.cu) instead of the fp32 planes e/hd/g/h1/h2
@@ -199,8 +199,10 @@ __device__ __forceinline__ void adam_one(float &th, float &m, float &v, float g,
 
 // ---- launchers (each enqueues on `st`, returns the number of kernels launched) ----
 // S1-S3 in one launch; also resets the loss accumulators and (count_total) adds S to the running sample count
+// dirs_copy (optional): [R,3] device buffer that receives the directions (host entry points: origins / dirs may be
+// device-mapped pinned HOST memory, read once here; the later kernels use the copy)
 int launch_march(const MarchParams &mp, const uint8_t *bits, const float *origins, const float *dirs,
-                 const Workspace &ws, int count_total, cudaStream_t st);
+                 const Workspace &ws, int count_total, cudaStream_t st, float *dirs_copy = nullptr);
 uint32_t march_scan_state_entries(uint32_t max_rays);
 // out_mode: 0 = fp32 planes ws.e, 1 = fp16 blob ws.blob_e, 2 = bf16 blob ws.blob_e
 int launch_encode(const LevelTable &lv, const float *rec, const Workspace &ws,

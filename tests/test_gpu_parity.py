@@ -338,13 +338,15 @@ def test_render_parity(nsm):
     f.close()
 
 
-def test_host_entry_point_matches_device_entry_point(nsm):
+@pytest.mark.parametrize("pinned", [True, False])
+def test_host_entry_point_matches_device_entry_point(nsm, pinned):
+    """pinned: the kernels read the host batch in place; pageable: staged by host-to-device copies."""
     w = configs.config1()
     f1, _, _ = make_pair(nsm, w, seed=7)
     f2, _, _ = make_pair(nsm, w, seed=7)
     b = w.batches[0]
     s1 = f1.nsm_train_step(nsm.DeviceBatch(b), w.lambda_d)
-    s2 = f2.nsm_train_step_host(nsm.HostBatch(b), w.lambda_d)
+    s2 = f2.nsm_train_step_host(nsm.HostBatch(b, pinned=pinned), w.lambda_d)
     assert s1["n_samples"] == s2["n_samples"] and abs(s1["loss"] - s2["loss"]) <= 1e-6 * abs(s1["loss"])
     a, b2 = f1.nsm_get_params()[0], f2.nsm_get_params()[0]
     assert np.abs(a - b2).max() <= 2.1e-2      # same gradients up to atomic order; Adam sign flips of noise-level entries
