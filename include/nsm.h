@@ -147,6 +147,12 @@ nsm_status nsm_train_step(nsm_field *f, const nsm_ray_batch *batch, float lambda
 nsm_status nsm_train_step_host(nsm_field *f, const nsm_ray_batch *host_batch, float lambda_d,
                                nsm_step_stats *host_stats);
 
+/* Debug: with NSM_TIMELINE=1 in the environment at nsm_create_field, every hot-path kernel stamps its first
+ * block's start and last block's end (%globaltimer, ns) into a ring of the last 64 training steps.  h_out (HOST)
+ * receives 64 x [2][n_kernels] words, slot = step % 64, kernel classes in the order of nsm_profile_read; a
+ * start of ~0 / end of 0 means "did not run".  Synchronises.  Costs a few atomics per block: not for timing runs. */
+nsm_status nsm_debug_timeline(nsm_field *f, uint64_t *h_out, uint64_t capacity_words, uint32_t *n_kernels);
+
 /* Options.
  * NSM_OPT_BATCH_READY (default 0).  With 0 the library reads a batch strictly in the order of the field's
  * stream.  With 1 the caller declares that the device buffers of every batch handed to nsm_train_step are

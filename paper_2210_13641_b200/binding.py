@@ -27,7 +27,7 @@ DEBUG_ITEMS = dict(counts=(0, np.uint32), offsets=(1, np.uint32), s_ray=(2, np.u
 EXPORTS = ["nsm_create_field", "nsm_destroy_field", "nsm_update_occupancy", "nsm_get_occupancy",
            "nsm_train_step", "nsm_train_step_host", "nsm_backward", "nsm_apply_adam", "nsm_debug_set_grad",
            "nsm_render", "nsm_render_host", "nsm_param_count", "nsm_get_params", "nsm_set_params",
-           "nsm_get_level_table", "nsm_debug_last_step", "nsm_total_samples", "nsm_profile", "nsm_set_option",
+           "nsm_get_level_table", "nsm_debug_last_step", "nsm_total_samples", "nsm_profile", "nsm_set_option", "nsm_debug_timeline",
            "nsm_profile_read", "nsm_launch_count", "nsm_mlp_path",
            "nsm_last_error", "nsm_version"]
 
@@ -93,6 +93,7 @@ def load_library():
         L.nsm_total_samples.argtypes = [vp, u64p]
         L.nsm_profile.argtypes = [vp, C.c_int]
         L.nsm_set_option.argtypes = [vp, C.c_int, C.c_uint32]
+        L.nsm_debug_timeline.argtypes = [vp, u64p, C.c_uint64, u32p]
         L.nsm_profile_read.argtypes = [vp, C.c_uint32, C.POINTER(C.c_char_p), C.POINTER(C.c_double), u64p, u32p]
         L.nsm_launch_count.argtypes = [vp]
         L.nsm_launch_count.restype = C.c_uint64
@@ -331,6 +332,13 @@ class Field:
         n = C.c_uint64()
         _check(self.lib.nsm_total_samples(self.h, C.byref(n)))
         return int(n.value)
+
+    def nsm_debug_timeline(self):
+        """[64, 2, n_kernels] uint64 globaltimer stamps (slot = step % 64); needs NSM_TIMELINE=1 at creation."""
+        buf = (C.c_uint64 * (64 * 2 * 32))()
+        nk = C.c_uint32()
+        _check(self.lib.nsm_debug_timeline(self.h, buf, 64 * 2 * 32, C.byref(nk)))
+        return np.frombuffer(buf, np.uint64)[:64 * 2 * nk.value].reshape(64, 2, nk.value).copy()
 
     def nsm_set_option(self, opt, value):
         _check(self.lib.nsm_set_option(self.h, int(opt), int(value)))

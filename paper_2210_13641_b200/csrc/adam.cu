@@ -58,7 +58,8 @@ __device__ __forceinline__ void adam_record(float *__restrict__ r, const float *
 
 template <int F>
 __global__ void __launch_bounds__(ADAM_THREADS) adam_table_kernel(float *__restrict__ rec, float *__restrict__ grad,
-                                                                  uint64_t n_entries, int sparse, AdamConst c) {
+                                                                  uint64_t n_entries, int sparse, AdamConst c,
+                                                                  unsigned long long *tl) {
   constexpr int CH = ADAM_CHUNK_FLOATS / F;            // entries per chunk
   constexpr int NV = ADAM_CHUNK_FLOATS / 4 / ADAM_THREADS;   // float4 loads per thread
   __shared__ float list_g[ADAM_CHUNK_FLOATS];          // compacted gradients, F floats per touched entry
@@ -67,6 +68,7 @@ __global__ void __launch_bounds__(ADAM_THREADS) adam_table_kernel(float *__restr
   const uint32_t tid = threadIdx.x, lane = tid & 31;
   pdl_wait();
   pdl_trigger();
+  tl_mark(tl, K_ADAM_TABLE, 0);
   const uint64_t e_base = (uint64_t)blockIdx.x * CH;
   const uint64_t n_float = n_entries * F;
   const float *g4 = grad + e_base * F;
@@ -118,7 +120,7 @@ __global__ void __launch_bounds__(ADAM_THREADS) adam_table_kernel(float *__restr
   }
   __syncthreads();
   const uint32_t n = cnt;
-  if (n == 0) return;
+  if (n == 0) { tl_mark(tl, K_ADAM_TABLE, 1); return; }
   // phase 2: two records in flight per thread
   for (uint32_t i0 = tid; i0 < n; i0 += 2 * ADAM_THREADS) {
     const uint32_t i1 = i0 + ADAM_THREADS;
@@ -138,6 +140,7 @@ __global__ void __launch_bounds__(ADAM_THREADS) adam_table_kernel(float *__restr
     const uint32_t q = j * ADAM_THREADS + tid;
     if (e_base * F + 4ull * q < n_float) st_hint_f4(o4 + 4 * q, make_float4(nz, nz, nz, nz), pol_last);
   }
+  tl_mark(tl, K_ADAM_TABLE, 1);
 }
 
 __global__ void adam_dense_kernel(float *__restrict__ theta, float *__restrict__ m, float *__restrict__ v,
@@ -154,16 +157,16 @@ __global__ void adam_dense_kernel(float *__restrict__ theta, float *__restrict__
 }  // namespace
 
 int launch_adam_table(const FieldParams &fp, uint32_t F, int sparse, float lr, float beta1, float beta2, float eps,
-                      float inv_bc1, float inv_bc2, int n_sms, cudaStream_t st) {
+                      float inv_bc1, float inv_bc2, int n_sms, cudaStream_t st, unsigned long long *tl) {
   (void)n_sms;
   AdamConst c{lr, beta1, beta2, eps, inv_bc1, inv_bc2};
   const uint64_t chunk = ADAM_CHUNK_FLOATS / F;
   dim3 grid((unsigned)((fp.n_entries + chunk - 1) / chunk)), block(ADAM_THREADS);
   switch (F) {
-    case 1: launch_pdl(adam_table_kernel<1>, grid, block, 0, st, fp.rec, fp.grad, fp.n_entries, sparse, c); break;
-    case 2: launch_pdl(adam_table_kernel<2>, grid, block, 0, st, fp.rec, fp.grad, fp.n_entries, sparse, c); break;
-    case 4: launch_pdl(adam_table_kernel<4>, grid, block, 0, st, fp.rec, fp.grad, fp.n_entries, sparse, c); break;
-    default: launch_pdl(adam_table_kernel<8>, grid, block, 0, st, fp.rec, fp.grad, fp.n_entries, sparse, c); break;
+    case 1: launch_pdl(adam_table_kernel<1>, grid, block, 0, st, fp.rec, fp.grad, fp.n_entries, sparse, c, tl); break;
+    case 2: launch_pdl(adam_table_kernel<2>, grid, block, 0, st, fp.rec, fp.grad, fp.n_entries, sparse, c, tl); break;
+    case 4: launch_pdl(adam_table_kernel<4>, grid, block, 0, st, fp.rec, fp.grad, fp.n_entries, sparse, c, tl); break;
+    default: launch_pdl(adam_table_kernel<8>, grid, block, 0, st, fp.rec, fp.grad, fp.n_entries, sparse, c, tl); break;
   }
   return 1;
 }

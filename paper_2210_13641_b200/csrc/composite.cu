@@ -44,6 +44,7 @@ __global__ void __launch_bounds__(256) composite_kernel(Workspace ws, uint32_t R
                                                         float *__restrict__ out_opacity) {
   pdl_wait();
   pdl_trigger();
+  tl_mark(ws.timeline, K_COMPOSITE, 0);
   const uint32_t r = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
   float l_rgb = 0.0f, l_d = 0.0f;  // lane 0 holds the ray's loss terms
   float gmax = 0.0f;               // max |gradient entering the MLP backward| seen by this thread
@@ -150,6 +151,7 @@ __global__ void __launch_bounds__(256) composite_kernel(Workspace ws, uint32_t R
     for (int sft = 16; sft > 0; sft >>= 1) gmax = fmaxf(gmax, __shfl_xor_sync(0xffffffffu, gmax, sft));
     if (lane == 0 && gmax > 0.f && isfinite(gmax)) atomicMax(ws.grad_absmax, __float_as_uint(gmax));
   }
+  tl_mark(ws.timeline, K_COMPOSITE, 1);
 }
 
 }  // namespace

@@ -103,6 +103,7 @@ __global__ void __launch_bounds__(256) encode_forward_kernel(LevelTable lv, cons
                                                              Workspace ws, const uint32_t *__restrict__ d_S) {
   pdl_wait();
   pdl_trigger();
+  tl_mark(ws.timeline, K_ENCODE, 0);
   const uint64_t S = *d_S;
   const uint64_t S_it = MODE == 0 ? S : ((S + NSM_TILE - 1) / NSM_TILE) * NSM_TILE;
   const uint64_t total = S_it * lv.n_levels;
@@ -156,6 +157,7 @@ __global__ void __launch_bounds__(256) encode_forward_kernel(LevelTable lv, cons
       }
     }
   }
+  tl_mark(ws.timeline, K_ENCODE, 1);
 }
 
 template <int F>
@@ -181,6 +183,7 @@ __global__ void __launch_bounds__(256) scatter_backward_kernel(LevelTable lv, fl
                                                                const uint32_t *__restrict__ d_S) {
   pdl_wait();
   pdl_trigger();
+  tl_mark(ws.timeline, K_SCATTER, 0);
   const uint64_t S = *d_S;
   const uint64_t total = S * lv.n_levels;
   const uint64_t pol_last = l2_evict_last();
@@ -205,6 +208,7 @@ __global__ void __launch_bounds__(256) scatter_backward_kernel(LevelTable lv, fl
       red_add_entry<F>(tab + (size_t)ci.slot[k] * F, g, pol_last);
     }
   }
+  tl_mark(ws.timeline, K_SCATTER, 1);
 }
 
 // gradient array <- canonical gradient and flags (debug / test entry point)

@@ -99,6 +99,7 @@ __global__ void __launch_bounds__(MARCH_WARPS * 32) march_fused_kernel(MarchPara
   volatile unsigned long long *state = ws.scan_state;
   pdl_wait();
   pdl_trigger();
+  tl_mark(ws.timeline, K_MARCH, 0);
   if (tid == 0) ticket_s = atomicAdd(ticket_ctr, 1u);
   __syncthreads();
   const uint32_t ticket = ticket_s;
@@ -218,6 +219,7 @@ __global__ void __launch_bounds__(MARCH_WARPS * 32) march_fused_kernel(MarchPara
     for (uint32_t i = tid; i < gridDim.x; i += MARCH_WARPS * 32) state[i] = 0ull;
     if (tid == 0) { *ticket_ctr = 0u; *done_ctr = 0u; }
   }
+  tl_mark(ws.timeline, K_MARCH, 1);
 }
 
 // S14 FROM_FIELD: the cell centres of a chunk of the occupancy grid as "samples".

@@ -93,24 +93,67 @@ __global__ void pack_weights_kernel(MlpShape ms, const float *__restrict__ Wm, u
   }
 }
 
-// S13 on the MLP weights (all of them, every step) fused with the image refresh: one thread per
-// weight updates theta, m, v, clears the gradient and writes the weight's three 16-bit image
-// elements.  Padding elements of the images stay zero from pack_weights_kernel.
+// Sum of the per-CTA weight-gradient slices written by mlp_backward_tc_kernel: CTA c wrote a slice iff it had a
+// tile, i.e. c < min(n_ctas, ceil(S / 128)).  Four warps per 32 weights: warp q adds slices q, q+4, ... (each load
+// is a coalesced 128 B row segment, eight in flight), then the four partial sums meet in shared memory.
+__device__ __forceinline__ float sum_wgrad_parts(const float *__restrict__ parts, uint32_t n_mlp, uint32_t n_parts, uint32_t p,
+                                                 uint32_t q, float *red /* [4][32] */) {
+  float acc = 0.f;
+  if (p < n_mlp) {
+    uint32_t c = q;
+    for (; c + 28 < n_parts; c += 32) {
+      float t[8];
+#pragma unroll
+      for (int u = 0; u < 8; ++u) t[u] = parts[(size_t)(c + 4 * u) * n_mlp + p];
+#pragma unroll
+      for (int u = 0; u < 8; ++u) acc += t[u];
+    }
+    for (; c < n_parts; c += 4) acc += parts[(size_t)c * n_mlp + p];
+  }
+  red[q * 32 + (threadIdx.x & 31)] = acc;
+  __syncthreads();
+  return red[threadIdx.x & 31] + red[32 + (threadIdx.x & 31)] + red[64 + (threadIdx.x & 31)] + red[96 + (threadIdx.x & 31)];
+}
+
+// slices -> mlp_grad (nsm_backward: the gradient is left in place for the debug getter / nsm_apply_adam)
+__global__ void __launch_bounds__(128) reduce_wgrad_kernel(const float *__restrict__ parts, uint32_t n_mlp, uint32_t n_ctas,
+                                                           const uint32_t *__restrict__ d_S, float *__restrict__ grad) {
+  __shared__ float red[128];
+  const uint32_t tiles = (*d_S + ROWS - 1) / ROWS, n_parts = tiles < n_ctas ? tiles : n_ctas;
+  const uint32_t p = blockIdx.x * 32 + (threadIdx.x & 31), q = threadIdx.x >> 5;
+  const float g = sum_wgrad_parts(parts, n_mlp, n_parts, p, q, red);
+  if (q == 0 && p < n_mlp) grad[p] += g;
+}
+
+// S13 on the MLP weights (all of them, every step) fused with the reduction of the weight-gradient slices and the
+// image refresh: the thread of weight p (warp 0 of its block) updates theta, m, v, clears the gradient and writes the
+// weight's three 16-bit image elements.  Padding elements of the images stay zero from pack_weights_kernel.
+// n_ctas = 0: the gradient is already complete in grad[] (after nsm_backward or nsm_debug_set_grad).
 template <typename T>
 __global__ void __launch_bounds__(128) adam_pack_kernel(MlpShape ms, float *__restrict__ theta, float *__restrict__ m_,
                                                         float *__restrict__ v_, float *__restrict__ grad, uint8_t *__restrict__ img_f,
-                                                        uint8_t *__restrict__ img_b, AdamConst c) {
+                                                        uint8_t *__restrict__ img_b, AdamConst c, const float *__restrict__ parts,
+                                                        uint32_t n_ctas, const uint32_t *__restrict__ d_S, unsigned long long *tl) {
+  __shared__ float red[128];
   pdl_wait();
   pdl_trigger();
-  const uint32_t p = blockIdx.x * blockDim.x + threadIdx.x;
-  if (p >= ms.n_mlp) return;
+  tl_mark(tl, K_ADAM_MLP, 0);
+  const uint32_t p = blockIdx.x * 32 + (threadIdx.x & 31), q = threadIdx.x >> 5;
+  float g = 0.f;
+  if (n_ctas) {
+    const uint32_t tiles = (*d_S + ROWS - 1) / ROWS;
+    g = sum_wgrad_parts(parts, ms.n_mlp, tiles < n_ctas ? tiles : n_ctas, p, q, red);
+  }
+  if (q != 0 || p >= ms.n_mlp) return;
+  g += grad[p];
   float th = theta[p], mm = m_[p], vv = v_[p];
-  adam_one(th, mm, vv, grad[p], c);
+  adam_one(th, mm, vv, g, c);
   theta[p] = th; m_[p] = mm; v_[p] = vv; grad[p] = 0.f;
   const uint32_t mi = p >= ms.o_c3 ? 4u : (p >= ms.o_c2 && ms.n_color_layers == 2) ? 3u : p >= ms.o_c1 ? 2u : p >= ms.o_d2 ? 1u : 0u;
   const MatImg mt = mat_img(ms, mi);
-  const uint32_t q = p - mt.off, n = q / mt.n_in, k = q - n * mt.n_in;
+  const uint32_t k0 = p - mt.off, n = k0 / mt.n_in, k = k0 - n * mt.n_in;
   put_weight<T>(mt, n, k, th, img_f, img_b);
+  tl_mark(tl, K_ADAM_MLP, 1);
 }
 
 // issue the k-steps of one layer: D[128 x N] = A[128 x K] * B[N x K]^T, both K-major
@@ -255,6 +298,7 @@ __global__ void __launch_bounds__(FWD_THREADS, 2) mlp_forward_tc_kernel(MlpShape
   pdl_wait();
   pdl_trigger();
   if (!has_tiles) return;
+  tl_mark(ws.timeline, K_MLP_FWD, 0);
   if (tid == 0) {   // the encoder's output: after the wait
     mbar_expect_tx(bar_e, e_bytes);
     bulk_g2s(sbase + FwdSmem::bufA, ws.blob_e + (size_t)blockIdx.x * e_bytes, e_bytes, bar_e);
@@ -372,6 +416,7 @@ __global__ void __launch_bounds__(FWD_THREADS, 2) mlp_forward_tc_kernel(MlpShape
   fence_before();
   __syncthreads();
   if (warp == 0) tmem_free<FWD_COLS>(tmem_base);
+  tl_mark(ws.timeline, K_MLP_FWD, 1);
 }
 
 // ------------------------------------------------------------------------------------- backward
@@ -447,7 +492,7 @@ __device__ __forceinline__ void masked_to_Y(uint32_t tlane, uint32_t mask, uint8
 // 8 warps per tile as in the forward kernel: warp w owns sample rows 32 (w & 3) .. +31 (TMEM lane quarter) and the
 // column half (w >> 2) of every 64-wide dgrad.
 template <typename T>
-__global__ void __launch_bounds__(BWD_THREADS, 2) mlp_backward_tc_kernel(MlpShape ms, float *__restrict__ gradW, Workspace ws,
+__global__ void __launch_bounds__(BWD_THREADS, 2) mlp_backward_tc_kernel(MlpShape ms, Workspace ws,
                                                                         const uint32_t *__restrict__ d_S) {
   extern __shared__ __align__(1024) uint8_t smem[];
   const uint32_t tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
@@ -501,6 +546,7 @@ __global__ void __launch_bounds__(BWD_THREADS, 2) mlp_backward_tc_kernel(MlpShap
   pdl_wait();     // the compositor's dL/dsigma, dL/dc and gradient maximum
   pdl_trigger();
   if (!has_tiles) return;
+  tl_mark(ws.timeline, K_MLP_BWD, 0);
   fence_async_smem();
   fence_before();
   __syncthreads();
@@ -637,6 +683,10 @@ __global__ void __launch_bounds__(BWD_THREADS, 2) mlp_backward_tc_kernel(MlpShap
   fence_before();
   __syncthreads();
   fence_after();
+  // Each CTA stores its sums into its own slice of ws.wgrad_part with plain, lane-coalesced stores; the slices are
+  // summed by the consumer (the MLP Adam kernel, or reduce_wgrad_kernel).  Atomics onto the 9-11 K shared addresses
+  // from every CTA serialise in L2 and kept the CTAs draining at exit for 40 % of the kernel (profiles/r1h).
+  float *part = ws.wgrad_part + (size_t)blockIdx.x * ms.n_mlp;
   // G[i][o] = dW[o][i]: rows = input features, ncols output columns
   auto flush = [&](uint32_t col, uint32_t g_off, uint32_t n_out, uint32_t n_in, uint32_t ncols) {
     float v[16];
@@ -647,7 +697,7 @@ __global__ void __launch_bounds__(BWD_THREADS, 2) mlp_backward_tc_kernel(MlpShap
 #pragma unroll
         for (int j = 0; j < 16; ++j) {
           const uint32_t o = c0 + j;
-          if (o < n_out && v[j] != 0.f) atomicAdd(gradW + g_off + o * n_in + row, v[j] * inv_scale);
+          if (o < n_out) part[g_off + o * n_in + row] = v[j] * inv_scale;
         }
     }
   };
@@ -661,7 +711,7 @@ __global__ void __launch_bounds__(BWD_THREADS, 2) mlp_backward_tc_kernel(MlpShap
 #pragma unroll
       for (int j = 0; j < 16; ++j) {
         const uint32_t i = half * 16 + j;
-        if (i < ms.Ci && v[j] != 0.f) atomicAdd(gradW + ms.o_c1 + row * ms.Ci + i, v[j] * inv_scale);
+        if (i < ms.Ci) part[ms.o_c1 + row * ms.Ci + i] = v[j] * inv_scale;
       }
   }
   flush(GW_D2, ms.o_d2, DO, H, 16);
@@ -669,6 +719,7 @@ __global__ void __launch_bounds__(BWD_THREADS, 2) mlp_backward_tc_kernel(MlpShap
   fence_before();
   __syncthreads();
   if (warp == 0) tmem_free<BWD_COLS>(tmem_base);
+  tl_mark(ws.timeline, K_MLP_BWD, 1);
 }
 
 // blob tile image -> fp32 rows [S][n_cols] (debug getter)
@@ -704,12 +755,19 @@ int launch_pack_weights(const MlpShape &ms, int bf16, const float *theta_mlp, co
 }
 
 int launch_adam_mlp_pack(const MlpShape &ms, int bf16, const FieldParams &fp, const Workspace &ws, const AdamConst &c,
-                         cudaStream_t st) {
-  const unsigned grid = (ms.n_mlp + 127) / 128;
-  if (bf16) launch_pdl(adam_pack_kernel<__nv_bfloat16>, dim3(grid), dim3(128), 0, st, ms, fp.mlp_theta, fp.mlp_m, fp.mlp_v, fp.mlp_grad, ws.wimg_fwd, ws.wimg_bwd, c);
-  else launch_pdl(adam_pack_kernel<__half>, dim3(grid), dim3(128), 0, st, ms, fp.mlp_theta, fp.mlp_m, fp.mlp_v, fp.mlp_grad, ws.wimg_fwd, ws.wimg_bwd, c);
+                         uint32_t n_ctas, const uint32_t *d_S, cudaStream_t st) {
+  const unsigned grid = (ms.n_mlp + 31) / 32;
+  if (bf16) launch_pdl(adam_pack_kernel<__nv_bfloat16>, dim3(grid), dim3(128), 0, st, ms, fp.mlp_theta, fp.mlp_m, fp.mlp_v, fp.mlp_grad, ws.wimg_fwd, ws.wimg_bwd, c, ws.wgrad_part, n_ctas, d_S, ws.timeline);
+  else launch_pdl(adam_pack_kernel<__half>, dim3(grid), dim3(128), 0, st, ms, fp.mlp_theta, fp.mlp_m, fp.mlp_v, fp.mlp_grad, ws.wimg_fwd, ws.wimg_bwd, c, ws.wgrad_part, n_ctas, d_S, ws.timeline);
   return 1;
 }
+
+int launch_reduce_wgrad(const MlpShape &ms, const Workspace &ws, float *grad_mlp, uint32_t n_ctas, const uint32_t *d_S, cudaStream_t st) {
+  reduce_wgrad_kernel<<<(ms.n_mlp + 31) / 32, 128, 0, st>>>(ws.wgrad_part, ms.n_mlp, n_ctas, d_S, grad_mlp);
+  return 1;
+}
+
+uint32_t mlp_tc_backward_ctas(int n_sms) { return 2u * (uint32_t)n_sms; }
 
 int launch_mlp_forward_tc(const MlpShape &ms, int bf16, const float *dirs, const Workspace &ws, const uint32_t *d_S,
                           int density_only, int save_blobs, int n_sms, cudaStream_t st) {
@@ -726,17 +784,17 @@ int launch_mlp_forward_tc(const MlpShape &ms, int bf16, const float *dirs, const
   return 1;
 }
 
-int launch_mlp_backward_tc(const MlpShape &ms, int bf16, float *grad_mlp, const Workspace &ws, const uint32_t *d_S,
+int launch_mlp_backward_tc(const MlpShape &ms, int bf16, const Workspace &ws, const uint32_t *d_S,
                            int n_sms, cudaStream_t st) {
   const size_t smem = BwdSmem::total;
   if (bf16) {
     static const cudaError_t once = cudaFuncSetAttribute(mlp_backward_tc_kernel<__nv_bfloat16>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     (void)once;
-    launch_pdl(mlp_backward_tc_kernel<__nv_bfloat16>, dim3(2 * n_sms), dim3(BWD_THREADS), smem, st, ms, grad_mlp, ws, d_S);
+    launch_pdl(mlp_backward_tc_kernel<__nv_bfloat16>, dim3(2 * n_sms), dim3(BWD_THREADS), smem, st, ms, ws, d_S);
   } else {
     static const cudaError_t once = cudaFuncSetAttribute(mlp_backward_tc_kernel<__half>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     (void)once;
-    launch_pdl(mlp_backward_tc_kernel<__half>, dim3(2 * n_sms), dim3(BWD_THREADS), smem, st, ms, grad_mlp, ws, d_S);
+    launch_pdl(mlp_backward_tc_kernel<__half>, dim3(2 * n_sms), dim3(BWD_THREADS), smem, st, ms, ws, d_S);
   }
   return 1;
 }

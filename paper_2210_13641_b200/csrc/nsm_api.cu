@@ -107,6 +107,8 @@ struct nsm_field {
   // behind it, and a call that wants them waits for that copy only, not for the backward pass and Adam
   cudaEvent_t ev_comp = nullptr, ev_stats = nullptr;
   bool stats_pending = false;
+  unsigned long long *timeline_base = nullptr;   // NSM_TIMELINE=1: ring of 64 steps x [2][K_COUNT] globaltimer stamps
+  uint32_t wgrad_parts = 0;   // > 0: the MLP weight gradient of the last backward is still in that many per-CTA slices
   bool batch_ready = false;   // NSM_OPT_BATCH_READY
   bool side_ok = false;       // nothing but a train step's Adam has been enqueued on `stream` since ev_pre_adam
   const char *mlp_path = "simt_fp32";
@@ -267,17 +269,24 @@ nsm_status clear_grads_if_dirty(nsm_field *f) {
   if (f->grads_dirty) {
     RUN(f, K_DEBUG, launch_set_grad(f->fp, nullptr, nullptr, f->stream));
     CUDA_TRY(cudaMemsetAsync(f->fp.mlp_grad, 0, sizeof(float) * f->fp.n_mlp, f->stream));
+    f->wgrad_parts = 0;
     f->grads_dirty = false;
   }
   return NSM_OK;
 }
 
 nsm_status enqueue_backward(nsm_field *f, const nsm_ray_batch *b, float lambda_d, bool march_on_side = false,
-                            float *dirs_copy = nullptr, bool want_stats = false) {
+                            float *dirs_copy = nullptr, bool want_stats = false, bool reduce_wgrad_now = false) {
   const uint32_t R = b->n_rays;
   const uint32_t *d_S = f->ws.offsets + R;
   nsm_status st = clear_grads_if_dirty(f);
   if (st != NSM_OK) return st;
+  if (f->timeline_base) {   // this step's slot of the ring; the slot used 8 steps from now is reset here, well ahead of its use
+    f->ws.timeline = f->timeline_base + (size_t)((f->step + 1) % 64) * 2 * K_COUNT;
+    unsigned long long *later = f->timeline_base + (size_t)((f->step + 9) % 64) * 2 * K_COUNT;
+    cudaMemsetAsync(later, 0xff, sizeof(unsigned long long) * K_COUNT, f->stream);
+    cudaMemsetAsync(later + K_COUNT, 0, sizeof(unsigned long long) * K_COUNT, f->stream);
+  }
   enqueue_forward(f, b, R, f->cfg.jitter != 0, f->step + 1, true, march_on_side, dirs_copy);
   f->side_ok = false;
   RUN(f, K_COMPOSITE, launch_composite_train(f->ws, R, b->rgb, b->depth, b->depth_var, lambda_d, f->cfg.bg, f->stream));
@@ -289,8 +298,14 @@ nsm_status enqueue_backward(nsm_field *f, const nsm_ray_batch *b, float lambda_d
     f->stats_pending = true;
   }
   if (f->use_tc)
-    RUN(f, K_MLP_BWD, launch_mlp_backward_tc(f->ms, f->cfg.mlp_precision == NSM_MLP_BF16, f->fp.mlp_grad, f->ws, d_S,
-                                             f->n_sms, f->stream));
+  {
+    RUN(f, K_MLP_BWD, launch_mlp_backward_tc(f->ms, f->cfg.mlp_precision == NSM_MLP_BF16, f->ws, d_S, f->n_sms, f->stream));
+    f->wgrad_parts = mlp_tc_backward_ctas(f->n_sms);
+    if (reduce_wgrad_now) {   // nsm_backward: leave the complete gradient in mlp_grad
+      RUN(f, K_MLP_BWD, launch_reduce_wgrad(f->ms, f->ws, f->fp.mlp_grad, f->wgrad_parts, d_S, f->stream));
+      f->wgrad_parts = 0;
+    }
+  }
   else
     RUN(f, K_MLP_BWD, launch_mlp_backward_simt(f->ms, f->fp.mlp_theta, f->fp.mlp_grad, dirs_copy ? dirs_copy : b->dirs,
                                                f->ws, d_S, f->n_sms, f->stream));
@@ -308,7 +323,8 @@ nsm_status enqueue_adam(nsm_field *f) {
   const double bc1 = 1.0 - std::pow((double)f->cfg.beta1, (double)t);
   const double bc2 = 1.0 - std::pow((double)f->cfg.beta2, (double)t);
   // the MLP Adam (9-11 K weights + the 16-bit image refresh) runs on the side stream beside the table Adam
-  const bool use_side = !f->prof.on;
+  static const bool no_side_adam = [] { const char *e = std::getenv("NSM_NO_SIDE_ADAM"); return e && e[0] == '1'; }();
+  const bool use_side = !f->prof.on && !no_side_adam;
   cudaStream_t s_mlp = use_side ? f->side : f->stream;
   if (use_side) {
     cudaEventRecord(f->ev_pre_adam, f->stream);
@@ -316,13 +332,15 @@ nsm_status enqueue_adam(nsm_field *f) {
   }
   if (f->use_tc) {
     const AdamConst c{f->cfg.lr, f->cfg.beta1, f->cfg.beta2, f->cfg.eps, (float)(1.0 / bc1), (float)(1.0 / bc2)};
-    RUN_ON(f, K_ADAM_MLP, s_mlp, launch_adam_mlp_pack(f->ms, f->cfg.mlp_precision == NSM_MLP_BF16, f->fp, f->ws, c, s_mlp));
+    RUN_ON(f, K_ADAM_MLP, s_mlp, launch_adam_mlp_pack(f->ms, f->cfg.mlp_precision == NSM_MLP_BF16, f->fp, f->ws, c, f->wgrad_parts,
+                                                      f->ws.offsets + f->last_R, s_mlp));
+    f->wgrad_parts = 0;
   } else {
     RUN_ON(f, K_ADAM_MLP, s_mlp, launch_adam_mlp(f->fp, f->cfg.lr, f->cfg.beta1, f->cfg.beta2, f->cfg.eps, (float)(1.0 / bc1),
                                                  (float)(1.0 / bc2), s_mlp));
   }
   RUN(f, K_ADAM_TABLE, launch_adam_table(f->fp, f->cfg.n_features, f->cfg.sparse_table_adam != 0, f->cfg.lr, f->cfg.beta1,
-                                         f->cfg.beta2, f->cfg.eps, (float)(1.0 / bc1), (float)(1.0 / bc2), f->n_sms, f->stream));
+                                         f->cfg.beta2, f->cfg.eps, (float)(1.0 / bc1), (float)(1.0 / bc2), f->n_sms, f->stream, f->ws.timeline));
   if (use_side) {   // join: everything later on the main stream sees the new MLP weights
     cudaEventRecord(f->ev_side, f->side);
     cudaStreamWaitEvent(f->stream, f->ev_side, 0);
@@ -449,16 +467,27 @@ nsm_status nsm_create_field(const nsm_field_config *cfg, void *cuda_stream, nsm_
   A(f->alloc(&ws.s_x, 3 * cap));
   ws.e = ws.hd = ws.g = ws.h1 = ws.h2 = nullptr;
   ws.blob_e = ws.blob_hd = ws.blob_ci = ws.blob_h1 = ws.blob_h2 = ws.wimg_fwd = ws.wimg_bwd = nullptr;
+  ws.wgrad_part = nullptr;
   if (f->use_tc) {   // 16-bit operand-tile blobs: 2 bytes per value, 128-row tiles
     A(f->alloc(&ws.blob_e, 4 * ms.LF * cap));   /* two-term (hi | lo) tiles */ A(f->alloc(&ws.blob_hd, 2 * ms.Hd * cap)); A(f->alloc(&ws.blob_ci, 2 * 32 * cap));
     A(f->alloc(&ws.blob_h1, 2 * ms.Hc * cap)); A(f->alloc(&ws.blob_h2, 2 * (ms.n_color_layers == 2 ? ms.Hc : 1) * cap));
     A(f->alloc(&ws.wimg_fwd, mlp_tc_wimg_bytes(0))); A(f->alloc(&ws.wimg_bwd, mlp_tc_wimg_bytes(1)));
+    A(f->alloc(&ws.wgrad_part, (size_t)mlp_tc_backward_ctas(f->n_sms) * ms.n_mlp));
   } else {
     A(f->alloc(&ws.e, ms.LF * cap)); A(f->alloc(&ws.hd, ms.Hd * cap)); A(f->alloc(&ws.g, ms.Do * cap));
     A(f->alloc(&ws.h1, ms.Hc * cap)); A(f->alloc(&ws.h2, (ms.n_color_layers == 2 ? ms.Hc : 1) * cap));
   }
   A(f->alloc(&ws.sigma, cap)); A(f->alloc(&ws.rgb, 3 * cap)); A(f->alloc(&ws.T_excl, cap));
   A(f->alloc(&ws.dsigma, cap)); A(f->alloc(&ws.drgb, 3 * cap)); A(f->alloc(&ws.de, ms.LF * cap));
+  ws.timeline = nullptr;
+  {
+    const char *tl = std::getenv("NSM_TIMELINE");
+    if (tl && tl[0] == '1') {
+      A(f->alloc(&f->timeline_base, 64 * 2 * K_COUNT));
+      for (int i = 0; i < 64 && e == cudaSuccess; ++i)
+        e = cudaMemsetAsync(f->timeline_base + (size_t)i * 2 * K_COUNT, 0xff, sizeof(unsigned long long) * K_COUNT, f->stream);
+    }
+  }
   A(f->alloc(&ws.loss_acc, 3)); A(f->alloc(&ws.total_samples, 1)); A(f->alloc(&ws.grad_absmax, 1));
   A(f->alloc(&f->stage_dev, 11 * (size_t)R)); A(f->alloc(&f->stage_out, 5 * (size_t)R));
   if (e == cudaSuccess) e = cudaMallocHost((void **)&f->pinned, sizeof(*f->pinned));
@@ -632,7 +661,7 @@ nsm_status nsm_backward(nsm_field *f, const nsm_ray_batch *batch, float lambda_d
   nsm_status st = validate_batch(f, batch, true, false);
   if (st != NSM_OK) return st;
   f->side_ok = false;
-  st = enqueue_backward(f, batch, lambda_d, false, nullptr, host_stats != nullptr);
+  st = enqueue_backward(f, batch, lambda_d, false, nullptr, host_stats != nullptr, true);
   if (st != NSM_OK) return st;
   st = read_stats(f, batch->n_rays, host_stats);
   if (st == NSM_OK && host_stats) host_stats->loss = host_stats->loss_rgb + (double)lambda_d * host_stats->loss_depth;
@@ -686,6 +715,16 @@ nsm_status nsm_train_step_host(nsm_field *f, const nsm_ray_batch *hb, float lamb
   return train_step_impl(f, &db, lambda_d, host_stats ? host_stats : &local, false);  // always syncs: host buffers may be reused
 }
 
+nsm_status nsm_debug_timeline(nsm_field *f, uint64_t *h_out, uint64_t capacity_words, uint32_t *n_kernels) {
+  if (!f || !h_out) return fail(NSM_ERR_INVALID_ARG, "NULL argument");
+  if (!f->timeline_base) return fail(NSM_ERR_INVALID_ARG, "timeline not enabled (create the field with NSM_TIMELINE=1 in the environment)");
+  if (capacity_words < 64ull * 2 * K_COUNT) return fail(NSM_ERR_CAPACITY, "timeline needs %d words", 64 * 2 * K_COUNT);
+  CUDA_TRY(cudaStreamSynchronize(f->stream));
+  CUDA_TRY(cudaMemcpy(h_out, f->timeline_base, sizeof(uint64_t) * 64 * 2 * K_COUNT, cudaMemcpyDeviceToHost));
+  if (n_kernels) *n_kernels = K_COUNT;
+  return NSM_OK;
+}
+
 nsm_status nsm_set_option(nsm_field *f, nsm_option opt, uint32_t value) {
   if (!f) return fail(NSM_ERR_INVALID_ARG, "field is NULL");
   switch (opt) {
@@ -698,6 +737,7 @@ nsm_status nsm_debug_set_grad(nsm_field *f, const float *d_grad, const uint8_t *
   if (!f) return fail(NSM_ERR_INVALID_ARG, "field is NULL");
   f->side_ok = false;
   if (!d_grad) return fail(NSM_ERR_INVALID_ARG, "d_grad is NULL");
+  f->wgrad_parts = 0;
   RUN(f, K_DEBUG, launch_set_grad(f->fp, d_grad, d_touched, f->stream));
   CUDA_TRY(cudaMemcpyAsync(f->fp.mlp_grad, d_grad + f->fp.n_table, sizeof(float) * f->fp.n_mlp, cudaMemcpyDeviceToDevice, f->stream));
   f->grads_dirty = true;

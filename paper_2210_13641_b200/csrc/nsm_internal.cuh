@@ -64,6 +64,8 @@ struct Workspace {
   // tensor-core path: 16-bit operand-tile images ("blobs", see mlp_tc.cu) instead of the fp32 planes e/hd/g/h1/h2
   uint8_t *blob_e, *blob_hd, *blob_ci, *blob_h1, *blob_h2;
   uint8_t *wimg_fwd, *wimg_bwd;       // 16-bit weight images, repacked whenever the MLP weights change
+  unsigned long long *timeline;       // debug (NSM_TIMELINE=1): [2][K_COUNT] first-block start / last-block end, globaltimer ns
+  float *wgrad_part;                  // [mlp_tc_backward_ctas][n_mlp] per-CTA weight-gradient slices of the tensor-core backward
   uint32_t *grad_absmax;              // bits of max |dL/d(pre-activation)| entering S11 this step (loss scale)
 };
 
@@ -72,6 +74,18 @@ enum KernelId {
   K_MARCH = 0, K_ENCODE, K_MLP_FWD, K_COMPOSITE, K_MLP_BWD, K_SCATTER,
   K_ADAM_TABLE, K_ADAM_MLP, K_OCC, K_DEBUG, K_COUNT
 };
+
+// Debug timeline: when ws.timeline is set, thread 0 of every block stamps the kernel class's earliest start
+// and latest end with %globaltimer.  Unlike CUDA events between launches this does not disturb PDL or the
+// two-stream overlap, so it shows the step as it really runs.
+__device__ __forceinline__ void tl_mark(unsigned long long *tl, int id, int end) {
+  if (tl && threadIdx.x == 0) {
+    unsigned long long t;
+    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
+    if (end) atomicMax(tl + K_COUNT + id, t);
+    else atomicMin(tl + id, t);
+  }
+}
 
 // Parameters.  Hash-table entries are stored as RECORDS of 4F floats,
 //   rec[e*4F + 0F .. 1F) = theta   rec[.. 1F..2F) = spare   rec[.. 2F..3F) = Adam m   rec[.. 3F..4F) = Adam v
@@ -227,8 +241,11 @@ size_t mlp_tc_wimg_bytes(int backward);
 int launch_pack_weights(const MlpShape &ms, int bf16, const float *theta_mlp, const Workspace &ws, cudaStream_t st);
 int launch_mlp_forward_tc(const MlpShape &ms, int bf16, const float *dirs, const Workspace &ws, const uint32_t *d_S,
                           int density_only, int save_blobs, int n_sms, cudaStream_t st);
-int launch_mlp_backward_tc(const MlpShape &ms, int bf16, float *grad_mlp, const Workspace &ws, const uint32_t *d_S,
+// weight gradients: one slice of ws.wgrad_part per CTA (mlp_tc_backward_ctas of them), summed by the consumer
+int launch_mlp_backward_tc(const MlpShape &ms, int bf16, const Workspace &ws, const uint32_t *d_S,
                            int n_sms, cudaStream_t st);
+uint32_t mlp_tc_backward_ctas(int n_sms);
+int launch_reduce_wgrad(const MlpShape &ms, const Workspace &ws, float *grad_mlp, uint32_t n_ctas, const uint32_t *d_S, cudaStream_t st);
 int launch_blob_to_rows(int bf16, const uint8_t *blob, uint32_t n_cols, int two_term, const uint32_t *d_S, float *rows,
                         cudaStream_t st);
 int launch_composite_train(const Workspace &ws, uint32_t R, const float *rgb, const float *depth,
@@ -237,12 +254,13 @@ int launch_composite_train(const Workspace &ws, uint32_t R, const float *rgb, co
 int launch_composite_render(const Workspace &ws, uint32_t R, float cut, const float bg[3],
                             float *out_rgb, float *out_depth, float *out_opacity, cudaStream_t st);
 int launch_adam_table(const FieldParams &fp, uint32_t F, int sparse, float lr, float beta1, float beta2,
-                      float eps, float inv_bc1, float inv_bc2, int n_sms, cudaStream_t st);
+                      float eps, float inv_bc1, float inv_bc2, int n_sms, cudaStream_t st, unsigned long long *tl = nullptr);
 int launch_adam_mlp(const FieldParams &fp, float lr, float beta1, float beta2, float eps, float inv_bc1,
                     float inv_bc2, cudaStream_t st);
 // tensor-core path: Adam on the MLP weights and, in the same launch, the refreshed 16-bit weight images
+// n_ctas > 0: the gradient is the sum of the backward kernel's slices (+ fp.mlp_grad); 0: fp.mlp_grad alone
 int launch_adam_mlp_pack(const MlpShape &ms, int bf16, const FieldParams &fp, const Workspace &ws, const AdamConst &c,
-                         cudaStream_t st);
+                         uint32_t n_ctas, const uint32_t *d_S, cudaStream_t st);
 int launch_occ_cells(uint32_t G, uint64_t first_cell, uint64_t n_cells, const Workspace &ws,
                      uint32_t *d_S, cudaStream_t st);
 int launch_occ_threshold(uint32_t G, uint64_t first_cell, uint64_t n_cells, const float *sigma,
