@@ -12,27 +12,31 @@ namespace {
 //     per thread; the array is L2-hot, the scatter has just written it).  Entries whose first word
 //     is not -0.0f (FieldParams: "referenced this step") are compacted into shared memory
 //     (index + gradient), warp-aggregated.
-//  2. The block walks the compact list: every thread has a touched entry, loads its record
-//     (theta | spare | m | v; one 32-byte sector for F = 2; two entries in flight per thread),
-//     updates and stores it.  The whole gradient chunk is then reset to -0.0f with coalesced
+//  2. The block walks the compact list: every thread has a touched entry, loads its theta (compact
+//     array) and its moment record (m | v; 16 bytes for F = 2; two entries in flight per thread),
+//     updates and stores them.  The whole gradient chunk is then reset to -0.0f with coalesced
 //     stores, so the next step's scatter starts from "untouched" without a separate pass.
 // sparse = 0 (dense Adam, textbook): every entry goes through phase 2.
 constexpr int ADAM_CHUNK_FLOATS = 4096;
 constexpr int ADAM_THREADS = 256;
 
+// one touched entry: theta (F floats of the compact array) and its moment record (m | v, 2F floats)
 template <int F>
-__device__ __forceinline__ void adam_record(float *__restrict__ r, const float *g, const AdamConst &c, uint64_t pol_ld, uint64_t pol) {
+__device__ __forceinline__ void adam_entry(float *__restrict__ th_p, float *__restrict__ mv_p, const float *g, const AdamConst &c,
+                                           uint64_t pol_ld, uint64_t pol_st) {
   float th[F], m[F], v[F];
   if constexpr (F == 1) {
-    const float4 t = ld_hint_f4(r, pol_ld);
-    th[0] = t.x; m[0] = t.z; v[0] = t.w;
+    th[0] = ld_hint_f1(th_p, pol_ld);
+    const float2 t = ld_hint_f2(mv_p, pol_ld);
+    m[0] = t.x; v[0] = t.y;
   } else if constexpr (F == 2) {
-    const float4 a = ld_hint_f4(r, pol_ld), b = ld_hint_f4(r + 4, pol_ld);
+    const float2 a = ld_hint_f2(th_p, pol_ld);
+    const float4 b = ld_hint_f4(mv_p, pol_ld);
     th[0] = a.x; th[1] = a.y; m[0] = b.x; m[1] = b.y; v[0] = b.z; v[1] = b.w;
   } else {
 #pragma unroll
     for (int i = 0; i < F / 4; ++i) {
-      const float4 a = ld_hint_f4(r + 4 * i, pol_ld), b = ld_hint_f4(r + 2 * F + 4 * i, pol_ld), d = ld_hint_f4(r + 3 * F + 4 * i, pol_ld);
+      const float4 a = ld_hint_f4(th_p + 4 * i, pol_ld), b = ld_hint_f4(mv_p + 4 * i, pol_ld), d = ld_hint_f4(mv_p + F + 4 * i, pol_ld);
       th[4 * i] = a.x; th[4 * i + 1] = a.y; th[4 * i + 2] = a.z; th[4 * i + 3] = a.w;
       m[4 * i] = b.x; m[4 * i + 1] = b.y; m[4 * i + 2] = b.z; m[4 * i + 3] = b.w;
       v[4 * i] = d.x; v[4 * i + 1] = d.y; v[4 * i + 2] = d.z; v[4 * i + 3] = d.w;
@@ -41,23 +45,23 @@ __device__ __forceinline__ void adam_record(float *__restrict__ r, const float *
 #pragma unroll
   for (int f = 0; f < F; ++f) adam_one(th[f], m[f], v[f], g[f], c);
   if constexpr (F == 1) {
-    st_hint_f1(r, th[0], pol);
-    st_hint_f2(r + 2, make_float2(m[0], v[0]), pol);
+    st_hint_f1(th_p, th[0], pol_st);
+    st_hint_f2(mv_p, make_float2(m[0], v[0]), pol_st);
   } else if constexpr (F == 2) {
-    st_hint_f2(r, make_float2(th[0], th[1]), pol);
-    st_hint_f4(r + 4, make_float4(m[0], m[1], v[0], v[1]), pol);
+    st_hint_f2(th_p, make_float2(th[0], th[1]), pol_st);
+    st_hint_f4(mv_p, make_float4(m[0], m[1], v[0], v[1]), pol_st);
   } else {
 #pragma unroll
     for (int i = 0; i < F / 4; ++i) {
-      st_hint_f4(r + 4 * i, make_float4(th[4 * i], th[4 * i + 1], th[4 * i + 2], th[4 * i + 3]), pol);
-      st_hint_f4(r + 2 * F + 4 * i, make_float4(m[4 * i], m[4 * i + 1], m[4 * i + 2], m[4 * i + 3]), pol);
-      st_hint_f4(r + 3 * F + 4 * i, make_float4(v[4 * i], v[4 * i + 1], v[4 * i + 2], v[4 * i + 3]), pol);
+      st_hint_f4(th_p + 4 * i, make_float4(th[4 * i], th[4 * i + 1], th[4 * i + 2], th[4 * i + 3]), pol_st);
+      st_hint_f4(mv_p + 4 * i, make_float4(m[4 * i], m[4 * i + 1], m[4 * i + 2], m[4 * i + 3]), pol_st);
+      st_hint_f4(mv_p + F + 4 * i, make_float4(v[4 * i], v[4 * i + 1], v[4 * i + 2], v[4 * i + 3]), pol_st);
     }
   }
 }
 
 template <int F>
-__global__ void __launch_bounds__(ADAM_THREADS) adam_table_kernel(float *__restrict__ rec, float *__restrict__ grad,
+__global__ void __launch_bounds__(ADAM_THREADS) adam_table_kernel(float *__restrict__ theta, float *__restrict__ mv, float *__restrict__ grad,
                                                                   uint64_t n_entries, int sparse, AdamConst c,
                                                                   unsigned long long *tl) {
   constexpr int CH = ADAM_CHUNK_FLOATS / F;            // entries per chunk
@@ -124,13 +128,12 @@ __global__ void __launch_bounds__(ADAM_THREADS) adam_table_kernel(float *__restr
   // phase 2: two records in flight per thread
   for (uint32_t i0 = tid; i0 < n; i0 += 2 * ADAM_THREADS) {
     const uint32_t i1 = i0 + ADAM_THREADS;
-    float *r0 = rec + (e_base + list_e[i0]) * 4 * F;
-    float *r1 = rec + (e_base + list_e[i1 < n ? i1 : i0]) * 4 * F;
-    if constexpr (F == 2) {   // touch the second record's sector early
-      asm volatile("prefetch.global.L2 [%0];" ::"l"(r1));
+    const uint64_t e0 = e_base + list_e[i0], e1 = e_base + list_e[i1 < n ? i1 : i0];
+    if constexpr (F == 2) {   // touch the second entry's moment record early
+      asm volatile("prefetch.global.L2 [%0];" ::"l"(mv + e1 * 2 * F));
     }
-    adam_record<F>(r0, list_g + i0 * F, c, pol_ld, pol_first);
-    if (i1 < n) adam_record<F>(r1, list_g + i1 * F, c, pol_ld, pol_first);
+    adam_entry<F>(theta + e0 * F, mv + e0 * 2 * F, list_g + i0 * F, c, pol_ld, pol_first);
+    if (i1 < n) adam_entry<F>(theta + e1 * F, mv + e1 * 2 * F, list_g + i1 * F, c, pol_ld, pol_first);
   }
   // reset the chunk's gradient words
   float *o4 = grad + e_base * F;
@@ -163,10 +166,10 @@ int launch_adam_table(const FieldParams &fp, uint32_t F, int sparse, float lr, f
   const uint64_t chunk = ADAM_CHUNK_FLOATS / F;
   dim3 grid((unsigned)((fp.n_entries + chunk - 1) / chunk)), block(ADAM_THREADS);
   switch (F) {
-    case 1: launch_pdl(adam_table_kernel<1>, grid, block, 0, st, fp.rec, fp.grad, fp.n_entries, sparse, c, tl); break;
-    case 2: launch_pdl(adam_table_kernel<2>, grid, block, 0, st, fp.rec, fp.grad, fp.n_entries, sparse, c, tl); break;
-    case 4: launch_pdl(adam_table_kernel<4>, grid, block, 0, st, fp.rec, fp.grad, fp.n_entries, sparse, c, tl); break;
-    default: launch_pdl(adam_table_kernel<8>, grid, block, 0, st, fp.rec, fp.grad, fp.n_entries, sparse, c, tl); break;
+    case 1: launch_pdl(adam_table_kernel<1>, grid, block, 0, st, fp.theta, fp.mv, fp.grad, fp.n_entries, sparse, c, tl); break;
+    case 2: launch_pdl(adam_table_kernel<2>, grid, block, 0, st, fp.theta, fp.mv, fp.grad, fp.n_entries, sparse, c, tl); break;
+    case 4: launch_pdl(adam_table_kernel<4>, grid, block, 0, st, fp.theta, fp.mv, fp.grad, fp.n_entries, sparse, c, tl); break;
+    default: launch_pdl(adam_table_kernel<8>, grid, block, 0, st, fp.theta, fp.mv, fp.grad, fp.n_entries, sparse, c, tl); break;
   }
   return 1;
 }

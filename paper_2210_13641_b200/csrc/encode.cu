@@ -99,7 +99,7 @@ __device__ __forceinline__ void load_entry(const float *p, float out[F]) {
 // tensor-core MLP kernels ([tile][8-column panel][128 rows][8 x 16 bit], mlp_tc.cu); the rows of
 // the last tile beyond S are zero-filled so the MMA never reads stale data.
 template <int F, int MODE>
-__global__ void __launch_bounds__(256) encode_forward_kernel(LevelTable lv, const float *__restrict__ rec,
+__global__ void __launch_bounds__(256) encode_forward_kernel(LevelTable lv, const float *__restrict__ theta,
                                                              Workspace ws, const uint32_t *__restrict__ d_S) {
   pdl_wait();
   pdl_trigger();
@@ -118,15 +118,15 @@ __global__ void __launch_bounds__(256) encode_forward_kernel(LevelTable lv, cons
     for (int f = 0; f < F; ++f) acc[f] = 0.0f;
     if (s < S) {
       CornerIndex ci = corner_index(lv, l, ws.s_x[s], ws.s_x[ws.cap + s], ws.s_x[2 * ws.cap + s]);
-      const float *tab = rec + lv.offset[l] * (4 * F);   // theta = the first F floats of a 4F-float record
+      const float *tab = theta + lv.offset[l] * F;
       float v[8][F];
 #pragma unroll
       if (lv.dense[l]) {   // coarse levels are re-read every step: normal policy; hashed levels stream through L2
 #pragma unroll
-        for (int k = 0; k < 8; ++k) load_entry<F>(tab + (size_t)ci.slot[k] * (4 * F), v[k]);  // 8 gathers in flight
+        for (int k = 0; k < 8; ++k) load_entry<F>(tab + (size_t)ci.slot[k] * F, v[k]);  // 8 gathers in flight
       } else {
 #pragma unroll
-        for (int k = 0; k < 8; ++k) load_entry_hint<F>(tab + (size_t)ci.slot[k] * (4 * F), v[k], pol_first);
+        for (int k = 0; k < 8; ++k) load_entry_hint<F>(tab + (size_t)ci.slot[k] * F, v[k], pol_first);
       }
 #pragma unroll
       for (int k = 0; k < 8; ++k) {
@@ -256,35 +256,39 @@ __global__ void planes_to_rows_kernel(const float *__restrict__ planes, uint64_t
   }
 }
 
-__global__ void pack_records_kernel(float *__restrict__ rec, uint32_t F, uint64_t n_entries, int which,
+__device__ __forceinline__ uint64_t param_index(uint32_t F, uint64_t e, uint32_t f, int which) {
+  return which == 0 ? e * F + f : e * 2 * F + (which == 3 ? F : 0) + f;
+}
+
+__global__ void pack_records_kernel(float *__restrict__ theta, float *__restrict__ mv, uint32_t F, uint64_t n_entries, int which,
                                     const float *__restrict__ src) {
   const uint64_t total = n_entries * F;
+  float *dst = which == 0 ? theta : mv;
   for (uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; i < total; i += (uint64_t)gridDim.x * blockDim.x) {
     const uint64_t e = i / F;
-    const uint32_t f = (uint32_t)(i - e * F);
-    rec[e * 4 * F + (uint64_t)which * F + f] = src ? src[i] : 0.f;
+    dst[param_index(F, e, (uint32_t)(i - e * F), which)] = src ? src[i] : 0.f;
   }
 }
 
-__global__ void unpack_records_kernel(const float *__restrict__ rec, uint32_t F, uint64_t n_entries, int which,
-                                      float *__restrict__ dst) {
+__global__ void unpack_records_kernel(const float *__restrict__ theta, const float *__restrict__ mv, uint32_t F, uint64_t n_entries,
+                                      int which, float *__restrict__ dst) {
   const uint64_t total = n_entries * F;
+  const float *src = which == 0 ? theta : mv;
   for (uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; i < total; i += (uint64_t)gridDim.x * blockDim.x) {
     const uint64_t e = i / F;
-    const uint32_t f = (uint32_t)(i - e * F);
-    dst[i] = rec[e * 4 * F + (uint64_t)which * F + f];
+    dst[i] = src[param_index(F, e, (uint32_t)(i - e * F), which)];
   }
 }
 
 }  // namespace
 
 int launch_pack_records(const FieldParams &fp, int which, const float *src, cudaStream_t st) {
-  pack_records_kernel<<<2048, 256, 0, st>>>(fp.rec, fp.F, fp.n_entries, which, src);
+  pack_records_kernel<<<2048, 256, 0, st>>>(fp.theta, fp.mv, fp.F, fp.n_entries, which, src);
   return 1;
 }
 
 int launch_unpack_records(const FieldParams &fp, int which, float *dst, cudaStream_t st) {
-  unpack_records_kernel<<<2048, 256, 0, st>>>(fp.rec, fp.F, fp.n_entries, which, dst);
+  unpack_records_kernel<<<2048, 256, 0, st>>>(fp.theta, fp.mv, fp.F, fp.n_entries, which, dst);
   return 1;
 }
 

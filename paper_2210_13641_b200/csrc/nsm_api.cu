@@ -252,7 +252,7 @@ void enqueue_forward(nsm_field *f, const nsm_ray_batch *b, uint32_t R, bool jitt
     RUN(f, K_MARCH, launch_march(mp, f->occ_full ? nullptr : f->fp.occ_bits, b->origins, b->dirs, f->ws, train ? 1 : 0, f->stream, dirs_copy));
   }
   const int bf16 = f->cfg.mlp_precision == NSM_MLP_BF16;
-  RUN(f, K_ENCODE, launch_encode(f->lv, f->fp.rec, f->ws, d_S, f->use_tc ? 1 + bf16 : 0, f->n_sms, f->stream));
+  RUN(f, K_ENCODE, launch_encode(f->lv, f->fp.theta, f->ws, d_S, f->use_tc ? 1 + bf16 : 0, f->n_sms, f->stream));
   if (f->use_tc)
     RUN(f, K_MLP_FWD, launch_mlp_forward_tc(f->ms, bf16, mlp_dirs, f->ws, d_S, 0, train ? 1 : 0, f->n_sms, f->stream));
   else
@@ -458,7 +458,7 @@ nsm_status nsm_create_field(const nsm_field_config *cfg, void *cuda_stream, nsm_
   const uint32_t R = cfg->max_rays;
   cudaError_t e = cudaSuccess;
   auto A = [&](cudaError_t r) { if (e == cudaSuccess) e = r; };
-  A(f->alloc(&fp.rec, 4 * fp.n_table));
+  A(f->alloc(&fp.theta, fp.n_table)); A(f->alloc(&fp.mv, 2 * fp.n_table));
   A(f->alloc(&fp.mlp_theta, fp.n_mlp)); A(f->alloc(&fp.mlp_m, fp.n_mlp)); A(f->alloc(&fp.mlp_v, fp.n_mlp)); A(f->alloc(&fp.mlp_grad, fp.n_mlp));
   A(f->alloc(&fp.grad, fp.n_table, false)); A(f->alloc(&fp.occ_bits, (G3 + 7) / 8 + 4));
   A(f->alloc(&ws.counts, R)); A(f->alloc(&ws.offsets, R + 1)); A(f->alloc(&ws.scan_state, march_scan_state_entries(R) + 1)); A(f->alloc(&ws.scan_ctr, 2));
@@ -639,7 +639,7 @@ nsm_status nsm_update_occupancy(nsm_field *f, nsm_occ_mode mode, const uint8_t *
       for (uint64_t first = 0; first < G3; first += chunk) {
         const uint64_t n = (G3 - first < chunk) ? G3 - first : chunk;
         RUN(f, K_OCC, launch_occ_cells(f->cfg.occ_res, first, n, f->ws, d_S, f->stream));
-        RUN(f, K_ENCODE, launch_encode(f->lv, f->fp.rec, f->ws, d_S, f->use_tc ? 1 + (f->cfg.mlp_precision == NSM_MLP_BF16) : 0,
+        RUN(f, K_ENCODE, launch_encode(f->lv, f->fp.theta, f->ws, d_S, f->use_tc ? 1 + (f->cfg.mlp_precision == NSM_MLP_BF16) : 0,
                                        f->n_sms, f->stream));
         if (f->use_tc)
           RUN(f, K_MLP_FWD, launch_mlp_forward_tc(f->ms, f->cfg.mlp_precision == NSM_MLP_BF16, nullptr, f->ws, d_S, 1, 0, f->n_sms,

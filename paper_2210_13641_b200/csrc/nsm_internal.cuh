@@ -87,13 +87,15 @@ __device__ __forceinline__ void tl_mark(unsigned long long *tl, int id, int end)
   }
 }
 
-// Parameters.  Hash-table entries are stored as RECORDS of 4F floats,
-//   rec[e*4F + 0F .. 1F) = theta   rec[.. 1F..2F) = spare   rec[.. 2F..3F) = Adam m   rec[.. 3F..4F) = Adam v
-// so that with F = 2 an entry is exactly one 32-byte DRAM/L2 sector: the touched-only Adam update
-// (a random 25 % of the entries per step at config 2) moves one sector per entry.  The GRADIENT is
-// a separate, compact array grad[e*F + f] (48.8 MB at config 2, L2-sized): the scatter's vector
-// reductions land in a table that fits the cache instead of one four times its size, and Adam
-// reads it as a dense coalesced stream.
+// Parameters.  Three arrays over the table entries, each sized for what reads it:
+//   theta[e*F + f]          the values the encoder gathers: compact (48.8 MB at config 2), so a 64-byte DRAM fetch
+//                           brings 8 entries (F = 2) and the x-neighbour corner pairs of a cell share a 16-byte word;
+//   mv[e*2F + 0..F) = m,    Adam moments, one 4F-byte record per entry (16 B for F = 2): only the table Adam touches
+//   mv[e*2F + F..2F) = v    them, for the random ~25 % of entries a step references;
+//   grad[e*F + f]           the gradient, compact like theta (L2-sized): the scatter's vector reductions land in a
+//                           table that fits the cache, and Adam reads it as a dense coalesced stream.
+// (Measured on B200, profiles/r1h: with theta inside 32-byte per-entry records the encoder moved 120 MB of DRAM
+// for 12 MB of useful theta and ran at 81 % of the HBM peak; DRAM fetches are 64 bytes.)
 //
 // Touched set without flags: between steps every gradient word holds -0.0f (bits 0x80000000).
 // The scatter never adds -0.0 or a magnitude below 2^-96 (those addends become +0.0), and under
@@ -105,7 +107,8 @@ __device__ __forceinline__ void tl_mark(unsigned long long *tl, int id, int end)
 #define NSM_GRAD_UNTOUCHED 0x80000000u
 #define NSM_GRAD_MIN_ADDEND 1.262177448e-29f   /* 2^-96 */
 struct FieldParams {
-  float *rec;                                       // [n_entries][4F]
+  float *theta;                                     // [n_entries][F]
+  float *mv;                                        // [n_entries][2F]
   float *grad;                                      // [n_entries][F]
   float *mlp_theta, *mlp_m, *mlp_v, *mlp_grad;      // [n_mlp] each, canonical order
   uint8_t *occ_bits;                                // [G^3/8]
@@ -219,14 +222,14 @@ int launch_march(const MarchParams &mp, const uint8_t *bits, const float *origin
                  const Workspace &ws, int count_total, cudaStream_t st, float *dirs_copy = nullptr);
 uint32_t march_scan_state_entries(uint32_t max_rays);
 // out_mode: 0 = fp32 planes ws.e, 1 = fp16 blob ws.blob_e, 2 = bf16 blob ws.blob_e
-int launch_encode(const LevelTable &lv, const float *rec, const Workspace &ws,
+int launch_encode(const LevelTable &lv, const float *theta, const Workspace &ws,
                   const uint32_t *d_S, int out_mode, int n_sms, cudaStream_t st);
 int launch_scatter(const LevelTable &lv, float *grad, const Workspace &ws,
                    const uint32_t *d_S, int n_sms, cudaStream_t st);
 // gradient array <- canonical gradient + touched flags (NULL: every entry touched); src == nullptr: all untouched
 int launch_set_grad(const FieldParams &fp, const float *src, const uint8_t *touched, cudaStream_t st);
 int launch_get_touched(const FieldParams &fp, uint8_t *dst, cudaStream_t st);
-// canonical [n_entries][F] <-> field `which` (0 theta, 2 m, 3 v) of the records; src == nullptr packs zeros
+// canonical [n_entries][F] <-> `which` (0 theta, 2 m, 3 v) of the internal arrays; src == nullptr packs zeros
 int launch_pack_records(const FieldParams &fp, int which, const float *src, cudaStream_t st);
 int launch_unpack_records(const FieldParams &fp, int which, float *dst, cudaStream_t st);
 int launch_mlp_forward_simt(const MlpShape &ms, const float *theta_mlp, const float *dirs,
