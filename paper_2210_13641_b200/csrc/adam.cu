@@ -62,7 +62,7 @@ __device__ __forceinline__ void adam_entry(float *__restrict__ th_p, float *__re
 
 template <int F>
 __global__ void __launch_bounds__(ADAM_THREADS) adam_table_kernel(float *__restrict__ theta, float *__restrict__ mv, float *__restrict__ grad,
-                                                                  uint64_t n_entries, int sparse, AdamConst c,
+                                                                  uint64_t first_entry, uint64_t n_entries, int sparse, AdamConst c,
                                                                   unsigned long long *tl) {
   constexpr int CH = ADAM_CHUNK_FLOATS / F;            // entries per chunk
   constexpr int NV = ADAM_CHUNK_FLOATS / 4 / ADAM_THREADS;   // float4 loads per thread
@@ -73,7 +73,7 @@ __global__ void __launch_bounds__(ADAM_THREADS) adam_table_kernel(float *__restr
   pdl_wait();
   pdl_trigger();
   tl_mark(tl, K_ADAM_TABLE, 0);
-  const uint64_t e_base = (uint64_t)blockIdx.x * CH;
+  const uint64_t e_base = first_entry + (uint64_t)blockIdx.x * CH;   // first_entry is a multiple of 4 entries (16-byte loads)
   const uint64_t n_float = n_entries * F;
   const float *g4 = grad + e_base * F;
   const uint64_t pol_first = l2_evict_first(), pol_last = l2_evict_last(), pol_ld = l2_evict_normal();
@@ -159,17 +159,18 @@ __global__ void adam_dense_kernel(float *__restrict__ theta, float *__restrict__
 
 }  // namespace
 
+// entries [first_entry, end_entry): a level group (first_entry must be a multiple of 4)
 int launch_adam_table(const FieldParams &fp, uint32_t F, int sparse, float lr, float beta1, float beta2, float eps,
-                      float inv_bc1, float inv_bc2, int n_sms, cudaStream_t st, unsigned long long *tl) {
-  (void)n_sms;
+                      float inv_bc1, float inv_bc2, uint64_t first_entry, uint64_t end_entry, cudaStream_t st,
+                      unsigned long long *tl) {
   AdamConst c{lr, beta1, beta2, eps, inv_bc1, inv_bc2};
   const uint64_t chunk = ADAM_CHUNK_FLOATS / F;
-  dim3 grid((unsigned)((fp.n_entries + chunk - 1) / chunk)), block(ADAM_THREADS);
+  dim3 grid((unsigned)((end_entry - first_entry + chunk - 1) / chunk)), block(ADAM_THREADS);
   switch (F) {
-    case 1: launch_pdl(adam_table_kernel<1>, grid, block, 0, st, fp.theta, fp.mv, fp.grad, fp.n_entries, sparse, c, tl); break;
-    case 2: launch_pdl(adam_table_kernel<2>, grid, block, 0, st, fp.theta, fp.mv, fp.grad, fp.n_entries, sparse, c, tl); break;
-    case 4: launch_pdl(adam_table_kernel<4>, grid, block, 0, st, fp.theta, fp.mv, fp.grad, fp.n_entries, sparse, c, tl); break;
-    default: launch_pdl(adam_table_kernel<8>, grid, block, 0, st, fp.theta, fp.mv, fp.grad, fp.n_entries, sparse, c, tl); break;
+    case 1: launch_pdl(adam_table_kernel<1>, grid, block, 0, st, fp.theta, fp.mv, fp.grad, first_entry, end_entry, sparse, c, tl); break;
+    case 2: launch_pdl(adam_table_kernel<2>, grid, block, 0, st, fp.theta, fp.mv, fp.grad, first_entry, end_entry, sparse, c, tl); break;
+    case 4: launch_pdl(adam_table_kernel<4>, grid, block, 0, st, fp.theta, fp.mv, fp.grad, first_entry, end_entry, sparse, c, tl); break;
+    default: launch_pdl(adam_table_kernel<8>, grid, block, 0, st, fp.theta, fp.mv, fp.grad, first_entry, end_entry, sparse, c, tl); break;
   }
   return 1;
 }

@@ -180,17 +180,17 @@ __device__ __forceinline__ void red_add_entry(float *p, const float g[F], uint64
 // themselves, see FieldParams in nsm_internal.cuh.
 template <int F>
 __global__ void __launch_bounds__(256) scatter_backward_kernel(LevelTable lv, float *__restrict__ grad, Workspace ws,
-                                                               const uint32_t *__restrict__ d_S) {
+                                                               const uint32_t *__restrict__ d_S, uint32_t l0, uint32_t l1) {
   pdl_wait();
   pdl_trigger();
   tl_mark(ws.timeline, K_SCATTER, 0);
   const uint64_t S = *d_S;
-  const uint64_t total = S * lv.n_levels;
+  const uint64_t total = S * (l1 - l0);
   const uint64_t pol_last = l2_evict_last();
   for (uint64_t wi = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; wi < total;
        wi += (uint64_t)gridDim.x * blockDim.x) {
-    const uint32_t l = (uint32_t)(wi / S);
-    const uint64_t s = wi - (uint64_t)l * S;
+    const uint32_t l = l0 + (uint32_t)(wi / S);
+    const uint64_t s = wi - (uint64_t)(l - l0) * S;
     CornerIndex ci = corner_index(lv, l, ws.s_x[s], ws.s_x[ws.cap + s], ws.s_x[2 * ws.cap + s]);
     float de[F];
 #pragma unroll
@@ -323,13 +323,13 @@ int launch_get_touched(const FieldParams &fp, uint8_t *dst, cudaStream_t st) {
 }
 
 int launch_scatter(const LevelTable &lv, float *grad, const Workspace &ws,
-                   const uint32_t *d_S, int n_sms, cudaStream_t st) {
+                   const uint32_t *d_S, uint32_t l0, uint32_t l1, int n_sms, cudaStream_t st) {
   dim3 grid(n_sms * 8), block(256);
   switch (lv.n_features) {
-    case 1: launch_pdl(scatter_backward_kernel<1>, grid, block, 0, st, lv, grad, ws, d_S); break;
-    case 2: launch_pdl(scatter_backward_kernel<2>, grid, block, 0, st, lv, grad, ws, d_S); break;
-    case 4: launch_pdl(scatter_backward_kernel<4>, grid, block, 0, st, lv, grad, ws, d_S); break;
-    default: launch_pdl(scatter_backward_kernel<8>, grid, block, 0, st, lv, grad, ws, d_S); break;
+    case 1: launch_pdl(scatter_backward_kernel<1>, grid, block, 0, st, lv, grad, ws, d_S, l0, l1); break;
+    case 2: launch_pdl(scatter_backward_kernel<2>, grid, block, 0, st, lv, grad, ws, d_S, l0, l1); break;
+    case 4: launch_pdl(scatter_backward_kernel<4>, grid, block, 0, st, lv, grad, ws, d_S, l0, l1); break;
+    default: launch_pdl(scatter_backward_kernel<8>, grid, block, 0, st, lv, grad, ws, d_S, l0, l1); break;
   }
   return 1;
 }

@@ -2,6 +2,7 @@
 // (parameters, Adam state, occupancy bits, workspace arena) and the host-side step scheduler
 // that enqueues the kernels of S1..S15 on the field's stream.  No arithmetic of the method is
 // done on the host except S0's integer level table and Adam's scalar bias corrections.
+#include <algorithm>
 #include <cmath>
 #include <cstdarg>
 #include <cstdio>
@@ -108,6 +109,8 @@ struct nsm_field {
   cudaEvent_t ev_comp = nullptr, ev_stats = nullptr;
   bool stats_pending = false;
   unsigned long long *timeline_base = nullptr;   // NSM_TIMELINE=1: ring of 64 steps x [2][K_COUNT] globaltimer stamps
+  bool scatter_pending = false;   // the backward pass stopped before S12: enqueue_adam interleaves scatter and Adam per level group
+  uint32_t n_groups = 1;          // level groups of the scatter + Adam phase (NSM_LEVEL_GROUPS)
   uint32_t wgrad_parts = 0;   // > 0: the MLP weight gradient of the last backward is still in that many per-CTA slices
   bool batch_ready = false;   // NSM_OPT_BATCH_READY
   bool side_ok = false;       // nothing but a train step's Adam has been enqueued on `stream` since ev_pre_adam
@@ -276,7 +279,8 @@ nsm_status clear_grads_if_dirty(nsm_field *f) {
 }
 
 nsm_status enqueue_backward(nsm_field *f, const nsm_ray_batch *b, float lambda_d, bool march_on_side = false,
-                            float *dirs_copy = nullptr, bool want_stats = false, bool reduce_wgrad_now = false) {
+                            float *dirs_copy = nullptr, bool want_stats = false, bool reduce_wgrad_now = false,
+                            bool defer_scatter = false) {
   const uint32_t R = b->n_rays;
   const uint32_t *d_S = f->ws.offsets + R;
   nsm_status st = clear_grads_if_dirty(f);
@@ -309,7 +313,9 @@ nsm_status enqueue_backward(nsm_field *f, const nsm_ray_batch *b, float lambda_d
   else
     RUN(f, K_MLP_BWD, launch_mlp_backward_simt(f->ms, f->fp.mlp_theta, f->fp.mlp_grad, dirs_copy ? dirs_copy : b->dirs,
                                                f->ws, d_S, f->n_sms, f->stream));
-  RUN(f, K_SCATTER, launch_scatter(f->lv, f->fp.grad, f->ws, d_S, f->n_sms, f->stream));
+  // train step: the scatter is issued by enqueue_adam, level group by level group, each followed by its Adam
+  f->scatter_pending = defer_scatter;
+  if (!defer_scatter) RUN(f, K_SCATTER, launch_scatter(f->lv, f->fp.grad, f->ws, d_S, 0, f->lv.n_levels, f->n_sms, f->stream));
   f->grads_dirty = true;
   f->last_R = R;
   f->last_K = b->n_candidates;
@@ -339,8 +345,39 @@ nsm_status enqueue_adam(nsm_field *f) {
     RUN_ON(f, K_ADAM_MLP, s_mlp, launch_adam_mlp(f->fp, f->cfg.lr, f->cfg.beta1, f->cfg.beta2, f->cfg.eps, (float)(1.0 / bc1),
                                                  (float)(1.0 / bc2), s_mlp));
   }
-  RUN(f, K_ADAM_TABLE, launch_adam_table(f->fp, f->cfg.n_features, f->cfg.sparse_table_adam != 0, f->cfg.lr, f->cfg.beta1,
-                                         f->cfg.beta2, f->cfg.eps, (float)(1.0 / bc1), (float)(1.0 / bc2), f->n_sms, f->stream, f->ws.timeline));
+  // S12 + S13 on the tables.  The scatter and the Adam pass can be issued per level group (NSM_LEVEL_GROUPS = G:
+  // scatter(group) then Adam(group), so that a group's slice of the gradient array stays in L2 between its three
+  // uses).  Measured on B200 at config 2 (profiles/r1j): G = 1 118.9 us/step, 2 138.2, 3 149.1, 4 160.8, 8 201.0 --
+  // every extra pair of launches costs ~19 us of ramp and tail, far more than the ~100 MB of DRAM traffic it saves,
+  // so the default is one group.  Group boundaries are level boundaries rounded DOWN to 4 entries.
+  {
+    const uint32_t L = f->lv.n_levels;
+    const uint64_t E = f->fp.n_entries;
+    const uint32_t G = f->scatter_pending ? (f->n_groups < L ? f->n_groups : L) : 1;
+    const uint32_t *d_S = f->ws.offsets + f->last_R;
+    const int sparse = f->cfg.sparse_table_adam != 0;
+    uint32_t l0 = 0;
+    uint64_t e0 = 0;
+    for (uint32_t g = 0; g < G; ++g) {
+      uint32_t l1 = L;
+      if (g + 1 < G) {   // first level boundary at or past the g+1-th share of the entries
+        l1 = l0 + 1;
+        while (l1 < L - (G - 1 - g) && f->lv.offset[l1] * G < E * (g + 1)) ++l1;
+      }
+      const uint64_t e1 = l1 == L ? E : (f->lv.offset[l1] & ~uint64_t(3));
+      if (f->scatter_pending) RUN(f, K_SCATTER, launch_scatter(f->lv, f->fp.grad, f->ws, d_S, l0, l1, f->n_sms, f->stream));
+      if (g + 1 == G && use_side) {   // the last scatter is in: the side stream (next step's marcher) may overwrite the samples
+        cudaEventRecord(f->ev_main, f->stream);
+        cudaStreamWaitEvent(f->side, f->ev_main, 0);
+      }
+      if (e1 > e0)
+        RUN(f, K_ADAM_TABLE, launch_adam_table(f->fp, f->cfg.n_features, sparse, f->cfg.lr, f->cfg.beta1, f->cfg.beta2, f->cfg.eps,
+                                               (float)(1.0 / bc1), (float)(1.0 / bc2), e0, e1, f->stream, f->ws.timeline));
+      l0 = l1;
+      e0 = e1;
+    }
+    f->scatter_pending = false;
+  }
   if (use_side) {   // join: everything later on the main stream sees the new MLP weights
     cudaEventRecord(f->ev_side, f->side);
     cudaStreamWaitEvent(f->stream, f->ev_side, 0);
@@ -507,6 +544,7 @@ nsm_status nsm_create_field(const nsm_field_config *cfg, void *cuda_stream, nsm_
     return fail(e == cudaErrorMemoryAllocation ? NSM_ERR_OOM : NSM_ERR_CUDA, "allocation failed: %s", cudaGetErrorString(e));
   }
   RUN(f, K_DEBUG, launch_set_grad(f->fp, nullptr, nullptr, f->stream));   // every gradient word = "untouched"
+  if (const char *g = std::getenv("NSM_LEVEL_GROUPS")) f->n_groups = (uint32_t)std::max(1, std::atoi(g));
   repack_weights(f);
   *out = f;
   return NSM_OK;
@@ -677,7 +715,7 @@ static nsm_status train_step_impl(nsm_field *f, const nsm_ray_batch *batch, floa
                                   bool batch_ready, float *dirs_copy = nullptr) {
   nsm_status st = validate_batch(f, batch, true, false);
   if (st != NSM_OK) return st;
-  st = enqueue_backward(f, batch, lambda_d, batch_ready, dirs_copy, host_stats != nullptr);
+  st = enqueue_backward(f, batch, lambda_d, batch_ready, dirs_copy, host_stats != nullptr, false, true);
   if (st != NSM_OK) return st;
   st = enqueue_adam(f);
   if (st != NSM_OK) return st;

@@ -224,8 +224,9 @@ uint32_t march_scan_state_entries(uint32_t max_rays);
 // out_mode: 0 = fp32 planes ws.e, 1 = fp16 blob ws.blob_e, 2 = bf16 blob ws.blob_e
 int launch_encode(const LevelTable &lv, const float *theta, const Workspace &ws,
                   const uint32_t *d_S, int out_mode, int n_sms, cudaStream_t st);
+// levels [l0, l1)
 int launch_scatter(const LevelTable &lv, float *grad, const Workspace &ws,
-                   const uint32_t *d_S, int n_sms, cudaStream_t st);
+                   const uint32_t *d_S, uint32_t l0, uint32_t l1, int n_sms, cudaStream_t st);
 // gradient array <- canonical gradient + touched flags (NULL: every entry touched); src == nullptr: all untouched
 int launch_set_grad(const FieldParams &fp, const float *src, const uint8_t *touched, cudaStream_t st);
 int launch_get_touched(const FieldParams &fp, uint8_t *dst, cudaStream_t st);
@@ -256,8 +257,10 @@ int launch_composite_train(const Workspace &ws, uint32_t R, const float *rgb, co
                            cudaStream_t st);
 int launch_composite_render(const Workspace &ws, uint32_t R, float cut, const float bg[3],
                             float *out_rgb, float *out_depth, float *out_opacity, cudaStream_t st);
+// table entries [first_entry, end_entry) (a level group; first_entry a multiple of 4)
 int launch_adam_table(const FieldParams &fp, uint32_t F, int sparse, float lr, float beta1, float beta2,
-                      float eps, float inv_bc1, float inv_bc2, int n_sms, cudaStream_t st, unsigned long long *tl = nullptr);
+                      float eps, float inv_bc1, float inv_bc2, uint64_t first_entry, uint64_t end_entry, cudaStream_t st,
+                      unsigned long long *tl = nullptr);
 int launch_adam_mlp(const FieldParams &fp, float lr, float beta1, float beta2, float eps, float inv_bc1,
                     float inv_bc2, cudaStream_t st);
 // tensor-core path: Adam on the MLP weights and, in the same launch, the refreshed 16-bit weight images
