@@ -10,90 +10,11 @@
 #include <cuda_fp16.h>
 
 #include "nsm_internal.cuh"
+#include "table_ops.cuh"
 
 namespace {
 
-struct CornerIndex {
-  uint32_t slot[8];
-  float w[3];
-};
-
-// Index path of S4 (fp32 ops explicit; integers bit-exact against the oracle).
-__device__ __forceinline__ CornerIndex corner_index(const LevelTable &lv, uint32_t l, float x0,
-                                                    float x1, float x2) {
-  CornerIndex ci;
-  const uint32_t N = lv.res[l];
-  const float Nf = __uint2float_rn(N);
-  uint32_t c0[3];
-  const float x[3] = {x0, x1, x2};
-#pragma unroll
-  for (int a = 0; a < 3; ++a) {
-    float pos = __fmul_rn(x[a], Nf);
-    int c = min(__float2int_rd(pos), (int)N - 1);
-    c = max(c, 0);
-    c0[a] = (uint32_t)c;
-    ci.w[a] = __fsub_rn(pos, __int2float_rn(c));
-  }
-  if (lv.dense[l]) {
-    const uint32_t side = N + 1;
-#pragma unroll
-    for (uint32_t k = 0; k < 8; ++k)
-      ci.slot[k] = (c0[0] + (k & 1u)) + side * ((c0[1] + ((k >> 1) & 1u)) + side * (c0[2] + ((k >> 2) & 1u)));
-  } else {
-#pragma unroll
-    for (uint32_t k = 0; k < 8; ++k)
-      ci.slot[k] = ((c0[0] + (k & 1u)) ^ ((c0[1] + ((k >> 1) & 1u)) * 2654435761u) ^
-                    ((c0[2] + ((k >> 2) & 1u)) * 805459861u)) & lv.t_mask;
-  }
-  return ci;
-}
-
-__device__ __forceinline__ float corner_weight(uint32_t k, const float w[3]) {
-  float a = (k & 1u) ? w[0] : 1.0f - w[0];
-  float b = (k & 2u) ? w[1] : 1.0f - w[1];
-  float c = (k & 4u) ? w[2] : 1.0f - w[2];
-  return a * b * c;
-}
-
-template <int F> struct Vec;
-template <> struct Vec<1> { using T = float; };
-template <> struct Vec<2> { using T = float2; };
-template <> struct Vec<4> { using T = float4; };
-
-// the same through an L2 cache-policy (hashed levels: stream, evict first)
-template <int F>
-__device__ __forceinline__ void load_entry_hint(const float *p, float out[F], uint64_t pol) {
-  if constexpr (F == 8) {
-    float4 a = ld_hint_f4(p, pol), b = ld_hint_f4(p + 4, pol);
-    out[0] = a.x; out[1] = a.y; out[2] = a.z; out[3] = a.w;
-    out[4] = b.x; out[5] = b.y; out[6] = b.z; out[7] = b.w;
-  } else if constexpr (F == 4) {
-    float4 a = ld_hint_f4(p, pol);
-    out[0] = a.x; out[1] = a.y; out[2] = a.z; out[3] = a.w;
-  } else if constexpr (F == 2) {
-    float2 a = ld_hint_f2(p, pol);
-    out[0] = a.x; out[1] = a.y;
-  } else {
-    out[0] = ld_hint_f1(p, pol);
-  }
-}
-
-template <int F>
-__device__ __forceinline__ void load_entry(const float *p, float out[F]) {
-  if constexpr (F == 8) {
-    float4 a = __ldg(reinterpret_cast<const float4 *>(p)), b = __ldg(reinterpret_cast<const float4 *>(p) + 1);
-    out[0] = a.x; out[1] = a.y; out[2] = a.z; out[3] = a.w;
-    out[4] = b.x; out[5] = b.y; out[6] = b.z; out[7] = b.w;
-  } else if constexpr (F == 4) {
-    float4 a = __ldg(reinterpret_cast<const float4 *>(p));
-    out[0] = a.x; out[1] = a.y; out[2] = a.z; out[3] = a.w;
-  } else if constexpr (F == 2) {
-    float2 a = __ldg(reinterpret_cast<const float2 *>(p));
-    out[0] = a.x; out[1] = a.y;
-  } else {
-    out[0] = __ldg(p);
-  }
-}
+using namespace tableops;
 
 // MODE 0: e -> fp32 planes [l*F+f][cap].  MODE 1 / 2: e -> fp16 / bf16 operand-tile blob of the
 // tensor-core MLP kernels ([tile][8-column panel][128 rows][8 x 16 bit], mlp_tc.cu); the rows of
@@ -160,24 +81,7 @@ __global__ void __launch_bounds__(256) encode_forward_kernel(LevelTable lv, cons
   tl_mark(ws.timeline, K_ENCODE, 1);
 }
 
-template <int F>
-__device__ __forceinline__ void red_add_entry(float *p, const float g[F], uint64_t pol) {
-  // vectorised no-return reductions (red.global.add.v2/v4.f32, sm_90+); the gradient array stays in L2
-  if constexpr (F == 8) {
-    red_hint_f4(p, make_float4(g[0], g[1], g[2], g[3]), pol);
-    red_hint_f4(p + 4, make_float4(g[4], g[5], g[6], g[7]), pol);
-  } else if constexpr (F == 4) {
-    red_hint_f4(p, make_float4(g[0], g[1], g[2], g[3]), pol);
-  } else if constexpr (F == 2) {
-    red_hint_f2(p, make_float2(g[0], g[1]), pol);
-  } else {
-    red_hint_f1(p, g[0], pol);
-  }
-}
-
-// S12: d theta[(offset_l + slot) F + f] += omega * dL/de[l F + f].  The touched set U is structural
-// (every referenced entry, independent of the gradient's value): it is carried by the gradient words
-// themselves, see FieldParams in nsm_internal.cuh.
+// S12, thread per (level, sample), level-major (see scatter_sample_level in table_ops.cuh).
 template <int F>
 __global__ void __launch_bounds__(256) scatter_backward_kernel(LevelTable lv, float *__restrict__ grad, Workspace ws,
                                                                const uint32_t *__restrict__ d_S, uint32_t l0, uint32_t l1) {
@@ -191,22 +95,7 @@ __global__ void __launch_bounds__(256) scatter_backward_kernel(LevelTable lv, fl
        wi += (uint64_t)gridDim.x * blockDim.x) {
     const uint32_t l = l0 + (uint32_t)(wi / S);
     const uint64_t s = wi - (uint64_t)(l - l0) * S;
-    CornerIndex ci = corner_index(lv, l, ws.s_x[s], ws.s_x[ws.cap + s], ws.s_x[2 * ws.cap + s]);
-    float de[F];
-#pragma unroll
-    for (int f = 0; f < F; ++f) de[f] = ws.de[(size_t)(l * F + f) * ws.cap + s];
-    float *tab = grad + lv.offset[l] * F;
-#pragma unroll
-    for (int k = 0; k < 8; ++k) {
-      float om = corner_weight(k, ci.w);
-      float g[F];
-#pragma unroll
-      for (int f = 0; f < F; ++f) {
-        const float v = om * de[f];
-        g[f] = fabsf(v) < NSM_GRAD_MIN_ADDEND ? 0.0f : v;   // never -0.0, never near-subnormal; NaN stays NaN
-      }
-      red_add_entry<F>(tab + (size_t)ci.slot[k] * F, g, pol_last);
-    }
+    scatter_sample_level<F>(lv, grad, ws, l, s, pol_last);
   }
   tl_mark(ws.timeline, K_SCATTER, 1);
 }

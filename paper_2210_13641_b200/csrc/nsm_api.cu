@@ -355,7 +355,7 @@ nsm_status enqueue_adam(nsm_field *f) {
     const uint64_t E = f->fp.n_entries;
     const uint32_t G = f->scatter_pending ? (f->n_groups < L ? f->n_groups : L) : 1;
     const uint32_t *d_S = f->ws.offsets + f->last_R;
-    const int sparse = f->cfg.sparse_table_adam != 0;
+    const int sparse = (f->cfg.sparse_table_adam != 0);
     uint32_t l0 = 0;
     uint64_t e0 = 0;
     for (uint32_t g = 0; g < G; ++g) {

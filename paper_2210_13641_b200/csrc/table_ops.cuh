@@ -1,0 +1,256 @@
+// table_ops.cuh — device code shared by the table kernels: the index path of S4 (corner slots and weights), the
+// eight-corner gather / vector reduction of one (sample, level), and the touched-only Adam update of one chunk of
+// entries.  Used by encode.cu (S4, S12) and adam.cu (S13).
+#pragma once
+#include "nsm_internal.cuh"
+
+namespace tableops {
+
+struct CornerIndex {
+  uint32_t slot[8];
+  float w[3];
+};
+
+// Index path of S4 (fp32 ops explicit; integers bit-exact against the oracle).
+__device__ __forceinline__ CornerIndex corner_index(const LevelTable &lv, uint32_t l, float x0,
+                                                    float x1, float x2) {
+  CornerIndex ci;
+  const uint32_t N = lv.res[l];
+  const float Nf = __uint2float_rn(N);
+  uint32_t c0[3];
+  const float x[3] = {x0, x1, x2};
+#pragma unroll
+  for (int a = 0; a < 3; ++a) {
+    float pos = __fmul_rn(x[a], Nf);
+    int c = min(__float2int_rd(pos), (int)N - 1);
+    c = max(c, 0);
+    c0[a] = (uint32_t)c;
+    ci.w[a] = __fsub_rn(pos, __int2float_rn(c));
+  }
+  if (lv.dense[l]) {
+    const uint32_t side = N + 1;
+#pragma unroll
+    for (uint32_t k = 0; k < 8; ++k)
+      ci.slot[k] = (c0[0] + (k & 1u)) + side * ((c0[1] + ((k >> 1) & 1u)) + side * (c0[2] + ((k >> 2) & 1u)));
+  } else {
+#pragma unroll
+    for (uint32_t k = 0; k < 8; ++k)
+      ci.slot[k] = ((c0[0] + (k & 1u)) ^ ((c0[1] + ((k >> 1) & 1u)) * 2654435761u) ^
+                    ((c0[2] + ((k >> 2) & 1u)) * 805459861u)) & lv.t_mask;
+  }
+  return ci;
+}
+
+__device__ __forceinline__ float corner_weight(uint32_t k, const float w[3]) {
+  float a = (k & 1u) ? w[0] : 1.0f - w[0];
+  float b = (k & 2u) ? w[1] : 1.0f - w[1];
+  float c = (k & 4u) ? w[2] : 1.0f - w[2];
+  return a * b * c;
+}
+
+template <int F> struct Vec;
+template <> struct Vec<1> { using T = float; };
+template <> struct Vec<2> { using T = float2; };
+template <> struct Vec<4> { using T = float4; };
+
+// the same through an L2 cache-policy (hashed levels: stream, evict first)
+template <int F>
+__device__ __forceinline__ void load_entry_hint(const float *p, float out[F], uint64_t pol) {
+  if constexpr (F == 8) {
+    float4 a = ld_hint_f4(p, pol), b = ld_hint_f4(p + 4, pol);
+    out[0] = a.x; out[1] = a.y; out[2] = a.z; out[3] = a.w;
+    out[4] = b.x; out[5] = b.y; out[6] = b.z; out[7] = b.w;
+  } else if constexpr (F == 4) {
+    float4 a = ld_hint_f4(p, pol);
+    out[0] = a.x; out[1] = a.y; out[2] = a.z; out[3] = a.w;
+  } else if constexpr (F == 2) {
+    float2 a = ld_hint_f2(p, pol);
+    out[0] = a.x; out[1] = a.y;
+  } else {
+    out[0] = ld_hint_f1(p, pol);
+  }
+}
+
+template <int F>
+__device__ __forceinline__ void load_entry(const float *p, float out[F]) {
+  if constexpr (F == 8) {
+    float4 a = __ldg(reinterpret_cast<const float4 *>(p)), b = __ldg(reinterpret_cast<const float4 *>(p) + 1);
+    out[0] = a.x; out[1] = a.y; out[2] = a.z; out[3] = a.w;
+    out[4] = b.x; out[5] = b.y; out[6] = b.z; out[7] = b.w;
+  } else if constexpr (F == 4) {
+    float4 a = __ldg(reinterpret_cast<const float4 *>(p));
+    out[0] = a.x; out[1] = a.y; out[2] = a.z; out[3] = a.w;
+  } else if constexpr (F == 2) {
+    float2 a = __ldg(reinterpret_cast<const float2 *>(p));
+    out[0] = a.x; out[1] = a.y;
+  } else {
+    out[0] = __ldg(p);
+  }
+}
+
+template <int F>
+__device__ __forceinline__ void red_add_entry(float *p, const float g[F], uint64_t pol) {
+  // vectorised no-return reductions (red.global.add.v2/v4.f32, sm_90+); the gradient array stays in L2
+  if constexpr (F == 8) {
+    red_hint_f4(p, make_float4(g[0], g[1], g[2], g[3]), pol);
+    red_hint_f4(p + 4, make_float4(g[4], g[5], g[6], g[7]), pol);
+  } else if constexpr (F == 4) {
+    red_hint_f4(p, make_float4(g[0], g[1], g[2], g[3]), pol);
+  } else if constexpr (F == 2) {
+    red_hint_f2(p, make_float2(g[0], g[1]), pol);
+  } else {
+    red_hint_f1(p, g[0], pol);
+  }
+}
+
+// S12 for one (sample, level): d theta[(offset_l + slot) F + f] += omega * dL/de[l F + f], eight vector reductions.
+// The touched set U is structural (every referenced entry, independent of the gradient's value): it is carried by
+// the gradient words themselves, see FieldParams in nsm_internal.cuh.
+template <int F>
+__device__ __forceinline__ void scatter_sample_level(const LevelTable &lv, float *__restrict__ grad, const Workspace &ws,
+                                                     uint32_t l, uint64_t s, uint64_t pol_last) {
+  CornerIndex ci = corner_index(lv, l, ws.s_x[s], ws.s_x[ws.cap + s], ws.s_x[2 * ws.cap + s]);
+  float de[F];
+#pragma unroll
+  for (int f = 0; f < F; ++f) de[f] = ws.de[(size_t)(l * F + f) * ws.cap + s];
+  float *tab = grad + lv.offset[l] * F;
+#pragma unroll
+  for (int k = 0; k < 8; ++k) {
+    float om = corner_weight(k, ci.w);
+    float g[F];
+#pragma unroll
+    for (int f = 0; f < F; ++f) {
+      const float v = om * de[f];
+      g[f] = fabsf(v) < NSM_GRAD_MIN_ADDEND ? 0.0f : v;   // never -0.0, never near-subnormal; NaN stays NaN
+    }
+    red_add_entry<F>(tab + (size_t)ci.slot[k] * F, g, pol_last);
+  }
+}
+
+constexpr int ADAM_CHUNK_FLOATS = 4096;
+constexpr int ADAM_THREADS = 256;
+
+// one touched entry: theta (F floats of the compact array) and its moment record (m | v, 2F floats)
+template <int F>
+__device__ __forceinline__ void adam_entry(float *__restrict__ th_p, float *__restrict__ mv_p, const float *g, const AdamConst &c,
+                                           uint64_t pol_ld, uint64_t pol_st) {
+  float th[F], m[F], v[F];
+  if constexpr (F == 1) {
+    th[0] = ld_hint_f1(th_p, pol_ld);
+    const float2 t = ld_hint_f2(mv_p, pol_ld);
+    m[0] = t.x; v[0] = t.y;
+  } else if constexpr (F == 2) {
+    const float2 a = ld_hint_f2(th_p, pol_ld);
+    const float4 b = ld_hint_f4(mv_p, pol_ld);
+    th[0] = a.x; th[1] = a.y; m[0] = b.x; m[1] = b.y; v[0] = b.z; v[1] = b.w;
+  } else {
+#pragma unroll
+    for (int i = 0; i < F / 4; ++i) {
+      const float4 a = ld_hint_f4(th_p + 4 * i, pol_ld), b = ld_hint_f4(mv_p + 4 * i, pol_ld), d = ld_hint_f4(mv_p + F + 4 * i, pol_ld);
+      th[4 * i] = a.x; th[4 * i + 1] = a.y; th[4 * i + 2] = a.z; th[4 * i + 3] = a.w;
+      m[4 * i] = b.x; m[4 * i + 1] = b.y; m[4 * i + 2] = b.z; m[4 * i + 3] = b.w;
+      v[4 * i] = d.x; v[4 * i + 1] = d.y; v[4 * i + 2] = d.z; v[4 * i + 3] = d.w;
+    }
+  }
+#pragma unroll
+  for (int f = 0; f < F; ++f) adam_one(th[f], m[f], v[f], g[f], c);
+  if constexpr (F == 1) {
+    st_hint_f1(th_p, th[0], pol_st);
+    st_hint_f2(mv_p, make_float2(m[0], v[0]), pol_st);
+  } else if constexpr (F == 2) {
+    st_hint_f2(th_p, make_float2(th[0], th[1]), pol_st);
+    st_hint_f4(mv_p, make_float4(m[0], m[1], v[0], v[1]), pol_st);
+  } else {
+#pragma unroll
+    for (int i = 0; i < F / 4; ++i) {
+      st_hint_f4(th_p + 4 * i, make_float4(th[4 * i], th[4 * i + 1], th[4 * i + 2], th[4 * i + 3]), pol_st);
+      st_hint_f4(mv_p + 4 * i, make_float4(m[4 * i], m[4 * i + 1], m[4 * i + 2], m[4 * i + 3]), pol_st);
+      st_hint_f4(mv_p + F + 4 * i, make_float4(v[4 * i], v[4 * i + 1], v[4 * i + 2], v[4 * i + 3]), pol_st);
+    }
+  }
+}
+
+// S13 for one chunk of ADAM_CHUNK_FLOATS / F consecutive entries starting at e_base (e_base * F a multiple of 4),
+// by a whole block of ADAM_THREADS threads.  Shared memory: list_g [ADAM_CHUNK_FLOATS], list_e [CH], cnt_p.  The caller
+// must __syncthreads() before reusing the shared arrays.
+template <int F>
+__device__ __forceinline__ void adam_chunk(float *__restrict__ theta, float *__restrict__ mv, float *__restrict__ grad,
+                                           uint64_t e_base, uint64_t n_entries, int sparse, const AdamConst &c, float *list_g,
+                                           uint16_t *list_e, uint32_t *cnt_p) {
+  constexpr int CH = ADAM_CHUNK_FLOATS / F;            // entries per chunk
+  constexpr int NV = ADAM_CHUNK_FLOATS / 4 / ADAM_THREADS;   // float4 loads per thread
+  const uint32_t tid = threadIdx.x, lane = tid & 31;
+  const uint64_t n_float = n_entries * F;
+  const float *g4 = grad + e_base * F;
+  // L2 policies, swept on B200 (profiles/r1k): theta / moment stores evict_first, everything else default.  Marking
+  // Adam's own gradient reads and resets evict_last (as the scatter's reductions are) costs 4 us per step.
+  const uint64_t pol_ld = l2_evict_normal(), pol_first = l2_evict_first(), pol_last = pol_ld;
+  if (tid == 0) *cnt_p = 0;
+  float4 gv[NV];
+#pragma unroll
+  for (int j = 0; j < NV; ++j) {
+    const uint32_t q = j * ADAM_THREADS + tid;         // float4 index inside the chunk
+    gv[j] = (e_base * F + 4ull * q < n_float) ? ld_hint_f4(g4 + 4 * q, pol_last) : make_float4(0.f, 0.f, 0.f, 0.f);   // the array is padded to 256 B
+  }
+  __syncthreads();
+#pragma unroll
+  for (int j = 0; j < NV; ++j) {
+    const uint32_t q = j * ADAM_THREADS + tid;
+    const float w[4] = {gv[j].x, gv[j].y, gv[j].z, gv[j].w};
+    if constexpr (F <= 4) {
+      constexpr int EPV = 4 / F;                       // entries per float4
+#pragma unroll
+      for (int i = 0; i < EPV; ++i) {
+        const uint32_t le = q * EPV + i;               // local entry index
+        const bool t = (e_base + le < n_entries) && (!sparse || __float_as_uint(w[i * F]) != NSM_GRAD_UNTOUCHED);
+        const uint32_t mk = __ballot_sync(0xffffffffu, t);
+        uint32_t base = 0;
+        if (lane == 0 && mk) base = atomicAdd(cnt_p, (uint32_t)__popc(mk));
+        base = __shfl_sync(0xffffffffu, base, 0);
+        if (t) {
+          const uint32_t pos = base + __popc(mk & ((1u << lane) - 1u));
+          list_e[pos] = (uint16_t)le;
+#pragma unroll
+          for (int f = 0; f < F; ++f) list_g[pos * F + f] = w[i * F + f];
+        }
+      }
+    } else {                                           // F = 8: an entry spans two float4 (q even: first half)
+      const uint32_t le = q >> 1;
+      const uint32_t first_word = __float_as_uint(__shfl_sync(0xffffffffu, w[0], lane & ~1u));
+      const bool t = (e_base + le < n_entries) && (!sparse || first_word != NSM_GRAD_UNTOUCHED);
+      const uint32_t mk = __ballot_sync(0xffffffffu, t && !(lane & 1u));
+      uint32_t base = 0;
+      if (lane == 0 && mk) base = atomicAdd(cnt_p, (uint32_t)__popc(mk));
+      base = __shfl_sync(0xffffffffu, base, 0);
+      if (t) {
+        const uint32_t pos = base + __popc(mk & ((1u << (lane & ~1u)) - 1u));
+        if (!(lane & 1u)) list_e[pos] = (uint16_t)le;
+#pragma unroll
+        for (int f = 0; f < 4; ++f) list_g[pos * F + (lane & 1u) * 4 + f] = w[f];
+      }
+    }
+  }
+  __syncthreads();
+  const uint32_t n = *cnt_p;
+  if (n == 0) return;
+  // phase 2: two records in flight per thread
+  for (uint32_t i0 = tid; i0 < n; i0 += 2 * ADAM_THREADS) {
+    const uint32_t i1 = i0 + ADAM_THREADS;
+    const uint64_t e0 = e_base + list_e[i0], e1 = e_base + list_e[i1 < n ? i1 : i0];
+    if constexpr (F == 2) {   // touch the second entry's moment record early
+      asm volatile("prefetch.global.L2 [%0];" ::"l"(mv + e1 * 2 * F));
+    }
+    adam_entry<F>(theta + e0 * F, mv + e0 * 2 * F, list_g + i0 * F, c, pol_ld, pol_first);
+    if (i1 < n) adam_entry<F>(theta + e1 * F, mv + e1 * 2 * F, list_g + i1 * F, c, pol_ld, pol_first);
+  }
+  // reset the chunk's gradient words
+  float *o4 = grad + e_base * F;
+  const float nz = __uint_as_float(NSM_GRAD_UNTOUCHED);
+#pragma unroll
+  for (int j = 0; j < NV; ++j) {
+    const uint32_t q = j * ADAM_THREADS + tid;
+    if (e_base * F + 4ull * q < n_float) st_hint_f4(o4 + 4 * q, make_float4(nz, nz, nz, nz), pol_last);
+  }
+}
+
+}  // namespace tableops
