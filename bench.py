@@ -117,7 +117,7 @@ def workload_config(w, extra=None, cfg=2):
              rays_per_step=w.batches[0].n_rays, candidates_per_ray=w.batches[0].n_candidates,
              occupancy_fraction=round(w.extra["occupancy_fraction"], 4) if "occupancy_fraction" in w.extra else None,
              lambda_d=w.lambda_d, table_params=None, mlp_precision=["fp32", "fp16", "bf16"][fc.mlp_precision],
-             l2="not flushed: the table records (theta, gradient, Adam m and v: 16 B per parameter, 195 MB at config 2) plus the "
+             l2="not flushed: the tables (theta, gradient, Adam m and v: 16 B per parameter, 195 MB at config 2) plus the "
                 "per-sample workspace exceed the 126 MB L2, and every step gets a fresh ray batch",
              batches=f"{len(w.batches)} distinct pre-generated batches, cycled")
     if extra:
@@ -197,6 +197,13 @@ def kernel_model(name, S, R, K, L, F, LF, U, E, mac, n_mlp):
     if name == "march":
         return dict(bound="alu", flops=40 * R * K)
     return dict(bound="hbm", bytes=0)
+
+
+# DRAM bytes (dram__bytes_read.sum + dram__bytes_write.sum) per launch from the `ncu --set full` capture of
+# profiles/r1l_ncu_full.md (config 2; cold cache, as ncu flushes before every kernel).  bench.py cannot run ncu:
+# these are recorded values, refreshed with each committed profile.
+NCU_TRAFFIC_CFG2 = {"adam_table": 157317888 + 65678848, "scatter": 37862400, "encode": 40513792 + 65792,
+                    "mlp_bwd": 11984384 + 256, "mlp_fwd": 3022848, "adam_mlp": 6556160, "composite": 643584, "march": 382208}
 
 
 def run_render(args, nsm, replicas, dev, rank, world, peaks):
@@ -384,7 +391,9 @@ def run_cuda(args):
         kernels.sort(key=lambda k: -k["share"])
         top = kernels[0]
         roofline = dict(kernel=top["kernel"], bound=top["bound"], achieved=top["achieved"], peak=top["peak"], unit=top["unit"],
-                        frac=top["frac"], traffic=None, share_of_step=top["share"], avg_us=top["avg_us"],
+                        frac=top["frac"], traffic=NCU_TRAFFIC_CFG2.get(top["kernel"]) if cfg == 2 else None,
+                        traffic_source="profiles/r1l_ncu_full.md (ncu --set full, per launch, cold cache)" if cfg == 2 else None,
+                        share_of_step=top["share"], avg_us=top["avg_us"],
                         peak_source=peaks["source"] if top["bound"] != "alu" else "derived: 148 SM x 128 FMA/clk x 2 x 1.965 GHz",
                         samples_per_launch=S_avg, touched_entries=U)
         # ---- CPU baseline: the oracle on the host cores, bounded sample
