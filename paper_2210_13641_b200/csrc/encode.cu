@@ -29,7 +29,7 @@ __global__ void __launch_bounds__(256) encode_forward_kernel(LevelTable lv, cons
   const uint64_t S_it = MODE == 0 ? S : ((S + NSM_TILE - 1) / NSM_TILE) * NSM_TILE;
   const uint64_t total = S_it * lv.n_levels;
   const uint32_t LF = lv.n_levels * F;
-  const uint64_t pol_first = l2_evict_first();
+  const uint64_t pol_first = l2_evict_first(), pol_normal = l2_evict_normal();
   for (uint64_t wi = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; wi < total;
        wi += (uint64_t)gridDim.x * blockDim.x) {
     const uint32_t l = (uint32_t)(wi / S_it);
@@ -41,13 +41,27 @@ __global__ void __launch_bounds__(256) encode_forward_kernel(LevelTable lv, cons
       CornerIndex ci = corner_index(lv, l, ws.s_x[s], ws.s_x[ws.cap + s], ws.s_x[2 * ws.cap + s]);
       const float *tab = theta + lv.offset[l] * F;
       float v[8][F];
+      // coarse (dense) levels are re-read every step: default policy; hashed levels stream through L2
+      const uint64_t pol = lv.dense[l] ? pol_normal : pol_first;
+      if constexpr (F == 2) {
+        // x-neighbour corners that form an aligned pair of entries come in with one 16-byte load (see scatter_sample_level)
+        const uint64_t e_l = lv.offset[l];
 #pragma unroll
-      if (lv.dense[l]) {   // coarse levels are re-read every step: normal policy; hashed levels stream through L2
-#pragma unroll
-        for (int k = 0; k < 8; ++k) load_entry<F>(tab + (size_t)ci.slot[k] * F, v[k]);  // 8 gathers in flight
+        for (int k = 0; k < 8; k += 2) {
+          const uint64_t a0 = e_l + ci.slot[k], a1 = e_l + ci.slot[k + 1];
+          if ((a0 ^ a1) == 1ull) {
+            const float4 q = ld_hint_f4(theta + (a0 & ~1ull) * 2, pol);
+            const bool odd = a0 & 1ull;
+            v[k][0] = odd ? q.z : q.x; v[k][1] = odd ? q.w : q.y;
+            v[k + 1][0] = odd ? q.x : q.z; v[k + 1][1] = odd ? q.y : q.w;
+          } else {
+            load_entry_hint<2>(tab + (size_t)ci.slot[k] * 2, v[k], pol);
+            load_entry_hint<2>(tab + (size_t)ci.slot[k + 1] * 2, v[k + 1], pol);
+          }
+        }
       } else {
 #pragma unroll
-        for (int k = 0; k < 8; ++k) load_entry_hint<F>(tab + (size_t)ci.slot[k] * F, v[k], pol_first);
+        for (int k = 0; k < 8; ++k) load_entry_hint<F>(tab + (size_t)ci.slot[k] * F, v[k], pol);  // 8 gathers in flight
       }
 #pragma unroll
       for (int k = 0; k < 8; ++k) {

@@ -114,16 +114,43 @@ __device__ __forceinline__ void scatter_sample_level(const LevelTable &lv, float
 #pragma unroll
   for (int f = 0; f < F; ++f) de[f] = ws.de[(size_t)(l * F + f) * ws.cap + s];
   float *tab = grad + lv.offset[l] * F;
+  if constexpr (F == 2) {
+    // The two x-neighbour corners (k, k+1) are adjacent entries whenever their slots differ in bit 0 only (always on
+    // a dense level, for even cell x on a hashed one: the hash XORs x in unmultiplied).  If the pair is also
+    // 16-byte aligned in the array, one red.v4 covers both entries: ~25 % fewer reductions at the L2.
+    const uint64_t e_l = lv.offset[l];
 #pragma unroll
-  for (int k = 0; k < 8; ++k) {
-    float om = corner_weight(k, ci.w);
-    float g[F];
+    for (int k = 0; k < 8; k += 2) {
+      float g0[2], g1[2];
+      const float om0 = corner_weight(k, ci.w), om1 = corner_weight(k + 1, ci.w);
 #pragma unroll
-    for (int f = 0; f < F; ++f) {
-      const float v = om * de[f];
-      g[f] = fabsf(v) < NSM_GRAD_MIN_ADDEND ? 0.0f : v;   // never -0.0, never near-subnormal; NaN stays NaN
+      for (int f = 0; f < 2; ++f) {
+        const float v0 = om0 * de[f], v1 = om1 * de[f];
+        g0[f] = fabsf(v0) < NSM_GRAD_MIN_ADDEND ? 0.0f : v0;   // never -0.0, never near-subnormal; NaN stays NaN
+        g1[f] = fabsf(v1) < NSM_GRAD_MIN_ADDEND ? 0.0f : v1;
+      }
+      const uint64_t a0 = e_l + ci.slot[k], a1 = e_l + ci.slot[k + 1];
+      if ((a0 ^ a1) == 1ull) {
+        float *p = grad + (a0 & ~1ull) * 2;
+        if (a0 & 1ull) red_hint_f4(p, make_float4(g1[0], g1[1], g0[0], g0[1]), pol_last);
+        else red_hint_f4(p, make_float4(g0[0], g0[1], g1[0], g1[1]), pol_last);
+      } else {
+        red_add_entry<2>(tab + (size_t)ci.slot[k] * 2, g0, pol_last);
+        red_add_entry<2>(tab + (size_t)ci.slot[k + 1] * 2, g1, pol_last);
+      }
     }
-    red_add_entry<F>(tab + (size_t)ci.slot[k] * F, g, pol_last);
+  } else {
+#pragma unroll
+    for (int k = 0; k < 8; ++k) {
+      float om = corner_weight(k, ci.w);
+      float g[F];
+#pragma unroll
+      for (int f = 0; f < F; ++f) {
+        const float v = om * de[f];
+        g[f] = fabsf(v) < NSM_GRAD_MIN_ADDEND ? 0.0f : v;   // never -0.0, never near-subnormal; NaN stays NaN
+      }
+      red_add_entry<F>(tab + (size_t)ci.slot[k] * F, g, pol_last);
+    }
   }
 }
 
