@@ -108,6 +108,7 @@ struct nsm_field {
   // behind it, and a call that wants them waits for that copy only, not for the backward pass and Adam
   cudaEvent_t ev_comp = nullptr, ev_stats = nullptr;
   bool stats_pending = false;
+  bool join_pending = false;   // ev_side (recorded behind the MLP Adam) has not been waited for on the main stream yet
   unsigned long long *timeline_base = nullptr;   // NSM_TIMELINE=1: ring of 64 steps x [2][K_COUNT] globaltimer stamps
   bool scatter_pending = false;   // the backward pass stopped before S12: enqueue_adam interleaves scatter and Adam per level group
   uint32_t n_groups = 1;          // level groups of the scatter + Adam phase (NSM_LEVEL_GROUPS)
@@ -219,6 +220,19 @@ nsm_status validate_batch(const nsm_field *f, const nsm_ray_batch *b, bool train
     }                                                                       \
   } while (0)
 
+// The side stream's last work (the MLP Adam of the previous step) is joined into the main stream lazily: a training
+// step that marches on the side stream joins behind its marcher anyway, every other entry point joins here.
+void join_side(nsm_field *f) {
+  if (f->join_pending) {
+    cudaStreamWaitEvent(f->stream, f->ev_side, 0);
+    f->join_pending = false;
+  }
+}
+void leave_fast_path(nsm_field *f) {
+  join_side(f);
+  f->side_ok = false;
+}
+
 MarchParams make_march(const nsm_field *f, const nsm_ray_batch *b, uint32_t R, bool jitter, uint32_t step) {
   MarchParams mp;
   for (int a = 0; a < 3; ++a) mp.aabb_min[a] = f->cfg.aabb_min[a];
@@ -251,7 +265,9 @@ void enqueue_forward(nsm_field *f, const nsm_ray_batch *b, uint32_t R, bool jitt
     RUN_ON(f, K_MARCH, f->side, launch_march(mp, f->occ_full ? nullptr : f->fp.occ_bits, b->origins, b->dirs, f->ws, train ? 1 : 0, f->side, dirs_copy));
     cudaEventRecord(f->ev_side, f->side);
     cudaStreamWaitEvent(f->stream, f->ev_side, 0);
+    f->join_pending = false;   // behind the marcher is behind the previous step's MLP Adam too
   } else {
+    join_side(f);
     RUN(f, K_MARCH, launch_march(mp, f->occ_full ? nullptr : f->fp.occ_bits, b->origins, b->dirs, f->ws, train ? 1 : 0, f->stream, dirs_copy));
   }
   const int bf16 = f->cfg.mlp_precision == NSM_MLP_BF16;
@@ -378,9 +394,9 @@ nsm_status enqueue_adam(nsm_field *f) {
     }
     f->scatter_pending = false;
   }
-  if (use_side) {   // join: everything later on the main stream sees the new MLP weights
+  if (use_side) {   // to be joined (lazily, join_side): everything later on the main stream must see the new MLP weights
     cudaEventRecord(f->ev_side, f->side);
-    cudaStreamWaitEvent(f->stream, f->ev_side, 0);
+    f->join_pending = true;
     f->side_ok = true;
   }
   f->step = t;
@@ -568,6 +584,7 @@ void nsm_destroy_field(nsm_field *f) {
 nsm_status nsm_total_samples(nsm_field *f, uint64_t *out) {
   if (!f || !out) return fail(NSM_ERR_INVALID_ARG, "NULL argument");
   unsigned long long v = 0;
+  leave_fast_path(f);   // the marcher (side stream) maintains the count
   CUDA_TRY(cudaMemcpyAsync(&v, f->ws.total_samples, sizeof v, cudaMemcpyDeviceToHost, f->stream));
   CUDA_TRY(cudaStreamSynchronize(f->stream));
   *out = v;
@@ -576,6 +593,7 @@ nsm_status nsm_total_samples(nsm_field *f, uint64_t *out) {
 
 nsm_status nsm_profile(nsm_field *f, int enable) {
   if (!f) return fail(NSM_ERR_INVALID_ARG, "field is NULL");
+  leave_fast_path(f);
   CUDA_TRY(cudaStreamSynchronize(f->stream));
   f->prof.collect();
   f->prof.on = enable != 0;
@@ -615,7 +633,7 @@ nsm_status nsm_get_level_table(const nsm_field *f, uint32_t *res, uint64_t *offs
 
 nsm_status nsm_get_params(nsm_field *f, float *d_theta, float *d_m, float *d_v, uint32_t *step) {
   if (!f) return fail(NSM_ERR_INVALID_ARG, "field is NULL");
-  f->side_ok = false;
+  leave_fast_path(f);
   const size_t mb = sizeof(float) * f->fp.n_mlp;
   float *dst[3] = {d_theta, d_m, d_v};
   const float *mlp[3] = {f->fp.mlp_theta, f->fp.mlp_m, f->fp.mlp_v};
@@ -632,7 +650,7 @@ nsm_status nsm_get_params(nsm_field *f, float *d_theta, float *d_m, float *d_v, 
 
 nsm_status nsm_set_params(nsm_field *f, const float *d_theta, const float *d_m, const float *d_v, uint32_t step) {
   if (!f) return fail(NSM_ERR_INVALID_ARG, "field is NULL");
-  f->side_ok = false;
+  leave_fast_path(f);
   const size_t mb = sizeof(float) * f->fp.n_mlp;
   const float *src[3] = {d_theta, d_m, d_v};
   float *mlp[3] = {f->fp.mlp_theta, f->fp.mlp_m, f->fp.mlp_v};
@@ -650,7 +668,7 @@ nsm_status nsm_set_params(nsm_field *f, const float *d_theta, const float *d_m, 
 
 nsm_status nsm_get_occupancy(nsm_field *f, uint8_t *d_bits) {
   if (!f || !d_bits) return fail(NSM_ERR_INVALID_ARG, "NULL argument");
-  f->side_ok = false;
+  leave_fast_path(f);
   const uint64_t G3 = (uint64_t)f->cfg.occ_res * f->cfg.occ_res * f->cfg.occ_res;
   if (f->occ_full) CUDA_TRY(cudaMemsetAsync(d_bits, 0xff, (G3 + 7) / 8, f->stream));
   else CUDA_TRY(cudaMemcpyAsync(d_bits, f->fp.occ_bits, (G3 + 7) / 8, cudaMemcpyDeviceToDevice, f->stream));
@@ -659,7 +677,7 @@ nsm_status nsm_get_occupancy(nsm_field *f, uint8_t *d_bits) {
 
 nsm_status nsm_update_occupancy(nsm_field *f, nsm_occ_mode mode, const uint8_t *d_bits) {
   if (!f) return fail(NSM_ERR_INVALID_ARG, "field is NULL");
-  f->side_ok = false;
+  leave_fast_path(f);
   const uint64_t G3 = (uint64_t)f->cfg.occ_res * f->cfg.occ_res * f->cfg.occ_res;
   switch (mode) {
     case NSM_OCC_FULL:
@@ -698,7 +716,7 @@ nsm_status nsm_update_occupancy(nsm_field *f, nsm_occ_mode mode, const uint8_t *
 nsm_status nsm_backward(nsm_field *f, const nsm_ray_batch *batch, float lambda_d, nsm_step_stats *host_stats) {
   nsm_status st = validate_batch(f, batch, true, false);
   if (st != NSM_OK) return st;
-  f->side_ok = false;
+  leave_fast_path(f);
   st = enqueue_backward(f, batch, lambda_d, false, nullptr, host_stats != nullptr, true);
   if (st != NSM_OK) return st;
   st = read_stats(f, batch->n_rays, host_stats);
@@ -708,6 +726,7 @@ nsm_status nsm_backward(nsm_field *f, const nsm_ray_batch *batch, float lambda_d
 
 nsm_status nsm_apply_adam(nsm_field *f) {
   if (!f) return fail(NSM_ERR_INVALID_ARG, "field is NULL");
+  leave_fast_path(f);
   return enqueue_adam(f);
 }
 
@@ -747,7 +766,7 @@ nsm_status nsm_train_step_host(nsm_field *f, const nsm_ray_batch *hb, float lamb
   db.depth = host_mapped(hb->depth); db.depth_var = host_mapped(hb->depth_var);
   if (db.origins && db.dirs && db.rgb && db.depth && db.depth_var)   // the call syncs: the host buffers are free on return
     return train_step_impl(f, &db, lambda_d, host_stats ? host_stats : &local, true, f->stage_dev + 3 * (size_t)f->cfg.max_rays);
-  f->side_ok = false;   // pageable memory: staging copies through the main stream
+  leave_fast_path(f);   // pageable memory: staging copies through the main stream
   st = stage_batch(f, hb, 0, hb->n_rays, true, &db);
   if (st != NSM_OK) return st;
   return train_step_impl(f, &db, lambda_d, host_stats ? host_stats : &local, false);  // always syncs: host buffers may be reused
@@ -766,14 +785,14 @@ nsm_status nsm_debug_timeline(nsm_field *f, uint64_t *h_out, uint64_t capacity_w
 nsm_status nsm_set_option(nsm_field *f, nsm_option opt, uint32_t value) {
   if (!f) return fail(NSM_ERR_INVALID_ARG, "field is NULL");
   switch (opt) {
-    case NSM_OPT_BATCH_READY: f->batch_ready = value != 0; f->side_ok = false; return NSM_OK;
+    case NSM_OPT_BATCH_READY: f->batch_ready = value != 0; leave_fast_path(f); return NSM_OK;
   }
   return fail(NSM_ERR_INVALID_ARG, "unknown option %d", (int)opt);
 }
 
 nsm_status nsm_debug_set_grad(nsm_field *f, const float *d_grad, const uint8_t *d_touched) {
   if (!f) return fail(NSM_ERR_INVALID_ARG, "field is NULL");
-  f->side_ok = false;
+  leave_fast_path(f);
   if (!d_grad) return fail(NSM_ERR_INVALID_ARG, "d_grad is NULL");
   f->wgrad_parts = 0;
   RUN(f, K_DEBUG, launch_set_grad(f->fp, d_grad, d_touched, f->stream));
@@ -786,7 +805,7 @@ static nsm_status render_chunks(nsm_field *f, const nsm_ray_batch *b, float cut,
                                 bool host) {
   nsm_status st = validate_batch(f, b, false, true);
   if (st != NSM_OK) return st;
-  f->side_ok = false;
+  leave_fast_path(f);
   if (!rgb || !depth) return fail(NSM_ERR_INVALID_ARG, "output pointers are NULL");
   if (!(cut >= 0.f)) return fail(NSM_ERR_INVALID_ARG, "transmittance_cut must be >= 0");
   const uint32_t M = f->cfg.max_rays;
@@ -830,7 +849,7 @@ nsm_status nsm_render_host(nsm_field *f, const nsm_ray_batch *hb, float cut, flo
 
 nsm_status nsm_debug_last_step(nsm_field *f, int item, void *d_out, uint64_t capacity_bytes, uint64_t *n_bytes_out) {
   if (!f) return fail(NSM_ERR_INVALID_ARG, "field is NULL");
-  f->side_ok = false;
+  leave_fast_path(f);
   if (f->last_R == 0) return fail(NSM_ERR_INVALID_ARG, "no step has been run yet");
   const uint32_t R = f->last_R;
   const uint32_t *d_S = f->ws.offsets + R;
