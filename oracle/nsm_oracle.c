@@ -788,3 +788,36 @@ int orc_render(const orc_config *cfg, const double *theta, const uint8_t *bits, 
   if (n_samples) *n_samples = total;
   return 0;
 }
+
+/* ---- F1: ray-batch sampler over a keyframe store (header comment of orc_sample_batch) ---------
+ * Plain loop over rays; every float operation is a single binary32 operation (the file is compiled with
+ * -ffp-contract=off, and fmaf / sqrtf / division are correctly rounded). */
+void orc_sample_batch(const orc_keyframe *kfs, uint32_t n_kf, uint64_t seed, uint32_t draw, uint32_t n_rays,
+                      uint32_t *kf_out, uint32_t *pix_out, float *origins, float *dirs, float *rgb, float *depth,
+                      float *depth_var) {
+  for (uint32_t r = 0; r < n_rays; ++r) {
+    const uint32_t h1 = orc_hash32(seed, draw, r, 0xffff0001u);
+    const uint32_t kf = (uint32_t)(((uint64_t)h1 * (uint64_t)n_kf) >> 32);
+    const orc_keyframe *k = &kfs[kf];
+    const uint32_t h2 = orc_hash32(seed, draw, r, 0xffff0002u);
+    const uint32_t pix = (uint32_t)(((uint64_t)h2 * ((uint64_t)k->width * k->height)) >> 32);
+    const uint32_t u = pix % k->width, v = pix / k->width;
+    const float xc = ((float)u - k->cx) / k->fx;
+    const float yc = ((float)v - k->cy) / k->fy;
+    const float n2 = fmaf(xc, xc, fmaf(yc, yc, 1.0f));
+    const float n = sqrtf(n2);
+    const float dx = xc / n, dy = yc / n, dz = 1.0f / n;
+    for (int i = 0; i < 3; ++i) {
+      float acc = k->R[3 * i + 2] * dz;
+      acc = fmaf(k->R[3 * i + 1], dy, acc);
+      acc = fmaf(k->R[3 * i + 0], dx, acc);
+      dirs[3 * (size_t)r + i] = acc;
+      origins[3 * (size_t)r + i] = k->t[i];
+      rgb[3 * (size_t)r + i] = k->rgb[3 * (size_t)pix + i];
+    }
+    depth[r] = k->depth[pix] * n;
+    depth_var[r] = k->depth_var[pix] * n2;
+    if (kf_out) kf_out[r] = kf;
+    if (pix_out) pix_out[r] = pix;
+  }
+}

@@ -21,6 +21,7 @@
  *   S13 Adam                              R16 (paper names no optimiser)
  *   S14 occupancy from field              R17
  *   S15 render with transmittance cut     PAPER.md:163; R15
+ *   F1  ray-batch sampler over keyframes   PAPER.md:157-159; DESIGN.md "F1"
  *
  * Precision: the INDEX PATH (everything that decides an integer, and the fp32 quantities
  * t, delta, x, w) is a fixed sequence of IEEE binary32 operations (compile with
@@ -142,6 +143,30 @@ int orc_occupancy_from_field(const orc_config *cfg, const double *theta, uint8_t
 /* S15. */
 int orc_render(const orc_config *cfg, const double *theta, const uint8_t *bits, const orc_batch *b,
                double cut, double *rgb, double *depth, double *opacity, uint64_t *n_samples);
+
+/* F1 ("the mapping thread ... optimizes all keyframes received", each with
+ * pose, image, depth map and the depth's marginal variance): the ray-batch sampler over a keyframe store.
+ * A keyframe is a pinhole view: pixel (u, v) has the camera-frame direction (xc, yc, 1), xc = (u - cx) / fx,
+ * yc = (v - cy) / fy; R (row-major) rotates camera to world, t is the camera centre.  depth is the z-depth map
+ * D(u, v) (what a SLAM front end estimates), depth_var its variance; rgb is [H, W, 3].
+ * For ray r of draw number `draw`:
+ *   kf   = (orc_hash32(seed, draw, r, 0xffff0001) * n_kf)      >> 32     uniform keyframe
+ *   pix  = (orc_hash32(seed, draw, r, 0xffff0002) * (W_kf H_kf)) >> 32   uniform pixel of it, u = pix % W, v = pix / W
+ *   n2   = fma(xc, xc, fma(yc, yc, 1)),  n = sqrt(n2)                     |(xc, yc, 1)|, all binary32, round to nearest
+ *   d_i  = fma(R[i][0], xc / n, fma(R[i][1], yc / n, R[i][2] * (1 / n)))  unit direction in the world
+ *   o    = t;  rgb copied;  depth_out = D * n  (range along the ray, reading R5);  var_out = depth_var * n2
+ * Every float operation above is one IEEE binary32 operation in the order written (index-path rule), so the CUDA
+ * sampler must reproduce the outputs bit for bit.  kf_out / pix_out may be NULL. */
+typedef struct {
+  uint32_t width, height;
+  float fx, fy, cx, cy;
+  float R[9];
+  float t[3];
+  const float *rgb, *depth, *depth_var;
+} orc_keyframe;
+void orc_sample_batch(const orc_keyframe *kfs, uint32_t n_kf, uint64_t seed, uint32_t draw, uint32_t n_rays,
+                      uint32_t *kf_out, uint32_t *pix_out, float *origins, float *dirs, float *rgb, float *depth,
+                      float *depth_var);
 
 /* Threads the library will use (1 unless built with -fopenmp). */
 int orc_num_threads(void);

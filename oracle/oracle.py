@@ -35,6 +35,12 @@ class OrcBatch(C.Structure):
                 ("n_candidates", C.c_uint32)]
 
 
+class OrcKeyframe(C.Structure):
+    _fields_ = [("width", C.c_uint32), ("height", C.c_uint32), ("fx", C.c_float), ("fy", C.c_float),
+                ("cx", C.c_float), ("cy", C.c_float), ("R", C.c_float * 9), ("t", C.c_float * 3),
+                ("rgb", C.POINTER(C.c_float)), ("depth", C.POINTER(C.c_float)), ("depth_var", C.POINTER(C.c_float))]
+
+
 class OrcStats(C.Structure):
     _fields_ = [("loss", C.c_double), ("loss_rgb", C.c_double), ("loss_depth", C.c_double),
                 ("n_samples", C.c_uint64), ("n_rays", C.c_uint32), ("step", C.c_uint32)]
@@ -83,6 +89,9 @@ def lib(omp=False):
         L.orc_occupancy_from_field.argtypes = [C.POINTER(OrcConfig), _f64p, _u8p, _f64p]
         L.orc_render.argtypes = [C.POINTER(OrcConfig), _f64p, _u8p, C.POINTER(OrcBatch), C.c_double,
                                  _f64p, _f64p, _f64p, _u64p]
+        L.orc_sample_batch.argtypes = [C.POINTER(OrcKeyframe), C.c_uint32, C.c_uint64, C.c_uint32, C.c_uint32,
+                                       _u32p, _u32p, _f32p, _f32p, _f32p, _f32p, _f32p]
+        L.orc_sample_batch.restype = None
         L.orc_num_threads.restype = C.c_int
         _LIBS[key] = L
     return _LIBS[key]
@@ -247,6 +256,31 @@ def adam(theta, m, v, g, step, lr, beta1, beta2, eps, mask=None, mask_group=1):
     mask = None if mask is None else np.ascontiguousarray(mask, np.uint8)
     lib().orc_adam(theta.size, _p(theta, _f64p), _p(m, _f64p), _p(v, _f64p), _p(g, _f64p),
                    _p(mask, _u8p), int(mask_group), int(step), lr, beta1, beta2, eps)
+
+
+def sample_batch(keyframes, seed, draw, n_rays):
+    """F1: the ray-batch sampler.  keyframes: list of dicts with width, height, fx, fy, cx, cy, R (3x3 camera-to-world),
+    t (3,), rgb [H,W,3], depth [H,W] (z-depth), depth_var [H,W].  Returns a dict of arrays (kf, pix, origins, dirs,
+    rgb, depth, depth_var)."""
+    arr = (OrcKeyframe * len(keyframes))()
+    keep = []
+    for a, k in zip(arr, keyframes):
+        a.width, a.height = int(k["width"]), int(k["height"])
+        a.fx, a.fy, a.cx, a.cy = (float(np.float32(k[n])) for n in ("fx", "fy", "cx", "cy"))
+        a.R[:] = [float(x) for x in np.asarray(k["R"], np.float32).reshape(9)]
+        a.t[:] = [float(x) for x in np.asarray(k["t"], np.float32).reshape(3)]
+        bufs = [np.ascontiguousarray(k[n], np.float32).reshape(-1) for n in ("rgb", "depth", "depth_var")]
+        assert bufs[0].size == 3 * a.width * a.height and bufs[1].size == bufs[2].size == a.width * a.height
+        keep.append(bufs)
+        a.rgb, a.depth, a.depth_var = (_p(b, _f32p) for b in bufs)
+    R = int(n_rays)
+    out = dict(kf=np.empty(R, np.uint32), pix=np.empty(R, np.uint32), origins=np.empty((R, 3), np.float32),
+               dirs=np.empty((R, 3), np.float32), rgb=np.empty((R, 3), np.float32), depth=np.empty(R, np.float32),
+               depth_var=np.empty(R, np.float32))
+    lib().orc_sample_batch(arr, len(keyframes), int(seed), int(draw), R, _p(out["kf"], _u32p), _p(out["pix"], _u32p),
+                           _p(out["origins"], _f32p), _p(out["dirs"], _f32p), _p(out["rgb"], _f32p),
+                           _p(out["depth"], _f32p), _p(out["depth_var"], _f32p))
+    return out
 
 
 class Oracle:

@@ -240,6 +240,20 @@ class KeyframeSet:
                                    range=r.astype(np.float32), outlier=outlier)
         return self._frames[i]
 
+    def store_frame(self, i):
+        """Keyframe i as a SLAM front end would hand it over: pinhole intrinsics, camera-to-world
+        rotation and centre, image, z-DEPTH map and its variance (the ranges of frame() divided by |(xc, yc, 1)|,
+        variances by its square)."""
+        fr = self.frame(i)
+        pix = np.arange(self.W * self.H)
+        u, v = pix % self.W, pix // self.W
+        n = np.sqrt(((u - self.cx) / self.fx) ** 2 + ((v - self.cy) / self.fy) ** 2 + 1.0)
+        return dict(width=self.W, height=self.H, fx=self.fx, fy=self.fy, cx=self.cx, cy=self.cy,
+                    R=self.rot[i].astype(np.float32), t=self.centres[i].astype(np.float32),
+                    rgb=fr["rgb"].reshape(self.H, self.W, 3),
+                    depth=(fr["depth"].astype(np.float64) / n).astype(np.float32).reshape(self.H, self.W),
+                    depth_var=(fr["var"].astype(np.float64) / n ** 2).astype(np.float32).reshape(self.H, self.W))
+
     def draw_batch(self, step, R, t_min, t_max, K, batch_cls):
         rng = np.random.Generator(np.random.PCG64([self.seed, 0xba7c, step]))
         kf = rng.integers(0, self.n, R)
