@@ -153,6 +153,33 @@ nsm_status nsm_train_step_host(nsm_field *f, const nsm_ray_batch *host_batch, fl
  * start of ~0 / end of 0 means "did not run".  Synchronises.  Costs a few atomics per block: not for timing runs. */
 nsm_status nsm_debug_timeline(nsm_field *f, uint64_t *h_out, uint64_t capacity_words, uint32_t *n_kernels);
 
+/* ---- Row F1: keyframe store and ray-batch sampler (the mapping thread optimises over all
+ * keyframes received so far, each with its pose, image, depth map and the depth's marginal variance). ----
+ * A keyframe is a pinhole view: pixel (u, v) looks along the camera-frame direction ((u-cx)/fx, (v-cy)/fy, 1);
+ * R (row-major) rotates camera to world, t is the camera centre in the world. */
+typedef struct {
+  uint32_t width, height;
+  float fx, fy, cx, cy;
+  float R[9];
+  float t[3];
+} nsm_keyframe_info;
+/* Copies the image [H,W,3], the z-depth map [H,W] and its variance [H,W] (DEVICE pointers, caller-owned, free after
+ * the call's work on the stream) into the library's store.  NSM_ERR_CAPACITY beyond 1024 keyframes. */
+nsm_status nsm_add_keyframe(nsm_field *f, const nsm_keyframe_info *info, const float *d_rgb, const float *d_depth,
+                            const float *d_depth_var, uint32_t *index_out);
+nsm_status nsm_keyframe_count(const nsm_field *f, uint32_t *n_out);
+/* Draw number `draw` of n_rays rays, uniform over (keyframe, pixel): for ray r
+ *   kf = (h(seed, draw, r, 0xffff0001) * n_keyframes) >> 32,  pix = (h(seed, draw, r, 0xffff0002) * (W H)) >> 32
+ * (h = the jitter hash of DESIGN.md S1, seed = config seed), unit world direction, origin t, colour, and the
+ * z-depth / variance converted to RANGE along the ray (x |(xc,yc,1)| and x its square).  Outputs are DEVICE
+ * buffers in the layout of nsm_ray_batch; bit-identical to the oracle's sampler. */
+nsm_status nsm_sample_batch(nsm_field *f, uint32_t n_rays, uint32_t draw, float *d_origins, float *d_dirs, float *d_rgb,
+                            float *d_depth, float *d_depth_var);
+/* nsm_train_step on the batch nsm_sample_batch would draw with draw = (steps taken so far) + 1, without the batch
+ * leaving the library: the sampler and the marcher of step i+1 run beside the table update of step i. */
+nsm_status nsm_train_step_sampled(nsm_field *f, uint32_t n_rays, float t_min, float t_max, uint32_t n_candidates,
+                                  float lambda_d, nsm_step_stats *host_stats);
+
 /* Options.
  * NSM_OPT_BATCH_READY (default 0).  With 0 the library reads a batch strictly in the order of the field's
  * stream.  With 1 the caller declares that the device buffers of every batch handed to nsm_train_step are

@@ -28,6 +28,7 @@ EXPORTS = ["nsm_create_field", "nsm_destroy_field", "nsm_update_occupancy", "nsm
            "nsm_train_step", "nsm_train_step_host", "nsm_backward", "nsm_apply_adam", "nsm_debug_set_grad",
            "nsm_render", "nsm_render_host", "nsm_param_count", "nsm_get_params", "nsm_set_params",
            "nsm_get_level_table", "nsm_debug_last_step", "nsm_total_samples", "nsm_profile", "nsm_set_option", "nsm_debug_timeline",
+           "nsm_add_keyframe", "nsm_keyframe_count", "nsm_sample_batch", "nsm_train_step_sampled",
            "nsm_profile_read", "nsm_launch_count", "nsm_mlp_path",
            "nsm_last_error", "nsm_version"]
 
@@ -49,6 +50,11 @@ class NsmRayBatch(C.Structure):
     _fields_ = [("n_rays", C.c_uint32), ("origins", C.c_void_p), ("dirs", C.c_void_p), ("rgb", C.c_void_p),
                 ("depth", C.c_void_p), ("depth_var", C.c_void_p), ("t_min", C.c_float), ("t_max", C.c_float),
                 ("n_candidates", C.c_uint32)]
+
+
+class NsmKeyframeInfo(C.Structure):
+    _fields_ = [("width", C.c_uint32), ("height", C.c_uint32), ("fx", C.c_float), ("fy", C.c_float),
+                ("cx", C.c_float), ("cy", C.c_float), ("R", C.c_float * 9), ("t", C.c_float * 3)]
 
 
 class NsmStepStats(C.Structure):
@@ -93,6 +99,10 @@ def load_library():
         L.nsm_total_samples.argtypes = [vp, u64p]
         L.nsm_profile.argtypes = [vp, C.c_int]
         L.nsm_set_option.argtypes = [vp, C.c_int, C.c_uint32]
+        L.nsm_add_keyframe.argtypes = [vp, C.POINTER(NsmKeyframeInfo), vp, vp, vp, u32p]
+        L.nsm_keyframe_count.argtypes = [vp, u32p]
+        L.nsm_sample_batch.argtypes = [vp, C.c_uint32, C.c_uint32, vp, vp, vp, vp, vp]
+        L.nsm_train_step_sampled.argtypes = [vp, C.c_uint32, C.c_float, C.c_float, C.c_uint32, C.c_float, C.POINTER(NsmStepStats)]
         L.nsm_debug_timeline.argtypes = [vp, u64p, C.c_uint64, u32p]
         L.nsm_profile_read.argtypes = [vp, C.c_uint32, C.POINTER(C.c_char_p), C.POINTER(C.c_double), u64p, u32p]
         L.nsm_launch_count.argtypes = [vp]
@@ -284,6 +294,45 @@ class Field:
 
     def nsm_train_step_host(self, host_batch, lambda_d, want_stats=True):
         return self._step(self.lib.nsm_train_step_host, host_batch, lambda_d, want_stats)
+
+    # ---- row F1: keyframe store and sampler
+    def nsm_add_keyframe(self, kf):
+        """kf: dict with width, height, fx, fy, cx, cy, R (3x3 camera-to-world), t (3,), rgb [H,W,3], depth [H,W]
+        (z-depth), depth_var [H,W]; arrays may be numpy (uploaded here) or CUDA tensors.  Returns the keyframe index."""
+        info = NsmKeyframeInfo()
+        info.width, info.height = int(kf["width"]), int(kf["height"])
+        info.fx, info.fy, info.cx, info.cy = (float(kf[n]) for n in ("fx", "fy", "cx", "cy"))
+        info.R[:] = [float(x) for x in np.asarray(kf["R"], np.float32).reshape(9)]
+        info.t[:] = [float(x) for x in np.asarray(kf["t"], np.float32).reshape(3)]
+        dev = []
+        for n in ("rgb", "depth", "depth_var"):
+            a = kf[n]
+            t = a if isinstance(a, torch.Tensor) else torch.as_tensor(np.ascontiguousarray(a, np.float32))
+            dev.append(t.to(self.device, torch.float32).contiguous())
+        idx = C.c_uint32()
+        _check(self.lib.nsm_add_keyframe(self.h, C.byref(info), dev[0].data_ptr(), dev[1].data_ptr(), dev[2].data_ptr(), C.byref(idx)))
+        torch.cuda.synchronize(self.device)      # the uploads above may be freed now
+        return int(idx.value)
+
+    def nsm_keyframe_count(self):
+        n = C.c_uint32()
+        _check(self.lib.nsm_keyframe_count(self.h, C.byref(n)))
+        return int(n.value)
+
+    def nsm_sample_batch(self, n_rays, draw):
+        """Draw `draw` of n_rays rays as CUDA tensors: dict(origins, dirs, rgb, depth, depth_var)."""
+        R = int(n_rays)
+        out = dict(origins=torch.empty((R, 3), device=self.device), dirs=torch.empty((R, 3), device=self.device),
+                   rgb=torch.empty((R, 3), device=self.device), depth=torch.empty(R, device=self.device),
+                   depth_var=torch.empty(R, device=self.device))
+        _check(self.lib.nsm_sample_batch(self.h, R, int(draw), *(out[k].data_ptr() for k in ("origins", "dirs", "rgb", "depth", "depth_var"))))
+        return out
+
+    def nsm_train_step_sampled(self, n_rays, t_min, t_max, n_candidates, lambda_d, want_stats=True):
+        st = NsmStepStats()
+        _check(self.lib.nsm_train_step_sampled(self.h, int(n_rays), float(t_min), float(t_max), int(n_candidates),
+                                               float(lambda_d), C.byref(st) if want_stats else None))
+        return _stats(st) if want_stats else None
 
     def nsm_backward(self, batch, lambda_d, want_stats=True):
         return self._step(self.lib.nsm_backward, batch, lambda_d, want_stats)

@@ -9,28 +9,10 @@
 
 namespace {
 
-// DESIGN.md S1.1 — jitter hash (two-multiply xorshift finaliser absorbing seed, step, r, k).
-__device__ __forceinline__ uint32_t mix32(uint32_t x) {
-  x ^= x >> 16;
-  x *= 0x7feb352du;
-  x ^= x >> 15;
-  x *= 0x846ca68bu;
-  x ^= x >> 16;
-  return x;
-}
-
 __device__ __forceinline__ float jitter_u(uint32_t h_seed_step_ray, uint32_t k, uint32_t jitter) {
   if (!jitter) return 0.5f;
-  uint32_t h = mix32(h_seed_step_ray ^ k);
+  uint32_t h = nsm_mix32(h_seed_step_ray ^ k);
   return __uint2float_rn(h >> 8) * 0x1p-24f;  // 24-bit integer, exact
-}
-
-__device__ __forceinline__ uint32_t ray_hash_prefix(uint64_t seed, uint32_t step, uint32_t r) {
-  uint32_t h = mix32((uint32_t)(seed & 0xffffffffu) ^ 0x9e3779b9u);
-  h = mix32(h ^ (uint32_t)(seed >> 32));
-  h = mix32(h ^ step);
-  h = mix32(h ^ r);
-  return h;
 }
 
 struct Candidate {
@@ -113,7 +95,7 @@ __global__ void __launch_bounds__(MARCH_WARPS * 32) march_fused_kernel(MarchPara
       d[a] = __ldg(dirs + 3 * (size_t)r + a);
     }
     if (dirs_copy && lane < 3) dirs_copy[3 * (size_t)r + lane] = lane == 0 ? d[0] : (lane == 1 ? d[1] : d[2]);
-    hpre = ray_hash_prefix(mp.seed, mp.step, r);
+    hpre = nsm_hash_prefix(mp.seed, mp.step, r);
     for (uint32_t wd0 = 0; wd0 < words; wd0 += 4) {   // four words at a time: their occupancy loads are independent
       bool live[4];
 #pragma unroll

@@ -49,7 +49,7 @@ uint32_t g_pdl_mask = [] {
 int g_cur_kernel = 0;
 
 static const char *kKernelNames[K_COUNT] = {"march", "encode", "mlp_fwd", "composite",
-                                            "mlp_bwd", "scatter", "adam_table", "adam_mlp", "occupancy", "debug"};
+                                            "mlp_bwd", "scatter", "adam_table", "adam_mlp", "occupancy", "debug", "sample"};
 
 // Optional per-kernel CUDA-event timing (bench.py's roofline leg).  When enabled every launch is
 // bracketed by two events on the field's stream and each step ends with a synchronise.
@@ -107,6 +107,9 @@ struct nsm_field {
   // the step's statistics (loss sums, S) are final after the compositor: they are copied out on the side stream right
   // behind it, and a call that wants them waits for that copy only, not for the backward pass and Adam
   cudaEvent_t ev_comp = nullptr, ev_stats = nullptr;
+  // F1: the keyframe store (library-owned device copies) and its device-side directory
+  std::vector<KeyframeDev> kf_host;
+  KeyframeDev *kf_dev = nullptr;
   bool stats_pending = false;
   bool join_pending = false;   // ev_side (recorded behind the MLP Adam) has not been waited for on the main stream yet
   unsigned long long *timeline_base = nullptr;   // NSM_TIMELINE=1: ring of 64 steps x [2][K_COUNT] globaltimer stamps
@@ -252,8 +255,10 @@ MarchParams make_march(const nsm_field *f, const nsm_ray_batch *b, uint32_t R, b
 // march_on_side: the marcher runs on the side stream, behind "scatter of the previous step done" only,
 // i.e. beside the previous step's table Adam (NSM_OPT_BATCH_READY; training steps only).
 // dirs_copy: see launch_march (zero-copy host batches); the MLP kernels then read the copy.
+// sample_draw >= 0: the batch is first drawn from the keyframe store (F1) into b's buffers (the field's staging area),
+// on the stream the marcher runs on.
 void enqueue_forward(nsm_field *f, const nsm_ray_batch *b, uint32_t R, bool jitter, uint32_t step, bool train,
-                     bool march_on_side = false, float *dirs_copy = nullptr) {
+                     bool march_on_side = false, float *dirs_copy = nullptr, int64_t sample_draw = -1) {
   const uint32_t *d_S = f->ws.offsets + R;
   const float *mlp_dirs = dirs_copy ? dirs_copy : b->dirs;
   MarchParams mp = make_march(f, b, R, jitter, step);
@@ -262,12 +267,20 @@ void enqueue_forward(nsm_field *f, const nsm_ray_batch *b, uint32_t R, bool jitt
       cudaEventRecord(f->ev_main, f->stream);
       cudaStreamWaitEvent(f->side, f->ev_main, 0);
     }
+    if (sample_draw >= 0)
+      RUN_ON(f, K_SAMPLE, f->side, launch_sample_batch(f->kf_dev, (uint32_t)f->kf_host.size(), f->cfg.seed, (uint32_t)sample_draw, R,
+                                                       (float *)b->origins, (float *)b->dirs, (float *)b->rgb, (float *)b->depth,
+                                                       (float *)b->depth_var, f->side));
     RUN_ON(f, K_MARCH, f->side, launch_march(mp, f->occ_full ? nullptr : f->fp.occ_bits, b->origins, b->dirs, f->ws, train ? 1 : 0, f->side, dirs_copy));
     cudaEventRecord(f->ev_side, f->side);
     cudaStreamWaitEvent(f->stream, f->ev_side, 0);
     f->join_pending = false;   // behind the marcher is behind the previous step's MLP Adam too
   } else {
     join_side(f);
+    if (sample_draw >= 0)
+      RUN(f, K_SAMPLE, launch_sample_batch(f->kf_dev, (uint32_t)f->kf_host.size(), f->cfg.seed, (uint32_t)sample_draw, R,
+                                           (float *)b->origins, (float *)b->dirs, (float *)b->rgb, (float *)b->depth,
+                                           (float *)b->depth_var, f->stream));
     RUN(f, K_MARCH, launch_march(mp, f->occ_full ? nullptr : f->fp.occ_bits, b->origins, b->dirs, f->ws, train ? 1 : 0, f->stream, dirs_copy));
   }
   const int bf16 = f->cfg.mlp_precision == NSM_MLP_BF16;
@@ -296,7 +309,7 @@ nsm_status clear_grads_if_dirty(nsm_field *f) {
 
 nsm_status enqueue_backward(nsm_field *f, const nsm_ray_batch *b, float lambda_d, bool march_on_side = false,
                             float *dirs_copy = nullptr, bool want_stats = false, bool reduce_wgrad_now = false,
-                            bool defer_scatter = false) {
+                            bool defer_scatter = false, int64_t sample_draw = -1) {
   const uint32_t R = b->n_rays;
   const uint32_t *d_S = f->ws.offsets + R;
   nsm_status st = clear_grads_if_dirty(f);
@@ -307,7 +320,7 @@ nsm_status enqueue_backward(nsm_field *f, const nsm_ray_batch *b, float lambda_d
     cudaMemsetAsync(later, 0xff, sizeof(unsigned long long) * K_COUNT, f->stream);
     cudaMemsetAsync(later + K_COUNT, 0, sizeof(unsigned long long) * K_COUNT, f->stream);
   }
-  enqueue_forward(f, b, R, f->cfg.jitter != 0, f->step + 1, true, march_on_side, dirs_copy);
+  enqueue_forward(f, b, R, f->cfg.jitter != 0, f->step + 1, true, march_on_side, dirs_copy, sample_draw);
   f->side_ok = false;
   RUN(f, K_COMPOSITE, launch_composite_train(f->ws, R, b->rgb, b->depth, b->depth_var, lambda_d, f->cfg.bg, f->stream));
   if (want_stats) {
@@ -532,6 +545,7 @@ nsm_status nsm_create_field(const nsm_field_config *cfg, void *cuda_stream, nsm_
   }
   A(f->alloc(&ws.sigma, cap)); A(f->alloc(&ws.rgb, 3 * cap)); A(f->alloc(&ws.T_excl, cap));
   A(f->alloc(&ws.dsigma, cap)); A(f->alloc(&ws.drgb, 3 * cap)); A(f->alloc(&ws.de, ms.LF * cap));
+  A(f->alloc(&f->kf_dev, NSM_MAX_KEYFRAMES));
   ws.timeline = nullptr;
   {
     const char *tl = std::getenv("NSM_TIMELINE");
@@ -731,10 +745,10 @@ nsm_status nsm_apply_adam(nsm_field *f) {
 }
 
 static nsm_status train_step_impl(nsm_field *f, const nsm_ray_batch *batch, float lambda_d, nsm_step_stats *host_stats,
-                                  bool batch_ready, float *dirs_copy = nullptr) {
+                                  bool batch_ready, float *dirs_copy = nullptr, int64_t sample_draw = -1) {
   nsm_status st = validate_batch(f, batch, true, false);
   if (st != NSM_OK) return st;
-  st = enqueue_backward(f, batch, lambda_d, batch_ready, dirs_copy, host_stats != nullptr, false, true);
+  st = enqueue_backward(f, batch, lambda_d, batch_ready, dirs_copy, host_stats != nullptr, false, true, sample_draw);
   if (st != NSM_OK) return st;
   st = enqueue_adam(f);
   if (st != NSM_OK) return st;
@@ -780,6 +794,69 @@ nsm_status nsm_debug_timeline(nsm_field *f, uint64_t *h_out, uint64_t capacity_w
   CUDA_TRY(cudaMemcpy(h_out, f->timeline_base, sizeof(uint64_t) * 64 * 2 * K_COUNT, cudaMemcpyDeviceToHost));
   if (n_kernels) *n_kernels = K_COUNT;
   return NSM_OK;
+}
+
+// ---- F1: keyframe store and sampled training -------------------------------------------------------------------
+nsm_status nsm_add_keyframe(nsm_field *f, const nsm_keyframe_info *info, const float *d_rgb, const float *d_depth,
+                            const float *d_depth_var, uint32_t *index_out) {
+  if (!f || !info || !d_rgb || !d_depth || !d_depth_var) return fail(NSM_ERR_INVALID_ARG, "NULL argument");
+  if (info->width == 0 || info->height == 0 || (uint64_t)info->width * info->height > (1ull << 31))
+    return fail(NSM_ERR_INVALID_ARG, "bad keyframe size %u x %u", info->width, info->height);
+  if (!(info->fx > 0.f) || !(info->fy > 0.f) || !std::isfinite(info->fx) || !std::isfinite(info->fy))
+    return fail(NSM_ERR_INVALID_ARG, "focal lengths must be positive");
+  if (f->kf_host.size() >= NSM_MAX_KEYFRAMES) return fail(NSM_ERR_CAPACITY, "keyframe store is full (%d)", NSM_MAX_KEYFRAMES);
+  leave_fast_path(f);
+  const size_t n = (size_t)info->width * info->height;
+  float *buf = nullptr;
+  CUDA_TRY(f->alloc(&buf, 5 * n, false));
+  CUDA_TRY(cudaMemcpyAsync(buf, d_rgb, sizeof(float) * 3 * n, cudaMemcpyDeviceToDevice, f->stream));
+  CUDA_TRY(cudaMemcpyAsync(buf + 3 * n, d_depth, sizeof(float) * n, cudaMemcpyDeviceToDevice, f->stream));
+  CUDA_TRY(cudaMemcpyAsync(buf + 4 * n, d_depth_var, sizeof(float) * n, cudaMemcpyDeviceToDevice, f->stream));
+  KeyframeDev k;
+  k.W = info->width; k.H = info->height;
+  k.fx = info->fx; k.fy = info->fy; k.cx = info->cx; k.cy = info->cy;
+  for (int i = 0; i < 9; ++i) k.R[i] = info->R[i];
+  for (int i = 0; i < 3; ++i) k.t[i] = info->t[i];
+  k.rgb = buf; k.depth = buf + 3 * n; k.var = buf + 4 * n;
+  f->kf_host.push_back(k);
+  const size_t idx = f->kf_host.size() - 1;
+  // the directory entry: a pageable source is copied out by the runtime before the call returns
+  CUDA_TRY(cudaMemcpyAsync(f->kf_dev + idx, &f->kf_host[idx], sizeof(KeyframeDev), cudaMemcpyHostToDevice, f->stream));
+  if (index_out) *index_out = (uint32_t)idx;
+  return NSM_OK;
+}
+
+nsm_status nsm_keyframe_count(const nsm_field *f, uint32_t *n_out) {
+  if (!f || !n_out) return fail(NSM_ERR_INVALID_ARG, "NULL argument");
+  *n_out = (uint32_t)f->kf_host.size();
+  return NSM_OK;
+}
+
+nsm_status nsm_sample_batch(nsm_field *f, uint32_t n_rays, uint32_t draw, float *d_origins, float *d_dirs, float *d_rgb,
+                            float *d_depth, float *d_depth_var) {
+  if (!f || !d_origins || !d_dirs || !d_rgb || !d_depth || !d_depth_var) return fail(NSM_ERR_INVALID_ARG, "NULL argument");
+  if (f->kf_host.empty()) return fail(NSM_ERR_INVALID_ARG, "the keyframe store is empty");
+  if (n_rays == 0) return fail(NSM_ERR_INVALID_ARG, "n_rays is 0");
+  leave_fast_path(f);
+  RUN(f, K_SAMPLE, launch_sample_batch(f->kf_dev, (uint32_t)f->kf_host.size(), f->cfg.seed, draw, n_rays, d_origins, d_dirs, d_rgb,
+                                       d_depth, d_depth_var, f->stream));
+  CUDA_TRY(cudaGetLastError());
+  return NSM_OK;
+}
+
+nsm_status nsm_train_step_sampled(nsm_field *f, uint32_t n_rays, float t_min, float t_max, uint32_t n_candidates, float lambda_d,
+                                  nsm_step_stats *host_stats) {
+  if (!f) return fail(NSM_ERR_INVALID_ARG, "field is NULL");
+  if (f->kf_host.empty()) return fail(NSM_ERR_INVALID_ARG, "the keyframe store is empty");
+  if (n_rays > f->cfg.max_rays) return fail(NSM_ERR_CAPACITY, "n_rays %u > max_rays %u", n_rays, f->cfg.max_rays);
+  // the batch lives in the field's staging area; the sampler and the marcher run beside the previous step's table Adam
+  const size_t M = f->cfg.max_rays;
+  nsm_ray_batch b;
+  b.n_rays = n_rays;
+  b.origins = f->stage_dev; b.dirs = f->stage_dev + 3 * M; b.rgb = f->stage_dev + 6 * M;
+  b.depth = f->stage_dev + 9 * M; b.depth_var = f->stage_dev + 10 * M;
+  b.t_min = t_min; b.t_max = t_max; b.n_candidates = n_candidates;
+  return train_step_impl(f, &b, lambda_d, host_stats, true, nullptr, (int64_t)(f->step + 1));
 }
 
 nsm_status nsm_set_option(nsm_field *f, nsm_option opt, uint32_t value) {

@@ -72,8 +72,37 @@ struct Workspace {
 // Kernel classes, for launch counting and the optional per-kernel event timing.
 enum KernelId {
   K_MARCH = 0, K_ENCODE, K_MLP_FWD, K_COMPOSITE, K_MLP_BWD, K_SCATTER,
-  K_ADAM_TABLE, K_ADAM_MLP, K_OCC, K_DEBUG, K_COUNT
+  K_ADAM_TABLE, K_ADAM_MLP, K_OCC, K_DEBUG, K_SAMPLE, K_COUNT
 };
+
+// DESIGN.md S1.1 -- the counter-based hash behind the jitter stream (S1) and the batch sampler (F1):
+// two-multiply xorshift finaliser absorbing seed, step, ray, k.  32-bit wrap-around arithmetic.
+__device__ __forceinline__ uint32_t nsm_mix32(uint32_t x) {
+  x ^= x >> 16;
+  x *= 0x7feb352du;
+  x ^= x >> 15;
+  x *= 0x846ca68bu;
+  x ^= x >> 16;
+  return x;
+}
+__device__ __forceinline__ uint32_t nsm_hash_prefix(uint64_t seed, uint32_t step, uint32_t r) {
+  uint32_t h = nsm_mix32((uint32_t)(seed & 0xffffffffu) ^ 0x9e3779b9u);
+  h = nsm_mix32(h ^ (uint32_t)(seed >> 32));
+  h = nsm_mix32(h ^ step);
+  h = nsm_mix32(h ^ r);
+  return h;
+}
+
+// F1: one keyframe of the device-side store (pinhole view; R rotates camera to world, row-major; t = camera centre;
+// rgb [H,W,3], z-depth [H,W] and its variance [H,W] are library-owned device copies)
+struct KeyframeDev {
+  uint32_t W, H;
+  float fx, fy, cx, cy;
+  float R[9];
+  float t[3];
+  const float *rgb, *depth, *var;
+};
+#define NSM_MAX_KEYFRAMES 1024
 
 // Debug timeline: when ws.timeline is set, thread 0 of every block stamps the kernel class's earliest start
 // and latest end with %globaltimer.  Unlike CUDA events between launches this does not disturb PDL or the
@@ -267,6 +296,9 @@ int launch_adam_mlp(const FieldParams &fp, float lr, float beta1, float beta2, f
 // n_ctas > 0: the gradient is the sum of the backward kernel's slices (+ fp.mlp_grad); 0: fp.mlp_grad alone
 int launch_adam_mlp_pack(const MlpShape &ms, int bf16, const FieldParams &fp, const Workspace &ws, const AdamConst &c,
                          uint32_t n_ctas, const uint32_t *d_S, cudaStream_t st);
+// F1: n_rays rays drawn uniformly over (keyframe, pixel) for draw number `draw`; outputs are a ray batch
+int launch_sample_batch(const KeyframeDev *kfs, uint32_t n_kf, uint64_t seed, uint32_t draw, uint32_t n_rays, float *origins,
+                        float *dirs, float *rgb, float *depth, float *depth_var, cudaStream_t st);
 int launch_occ_cells(uint32_t G, uint64_t first_cell, uint64_t n_cells, const Workspace &ws,
                      uint32_t *d_S, cudaStream_t st);
 int launch_occ_threshold(uint32_t G, uint64_t first_cell, uint64_t n_cells, const float *sigma,

@@ -386,3 +386,54 @@ def test_batch_ready_option_gives_the_same_steps(nsm):
     ca, cb = fa.nsm_debug_last_step("counts"), fb.nsm_debug_last_step("counts")
     assert np.array_equal(ca, cb)
     fa.close(); fb.close()
+
+
+# ---------------------------------------------------------------------------- row F1: keyframe store + sampler
+
+def _small_store(seed=3, n=3, width=60, height=34):
+    from workloads import scenes
+    room = scenes.Room(seed)
+    kfs = scenes.KeyframeSet(room, seed, n, width=width, height=height)
+    return [kfs.store_frame(i) for i in range(n)]
+
+
+def test_sampler_bit_exact_against_the_oracle(nsm):
+    """nsm_sample_batch vs orc_sample_batch: every output word identical (index-path rule), keyframes of different
+    sizes, several draws, a ragged ray count."""
+    w = configs.config1()
+    f = nsm.Field(w.field, "cuda:0")
+    store = _small_store() + _small_store(seed=4, n=1, width=31, height=17)
+    for i, kf in enumerate(store):
+        assert f.nsm_add_keyframe(kf) == i
+    assert f.nsm_keyframe_count() == len(store)
+    for draw, R in ((1, 4099), (2, 1), (77, 257)):
+        g = f.nsm_sample_batch(R, draw)
+        ref = orc.sample_batch(store, w.field.seed, draw, R)
+        for k in ("origins", "dirs", "rgb", "depth", "depth_var"):
+            assert np.array_equal(g[k].cpu().numpy().view(np.uint32), ref[k].view(np.uint32)), (draw, k)
+    f.close()
+
+
+def test_train_step_sampled_equals_a_step_on_the_sampled_batch(nsm):
+    w = configs.config3(R=2048, K=128, n_keyframes=2, n_batches=1, width=120, height=68)
+    fa, _, _ = make_pair(nsm, w, seed=10, table_scale=0.05)
+    fb, _, _ = make_pair(nsm, w, seed=10, table_scale=0.05)
+    store = [w.extra["keyframes"].store_frame(i) for i in range(2)]
+    with pytest.raises(nsm.NsmError):
+        fa.nsm_train_step_sampled(2048, 0.05, 10.5, 128, 1.0)          # empty store
+    for kf in store:
+        fa.nsm_add_keyframe(kf)
+    for step in range(1, 5):
+        ref = orc.sample_batch(store, w.field.seed, step, 2048)
+        b = configs.RayBatch(ref["origins"], ref["dirs"], ref["rgb"], ref["depth"], ref["depth_var"], 0.05, 10.5, 128)
+        sa = fa.nsm_train_step_sampled(2048, 0.05, 10.5, 128, w.lambda_d, want_stats=(step % 2 == 0))
+        sb = fb.nsm_train_step(nsm.DeviceBatch(b), w.lambda_d)
+        if sa is not None:
+            assert sa["n_samples"] == sb["n_samples"] and sa["step"] == sb["step"] == step
+            assert abs(sa["loss"] - sb["loss"]) <= 2e-3 * abs(sb["loss"]), (step, sa["loss"], sb["loss"])
+    assert np.array_equal(fa.nsm_debug_last_step("counts"), fb.nsm_debug_last_step("counts"))
+    assert np.array_equal(fa.nsm_debug_last_step("s_x").view(np.uint32), fb.nsm_debug_last_step("s_x").view(np.uint32))
+    with pytest.raises(nsm.NsmError) as ei:
+        fa.nsm_train_step_sampled(w.field.max_rays + 1, 0.05, 10.5, 128, 1.0)
+    assert ei.value.status == 4
+    fa.close(); fb.close()
