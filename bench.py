@@ -347,6 +347,26 @@ def run_cuda(args):
     h2d = hbatches[0].bytes_in()
     d2h = 2 * 8 + 4   # the stats read-back: two double accumulators and the sample count
 
+    # ---- config 3 only: the same steps with the batches drawn on the device from the keyframe store (row F1)
+    sampled = None
+    if cfg == 3 and "keyframes" in w.extra:
+        kfs = w.extra["keyframes"]
+        for i in range(kfs.n):
+            f.nsm_add_keyframe(kfs.store_frame(i))
+        b0_ = w.batches[0]
+
+        def sampled_step(i):
+            if refresh and i > 0 and i % refresh == 0:
+                f.nsm_update_occupancy(nsm.NSM_OCC_FROM_FIELD, sync=False)
+            f.nsm_train_step_sampled(b0_.n_rays, b0_.t_min, b0_.t_max, b0_.n_candidates, lam, want_stats=False)
+        for i in range(W):
+            sampled_step(i)
+        s3 = f.nsm_total_samples()
+        t_s = timed(K, sampled_step, W + 2 * K)
+        v_s, _, _ = replicas.aggregate_throughput(f.nsm_total_samples() - s3, t_s)
+        sampled = dict(value=v_s, unit=UNIT, ms_per_step=1e3 * t_s / K, keyframes=kfs.n,
+                       store_bytes=kfs.n * kfs.W * kfs.H * 5 * 4, api="nsm_train_step_sampled")
+
     line = None
     if rank == 0:
         # ---- per-kernel pass (CUDA events around every launch on the field's stream; separate from the headline timing)
@@ -407,7 +427,7 @@ def run_cuda(args):
                     config=workload_config(w, cfg=cfg, extra=dict(table_params=f.n_table, mlp_params=f.n_mlp, mlp_path=f.nsm_mlp_path(),
                                                    parallelism=f"{world} independent replica(s)",
                                                    samples_per_step=total_samples / K / world)),
-                    rays_per_s=world * K * b0.n_rays / t_max, clocks=clocks,
+                    rays_per_s=world * K * b0.n_rays / t_max, clocks=clocks, sampled=sampled,
                     e2e=dict(value=e2e_value, unit=UNIT, h2d_bytes_per_step=h2d, d2h_bytes_per_step=d2h,
                              ms_per_step=1e3 * t_e2e / K),
                     gpu_launches=launches, roofline=roofline, kernels=kernels, cpu_baseline=cpu_baseline)
