@@ -449,3 +449,73 @@ def test_depth_loss_ablation_replay(nsm):
     assert wtd["depth_l1_m"] < 0.7 * none["depth_l1_m"], (none, wtd)                 # held-out view
     assert wtd["depth_l1_seen_m"] < 0.5 * none["depth_l1_seen_m"], (none, wtd)       # a training view
     assert wtd["psnr_seen"] > 18.0 and none["psnr_seen"] > 18.0, (none, wtd)
+
+
+def _first_rays(b, n):
+    return replace(b, origins=b.origins[:n].copy(), dirs=b.dirs[:n].copy(),
+                   rgb=None if b.rgb is None else b.rgb[:n].copy(), depth=None if b.depth is None else b.depth[:n].copy(),
+                   depth_var=None if b.depth_var is None else b.depth_var[:n].copy())
+
+
+def test_config3_full_size_batch_on_sampled_rays(nsm):
+    """BASELINE.json configs[2] in the launch configuration bench.py times (2^14 rays x 128 candidates, FULL occupancy:
+    ~1 M live samples).  Rays are independent given the parameters and ray r's jitter depends on r only, so the oracle
+    run on the FIRST 192 rays alone must reproduce those rays' sample lists bit for bit and their per-sample and
+    per-ray forward values within tolerance; the rest is checked through properties that hold at any size."""
+    w = configs.config3(n_keyframes=2, n_batches=1, width=600, height=340)       # R = 2^14, K = 128
+    f, O, theta0 = make_pair(nsm, w, seed=11, table_scale=0.05)
+    b = w.batches[0]
+    assert b.n_rays == 1 << 14
+    tol = tol_for(w.field, f.nsm_mlp_path())
+    st = f.nsm_backward(nsm.DeviceBatch(b), w.lambda_d)
+    n = 192
+    so, tr = O.train_step(_first_rays(b, n), w.lambda_d, apply_adam=False,
+                          trace=("counts", "offsets", "s_k", "s_t", "s_x", "sigma", "rgb", "C", "D_hat", "O"))
+    counts, offsets = f.nsm_debug_last_step("counts"), f.nsm_debug_last_step("offsets")
+    assert np.array_equal(counts[:n], tr["counts"]) and np.array_equal(offsets[:n + 1], tr["offsets"])
+    S_n = int(tr["offsets"][-1])
+    assert np.array_equal(f.nsm_debug_last_step("s_k")[:S_n], tr["s_k"])
+    for k in ("s_t", "s_x"):
+        assert np.array_equal(f.nsm_debug_last_step(k)[:S_n].view(np.uint32), tr[k].view(np.uint32)), k
+    for k in ("sigma", "rgb"):
+        assert_close(k, f.nsm_debug_last_step(k)[:S_n], tr[k], tol)
+    for k in ("C", "D_hat", "O"):
+        assert_close(k, f.nsm_debug_last_step(k)[:n], tr[k], tol)
+    # properties at full size
+    assert st["n_samples"] == int(counts.astype(np.int64).sum()) == int(offsets[-1]) and st["n_samples"] > 500000
+    assert np.array_equal(np.diff(offsets.astype(np.int64)), counts)
+    s_ray = f.nsm_debug_last_step("s_ray")
+    assert np.array_equal(np.bincount(s_ray, minlength=b.n_rays), counts) and np.all(np.diff(s_ray.astype(np.int64)) >= 0)
+    Oacc = f.nsm_debug_last_step("O")
+    assert np.all(Oacc >= -1e-6) and np.all(Oacc <= 1 + 1e-5)
+    touched = f.nsm_debug_last_step("touched").astype(bool)
+    grad = f.nsm_debug_last_step("grad")
+    assert not grad[:f.n_table][np.repeat(~touched, w.field.n_features)].any()      # untouched entries: exactly zero gradient
+    f.close()
+
+
+def test_config5_full_frame_render_on_sampled_rays(nsm):
+    """BASELINE.json configs[4] at full size: one 1200x680 view (816 000 rays, chunked by max_rays), 256 candidates,
+    cut 1e-4; the oracle renders the first 160 rays (one chunk prefix) and a property check covers the image."""
+    w = configs.config3(R=2048, K=128, n_keyframes=2, n_batches=4, width=300, height=170)
+    fc = replace(w.field, max_candidates=256, max_rays=1 << 16)
+    w = replace(w, field=fc)
+    f, O, theta0 = make_pair(nsm, w, seed=12, table_scale=0.05)
+    for b in w.batches:
+        f.nsm_train_step(nsm.DeviceBatch(b), w.lambda_d, want_stats=False)
+    O.theta = f.nsm_get_params()[0].astype(np.float64)
+    f.nsm_update_occupancy(nsm.NSM_OCC_FROM_FIELD)
+    O.set_occupancy(f.nsm_get_occupancy())
+    view = configs.config5_views(seed=3, n_views=1)[0]
+    assert view.n_rays == 1200 * 680
+    rgb, dep, opa = (t.cpu().numpy() for t in f.nsm_render(nsm.DeviceBatch(view), 1e-4))
+    tol = tol_for(fc, f.nsm_mlp_path())
+    n = 160
+    r_ref, d_ref, o_ref, _ = O.render(_first_rays(view, n), 1e-4)
+    allow = 1.3e-4
+    assert np.abs(rgb[:n] - r_ref).max() <= tol * max(np.abs(r_ref).max(), 1e-3) + allow
+    assert np.abs(dep[:n] - d_ref).max() <= tol * max(np.abs(d_ref).max(), 1e-3) + allow * view.t_max
+    assert np.abs(opa[:n] - o_ref).max() <= tol + allow
+    assert np.isfinite(rgb).all() and rgb.min() >= -1e-6 and rgb.max() <= 1 + 1e-5
+    assert opa.min() >= -1e-6 and opa.max() <= 1 + 1e-5 and dep.min() >= 0 and dep.max() <= view.t_max * (1 + 1e-5)
+    f.close()
