@@ -325,6 +325,35 @@ void orc_sh(uint32_t n, const double d[3], double *Y) {
   }
 }
 
+/* F2: rotation derivative of the direction encoding.  For d <- exp(omega^) d the first-order change is
+ * delta d = omega x d, i.e. delta z = omega_x y - omega_y x and delta phi = omega_z - z (omega_x x + omega_y y) / (x^2 + y^2)
+ * (phi = atan2(y, x)).  With dY/dz from (1 - z^2) dP_l^m/dz = (l + m) P_{l-1}^m - l z P_l^m and dY/dphi from the
+ * cos / sin factors, out[k] = sum_j gY[j] dY_j/d(omega_k).  Undefined at the poles (x = y = 0). */
+static void sh_rotation_gradient(uint32_t n, const double d[3], const double *gY, double out[3]) {
+  const double pi = 3.14159265358979323846;
+  const double x = d[0], y = d[1], z = d[2], rho2 = x * x + y * y;
+  const double phi = atan2(y, x);
+  double gz = 0.0, gphi = 0.0; /* dL/dz, dL/dphi */
+  for (int l = 0; l < (int)n; ++l) {
+    for (int m = 0; m <= l; ++m) {
+      double K = sqrt((double)(2 * l + 1) / (4.0 * pi) * factorial(l - m) / factorial(l + m));
+      double P = legendre_P(l, m, z);
+      double Pm1 = (l - 1 >= m) ? legendre_P(l - 1, m, z) : 0.0;
+      double dP = ((double)(l + m) * Pm1 - (double)l * z * P) / (1.0 - z * z);
+      if (m == 0) {
+        gz += gY[l * l + l] * K * dP;
+      } else {
+        double c = cos((double)m * phi), sn = sin((double)m * phi), a = sqrt(2.0) * K;
+        gz += gY[l * l + l + m] * a * c * dP + gY[l * l + l - m] * a * sn * dP;
+        gphi += gY[l * l + l + m] * a * (-(double)m * sn) * P + gY[l * l + l - m] * a * ((double)m * c) * P;
+      }
+    }
+  }
+  out[0] = gz * y + gphi * (-z * x / rho2);
+  out[1] = gz * (-x) + gphi * (-z * y / rho2);
+  out[2] = gphi;
+}
+
 /* ------------------------------------------------------------------ S5, S7: MLPs ---------- */
 
 typedef struct {
@@ -428,7 +457,7 @@ static void linear_backward(const double *W, double *dW, uint32_t n_out, uint32_
 
 /* S11 for one sample: given dL/dsigma and dL/drgb, accumulate dW (MLP block) and return dL/de. */
 static void mlp_backward(const orc_mlp *M, const double *Wm, double *dWm, const double *act,
-                         double dsigma, const double drgb[3], double *de) {
+                         double dsigma, const double drgb[3], double *de, double *dci_out) {
   const double *e = act + M->a_e, *hd = act + M->a_hd, *g = act + M->a_g, *ci = act + M->a_ci;
   const double *h1 = act + M->a_h1, *h2 = act + M->a_h2, *rgb = act + M->a_rgb;
   double dpre[3], dh2[ORC_MAX_WIDTH], dh1[ORC_MAX_WIDTH], dci[ORC_MAX_WIDTH], dg[ORC_MAX_WIDTH],
@@ -446,6 +475,8 @@ static void mlp_backward(const orc_mlp *M, const double *Wm, double *dWm, const 
   for (uint32_t i = 0; i < M->Hc; ++i)
     if (!(h1[i] > 0.0)) dh1[i] = 0.0;
   linear_backward(Wm + M->o_c1, dWm + M->o_c1, M->Hc, M->Ci, ci, dh1, dci);
+  if (dci_out)
+    for (uint32_t i = 0; i < M->Ci; ++i) dci_out[i] = dci[i]; /* dL/d(colour input): geo slice, then the SH terms */
   /* density outputs: geo slice from the colour net, g0 from sigma (0 if clamped) */
   for (uint32_t i = 0; i < M->Do; ++i) dg[i] = 0.0;
   for (uint32_t i = 0; i < M->geo_cnt; ++i) dg[M->geo_off + i] += dci[i];
@@ -622,16 +653,58 @@ int orc_train_step(const orc_config *cfg, double *theta, double *m, double *v, u
   }
 
   /* S11, S12 per sample */
+  /* F2 accumulators: dL/do, sum_s t_s dL/dp_s, sum_s dL/dY_s per ray */
+  const int want_pose = trace->g_o || trace->tau || trace->dx;
+  double *pose_o = NULL, *pose_d = NULL, *pose_Y = NULL;
+  if (want_pose) {
+    pose_o = calloc(3 * (size_t)R + 1, sizeof(double));
+    pose_d = calloc(3 * (size_t)R + 1, sizeof(double));
+    pose_Y = calloc((size_t)(M.n_sh + 1) * R + 1, sizeof(double));
+    if (!pose_o || !pose_d || !pose_Y) { free(pose_o); free(pose_d); free(pose_Y); goto done; }
+  }
   {
     double *dWm = grad + n_table;
 #pragma omp parallel
     {
       double *dW_local = calloc(M.n_mlp + 1, sizeof(double));
-      double de[ORC_MAX_WIDTH];
+      double de[ORC_MAX_WIDTH], dci[ORC_MAX_WIDTH];
 #pragma omp for schedule(static)
       for (int64_t s = 0; s < (int64_t)S; ++s) {
         const double *a = act + (size_t)M.a_stride * s;
-        mlp_backward(&M, Wm, dW_local, a, dsigma[s], drgb + 3 * s, de);
+        mlp_backward(&M, Wm, dW_local, a, dsigma[s], drgb + 3 * s, de, dci);
+        if (want_pose) {
+          /* dL/dx_c = sum_l N_l sum_corners (d omega / d w_c) (theta[corner] . dL/de_l): w_c = x_c N_l - c0_c */
+          double dxs[3] = {0.0, 0.0, 0.0};
+          for (uint32_t l = 0; l < L; ++l) {
+            const uint32_t *slot = slots + ((size_t)s * L + l) * 8;
+            const float *w = wfr + ((size_t)s * L + l) * 3;
+            for (uint32_t corner = 0; corner < 8; ++corner) {
+              const double *entry = theta + (lv.off[l] + slot[corner]) * F;
+              double dot = 0.0;
+              for (uint32_t f = 0; f < F; ++f) dot += entry[f] * de[l * F + f];
+              for (int c = 0; c < 3; ++c) {
+                double dom = ((corner >> c) & 1u) ? 1.0 : -1.0;
+                for (int c2 = 0; c2 < 3; ++c2)
+                  if (c2 != c) dom *= ((corner >> c2) & 1u) ? (double)w[c2] : 1.0 - (double)w[c2];
+                dxs[c] += (double)lv.res[l] * dom * dot;
+              }
+            }
+          }
+          if (trace->dx) for (int c = 0; c < 3; ++c) trace->dx[3 * (size_t)s + c] = dxs[c];
+          const uint32_t r = s_ray[s];
+          const double inv_extent = (double)(1.0f / cfg->aabb_extent);
+          for (int c = 0; c < 3; ++c) {
+            const double dp = dxs[c] * inv_extent;
+#pragma omp atomic
+            pose_o[3 * (size_t)r + c] += dp;
+#pragma omp atomic
+            pose_d[3 * (size_t)r + c] += (double)s_t[s] * dp;
+          }
+          for (uint32_t j = 0; j < M.n_sh; ++j) {
+#pragma omp atomic
+            pose_Y[(size_t)M.n_sh * r + j] += dci[M.geo_cnt + j];
+          }
+        }
         for (uint32_t l = 0; l < L; ++l) {
           const uint32_t *slot = slots + ((size_t)s * L + l) * 8;
           const float *w = wfr + ((size_t)s * L + l) * 3;
@@ -651,6 +724,22 @@ int orc_train_step(const orc_config *cfg, double *theta, double *m, double *v, u
       for (uint64_t i = 0; i < M.n_mlp; ++i) dWm[i] += dW_local[i];
       free(dW_local);
     }
+  }
+
+  if (want_pose) {
+    for (uint32_t r = 0; r < R; ++r) {
+      const double d[3] = {(double)b->dirs[3 * (size_t)r], (double)b->dirs[3 * (size_t)r + 1], (double)b->dirs[3 * (size_t)r + 2]};
+      const double *gd = pose_d + 3 * (size_t)r;
+      double rot[3];
+      sh_rotation_gradient(cfg->sh_degree, d, pose_Y + (size_t)M.n_sh * r, rot);
+      if (trace->g_o) for (int c = 0; c < 3; ++c) trace->g_o[3 * (size_t)r + c] = pose_o[3 * (size_t)r + c];
+      if (trace->tau) {
+        trace->tau[3 * (size_t)r + 0] = d[1] * gd[2] - d[2] * gd[1] + rot[0];
+        trace->tau[3 * (size_t)r + 1] = d[2] * gd[0] - d[0] * gd[2] + rot[1];
+        trace->tau[3 * (size_t)r + 2] = d[0] * gd[1] - d[1] * gd[0] + rot[2];
+      }
+    }
+    free(pose_o); free(pose_d); free(pose_Y);
   }
 
   /* trace copies before the update */

@@ -22,6 +22,7 @@
  *   S14 occupancy from field              R17
  *   S15 render with transmittance cut     PAPER.md:163; R15
  *   F1  ray-batch sampler over keyframes   PAPER.md:157-159; DESIGN.md "F1"
+ *   F2  pose gradients dL/do, d x dL/dd    PAPER.md:120,130-133 (Eq. 3 over T); DESIGN.md "F2" (row f2)
  *
  * Precision: the INDEX PATH (everything that decides an integer, and the fp32 quantities
  * t, delta, x, w) is a fixed sequence of IEEE binary32 operations (compile with
@@ -91,6 +92,14 @@ typedef struct {
   double   *dsigma, *drgb; /* [S], [S,3]  dL/dsigma_i, dL/dc_i */
   double   *grad;        /* [P]  canonical flat layout: tables then MLP matrices */
   uint8_t  *touched;     /* [n_entries]  1 if the (level,slot) entry was referenced this step */
+  /* Row f2 (L_M is minimised over the poses T as well): per-ray gradients of L with respect to the
+   * ray, through x = (o + t d - aabb_min) / extent into the encoding (S4's trilinear weights) and through Y(d) (S6):
+   *   g_o[r]  = dL/do_r                                         (translation part of the keyframe's se(3) gradient: sum over its rays)
+   *   tau[r]  = d/d(omega) L with d_r <- exp(omega^) d_r at omega = 0  (rotation part: d x dL/dd, tangential, so the value
+   *             of Y off the unit sphere never enters) */
+  double   *g_o;         /* [R,3] */
+  double   *tau;         /* [R,3] */
+  double   *dx;          /* [S,3]  dL/dx_s, x the normalised sample position */
 } orc_trace;
 
 /* S0.  res[L], offset[L+1] (in entries).  Returns 0, or -1 on a bad config. */

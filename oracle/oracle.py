@@ -51,7 +51,7 @@ class OrcTrace(C.Structure):
                 ("s_t", _f32p), ("s_delta", _f32p), ("s_x", _f32p), ("slots", _u32p), ("w", _f32p),
                 ("e", _f64p), ("sigma", _f64p), ("rgb", _f64p), ("C", _f64p), ("D_hat", _f64p),
                 ("O", _f64p), ("dsigma", _f64p), ("drgb", _f64p), ("grad", _f64p),
-                ("touched", _u8p)]
+                ("touched", _u8p), ("g_o", _f64p), ("tau", _f64p), ("dx", _f64p)]
 
 
 _LIBS = {}
@@ -329,7 +329,8 @@ class Oracle:
                       sigma=((cap,), np.float64), rgb=((cap, 3), np.float64),
                       C=((R, 3), np.float64), D_hat=((R,), np.float64), O=((R,), np.float64),
                       dsigma=((cap,), np.float64), drgb=((cap, 3), np.float64),
-                      grad=((P,), np.float64), touched=((self.n_entries,), np.uint8))
+                      grad=((P,), np.float64), touched=((self.n_entries,), np.uint8),
+                      g_o=((R, 3), np.float64), tau=((R, 3), np.float64), dx=((cap, 3), np.float64))
         tr = OrcTrace()
         out = {}
         for name in trace:

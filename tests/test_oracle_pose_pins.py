@@ -1,0 +1,109 @@
+"""Pins of the oracle's pose gradients (row f2; Eq. 3 is minimised over the poses T too): central finite
+differences of the oracle's own loss under a translation of a ray's origin and a rotation of its direction, plus two
+structural cases.  CPU only."""
+from dataclasses import replace
+
+import numpy as np
+import pytest
+
+from oracle import oracle as orc
+from workloads import configs
+
+
+def tiny(sh_degree=3, seed=0, R=10, K=16):
+    w = configs.config1()
+    fc = replace(w.field, sh_degree=sh_degree, max_rays=R, max_candidates=K)
+    b = w.batches[0]
+    b = replace(b, origins=b.origins[:R].copy(), dirs=b.dirs[:R].copy(), rgb=b.rgb[:R].copy(), depth=b.depth[:R].copy(),
+                depth_var=b.depth_var[:R].copy(), n_candidates=K)
+    n_table, n_mlp = orc.param_count(fc)
+    theta = configs.init_params(seed, n_table, orc.mlp_shapes(fc)).astype(np.float64)
+    theta[:n_table] *= 3e3                       # tables that matter: the field varies across cells
+    theta[n_table:] *= 1.5
+    return fc, b, theta
+
+
+def loss(fc, theta, b, lam=0.3):
+    O = orc.Oracle(fc, theta.copy())
+    return O.train_step(b, lam, apply_adam=False)[0]["loss"]
+
+
+def rot(axis, ang):
+    K = np.zeros((3, 3))
+    a = np.eye(3)[axis]
+    K[0, 1], K[0, 2], K[1, 0], K[1, 2], K[2, 0], K[2, 1] = -a[2], a[1], a[2], -a[0], -a[1], a[0]
+    return np.eye(3) + np.sin(ang) * K + (1 - np.cos(ang)) * K @ K
+
+
+def fd_check(name, analytic, perturb, h, n, tol):
+    """analytic[i]: claimed derivative; perturb(i, s) -> batch perturbed by s*h along coordinate i."""
+    ok = skipped = 0
+    worst = 0.0
+    scale = np.abs(analytic).max()
+    for i in range(n):
+        lp, l0, lm = perturb(i, +1), perturb(i, 0), perturb(i, -1)
+        fd = (lp - lm) / (2 * h)
+        curv = abs(lp - 2 * l0 + lm) / h          # a kink of the piecewise-trilinear field inside the stencil
+        if curv > 0.02 * scale:
+            skipped += 1
+            continue
+        worst = max(worst, abs(fd - analytic[i]) / scale)
+        ok += 1
+    assert ok >= 0.5 * n, (name, ok, skipped)
+    assert worst <= tol, (name, worst)
+    return ok, skipped
+
+
+@pytest.mark.parametrize("sh_degree", [1, 3, 4])
+def test_translation_and_rotation_gradients_by_finite_differences(sh_degree):
+    fc, b, theta = tiny(sh_degree)
+    O = orc.Oracle(fc, theta.copy())
+    _, tr = O.train_step(b, 0.3, apply_adam=False, trace=("g_o", "tau"))
+    R = b.n_rays
+    h = 2.0 ** -13      # small against the finest cell (extent 5 / 32): few stencils straddle a kink of the trilinear field
+
+    def shift(i, s):
+        r, c = divmod(i, 3)
+        o = b.origins.copy()
+        o[r, c] += np.float32(s * h)
+        return loss(fc, theta, replace(b, origins=o))
+
+    def turn(i, s):
+        r, k = divmod(i, 3)
+        d = b.dirs.astype(np.float64).copy()
+        d[r] = rot(k, s * h) @ d[r]
+        return loss(fc, theta, replace(b, dirs=d.astype(np.float32)))
+
+    fd_check("g_o", tr["g_o"].reshape(-1), shift, h, 3 * R, 1e-2)
+    fd_check("tau", tr["tau"].reshape(-1), turn, h, 3 * R, 1e-2)
+    assert np.abs(tr["g_o"]).max() > 0 and np.abs(tr["tau"]).max() > 0
+
+
+def test_constant_tables_leave_only_the_direction_encoding():
+    """With every table entry equal the encoding does not depend on x: dL/do = 0 exactly and dL/dx = 0; the rotation
+    gradient is then the SH path alone and vanishes too when Y is the constant Y_00 (sh_degree = 1)."""
+    for n, expect_tau in ((1, False), (3, True)):
+        fc, b, theta = tiny(n)
+        n_table, _ = orc.param_count(fc)
+        theta[:n_table] = 0.37
+        O = orc.Oracle(fc, theta.copy())
+        _, tr = O.train_step(b, 0.3, apply_adam=False, trace=("g_o", "tau", "dx"))
+        assert np.abs(tr["dx"]).max() <= 1e-12 and np.abs(tr["g_o"]).max() <= 1e-12
+        assert (np.abs(tr["tau"]).max() > 1e-9) == expect_tau
+
+
+def test_translation_gradient_is_the_sum_of_the_sample_gradients():
+    """dL/do_r = (1/extent) sum_s dL/dx_s over the ray's samples; a whole-batch translation is the sum over rays."""
+    fc, b, theta = tiny(3)
+    O = orc.Oracle(fc, theta.copy())
+    _, tr = O.train_step(b, 0.3, apply_adam=False, trace=("g_o", "dx", "s_ray"))
+    acc = np.zeros_like(tr["g_o"])
+    np.add.at(acc, tr["s_ray"], tr["dx"] * float(np.float32(1.0) / np.float32(fc.aabb_extent)))   # S0's fp32 inv_extent
+    assert np.abs(acc - tr["g_o"]).max() <= 1e-12 * max(1.0, np.abs(acc).max())
+    h = 2.0 ** -13
+    for c in range(3):
+        o = b.origins.copy()
+        lp = loss(fc, theta, replace(b, origins=(o + np.float32(h) * np.eye(3, dtype=np.float32)[c])))
+        lm = loss(fc, theta, replace(b, origins=(o - np.float32(h) * np.eye(3, dtype=np.float32)[c])))
+        fd, an = (lp - lm) / (2 * h), tr["g_o"][:, c].sum()
+        assert abs(fd - an) <= 0.03 * np.abs(tr["g_o"]).sum(0).max() + 1e-9, (c, fd, an)
