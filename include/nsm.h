@@ -180,13 +180,26 @@ nsm_status nsm_sample_batch(nsm_field *f, uint32_t n_rays, uint32_t draw, float 
 nsm_status nsm_train_step_sampled(nsm_field *f, uint32_t n_rays, float t_min, float t_max, uint32_t n_candidates,
                                   float lambda_d, nsm_step_stats *host_stats);
 
+/* ---- Row f2: pose gradients (L_M(T, Theta) is minimised over the poses T too). ----
+ * With NSM_OPT_POSE_GRADIENTS set, after nsm_backward / a training step:
+ *   d_g_o [R,3]  dL/do_r                                    (a keyframe's translation gradient is the sum over its rays)
+ *   d_tau [R,3]  d/d(omega) L for d_r <- exp(omega^) d_r    (= d_r x dL/dd_r; its rotation gradient likewise)
+ * through the sample positions (S4's trilinear weights) and the direction encoding (S6), with the parameters the
+ * step's forward pass used.  After nsm_train_step_sampled, nsm_keyframe_pose_gradients returns those sums per
+ * keyframe: d_out [n_keyframes, 6] = (translation | rotation), in the world frame, rotation about the camera centre. */
+nsm_status nsm_pose_gradients(nsm_field *f, float *d_g_o, float *d_tau);
+nsm_status nsm_keyframe_pose_gradients(nsm_field *f, float *d_out);
+
 /* Options.
  * NSM_OPT_BATCH_READY (default 0).  With 0 the library reads a batch strictly in the order of the field's
  * stream.  With 1 the caller declares that the device buffers of every batch handed to nsm_train_step are
  * complete when the call is made (e.g. a pre-staged keyframe store) and stay unmodified until the step has
  * run: the library may then march the batch (S1-S3 read origins/dirs only) on an internal stream BESIDE the
  * previous step's table update, ahead of work queued earlier on the field's stream.  Results are identical. */
-typedef enum { NSM_OPT_BATCH_READY = 0 } nsm_option;
+/* NSM_OPT_POSE_GRADIENTS (default 0).  With 1 every training step / nsm_backward also computes the gradients of
+ * the loss with respect to the rays (row f2, below); costs two extra kernels per step and 19 floats per sample
+ * of workspace. */
+typedef enum { NSM_OPT_BATCH_READY = 0, NSM_OPT_POSE_GRADIENTS = 1 } nsm_option;
 nsm_status nsm_set_option(nsm_field *f, nsm_option opt, uint32_t value);
 
 /* S1-S12 only: forward + backward, gradients left in place for nsm_debug_last_step; and S13

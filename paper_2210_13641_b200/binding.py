@@ -16,7 +16,7 @@ LIB_PATH = os.path.join(_HERE, "libnsm.so")
 NSM_OK, NSM_ERR_INVALID_ARG, NSM_ERR_OOM, NSM_ERR_CUDA, NSM_ERR_CAPACITY, NSM_ERR_UNIMPLEMENTED = range(6)
 NSM_MLP_FP32, NSM_MLP_FP16, NSM_MLP_BF16 = 0, 1, 2
 NSM_OCC_FULL, NSM_OCC_SET, NSM_OCC_FROM_FIELD = 0, 1, 2
-NSM_OPT_BATCH_READY = 0
+NSM_OPT_BATCH_READY, NSM_OPT_POSE_GRADIENTS = 0, 1
 
 DEBUG_ITEMS = dict(counts=(0, np.uint32), offsets=(1, np.uint32), s_ray=(2, np.uint32), s_k=(3, np.uint32),
                    s_t=(4, np.float32), s_delta=(5, np.float32), s_x=(6, np.float32), slots=(7, np.uint32),
@@ -29,6 +29,7 @@ EXPORTS = ["nsm_create_field", "nsm_destroy_field", "nsm_update_occupancy", "nsm
            "nsm_render", "nsm_render_host", "nsm_param_count", "nsm_get_params", "nsm_set_params",
            "nsm_get_level_table", "nsm_debug_last_step", "nsm_total_samples", "nsm_profile", "nsm_set_option", "nsm_debug_timeline",
            "nsm_add_keyframe", "nsm_keyframe_count", "nsm_sample_batch", "nsm_train_step_sampled",
+           "nsm_pose_gradients", "nsm_keyframe_pose_gradients",
            "nsm_profile_read", "nsm_launch_count", "nsm_mlp_path",
            "nsm_last_error", "nsm_version"]
 
@@ -99,6 +100,8 @@ def load_library():
         L.nsm_total_samples.argtypes = [vp, u64p]
         L.nsm_profile.argtypes = [vp, C.c_int]
         L.nsm_set_option.argtypes = [vp, C.c_int, C.c_uint32]
+        L.nsm_pose_gradients.argtypes = [vp, vp, vp]
+        L.nsm_keyframe_pose_gradients.argtypes = [vp, vp]
         L.nsm_add_keyframe.argtypes = [vp, C.POINTER(NsmKeyframeInfo), vp, vp, vp, u32p]
         L.nsm_keyframe_count.argtypes = [vp, u32p]
         L.nsm_sample_batch.argtypes = [vp, C.c_uint32, C.c_uint32, vp, vp, vp, vp, vp]
@@ -333,6 +336,19 @@ class Field:
         _check(self.lib.nsm_train_step_sampled(self.h, int(n_rays), float(t_min), float(t_max), int(n_candidates),
                                                float(lambda_d), C.byref(st) if want_stats else None))
         return _stats(st) if want_stats else None
+
+    # ---- row f2: pose gradients
+    def nsm_pose_gradients(self, n_rays):
+        """(dL/do [R,3], rotation gradient d x dL/dd [R,3]) of the last step (needs NSM_OPT_POSE_GRADIENTS)."""
+        go = torch.empty((int(n_rays), 3), device=self.device)
+        tau = torch.empty((int(n_rays), 3), device=self.device)
+        _check(self.lib.nsm_pose_gradients(self.h, go.data_ptr(), tau.data_ptr()))
+        return go, tau
+
+    def nsm_keyframe_pose_gradients(self):
+        out = torch.empty((self.nsm_keyframe_count(), 6), device=self.device)
+        _check(self.lib.nsm_keyframe_pose_gradients(self.h, out.data_ptr()))
+        return out
 
     def nsm_backward(self, batch, lambda_d, want_stats=True):
         return self._step(self.lib.nsm_backward, batch, lambda_d, want_stats)

@@ -637,6 +637,10 @@ __global__ void __launch_bounds__(BWD_THREADS, 2) mlp_backward_tc_kernel(MlpShap
       for (int j = 0; j < 16; ++j) dg[j] = 0.f;
 #pragma unroll
       for (int j = 0; j < 15; ++j) dg[1 + j] = dci[j];   // geo slice (1, 15), see mlp_tc_supported()
+      if (ws.dY && valid) {                              // row f2: dL/dY, the 16 SH slots of the colour input
+#pragma unroll
+        for (int j = 0; j < 16; ++j) ws.dY[(size_t)j * ws.cap + s] = dci[15 + j] * inv_scale;
+      }
       // sigma = exp(clamp(g0, -15, 15)): the clamp is active iff sigma sits on a bound
       if (valid && sig > 3.0590232e-07f * 1.0001f && sig < 3269017.4f * 0.9999f) dg[0] += dsig * sig * scale;
       emit16<T, false>(dg, bufY, nullptr, row, 0, true);

@@ -49,7 +49,7 @@ uint32_t g_pdl_mask = [] {
 int g_cur_kernel = 0;
 
 static const char *kKernelNames[K_COUNT] = {"march", "encode", "mlp_fwd", "composite",
-                                            "mlp_bwd", "scatter", "adam_table", "adam_mlp", "occupancy", "debug", "sample"};
+                                            "mlp_bwd", "scatter", "adam_table", "adam_mlp", "occupancy", "debug", "sample", "pose"};
 
 // Optional per-kernel CUDA-event timing (bench.py's roofline leg).  When enabled every launch is
 // bracketed by two events on the field's stream and each step ends with a synchronise.
@@ -110,6 +110,10 @@ struct nsm_field {
   // F1: the keyframe store (library-owned device copies) and its device-side directory
   std::vector<KeyframeDev> kf_host;
   KeyframeDev *kf_dev = nullptr;
+  // row f2: pose gradients (NSM_OPT_POSE_GRADIENTS)
+  bool pose_grads = false, last_sampled = false;
+  float *pose_go = nullptr, *pose_tau = nullptr, *kf_grad = nullptr;   // [max_rays,3] x2, [NSM_MAX_KEYFRAMES,6]
+  uint32_t *ray_kf = nullptr;                                           // [max_rays] keyframe of every sampled ray
   bool stats_pending = false;
   bool join_pending = false;   // ev_side (recorded behind the MLP Adam) has not been waited for on the main stream yet
   unsigned long long *timeline_base = nullptr;   // NSM_TIMELINE=1: ring of 64 steps x [2][K_COUNT] globaltimer stamps
@@ -270,7 +274,7 @@ void enqueue_forward(nsm_field *f, const nsm_ray_batch *b, uint32_t R, bool jitt
     if (sample_draw >= 0)
       RUN_ON(f, K_SAMPLE, f->side, launch_sample_batch(f->kf_dev, (uint32_t)f->kf_host.size(), f->cfg.seed, (uint32_t)sample_draw, R,
                                                        (float *)b->origins, (float *)b->dirs, (float *)b->rgb, (float *)b->depth,
-                                                       (float *)b->depth_var, f->side));
+                                                       (float *)b->depth_var, f->pose_grads ? f->ray_kf : nullptr, f->side));
     RUN_ON(f, K_MARCH, f->side, launch_march(mp, f->occ_full ? nullptr : f->fp.occ_bits, b->origins, b->dirs, f->ws, train ? 1 : 0, f->side, dirs_copy));
     cudaEventRecord(f->ev_side, f->side);
     cudaStreamWaitEvent(f->stream, f->ev_side, 0);
@@ -280,7 +284,7 @@ void enqueue_forward(nsm_field *f, const nsm_ray_batch *b, uint32_t R, bool jitt
     if (sample_draw >= 0)
       RUN(f, K_SAMPLE, launch_sample_batch(f->kf_dev, (uint32_t)f->kf_host.size(), f->cfg.seed, (uint32_t)sample_draw, R,
                                            (float *)b->origins, (float *)b->dirs, (float *)b->rgb, (float *)b->depth,
-                                           (float *)b->depth_var, f->stream));
+                                           (float *)b->depth_var, f->pose_grads ? f->ray_kf : nullptr, f->stream));
     RUN(f, K_MARCH, launch_march(mp, f->occ_full ? nullptr : f->fp.occ_bits, b->origins, b->dirs, f->ws, train ? 1 : 0, f->stream, dirs_copy));
   }
   const int bf16 = f->cfg.mlp_precision == NSM_MLP_BF16;
@@ -342,6 +346,13 @@ nsm_status enqueue_backward(nsm_field *f, const nsm_ray_batch *b, float lambda_d
   else
     RUN(f, K_MLP_BWD, launch_mlp_backward_simt(f->ms, f->fp.mlp_theta, f->fp.mlp_grad, dirs_copy ? dirs_copy : b->dirs,
                                                f->ws, d_S, f->n_sms, f->stream));
+  if (f->pose_grads) {   // row f2: needs dL/de, dL/dY of this step and the PRE-update theta: between the MLP backward and Adam
+    f->last_sampled = sample_draw >= 0;
+    if (f->last_sampled) CUDA_TRY(cudaMemsetAsync(f->kf_grad, 0, sizeof(float) * 6 * f->kf_host.size(), f->stream));
+    RUN(f, K_POSE, launch_pose_gradients(f->lv, f->fp.theta, f->ws, d_S, R, dirs_copy ? dirs_copy : b->dirs, 1.0f / f->cfg.aabb_extent,
+                                         f->cfg.sh_degree, f->pose_go, f->pose_tau, f->last_sampled ? f->ray_kf : nullptr, f->kf_grad,
+                                         f->n_sms, f->stream));
+  }
   // train step: the scatter is issued by enqueue_adam, level group by level group, each followed by its Adam
   f->scatter_pending = defer_scatter;
   if (!defer_scatter) RUN(f, K_SCATTER, launch_scatter(f->lv, f->fp.grad, f->ws, d_S, 0, f->lv.n_levels, f->n_sms, f->stream));
@@ -546,6 +557,7 @@ nsm_status nsm_create_field(const nsm_field_config *cfg, void *cuda_stream, nsm_
   A(f->alloc(&ws.sigma, cap)); A(f->alloc(&ws.rgb, 3 * cap)); A(f->alloc(&ws.T_excl, cap));
   A(f->alloc(&ws.dsigma, cap)); A(f->alloc(&ws.drgb, 3 * cap)); A(f->alloc(&ws.de, ms.LF * cap));
   A(f->alloc(&f->kf_dev, NSM_MAX_KEYFRAMES));
+  ws.dY = ws.dx = nullptr;
   ws.timeline = nullptr;
   {
     const char *tl = std::getenv("NSM_TIMELINE");
@@ -839,7 +851,7 @@ nsm_status nsm_sample_batch(nsm_field *f, uint32_t n_rays, uint32_t draw, float 
   if (n_rays == 0) return fail(NSM_ERR_INVALID_ARG, "n_rays is 0");
   leave_fast_path(f);
   RUN(f, K_SAMPLE, launch_sample_batch(f->kf_dev, (uint32_t)f->kf_host.size(), f->cfg.seed, draw, n_rays, d_origins, d_dirs, d_rgb,
-                                       d_depth, d_depth_var, f->stream));
+                                       d_depth, d_depth_var, nullptr, f->stream));
   CUDA_TRY(cudaGetLastError());
   return NSM_OK;
 }
@@ -859,10 +871,43 @@ nsm_status nsm_train_step_sampled(nsm_field *f, uint32_t n_rays, float t_min, fl
   return train_step_impl(f, &b, lambda_d, host_stats, true, nullptr, (int64_t)(f->step + 1));
 }
 
+// ---- row f2: pose gradients --------------------------------------------------------------------------------
+nsm_status nsm_pose_gradients(nsm_field *f, float *d_g_o, float *d_tau) {
+  if (!f || !d_g_o || !d_tau) return fail(NSM_ERR_INVALID_ARG, "NULL argument");
+  if (!f->pose_grads || f->last_R == 0 || f->last_was_render)
+    return fail(NSM_ERR_INVALID_ARG, "no pose gradients: set NSM_OPT_POSE_GRADIENTS and run a training step / nsm_backward first");
+  leave_fast_path(f);
+  CUDA_TRY(cudaMemcpyAsync(d_g_o, f->pose_go, sizeof(float) * 3 * f->last_R, cudaMemcpyDeviceToDevice, f->stream));
+  CUDA_TRY(cudaMemcpyAsync(d_tau, f->pose_tau, sizeof(float) * 3 * f->last_R, cudaMemcpyDeviceToDevice, f->stream));
+  return NSM_OK;
+}
+
+nsm_status nsm_keyframe_pose_gradients(nsm_field *f, float *d_out) {
+  if (!f || !d_out) return fail(NSM_ERR_INVALID_ARG, "NULL argument");
+  if (!f->pose_grads || !f->last_sampled || f->last_was_render)
+    return fail(NSM_ERR_INVALID_ARG, "no keyframe gradients: set NSM_OPT_POSE_GRADIENTS and run nsm_train_step_sampled first");
+  leave_fast_path(f);
+  CUDA_TRY(cudaMemcpyAsync(d_out, f->kf_grad, sizeof(float) * 6 * f->kf_host.size(), cudaMemcpyDeviceToDevice, f->stream));
+  return NSM_OK;
+}
+
 nsm_status nsm_set_option(nsm_field *f, nsm_option opt, uint32_t value) {
   if (!f) return fail(NSM_ERR_INVALID_ARG, "field is NULL");
   switch (opt) {
     case NSM_OPT_BATCH_READY: f->batch_ready = value != 0; leave_fast_path(f); return NSM_OK;
+    case NSM_OPT_POSE_GRADIENTS: {
+      leave_fast_path(f);
+      if (value && !f->ws.dY) {   // workspace of row f2, allocated on first use
+        cudaError_t e = cudaSuccess;
+        auto A = [&](cudaError_t r) { if (e == cudaSuccess) e = r; };
+        A(f->alloc(&f->ws.dY, 16 * f->ws.cap)); A(f->alloc(&f->ws.dx, 3 * f->ws.cap));
+        A(f->alloc(&f->pose_go, 3 * (size_t)f->cfg.max_rays)); A(f->alloc(&f->pose_tau, 3 * (size_t)f->cfg.max_rays));
+        A(f->alloc(&f->kf_grad, 6 * NSM_MAX_KEYFRAMES)); A(f->alloc(&f->ray_kf, f->cfg.max_rays));
+        if (e != cudaSuccess) { cudaGetLastError(); return fail(NSM_ERR_OOM, "pose-gradient workspace: %s", cudaGetErrorString(e)); }
+      }
+      f->pose_grads = value != 0;
+      return NSM_OK;
+    }
   }
   return fail(NSM_ERR_INVALID_ARG, "unknown option %d", (int)opt);
 }

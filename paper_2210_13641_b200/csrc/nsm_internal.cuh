@@ -58,6 +58,9 @@ struct Workspace {
   float *dsigma;         // [cap]
   float *drgb;           // [cap,3]
   float *de;             // [LF][cap]
+  // row f2 (pose gradients; allocated when NSM_OPT_POSE_GRADIENTS is set, else NULL and nothing below is written)
+  float *dY;             // [16][cap] dL/dY of every sample (the SH slots of the colour MLP's input gradient)
+  float *dx;             // [3][cap]  dL/dx of every sample
   // loss accumulators: [0]=sum rgb, [1]=sum depth, [2]=S of the step (doubles); device
   double *loss_acc;
   unsigned long long *total_samples;  // running sum of S over training steps (device)
@@ -72,7 +75,7 @@ struct Workspace {
 // Kernel classes, for launch counting and the optional per-kernel event timing.
 enum KernelId {
   K_MARCH = 0, K_ENCODE, K_MLP_FWD, K_COMPOSITE, K_MLP_BWD, K_SCATTER,
-  K_ADAM_TABLE, K_ADAM_MLP, K_OCC, K_DEBUG, K_SAMPLE, K_COUNT
+  K_ADAM_TABLE, K_ADAM_MLP, K_OCC, K_DEBUG, K_SAMPLE, K_POSE, K_COUNT
 };
 
 // DESIGN.md S1.1 -- the counter-based hash behind the jitter stream (S1) and the batch sampler (F1):
@@ -297,8 +300,14 @@ int launch_adam_mlp(const FieldParams &fp, float lr, float beta1, float beta2, f
 int launch_adam_mlp_pack(const MlpShape &ms, int bf16, const FieldParams &fp, const Workspace &ws, const AdamConst &c,
                          uint32_t n_ctas, const uint32_t *d_S, cudaStream_t st);
 // F1: n_rays rays drawn uniformly over (keyframe, pixel) for draw number `draw`; outputs are a ray batch
+// ray_kf (optional): [n_rays] keyframe index of every ray
 int launch_sample_batch(const KeyframeDev *kfs, uint32_t n_kf, uint64_t seed, uint32_t draw, uint32_t n_rays, float *origins,
-                        float *dirs, float *rgb, float *depth, float *depth_var, cudaStream_t st);
+                        float *dirs, float *rgb, float *depth, float *depth_var, uint32_t *ray_kf, cudaStream_t st);
+// f2: per-ray dL/do and rotation gradient from ws.de / ws.dY (after the MLP backward, before Adam); ray_kf + kf_grad
+// (optional): accumulate the per-keyframe 6-vectors [n_kf][6] (kf_grad must be zeroed by the caller)
+int launch_pose_gradients(const LevelTable &lv, const float *theta, const Workspace &ws, const uint32_t *d_S, uint32_t R,
+                          const float *dirs, float inv_extent, uint32_t sh_degree, float *g_o, float *tau, const uint32_t *ray_kf,
+                          float *kf_grad, int n_sms, cudaStream_t st);
 int launch_occ_cells(uint32_t G, uint64_t first_cell, uint64_t n_cells, const Workspace &ws,
                      uint32_t *d_S, cudaStream_t st);
 int launch_occ_threshold(uint32_t G, uint64_t first_cell, uint64_t n_cells, const float *sigma,

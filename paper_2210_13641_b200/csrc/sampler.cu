@@ -13,7 +13,8 @@ namespace {
 __global__ void __launch_bounds__(256) sample_batch_kernel(const KeyframeDev *__restrict__ kfs, uint32_t n_kf, uint64_t seed,
                                                            uint32_t draw, uint32_t n_rays, float *__restrict__ origins,
                                                            float *__restrict__ dirs, float *__restrict__ rgb,
-                                                           float *__restrict__ depth, float *__restrict__ depth_var) {
+                                                           float *__restrict__ depth, float *__restrict__ depth_var,
+                                                           uint32_t *__restrict__ ray_kf) {
   const uint32_t r = blockIdx.x * blockDim.x + threadIdx.x;
   if (r >= n_rays) return;
   const uint32_t hp = nsm_hash_prefix(seed, draw, r);
@@ -37,12 +38,13 @@ __global__ void __launch_bounds__(256) sample_batch_kernel(const KeyframeDev *__
   }
   depth[r] = __fmul_rn(__ldg(k.depth + pix), n);
   depth_var[r] = __fmul_rn(__ldg(k.var + pix), n2);
+  if (ray_kf) ray_kf[r] = kf;
 }
 
 }  // namespace
 
 int launch_sample_batch(const KeyframeDev *kfs, uint32_t n_kf, uint64_t seed, uint32_t draw, uint32_t n_rays, float *origins,
-                        float *dirs, float *rgb, float *depth, float *depth_var, cudaStream_t st) {
-  sample_batch_kernel<<<(n_rays + 255) / 256, 256, 0, st>>>(kfs, n_kf, seed, draw, n_rays, origins, dirs, rgb, depth, depth_var);
+                        float *dirs, float *rgb, float *depth, float *depth_var, uint32_t *ray_kf, cudaStream_t st) {
+  sample_batch_kernel<<<(n_rays + 255) / 256, 256, 0, st>>>(kfs, n_kf, seed, draw, n_rays, origins, dirs, rgb, depth, depth_var, ray_kf);
   return 1;
 }

@@ -519,3 +519,68 @@ def test_config5_full_frame_render_on_sampled_rays(nsm):
     assert np.isfinite(rgb).all() and rgb.min() >= -1e-6 and rgb.max() <= 1 + 1e-5
     assert opa.min() >= -1e-6 and opa.max() <= 1 + 1e-5 and dep.min() >= 0 and dep.max() <= view.t_max * (1 + 1e-5)
     f.close()
+
+
+# ---------------------------------------------------------------------------- row f2: pose gradients
+
+def _check_pose(nsm, f, O, b, lam, tol):
+    f.nsm_backward(nsm.DeviceBatch(b), lam)
+    go, tau = (t.cpu().numpy().astype(np.float64) for t in f.nsm_pose_gradients(b.n_rays))
+    _, tr = O.train_step(b, lam, apply_adam=False, trace=("g_o", "tau"))
+    for name, got, ref in (("g_o", go, tr["g_o"]), ("tau", tau, tr["tau"])):
+        assert np.abs(ref).max() > 0, name
+        assert np.linalg.norm(got - ref) <= tol * np.linalg.norm(ref), (name, np.linalg.norm(got - ref) / np.linalg.norm(ref))
+        err = np.abs(got - ref) / np.abs(ref).max()
+        if f.nsm_mlp_path() == "simt_fp32":
+            assert err.max() <= tol, (name, err.max())
+        else:   # 16-bit MLP operands: a ReLU mask flipped against float64 moves single rays by a whole term (as in P4)
+            assert np.mean(err <= tol) >= 0.999 and err.max() <= 10 * tol, (name, np.mean(err <= tol), err.max())
+    return go, tau, tr
+
+
+def test_pose_gradients_fp32_path(nsm):
+    """dL/do and d x dL/dd of every ray against the oracle (config 1: fp32 CUDA-core MLPs, SH degree 2; variant with SH
+    degree 4 and a background colour)."""
+    for sh_degree, bg in ((2, (0.0, 0.0, 0.0)), (4, (0.2, 0.4, 0.1))):
+        w = configs.config1(variant_b=True)
+        w = replace(w, field=replace(w.field, sh_degree=sh_degree, bg=bg))
+        f, O, _ = make_pair(nsm, w, seed=13, table_scale=0.3, mlp_scale=1.5)
+        f.nsm_set_option(nsm.NSM_OPT_POSE_GRADIENTS, 1)
+        _check_pose(nsm, f, O, w.batches[0], 0.4, 1e-3)
+        f.close()
+
+
+def test_pose_gradients_tensor_core_path_and_keyframe_sums(nsm):
+    """The 16-bit tensor-core configuration (SH degree 4), through nsm_train_step_sampled: per-ray gradients against the
+    oracle on the oracle-drawn batch, and the per-keyframe se(3) sums against numpy sums of the oracle's per-ray values."""
+    w = configs.config3(R=2048, K=128, n_keyframes=3, n_batches=1, width=120, height=68)
+    f, O, _ = make_pair(nsm, w, seed=14, table_scale=0.05)
+    assert f.nsm_mlp_path().startswith("tcgen05")
+    tol = tol_for(w.field, f.nsm_mlp_path())
+    f.nsm_set_option(nsm.NSM_OPT_POSE_GRADIENTS, 1)
+    _check_pose(nsm, f, O, w.batches[0], w.lambda_d, tol)
+    store = [w.extra["keyframes"].store_frame(i) for i in range(3)]
+    for kf in store:
+        f.nsm_add_keyframe(kf)
+    f.nsm_train_step_sampled(2048, 0.05, 10.5, 128, w.lambda_d)
+    ref = orc.sample_batch(store, w.field.seed, 1, 2048)
+    b = configs.RayBatch(ref["origins"], ref["dirs"], ref["rgb"], ref["depth"], ref["depth_var"], 0.05, 10.5, 128)
+    _, tr = O.train_step(b, w.lambda_d, apply_adam=False, trace=("g_o", "tau"))
+    go, tau = (t.cpu().numpy().astype(np.float64) for t in f.nsm_pose_gradients(2048))
+    assert np.linalg.norm(go - tr["g_o"]) <= tol * np.linalg.norm(tr["g_o"])
+    assert np.linalg.norm(tau - tr["tau"]) <= tol * np.linalg.norm(tr["tau"])
+    kg = f.nsm_keyframe_pose_gradients().cpu().numpy().astype(np.float64)
+    want = np.zeros((3, 6))
+    np.add.at(want[:, :3], ref["kf"], tr["g_o"])
+    np.add.at(want[:, 3:], ref["kf"], tr["tau"])
+    # sums over ~700 rays of signed per-ray values: compare against the size of what is summed
+    size = np.zeros((3, 6))
+    np.add.at(size[:, :3], ref["kf"], np.abs(tr["g_o"]))
+    np.add.at(size[:, 3:], ref["kf"], np.abs(tr["tau"]))
+    assert np.all(np.abs(kg - want) <= tol * size + 1e-12), (kg, want)
+    # without the option the getters refuse
+    f2, _, _ = make_pair(nsm, w, seed=14, table_scale=0.05)
+    f2.nsm_backward(nsm.DeviceBatch(w.batches[0]), w.lambda_d)
+    with pytest.raises(nsm.NsmError):
+        f2.nsm_pose_gradients(2048)
+    f.close(); f2.close()
