@@ -910,3 +910,36 @@ void orc_sample_batch(const orc_keyframe *kfs, uint32_t n_kf, uint64_t seed, uin
     if (pix_out) pix_out[r] = pix;
   }
 }
+
+/* ---- F2, the update (header comment of orc_pose_step) ---------------------------------------------------------- */
+void orc_pose_step(double *R, double *t, double *m, double *v, uint32_t *count, const double *g, double lr_t, double lr_r,
+                   double beta1, double beta2, double eps) {
+  const uint32_t k = *count + 1;
+  const double bc1 = 1.0 - pow(beta1, (double)k), bc2 = 1.0 - pow(beta2, (double)k);
+  double delta[6];
+  for (int i = 0; i < 6; ++i) {
+    m[i] = beta1 * m[i] + (1.0 - beta1) * g[i];
+    v[i] = beta2 * v[i] + (1.0 - beta2) * g[i] * g[i];
+    delta[i] = (i < 3 ? lr_t : lr_r) * (m[i] / bc1) / (sqrt(v[i] / bc2) + eps);
+  }
+  for (int i = 0; i < 3; ++i) t[i] -= delta[i];
+  /* E = exp(-[w]x), w = delta_omega: E = I - sin(a)/a [w]x + (1 - cos a)/a^2 [w]x^2, a = |w| */
+  const double w[3] = {delta[3], delta[4], delta[5]};
+  const double a2 = w[0] * w[0] + w[1] * w[1] + w[2] * w[2], a = sqrt(a2);
+  const double A = a > 1e-12 ? sin(a) / a : 1.0, B = a > 1e-12 ? (1.0 - cos(a)) / a2 : 0.5;
+  const double K[9] = {0.0, -w[2], w[1], w[2], 0.0, -w[0], -w[1], w[0], 0.0};
+  double K2[9], E[9], Rn[9];
+  for (int i = 0; i < 3; ++i)
+    for (int j = 0; j < 3; ++j) {
+      K2[3 * i + j] = 0.0;
+      for (int q = 0; q < 3; ++q) K2[3 * i + j] += K[3 * i + q] * K[3 * q + j];
+    }
+  for (int i = 0; i < 9; ++i) E[i] = ((i % 4 == 0) ? 1.0 : 0.0) - A * K[i] + B * K2[i];
+  for (int i = 0; i < 3; ++i)
+    for (int j = 0; j < 3; ++j) {
+      Rn[3 * i + j] = 0.0;
+      for (int q = 0; q < 3; ++q) Rn[3 * i + j] += E[3 * i + q] * R[3 * q + j];
+    }
+  for (int i = 0; i < 9; ++i) R[i] = Rn[i];
+  *count = k;
+}

@@ -177,6 +177,16 @@ void orc_sample_batch(const orc_keyframe *kfs, uint32_t n_kf, uint64_t seed, uin
                       uint32_t *kf_out, uint32_t *pix_out, float *origins, float *dirs, float *rgb, float *depth,
                       float *depth_var);
 
+/* F2, the update: one Adam step on a keyframe's se(3) gradient g = (dL/dt | dL/d(omega)) (translation of the camera
+ * centre; rotation about it, world frame, as delivered by the per-ray sums of orc_trace.g_o / tau):
+ *   m <- b1 m + (1-b1) g,  v <- b2 v + (1-b2) g^2,  delta = lr * (m / (1-b1^k)) / (sqrt(v / (1-b2^k)) + eps)   per component,
+ *   lr = lr_t for the three translation components and lr_r for the three rotation components, k = *count + 1
+ *   (the number of updates this keyframe has received: a keyframe without rays in the batch is not updated at all);
+ *   t <- t - delta_t;   R <- exp(-[delta_omega]x) R   (Rodrigues' formula; R rotates camera to world).
+ * R [9] row-major, t [3], m [6], v [6] are updated in place. */
+void orc_pose_step(double *R, double *t, double *m, double *v, uint32_t *count, const double *g, double lr_t, double lr_r,
+                   double beta1, double beta2, double eps);
+
 /* Threads the library will use (1 unless built with -fopenmp). */
 int orc_num_threads(void);
 

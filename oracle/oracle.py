@@ -92,6 +92,9 @@ def lib(omp=False):
         L.orc_sample_batch.argtypes = [C.POINTER(OrcKeyframe), C.c_uint32, C.c_uint64, C.c_uint32, C.c_uint32,
                                        _u32p, _u32p, _f32p, _f32p, _f32p, _f32p, _f32p]
         L.orc_sample_batch.restype = None
+        L.orc_pose_step.argtypes = [_f64p, _f64p, _f64p, _f64p, _u32p, _f64p, C.c_double, C.c_double, C.c_double,
+                                    C.c_double, C.c_double]
+        L.orc_pose_step.restype = None
         L.orc_num_threads.restype = C.c_int
         _LIBS[key] = L
     return _LIBS[key]
@@ -281,6 +284,17 @@ def sample_batch(keyframes, seed, draw, n_rays):
                            _p(out["origins"], _f32p), _p(out["dirs"], _f32p), _p(out["rgb"], _f32p),
                            _p(out["depth"], _f32p), _p(out["depth_var"], _f32p))
     return out
+
+
+def pose_step(R, t, m, v, count, g, lr_t, lr_r, beta1=0.9, beta2=0.99, eps=1e-15):
+    """F2 update of one keyframe, in place on float64 arrays R (3,3), t (3,), m (6,), v (6,); returns the new count."""
+    for a in (R, t, m, v):
+        assert a.dtype == np.float64 and a.flags["C_CONTIGUOUS"]
+    cnt = np.array([count], np.uint32)
+    g = np.ascontiguousarray(g, np.float64)
+    lib().orc_pose_step(_p(R, _f64p), _p(t, _f64p), _p(m, _f64p), _p(v, _f64p), _p(cnt, _u32p), _p(g, _f64p),
+                        float(lr_t), float(lr_r), float(beta1), float(beta2), float(eps))
+    return int(cnt[0])
 
 
 class Oracle:

@@ -107,3 +107,68 @@ def test_translation_gradient_is_the_sum_of_the_sample_gradients():
         lm = loss(fc, theta, replace(b, origins=(o - np.float32(h) * np.eye(3, dtype=np.float32)[c])))
         fd, an = (lp - lm) / (2 * h), tr["g_o"][:, c].sum()
         assert abs(fd - an) <= 0.03 * np.abs(tr["g_o"]).sum(0).max() + 1e-9, (c, fd, an)
+
+
+def test_pose_step_exponential_map_and_adam():
+    """The update R <- exp(-[w]x) R against scipy's matrix exponential, orthonormality, the first Adam step's closed form
+    (delta = lr sign(g)), torch.optim.Adam on the 6-vector over several steps, and the world-frame convention: the
+    update by w turns every world direction d = R d_cam by exp(-[w]x), which is what tau = dL/d(omega) is the gradient of."""
+    import scipy.linalg
+    import torch
+    rng = np.random.default_rng(5)
+    R0 = rot(0, 0.4) @ rot(1, -0.9) @ rot(2, 0.2)
+    t0 = rng.normal(size=3)
+    g = rng.normal(size=6) * np.array([1, 1e-3, 10, 1e-2, 1, 5])
+    R, t, m, v = R0.copy(), t0.copy(), np.zeros(6), np.zeros(6)
+    cnt = orc.pose_step(R, t, m, v, 0, g, 1e-3, 2e-3)
+    assert cnt == 1
+    assert np.abs(t - (t0 - 1e-3 * np.sign(g[:3]))).max() <= 1e-12          # Adam step 1: -lr sign(g)
+    w = 2e-3 * np.sign(g[3:])
+    K = np.array([[0, -w[2], w[1]], [w[2], 0, -w[0]], [-w[1], w[0], 0]])
+    assert np.abs(R - scipy.linalg.expm(-K) @ R0).max() <= 1e-13
+    assert np.abs(R @ R.T - np.eye(3)).max() <= 1e-13 and abs(np.linalg.det(R) - 1) <= 1e-13
+    # several steps against torch.optim.Adam on the raw 6-vector with per-group learning rates
+    p_t = torch.zeros(3, dtype=torch.float64, requires_grad=True)
+    p_r = torch.zeros(3, dtype=torch.float64, requires_grad=True)
+    opt = torch.optim.Adam([dict(params=[p_t], lr=1e-3), dict(params=[p_r], lr=2e-3)], betas=(0.9, 0.99), eps=1e-15)
+    R, t, m, v, cnt = R0.copy(), t0.copy(), np.zeros(6), np.zeros(6), 0
+    Racc = R0.copy()
+    for k in range(6):
+        gk = rng.normal(size=6)
+        prev_r = p_r.detach().numpy().copy()
+        p_t.grad, p_r.grad = torch.tensor(gk[:3]), torch.tensor(gk[3:])
+        opt.step()
+        cnt = orc.pose_step(R, t, m, v, cnt, gk, 1e-3, 2e-3)
+        assert np.abs(t - (t0 + p_t.detach().numpy())).max() <= 1e-12
+        dw = -(p_r.detach().numpy() - prev_r)                                # this step's delta_omega
+        Kk = np.array([[0, -dw[2], dw[1]], [dw[2], 0, -dw[0]], [-dw[1], dw[0], 0]])
+        Racc = scipy.linalg.expm(-Kk) @ Racc
+        assert np.abs(R - Racc).max() <= 1e-12
+    # tiny and zero rotations stay finite and exact to first order
+    R, t, m, v = R0.copy(), t0.copy(), np.zeros(6), np.zeros(6)
+    orc.pose_step(R, t, m, v, 0, np.array([0, 0, 0, 1e-30, 0, 0.0]), 1e-3, 1e-20)
+    assert np.isfinite(R).all() and np.abs(R - R0).max() <= 1e-15
+
+
+def test_pose_step_descends_the_loss():
+    """Moving one keyframe's rays by a small se(3) step against (g_o sums | tau sums) lowers the oracle's loss by the
+    first-order amount -|g|^2 step (the sums ARE the keyframe gradient, in the convention the update uses)."""
+    fc, b, theta = tiny(3)
+    O = orc.Oracle(fc, theta.copy())
+    st, tr = O.train_step(b, 0.3, apply_adam=False, trace=("g_o", "tau"))
+    G = np.concatenate([tr["g_o"].sum(0), tr["tau"].sum(0)])
+    # all rays as one rigid body rotating about a common centre c: o <- c + E (o - c), d <- E d, then o <- o - eps g_t
+    c = b.origins.astype(np.float64).mean(0)
+    # gradient of that motion: translation = sum g_o; rotation = sum (tau + (o - c) x g_o)
+    G[3:] += np.cross(b.origins.astype(np.float64) - c, tr["g_o"]).sum(0)
+    eps = 2.0 ** -12 / np.abs(G).max()
+    w = eps * G[3:]
+    K = np.array([[0, -w[2], w[1]], [w[2], 0, -w[0]], [-w[1], w[0], 0]])
+    import scipy.linalg
+    E = scipy.linalg.expm(-K)
+    o2 = c + (b.origins.astype(np.float64) - c) @ E.T - eps * G[:3]
+    d2 = b.dirs.astype(np.float64) @ E.T
+    l2 = loss(fc, theta, replace(b, origins=o2.astype(np.float32), dirs=d2.astype(np.float32)))
+    predicted = -eps * (G ** 2).sum()
+    assert l2 < st["loss"]
+    assert abs((l2 - st["loss"]) - predicted) <= 0.15 * abs(predicted), (l2 - st["loss"], predicted)
