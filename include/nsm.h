@@ -189,6 +189,12 @@ nsm_status nsm_train_step_sampled(nsm_field *f, uint32_t n_rays, float t_min, fl
  * keyframe: d_out [n_keyframes, 6] = (translation | rotation), in the world frame, rotation about the camera centre. */
 nsm_status nsm_pose_gradients(nsm_field *f, float *d_g_o, float *d_tau);
 nsm_status nsm_keyframe_pose_gradients(nsm_field *f, float *d_out);
+/* The update: one Adam step (the field's beta1, beta2, eps; bias correction by the number of updates the keyframe has
+ * received) on the 6-vector of every keyframe that had rays in the last sampled batch, then t <- t - delta_t and
+ * R <- exp(-[delta_omega]x) R in the keyframe store.  Consumes the gradients of the last nsm_train_step_sampled. */
+nsm_status nsm_apply_pose_step(nsm_field *f, float lr_translation, float lr_rotation);
+/* Current pose of a keyframe (HOST outputs R [9] row-major camera-to-world, t [3]); synchronises. */
+nsm_status nsm_get_keyframe_pose(nsm_field *f, uint32_t index, float *h_R, float *h_t);
 
 /* Options.
  * NSM_OPT_BATCH_READY (default 0).  With 0 the library reads a batch strictly in the order of the field's

@@ -29,7 +29,7 @@ EXPORTS = ["nsm_create_field", "nsm_destroy_field", "nsm_update_occupancy", "nsm
            "nsm_render", "nsm_render_host", "nsm_param_count", "nsm_get_params", "nsm_set_params",
            "nsm_get_level_table", "nsm_debug_last_step", "nsm_total_samples", "nsm_profile", "nsm_set_option", "nsm_debug_timeline",
            "nsm_add_keyframe", "nsm_keyframe_count", "nsm_sample_batch", "nsm_train_step_sampled",
-           "nsm_pose_gradients", "nsm_keyframe_pose_gradients",
+           "nsm_pose_gradients", "nsm_keyframe_pose_gradients", "nsm_apply_pose_step", "nsm_get_keyframe_pose",
            "nsm_profile_read", "nsm_launch_count", "nsm_mlp_path",
            "nsm_last_error", "nsm_version"]
 
@@ -102,6 +102,8 @@ def load_library():
         L.nsm_set_option.argtypes = [vp, C.c_int, C.c_uint32]
         L.nsm_pose_gradients.argtypes = [vp, vp, vp]
         L.nsm_keyframe_pose_gradients.argtypes = [vp, vp]
+        L.nsm_apply_pose_step.argtypes = [vp, C.c_float, C.c_float]
+        L.nsm_get_keyframe_pose.argtypes = [vp, C.c_uint32, C.POINTER(C.c_float), C.POINTER(C.c_float)]
         L.nsm_add_keyframe.argtypes = [vp, C.POINTER(NsmKeyframeInfo), vp, vp, vp, u32p]
         L.nsm_keyframe_count.argtypes = [vp, u32p]
         L.nsm_sample_batch.argtypes = [vp, C.c_uint32, C.c_uint32, vp, vp, vp, vp, vp]
@@ -349,6 +351,14 @@ class Field:
         out = torch.empty((self.nsm_keyframe_count(), 6), device=self.device)
         _check(self.lib.nsm_keyframe_pose_gradients(self.h, out.data_ptr()))
         return out
+
+    def nsm_apply_pose_step(self, lr_translation, lr_rotation):
+        _check(self.lib.nsm_apply_pose_step(self.h, float(lr_translation), float(lr_rotation)))
+
+    def nsm_get_keyframe_pose(self, index):
+        R, t = (C.c_float * 9)(), (C.c_float * 3)()
+        _check(self.lib.nsm_get_keyframe_pose(self.h, int(index), R, t))
+        return np.array(R, np.float32).reshape(3, 3), np.array(t, np.float32)
 
     def nsm_backward(self, batch, lambda_d, want_stats=True):
         return self._step(self.lib.nsm_backward, batch, lambda_d, want_stats)

@@ -112,7 +112,9 @@ struct nsm_field {
   KeyframeDev *kf_dev = nullptr;
   // row f2: pose gradients (NSM_OPT_POSE_GRADIENTS)
   bool pose_grads = false, last_sampled = false;
-  float *pose_go = nullptr, *pose_tau = nullptr, *kf_grad = nullptr;   // [max_rays,3] x2, [NSM_MAX_KEYFRAMES,6]
+  float *pose_go = nullptr, *pose_tau = nullptr, *kf_grad = nullptr;   // [max_rays,3] x2, [NSM_MAX_KEYFRAMES,NSM_KF_GRAD_STRIDE]
+  float *kf_pose_m = nullptr, *kf_pose_v = nullptr;                    // Adam moments of the keyframe poses [NSM_MAX_KEYFRAMES,6]
+  uint32_t *kf_pose_cnt = nullptr;                                     // updates received per keyframe
   uint32_t *ray_kf = nullptr;                                           // [max_rays] keyframe of every sampled ray
   bool stats_pending = false;
   bool join_pending = false;   // ev_side (recorded behind the MLP Adam) has not been waited for on the main stream yet
@@ -348,7 +350,7 @@ nsm_status enqueue_backward(nsm_field *f, const nsm_ray_batch *b, float lambda_d
                                                f->ws, d_S, f->n_sms, f->stream));
   if (f->pose_grads) {   // row f2: needs dL/de, dL/dY of this step and the PRE-update theta: between the MLP backward and Adam
     f->last_sampled = sample_draw >= 0;
-    if (f->last_sampled) CUDA_TRY(cudaMemsetAsync(f->kf_grad, 0, sizeof(float) * 6 * f->kf_host.size(), f->stream));
+    if (f->last_sampled) CUDA_TRY(cudaMemsetAsync(f->kf_grad, 0, sizeof(float) * NSM_KF_GRAD_STRIDE * f->kf_host.size(), f->stream));
     RUN(f, K_POSE, launch_pose_gradients(f->lv, f->fp.theta, f->ws, d_S, R, dirs_copy ? dirs_copy : b->dirs, 1.0f / f->cfg.aabb_extent,
                                          f->cfg.sh_degree, f->pose_go, f->pose_tau, f->last_sampled ? f->ray_kf : nullptr, f->kf_grad,
                                          f->n_sms, f->stream));
@@ -887,7 +889,33 @@ nsm_status nsm_keyframe_pose_gradients(nsm_field *f, float *d_out) {
   if (!f->pose_grads || !f->last_sampled || f->last_was_render)
     return fail(NSM_ERR_INVALID_ARG, "no keyframe gradients: set NSM_OPT_POSE_GRADIENTS and run nsm_train_step_sampled first");
   leave_fast_path(f);
-  CUDA_TRY(cudaMemcpyAsync(d_out, f->kf_grad, sizeof(float) * 6 * f->kf_host.size(), cudaMemcpyDeviceToDevice, f->stream));
+  CUDA_TRY(cudaMemcpy2DAsync(d_out, sizeof(float) * 6, f->kf_grad, sizeof(float) * NSM_KF_GRAD_STRIDE, sizeof(float) * 6,
+                             f->kf_host.size(), cudaMemcpyDeviceToDevice, f->stream));
+  return NSM_OK;
+}
+
+nsm_status nsm_apply_pose_step(nsm_field *f, float lr_translation, float lr_rotation) {
+  if (!f) return fail(NSM_ERR_INVALID_ARG, "field is NULL");
+  if (!f->pose_grads || !f->last_sampled || f->last_was_render)
+    return fail(NSM_ERR_INVALID_ARG, "no keyframe gradients: set NSM_OPT_POSE_GRADIENTS and run nsm_train_step_sampled first");
+  if (!(lr_translation >= 0.f) || !(lr_rotation >= 0.f)) return fail(NSM_ERR_INVALID_ARG, "learning rates must be >= 0");
+  leave_fast_path(f);
+  RUN(f, K_POSE, launch_pose_step(f->kf_dev, (uint32_t)f->kf_host.size(), f->kf_grad, f->kf_pose_m, f->kf_pose_v, f->kf_pose_cnt,
+                                  lr_translation, lr_rotation, f->cfg.beta1, f->cfg.beta2, f->cfg.eps, f->stream));
+  f->last_sampled = false;   // the gradients are consumed
+  CUDA_TRY(cudaGetLastError());
+  return NSM_OK;
+}
+
+nsm_status nsm_get_keyframe_pose(nsm_field *f, uint32_t index, float *h_R, float *h_t) {
+  if (!f || !h_R || !h_t) return fail(NSM_ERR_INVALID_ARG, "NULL argument");
+  if (index >= f->kf_host.size()) return fail(NSM_ERR_INVALID_ARG, "keyframe index %u out of range", index);
+  leave_fast_path(f);
+  KeyframeDev k;
+  CUDA_TRY(cudaMemcpyAsync(&k, f->kf_dev + index, sizeof k, cudaMemcpyDeviceToHost, f->stream));
+  CUDA_TRY(cudaStreamSynchronize(f->stream));
+  for (int i = 0; i < 9; ++i) h_R[i] = k.R[i];
+  for (int i = 0; i < 3; ++i) h_t[i] = k.t[i];
   return NSM_OK;
 }
 
@@ -902,7 +930,9 @@ nsm_status nsm_set_option(nsm_field *f, nsm_option opt, uint32_t value) {
         auto A = [&](cudaError_t r) { if (e == cudaSuccess) e = r; };
         A(f->alloc(&f->ws.dY, 16 * f->ws.cap)); A(f->alloc(&f->ws.dx, 3 * f->ws.cap));
         A(f->alloc(&f->pose_go, 3 * (size_t)f->cfg.max_rays)); A(f->alloc(&f->pose_tau, 3 * (size_t)f->cfg.max_rays));
-        A(f->alloc(&f->kf_grad, 6 * NSM_MAX_KEYFRAMES)); A(f->alloc(&f->ray_kf, f->cfg.max_rays));
+        A(f->alloc(&f->kf_grad, NSM_KF_GRAD_STRIDE * NSM_MAX_KEYFRAMES)); A(f->alloc(&f->ray_kf, f->cfg.max_rays));
+        A(f->alloc(&f->kf_pose_m, 6 * NSM_MAX_KEYFRAMES)); A(f->alloc(&f->kf_pose_v, 6 * NSM_MAX_KEYFRAMES));
+        A(f->alloc(&f->kf_pose_cnt, NSM_MAX_KEYFRAMES));
         if (e != cudaSuccess) { cudaGetLastError(); return fail(NSM_ERR_OOM, "pose-gradient workspace: %s", cudaGetErrorString(e)); }
       }
       f->pose_grads = value != 0;

@@ -106,6 +106,7 @@ struct KeyframeDev {
   const float *rgb, *depth, *var;
 };
 #define NSM_MAX_KEYFRAMES 1024
+#define NSM_KF_GRAD_STRIDE 8   /* per keyframe: dL/dt (3), dL/d(omega) (3), number of rays in the batch, pad */
 
 // Debug timeline: when ws.timeline is set, thread 0 of every block stamps the kernel class's earliest start
 // and latest end with %globaltimer.  Unlike CUDA events between launches this does not disturb PDL or the
@@ -304,10 +305,13 @@ int launch_adam_mlp_pack(const MlpShape &ms, int bf16, const FieldParams &fp, co
 int launch_sample_batch(const KeyframeDev *kfs, uint32_t n_kf, uint64_t seed, uint32_t draw, uint32_t n_rays, float *origins,
                         float *dirs, float *rgb, float *depth, float *depth_var, uint32_t *ray_kf, cudaStream_t st);
 // f2: per-ray dL/do and rotation gradient from ws.de / ws.dY (after the MLP backward, before Adam); ray_kf + kf_grad
-// (optional): accumulate the per-keyframe 6-vectors [n_kf][6] (kf_grad must be zeroed by the caller)
+// (optional): accumulate the per-keyframe vectors [n_kf][NSM_KF_GRAD_STRIDE] (kf_grad must be zeroed by the caller)
 int launch_pose_gradients(const LevelTable &lv, const float *theta, const Workspace &ws, const uint32_t *d_S, uint32_t R,
                           const float *dirs, float inv_extent, uint32_t sh_degree, float *g_o, float *tau, const uint32_t *ray_kf,
                           float *kf_grad, int n_sms, cudaStream_t st);
+// f2, the update: Adam + exponential map on the keyframes that received rays (kf_grad: [n_kf][NSM_KF_GRAD_STRIDE])
+int launch_pose_step(KeyframeDev *kfs, uint32_t n_kf, const float *kf_grad, float *pm, float *pv, uint32_t *pcnt, float lr_t,
+                     float lr_r, float beta1, float beta2, float eps, cudaStream_t st);
 int launch_occ_cells(uint32_t G, uint64_t first_cell, uint64_t n_cells, const Workspace &ws,
                      uint32_t *d_S, cudaStream_t st);
 int launch_occ_threshold(uint32_t G, uint64_t first_cell, uint64_t n_cells, const float *sigma,

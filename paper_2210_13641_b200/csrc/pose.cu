@@ -123,15 +123,74 @@ __global__ void __launch_bounds__(256) pose_ray_kernel(Workspace ws, uint32_t R,
     const float t0 = y * g[2] - z * g[1], t1 = z * g[0] - x * g[2], t2 = x * g[1] - y * g[0];
     g_o[3 * (size_t)r] = so[0]; g_o[3 * (size_t)r + 1] = so[1]; g_o[3 * (size_t)r + 2] = so[2];
     tau[3 * (size_t)r] = t0; tau[3 * (size_t)r + 1] = t1; tau[3 * (size_t)r + 2] = t2;
-    if (ray_kf) {   // per-keyframe se(3) gradient (translation | rotation)
-      float *kg = kf_grad + 6 * (size_t)ray_kf[r];
+    if (ray_kf) {   // per-keyframe se(3) gradient (translation | rotation | number of rays | pad)
+      float *kg = kf_grad + NSM_KF_GRAD_STRIDE * (size_t)ray_kf[r];
       atomicAdd(kg, so[0]); atomicAdd(kg + 1, so[1]); atomicAdd(kg + 2, so[2]);
       atomicAdd(kg + 3, t0); atomicAdd(kg + 4, t1); atomicAdd(kg + 5, t2);
+      atomicAdd(kg + 6, 1.0f);
     }
   }
 }
 
+// F2, the update: Adam on every keyframe's 6-vector that received rays in this batch, then t <- t - delta_t and
+// R <- exp(-[delta_omega]x) R (Rodrigues), written into the device-side keyframe directory.  One thread per keyframe;
+// the few transcendental operations run in double.
+__global__ void pose_step_kernel(KeyframeDev *__restrict__ kfs, uint32_t n_kf, const float *__restrict__ kf_grad,
+                                 float *__restrict__ pm, float *__restrict__ pv, uint32_t *__restrict__ pcnt, float lr_t, float lr_r,
+                                 float beta1, float beta2, float eps) {
+  const uint32_t k = blockIdx.x * blockDim.x + threadIdx.x;
+  if (k >= n_kf) return;
+  const float *g = kf_grad + NSM_KF_GRAD_STRIDE * (size_t)k;
+  if (!(g[6] > 0.f)) return;                       // no ray of this keyframe in the batch: untouched
+  const uint32_t cnt = pcnt[k] + 1;
+  const double bc1 = 1.0 - pow((double)beta1, (double)cnt), bc2 = 1.0 - pow((double)beta2, (double)cnt);
+  double delta[6];
+#pragma unroll
+  for (int i = 0; i < 6; ++i) {
+    const float m = beta1 * pm[6 * k + i] + (1.f - beta1) * g[i];
+    const float v = beta2 * pv[6 * k + i] + (1.f - beta2) * g[i] * g[i];
+    pm[6 * k + i] = m; pv[6 * k + i] = v;
+    delta[i] = (double)(i < 3 ? lr_t : lr_r) * ((double)m / bc1) / (sqrt((double)v / bc2) + (double)eps);
+  }
+  KeyframeDev kf = kfs[k];
+#pragma unroll
+  for (int i = 0; i < 3; ++i) kf.t[i] = (float)((double)kf.t[i] - delta[i]);
+  const double w0 = delta[3], w1 = delta[4], w2 = delta[5];
+  const double a2 = w0 * w0 + w1 * w1 + w2 * w2, a = sqrt(a2);
+  const double A = a > 1e-12 ? sin(a) / a : 1.0, B = a > 1e-12 ? (1.0 - cos(a)) / a2 : 0.5;
+  const double K[9] = {0.0, -w2, w1, w2, 0.0, -w0, -w1, w0, 0.0};
+  double E[9], Rn[9];
+#pragma unroll
+  for (int i = 0; i < 3; ++i)
+#pragma unroll
+    for (int j = 0; j < 3; ++j) {
+      double k2 = 0.0;
+#pragma unroll
+      for (int q = 0; q < 3; ++q) k2 += K[3 * i + q] * K[3 * q + j];
+      E[3 * i + j] = (i == j ? 1.0 : 0.0) - A * K[3 * i + j] + B * k2;
+    }
+#pragma unroll
+  for (int i = 0; i < 3; ++i)
+#pragma unroll
+    for (int j = 0; j < 3; ++j) {
+      double acc = 0.0;
+#pragma unroll
+      for (int q = 0; q < 3; ++q) acc += E[3 * i + q] * (double)kf.R[3 * q + j];
+      Rn[3 * i + j] = acc;
+    }
+#pragma unroll
+  for (int i = 0; i < 9; ++i) kf.R[i] = (float)Rn[i];
+  kfs[k] = kf;
+  pcnt[k] = cnt;
+}
+
 }  // namespace
+
+int launch_pose_step(KeyframeDev *kfs, uint32_t n_kf, const float *kf_grad, float *pm, float *pv, uint32_t *pcnt, float lr_t,
+                     float lr_r, float beta1, float beta2, float eps, cudaStream_t st) {
+  pose_step_kernel<<<(n_kf + 63) / 64, 64, 0, st>>>(kfs, n_kf, kf_grad, pm, pv, pcnt, lr_t, lr_r, beta1, beta2, eps);
+  return 1;
+}
 
 int launch_pose_gradients(const LevelTable &lv, const float *theta, const Workspace &ws, const uint32_t *d_S, uint32_t R,
                           const float *dirs, float inv_extent, uint32_t sh_degree, float *g_o, float *tau, const uint32_t *ray_kf,

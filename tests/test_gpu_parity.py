@@ -584,3 +584,37 @@ def test_pose_gradients_tensor_core_path_and_keyframe_sums(nsm):
     with pytest.raises(nsm.NsmError):
         f2.nsm_pose_gradients(2048)
     f.close(); f2.close()
+
+
+def test_pose_update_step_against_the_oracle(nsm):
+    """nsm_apply_pose_step vs orc_pose_step fed with the SAME keyframe gradients (the kernel's own arithmetic: Adam with a
+    per-keyframe update count, Rodrigues' formula), over several sampled steps; a keyframe without rays in the batch keeps
+    its pose and its Adam state."""
+    w = configs.config3(R=1024, K=128, n_keyframes=3, n_batches=1, width=120, height=68)
+    f, _, _ = make_pair(nsm, w, seed=15, table_scale=0.05)
+    f.nsm_set_option(nsm.NSM_OPT_POSE_GRADIENTS, 1)
+    store = [w.extra["keyframes"].store_frame(i) for i in range(3)]
+    for kf in store:
+        f.nsm_add_keyframe(kf)
+    R = [np.asarray(k["R"], np.float32).astype(np.float64).copy() for k in store]
+    t = [np.asarray(k["t"], np.float32).astype(np.float64).copy() for k in store]
+    m, v, cnt = [np.zeros(6) for _ in store], [np.zeros(6) for _ in store], [0, 0, 0]
+    lr_t, lr_r = 2e-3, 1e-3
+    fc = w.field
+    for step, n_rays in enumerate((1024, 1, 512, 1024, 2)):
+        f.nsm_train_step_sampled(n_rays, 0.05, 10.5, 128, w.lambda_d, want_stats=False)
+        kg = f.nsm_keyframe_pose_gradients().cpu().numpy().astype(np.float64)
+        drawn = orc.sample_batch(store, fc.seed, step + 1, n_rays)["kf"]     # which keyframes have rays (indices only)
+        f.nsm_apply_pose_step(lr_t, lr_r)
+        for k in range(3):
+            if (drawn == k).any():
+                cnt[k] = orc.pose_step(R[k], t[k], m[k], v[k], cnt[k], kg[k], lr_t, lr_r, float(np.float32(fc.beta1)),
+                                       float(np.float32(fc.beta2)), float(np.float32(fc.eps)))
+            else:
+                assert not kg[k].any()
+            Rg, tg = f.nsm_get_keyframe_pose(k)
+            assert np.abs(Rg - R[k]).max() <= 2e-6 and np.abs(tg - t[k]).max() <= 2e-6 * max(1.0, np.abs(t[k]).max()), (step, k)
+            assert np.abs(Rg.astype(np.float64) @ Rg.T.astype(np.float64) - np.eye(3)).max() <= 1e-5
+    with pytest.raises(nsm.NsmError):
+        f.nsm_apply_pose_step(lr_t, lr_r)          # the gradients were consumed
+    f.close()
