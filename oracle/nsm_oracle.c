@@ -829,6 +829,41 @@ int orc_occupancy_from_field(const orc_config *cfg, const double *theta, uint8_t
   return 0;
 }
 
+/* F4: decayed running maximum with a strided partial refresh (header comment of orc_occupancy_decay_update). */
+static double cell_sigma(const orc_config *cfg, const orc_levels *lv, const orc_mlp *M, const double *theta, uint64_t cell) {
+  const uint32_t G = cfg->occ_res;
+  const uint32_t gx = (uint32_t)(cell % G), gy = (uint32_t)((cell / G) % G), gz = (uint32_t)(cell / ((uint64_t)G * G));
+  const double *Wm = theta + lv->off[lv->L] * lv->F;
+  double e[ORC_MAX_WIDTH], hd[ORC_MAX_WIDTH];
+  float x[3] = {((float)gx + 0.5f) / (float)G, ((float)gy + 0.5f) / (float)G, ((float)gz + 0.5f) / (float)G};
+  encode_point(lv, theta, x, NULL, NULL, e);
+  linear(Wm + M->o_d1, M->Hd, M->LF, e, hd, 1);
+  double g0 = 0.0;
+  for (uint32_t i = 0; i < M->Hd; ++i) g0 += Wm[M->o_d2 + i] * hd[i];
+  double g0c = g0 < -15.0 ? -15.0 : (g0 > 15.0 ? 15.0 : g0);
+  return exp(g0c);
+}
+
+int orc_occupancy_decay_update(const orc_config *cfg, const double *theta, double *grid, uint32_t update_index,
+                               uint32_t n_sub, double decay, uint8_t *bits_out, double *visited_sigma) {
+  orc_levels lv;
+  orc_mlp M;
+  if (levels_init(cfg, &lv) != 0 || mlp_init(cfg, &M) != 0 || n_sub == 0) return -1;
+  const uint64_t cells = (uint64_t)cfg->occ_res * cfg->occ_res * cfg->occ_res;
+  memset(bits_out, 0, (cells + 7) / 8);
+  for (uint64_t c = 0; c < cells; ++c) {
+    grid[c] *= decay;
+    if (visited_sigma) visited_sigma[c] = -1.0;
+    if (c % n_sub == update_index % n_sub) {
+      const double s = cell_sigma(cfg, &lv, &M, theta, c);
+      if (s > grid[c]) grid[c] = s;
+      if (visited_sigma) visited_sigma[c] = s;
+    }
+    if (grid[c] > (double)cfg->occ_sigma_threshold) bits_out[c >> 3] |= (uint8_t)(1u << (c & 7));
+  }
+  return 0;
+}
+
 /* ------------------------------------------------------------------ S15: render ----------- */
 
 int orc_render(const orc_config *cfg, const double *theta, const uint8_t *bits, const orc_batch *b,

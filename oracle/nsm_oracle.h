@@ -23,6 +23,7 @@
  *   S15 render with transmittance cut     PAPER.md:163; R15
  *   F1  ray-batch sampler over keyframes   PAPER.md:157-159; DESIGN.md "F1"
  *   F2  pose gradients dL/do, d x dL/dd    PAPER.md:120,130-133 (Eq. 3 over T); DESIGN.md "F2" (row f2)
+ *   F4  decayed partial occupancy refresh  paper silent -> [17]; DESIGN.md "F4" (row f4)
  *
  * Precision: the INDEX PATH (everything that decides an integer, and the fp32 quantities
  * t, delta, x, w) is a fixed sequence of IEEE binary32 operations (compile with
@@ -148,6 +149,16 @@ void orc_adam(uint64_t n, double *theta, double *m, double *v, const double *g, 
 /* S14 FROM_FIELD: bits_out has G^3/8 bytes.  sigma_out (may be NULL) gets G^3 densities. */
 int orc_occupancy_from_field(const orc_config *cfg, const double *theta, uint8_t *bits_out,
                              double *sigma_out);
+
+/* F4 (the paper is silent, [17] keeps a decayed running maximum of the density and refreshes only
+ * part of the grid per update): `grid` [G^3] is the running density, `update_index` the number of decay updates done so far.
+ *   every cell:                                   grid[c] <- decay * grid[c]
+ *   cells with c mod n_sub == update_index mod n_sub:   grid[c] <- max(grid[c], sigma(centre of c))      (1/n_sub of the grid)
+ *   bit[c] = grid[c] > occ_sigma_threshold
+ * so n_sub consecutive updates visit every cell exactly once, and n_sub = 1, decay = 0 is S14's FROM_FIELD.  A FROM_FIELD
+ * refresh sets grid[c] = sigma(c).  visited_sigma (may be NULL) gets sigma for the visited cells and -1 elsewhere. */
+int orc_occupancy_decay_update(const orc_config *cfg, const double *theta, double *grid, uint32_t update_index,
+                               uint32_t n_sub, double decay, uint8_t *bits_out, double *visited_sigma);
 
 /* S15. */
 int orc_render(const orc_config *cfg, const double *theta, const uint8_t *bits, const orc_batch *b,

@@ -92,6 +92,8 @@ def lib(omp=False):
         L.orc_sample_batch.argtypes = [C.POINTER(OrcKeyframe), C.c_uint32, C.c_uint64, C.c_uint32, C.c_uint32,
                                        _u32p, _u32p, _f32p, _f32p, _f32p, _f32p, _f32p]
         L.orc_sample_batch.restype = None
+        L.orc_occupancy_decay_update.argtypes = [C.POINTER(OrcConfig), _f64p, _f64p, C.c_uint32, C.c_uint32, C.c_double,
+                                                 _u8p, _f64p]
         L.orc_pose_step.argtypes = [_f64p, _f64p, _f64p, _f64p, _u32p, _f64p, C.c_double, C.c_double, C.c_double,
                                     C.c_double, C.c_double]
         L.orc_pose_step.restype = None
@@ -327,7 +329,23 @@ class Oracle:
                                              _p(bits, _u8p), _p(sig, _f64p)) != 0:
             raise ValueError("orc_occupancy_from_field failed")
         self.bits = bits
+        if sig is not None:
+            self.occ_grid, self.occ_updates = sig.copy(), 0     # F4: a full refresh seeds the running grid
         return (bits, sig) if want_sigma else bits
+
+    def occupancy_decay_update(self, n_sub, decay, want_sigma=False):
+        """F4: decayed running-maximum grid with a strided 1/n_sub refresh; keeps self.occ_grid and self.occ_updates."""
+        G = self.fc.occ_res
+        if getattr(self, "occ_grid", None) is None:
+            self.occ_grid, self.occ_updates = np.zeros(G ** 3, np.float64), 0
+        bits = np.zeros((G ** 3 + 7) // 8, np.uint8)
+        vis = np.zeros(G ** 3, np.float64) if want_sigma else None
+        if self.lib.orc_occupancy_decay_update(C.byref(self.cfg), _p(self.theta, _f64p), _p(self.occ_grid, _f64p),
+                                               self.occ_updates, int(n_sub), float(decay), _p(bits, _u8p), _p(vis, _f64p)) != 0:
+            raise ValueError("orc_occupancy_decay_update failed")
+        self.occ_updates += 1
+        self.bits = bits
+        return (bits, vis) if want_sigma else bits
 
     def train_step(self, batch, lambda_d, jitter=True, apply_adam=True, trace=(), ):
         """trace: iterable of OrcTrace field names to return.  Returns (stats dict, trace dict)."""
