@@ -153,6 +153,16 @@ nsm_status nsm_train_step_host(nsm_field *f, const nsm_ray_batch *host_batch, fl
  * start of ~0 / end of 0 means "did not run".  Synchronises.  Costs a few atomics per block: not for timing runs. */
 nsm_status nsm_debug_timeline(nsm_field *f, uint64_t *h_out, uint64_t capacity_words, uint32_t *n_kernels);
 
+/* ---- Row f4: decayed partial occupancy refresh (the paper is silent; [17] keeps a decayed running maximum of the
+ * density and refreshes part of the grid per update).  The library keeps a running density per cell, seeded by
+ * nsm_update_occupancy(NSM_OCC_FROM_FIELD).  One call:  every cell  grid <- decay * grid;  the cells
+ * c = (k mod n_subsets) + j * n_subsets (k = number of decay updates since the last full refresh)
+ * grid <- max(grid, sigma(cell centre));  bit = grid > occ_sigma_threshold.  n_subsets consecutive calls visit every
+ * cell exactly once; (n_subsets = 1, decay = 0) equals FROM_FIELD.  Costs G^3 / n_subsets field evaluations. */
+nsm_status nsm_update_occupancy_decay(nsm_field *f, uint32_t n_subsets, float decay);
+/* The running density grid [G^3] (DEVICE output), for inspection and parity. */
+nsm_status nsm_get_occupancy_grid(nsm_field *f, float *d_grid);
+
 /* ---- Row F1: keyframe store and ray-batch sampler (the mapping thread optimises over all
  * keyframes received so far, each with its pose, image, depth map and the depth's marginal variance). ----
  * A keyframe is a pinhole view: pixel (u, v) looks along the camera-frame direction ((u-cx)/fx, (v-cy)/fy, 1);

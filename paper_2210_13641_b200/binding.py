@@ -30,6 +30,7 @@ EXPORTS = ["nsm_create_field", "nsm_destroy_field", "nsm_update_occupancy", "nsm
            "nsm_get_level_table", "nsm_debug_last_step", "nsm_total_samples", "nsm_profile", "nsm_set_option", "nsm_debug_timeline",
            "nsm_add_keyframe", "nsm_keyframe_count", "nsm_sample_batch", "nsm_train_step_sampled",
            "nsm_pose_gradients", "nsm_keyframe_pose_gradients", "nsm_apply_pose_step", "nsm_get_keyframe_pose",
+           "nsm_update_occupancy_decay", "nsm_get_occupancy_grid",
            "nsm_profile_read", "nsm_launch_count", "nsm_mlp_path",
            "nsm_last_error", "nsm_version"]
 
@@ -102,6 +103,8 @@ def load_library():
         L.nsm_set_option.argtypes = [vp, C.c_int, C.c_uint32]
         L.nsm_pose_gradients.argtypes = [vp, vp, vp]
         L.nsm_keyframe_pose_gradients.argtypes = [vp, vp]
+        L.nsm_update_occupancy_decay.argtypes = [vp, C.c_uint32, C.c_float]
+        L.nsm_get_occupancy_grid.argtypes = [vp, vp]
         L.nsm_apply_pose_step.argtypes = [vp, C.c_float, C.c_float]
         L.nsm_get_keyframe_pose.argtypes = [vp, C.c_uint32, C.POINTER(C.c_float), C.POINTER(C.c_float)]
         L.nsm_add_keyframe.argtypes = [vp, C.POINTER(NsmKeyframeInfo), vp, vp, vp, u32p]
@@ -351,6 +354,18 @@ class Field:
         out = torch.empty((self.nsm_keyframe_count(), 6), device=self.device)
         _check(self.lib.nsm_keyframe_pose_gradients(self.h, out.data_ptr()))
         return out
+
+    # ---- row f4: decayed partial occupancy refresh
+    def nsm_update_occupancy_decay(self, n_subsets, decay, sync=True):
+        _check(self.lib.nsm_update_occupancy_decay(self.h, int(n_subsets), float(decay)))
+        if sync:
+            torch.cuda.synchronize(self.device)
+
+    def nsm_get_occupancy_grid(self):
+        G = self.fc.occ_res
+        out = torch.empty(G ** 3, device=self.device)
+        _check(self.lib.nsm_get_occupancy_grid(self.h, out.data_ptr()))
+        return out.cpu().numpy()
 
     def nsm_apply_pose_step(self, lr_translation, lr_rotation):
         _check(self.lib.nsm_apply_pose_step(self.h, float(lr_translation), float(lr_rotation)))

@@ -219,13 +219,52 @@ __global__ void occ_cells_kernel(uint32_t G, uint64_t first_cell, uint64_t n_cel
   ws.s_ray[i] = 0;
 }
 
-// bit = sigma > thr; one warp packs 32 cells into one word (first_cell is a multiple of 32).
+// bit = sigma > thr; one warp packs 32 cells into one word (first_cell is a multiple of 32).  The densities also
+// seed the running grid of the decayed refresh (F4).
 __global__ void occ_threshold_kernel(uint64_t first_cell, uint64_t n_cells,
-                                     const float *__restrict__ sigma, float thr, uint32_t *bits32) {
+                                     const float *__restrict__ sigma, float thr, uint32_t *bits32, float *__restrict__ grid) {
   uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
   bool on = i < n_cells && sigma[i] > thr;
+  if (i < n_cells) grid[first_cell + i] = sigma[i];
   uint32_t m = __ballot_sync(0xffffffffu, on);
   if ((threadIdx.x & 31) == 0 && i < n_cells) bits32[(first_cell + i) >> 5] = m;
+}
+
+// ---- F4 (row f4; paper silent, after [17]): decayed running maximum of the density with a strided partial refresh ----
+//   every cell: grid <- decay * grid;   cells c = c0 + j * n_sub (c0 = update index mod n_sub): grid <- max(grid, sigma(c));
+//   bit = grid > thr.   n_sub consecutive updates visit every cell exactly once.
+__global__ void occ_cells_strided_kernel(uint32_t G, uint64_t first_cell, uint32_t stride, uint64_t n_cells, Workspace ws,
+                                         uint32_t *d_S) {
+  uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i == 0) *d_S = (uint32_t)n_cells;
+  if (i >= n_cells) return;
+  uint64_t cell = first_cell + i * stride;
+  uint32_t gx = (uint32_t)(cell % G), gy = (uint32_t)((cell / G) % G), gz = (uint32_t)(cell / ((uint64_t)G * G));
+  const float Gf = __uint2float_rn(G);
+  ws.s_x[i] = __fdiv_rn(__fadd_rn(__uint2float_rn(gx), 0.5f), Gf);
+  ws.s_x[ws.cap + i] = __fdiv_rn(__fadd_rn(__uint2float_rn(gy), 0.5f), Gf);
+  ws.s_x[2 * ws.cap + i] = __fdiv_rn(__fadd_rn(__uint2float_rn(gz), 0.5f), Gf);
+  ws.s_ray[i] = 0;
+}
+
+__global__ void occ_decay_kernel(float *__restrict__ grid, uint64_t n_cells, float decay) {
+  for (uint64_t c = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; c < n_cells; c += (uint64_t)gridDim.x * blockDim.x)
+    grid[c] *= decay;
+}
+
+__global__ void occ_max_visited_kernel(float *__restrict__ grid, uint64_t first_cell, uint32_t stride, uint64_t n_visited,
+                                       const float *__restrict__ sigma) {
+  uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n_visited) return;
+  float *g = grid + first_cell + i * stride;
+  *g = fmaxf(*g, sigma[i]);
+}
+
+__global__ void occ_bits_from_grid_kernel(const float *__restrict__ grid, uint64_t n_cells, float thr, uint32_t *bits32) {
+  uint64_t c = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  bool on = c < n_cells && grid[c] > thr;
+  uint32_t m = __ballot_sync(0xffffffffu, on);
+  if ((threadIdx.x & 31) == 0 && c < n_cells) bits32[c >> 5] = m;
 }
 
 }  // namespace
@@ -246,9 +285,30 @@ int launch_occ_cells(uint32_t G, uint64_t first_cell, uint64_t n_cells, const Wo
 }
 
 int launch_occ_threshold(uint32_t G, uint64_t first_cell, uint64_t n_cells, const float *sigma,
-                         float thr, uint8_t *bits, cudaStream_t st) {
+                         float thr, uint8_t *bits, float *grid, cudaStream_t st) {
   (void)G;
   occ_threshold_kernel<<<(unsigned)((n_cells + 255) / 256), 256, 0, st>>>(first_cell, n_cells, sigma, thr,
-                                                                         (uint32_t *)bits);
+                                                                         (uint32_t *)bits, grid);
+  return 1;
+}
+
+int launch_occ_cells_strided(uint32_t G, uint64_t first_cell, uint32_t stride, uint64_t n_cells, const Workspace &ws, uint32_t *d_S,
+                             cudaStream_t st) {
+  occ_cells_strided_kernel<<<(unsigned)((n_cells + 255) / 256), 256, 0, st>>>(G, first_cell, stride, n_cells, ws, d_S);
+  return 1;
+}
+
+int launch_occ_decay(float *grid, uint64_t n_cells, float decay, cudaStream_t st) {
+  occ_decay_kernel<<<1184, 256, 0, st>>>(grid, n_cells, decay);
+  return 1;
+}
+
+int launch_occ_max_visited(float *grid, uint64_t first_cell, uint32_t stride, uint64_t n_visited, const float *sigma, cudaStream_t st) {
+  occ_max_visited_kernel<<<(unsigned)((n_visited + 255) / 256), 256, 0, st>>>(grid, first_cell, stride, n_visited, sigma);
+  return 1;
+}
+
+int launch_occ_bits_from_grid(const float *grid, uint64_t n_cells, float thr, uint8_t *bits, cudaStream_t st) {
+  occ_bits_from_grid_kernel<<<(unsigned)((n_cells + 255) / 256), 256, 0, st>>>(grid, n_cells, thr, (uint32_t *)bits);
   return 1;
 }

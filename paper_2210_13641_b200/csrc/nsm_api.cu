@@ -91,6 +91,7 @@ struct nsm_field {
   uint32_t step = 0;
   uint64_t launches = 0;
   bool occ_full = true;
+  uint32_t occ_updates = 0;   // F4: decayed partial refreshes since the last full one
   bool grads_dirty = false;
   // state of the last step, for the debug getter
   uint32_t last_R = 0, last_K = 0;
@@ -540,6 +541,7 @@ nsm_status nsm_create_field(const nsm_field_config *cfg, void *cuda_stream, nsm_
   A(f->alloc(&fp.theta, fp.n_table)); A(f->alloc(&fp.mv, 2 * fp.n_table));
   A(f->alloc(&fp.mlp_theta, fp.n_mlp)); A(f->alloc(&fp.mlp_m, fp.n_mlp)); A(f->alloc(&fp.mlp_v, fp.n_mlp)); A(f->alloc(&fp.mlp_grad, fp.n_mlp));
   A(f->alloc(&fp.grad, fp.n_table, false)); A(f->alloc(&fp.occ_bits, (G3 + 7) / 8 + 4));
+  A(f->alloc(&fp.occ_grid, G3));
   A(f->alloc(&ws.counts, R)); A(f->alloc(&ws.offsets, R + 1)); A(f->alloc(&ws.scan_state, march_scan_state_entries(R) + 1)); A(f->alloc(&ws.scan_ctr, 2));
   A(f->alloc(&ws.C, 3 * (size_t)R)); A(f->alloc(&ws.D_hat, R)); A(f->alloc(&ws.O, R));
   A(f->alloc(&ws.s_ray, cap)); A(f->alloc(&ws.s_k, cap)); A(f->alloc(&ws.s_t, cap)); A(f->alloc(&ws.s_delta, cap));
@@ -731,14 +733,54 @@ nsm_status nsm_update_occupancy(nsm_field *f, nsm_occ_mode mode, const uint8_t *
         else
           RUN(f, K_MLP_FWD, launch_mlp_forward_simt(f->ms, f->fp.mlp_theta, nullptr, f->ws, d_S, 1, f->n_sms, f->stream));
         RUN(f, K_OCC, launch_occ_threshold(f->cfg.occ_res, first, n, f->ws.sigma, f->cfg.occ_sigma_threshold,
-                                           f->fp.occ_bits, f->stream));
+                                           f->fp.occ_bits, f->fp.occ_grid, f->stream));
       }
       f->occ_full = false;
+      f->occ_updates = 0;
       CUDA_TRY(cudaGetLastError());
       return NSM_OK;
     }
   }
   return fail(NSM_ERR_INVALID_ARG, "bad occupancy mode %d", (int)mode);
+}
+
+// F4: decayed running maximum + strided partial refresh (paper silent, after [17])
+nsm_status nsm_update_occupancy_decay(nsm_field *f, uint32_t n_subsets, float decay) {
+  if (!f) return fail(NSM_ERR_INVALID_ARG, "field is NULL");
+  if (n_subsets == 0) return fail(NSM_ERR_INVALID_ARG, "n_subsets is 0");
+  if (!(decay >= 0.f && decay <= 1.f)) return fail(NSM_ERR_INVALID_ARG, "decay must be in [0, 1]");
+  leave_fast_path(f);
+  const uint64_t G3 = (uint64_t)f->cfg.occ_res * f->cfg.occ_res * f->cfg.occ_res;
+  const uint64_t c0 = f->occ_updates % n_subsets;
+  const uint64_t n_vis = c0 < G3 ? (G3 - c0 + n_subsets - 1) / n_subsets : 0;
+  const uint64_t chunk = f->ws.cap & ~uint64_t(31);
+  const int bf16 = f->cfg.mlp_precision == NSM_MLP_BF16;
+  uint32_t *d_S = f->ws.offsets;
+  RUN(f, K_OCC, launch_occ_decay(f->fp.occ_grid, G3, decay, f->stream));
+  for (uint64_t j0 = 0; j0 < n_vis; j0 += chunk) {
+    const uint64_t n = (n_vis - j0 < chunk) ? n_vis - j0 : chunk;
+    const uint64_t first = c0 + j0 * n_subsets;
+    RUN(f, K_OCC, launch_occ_cells_strided(f->cfg.occ_res, first, n_subsets, n, f->ws, d_S, f->stream));
+    RUN(f, K_ENCODE, launch_encode(f->lv, f->fp.theta, f->ws, d_S, f->use_tc ? 1 + bf16 : 0, f->n_sms, f->stream));
+    if (f->use_tc)
+      RUN(f, K_MLP_FWD, launch_mlp_forward_tc(f->ms, bf16, nullptr, f->ws, d_S, 1, 0, f->n_sms, f->stream));
+    else
+      RUN(f, K_MLP_FWD, launch_mlp_forward_simt(f->ms, f->fp.mlp_theta, nullptr, f->ws, d_S, 1, f->n_sms, f->stream));
+    RUN(f, K_OCC, launch_occ_max_visited(f->fp.occ_grid, first, n_subsets, n, f->ws.sigma, f->stream));
+  }
+  RUN(f, K_OCC, launch_occ_bits_from_grid(f->fp.occ_grid, G3, f->cfg.occ_sigma_threshold, f->fp.occ_bits, f->stream));
+  f->occ_full = false;
+  f->occ_updates += 1;
+  CUDA_TRY(cudaGetLastError());
+  return NSM_OK;
+}
+
+nsm_status nsm_get_occupancy_grid(nsm_field *f, float *d_grid) {
+  if (!f || !d_grid) return fail(NSM_ERR_INVALID_ARG, "NULL argument");
+  leave_fast_path(f);
+  const uint64_t G3 = (uint64_t)f->cfg.occ_res * f->cfg.occ_res * f->cfg.occ_res;
+  CUDA_TRY(cudaMemcpyAsync(d_grid, f->fp.occ_grid, sizeof(float) * G3, cudaMemcpyDeviceToDevice, f->stream));
+  return NSM_OK;
 }
 
 nsm_status nsm_backward(nsm_field *f, const nsm_ray_batch *batch, float lambda_d, nsm_step_stats *host_stats) {

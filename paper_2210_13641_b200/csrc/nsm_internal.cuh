@@ -145,6 +145,7 @@ struct FieldParams {
   float *grad;                                      // [n_entries][F]
   float *mlp_theta, *mlp_m, *mlp_v, *mlp_grad;      // [n_mlp] each, canonical order
   uint8_t *occ_bits;                                // [G^3/8]
+  float *occ_grid;                                  // [G^3] running density of the decayed refresh (F4); seeded by FROM_FIELD
   uint64_t n_entries, n_table, n_mlp;
   uint32_t F;
 };
@@ -315,7 +316,13 @@ int launch_pose_step(KeyframeDev *kfs, uint32_t n_kf, const float *kf_grad, floa
 int launch_occ_cells(uint32_t G, uint64_t first_cell, uint64_t n_cells, const Workspace &ws,
                      uint32_t *d_S, cudaStream_t st);
 int launch_occ_threshold(uint32_t G, uint64_t first_cell, uint64_t n_cells, const float *sigma,
-                         float thr, uint8_t *bits, cudaStream_t st);
+                         float thr, uint8_t *bits, float *grid, cudaStream_t st);
+// F4: decayed running-maximum density grid with a strided partial refresh
+int launch_occ_cells_strided(uint32_t G, uint64_t first_cell, uint32_t stride, uint64_t n_cells, const Workspace &ws, uint32_t *d_S,
+                             cudaStream_t st);
+int launch_occ_decay(float *grid, uint64_t n_cells, float decay, cudaStream_t st);
+int launch_occ_max_visited(float *grid, uint64_t first_cell, uint32_t stride, uint64_t n_visited, const float *sigma, cudaStream_t st);
+int launch_occ_bits_from_grid(const float *grid, uint64_t n_cells, float thr, uint8_t *bits, cudaStream_t st);
 int launch_debug_slots(const LevelTable &lv, const Workspace &ws, const uint32_t *d_S,
                        uint32_t *slots, float *w, cudaStream_t st);
 int launch_planes_to_rows(const float *planes, uint64_t cap, uint32_t n_planes, const uint32_t *d_S,

@@ -618,3 +618,54 @@ def test_pose_update_step_against_the_oracle(nsm):
     with pytest.raises(nsm.NsmError):
         f.nsm_apply_pose_step(lr_t, lr_r)          # the gradients were consumed
     f.close()
+
+
+# ---------------------------------------------------------------------------- row f4: decayed partial occupancy refresh
+
+def test_occupancy_decay_update_against_the_oracle(nsm):
+    """nsm_update_occupancy_decay vs orc_occupancy_decay_update while the field trains: the running grid within tolerance,
+    the bits equal outside the tolerance band around the threshold, and the marcher using them (counts bit-exact given
+    the same bits); (n_subsets = 1, decay = 0) equals FROM_FIELD bit for bit on the GPU."""
+    w = configs.config3(R=2048, K=128, n_keyframes=3, n_batches=6, width=300, height=170)
+    w = replace(w, field=replace(w.field, occ_sigma_threshold=1.0))   # sigma = exp(g0) straddles 1: a non-trivial bitfield
+    f, O, _ = make_pair(nsm, w, seed=16, table_scale=0.5)
+    tol = tol_for(w.field, f.nsm_mlp_path())
+    thr = float(np.float32(w.field.occ_sigma_threshold))
+    G3 = w.field.occ_res ** 3
+
+    def sync_params():
+        th, _, _, step = f.nsm_get_params()
+        O.theta, O.step = th.astype(np.float64), step
+
+    for b in w.batches[:3]:
+        f.nsm_train_step(nsm.DeviceBatch(b), w.lambda_d, want_stats=False)
+    sync_params()
+    f.nsm_update_occupancy(nsm.NSM_OCC_FROM_FIELD)
+    bits_ref, sig = O.occupancy_from_field(want_sigma=True)          # seeds O.occ_grid
+    grid = f.nsm_get_occupancy_grid()
+    assert np.abs(grid - sig).max() <= tol * max(sig.max(), thr)
+    for u, (n_sub, decay) in enumerate(((4, 0.95), (4, 0.95), (4, 0.95), (4, 0.95), (3, 0.5), (7, 1.0))):
+        f.nsm_train_step(nsm.DeviceBatch(w.batches[3 + u % 3]), w.lambda_d, want_stats=False)
+        sync_params()
+        f.nsm_update_occupancy_decay(n_sub, decay)
+        bits_o = np.unpackbits(O.occupancy_decay_update(n_sub, decay), bitorder="little")[:G3].astype(bool)
+        grid = f.nsm_get_occupancy_grid().astype(np.float64)
+        assert np.abs(grid - O.occ_grid).max() <= tol * max(O.occ_grid.max(), thr), (u, np.abs(grid - O.occ_grid).max())
+        bits_g = np.unpackbits(f.nsm_get_occupancy(), bitorder="little")[:G3].astype(bool)
+        band = np.abs(O.occ_grid - thr) <= tol * max(thr, 1e-30) + tol * np.abs(O.occ_grid)
+        assert np.array_equal(bits_g[~band], bits_o[~band]), u
+        O.occ_grid = grid.copy()                                     # keep the two histories together (the max is not linear)
+    assert 0.02 < bits_g.mean() < 0.98, bits_g.mean()
+    # the marcher runs on these bits
+    O.set_occupancy(f.nsm_get_occupancy())
+    st = f.nsm_backward(nsm.DeviceBatch(w.batches[0]), w.lambda_d)
+    so, tr = O.train_step(w.batches[0], w.lambda_d, apply_adam=False, trace=("counts",))
+    assert st["n_samples"] == so["n_samples"] and np.array_equal(f.nsm_debug_last_step("counts"), tr["counts"])
+    # reduction to S14 on the GPU itself
+    f.nsm_update_occupancy(nsm.NSM_OCC_FROM_FIELD)
+    a = f.nsm_get_occupancy().copy()
+    f.nsm_update_occupancy_decay(1, 0.0)
+    assert np.array_equal(f.nsm_get_occupancy(), a)
+    with pytest.raises(nsm.NsmError):
+        f.nsm_update_occupancy_decay(0, 0.9)
+    f.close()
