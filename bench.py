@@ -206,6 +206,27 @@ NCU_TRAFFIC_CFG2 = {"adam_table": 157317888 + 65678848, "scatter": 37862400, "en
                     "mlp_bwd": 11984384 + 256, "mlp_fwd": 3022848, "adam_mlp": 6556160, "composite": 643584, "march": 382208}
 
 
+def run_probe_l2():
+    """The L2 random-access rates the encoder / scatter rooflines are quoted against (nsm_probe_l2)."""
+    import torch
+    import paper_2210_13641_b200 as nsm
+    from paper_2210_13641_b200 import build as nsm_build
+    nsm_build.build()
+    torch.cuda.set_device(0)
+    rows = []
+    for mb in (12, 24, 48, 64, 96, 128, 195, 390):
+        g = nsm.probe_l2(mb << 20, 1 << 22, False)
+        r = nsm.probe_l2(mb << 20, 1 << 22, True)
+        rows.append(dict(table_mb=mb, gathers_per_s=g, reductions_per_s=r))
+    print(json.dumps(dict(probe="nsm_probe_l2: 2^22 random 8-byte gathers / red.global.add.v2.f32 per launch, best of 8", rows=rows)))
+    return 0
+
+
+# L2 random-access peaks from `python bench.py --probe-l2` on B200 (profiles/r1p_l2_probe.md): table resident in L2
+L2_RANDOM_GATHERS_PER_S = 202e9
+L2_RANDOM_REDUCTIONS_PER_S = 160e9
+
+
 def run_render(args, nsm, replicas, dev, rank, world, peaks):
     """Config 5: forward-only full-frame render (rays/s, samples/s) of a field trained on config 3's data."""
     import torch
@@ -407,6 +428,12 @@ def run_cuda(args):
                 k.update(achieved=model["flops"] / avg_s / 1e12 if avg_s > 0 else 0.0, unit="TFLOP/s", peak=peak,
                          algorithmic_flops=model["flops"])
             k["frac"] = k["achieved"] / k["peak"]
+            if name in ("encode", "scatter") and avg_s > 0:
+                # what actually bounds S4 / S12 while the tables fit the L2: its random-access rate (8 corners per sample-level)
+                acc = 8 * L * S_avg / avg_s
+                pk = L2_RANDOM_GATHERS_PER_S if name == "encode" else L2_RANDOM_REDUCTIONS_PER_S
+                k["l2_random"] = dict(achieved_accesses_per_s=acc, peak_accesses_per_s=pk, frac=acc / pk,
+                                      peak_source="nsm_probe_l2, 48 MB table (profiles/r1p_l2_probe.md)")
             kernels.append(k)
         kernels.sort(key=lambda k: -k["share"])
         top = kernels[0]
@@ -445,9 +472,13 @@ def main():
     ap.add_argument("--steps", type=int, default=None, help="timed steps (default 2000; 40 for --impl reference)")
     ap.add_argument("--warmup", type=int, default=None, help="untimed warm-up steps (default 20; 2 for --impl reference)")
     ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
+    ap.add_argument("--probe-l2", action="store_true", help="print the random-gather / vector-reduction rates of nsm_probe_l2 "
+                    "over table sizes from L2-resident to DRAM-resident (one JSON line) and exit")
     ap.add_argument("--config", type=int, default=2, choices=[1, 2, 3, 4, 5],
                     help="BASELINE.json config to run (default 2 = configs[1], the one the metric is quoted on)")
     args = ap.parse_args()
+    if args.probe_l2:
+        return run_probe_l2()
     if args.steps is None:
         args.steps = 40 if args.impl == "reference" else {1: 2000, 2: 2000, 3: 100, 4: 200, 5: 3}[args.config]
     if args.warmup is None:

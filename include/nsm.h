@@ -153,6 +153,11 @@ nsm_status nsm_train_step_host(nsm_field *f, const nsm_ray_batch *host_batch, fl
  * start of ~0 / end of 0 means "did not run".  Synchronises.  Costs a few atomics per block: not for timing runs. */
 nsm_status nsm_debug_timeline(nsm_field *f, uint64_t *h_out, uint64_t capacity_words, uint32_t *n_kernels);
 
+/* Micro-benchmark behind the L2 figures the rooflines of S4 / S12 are quoted against (MEASURED_PEAKS.json has HBM and
+ * bf16 only): n_accesses random 8-byte gathers (reductions = 0) or red.global.add.v2.f32 (reductions = 1) over a
+ * scratch table of table_bytes; *seconds_out = best of 8 timed launches after 4 warm-up launches.  Needs no field. */
+nsm_status nsm_probe_l2(uint64_t table_bytes, uint64_t n_accesses, int reductions, double *seconds_out);
+
 /* ---- Row f4: decayed partial occupancy refresh (the paper is silent; [17] keeps a decayed running maximum of the
  * density and refreshes part of the grid per update).  The library keeps a running density per cell, seeded by
  * nsm_update_occupancy(NSM_OCC_FROM_FIELD).  One call:  every cell  grid <- decay * grid;  the cells

@@ -30,7 +30,7 @@ EXPORTS = ["nsm_create_field", "nsm_destroy_field", "nsm_update_occupancy", "nsm
            "nsm_get_level_table", "nsm_debug_last_step", "nsm_total_samples", "nsm_profile", "nsm_set_option", "nsm_debug_timeline",
            "nsm_add_keyframe", "nsm_keyframe_count", "nsm_sample_batch", "nsm_train_step_sampled",
            "nsm_pose_gradients", "nsm_keyframe_pose_gradients", "nsm_apply_pose_step", "nsm_get_keyframe_pose",
-           "nsm_update_occupancy_decay", "nsm_get_occupancy_grid",
+           "nsm_update_occupancy_decay", "nsm_get_occupancy_grid", "nsm_probe_l2",
            "nsm_profile_read", "nsm_launch_count", "nsm_mlp_path",
            "nsm_last_error", "nsm_version"]
 
@@ -103,6 +103,7 @@ def load_library():
         L.nsm_set_option.argtypes = [vp, C.c_int, C.c_uint32]
         L.nsm_pose_gradients.argtypes = [vp, vp, vp]
         L.nsm_keyframe_pose_gradients.argtypes = [vp, vp]
+        L.nsm_probe_l2.argtypes = [C.c_uint64, C.c_uint64, C.c_int, C.POINTER(C.c_double)]
         L.nsm_update_occupancy_decay.argtypes = [vp, C.c_uint32, C.c_float]
         L.nsm_get_occupancy_grid.argtypes = [vp, vp]
         L.nsm_apply_pose_step.argtypes = [vp, C.c_float, C.c_float]
@@ -178,6 +179,13 @@ class DeviceBatch:
         b.rgb, b.depth, b.depth_var = _dev_ptr(self.rgb), _dev_ptr(self.depth), _dev_ptr(self.depth_var)
         b.t_min, b.t_max, b.n_candidates = self.t_min, self.t_max, self.n_candidates
         return b
+
+
+def probe_l2(table_bytes, n_accesses=1 << 22, reductions=False):
+    """Random 8-byte gathers (or vector reductions) per second over a scratch table of table_bytes (nsm_probe_l2)."""
+    sec = C.c_double()
+    _check(load_library().nsm_probe_l2(int(table_bytes), int(n_accesses), int(bool(reductions)), C.byref(sec)))
+    return n_accesses / sec.value
 
 
 class HostBatch:

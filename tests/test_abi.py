@@ -21,7 +21,7 @@ def lib():
 def declared_symbols():
     src = open(os.path.join(ROOT, "include", "nsm.h")).read()
     src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
-    return sorted(set(re.findall(r"\b(nsm_[a-z_]+)\s*\(", src)))
+    return sorted(set(re.findall(r"\b(nsm_[a-z0-9_]+)\s*\(", src)))
 
 
 def test_every_declared_symbol_is_exported(lib):
