@@ -200,10 +200,10 @@ def kernel_model(name, S, R, K, L, F, LF, U, E, mac, n_mlp):
 
 
 # DRAM bytes (dram__bytes_read.sum + dram__bytes_write.sum) per launch from the `ncu --set full` capture of
-# profiles/r1l_ncu_full.md (config 2; cold cache, as ncu flushes before every kernel).  bench.py cannot run ncu:
+# profiles/r1q_ncu_full.md (config 2; cold cache, as ncu flushes before every kernel).  bench.py cannot run ncu:
 # these are recorded values, refreshed with each committed profile.
-NCU_TRAFFIC_CFG2 = {"adam_table": 157317888 + 65678848, "scatter": 37862400, "encode": 40513792 + 65792,
-                    "mlp_bwd": 11984384 + 256, "mlp_fwd": 3022848, "adam_mlp": 6556160, "composite": 643584, "march": 382208}
+NCU_TRAFFIC_CFG2 = {"adam_table": 223813888, "scatter": 37892864, "encode": 40574208, "mlp_bwd": 11985152, "mlp_fwd": 3022592,
+                    "adam_mlp": 6556160, "composite": 643840, "march": 381952}
 
 
 def run_probe_l2():
@@ -387,6 +387,19 @@ def run_cuda(args):
         v_s, _, _ = replicas.aggregate_throughput(f.nsm_total_samples() - s3, t_s)
         sampled = dict(value=v_s, unit=UNIT, ms_per_step=1e3 * t_s / K, keyframes=kfs.n,
                        store_bytes=kfs.n * kfs.W * kfs.H * 5 * 4, api="nsm_train_step_sampled")
+        if args.pose:   # row f2: the same leg with the pose gradients computed and the keyframe poses stepped every step
+            f.nsm_set_option(nsm.NSM_OPT_POSE_GRADIENTS, 1)
+
+            def pose_step(i):
+                sampled_step(i)
+                f.nsm_apply_pose_step(0.0, 0.0)          # zero learning rates: the full update path, poses unchanged
+            for i in range(W):
+                pose_step(i)
+            s4 = f.nsm_total_samples()
+            t_p = timed(K, pose_step, W + 3 * K)
+            v_p, _, _ = replicas.aggregate_throughput(f.nsm_total_samples() - s4, t_p)
+            sampled["with_pose_gradients"] = dict(value=v_p, unit=UNIT, ms_per_step=1e3 * t_p / K,
+                                                  api="nsm_train_step_sampled + nsm_apply_pose_step, NSM_OPT_POSE_GRADIENTS")
 
     line = None
     if rank == 0:
@@ -439,7 +452,7 @@ def run_cuda(args):
         top = kernels[0]
         roofline = dict(kernel=top["kernel"], bound=top["bound"], achieved=top["achieved"], peak=top["peak"], unit=top["unit"],
                         frac=top["frac"], traffic=NCU_TRAFFIC_CFG2.get(top["kernel"]) if cfg == 2 else None,
-                        traffic_source="profiles/r1l_ncu_full.md (ncu --set full, per launch, cold cache)" if cfg == 2 else None,
+                        traffic_source="profiles/r1q_ncu_full.md (ncu --set full, per launch, cold cache)" if cfg == 2 else None,
                         share_of_step=top["share"], avg_us=top["avg_us"],
                         peak_source=peaks["source"] if top["bound"] != "alu" else "derived: 148 SM x 128 FMA/clk x 2 x 1.965 GHz",
                         samples_per_launch=S_avg, touched_entries=U)
@@ -472,6 +485,7 @@ def main():
     ap.add_argument("--steps", type=int, default=None, help="timed steps (default 2000; 40 for --impl reference)")
     ap.add_argument("--warmup", type=int, default=None, help="untimed warm-up steps (default 20; 2 for --impl reference)")
     ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
+    ap.add_argument("--pose", action="store_true", help="config 3: add a sampled leg with pose gradients and pose steps (row f2)")
     ap.add_argument("--probe-l2", action="store_true", help="print the random-gather / vector-reduction rates of nsm_probe_l2 "
                     "over table sizes from L2-resident to DRAM-resident (one JSON line) and exit")
     ap.add_argument("--config", type=int, default=2, choices=[1, 2, 3, 4, 5],

@@ -7,7 +7,7 @@
 // weights: dL/dx_c = sum_l N_l sum_corners (d omega / d w_c) theta[corner] . dL/de_l) and the direction encoding Y(d)
 // (S6; dL/dY comes out of the colour MLP's first-layer dgrad).  Liveness, t and delta are piecewise constant in the pose.
 //
-// pose_dx_kernel: one warp per sample, lane = level: the 8 corner gathers of S4 once more (theta is still the
+// pose_dx_kernel: 16 or 32 lanes per sample, lane = level: the 8 corner gathers of S4 once more (theta is still the
 // pre-update theta: this runs between the MLP backward and Adam), dotted with dL/de; warp-reduced over levels.
 // pose_ray_kernel: one warp per ray: sums dL/dx, t dL/dx and dL/dY over the ray's samples, applies the polynomial SH
 // Jacobian (S6, degree <= 4) and the cross products.
@@ -24,15 +24,17 @@ __device__ __forceinline__ float warp_sum(float v) {
   return v;
 }
 
-template <int F>
+// LPS lanes per sample (16 when L <= 16: two samples per warp; else 32), lane = level.
+template <int F, int LPS>
 __global__ void __launch_bounds__(256) pose_dx_kernel(LevelTable lv, const float *__restrict__ theta, Workspace ws,
                                                       const uint32_t *__restrict__ d_S) {
   const uint64_t S = *d_S;
-  const uint32_t lane = threadIdx.x & 31;
-  const uint64_t warp0 = ((uint64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5, n_warps = ((uint64_t)gridDim.x * blockDim.x) >> 5;
-  for (uint64_t s = warp0; s < S; s += n_warps) {
+  const uint32_t lane = threadIdx.x & (LPS - 1);
+  const uint64_t group0 = ((uint64_t)blockIdx.x * blockDim.x + threadIdx.x) / LPS, n_groups = ((uint64_t)gridDim.x * blockDim.x) / LPS;
+  const uint64_t S_pad = (S + (32 / LPS) - 1) / (32 / LPS) * (32 / LPS);   // whole warps stay converged for the shuffles
+  for (uint64_t s = group0; s < S_pad; s += n_groups) {
     float acc[3] = {0.f, 0.f, 0.f};
-    if (lane < lv.n_levels) {
+    if (s < S && lane < lv.n_levels) {
       const uint32_t l = lane;
       const CornerIndex ci = corner_index(lv, l, ws.s_x[s], ws.s_x[ws.cap + s], ws.s_x[2 * ws.cap + s]);
       float de[F];
@@ -56,8 +58,10 @@ __global__ void __launch_bounds__(256) pose_dx_kernel(LevelTable lv, const float
       }
     }
 #pragma unroll
-    for (int c = 0; c < 3; ++c) acc[c] = warp_sum(acc[c]);
-    if (lane < 3) ws.dx[(size_t)lane * ws.cap + s] = lane == 0 ? acc[0] : (lane == 1 ? acc[1] : acc[2]);
+    for (int c = 0; c < 3; ++c)
+#pragma unroll
+      for (int sft = LPS / 2; sft > 0; sft >>= 1) acc[c] += __shfl_xor_sync(0xffffffffu, acc[c], sft);
+    if (s < S && lane < 3) ws.dx[(size_t)lane * ws.cap + s] = lane == 0 ? acc[0] : (lane == 1 ? acc[1] : acc[2]);
   }
 }
 
@@ -196,11 +200,12 @@ int launch_pose_gradients(const LevelTable &lv, const float *theta, const Worksp
                           const float *dirs, float inv_extent, uint32_t sh_degree, float *g_o, float *tau, const uint32_t *ray_kf,
                           float *kf_grad, int n_sms, cudaStream_t st) {
   dim3 grid(n_sms * 8), block(256);
+  const bool half = lv.n_levels <= 16;
   switch (lv.n_features) {
-    case 1: pose_dx_kernel<1><<<grid, block, 0, st>>>(lv, theta, ws, d_S); break;
-    case 2: pose_dx_kernel<2><<<grid, block, 0, st>>>(lv, theta, ws, d_S); break;
-    case 4: pose_dx_kernel<4><<<grid, block, 0, st>>>(lv, theta, ws, d_S); break;
-    default: pose_dx_kernel<8><<<grid, block, 0, st>>>(lv, theta, ws, d_S); break;
+    case 1: if (half) pose_dx_kernel<1, 16><<<grid, block, 0, st>>>(lv, theta, ws, d_S); else pose_dx_kernel<1, 32><<<grid, block, 0, st>>>(lv, theta, ws, d_S); break;
+    case 2: if (half) pose_dx_kernel<2, 16><<<grid, block, 0, st>>>(lv, theta, ws, d_S); else pose_dx_kernel<2, 32><<<grid, block, 0, st>>>(lv, theta, ws, d_S); break;
+    case 4: if (half) pose_dx_kernel<4, 16><<<grid, block, 0, st>>>(lv, theta, ws, d_S); else pose_dx_kernel<4, 32><<<grid, block, 0, st>>>(lv, theta, ws, d_S); break;
+    default: if (half) pose_dx_kernel<8, 16><<<grid, block, 0, st>>>(lv, theta, ws, d_S); else pose_dx_kernel<8, 32><<<grid, block, 0, st>>>(lv, theta, ws, d_S); break;
   }
   pose_ray_kernel<<<(R + 7) / 8, 256, 0, st>>>(ws, R, dirs, inv_extent, sh_degree, g_o, tau, ray_kf, kf_grad);
   return 2;
