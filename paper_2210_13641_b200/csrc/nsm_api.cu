@@ -351,10 +351,9 @@ nsm_status enqueue_backward(nsm_field *f, const nsm_ray_batch *b, float lambda_d
                                                f->ws, d_S, f->n_sms, f->stream));
   if (f->pose_grads) {   // row f2: needs dL/de, dL/dY of this step and the PRE-update theta: between the MLP backward and Adam
     f->last_sampled = sample_draw >= 0;
-    if (f->last_sampled) CUDA_TRY(cudaMemsetAsync(f->kf_grad, 0, sizeof(float) * NSM_KF_GRAD_STRIDE * f->kf_host.size(), f->stream));
     RUN(f, K_POSE, launch_pose_gradients(f->lv, f->fp.theta, f->ws, d_S, R, dirs_copy ? dirs_copy : b->dirs, 1.0f / f->cfg.aabb_extent,
                                          f->cfg.sh_degree, f->pose_go, f->pose_tau, f->last_sampled ? f->ray_kf : nullptr, f->kf_grad,
-                                         f->n_sms, f->stream));
+                                         (uint32_t)f->kf_host.size(), f->n_sms, f->stream));
   }
   // train step: the scatter is issued by enqueue_adam, level group by level group, each followed by its Adam
   f->scatter_pending = defer_scatter;

@@ -306,10 +306,10 @@ int launch_adam_mlp_pack(const MlpShape &ms, int bf16, const FieldParams &fp, co
 int launch_sample_batch(const KeyframeDev *kfs, uint32_t n_kf, uint64_t seed, uint32_t draw, uint32_t n_rays, float *origins,
                         float *dirs, float *rgb, float *depth, float *depth_var, uint32_t *ray_kf, cudaStream_t st);
 // f2: per-ray dL/do and rotation gradient from ws.de / ws.dY (after the MLP backward, before Adam); ray_kf + kf_grad
-// (optional): accumulate the per-keyframe vectors [n_kf][NSM_KF_GRAD_STRIDE] (kf_grad must be zeroed by the caller)
+// (optional): the per-keyframe vectors [n_kf][NSM_KF_GRAD_STRIDE], written (not accumulated) by a block per keyframe
 int launch_pose_gradients(const LevelTable &lv, const float *theta, const Workspace &ws, const uint32_t *d_S, uint32_t R,
                           const float *dirs, float inv_extent, uint32_t sh_degree, float *g_o, float *tau, const uint32_t *ray_kf,
-                          float *kf_grad, int n_sms, cudaStream_t st);
+                          float *kf_grad, uint32_t n_kf, int n_sms, cudaStream_t st);
 // f2, the update: Adam + exponential map on the keyframes that received rays (kf_grad: [n_kf][NSM_KF_GRAD_STRIDE])
 int launch_pose_step(KeyframeDev *kfs, uint32_t n_kf, const float *kf_grad, float *pm, float *pv, uint32_t *pcnt, float lr_t,
                      float lr_r, float beta1, float beta2, float eps, cudaStream_t st);

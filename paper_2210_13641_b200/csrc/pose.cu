@@ -92,8 +92,7 @@ __device__ __forceinline__ void sh_grad_dot(uint32_t n, float x, float y, float 
 }
 
 __global__ void __launch_bounds__(256) pose_ray_kernel(Workspace ws, uint32_t R, const float *__restrict__ dirs, float inv_extent,
-                                                       uint32_t sh_degree, float *__restrict__ g_o, float *__restrict__ tau,
-                                                       const uint32_t *__restrict__ ray_kf, float *__restrict__ kf_grad) {
+                                                       uint32_t sh_degree, float *__restrict__ g_o, float *__restrict__ tau) {
   const uint32_t r = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
   if (r >= R) return;
   const uint32_t off = ws.offsets[r], n = ws.offsets[r + 1] - off;
@@ -127,12 +126,34 @@ __global__ void __launch_bounds__(256) pose_ray_kernel(Workspace ws, uint32_t R,
     const float t0 = y * g[2] - z * g[1], t1 = z * g[0] - x * g[2], t2 = x * g[1] - y * g[0];
     g_o[3 * (size_t)r] = so[0]; g_o[3 * (size_t)r + 1] = so[1]; g_o[3 * (size_t)r + 2] = so[2];
     tau[3 * (size_t)r] = t0; tau[3 * (size_t)r + 1] = t1; tau[3 * (size_t)r + 2] = t2;
-    if (ray_kf) {   // per-keyframe se(3) gradient (translation | rotation | number of rays | pad)
-      float *kg = kf_grad + NSM_KF_GRAD_STRIDE * (size_t)ray_kf[r];
-      atomicAdd(kg, so[0]); atomicAdd(kg + 1, so[1]); atomicAdd(kg + 2, so[2]);
-      atomicAdd(kg + 3, t0); atomicAdd(kg + 4, t1); atomicAdd(kg + 5, t2);
-      atomicAdd(kg + 6, 1.0f);
+  }
+}
+
+// Per-keyframe se(3) gradient (translation | rotation | number of rays | pad): one block per keyframe scans the batch
+// for its rays and sums their g_o and tau.  Deterministic, and no hot atomics: with ~10 keyframes the obvious
+// atomicAdd per ray puts 16 K reductions on each of 70 addresses (33 us of same-address serialisation at 2^14 rays).
+__global__ void __launch_bounds__(256) pose_kf_reduce_kernel(uint32_t R, const uint32_t *__restrict__ ray_kf, const float *__restrict__ g_o,
+                                                             const float *__restrict__ tau, float *__restrict__ kf_grad) {
+  __shared__ float red[8][7];
+  const uint32_t k = blockIdx.x, lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+  float acc[7] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
+  for (uint32_t r = threadIdx.x; r < R; r += blockDim.x) {
+    if (ray_kf[r] == k) {
+#pragma unroll
+      for (int c = 0; c < 3; ++c) { acc[c] += g_o[3 * (size_t)r + c]; acc[3 + c] += tau[3 * (size_t)r + c]; }
+      acc[6] += 1.f;
     }
+  }
+#pragma unroll
+  for (int i = 0; i < 7; ++i) {
+    acc[i] = warp_sum(acc[i]);
+    if (lane == 0) red[wid][i] = acc[i];
+  }
+  __syncthreads();
+  if (threadIdx.x < 7) {
+    float v = 0.f;
+    for (int w = 0; w < 8; ++w) v += red[w][threadIdx.x];
+    kf_grad[NSM_KF_GRAD_STRIDE * (size_t)k + threadIdx.x] = v;
   }
 }
 
@@ -198,7 +219,7 @@ int launch_pose_step(KeyframeDev *kfs, uint32_t n_kf, const float *kf_grad, floa
 
 int launch_pose_gradients(const LevelTable &lv, const float *theta, const Workspace &ws, const uint32_t *d_S, uint32_t R,
                           const float *dirs, float inv_extent, uint32_t sh_degree, float *g_o, float *tau, const uint32_t *ray_kf,
-                          float *kf_grad, int n_sms, cudaStream_t st) {
+                          float *kf_grad, uint32_t n_kf, int n_sms, cudaStream_t st) {
   dim3 grid(n_sms * 8), block(256);
   const bool half = lv.n_levels <= 16;
   switch (lv.n_features) {
@@ -207,6 +228,7 @@ int launch_pose_gradients(const LevelTable &lv, const float *theta, const Worksp
     case 4: if (half) pose_dx_kernel<4, 16><<<grid, block, 0, st>>>(lv, theta, ws, d_S); else pose_dx_kernel<4, 32><<<grid, block, 0, st>>>(lv, theta, ws, d_S); break;
     default: if (half) pose_dx_kernel<8, 16><<<grid, block, 0, st>>>(lv, theta, ws, d_S); else pose_dx_kernel<8, 32><<<grid, block, 0, st>>>(lv, theta, ws, d_S); break;
   }
-  pose_ray_kernel<<<(R + 7) / 8, 256, 0, st>>>(ws, R, dirs, inv_extent, sh_degree, g_o, tau, ray_kf, kf_grad);
-  return 2;
+  pose_ray_kernel<<<(R + 7) / 8, 256, 0, st>>>(ws, R, dirs, inv_extent, sh_degree, g_o, tau);
+  if (ray_kf && n_kf) pose_kf_reduce_kernel<<<n_kf, 256, 0, st>>>(R, ray_kf, g_o, tau, kf_grad);
+  return ray_kf && n_kf ? 3 : 2;
 }
