@@ -95,7 +95,11 @@ __global__ void __launch_bounds__(256) encode_forward_kernel(LevelTable lv, cons
   tl_mark(ws.timeline, K_ENCODE, 1);
 }
 
-// S12, thread per (level, sample), level-major (see scatter_sample_level in table_ops.cuh).
+// S12, thread per (level, sample), level-major (see table_ops.cuh).  On DENSE (coarse) levels consecutive samples of a
+// ray sit in the same cell for several steps (level 0: ~6 samples per cell at config 3), and every sample of a cell adds
+// to the same eight entries: when a warp holds one dense level, the contributions of each run of equal cells are summed
+// with a segmented warp scan and only the run's first lane issues the reductions -- the L2 reduction rate is what bounds
+// this kernel (profiles/r1p), so fewer reductions is the only way to make it faster.
 template <int F>
 __global__ void __launch_bounds__(256) scatter_backward_kernel(LevelTable lv, float *__restrict__ grad, Workspace ws,
                                                                const uint32_t *__restrict__ d_S, uint32_t l0, uint32_t l1) {
@@ -105,11 +109,39 @@ __global__ void __launch_bounds__(256) scatter_backward_kernel(LevelTable lv, fl
   const uint64_t S = *d_S;
   const uint64_t total = S * (l1 - l0);
   const uint64_t pol_last = l2_evict_last();
-  for (uint64_t wi = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; wi < total;
-       wi += (uint64_t)gridDim.x * blockDim.x) {
-    const uint32_t l = l0 + (uint32_t)(wi / S);
-    const uint64_t s = wi - (uint64_t)(l - l0) * S;
-    scatter_sample_level<F>(lv, grad, ws, l, s, pol_last);
+  const uint32_t lane = threadIdx.x & 31;
+  const uint64_t stride = (uint64_t)gridDim.x * blockDim.x;
+  for (uint64_t wb = (uint64_t)blockIdx.x * blockDim.x + (threadIdx.x & ~31u); wb < total; wb += stride) {   // warp-uniform
+    const uint64_t wi = wb + lane;
+    const bool valid = wi < total;
+    const uint32_t l = l0 + (uint32_t)((valid ? wi : wb) / S);
+    const uint64_t s = (valid ? wi : wb) - (uint64_t)(l - l0) * S;
+    const uint32_t l_first = __shfl_sync(0xffffffffu, l, 0);
+    const bool one_dense_level = __all_sync(0xffffffffu, l == l_first) && lv.dense[l_first];
+    if (!one_dense_level) {
+      if (valid) scatter_sample_level<F>(lv, grad, ws, l, s, pol_last);
+      continue;
+    }
+    uint32_t slot[8];
+    float val[8][F];
+    corner_contributions<F>(lv, ws, l, s, slot, val);
+    // runs of equal cells (slot[0] identifies the cell on a dense level); invalid lanes form runs of their own
+    const uint32_t key = valid ? slot[0] : 0xffffffffu - lane;
+    const uint32_t prev = __shfl_up_sync(0xffffffffu, key, 1);
+    const uint32_t heads = __ballot_sync(0xffffffffu, lane == 0 || key != prev);
+    const uint32_t later = lane == 31 ? 0u : heads >> (lane + 1);
+    const uint32_t run_end = later ? lane + (uint32_t)__ffs(later) : 32u;      // first lane of the next run
+#pragma unroll
+    for (int d = 1; d < 32; d <<= 1) {   // segmented suffix sum: the run's first lane ends up with the run's total
+#pragma unroll
+      for (int k = 0; k < 8; ++k)
+#pragma unroll
+        for (int f = 0; f < F; ++f) {
+          const float o = __shfl_down_sync(0xffffffffu, val[k][f], d);
+          if (lane + d < run_end) val[k][f] += o;
+        }
+    }
+    if (valid && ((heads >> lane) & 1u)) issue_corner_reds<F>(lv, grad, l, slot, val, pol_last);
   }
   tl_mark(ws.timeline, K_SCATTER, 1);
 }

@@ -103,16 +103,17 @@ __device__ __forceinline__ void red_add_entry(float *p, const float g[F], uint64
   }
 }
 
-// S12 for one (sample, level): d theta[(offset_l + slot) F + f] += omega * dL/de[l F + f], eight vector reductions.
-// The touched set U is structural (every referenced entry, independent of the gradient's value): it is carried by
-// the gradient words themselves, see FieldParams in nsm_internal.cuh.
+// S12 for one cell of one level: the eight corner reductions d theta[(offset_l + slot) F + f] += val[corner][f].
+// Addends are canonicalised here (never -0.0, never near-subnormal; NaN stays NaN): the touched set U is structural
+// (every referenced entry, independent of the gradient's value) and is carried by the gradient words themselves, see
+// FieldParams in nsm_internal.cuh.
 template <int F>
-__device__ __forceinline__ void scatter_sample_level(const LevelTable &lv, float *__restrict__ grad, const Workspace &ws,
-                                                     uint32_t l, uint64_t s, uint64_t pol_last) {
-  CornerIndex ci = corner_index(lv, l, ws.s_x[s], ws.s_x[ws.cap + s], ws.s_x[2 * ws.cap + s]);
-  float de[F];
+__device__ __forceinline__ void issue_corner_reds(const LevelTable &lv, float *__restrict__ grad, uint32_t l, const uint32_t slot[8],
+                                                  float val[8][F], uint64_t pol_last) {
 #pragma unroll
-  for (int f = 0; f < F; ++f) de[f] = ws.de[(size_t)(l * F + f) * ws.cap + s];
+  for (int k = 0; k < 8; ++k)
+#pragma unroll
+    for (int f = 0; f < F; ++f) val[k][f] = fabsf(val[k][f]) < NSM_GRAD_MIN_ADDEND ? 0.0f : val[k][f];
   float *tab = grad + lv.offset[l] * F;
   if constexpr (F == 2) {
     // The two x-neighbour corners (k, k+1) are adjacent entries whenever their slots differ in bit 0 only (always on
@@ -121,37 +122,46 @@ __device__ __forceinline__ void scatter_sample_level(const LevelTable &lv, float
     const uint64_t e_l = lv.offset[l];
 #pragma unroll
     for (int k = 0; k < 8; k += 2) {
-      float g0[2], g1[2];
-      const float om0 = corner_weight(k, ci.w), om1 = corner_weight(k + 1, ci.w);
-#pragma unroll
-      for (int f = 0; f < 2; ++f) {
-        const float v0 = om0 * de[f], v1 = om1 * de[f];
-        g0[f] = fabsf(v0) < NSM_GRAD_MIN_ADDEND ? 0.0f : v0;   // never -0.0, never near-subnormal; NaN stays NaN
-        g1[f] = fabsf(v1) < NSM_GRAD_MIN_ADDEND ? 0.0f : v1;
-      }
-      const uint64_t a0 = e_l + ci.slot[k], a1 = e_l + ci.slot[k + 1];
+      const uint64_t a0 = e_l + slot[k], a1 = e_l + slot[k + 1];
       if ((a0 ^ a1) == 1ull) {
         float *p = grad + (a0 & ~1ull) * 2;
-        if (a0 & 1ull) red_hint_f4(p, make_float4(g1[0], g1[1], g0[0], g0[1]), pol_last);
-        else red_hint_f4(p, make_float4(g0[0], g0[1], g1[0], g1[1]), pol_last);
+        if (a0 & 1ull) red_hint_f4(p, make_float4(val[k + 1][0], val[k + 1][1], val[k][0], val[k][1]), pol_last);
+        else red_hint_f4(p, make_float4(val[k][0], val[k][1], val[k + 1][0], val[k + 1][1]), pol_last);
       } else {
-        red_add_entry<2>(tab + (size_t)ci.slot[k] * 2, g0, pol_last);
-        red_add_entry<2>(tab + (size_t)ci.slot[k + 1] * 2, g1, pol_last);
+        red_add_entry<2>(tab + (size_t)slot[k] * 2, val[k], pol_last);
+        red_add_entry<2>(tab + (size_t)slot[k + 1] * 2, val[k + 1], pol_last);
       }
     }
   } else {
 #pragma unroll
-    for (int k = 0; k < 8; ++k) {
-      float om = corner_weight(k, ci.w);
-      float g[F];
-#pragma unroll
-      for (int f = 0; f < F; ++f) {
-        const float v = om * de[f];
-        g[f] = fabsf(v) < NSM_GRAD_MIN_ADDEND ? 0.0f : v;   // never -0.0, never near-subnormal; NaN stays NaN
-      }
-      red_add_entry<F>(tab + (size_t)ci.slot[k] * F, g, pol_last);
-    }
+    for (int k = 0; k < 8; ++k) red_add_entry<F>(tab + (size_t)slot[k] * F, val[k], pol_last);
   }
+}
+
+// the corner slots of (sample s, level l) and its eight contributions omega_corner * dL/de[l F + f]
+template <int F>
+__device__ __forceinline__ void corner_contributions(const LevelTable &lv, const Workspace &ws, uint32_t l, uint64_t s,
+                                                     uint32_t slot[8], float val[8][F]) {
+  const CornerIndex ci = corner_index(lv, l, ws.s_x[s], ws.s_x[ws.cap + s], ws.s_x[2 * ws.cap + s]);
+  float de[F];
+#pragma unroll
+  for (int f = 0; f < F; ++f) de[f] = ws.de[(size_t)(l * F + f) * ws.cap + s];
+#pragma unroll
+  for (int k = 0; k < 8; ++k) {
+    slot[k] = ci.slot[k];
+    const float om = corner_weight(k, ci.w);
+#pragma unroll
+    for (int f = 0; f < F; ++f) val[k][f] = om * de[f];
+  }
+}
+
+template <int F>
+__device__ __forceinline__ void scatter_sample_level(const LevelTable &lv, float *__restrict__ grad, const Workspace &ws,
+                                                     uint32_t l, uint64_t s, uint64_t pol_last) {
+  uint32_t slot[8];
+  float val[8][F];
+  corner_contributions<F>(lv, ws, l, s, slot, val);
+  issue_corner_reds<F>(lv, grad, l, slot, val, pol_last);
 }
 
 constexpr int ADAM_CHUNK_FLOATS = 4096;
