@@ -30,21 +30,44 @@ __global__ void __launch_bounds__(256) encode_forward_kernel(LevelTable lv, cons
   const uint64_t total = S_it * lv.n_levels;
   const uint32_t LF = lv.n_levels * F;
   const uint64_t pol_first = l2_evict_first(), pol_normal = l2_evict_normal();
-  for (uint64_t wi = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; wi < total;
-       wi += (uint64_t)gridDim.x * blockDim.x) {
-    const uint32_t l = (uint32_t)(wi / S_it);
-    const uint64_t s = wi - (uint64_t)l * S_it;
+  const uint32_t lane = threadIdx.x & 31;
+  for (uint64_t wb = (uint64_t)blockIdx.x * blockDim.x + (threadIdx.x & ~31u); wb < total;
+       wb += (uint64_t)gridDim.x * blockDim.x) {   // warp-uniform trip count: the dense-level path below uses warp collectives
+    const uint64_t wi = wb + lane;
+    const bool in_range = wi < total;
+    const uint32_t l = (uint32_t)((in_range ? wi : wb) / S_it);
+    const uint64_t s = (in_range ? wi : wb) - (uint64_t)l * S_it;
+    const bool live = in_range && s < S;
     float acc[F];
 #pragma unroll
     for (int f = 0; f < F; ++f) acc[f] = 0.0f;
-    if (s < S) {
-      CornerIndex ci = corner_index(lv, l, ws.s_x[s], ws.s_x[ws.cap + s], ws.s_x[2 * ws.cap + s]);
+    // On a dense (coarse) level consecutive samples of a ray share their cell for several steps: when the warp holds one
+    // dense level, only the first lane of each run of equal cells gathers the eight corners, the others take them by
+    // shuffle (the L2's random-access rate bounds this kernel, profiles/r1p).
+    const uint32_t l_first = __shfl_sync(0xffffffffu, l, 0);
+    const bool one_dense_level = __all_sync(0xffffffffu, l == l_first) && lv.dense[l_first];
+    CornerIndex ci;
+    if (live) ci = corner_index(lv, l, ws.s_x[s], ws.s_x[ws.cap + s], ws.s_x[2 * ws.cap + s]);
+    uint32_t head_lane = lane;
+    bool gathers = live;
+    if (one_dense_level) {
+      const uint32_t key = live ? ci.slot[0] : 0xffffffffu - lane;
+      const uint32_t prev = __shfl_up_sync(0xffffffffu, key, 1);
+      const uint32_t heads = __ballot_sync(0xffffffffu, lane == 0 || key != prev);
+      head_lane = 31u - (uint32_t)__clz(heads & (0xffffffffu >> (31u - lane)));
+      gathers = live && head_lane == lane;
+    }
+    float v[8][F];
+#pragma unroll
+    for (int k = 0; k < 8; ++k)
+#pragma unroll
+      for (int f = 0; f < F; ++f) v[k][f] = 0.f;
+    if (gathers) {
       const float *tab = theta + lv.offset[l] * F;
-      float v[8][F];
       // coarse (dense) levels are re-read every step: default policy; hashed levels stream through L2
       const uint64_t pol = lv.dense[l] ? pol_normal : pol_first;
       if constexpr (F == 2) {
-        // x-neighbour corners that form an aligned pair of entries come in with one 16-byte load (see scatter_sample_level)
+        // x-neighbour corners that form an aligned pair of entries come in with one 16-byte load (see issue_corner_reds)
         const uint64_t e_l = lv.offset[l];
 #pragma unroll
         for (int k = 0; k < 8; k += 2) {
@@ -63,6 +86,14 @@ __global__ void __launch_bounds__(256) encode_forward_kernel(LevelTable lv, cons
 #pragma unroll
         for (int k = 0; k < 8; ++k) load_entry_hint<F>(tab + (size_t)ci.slot[k] * F, v[k], pol);  // 8 gathers in flight
       }
+    }
+    if (one_dense_level) {
+#pragma unroll
+      for (int k = 0; k < 8; ++k)
+#pragma unroll
+        for (int f = 0; f < F; ++f) v[k][f] = __shfl_sync(0xffffffffu, v[k][f], head_lane);
+    }
+    if (live) {
 #pragma unroll
       for (int k = 0; k < 8; ++k) {
         float om = corner_weight(k, ci.w);
@@ -70,6 +101,7 @@ __global__ void __launch_bounds__(256) encode_forward_kernel(LevelTable lv, cons
         for (int f = 0; f < F; ++f) acc[f] = fmaf(om, v[k][f], acc[f]);
       }
     }
+    if (!in_range) continue;
     if (MODE == 0) {
 #pragma unroll
       for (int f = 0; f < F; ++f) ws.e[(size_t)(l * F + f) * ws.cap + s] = acc[f];
