@@ -272,7 +272,22 @@ struct FwdSmem {
 // hardware's lane-quarter rule -- and the column half (w >> 2) of every 64-wide layer, so the
 // accumulator read-back / two-term split / store of a layer is shared by two warps per SM
 // sub-partition (four with the second resident CTA).
-template <typename T>
+// SPLIT = true: two-term (hi + lo) operands, three MMA groups per layer -- the training forward, whose ReLU masks the
+// backward pass reuses and must agree with the float64 oracle.  SPLIT = false: plain 16-bit operands (one MMA group, half
+// the read-back work and half the operand bytes) for the forward-only uses: render (S15) and the occupancy refresh.
+template <bool SPLIT>
+__device__ __forceinline__ void issue_fwd(uint32_t tmem_d, uint32_t a, uint32_t a_lo, uint32_t b, uint32_t b_lo, uint32_t K, uint32_t N,
+                                          uint32_t NP, uint32_t fmt, uint32_t bar) {
+  if constexpr (SPLIT) issue_layer_split(tmem_d, a, a_lo, b, b_lo, K, N, NP, fmt, bar);
+  else issue_layer(tmem_d, a, b, K, N, NP, fmt, bar);
+}
+template <typename T, bool RELU, bool SPLIT>
+__device__ __forceinline__ void emit_fwd(float *v, uint8_t *tile, uint32_t lo_off, uint8_t *blob, uint32_t row, uint32_t c0, bool valid) {
+  if constexpr (SPLIT) emit16s<T, RELU>(v, tile, lo_off, blob, row, c0, valid);
+  else emit16<T, RELU>(v, tile, blob, row, c0, valid);
+}
+
+template <typename T, bool SPLIT>
 __global__ void __launch_bounds__(FWD_THREADS, 2) mlp_forward_tc_kernel(MlpShape ms, const float *__restrict__ dirs, Workspace ws,
                                                                        const uint32_t *__restrict__ d_S, int density_only,
                                                                        int save_blobs) {
@@ -282,7 +297,8 @@ __global__ void __launch_bounds__(FWD_THREADS, 2) mlp_forward_tc_kernel(MlpShape
   const uint32_t sbase = smem_u32(smem);
   const uint32_t bar_mma = sbase + FwdSmem::bar_mma, bar_w = sbase + FwdSmem::bar_w, bar_e = sbase + FwdSmem::bar_e;
   const uint32_t LF = ms.LF;
-  const uint32_t e_half = LF * ROWS * 2, e_bytes = 2 * e_half;   // hi | lo
+  const uint32_t e_half = LF * ROWS * 2, e_stride = 2 * e_half;   // the encoder writes hi | lo per tile
+  const uint32_t e_bytes = SPLIT ? e_stride : e_half, w_bytes = SPLIT ? 2 * WImg::f_total : WImg::f_total;
   // Before pdl_wait(): only data produced at least two kernels back (S from the marcher, the weight images).
   const uint64_t S = *d_S;
   const bool has_tiles = (uint64_t)blockIdx.x * ROWS < S;
@@ -290,8 +306,8 @@ __global__ void __launch_bounds__(FWD_THREADS, 2) mlp_forward_tc_kernel(MlpShape
     if (tid == 0) {
       mbar_init(bar_mma, 1); mbar_init(bar_w, 1); mbar_init(bar_e, 1);
       fence_async_smem();
-      mbar_expect_tx(bar_w, 2 * WImg::f_total);
-      bulk_g2s(sbase + FwdSmem::w, ws.wimg_fwd, 2 * WImg::f_total, bar_w);
+      mbar_expect_tx(bar_w, w_bytes);
+      bulk_g2s(sbase + FwdSmem::w, ws.wimg_fwd, w_bytes, bar_w);
     }
     if (warp == 0) tmem_alloc<FWD_COLS>(sbase + FwdSmem::tmem);
   }
@@ -301,7 +317,7 @@ __global__ void __launch_bounds__(FWD_THREADS, 2) mlp_forward_tc_kernel(MlpShape
   tl_mark(ws.timeline, K_MLP_FWD, 0);
   if (tid == 0) {   // the encoder's output: after the wait
     mbar_expect_tx(bar_e, e_bytes);
-    bulk_g2s(sbase + FwdSmem::bufA, ws.blob_e + (size_t)blockIdx.x * e_bytes, e_bytes, bar_e);
+    bulk_g2s(sbase + FwdSmem::bufA, ws.blob_e + (size_t)blockIdx.x * e_stride, e_bytes, bar_e);
   }
   fence_before();
   __syncthreads();
@@ -323,7 +339,7 @@ __global__ void __launch_bounds__(FWD_THREADS, 2) mlp_forward_tc_kernel(MlpShape
     if (tid == 0) {
       mbar_wait(bar_e, ph_e);
       fence_after();
-      issue_layer_split(tmem_base + COL_D1, sA, e_half, sW + WImg::f_d1, WImg::f_total, LF, H, H, fmt, bar_mma);
+      issue_fwd<SPLIT>(tmem_base + COL_D1, sA, e_half, sW + WImg::f_d1, WImg::f_total, LF, H, H, fmt, bar_mma);
     }
     ph_e ^= 1;
     mbar_wait(bar_mma, ph_mma); ph_mma ^= 1; fence_after();
@@ -332,10 +348,10 @@ __global__ void __launch_bounds__(FWD_THREADS, 2) mlp_forward_tc_kernel(MlpShape
     for (uint32_t c0 = 0; c0 < 32; c0 += 16) {
       tmem_ld16(tlane + COL_D1 + cb + c0, v);
       tmem_ld_wait();
-      emit16s<T, true>(v, bufB, TILE_BYTES, blob_hd, row, cb + c0, valid);
+      emit_fwd<T, true, SPLIT>(v, bufB, TILE_BYTES, blob_hd, row, cb + c0, valid);
     }
     fence_async_smem(); fence_before(); __syncthreads();
-    if (tid == 0) { fence_after(); issue_layer_split(tmem_base + COL_D2, sB, TILE_BYTES, sW + WImg::f_d2, WImg::f_total, H, DO, DO, fmt, bar_mma); }
+    if (tid == 0) { fence_after(); issue_fwd<SPLIT>(tmem_base + COL_D2, sB, TILE_BYTES, sW + WImg::f_d2, WImg::f_total, H, DO, DO, fmt, bar_mma); }
     mbar_wait(bar_mma, ph_mma); ph_mma ^= 1; fence_after();
     float g[16];
     tmem_ld16(tlane + COL_D2, g);
@@ -345,7 +361,7 @@ __global__ void __launch_bounds__(FWD_THREADS, 2) mlp_forward_tc_kernel(MlpShape
       fence_before(); __syncthreads();
       if (tid == 0) {   // buffer A is free: the CTA's next encoder tile
         const uint64_t nxt = tile + gridDim.x;
-        if (nxt * ROWS < S) { mbar_expect_tx(bar_e, e_bytes); bulk_g2s(sA, ws.blob_e + (size_t)nxt * e_bytes, e_bytes, bar_e); }
+        if (nxt * ROWS < S) { mbar_expect_tx(bar_e, e_bytes); bulk_g2s(sA, ws.blob_e + (size_t)nxt * e_stride, e_bytes, bar_e); }
       }
       continue;
     }
@@ -368,39 +384,39 @@ __global__ void __launch_bounds__(FWD_THREADS, 2) mlp_forward_tc_kernel(MlpShape
 #pragma unroll
       for (int j = 0; j < 16; ++j) ci[15 + j] = Y[j];
       uint8_t *blob_ci = save_blobs ? ws.blob_ci + (size_t)tile * (CIP * ROWS * 2) : nullptr;
-      if (half == 0) emit16s<T, false>(ci, bufA, TILE_BYTES, blob_ci, row, 0, valid);
-      else emit16s<T, false>(ci + 16, bufA, TILE_BYTES, blob_ci, row, 16, valid);
+      if (half == 0) emit_fwd<T, false, SPLIT>(ci, bufA, TILE_BYTES, blob_ci, row, 0, valid);
+      else emit_fwd<T, false, SPLIT>(ci + 16, bufA, TILE_BYTES, blob_ci, row, 16, valid);
     }
     fence_async_smem(); fence_before(); __syncthreads();
-    if (tid == 0) { fence_after(); issue_layer_split(tmem_base + COL_C1, sA, TILE_BYTES, sW + WImg::f_c1, WImg::f_total, CIP, H, H, fmt, bar_mma); }
+    if (tid == 0) { fence_after(); issue_fwd<SPLIT>(tmem_base + COL_C1, sA, TILE_BYTES, sW + WImg::f_c1, WImg::f_total, CIP, H, H, fmt, bar_mma); }
     mbar_wait(bar_mma, ph_mma); ph_mma ^= 1; fence_after();
     uint8_t *blob_h1 = save_blobs ? ws.blob_h1 + (size_t)tile * (H * ROWS * 2) : nullptr;
 #pragma unroll
     for (uint32_t c0 = 0; c0 < 32; c0 += 16) {
       tmem_ld16(tlane + COL_C1 + cb + c0, v);
       tmem_ld_wait();
-      emit16s<T, true>(v, bufB, TILE_BYTES, blob_h1, row, cb + c0, valid);
+      emit_fwd<T, true, SPLIT>(v, bufB, TILE_BYTES, blob_h1, row, cb + c0, valid);
     }
     uint32_t sLast = sB;
     if (ms.n_color_layers == 2) {
       fence_async_smem(); fence_before(); __syncthreads();
-      if (tid == 0) { fence_after(); issue_layer_split(tmem_base + COL_C2, sB, TILE_BYTES, sW + WImg::f_c2, WImg::f_total, H, H, H, fmt, bar_mma); }
+      if (tid == 0) { fence_after(); issue_fwd<SPLIT>(tmem_base + COL_C2, sB, TILE_BYTES, sW + WImg::f_c2, WImg::f_total, H, H, H, fmt, bar_mma); }
       mbar_wait(bar_mma, ph_mma); ph_mma ^= 1; fence_after();
       uint8_t *blob_h2 = save_blobs ? ws.blob_h2 + (size_t)tile * (H * ROWS * 2) : nullptr;
 #pragma unroll
       for (uint32_t c0 = 0; c0 < 32; c0 += 16) {
         tmem_ld16(tlane + COL_C2 + cb + c0, v);
         tmem_ld_wait();
-        emit16s<T, true>(v, bufA, TILE_BYTES, blob_h2, row, cb + c0, valid);
+        emit_fwd<T, true, SPLIT>(v, bufA, TILE_BYTES, blob_h2, row, cb + c0, valid);
       }
       sLast = sA;
     }
     fence_async_smem(); fence_before(); __syncthreads();
-    if (tid == 0) { fence_after(); issue_layer_split(tmem_base + COL_C3, sLast, TILE_BYTES, sW + WImg::f_c3, WImg::f_total, H, 16, 16, fmt, bar_mma); }
+    if (tid == 0) { fence_after(); issue_fwd<SPLIT>(tmem_base + COL_C3, sLast, TILE_BYTES, sW + WImg::f_c3, WImg::f_total, H, 16, 16, fmt, bar_mma); }
     mbar_wait(bar_mma, ph_mma); ph_mma ^= 1; fence_after();
     if (tid == 0) {   // every buffer is free: the CTA's next encoder tile
       const uint64_t nxt = tile + gridDim.x;
-      if (nxt * ROWS < S) { mbar_expect_tx(bar_e, e_bytes); bulk_g2s(sA, ws.blob_e + (size_t)nxt * e_bytes, e_bytes, bar_e); }
+      if (nxt * ROWS < S) { mbar_expect_tx(bar_e, e_bytes); bulk_g2s(sA, ws.blob_e + (size_t)nxt * e_stride, e_bytes, bar_e); }
     }
     if (half == 0) {
       tmem_ld16(tlane + COL_C3, v);
@@ -773,17 +789,25 @@ int launch_reduce_wgrad(const MlpShape &ms, const Workspace &ws, float *grad_mlp
 
 uint32_t mlp_tc_backward_ctas(int n_sms) { return 2u * (uint32_t)n_sms; }
 
+template <typename T, bool SPLIT>
+static void launch_fwd_variant(const MlpShape &ms, const float *dirs, const Workspace &ws, const uint32_t *d_S, int density_only,
+                               int save_blobs, int n_sms, cudaStream_t st) {
+  static const cudaError_t once = cudaFuncSetAttribute(mlp_forward_tc_kernel<T, SPLIT>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                                       (int)FwdSmem::total);
+  (void)once;
+  launch_pdl(mlp_forward_tc_kernel<T, SPLIT>, dim3(2 * n_sms), dim3(FWD_THREADS), (size_t)FwdSmem::total, st, ms, dirs, ws, d_S,
+             density_only, save_blobs);
+}
+
 int launch_mlp_forward_tc(const MlpShape &ms, int bf16, const float *dirs, const Workspace &ws, const uint32_t *d_S,
                           int density_only, int save_blobs, int n_sms, cudaStream_t st) {
-  const size_t smem = FwdSmem::total;
+  // the training forward (save_blobs) runs two-term operands; render and occupancy refresh run plain 16-bit operands
   if (bf16) {
-    static const cudaError_t once = cudaFuncSetAttribute(mlp_forward_tc_kernel<__nv_bfloat16>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    (void)once;
-    launch_pdl(mlp_forward_tc_kernel<__nv_bfloat16>, dim3(2 * n_sms), dim3(FWD_THREADS), smem, st, ms, dirs, ws, d_S, density_only, save_blobs);
+    if (save_blobs) launch_fwd_variant<__nv_bfloat16, true>(ms, dirs, ws, d_S, density_only, save_blobs, n_sms, st);
+    else launch_fwd_variant<__nv_bfloat16, false>(ms, dirs, ws, d_S, density_only, save_blobs, n_sms, st);
   } else {
-    static const cudaError_t once = cudaFuncSetAttribute(mlp_forward_tc_kernel<__half>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    (void)once;
-    launch_pdl(mlp_forward_tc_kernel<__half>, dim3(2 * n_sms), dim3(FWD_THREADS), smem, st, ms, dirs, ws, d_S, density_only, save_blobs);
+    if (save_blobs) launch_fwd_variant<__half, true>(ms, dirs, ws, d_S, density_only, save_blobs, n_sms, st);
+    else launch_fwd_variant<__half, false>(ms, dirs, ws, d_S, density_only, save_blobs, n_sms, st);
   }
   return 1;
 }
