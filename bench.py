@@ -202,8 +202,8 @@ def kernel_model(name, S, R, K, L, F, LF, U, E, mac, n_mlp):
 # DRAM bytes (dram__bytes_read.sum + dram__bytes_write.sum) per launch from the `ncu --set full` capture of
 # profiles/r1q_ncu_full.md (config 2; cold cache, as ncu flushes before every kernel).  bench.py cannot run ncu:
 # these are recorded values, refreshed with each committed profile.
-NCU_TRAFFIC_CFG2 = {"adam_table": 223875584, "scatter": 37828864, "encode": 40565760, "mlp_bwd": 11985152, "mlp_fwd": 3023104,
-                    "adam_mlp": 6556416, "composite": 643328, "march": 381952}
+NCU_TRAFFIC_CFG2 = {"adam_table": 223383296, "scatter": 38011904, "encode": 40556800, "mlp_bwd": 11984640, "mlp_fwd": 3022592,
+                    "adam_mlp": 6555904, "composite": 643072, "march": 381952}
 
 
 def run_probe_l2():
