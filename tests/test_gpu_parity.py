@@ -669,3 +669,31 @@ def test_occupancy_decay_update_against_the_oracle(nsm):
     with pytest.raises(nsm.NsmError):
         f.nsm_update_occupancy_decay(0, 0.9)
     f.close()
+
+
+# ---------------------------------------------------------------------------- measurement helpers of the boundary
+
+def test_timeline_and_l2_probe(nsm, monkeypatch):
+    """nsm_debug_timeline: with NSM_TIMELINE=1 every hot-path kernel of a step stamps start <= end, and the kernels of one
+    stream appear in launch order; nsm_probe_l2 returns a plausible rate (cache-resident faster than DRAM-resident)."""
+    monkeypatch.setenv("NSM_TIMELINE", "1")
+    w = configs.config2(R=1024, K=128)
+    f = nsm.Field(w.field, "cuda:0")
+    f.nsm_set_params(configs.init_params(2, f.n_table, f.mlp_shapes()))
+    f.nsm_update_occupancy(nsm.NSM_OCC_SET, w.bits)
+    for _ in range(3):
+        f.nsm_train_step(nsm.DeviceBatch(w.batches[0]), w.lambda_d)
+    tl = f.nsm_debug_timeline().astype(np.int64)
+    a = tl[3 % 64]                                           # slot of step 3
+    names = ["march", "encode", "mlp_fwd", "composite", "mlp_bwd", "scatter", "adam_table", "adam_mlp"]
+    start, end = a[0][:8], a[1][:8]
+    assert np.all(end >= start) and np.all(end > 0), dict(zip(names, zip(start, end)))
+    order = [0, 1, 2, 3, 4, 5, 6]                            # the field's stream: march .. adam_table
+    assert all(start[order[i + 1]] >= start[order[i]] for i in range(6)), start
+    assert start[7] >= end[4]                                # the MLP Adam (side stream) starts after the MLP backward
+    f.close()
+    monkeypatch.delenv("NSM_TIMELINE")
+    fast = nsm.probe_l2(24 << 20, 1 << 21, False)
+    slow = nsm.probe_l2(1 << 30, 1 << 21, False)
+    red = nsm.probe_l2(24 << 20, 1 << 21, True)
+    assert 5e9 < slow < fast < 1e12 and 5e9 < red < 1e12, (fast, slow, red)
