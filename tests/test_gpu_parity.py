@@ -697,3 +697,25 @@ def test_timeline_and_l2_probe(nsm, monkeypatch):
     slow = nsm.probe_l2(1 << 30, 1 << 21, False)
     red = nsm.probe_l2(24 << 20, 1 << 21, True)
     assert 5e9 < slow < fast < 1e12 and 5e9 < red < 1e12, (fast, slow, red)
+
+
+@pytest.mark.parametrize("F,L,log2T", [(1, 6, 12), (8, 3, 11), (4, 5, 10)])
+def test_other_feature_widths(nsm, F, L, log2T):
+    """The table kernels are templated on F = 1, 2, 4, 8 (configs 1-3, 5 use 2, config 4 uses 4): backward parity (P1-P4) and
+    one Adam step for the widths the configurations do not cover, dense and hashed levels both present."""
+    w = configs.config1(variant_b=True)
+    fc = replace(w.field, n_features=F, n_levels=L, log2_table_size=log2T, n_min=4, n_max=48)
+    w = replace(w, field=fc)
+    f, O, theta0 = make_pair(nsm, w, seed=20 + F, table_scale=0.2)
+    assert any(O.res[l] ** 3 > (1 << log2T) for l in range(L)) and (O.res[0] + 1) ** 3 <= (1 << log2T)   # hashed and dense
+    b = w.batches[0]
+    check_backward(nsm, f, O, b, w.lambda_d, 1e-4)
+    f.nsm_apply_adam()
+    O.train_step(b, w.lambda_d)
+    th, m, v, step = f.nsm_get_params()
+    assert step == 1
+    assert_close("m", m, O.m, 1e-4)
+    assert_close("v", v, O.v, 2e-4)
+    untouched = np.abs(O.m[:O.n_table]) == 0
+    assert np.array_equal(th[:O.n_table][untouched], theta0[:O.n_table][untouched])
+    f.close()
