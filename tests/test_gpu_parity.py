@@ -309,11 +309,12 @@ def test_occupancy_set_get_roundtrip(nsm):
     f.close()
 
 
-def test_render_parity(nsm):
+@pytest.mark.parametrize("precision", [1, 2])
+def test_render_parity(nsm, precision):
     """P8: nsm_render vs the oracle's S15 on a pixel-strided view of the room, field = a few GPU
-    training steps on config-3-style data (parameters copied to the oracle)."""
+    training steps on config-3-style data (parameters copied to the oracle); fp16 and bf16 tensor-core MLPs."""
     w = configs.config3(R=2048, K=128, n_keyframes=3, n_batches=6, width=300, height=170)
-    fc = replace(w.field, bg=(0.1, 0.2, 0.3), max_candidates=256)
+    fc = replace(w.field, bg=(0.1, 0.2, 0.3), max_candidates=256, mlp_precision=precision)
     w = replace(w, field=fc)
     f, O, theta0 = make_pair(nsm, w, seed=6, table_scale=0.05)
     for b in w.batches:
