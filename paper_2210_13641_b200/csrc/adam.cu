@@ -17,8 +17,8 @@ using namespace tableops;
 //     (index + gradient), warp-aggregated.
 //  2. The block walks the compact list: every thread has a touched entry, loads its theta (compact
 //     array) and its moment record (m | v; 16 bytes for F = 2; two entries in flight per thread),
-//     updates and stores them.  The whole gradient chunk is then reset to -0.0f with coalesced
-//     stores, so the next step's scatter starts from "untouched" without a separate pass.
+//     updates and stores them.  The 16-byte gradient words that held a touched entry are then reset to
+//     -0.0f, so the next step's scatter starts from "untouched" without a separate pass.
 // sparse = 0 (dense Adam, textbook): every entry goes through phase 2.
 template <int F>
 __global__ void __launch_bounds__(ADAM_THREADS) adam_table_kernel(float *__restrict__ theta, float *__restrict__ mv, float *__restrict__ grad,

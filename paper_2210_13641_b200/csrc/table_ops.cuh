@@ -224,6 +224,7 @@ __device__ __forceinline__ void adam_chunk(float *__restrict__ theta, float *__r
   const uint64_t pol_ld = l2_evict_normal(), pol_first = l2_evict_first(), pol_last = pol_ld;
   if (tid == 0) *cnt_p = 0;
   float4 gv[NV];
+  uint32_t dirty = 0;                                  // bit j: the thread's j-th 16-byte word holds a touched entry
 #pragma unroll
   for (int j = 0; j < NV; ++j) {
     const uint32_t q = j * ADAM_THREADS + tid;         // float4 index inside the chunk
@@ -240,6 +241,7 @@ __device__ __forceinline__ void adam_chunk(float *__restrict__ theta, float *__r
       for (int i = 0; i < EPV; ++i) {
         const uint32_t le = q * EPV + i;               // local entry index
         const bool t = (e_base + le < n_entries) && (!sparse || __float_as_uint(w[i * F]) != NSM_GRAD_UNTOUCHED);
+        if (t) dirty |= 1u << j;
         const uint32_t mk = __ballot_sync(0xffffffffu, t);
         uint32_t base = 0;
         if (lane == 0 && mk) base = atomicAdd(cnt_p, (uint32_t)__popc(mk));
@@ -255,6 +257,7 @@ __device__ __forceinline__ void adam_chunk(float *__restrict__ theta, float *__r
       const uint32_t le = q >> 1;
       const uint32_t first_word = __float_as_uint(__shfl_sync(0xffffffffu, w[0], lane & ~1u));
       const bool t = (e_base + le < n_entries) && (!sparse || first_word != NSM_GRAD_UNTOUCHED);
+      if (t) dirty |= 1u << j;
       const uint32_t mk = __ballot_sync(0xffffffffu, t && !(lane & 1u));
       uint32_t base = 0;
       if (lane == 0 && mk) base = atomicAdd(cnt_p, (uint32_t)__popc(mk));
@@ -286,7 +289,9 @@ __device__ __forceinline__ void adam_chunk(float *__restrict__ theta, float *__r
 #pragma unroll
   for (int j = 0; j < NV; ++j) {
     const uint32_t q = j * ADAM_THREADS + tid;
-    if (e_base * F + 4ull * q < n_float) st_hint_f4(o4 + 4 * q, make_float4(nz, nz, nz, nz), pol_last);
+    // only the words that held a touched entry: the others are -0.0 already (with tables far larger than the L2 the
+    // dense rewrite was half of this kernel's DRAM traffic)
+    if (((dirty >> j) & 1u) && e_base * F + 4ull * q < n_float) st_hint_f4(o4 + 4 * q, make_float4(nz, nz, nz, nz), pol_last);
   }
 }
 
