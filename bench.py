@@ -202,8 +202,8 @@ def kernel_model(name, S, R, K, L, F, LF, U, E, mac, n_mlp):
 # DRAM bytes (dram__bytes_read.sum + dram__bytes_write.sum) per launch from the `ncu --set full` capture of
 # profiles/r1q_ncu_full.md (config 2; cold cache, as ncu flushes before every kernel).  bench.py cannot run ncu:
 # these are recorded values, refreshed with each committed profile.
-NCU_TRAFFIC_CFG2 = {"adam_table": 223383296, "scatter": 38011904, "encode": 40556800, "mlp_bwd": 11984640, "mlp_fwd": 3022592,
-                    "adam_mlp": 6555904, "composite": 643072, "march": 381952}
+NCU_TRAFFIC_CFG2 = {"adam_table": 213411328, "scatter": 37968128, "encode": 40532736, "mlp_bwd": 11986432, "mlp_fwd": 3022336,
+                    "adam_mlp": 6556160, "composite": 643584, "march": 381952}
 
 
 def run_probe_l2():
