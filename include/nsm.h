@@ -20,7 +20,8 @@
  *     pointer owned by the caller (e.g. torch.Tensor.data_ptr()); the *_host entry points take
  *     HOST pointers instead and perform the copies themselves.  The library never retains a
  *     caller pointer past the call.
- *   - The field owns parameters, Adam state, occupancy bits and workspace.
+ *   - The field owns parameters, Adam state, occupancy bits and workspace.  A field is used from one host thread
+ *     at a time (different fields may be driven from different threads).
  *   - All work is enqueued on the CUDA stream given at creation (plus an internal side stream that
  *     is joined back into it before the call returns); calls return without waiting unless a host
  *     stats pointer is passed or the entry point takes host buffers.  Such a call waits until the

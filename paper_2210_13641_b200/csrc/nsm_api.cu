@@ -46,7 +46,7 @@ uint32_t g_pdl_mask = [] {
   const char *e = std::getenv("NSM_PDL_MASK");
   return e ? (uint32_t)std::strtoul(e, nullptr, 0) : 0xdeu;
 }();
-int g_cur_kernel = 0;
+thread_local int g_cur_kernel = 0;   // kernel class of the launch in progress on this host thread (RUN macro)
 
 static const char *kKernelNames[K_COUNT] = {"march", "encode", "mlp_fwd", "composite",
                                             "mlp_bwd", "scatter", "adam_table", "adam_mlp", "occupancy", "debug", "sample", "pose"};

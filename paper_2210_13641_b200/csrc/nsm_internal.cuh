@@ -163,7 +163,7 @@ __device__ __forceinline__ void pdl_trigger() { asm volatile("griddepcontrol.lau
 
 // Which kernel classes (bit = KernelId) are launched with the PDL attribute; NSM_PDL_MASK overrides (tuning knob).
 extern uint32_t g_pdl_mask;
-extern int g_cur_kernel;
+extern thread_local int g_cur_kernel;
 
 template <typename... KArgs, typename... Args>
 inline cudaError_t launch_pdl(void (*kernel)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t st, Args... args) {
