@@ -343,6 +343,10 @@ __global__ void __launch_bounds__(FWD_THREADS, 2) mlp_forward_tc_kernel(MlpShape
     }
     ph_e ^= 1;
     mbar_wait(bar_mma, ph_mma); ph_mma ^= 1; fence_after();
+    if (density_only && tid == 0) {   // the density layers never write buffer A again: fetch the CTA's next encoder tile now
+      const uint64_t nxt = tile + gridDim.x;
+      if (nxt * ROWS < S) { mbar_expect_tx(bar_e, e_bytes); bulk_g2s(sA, ws.blob_e + (size_t)nxt * e_stride, e_bytes, bar_e); }
+    }
     uint8_t *blob_hd = (save_blobs && !density_only) ? ws.blob_hd + (size_t)tile * (H * ROWS * 2) : nullptr;
 #pragma unroll
     for (uint32_t c0 = 0; c0 < 32; c0 += 16) {
@@ -358,11 +362,7 @@ __global__ void __launch_bounds__(FWD_THREADS, 2) mlp_forward_tc_kernel(MlpShape
     tmem_ld_wait();
     if (valid && half == 0) ws.sigma[s] = expf(fminf(fmaxf(g[0], -15.f), 15.f));
     if (density_only) {
-      fence_before(); __syncthreads();
-      if (tid == 0) {   // buffer A is free: the CTA's next encoder tile
-        const uint64_t nxt = tile + gridDim.x;
-        if (nxt * ROWS < S) { mbar_expect_tx(bar_e, e_bytes); bulk_g2s(sA, ws.blob_e + (size_t)nxt * e_stride, e_bytes, bar_e); }
-      }
+      fence_before(); __syncthreads();   // all reads of COL_D2 are done before the next tile's MMAs
       continue;
     }
     // ---- colour input [g slice, Y(d), 0 pad] -> buffer A (K = 32); each column half emits its 16 columns
