@@ -125,7 +125,8 @@ typedef enum {
   NSM_DBG_TOUCHED = 18   /* u8  [n_entries] valid after nsm_backward */
 } nsm_debug_item;
 
-/* Create a field on the current CUDA device.  cuda_stream: a cudaStream_t (NULL = default
+/* Create a field on the current CUDA device (which must be an sm_100 part: the library holds sm_100a code only); the
+ * field stays on that device and every later call makes it current.  cuda_stream: a cudaStream_t (NULL = default
  * stream).  Parameters start at zero (tables) / zero (MLPs): upload theta_0 with
  * nsm_set_params.  Occupancy starts FULL.  Fails with NSM_ERR_INVALID_ARG on a bad config,
  * NSM_ERR_UNIMPLEMENTED on an unsupported shape, NSM_ERR_OOM / NSM_ERR_CUDA otherwise. */
@@ -148,23 +149,20 @@ nsm_status nsm_train_step(nsm_field *f, const nsm_ray_batch *batch, float lambda
 nsm_status nsm_train_step_host(nsm_field *f, const nsm_ray_batch *host_batch, float lambda_d,
                                nsm_step_stats *host_stats);
 
-/* Debug: with NSM_TIMELINE=1 in the environment at nsm_create_field, every hot-path kernel stamps its first
- * block's start and last block's end (%globaltimer, ns) into a ring of the last 64 training steps.  h_out (HOST)
- * receives 64 x [2][n_kernels] words, slot = step % 64, kernel classes in the order of nsm_profile_read; a
- * start of ~0 / end of 0 means "did not run".  Synchronises.  Costs a few atomics per block: not for timing runs. */
+/* Debug: with NSM_OPT_DEBUG_TIMELINE set, every hot-path kernel stamps its first block's start and last block's end
+ * (%globaltimer, ns) into a ring of the last 64 training steps.  h_out (HOST) receives 64 x [2][n_kernels] words,
+ * slot = step % 64, kernel classes in the order of nsm_profile_read; a start of ~0 / end of 0 means "did not run".
+ * Synchronises.  Costs a few atomics per block: not for timing runs. */
 nsm_status nsm_debug_timeline(nsm_field *f, uint64_t *h_out, uint64_t capacity_words, uint32_t *n_kernels);
-
-/* Micro-benchmark behind the L2 figures the rooflines of S4 / S12 are quoted against (MEASURED_PEAKS.json has HBM and
- * bf16 only): n_accesses random 8-byte gathers (reductions = 0) or red.global.add.v2.f32 (reductions = 1) over a
- * scratch table of table_bytes; *seconds_out = best of 8 timed launches after 4 warm-up launches.  Needs no field. */
-nsm_status nsm_probe_l2(uint64_t table_bytes, uint64_t n_accesses, int reductions, double *seconds_out);
 
 /* ---- Row f4: decayed partial occupancy refresh (the paper is silent; [17] keeps a decayed running maximum of the
  * density and refreshes part of the grid per update).  The library keeps a running density per cell, seeded by
  * nsm_update_occupancy(NSM_OCC_FROM_FIELD).  One call:  every cell  grid <- decay * grid;  the cells
  * c = (k mod n_subsets) + j * n_subsets (k = number of decay updates since the last full refresh)
  * grid <- max(grid, sigma(cell centre));  bit = grid > occ_sigma_threshold.  n_subsets consecutive calls visit every
- * cell exactly once; (n_subsets = 1, decay = 0) equals FROM_FIELD.  Costs G^3 / n_subsets field evaluations. */
+ * cell exactly once; (n_subsets = 1, decay = 0) equals FROM_FIELD.  Costs G^3 / n_subsets field evaluations.
+ * NSM_OCC_SET and NSM_OCC_FULL discard the running grid: until the next FROM_FIELD pass has seeded it again this call
+ * fails with NSM_ERR_INVALID_ARG (a partial pass would cull every cell it does not visit). */
 nsm_status nsm_update_occupancy_decay(nsm_field *f, uint32_t n_subsets, float decay);
 /* The running density grid [G^3] (DEVICE output), for inspection and parity. */
 nsm_status nsm_get_occupancy_grid(nsm_field *f, float *d_grid);
@@ -221,7 +219,9 @@ nsm_status nsm_get_keyframe_pose(nsm_field *f, uint32_t index, float *h_R, float
 /* NSM_OPT_POSE_GRADIENTS (default 0).  With 1 every training step / nsm_backward also computes the gradients of
  * the loss with respect to the rays (row f2, below); costs two extra kernels per step and 19 floats per sample
  * of workspace. */
-typedef enum { NSM_OPT_BATCH_READY = 0, NSM_OPT_POSE_GRADIENTS = 1 } nsm_option;
+/* NSM_OPT_DEBUG_TIMELINE (default 0).  With 1 the kernels of every training step record the in-kernel timeline that
+ * nsm_debug_timeline reads. */
+typedef enum { NSM_OPT_BATCH_READY = 0, NSM_OPT_POSE_GRADIENTS = 1, NSM_OPT_DEBUG_TIMELINE = 2 } nsm_option;
 nsm_status nsm_set_option(nsm_field *f, nsm_option opt, uint32_t value);
 
 /* S1-S12 only: forward + backward, gradients left in place for nsm_debug_last_step; and S13

@@ -16,7 +16,7 @@ LIB_PATH = os.path.join(_HERE, "libnsm.so")
 NSM_OK, NSM_ERR_INVALID_ARG, NSM_ERR_OOM, NSM_ERR_CUDA, NSM_ERR_CAPACITY, NSM_ERR_UNIMPLEMENTED = range(6)
 NSM_MLP_FP32, NSM_MLP_FP16, NSM_MLP_BF16 = 0, 1, 2
 NSM_OCC_FULL, NSM_OCC_SET, NSM_OCC_FROM_FIELD = 0, 1, 2
-NSM_OPT_BATCH_READY, NSM_OPT_POSE_GRADIENTS = 0, 1
+NSM_OPT_BATCH_READY, NSM_OPT_POSE_GRADIENTS, NSM_OPT_DEBUG_TIMELINE = 0, 1, 2
 
 DEBUG_ITEMS = dict(counts=(0, np.uint32), offsets=(1, np.uint32), s_ray=(2, np.uint32), s_k=(3, np.uint32),
                    s_t=(4, np.float32), s_delta=(5, np.float32), s_x=(6, np.float32), slots=(7, np.uint32),
@@ -30,7 +30,7 @@ EXPORTS = ["nsm_create_field", "nsm_destroy_field", "nsm_update_occupancy", "nsm
            "nsm_get_level_table", "nsm_debug_last_step", "nsm_total_samples", "nsm_profile", "nsm_set_option", "nsm_debug_timeline",
            "nsm_add_keyframe", "nsm_keyframe_count", "nsm_sample_batch", "nsm_train_step_sampled",
            "nsm_pose_gradients", "nsm_keyframe_pose_gradients", "nsm_apply_pose_step", "nsm_get_keyframe_pose",
-           "nsm_update_occupancy_decay", "nsm_get_occupancy_grid", "nsm_probe_l2",
+           "nsm_update_occupancy_decay", "nsm_get_occupancy_grid",
            "nsm_profile_read", "nsm_launch_count", "nsm_mlp_path",
            "nsm_last_error", "nsm_version"]
 
@@ -103,7 +103,6 @@ def load_library():
         L.nsm_set_option.argtypes = [vp, C.c_int, C.c_uint32]
         L.nsm_pose_gradients.argtypes = [vp, vp, vp]
         L.nsm_keyframe_pose_gradients.argtypes = [vp, vp]
-        L.nsm_probe_l2.argtypes = [C.c_uint64, C.c_uint64, C.c_int, C.POINTER(C.c_double)]
         L.nsm_update_occupancy_decay.argtypes = [vp, C.c_uint32, C.c_float]
         L.nsm_get_occupancy_grid.argtypes = [vp, vp]
         L.nsm_apply_pose_step.argtypes = [vp, C.c_float, C.c_float]
@@ -179,13 +178,6 @@ class DeviceBatch:
         b.rgb, b.depth, b.depth_var = _dev_ptr(self.rgb), _dev_ptr(self.depth), _dev_ptr(self.depth_var)
         b.t_min, b.t_max, b.n_candidates = self.t_min, self.t_max, self.n_candidates
         return b
-
-
-def probe_l2(table_bytes, n_accesses=1 << 22, reductions=False):
-    """Random 8-byte gathers (or vector reductions) per second over a scratch table of table_bytes (nsm_probe_l2)."""
-    sec = C.c_double()
-    _check(load_library().nsm_probe_l2(int(table_bytes), int(n_accesses), int(bool(reductions)), C.byref(sec)))
-    return n_accesses / sec.value
 
 
 class HostBatch:
@@ -432,7 +424,7 @@ class Field:
         return int(n.value)
 
     def nsm_debug_timeline(self):
-        """[64, 2, n_kernels] uint64 globaltimer stamps (slot = step % 64); needs NSM_TIMELINE=1 at creation."""
+        """[64, 2, n_kernels] uint64 globaltimer stamps (slot = step % 64); needs NSM_OPT_DEBUG_TIMELINE."""
         buf = (C.c_uint64 * (64 * 2 * 32))()
         nk = C.c_uint32()
         _check(self.lib.nsm_debug_timeline(self.h, buf, 64 * 2 * 32, C.byref(nk)))

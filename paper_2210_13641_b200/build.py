@@ -8,6 +8,9 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 ROOT = os.path.dirname(HERE)
 CSRC = os.path.join(HERE, "csrc")
 OUT = os.path.join(HERE, "libnsm.so")
+# bench-only micro-benchmark (csrc/bench_probe/): its own shared object, loaded by bench.py only; not in include/nsm.h
+PROBE_SRC = os.path.join(CSRC, "bench_probe", "l2_probe.cu")
+PROBE_OUT = os.path.join(HERE, "libnsm_bench_probe.so")
 BUILD = os.path.join(HERE, "build")
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-std=c++17", "-lineinfo",
@@ -19,11 +22,24 @@ def sources():
 
 
 def _deps_mtime():
-    paths = [os.path.join(CSRC, f) for f in os.listdir(CSRC)] + [os.path.join(ROOT, "include", "nsm.h")]
+    paths = [os.path.join(CSRC, f) for f in os.listdir(CSRC) if f.endswith((".cu", ".cuh"))] + [os.path.join(ROOT, "include", "nsm.h")]
     return max(os.path.getmtime(p) for p in paths)
 
 
+def build_probe(force=False):
+    if not force and os.path.exists(PROBE_OUT) and os.path.getmtime(PROBE_OUT) >= os.path.getmtime(PROBE_SRC):
+        return PROBE_OUT
+    cmd = [NVCC, "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-std=c++17", "-lineinfo", "-Xcompiler", "-fPIC", "-shared",
+           PROBE_SRC, "-o", PROBE_OUT + ".tmp", "-lcudart"]
+    r = subprocess.run(cmd, capture_output=True, text=True)
+    if r.returncode != 0:
+        raise RuntimeError(f"nvcc failed on {PROBE_SRC}:\n{r.stdout}\n{r.stderr}")
+    os.replace(PROBE_OUT + ".tmp", PROBE_OUT)
+    return PROBE_OUT
+
+
 def build(force=False, verbose=False):
+    build_probe(force)
     if not force and os.path.exists(OUT) and os.path.getmtime(OUT) >= _deps_mtime():
         return OUT
     os.makedirs(BUILD, exist_ok=True)

@@ -1,11 +1,11 @@
-// probe.cu — micro-benchmark behind the L2 figures of DESIGN.md "Kernels" ("measure L2
-// bandwidth and atomic throughput yourself; MEASURED_PEAKS.json has HBM and bf16 only").  Random 8-byte gathers and
-// random red.global.add.v2.f32 over a table of a given size: the access pattern of the encoder (S4) and of the
-// scatter (S12) with every locality removed.  nsm_probe_l2 times one launch with CUDA events after warm-up launches.
+// l2_probe.cu — bench-only micro-benchmark (NOT part of libnsm.so or of include/nsm.h): built as its own shared object,
+// libnsm_bench_probe.so, and loaded by bench.py alone.  It measures, inside the bench run, the peak the encoder (S4) and
+// the scatter (S12) are quoted against while the tables fit the L2 ("measure L2 bandwidth and
+// atomic throughput yourself; MEASURED_PEAKS.json has HBM and bf16 only"): random 8-byte gathers and random
+// red.global.add.v2.f32 over a table of a given size -- those kernels' access pattern with every locality removed.
+// One launch is timed with CUDA events after warm-up launches; best of 8.
 #include <cuda_runtime.h>
 #include <stdint.h>
-
-#include "nsm.h"
 
 namespace {
 
@@ -39,14 +39,15 @@ __global__ void probe_red_kernel(float2 *__restrict__ tab, uint32_t n_entries, u
 
 }  // namespace
 
-extern "C" nsm_status nsm_probe_l2(uint64_t table_bytes, uint64_t n_accesses, int reductions, double *seconds_out) {
-  if (!seconds_out || table_bytes < 64 || n_accesses < 8) return NSM_ERR_INVALID_ARG;
+// returns 0 on success, 1 bad argument, 2 out of memory, 3 CUDA error; *seconds_out = duration of one launch
+extern "C" int nsm_bench_probe_l2(uint64_t table_bytes, uint64_t n_accesses, int reductions, double *seconds_out) {
+  if (!seconds_out || table_bytes < 64 || n_accesses < 8) return 1;
   float2 *tab = nullptr;
   float *sink = nullptr;
   if (cudaMalloc(&tab, table_bytes) != cudaSuccess || cudaMalloc(&sink, 4) != cudaSuccess) {
     cudaGetLastError();
     cudaFree(tab);
-    return NSM_ERR_OOM;
+    return 2;
   }
   cudaMemset(tab, 0, table_bytes);
   const uint32_t n_entries = (uint32_t)(table_bytes / 8);
@@ -70,7 +71,7 @@ extern "C" nsm_status nsm_probe_l2(uint64_t table_bytes, uint64_t n_accesses, in
   cudaEventDestroy(b);
   cudaFree(tab);
   cudaFree(sink);
-  if (cudaGetLastError() != cudaSuccess) return NSM_ERR_CUDA;
+  if (cudaGetLastError() != cudaSuccess) return 3;
   *seconds_out = (double)best * 1e-3;
-  return NSM_OK;
+  return 0;
 }

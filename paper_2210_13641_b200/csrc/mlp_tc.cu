@@ -789,12 +789,21 @@ int launch_reduce_wgrad(const MlpShape &ms, const Workspace &ws, float *grad_mlp
 
 uint32_t mlp_tc_backward_ctas(int n_sms) { return 2u * (uint32_t)n_sms; }
 
+// The kernels need more than 48 KB of dynamic shared memory: an opt-in that CUDA keeps per device.
+cudaError_t mlp_tc_prepare_device() {
+  const auto attr = cudaFuncAttributeMaxDynamicSharedMemorySize;
+  cudaError_t e = cudaFuncSetAttribute(mlp_forward_tc_kernel<__half, true>, attr, (int)FwdSmem::total);
+  if (e == cudaSuccess) e = cudaFuncSetAttribute(mlp_forward_tc_kernel<__half, false>, attr, (int)FwdSmem::total);
+  if (e == cudaSuccess) e = cudaFuncSetAttribute(mlp_forward_tc_kernel<__nv_bfloat16, true>, attr, (int)FwdSmem::total);
+  if (e == cudaSuccess) e = cudaFuncSetAttribute(mlp_forward_tc_kernel<__nv_bfloat16, false>, attr, (int)FwdSmem::total);
+  if (e == cudaSuccess) e = cudaFuncSetAttribute(mlp_backward_tc_kernel<__half>, attr, (int)BwdSmem::total);
+  if (e == cudaSuccess) e = cudaFuncSetAttribute(mlp_backward_tc_kernel<__nv_bfloat16>, attr, (int)BwdSmem::total);
+  return e;
+}
+
 template <typename T, bool SPLIT>
 static void launch_fwd_variant(const MlpShape &ms, const float *dirs, const Workspace &ws, const uint32_t *d_S, int density_only,
                                int save_blobs, int n_sms, cudaStream_t st) {
-  static const cudaError_t once = cudaFuncSetAttribute(mlp_forward_tc_kernel<T, SPLIT>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                                       (int)FwdSmem::total);
-  (void)once;
   launch_pdl(mlp_forward_tc_kernel<T, SPLIT>, dim3(2 * n_sms), dim3(FWD_THREADS), (size_t)FwdSmem::total, st, ms, dirs, ws, d_S,
              density_only, save_blobs);
 }
@@ -816,12 +825,8 @@ int launch_mlp_backward_tc(const MlpShape &ms, int bf16, const Workspace &ws, co
                            int n_sms, cudaStream_t st) {
   const size_t smem = BwdSmem::total;
   if (bf16) {
-    static const cudaError_t once = cudaFuncSetAttribute(mlp_backward_tc_kernel<__nv_bfloat16>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    (void)once;
     launch_pdl(mlp_backward_tc_kernel<__nv_bfloat16>, dim3(2 * n_sms), dim3(BWD_THREADS), smem, st, ms, ws, d_S);
   } else {
-    static const cudaError_t once = cudaFuncSetAttribute(mlp_backward_tc_kernel<__half>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    (void)once;
     launch_pdl(mlp_backward_tc_kernel<__half>, dim3(2 * n_sms), dim3(BWD_THREADS), smem, st, ms, ws, d_S);
   }
   return 1;

@@ -42,10 +42,7 @@ nsm_status fail(nsm_status st, const char *fmt, ...) {
 // config 2 (profiles/r1g_pdl_sweep.md): 148.7 us/step without PDL, 135.5 us with this mask; letting the
 // table Adam's blocks become resident under the scatter, or the marcher's under the MLP Adam, costs
 // more than the launch gap it hides (149 us / 184 us).
-uint32_t g_pdl_mask = [] {
-  const char *e = std::getenv("NSM_PDL_MASK");
-  return e ? (uint32_t)std::strtoul(e, nullptr, 0) : 0xdeu;
-}();
+const uint32_t g_pdl_mask = 0xdeu;
 thread_local int g_cur_kernel = 0;   // kernel class of the launch in progress on this host thread (RUN macro)
 
 static const char *kKernelNames[K_COUNT] = {"march", "encode", "mlp_fwd", "composite",
@@ -82,6 +79,7 @@ struct nsm_field {
   Profiler prof;
   uint64_t launches_by[K_COUNT] = {0};
   cudaStream_t stream = nullptr;
+  int device = 0;             // the CUDA device the field lives on (current at creation); every entry point runs there
   int n_sms = 148;
   LevelTable lv;
   MlpShape ms;
@@ -92,6 +90,7 @@ struct nsm_field {
   uint64_t launches = 0;
   bool occ_full = true;
   uint32_t occ_updates = 0;   // F4: decayed partial refreshes since the last full one
+  bool grid_seeded = false;   // F4: the running density grid holds a full FROM_FIELD pass (SET / FULL invalidate it)
   bool grads_dirty = false;
   // state of the last step, for the debug getter
   uint32_t last_R = 0, last_K = 0;
@@ -119,9 +118,9 @@ struct nsm_field {
   uint32_t *ray_kf = nullptr;                                           // [max_rays] keyframe of every sampled ray
   bool stats_pending = false;
   bool join_pending = false;   // ev_side (recorded behind the MLP Adam) has not been waited for on the main stream yet
-  unsigned long long *timeline_base = nullptr;   // NSM_TIMELINE=1: ring of 64 steps x [2][K_COUNT] globaltimer stamps
-  bool scatter_pending = false;   // the backward pass stopped before S12: enqueue_adam interleaves scatter and Adam per level group
-  uint32_t n_groups = 1;          // level groups of the scatter + Adam phase (NSM_LEVEL_GROUPS)
+  unsigned long long *timeline_base = nullptr;   // NSM_OPT_DEBUG_TIMELINE: ring of 64 steps x [2][K_COUNT] globaltimer stamps
+  bool timeline_on = false;
+  bool scatter_pending = false;   // the backward pass stopped before S12: enqueue_adam issues the scatter right before the table Adam
   uint32_t wgrad_parts = 0;   // > 0: the MLP weight gradient of the last backward is still in that many per-CTA slices
   bool batch_ready = false;   // NSM_OPT_BATCH_READY
   bool side_ok = false;       // nothing but a train step's Adam has been enqueued on `stream` since ev_pre_adam
@@ -232,16 +231,24 @@ nsm_status validate_batch(const nsm_field *f, const nsm_ray_batch *b, bool train
 
 // The side stream's last work (the MLP Adam of the previous step) is joined into the main stream lazily: a training
 // step that marches on the side stream joins behind its marcher anyway, every other entry point joins here.
-void join_side(nsm_field *f) {
+cudaError_t join_side(nsm_field *f) {
+  cudaError_t e = cudaSuccess;
   if (f->join_pending) {
-    cudaStreamWaitEvent(f->stream, f->ev_side, 0);
+    e = cudaStreamWaitEvent(f->stream, f->ev_side, 0);
     f->join_pending = false;
   }
+  return e;
 }
-void leave_fast_path(nsm_field *f) {
-  join_side(f);
+// Every entry point other than a training step calls this first: it makes the field's device current, joins the side
+// stream and leaves the two-stream fast path.  A failure here is reported by the entry point's own CUDA_TRY of
+// cudaGetLastError / its first CUDA call (the error is sticky).
+cudaError_t leave_fast_path(nsm_field *f) {
+  cudaError_t e = cudaSetDevice(f->device);
+  const cudaError_t e2 = join_side(f);
   f->side_ok = false;
+  return e != cudaSuccess ? e : e2;
 }
+#define LEAVE_FAST_PATH(f) CUDA_TRY(leave_fast_path(f))
 
 MarchParams make_march(const nsm_field *f, const nsm_ray_batch *b, uint32_t R, bool jitter, uint32_t step) {
   MarchParams mp;
@@ -264,26 +271,26 @@ MarchParams make_march(const nsm_field *f, const nsm_ray_batch *b, uint32_t R, b
 // dirs_copy: see launch_march (zero-copy host batches); the MLP kernels then read the copy.
 // sample_draw >= 0: the batch is first drawn from the keyframe store (F1) into b's buffers (the field's staging area),
 // on the stream the marcher runs on.
-void enqueue_forward(nsm_field *f, const nsm_ray_batch *b, uint32_t R, bool jitter, uint32_t step, bool train,
-                     bool march_on_side = false, float *dirs_copy = nullptr, int64_t sample_draw = -1) {
+nsm_status enqueue_forward(nsm_field *f, const nsm_ray_batch *b, uint32_t R, bool jitter, uint32_t step, bool train,
+                           bool march_on_side = false, float *dirs_copy = nullptr, int64_t sample_draw = -1) {
   const uint32_t *d_S = f->ws.offsets + R;
   const float *mlp_dirs = dirs_copy ? dirs_copy : b->dirs;
   MarchParams mp = make_march(f, b, R, jitter, step);
   if (march_on_side && !f->prof.on) {
     if (!f->side_ok) {   // other work has been enqueued on the main stream since the last Adam: order behind all of it
-      cudaEventRecord(f->ev_main, f->stream);
-      cudaStreamWaitEvent(f->side, f->ev_main, 0);
+      CUDA_TRY(cudaEventRecord(f->ev_main, f->stream));
+      CUDA_TRY(cudaStreamWaitEvent(f->side, f->ev_main, 0));
     }
     if (sample_draw >= 0)
       RUN_ON(f, K_SAMPLE, f->side, launch_sample_batch(f->kf_dev, (uint32_t)f->kf_host.size(), f->cfg.seed, (uint32_t)sample_draw, R,
                                                        (float *)b->origins, (float *)b->dirs, (float *)b->rgb, (float *)b->depth,
                                                        (float *)b->depth_var, f->pose_grads ? f->ray_kf : nullptr, f->side));
     RUN_ON(f, K_MARCH, f->side, launch_march(mp, f->occ_full ? nullptr : f->fp.occ_bits, b->origins, b->dirs, f->ws, train ? 1 : 0, f->side, dirs_copy));
-    cudaEventRecord(f->ev_side, f->side);
-    cudaStreamWaitEvent(f->stream, f->ev_side, 0);
+    CUDA_TRY(cudaEventRecord(f->ev_side, f->side));
+    CUDA_TRY(cudaStreamWaitEvent(f->stream, f->ev_side, 0));
     f->join_pending = false;   // behind the marcher is behind the previous step's MLP Adam too
   } else {
-    join_side(f);
+    CUDA_TRY(join_side(f));
     if (sample_draw >= 0)
       RUN(f, K_SAMPLE, launch_sample_batch(f->kf_dev, (uint32_t)f->kf_host.size(), f->cfg.seed, (uint32_t)sample_draw, R,
                                            (float *)b->origins, (float *)b->dirs, (float *)b->rgb, (float *)b->depth,
@@ -296,6 +303,7 @@ void enqueue_forward(nsm_field *f, const nsm_ray_batch *b, uint32_t R, bool jitt
     RUN(f, K_MLP_FWD, launch_mlp_forward_tc(f->ms, bf16, mlp_dirs, f->ws, d_S, 0, train ? 1 : 0, f->n_sms, f->stream));
   else
     RUN(f, K_MLP_FWD, launch_mlp_forward_simt(f->ms, f->fp.mlp_theta, mlp_dirs, f->ws, d_S, 0, f->n_sms, f->stream));
+  return NSM_OK;
 }
 
 // the tensor-core kernels read 16-bit weight images: repack after every change of the MLP weights
@@ -321,13 +329,14 @@ nsm_status enqueue_backward(nsm_field *f, const nsm_ray_batch *b, float lambda_d
   const uint32_t *d_S = f->ws.offsets + R;
   nsm_status st = clear_grads_if_dirty(f);
   if (st != NSM_OK) return st;
-  if (f->timeline_base) {   // this step's slot of the ring; the slot used 8 steps from now is reset here, well ahead of its use
+  if (f->timeline_on) {   // this step's slot of the ring; the slot used 8 steps from now is reset here, well ahead of its use
     f->ws.timeline = f->timeline_base + (size_t)((f->step + 1) % 64) * 2 * K_COUNT;
     unsigned long long *later = f->timeline_base + (size_t)((f->step + 9) % 64) * 2 * K_COUNT;
-    cudaMemsetAsync(later, 0xff, sizeof(unsigned long long) * K_COUNT, f->stream);
-    cudaMemsetAsync(later + K_COUNT, 0, sizeof(unsigned long long) * K_COUNT, f->stream);
+    CUDA_TRY(cudaMemsetAsync(later, 0xff, sizeof(unsigned long long) * K_COUNT, f->stream));
+    CUDA_TRY(cudaMemsetAsync(later + K_COUNT, 0, sizeof(unsigned long long) * K_COUNT, f->stream));
   }
-  enqueue_forward(f, b, R, f->cfg.jitter != 0, f->step + 1, true, march_on_side, dirs_copy, sample_draw);
+  st = enqueue_forward(f, b, R, f->cfg.jitter != 0, f->step + 1, true, march_on_side, dirs_copy, sample_draw);
+  if (st != NSM_OK) return st;
   f->side_ok = false;
   RUN(f, K_COMPOSITE, launch_composite_train(f->ws, R, b->rgb, b->depth, b->depth_var, lambda_d, f->cfg.bg, f->stream));
   if (want_stats) {
@@ -355,9 +364,9 @@ nsm_status enqueue_backward(nsm_field *f, const nsm_ray_batch *b, float lambda_d
                                          f->cfg.sh_degree, f->pose_go, f->pose_tau, f->last_sampled ? f->ray_kf : nullptr, f->kf_grad,
                                          (uint32_t)f->kf_host.size(), f->n_sms, f->stream));
   }
-  // train step: the scatter is issued by enqueue_adam, level group by level group, each followed by its Adam
+  // train step: the scatter is issued by enqueue_adam, behind the MLP Adam's hand-off to the side stream
   f->scatter_pending = defer_scatter;
-  if (!defer_scatter) RUN(f, K_SCATTER, launch_scatter(f->lv, f->fp.grad, f->ws, d_S, 0, f->lv.n_levels, f->n_sms, f->stream));
+  if (!defer_scatter) RUN(f, K_SCATTER, launch_scatter(f->lv, f->fp.grad, f->fp.touched, f->ws, d_S, f->n_sms, f->stream));
   f->grads_dirty = true;
   f->last_R = R;
   f->last_K = b->n_candidates;
@@ -370,13 +379,12 @@ nsm_status enqueue_adam(nsm_field *f) {
   const uint32_t t = f->step + 1;
   const double bc1 = 1.0 - std::pow((double)f->cfg.beta1, (double)t);
   const double bc2 = 1.0 - std::pow((double)f->cfg.beta2, (double)t);
-  // the MLP Adam (9-11 K weights + the 16-bit image refresh) runs on the side stream beside the table Adam
-  static const bool no_side_adam = [] { const char *e = std::getenv("NSM_NO_SIDE_ADAM"); return e && e[0] == '1'; }();
-  const bool use_side = !f->prof.on && !no_side_adam;
+  // the MLP Adam (9-11 K weights + the 16-bit image refresh) runs on the side stream beside the scatter and the table Adam
+  const bool use_side = !f->prof.on;
   cudaStream_t s_mlp = use_side ? f->side : f->stream;
   if (use_side) {
-    cudaEventRecord(f->ev_pre_adam, f->stream);
-    cudaStreamWaitEvent(f->side, f->ev_pre_adam, 0);
+    CUDA_TRY(cudaEventRecord(f->ev_pre_adam, f->stream));
+    CUDA_TRY(cudaStreamWaitEvent(f->side, f->ev_pre_adam, 0));
   }
   if (f->use_tc) {
     const AdamConst c{f->cfg.lr, f->cfg.beta1, f->cfg.beta2, f->cfg.eps, (float)(1.0 / bc1), (float)(1.0 / bc2)};
@@ -387,41 +395,20 @@ nsm_status enqueue_adam(nsm_field *f) {
     RUN_ON(f, K_ADAM_MLP, s_mlp, launch_adam_mlp(f->fp, f->cfg.lr, f->cfg.beta1, f->cfg.beta2, f->cfg.eps, (float)(1.0 / bc1),
                                                  (float)(1.0 / bc2), s_mlp));
   }
-  // S12 + S13 on the tables.  The scatter and the Adam pass can be issued per level group (NSM_LEVEL_GROUPS = G:
-  // scatter(group) then Adam(group), so that a group's slice of the gradient array stays in L2 between its three
-  // uses).  Measured on B200 at config 2 (profiles/r1j): G = 1 118.9 us/step, 2 138.2, 3 149.1, 4 160.8, 8 201.0 --
-  // every extra pair of launches costs ~19 us of ramp and tail, far more than the ~100 MB of DRAM traffic it saves,
-  // so the default is one group.  Group boundaries are level boundaries rounded DOWN to 4 entries.
-  {
-    const uint32_t L = f->lv.n_levels;
-    const uint64_t E = f->fp.n_entries;
-    const uint32_t G = f->scatter_pending ? (f->n_groups < L ? f->n_groups : L) : 1;
-    const uint32_t *d_S = f->ws.offsets + f->last_R;
-    const int sparse = (f->cfg.sparse_table_adam != 0);
-    uint32_t l0 = 0;
-    uint64_t e0 = 0;
-    for (uint32_t g = 0; g < G; ++g) {
-      uint32_t l1 = L;
-      if (g + 1 < G) {   // first level boundary at or past the g+1-th share of the entries
-        l1 = l0 + 1;
-        while (l1 < L - (G - 1 - g) && f->lv.offset[l1] * G < E * (g + 1)) ++l1;
-      }
-      const uint64_t e1 = l1 == L ? E : (f->lv.offset[l1] & ~uint64_t(3));
-      if (f->scatter_pending) RUN(f, K_SCATTER, launch_scatter(f->lv, f->fp.grad, f->ws, d_S, l0, l1, f->n_sms, f->stream));
-      if (g + 1 == G && use_side) {   // the last scatter is in: the side stream (next step's marcher) may overwrite the samples
-        cudaEventRecord(f->ev_main, f->stream);
-        cudaStreamWaitEvent(f->side, f->ev_main, 0);
-      }
-      if (e1 > e0)
-        RUN(f, K_ADAM_TABLE, launch_adam_table(f->fp, f->cfg.n_features, sparse, f->cfg.lr, f->cfg.beta1, f->cfg.beta2, f->cfg.eps,
-                                               (float)(1.0 / bc1), (float)(1.0 / bc2), e0, e1, f->stream, f->ws.timeline));
-      l0 = l1;
-      e0 = e1;
-    }
-    f->scatter_pending = false;
+  // S12 + S13 on the tables: one scatter, one Adam.  (Issuing them per level group, so that a group's slice of the
+  // gradient array stays in L2 between its uses, was measured in round 1 -- profiles/r1j: every extra pair of launches
+  // costs ~19 us of ramp and tail, more than the DRAM traffic it saves.)
+  if (f->scatter_pending)
+    RUN(f, K_SCATTER, launch_scatter(f->lv, f->fp.grad, f->fp.touched, f->ws, f->ws.offsets + f->last_R, f->n_sms, f->stream));
+  f->scatter_pending = false;
+  if (use_side) {   // the scatter is in: the side stream (next step's marcher) may overwrite the samples
+    CUDA_TRY(cudaEventRecord(f->ev_main, f->stream));
+    CUDA_TRY(cudaStreamWaitEvent(f->side, f->ev_main, 0));
   }
+  RUN(f, K_ADAM_TABLE, launch_adam_table(f->fp, f->cfg.n_features, f->cfg.sparse_table_adam != 0, f->cfg.lr, f->cfg.beta1, f->cfg.beta2,
+                                         f->cfg.eps, (float)(1.0 / bc1), (float)(1.0 / bc2), f->stream, f->ws.timeline));
   if (use_side) {   // to be joined (lazily, join_side): everything later on the main stream must see the new MLP weights
-    cudaEventRecord(f->ev_side, f->side);
+    CUDA_TRY(cudaEventRecord(f->ev_side, f->side));
     f->join_pending = true;
     f->side_ok = true;
   }
@@ -489,11 +476,13 @@ nsm_status nsm_create_field(const nsm_field_config *cfg, void *cuda_stream, nsm_
   CUDA_TRY(cudaGetDevice(&dev));
   cudaDeviceProp prop;
   CUDA_TRY(cudaGetDeviceProperties(&prop, dev));
-  if (prop.major < 10) return fail(NSM_ERR_CUDA, "device sm_%d%d is not sm_100: built for B200 only", prop.major, prop.minor);
+  if (prop.major != 10 || prop.minor != 0)   // the library holds sm_100a code only (tcgen05 / TMEM paths are not forward-compatible)
+    return fail(NSM_ERR_CUDA, "device sm_%d%d is not sm_100: built for B200 (sm_100a) only", prop.major, prop.minor);
 
   nsm_field *f = new (std::nothrow) nsm_field();
   if (!f) return fail(NSM_ERR_OOM, "host allocation failed");
   f->cfg = *cfg;
+  f->device = dev;
   f->stream = (cudaStream_t)cuda_stream;
   f->n_sms = prop.multiProcessorCount;
   build_levels(*cfg, f->lv);
@@ -517,12 +506,17 @@ nsm_status nsm_create_field(const nsm_field_config *cfg, void *cuda_stream, nsm_
                 (size_t)prop.sharedMemPerBlockOptin);
   }
 
-  // 16-bit configurations run the MLPs on tcgen05 when the shapes fit its tiles (NSM_FORCE_SIMT=1
-  // keeps the fp32 CUDA-core kernels, for A/B debugging)
-  const char *force = std::getenv("NSM_FORCE_SIMT");
-  if (cfg->mlp_precision != NSM_MLP_FP32 && mlp_tc_supported(ms) && !(force && force[0] == '1')) {
+  // 16-bit configurations run the MLPs on tcgen05 when the shapes fit its tiles; the kernels' shared-memory opt-in is a
+  // per-device attribute, set here for the field's device
+  if (cfg->mlp_precision != NSM_MLP_FP32 && mlp_tc_supported(ms)) {
     f->use_tc = true;
     f->mlp_path = cfg->mlp_precision == NSM_MLP_BF16 ? "tcgen05_bf16" : "tcgen05_f16";
+    const cudaError_t ea = mlp_tc_prepare_device();
+    if (ea != cudaSuccess) {
+      delete f;
+      cudaGetLastError();
+      return fail(NSM_ERR_CUDA, "tcgen05 kernel attributes: %s", cudaGetErrorString(ea));
+    }
   }
   FieldParams &fp = f->fp;
   fp.n_entries = f->lv.offset[cfg->n_levels];
@@ -539,7 +533,7 @@ nsm_status nsm_create_field(const nsm_field_config *cfg, void *cuda_stream, nsm_
   auto A = [&](cudaError_t r) { if (e == cudaSuccess) e = r; };
   A(f->alloc(&fp.theta, fp.n_table)); A(f->alloc(&fp.mv, 2 * fp.n_table));
   A(f->alloc(&fp.mlp_theta, fp.n_mlp)); A(f->alloc(&fp.mlp_m, fp.n_mlp)); A(f->alloc(&fp.mlp_v, fp.n_mlp)); A(f->alloc(&fp.mlp_grad, fp.n_mlp));
-  A(f->alloc(&fp.grad, fp.n_table, false)); A(f->alloc(&fp.occ_bits, (G3 + 7) / 8 + 4));
+  A(f->alloc(&fp.grad, fp.n_table)); A(f->alloc(&fp.touched, (fp.n_entries + 31) / 32 + 1)); A(f->alloc(&fp.occ_bits, (G3 + 7) / 8 + 4));
   A(f->alloc(&fp.occ_grid, G3));
   A(f->alloc(&ws.counts, R)); A(f->alloc(&ws.offsets, R + 1)); A(f->alloc(&ws.scan_state, march_scan_state_entries(R) + 1)); A(f->alloc(&ws.scan_ctr, 2));
   A(f->alloc(&ws.C, 3 * (size_t)R)); A(f->alloc(&ws.D_hat, R)); A(f->alloc(&ws.O, R));
@@ -562,14 +556,6 @@ nsm_status nsm_create_field(const nsm_field_config *cfg, void *cuda_stream, nsm_
   A(f->alloc(&f->kf_dev, NSM_MAX_KEYFRAMES));
   ws.dY = ws.dx = nullptr;
   ws.timeline = nullptr;
-  {
-    const char *tl = std::getenv("NSM_TIMELINE");
-    if (tl && tl[0] == '1') {
-      A(f->alloc(&f->timeline_base, 64 * 2 * K_COUNT));
-      for (int i = 0; i < 64 && e == cudaSuccess; ++i)
-        e = cudaMemsetAsync(f->timeline_base + (size_t)i * 2 * K_COUNT, 0xff, sizeof(unsigned long long) * K_COUNT, f->stream);
-    }
-  }
   A(f->alloc(&ws.loss_acc, 3)); A(f->alloc(&ws.total_samples, 1)); A(f->alloc(&ws.grad_absmax, 1));
   A(f->alloc(&f->stage_dev, 11 * (size_t)R)); A(f->alloc(&f->stage_out, 5 * (size_t)R));
   if (e == cudaSuccess) e = cudaMallocHost((void **)&f->pinned, sizeof(*f->pinned));
@@ -588,9 +574,7 @@ nsm_status nsm_create_field(const nsm_field_config *cfg, void *cuda_stream, nsm_
     cudaGetLastError();
     return fail(e == cudaErrorMemoryAllocation ? NSM_ERR_OOM : NSM_ERR_CUDA, "allocation failed: %s", cudaGetErrorString(e));
   }
-  RUN(f, K_DEBUG, launch_set_grad(f->fp, nullptr, nullptr, f->stream));   // every gradient word = "untouched"
-  if (const char *g = std::getenv("NSM_LEVEL_GROUPS")) f->n_groups = (uint32_t)std::max(1, std::atoi(g));
-  repack_weights(f);
+  repack_weights(f);   // gradient array and touched bitmap start zeroed (alloc)
   *out = f;
   return NSM_OK;
 }
@@ -613,7 +597,7 @@ void nsm_destroy_field(nsm_field *f) {
 nsm_status nsm_total_samples(nsm_field *f, uint64_t *out) {
   if (!f || !out) return fail(NSM_ERR_INVALID_ARG, "NULL argument");
   unsigned long long v = 0;
-  leave_fast_path(f);   // the marcher (side stream) maintains the count
+  LEAVE_FAST_PATH(f);   // the marcher (side stream) maintains the count
   CUDA_TRY(cudaMemcpyAsync(&v, f->ws.total_samples, sizeof v, cudaMemcpyDeviceToHost, f->stream));
   CUDA_TRY(cudaStreamSynchronize(f->stream));
   *out = v;
@@ -622,7 +606,7 @@ nsm_status nsm_total_samples(nsm_field *f, uint64_t *out) {
 
 nsm_status nsm_profile(nsm_field *f, int enable) {
   if (!f) return fail(NSM_ERR_INVALID_ARG, "field is NULL");
-  leave_fast_path(f);
+  LEAVE_FAST_PATH(f);
   CUDA_TRY(cudaStreamSynchronize(f->stream));
   f->prof.collect();
   f->prof.on = enable != 0;
@@ -662,7 +646,7 @@ nsm_status nsm_get_level_table(const nsm_field *f, uint32_t *res, uint64_t *offs
 
 nsm_status nsm_get_params(nsm_field *f, float *d_theta, float *d_m, float *d_v, uint32_t *step) {
   if (!f) return fail(NSM_ERR_INVALID_ARG, "field is NULL");
-  leave_fast_path(f);
+  LEAVE_FAST_PATH(f);
   const size_t mb = sizeof(float) * f->fp.n_mlp;
   float *dst[3] = {d_theta, d_m, d_v};
   const float *mlp[3] = {f->fp.mlp_theta, f->fp.mlp_m, f->fp.mlp_v};
@@ -679,7 +663,7 @@ nsm_status nsm_get_params(nsm_field *f, float *d_theta, float *d_m, float *d_v, 
 
 nsm_status nsm_set_params(nsm_field *f, const float *d_theta, const float *d_m, const float *d_v, uint32_t step) {
   if (!f) return fail(NSM_ERR_INVALID_ARG, "field is NULL");
-  leave_fast_path(f);
+  LEAVE_FAST_PATH(f);
   const size_t mb = sizeof(float) * f->fp.n_mlp;
   const float *src[3] = {d_theta, d_m, d_v};
   float *mlp[3] = {f->fp.mlp_theta, f->fp.mlp_m, f->fp.mlp_v};
@@ -697,7 +681,7 @@ nsm_status nsm_set_params(nsm_field *f, const float *d_theta, const float *d_m, 
 
 nsm_status nsm_get_occupancy(nsm_field *f, uint8_t *d_bits) {
   if (!f || !d_bits) return fail(NSM_ERR_INVALID_ARG, "NULL argument");
-  leave_fast_path(f);
+  LEAVE_FAST_PATH(f);
   const uint64_t G3 = (uint64_t)f->cfg.occ_res * f->cfg.occ_res * f->cfg.occ_res;
   if (f->occ_full) CUDA_TRY(cudaMemsetAsync(d_bits, 0xff, (G3 + 7) / 8, f->stream));
   else CUDA_TRY(cudaMemcpyAsync(d_bits, f->fp.occ_bits, (G3 + 7) / 8, cudaMemcpyDeviceToDevice, f->stream));
@@ -706,16 +690,20 @@ nsm_status nsm_get_occupancy(nsm_field *f, uint8_t *d_bits) {
 
 nsm_status nsm_update_occupancy(nsm_field *f, nsm_occ_mode mode, const uint8_t *d_bits) {
   if (!f) return fail(NSM_ERR_INVALID_ARG, "field is NULL");
-  leave_fast_path(f);
+  LEAVE_FAST_PATH(f);
   const uint64_t G3 = (uint64_t)f->cfg.occ_res * f->cfg.occ_res * f->cfg.occ_res;
   switch (mode) {
     case NSM_OCC_FULL:
       f->occ_full = true;
+      f->grid_seeded = false;
+      f->occ_updates = 0;
       return NSM_OK;
     case NSM_OCC_SET:
       if (!d_bits) return fail(NSM_ERR_INVALID_ARG, "d_bits is NULL");
       CUDA_TRY(cudaMemcpyAsync(f->fp.occ_bits, d_bits, (G3 + 7) / 8, cudaMemcpyDeviceToDevice, f->stream));
       f->occ_full = false;
+      f->grid_seeded = false;
+      f->occ_updates = 0;
       return NSM_OK;
     case NSM_OCC_FROM_FIELD: {
       // the cell centres go through S4 + S5 in chunks of the workspace capacity (multiples of 32)
@@ -735,6 +723,7 @@ nsm_status nsm_update_occupancy(nsm_field *f, nsm_occ_mode mode, const uint8_t *
                                            f->fp.occ_bits, f->fp.occ_grid, f->stream));
       }
       f->occ_full = false;
+      f->grid_seeded = true;
       f->occ_updates = 0;
       CUDA_TRY(cudaGetLastError());
       return NSM_OK;
@@ -748,7 +737,9 @@ nsm_status nsm_update_occupancy_decay(nsm_field *f, uint32_t n_subsets, float de
   if (!f) return fail(NSM_ERR_INVALID_ARG, "field is NULL");
   if (n_subsets == 0) return fail(NSM_ERR_INVALID_ARG, "n_subsets is 0");
   if (!(decay >= 0.f && decay <= 1.f)) return fail(NSM_ERR_INVALID_ARG, "decay must be in [0, 1]");
-  leave_fast_path(f);
+  if (!f->grid_seeded)   // after SET / FULL the running grid says nothing about the cells a partial pass does not visit
+    return fail(NSM_ERR_INVALID_ARG, "the running density grid is not seeded: call nsm_update_occupancy(NSM_OCC_FROM_FIELD) first");
+  LEAVE_FAST_PATH(f);
   const uint64_t G3 = (uint64_t)f->cfg.occ_res * f->cfg.occ_res * f->cfg.occ_res;
   const uint64_t c0 = f->occ_updates % n_subsets;
   const uint64_t n_vis = c0 < G3 ? (G3 - c0 + n_subsets - 1) / n_subsets : 0;
@@ -776,7 +767,7 @@ nsm_status nsm_update_occupancy_decay(nsm_field *f, uint32_t n_subsets, float de
 
 nsm_status nsm_get_occupancy_grid(nsm_field *f, float *d_grid) {
   if (!f || !d_grid) return fail(NSM_ERR_INVALID_ARG, "NULL argument");
-  leave_fast_path(f);
+  LEAVE_FAST_PATH(f);
   const uint64_t G3 = (uint64_t)f->cfg.occ_res * f->cfg.occ_res * f->cfg.occ_res;
   CUDA_TRY(cudaMemcpyAsync(d_grid, f->fp.occ_grid, sizeof(float) * G3, cudaMemcpyDeviceToDevice, f->stream));
   return NSM_OK;
@@ -785,7 +776,7 @@ nsm_status nsm_get_occupancy_grid(nsm_field *f, float *d_grid) {
 nsm_status nsm_backward(nsm_field *f, const nsm_ray_batch *batch, float lambda_d, nsm_step_stats *host_stats) {
   nsm_status st = validate_batch(f, batch, true, false);
   if (st != NSM_OK) return st;
-  leave_fast_path(f);
+  LEAVE_FAST_PATH(f);
   st = enqueue_backward(f, batch, lambda_d, false, nullptr, host_stats != nullptr, true);
   if (st != NSM_OK) return st;
   st = read_stats(f, batch->n_rays, host_stats);
@@ -795,7 +786,7 @@ nsm_status nsm_backward(nsm_field *f, const nsm_ray_batch *batch, float lambda_d
 
 nsm_status nsm_apply_adam(nsm_field *f) {
   if (!f) return fail(NSM_ERR_INVALID_ARG, "field is NULL");
-  leave_fast_path(f);
+  LEAVE_FAST_PATH(f);
   return enqueue_adam(f);
 }
 
@@ -835,7 +826,7 @@ nsm_status nsm_train_step_host(nsm_field *f, const nsm_ray_batch *hb, float lamb
   db.depth = host_mapped(hb->depth); db.depth_var = host_mapped(hb->depth_var);
   if (db.origins && db.dirs && db.rgb && db.depth && db.depth_var)   // the call syncs: the host buffers are free on return
     return train_step_impl(f, &db, lambda_d, host_stats ? host_stats : &local, true, f->stage_dev + 3 * (size_t)f->cfg.max_rays);
-  leave_fast_path(f);   // pageable memory: staging copies through the main stream
+  LEAVE_FAST_PATH(f);   // pageable memory: staging copies through the main stream
   st = stage_batch(f, hb, 0, hb->n_rays, true, &db);
   if (st != NSM_OK) return st;
   return train_step_impl(f, &db, lambda_d, host_stats ? host_stats : &local, false);  // always syncs: host buffers may be reused
@@ -843,7 +834,7 @@ nsm_status nsm_train_step_host(nsm_field *f, const nsm_ray_batch *hb, float lamb
 
 nsm_status nsm_debug_timeline(nsm_field *f, uint64_t *h_out, uint64_t capacity_words, uint32_t *n_kernels) {
   if (!f || !h_out) return fail(NSM_ERR_INVALID_ARG, "NULL argument");
-  if (!f->timeline_base) return fail(NSM_ERR_INVALID_ARG, "timeline not enabled (create the field with NSM_TIMELINE=1 in the environment)");
+  if (!f->timeline_base) return fail(NSM_ERR_INVALID_ARG, "timeline not enabled (nsm_set_option(NSM_OPT_DEBUG_TIMELINE, 1))");
   if (capacity_words < 64ull * 2 * K_COUNT) return fail(NSM_ERR_CAPACITY, "timeline needs %d words", 64 * 2 * K_COUNT);
   CUDA_TRY(cudaStreamSynchronize(f->stream));
   CUDA_TRY(cudaMemcpy(h_out, f->timeline_base, sizeof(uint64_t) * 64 * 2 * K_COUNT, cudaMemcpyDeviceToHost));
@@ -860,7 +851,7 @@ nsm_status nsm_add_keyframe(nsm_field *f, const nsm_keyframe_info *info, const f
   if (!(info->fx > 0.f) || !(info->fy > 0.f) || !std::isfinite(info->fx) || !std::isfinite(info->fy))
     return fail(NSM_ERR_INVALID_ARG, "focal lengths must be positive");
   if (f->kf_host.size() >= NSM_MAX_KEYFRAMES) return fail(NSM_ERR_CAPACITY, "keyframe store is full (%d)", NSM_MAX_KEYFRAMES);
-  leave_fast_path(f);
+  LEAVE_FAST_PATH(f);
   const size_t n = (size_t)info->width * info->height;
   float *buf = nullptr;
   CUDA_TRY(f->alloc(&buf, 5 * n, false));
@@ -892,7 +883,7 @@ nsm_status nsm_sample_batch(nsm_field *f, uint32_t n_rays, uint32_t draw, float 
   if (!f || !d_origins || !d_dirs || !d_rgb || !d_depth || !d_depth_var) return fail(NSM_ERR_INVALID_ARG, "NULL argument");
   if (f->kf_host.empty()) return fail(NSM_ERR_INVALID_ARG, "the keyframe store is empty");
   if (n_rays == 0) return fail(NSM_ERR_INVALID_ARG, "n_rays is 0");
-  leave_fast_path(f);
+  LEAVE_FAST_PATH(f);
   RUN(f, K_SAMPLE, launch_sample_batch(f->kf_dev, (uint32_t)f->kf_host.size(), f->cfg.seed, draw, n_rays, d_origins, d_dirs, d_rgb,
                                        d_depth, d_depth_var, nullptr, f->stream));
   CUDA_TRY(cudaGetLastError());
@@ -919,7 +910,7 @@ nsm_status nsm_pose_gradients(nsm_field *f, float *d_g_o, float *d_tau) {
   if (!f || !d_g_o || !d_tau) return fail(NSM_ERR_INVALID_ARG, "NULL argument");
   if (!f->pose_grads || f->last_R == 0 || f->last_was_render)
     return fail(NSM_ERR_INVALID_ARG, "no pose gradients: set NSM_OPT_POSE_GRADIENTS and run a training step / nsm_backward first");
-  leave_fast_path(f);
+  LEAVE_FAST_PATH(f);
   CUDA_TRY(cudaMemcpyAsync(d_g_o, f->pose_go, sizeof(float) * 3 * f->last_R, cudaMemcpyDeviceToDevice, f->stream));
   CUDA_TRY(cudaMemcpyAsync(d_tau, f->pose_tau, sizeof(float) * 3 * f->last_R, cudaMemcpyDeviceToDevice, f->stream));
   return NSM_OK;
@@ -929,7 +920,7 @@ nsm_status nsm_keyframe_pose_gradients(nsm_field *f, float *d_out) {
   if (!f || !d_out) return fail(NSM_ERR_INVALID_ARG, "NULL argument");
   if (!f->pose_grads || !f->last_sampled || f->last_was_render)
     return fail(NSM_ERR_INVALID_ARG, "no keyframe gradients: set NSM_OPT_POSE_GRADIENTS and run nsm_train_step_sampled first");
-  leave_fast_path(f);
+  LEAVE_FAST_PATH(f);
   CUDA_TRY(cudaMemcpy2DAsync(d_out, sizeof(float) * 6, f->kf_grad, sizeof(float) * NSM_KF_GRAD_STRIDE, sizeof(float) * 6,
                              f->kf_host.size(), cudaMemcpyDeviceToDevice, f->stream));
   return NSM_OK;
@@ -940,7 +931,7 @@ nsm_status nsm_apply_pose_step(nsm_field *f, float lr_translation, float lr_rota
   if (!f->pose_grads || !f->last_sampled || f->last_was_render)
     return fail(NSM_ERR_INVALID_ARG, "no keyframe gradients: set NSM_OPT_POSE_GRADIENTS and run nsm_train_step_sampled first");
   if (!(lr_translation >= 0.f) || !(lr_rotation >= 0.f)) return fail(NSM_ERR_INVALID_ARG, "learning rates must be >= 0");
-  leave_fast_path(f);
+  LEAVE_FAST_PATH(f);
   RUN(f, K_POSE, launch_pose_step(f->kf_dev, (uint32_t)f->kf_host.size(), f->kf_grad, f->kf_pose_m, f->kf_pose_v, f->kf_pose_cnt,
                                   lr_translation, lr_rotation, f->cfg.beta1, f->cfg.beta2, f->cfg.eps, f->stream));
   f->last_sampled = false;   // the gradients are consumed
@@ -951,7 +942,7 @@ nsm_status nsm_apply_pose_step(nsm_field *f, float lr_translation, float lr_rota
 nsm_status nsm_get_keyframe_pose(nsm_field *f, uint32_t index, float *h_R, float *h_t) {
   if (!f || !h_R || !h_t) return fail(NSM_ERR_INVALID_ARG, "NULL argument");
   if (index >= f->kf_host.size()) return fail(NSM_ERR_INVALID_ARG, "keyframe index %u out of range", index);
-  leave_fast_path(f);
+  LEAVE_FAST_PATH(f);
   KeyframeDev k;
   CUDA_TRY(cudaMemcpyAsync(&k, f->kf_dev + index, sizeof k, cudaMemcpyDeviceToHost, f->stream));
   CUDA_TRY(cudaStreamSynchronize(f->stream));
@@ -963,9 +954,9 @@ nsm_status nsm_get_keyframe_pose(nsm_field *f, uint32_t index, float *h_R, float
 nsm_status nsm_set_option(nsm_field *f, nsm_option opt, uint32_t value) {
   if (!f) return fail(NSM_ERR_INVALID_ARG, "field is NULL");
   switch (opt) {
-    case NSM_OPT_BATCH_READY: f->batch_ready = value != 0; leave_fast_path(f); return NSM_OK;
+    case NSM_OPT_BATCH_READY: f->batch_ready = value != 0; LEAVE_FAST_PATH(f); return NSM_OK;
     case NSM_OPT_POSE_GRADIENTS: {
-      leave_fast_path(f);
+      LEAVE_FAST_PATH(f);
       if (value && !f->ws.dY) {   // workspace of row f2, allocated on first use
         cudaError_t e = cudaSuccess;
         auto A = [&](cudaError_t r) { if (e == cudaSuccess) e = r; };
@@ -979,13 +970,24 @@ nsm_status nsm_set_option(nsm_field *f, nsm_option opt, uint32_t value) {
       f->pose_grads = value != 0;
       return NSM_OK;
     }
+    case NSM_OPT_DEBUG_TIMELINE: {
+      LEAVE_FAST_PATH(f);
+      if (value && !f->timeline_base) {
+        CUDA_TRY(f->alloc(&f->timeline_base, 64 * 2 * K_COUNT));
+        for (int i = 0; i < 64; ++i)
+          CUDA_TRY(cudaMemsetAsync(f->timeline_base + (size_t)i * 2 * K_COUNT, 0xff, sizeof(unsigned long long) * K_COUNT, f->stream));
+      }
+      if (!value) f->ws.timeline = nullptr;   // the ring stays allocated; kernels stop stamping
+      f->timeline_on = value != 0;
+      return NSM_OK;
+    }
   }
   return fail(NSM_ERR_INVALID_ARG, "unknown option %d", (int)opt);
 }
 
 nsm_status nsm_debug_set_grad(nsm_field *f, const float *d_grad, const uint8_t *d_touched) {
   if (!f) return fail(NSM_ERR_INVALID_ARG, "field is NULL");
-  leave_fast_path(f);
+  LEAVE_FAST_PATH(f);
   if (!d_grad) return fail(NSM_ERR_INVALID_ARG, "d_grad is NULL");
   f->wgrad_parts = 0;
   RUN(f, K_DEBUG, launch_set_grad(f->fp, d_grad, d_touched, f->stream));
@@ -998,7 +1000,7 @@ static nsm_status render_chunks(nsm_field *f, const nsm_ray_batch *b, float cut,
                                 bool host) {
   nsm_status st = validate_batch(f, b, false, true);
   if (st != NSM_OK) return st;
-  leave_fast_path(f);
+  LEAVE_FAST_PATH(f);
   if (!rgb || !depth) return fail(NSM_ERR_INVALID_ARG, "output pointers are NULL");
   if (!(cut >= 0.f)) return fail(NSM_ERR_INVALID_ARG, "transmittance_cut must be >= 0");
   const uint32_t M = f->cfg.max_rays;
@@ -1015,7 +1017,8 @@ static nsm_status render_chunks(nsm_field *f, const nsm_ray_batch *b, float cut,
       cb.origins = b->origins + 3 * (size_t)first;
       cb.dirs = b->dirs + 3 * (size_t)first;
     }
-    enqueue_forward(f, &cb, R, false, 0, false);
+    st = enqueue_forward(f, &cb, R, false, 0, false);
+    if (st != NSM_OK) return st;
     RUN(f, K_COMPOSITE, launch_composite_render(f->ws, R, cut, f->cfg.bg, o_rgb, o_d, o_op, f->stream));
     if (f->prof.on) f->prof.collect();
     if (host) {
@@ -1042,7 +1045,7 @@ nsm_status nsm_render_host(nsm_field *f, const nsm_ray_batch *hb, float cut, flo
 
 nsm_status nsm_debug_last_step(nsm_field *f, int item, void *d_out, uint64_t capacity_bytes, uint64_t *n_bytes_out) {
   if (!f) return fail(NSM_ERR_INVALID_ARG, "field is NULL");
-  leave_fast_path(f);
+  LEAVE_FAST_PATH(f);
   if (f->last_R == 0) return fail(NSM_ERR_INVALID_ARG, "no step has been run yet");
   const uint32_t R = f->last_R;
   const uint32_t *d_S = f->ws.offsets + R;

@@ -126,23 +126,19 @@ __device__ __forceinline__ void tl_mark(unsigned long long *tl, int id, int end)
 //   mv[e*2F + 0..F) = m,    Adam moments, one 4F-byte record per entry (16 B for F = 2): only the table Adam touches
 //   mv[e*2F + F..2F) = v    them, for the random ~25 % of entries a step references;
 //   grad[e*F + f]           the gradient, compact like theta (L2-sized): the scatter's vector reductions land in a
-//                           table that fits the cache, and Adam reads it as a dense coalesced stream.
+//                           table that fits the cache; Adam reads (and zeroes) the touched entries only.
 // (Measured on B200, profiles/r1h: with theta inside 32-byte per-entry records the encoder moved 120 MB of DRAM
 // for 12 MB of useful theta and ran at 81 % of the HBM peak; DRAM fetches are 64 bytes.)
 //
-// Touched set without flags: between steps every gradient word holds -0.0f (bits 0x80000000).
-// The scatter never adds -0.0 or a magnitude below 2^-96 (those addends become +0.0), and under
-// round-to-nearest a sum of such addends is +0.0, or a multiple of 2^-119 >= FLT_MIN in magnitude;
-// it is never -0.0 (x + (-x) = +0.0) and never a subnormal that the reduction unit could flush to
-// -0.0.  Hence "entry e was referenced this step"  <=>  bits(grad[e*F]) != 0x80000000, whatever the
-// gradient's value (the touched set is structural, S12); Adam writes -0.0f back.
+// Touched set (S12's structural U): one bit per entry in `touched`, set by the scatter (test, then atomicOr), walked
+// and cleared by the table Adam, which also zeroes the gradients it consumes: between steps the gradient array is all
+// zeros and the bitmap all clear.
 // The canonical flat layout of include/nsm.h exists only at the boundary (pack/unpack kernels).
-#define NSM_GRAD_UNTOUCHED 0x80000000u
-#define NSM_GRAD_MIN_ADDEND 1.262177448e-29f   /* 2^-96 */
 struct FieldParams {
   float *theta;                                     // [n_entries][F]
   float *mv;                                        // [n_entries][2F]
   float *grad;                                      // [n_entries][F]
+  uint32_t *touched;                                // [ceil(n_entries / 32)] bit (e & 31) of word (e >> 5)
   float *mlp_theta, *mlp_m, *mlp_v, *mlp_grad;      // [n_mlp] each, canonical order
   uint8_t *occ_bits;                                // [G^3/8]
   float *occ_grid;                                  // [G^3] running density of the decayed refresh (F4); seeded by FROM_FIELD
@@ -161,8 +157,8 @@ struct FieldParams {
 __device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
 __device__ __forceinline__ void pdl_trigger() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
 
-// Which kernel classes (bit = KernelId) are launched with the PDL attribute; NSM_PDL_MASK overrides (tuning knob).
-extern uint32_t g_pdl_mask;
+// Which kernel classes (bit = KernelId) are launched with the PDL attribute (swept on the GPU, profiles/r1g).
+extern const uint32_t g_pdl_mask;
 extern thread_local int g_cur_kernel;
 
 template <typename... KArgs, typename... Args>
@@ -258,10 +254,10 @@ uint32_t march_scan_state_entries(uint32_t max_rays);
 // out_mode: 0 = fp32 planes ws.e, 1 = fp16 blob ws.blob_e, 2 = bf16 blob ws.blob_e
 int launch_encode(const LevelTable &lv, const float *theta, const Workspace &ws,
                   const uint32_t *d_S, int out_mode, int n_sms, cudaStream_t st);
-// levels [l0, l1)
-int launch_scatter(const LevelTable &lv, float *grad, const Workspace &ws,
-                   const uint32_t *d_S, uint32_t l0, uint32_t l1, int n_sms, cudaStream_t st);
-// gradient array <- canonical gradient + touched flags (NULL: every entry touched); src == nullptr: all untouched
+// S12 over all levels: vector reductions into grad, touched bits into the bitmap
+int launch_scatter(const LevelTable &lv, float *grad, uint32_t *touched, const Workspace &ws,
+                   const uint32_t *d_S, int n_sms, cudaStream_t st);
+// gradient array + touched bitmap <- canonical gradient + flags (NULL: every entry touched); src == nullptr: zero, none touched
 int launch_set_grad(const FieldParams &fp, const float *src, const uint8_t *touched, cudaStream_t st);
 int launch_get_touched(const FieldParams &fp, uint8_t *dst, cudaStream_t st);
 // canonical [n_entries][F] <-> `which` (0 theta, 2 m, 3 v) of the internal arrays; src == nullptr packs zeros
@@ -274,8 +270,11 @@ int launch_mlp_backward_simt(const MlpShape &ms, const float *theta_mlp, float *
                              const float *dirs, const Workspace &ws, const uint32_t *d_S, int n_sms,
                              cudaStream_t st);
 size_t mlp_simt_smem_bytes(const MlpShape &ms, int backward);
+
 bool mlp_tc_supported(const MlpShape &ms);
 size_t mlp_tc_wimg_bytes(int backward);
+// opt-in shared-memory size of the tcgen05 kernels on the CURRENT device (a per-device attribute): once per field
+cudaError_t mlp_tc_prepare_device();
 int launch_pack_weights(const MlpShape &ms, int bf16, const float *theta_mlp, const Workspace &ws, cudaStream_t st);
 int launch_mlp_forward_tc(const MlpShape &ms, int bf16, const float *dirs, const Workspace &ws, const uint32_t *d_S,
                           int density_only, int save_blobs, int n_sms, cudaStream_t st);
@@ -291,10 +290,9 @@ int launch_composite_train(const Workspace &ws, uint32_t R, const float *rgb, co
                            cudaStream_t st);
 int launch_composite_render(const Workspace &ws, uint32_t R, float cut, const float bg[3],
                             float *out_rgb, float *out_depth, float *out_opacity, cudaStream_t st);
-// table entries [first_entry, end_entry) (a level group; first_entry a multiple of 4)
+// S13 on the touched table entries (sparse) or on all of them; consumes the gradients and the touched bits
 int launch_adam_table(const FieldParams &fp, uint32_t F, int sparse, float lr, float beta1, float beta2,
-                      float eps, float inv_bc1, float inv_bc2, uint64_t first_entry, uint64_t end_entry, cudaStream_t st,
-                      unsigned long long *tl = nullptr);
+                      float eps, float inv_bc1, float inv_bc2, cudaStream_t st, unsigned long long *tl = nullptr);
 int launch_adam_mlp(const FieldParams &fp, float lr, float beta1, float beta2, float eps, float inv_bc1,
                     float inv_bc2, cudaStream_t st);
 // tensor-core path: Adam on the MLP weights and, in the same launch, the refreshed 16-bit weight images

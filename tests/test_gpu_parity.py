@@ -16,56 +16,7 @@ FWD_ITEMS = ("counts", "offsets", "s_ray", "s_k", "s_t", "s_delta", "s_x", "slot
              "C", "D_hat", "O", "dsigma", "drgb", "grad", "touched")
 
 
-@pytest.fixture(scope="module")
-def nsm():
-    import torch
-    if not torch.cuda.is_available():
-        pytest.skip("needs a CUDA device")
-    from paper_2210_13641_b200 import build
-    build.build()
-    import paper_2210_13641_b200 as mod
-    return mod
-
-
-# the encoder output is fp32 on the CUDA-core path and a two-term 16-bit expansion on the tensor-core path
-E_TOL = {"simt_fp32": 1e-4, "tcgen05_f16": 1e-4, "tcgen05_bf16": 1e-4}   # two-term (hi + lo) tiles
-
-
-def tol_for(fc, path):
-    """BASELINE.json north_star: 1e-4 on the fp32 configuration, 2e-2 where the configuration asks
-    for fp16/bf16 MLPs.  While such a configuration still runs on the fp32 CUDA-core path it is held
-    to 1e-3 (fp32 with the cancellation of up to 512 samples per ray in S10 and of colliding hash
-    slots in S12; DESIGN.md "Tolerances")."""
-    if fc.mlp_precision == 0:
-        return 1e-4
-    return 1e-3 if path == "simt_fp32" else 2e-2
-
-
-def assert_close(name, got, ref, tol, scale=None):
-    got = np.asarray(got, np.float64)
-    ref = np.asarray(ref, np.float64)
-    assert got.shape == ref.shape, (name, got.shape, ref.shape)
-    if ref.size == 0:
-        return
-    s = np.abs(ref).max() if scale is None else scale
-    err = np.abs(got - ref) - tol * np.maximum(np.abs(ref), s)
-    assert err.max() <= 0, f"{name}: max excess {err.max():.3e}, scale {s:.3e}, worst at {np.argmax(err)}"
-
-
-def make_pair(nsm, w, seed=0, table_scale=0.1, mlp_scale=1.0):
-    fc = w.field
-    f = nsm.Field(fc, "cuda:0")
-    theta0 = configs.init_params(seed, f.n_table, f.mlp_shapes())
-    theta0[:f.n_table] *= table_scale / 1e-4
-    theta0[f.n_table:] *= mlp_scale
-    f.nsm_set_params(theta0)
-    O = orc.Oracle(fc, theta0)
-    assert (O.n_table, O.n_mlp) == (f.n_table, f.n_mlp)
-    assert np.array_equal(O.res, f.res) and np.array_equal(O.offset, f.offset)          # P1: S0 tables
-    if w.bits is not None:
-        f.nsm_update_occupancy(nsm.NSM_OCC_SET, w.bits)
-        O.set_occupancy(w.bits)
-    return f, O, theta0
+from tests.gpu_common import E_TOL, assert_close, make_pair, tol_for  # noqa: E402
 
 
 def check_backward(nsm, f, O, b, lam, tol, per_level_grad=True):
@@ -106,15 +57,11 @@ def check_backward(nsm, f, O, b, lam, tol, per_level_grad=True):
             assert np.abs(gr).max() <= 1e-12, name
             continue
         assert np.linalg.norm(gr - rr) <= tol * nrm, (name, np.linalg.norm(gr - rr) / nrm)
-        # element-wise: every entry within tol*max|g_ref| in fp32.  With 16-bit MLP operands a hidden
-        # pre-activation within rounding of zero flips its ReLU mask against float64 and moves the few-sample
-        # entries of the fine levels by a whole term: there 99.9 % of the entries must be within tol*max and
-        # all within 10*tol*max.
+        # element-wise (P4 as SURVEY.md 8(c) states it): every entry within tol * max|g_ref| of its tensor, on every
+        # path.  Measured worst case on the tensor-core paths with the two-term forward (ReLU masks agree with the
+        # oracle): 4.2e-3 (fp16, cfg 3), 9.2e-3 (bf16, cfg 4 shapes) -- DESIGN.md "Tolerances".
         err = np.abs(gr - rr) / np.abs(rr).max()
-        if f.fc.mlp_precision == 0 or f.nsm_mlp_path() == "simt_fp32":
-            assert err.max() <= tol, (name, err.max())
-        else:
-            assert np.mean(err <= tol) >= 0.999 and err.max() <= 10 * tol, (name, np.mean(err <= tol), err.max())
+        assert err.max() <= tol, (name, err.max())
     return st, so, g, tr
 
 
@@ -532,10 +479,7 @@ def _check_pose(nsm, f, O, b, lam, tol):
         assert np.abs(ref).max() > 0, name
         assert np.linalg.norm(got - ref) <= tol * np.linalg.norm(ref), (name, np.linalg.norm(got - ref) / np.linalg.norm(ref))
         err = np.abs(got - ref) / np.abs(ref).max()
-        if f.nsm_mlp_path() == "simt_fp32":
-            assert err.max() <= tol, (name, err.max())
-        else:   # 16-bit MLP operands: a ReLU mask flipped against float64 moves single rays by a whole term (as in P4)
-            assert np.mean(err <= tol) >= 0.999 and err.max() <= 10 * tol, (name, np.mean(err <= tol), err.max())
+        assert err.max() <= tol, (name, err.max())                  # P4, element-wise, every path
     return go, tau, tr
 
 
@@ -669,19 +613,30 @@ def test_occupancy_decay_update_against_the_oracle(nsm):
     assert np.array_equal(f.nsm_get_occupancy(), a)
     with pytest.raises(nsm.NsmError):
         f.nsm_update_occupancy_decay(0, 0.9)
+    # SET / FULL discard the running grid: a partial pass would cull every cell it does not visit, so the call refuses
+    # until FROM_FIELD has seeded the grid again, and the strided schedule restarts at subset 0
+    for mode, arg in ((nsm.NSM_OCC_FULL, None), (nsm.NSM_OCC_SET, a)):
+        f.nsm_update_occupancy(mode, arg)
+        with pytest.raises(nsm.NsmError) as ei:
+            f.nsm_update_occupancy_decay(4, 0.9)
+        assert ei.value.status == 1
+    f.nsm_update_occupancy(nsm.NSM_OCC_FROM_FIELD)
+    f.nsm_update_occupancy_decay(4, 0.9)
     f.close()
 
 
 # ---------------------------------------------------------------------------- measurement helpers of the boundary
 
-def test_timeline_and_l2_probe(nsm, monkeypatch):
-    """nsm_debug_timeline: with NSM_TIMELINE=1 every hot-path kernel of a step stamps start <= end, and the kernels of one
-    stream appear in launch order; nsm_probe_l2 returns a plausible rate (cache-resident faster than DRAM-resident)."""
-    monkeypatch.setenv("NSM_TIMELINE", "1")
+def test_debug_timeline(nsm):
+    """nsm_debug_timeline: with NSM_OPT_DEBUG_TIMELINE every hot-path kernel of a step stamps start <= end, and the kernels
+    of one stream appear in launch order."""
     w = configs.config2(R=1024, K=128)
     f = nsm.Field(w.field, "cuda:0")
     f.nsm_set_params(configs.init_params(2, f.n_table, f.mlp_shapes()))
     f.nsm_update_occupancy(nsm.NSM_OCC_SET, w.bits)
+    with pytest.raises(nsm.NsmError):
+        f.nsm_debug_timeline()                               # not enabled yet
+    f.nsm_set_option(nsm.NSM_OPT_DEBUG_TIMELINE, 1)
     for _ in range(3):
         f.nsm_train_step(nsm.DeviceBatch(w.batches[0]), w.lambda_d)
     tl = f.nsm_debug_timeline().astype(np.int64)
@@ -693,11 +648,6 @@ def test_timeline_and_l2_probe(nsm, monkeypatch):
     assert all(start[order[i + 1]] >= start[order[i]] for i in range(6)), start
     assert start[7] >= end[4]                                # the MLP Adam (side stream) starts after the MLP backward
     f.close()
-    monkeypatch.delenv("NSM_TIMELINE")
-    fast = nsm.probe_l2(24 << 20, 1 << 21, False)
-    slow = nsm.probe_l2(1 << 30, 1 << 21, False)
-    red = nsm.probe_l2(24 << 20, 1 << 21, True)
-    assert 5e9 < slow < fast < 1e12 and 5e9 < red < 1e12, (fast, slow, red)
 
 
 @pytest.mark.parametrize("F,L,log2T", [(1, 6, 12), (8, 3, 11), (4, 5, 10)])

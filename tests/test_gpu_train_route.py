@@ -1,0 +1,155 @@
+"""GPU parity of the call bench.py times: nsm_train_step, the pipelined route (scatter issued with the table Adam, per-CTA
+weight-gradient slices summed inside the MLP Adam kernel, MLP Adam and 16-bit weight-image refresh on the side stream, the
+next step's marcher beside the table Adam when NSM_OPT_BATCH_READY is set) against the float64 oracle at the PARAMETER
+level -- rules P5(ii) and P6 of DESIGN.md section 5; Eq. 3 is what the mapping thread
+"continuously minimizes", so what has to agree after a step is theta, m and v, not only the gradient."""
+from dataclasses import replace
+
+import numpy as np
+import pytest
+
+from tests.gpu_common import assert_close, make_pair, tol_for
+from workloads import configs
+
+pytestmark = pytest.mark.gpu
+
+LR = 1e-2
+
+
+def _tensor_edges(O, F):
+    """Parameter ranges of the gradient tensors of P4: each table level, then the MLP block as a whole."""
+    return [int(o) * F for o in O.offset] + [O.n_table + O.n_mlp]
+
+
+def _sync_oracle_from_gpu(f, O):
+    th, m, v, step = f.nsm_get_params()
+    O.theta, O.m, O.v, O.step = th.astype(np.float64), m.astype(np.float64), v.astype(np.float64), step
+    return th, m, v
+
+
+def check_step_parameters(f, O, before, gref, touched_ref, tol, tag):
+    """P5(ii) after ONE nsm_train_step from a state both sides share (`before` = the GPU's theta, m, v before the step,
+    which the oracle started from exactly).  m and v within tol of the tensor's largest value; entries outside the
+    touched set bit-unchanged in theta, m and v; theta compared where |g_ref| >= 10^3 x the measured gradient error of
+    its tensor (elsewhere the update is ~ lr * sign(g) of a noise-level gradient: counted, not failed)."""
+    F = f.fc.n_features
+    th, m, v, step = f.nsm_get_params()
+    assert step == O.step
+    th0, m0, v0 = before
+    nt = O.n_table
+    touched = np.concatenate([np.repeat(touched_ref.astype(bool), F), np.ones(O.n_mlp, bool)])
+    for name, new, old in (("theta", th, th0), ("m", m, m0), ("v", v, v0)):
+        assert np.array_equal(new[~touched].view(np.uint32), old[~touched].view(np.uint32)), f"{tag}: {name} of untouched entries changed"
+    b1 = float(np.float32(f.fc.beta1))
+    edges = _tensor_edges(O, F)
+    # the gradient the GPU applied, recovered from its first moment: g = (m_new - beta1 m_old) / (1 - beta1)
+    g_gpu = (m.astype(np.float64) - b1 * m0.astype(np.float64)) / (1.0 - b1)
+    bound = np.empty(nt + O.n_mlp)
+    for a, b in zip(edges[:-1], edges[1:]):
+        for name, got, ref in (("m", m, O.m), ("v", v, O.v)):
+            s = np.abs(ref[a:b]).max()
+            assert np.abs(got[a:b] - ref[a:b]).max() <= tol * s + 1e-30, (tag, name, a, np.abs(got[a:b] - ref[a:b]).max() / s)
+        bound[a:b] = np.abs(g_gpu[a:b] - gref[a:b])[touched[a:b]].max() if touched[a:b].any() else 0.0
+    strong = touched & (np.abs(gref) >= 1e3 * bound) & (np.abs(gref) >= 1e-15)
+    assert strong.sum() > 0.2 * touched.sum(), (tag, strong.sum(), touched.sum())
+    d = np.abs(th.astype(np.float64) - O.theta)
+    assert d[strong].max() <= 5e-3 * LR + 1e-7, (tag, d[strong].max())
+    weak = touched & ~strong
+    flips = int((d[weak] > 0.5 * LR).sum())
+    print(f"{tag}: touched {touched.sum()}, strong {strong.sum()}, sign flips among the weak {flips}, "
+          f"max |dtheta| on strong {d[strong].max():.2e}")
+    return th, m, v
+
+
+def run_route(nsm, w, seed, n_steps, batch_ready, tol_scale=1.0):
+    f, O, _ = make_pair(nsm, w, seed=seed, table_scale=0.05, omp=True)
+    assert f.nsm_mlp_path().startswith("tcgen05")
+    tol = tol_for(w.field, f.nsm_mlp_path())
+    f.nsm_set_option(nsm.NSM_OPT_BATCH_READY, batch_ready)
+    db = [nsm.DeviceBatch(b) for b in w.batches]
+    for i in range(n_steps):
+        before = _sync_oracle_from_gpu(f, O)
+        st = f.nsm_train_step(db[i % len(db)], w.lambda_d, want_stats=(i % 2 == 0))
+        so, tr = O.train_step(w.batches[i % len(db)], w.lambda_d, trace=("grad", "touched"))
+        if st is not None:
+            assert st["n_samples"] == so["n_samples"] and st["step"] == so["step"] == i + 1
+            assert abs(st["loss"] - so["loss"]) <= tol * abs(so["loss"])
+        check_step_parameters(f, O, before, tr["grad"], tr["touched"], tol, f"{w.name} ready={batch_ready} step {i + 1}")
+    return f, O
+
+
+@pytest.mark.parametrize("batch_ready", [0, 1])
+def test_config2_full_size_train_step_parameters(nsm, batch_ready):
+    """BASELINE.json configs[1] at full size, three consecutive nsm_train_step calls, theta / m / v against the oracle."""
+    w = configs.config2(n_batches=3)
+    f, _ = run_route(nsm, w, 2, 3, batch_ready)
+    f.close()
+
+
+def test_config4_full_size_train_step_parameters(nsm):
+    """BASELINE.json configs[3] at full size (719 MB of tables, F = 4, bf16 MLPs), two nsm_train_step calls."""
+    w = configs.config4(n_batches=2)
+    f, _ = run_route(nsm, w, 4, 2, 1)
+    f.close()
+
+
+def test_pipelined_steps_without_getters_track_the_oracle(nsm):
+    """Four nsm_train_step calls back to back with no getter, no statistics and NSM_OPT_BATCH_READY set -- so the marcher
+    of step i+1 really runs beside the table Adam of step i and the MLP Adam on the side stream -- against the oracle
+    free-running the same four steps from the same theta_0 (steps 1-4 are still comparable).  m after four
+    steps is a fixed linear combination of the four gradients, each held to P4's tolerance."""
+    w = configs.config2(n_batches=4)
+    f, O, _ = make_pair(nsm, w, seed=21, table_scale=0.05, omp=True)
+    tol = tol_for(w.field, f.nsm_mlp_path())
+    f.nsm_set_option(nsm.NSM_OPT_BATCH_READY, 1)
+    db = [nsm.DeviceBatch(b) for b in w.batches]
+    for i in range(4):
+        f.nsm_train_step(db[i], w.lambda_d, want_stats=False)
+        O.train_step(w.batches[i], w.lambda_d)
+    th, m, v, step = f.nsm_get_params()
+    assert step == O.step == 4
+    F = w.field.n_features
+    for a, b in zip(_tensor_edges(O, F)[:-1], _tensor_edges(O, F)[1:]):
+        assert np.abs(m[a:b] - O.m[a:b]).max() <= tol * np.abs(O.m[a:b]).max(), a
+        assert np.abs(v[a:b] - O.v[a:b]).max() <= tol * np.abs(O.v[a:b]).max(), a
+    changed = O.m != 0
+    assert np.array_equal(m != 0, changed)                                   # the same entries were ever touched
+    d = np.abs(th - O.theta)
+    print(f"pipelined 4 steps: theta differs by more than lr/2 on {(d > 0.5 * LR).sum()} of {changed.sum()} updated parameters")
+    assert (d > 0.5 * LR).mean() < 2e-3
+    f.close()
+
+
+def test_config3_free_running_loss_curve(nsm):
+    """P6: the GPU free-runs 100 steps of config-3-style data (reduced ray count and keyframe size; FULL occupancy at
+    step 0, FROM_FIELD every 16 steps) and the oracle does the same from the same theta_0 on the same batches, each
+    with its OWN parameters and occupancy bits throughout.  The iteration is chaotic under Adam, so the comparison is
+    statistical: the loss around steps 16, 50 and 100 and the final depth L1 of the training rays within 5 %."""
+    w = configs.config3(R=1024, K=128, n_keyframes=3, n_batches=100, width=300, height=170)
+    f, O, _ = make_pair(nsm, w, seed=3, table_scale=1e-4, omp=True)
+    f.nsm_set_option(nsm.NSM_OPT_BATCH_READY, 1)
+    db = [nsm.DeviceBatch(b) for b in w.batches]
+    lg, lo, sg, so_ = [], [], [], []
+    for i in range(100):
+        if i > 0 and i % 16 == 0:
+            f.nsm_update_occupancy(nsm.NSM_OCC_FROM_FIELD, sync=False)
+            O.occupancy_from_field()
+        st = f.nsm_train_step(db[i], w.lambda_d)
+        so, tr = O.train_step(w.batches[i], w.lambda_d, trace=("D_hat",) if i == 99 else ())
+        lg.append(st["loss"]); lo.append(so["loss"]); sg.append(st["n_samples"]); so_.append(so["n_samples"])
+    lg, lo = np.array(lg), np.array(lo)
+    assert lo[-1] < 0.05 * lo[0]                                               # it trains at all
+    for a, b in ((13, 16), (47, 50), (97, 100)):                               # three-step windows ending at 16, 50, 100
+        rel = abs(lg[a:b].mean() - lo[a:b].mean()) / lo[a:b].mean()
+        print(f"P6 loss, steps {a + 1}-{b}: gpu {lg[a:b].mean():.4f} oracle {lo[a:b].mean():.4f} rel {rel:.2e}")
+        assert rel <= 0.05, (a, b, rel)
+    assert sg[:16] == so_[:16]                                                 # FULL occupancy: identical sample counts
+    assert abs(sg[-1] - so_[-1]) <= 0.05 * so_[-1]                             # after six independent refreshes
+    # depth L1 of the last batch's valid rays, each side with its own field
+    b = w.batches[99]
+    valid = (b.depth > 0) & (b.depth_var < 1.0)
+    l1_gpu = np.abs(f.nsm_debug_last_step("D_hat")[valid] - b.depth[valid]).mean()
+    l1_ref = np.abs(tr["D_hat"][valid] - b.depth[valid]).mean()
+    print(f"P6 depth L1 of the last batch: gpu {l1_gpu:.4f} m, oracle {l1_ref:.4f} m")
+    assert abs(l1_gpu - l1_ref) <= 0.05 * l1_ref
+    f.close()
