@@ -122,7 +122,11 @@ typedef enum {
   NSM_DBG_DSIGMA = 15,   /* f32 [S] */
   NSM_DBG_DRGB = 16,     /* f32 [S,3] */
   NSM_DBG_GRAD = 17,     /* f32 [P]        canonical layout; valid after nsm_backward */
-  NSM_DBG_TOUCHED = 18   /* u8  [n_entries] valid after nsm_backward */
+  NSM_DBG_TOUCHED = 18,  /* u8  [n_entries] valid after nsm_backward */
+  /* the hidden activations the backward pass takes its ReLU masks from (training steps / nsm_backward only) */
+  NSM_DBG_HIDDEN_DENSITY = 19, /* f32 [S, density_hidden]  h  = ReLU(W_d1 e) */
+  NSM_DBG_HIDDEN_COLOR1 = 20,  /* f32 [S, color_hidden]    h1 = ReLU(W_c1 [g slice, Y]) */
+  NSM_DBG_HIDDEN_COLOR2 = 21   /* f32 [S, color_hidden]    h2 = ReLU(W_c2 h1); empty with one hidden colour layer */
 } nsm_debug_item;
 
 /* Create a field on the current CUDA device (which must be an sm_100 part: the library holds sm_100a code only); the

@@ -22,7 +22,8 @@ DEBUG_ITEMS = dict(counts=(0, np.uint32), offsets=(1, np.uint32), s_ray=(2, np.u
                    s_t=(4, np.float32), s_delta=(5, np.float32), s_x=(6, np.float32), slots=(7, np.uint32),
                    w=(8, np.float32), e=(9, np.float32), sigma=(10, np.float32), rgb=(11, np.float32),
                    C=(12, np.float32), D_hat=(13, np.float32), O=(14, np.float32), dsigma=(15, np.float32),
-                   drgb=(16, np.float32), grad=(17, np.float32), touched=(18, np.uint8))
+                   drgb=(16, np.float32), grad=(17, np.float32), touched=(18, np.uint8),
+                   hidden_density=(19, np.float32), hidden_color1=(20, np.float32), hidden_color2=(21, np.float32))
 
 EXPORTS = ["nsm_create_field", "nsm_destroy_field", "nsm_update_occupancy", "nsm_get_occupancy",
            "nsm_train_step", "nsm_train_step_host", "nsm_backward", "nsm_apply_adam", "nsm_debug_set_grad",
@@ -415,7 +416,9 @@ class Field:
         torch.cuda.synchronize(self.device)
         a = buf[:n.value].cpu().numpy().view(dt)
         L, F = self.fc.n_levels, self.fc.n_features
-        shape = dict(s_x=(-1, 3), slots=(-1, L, 8), w=(-1, L, 3), e=(-1, L * F), rgb=(-1, 3), C=(-1, 3), drgb=(-1, 3))
+        shape = dict(s_x=(-1, 3), slots=(-1, L, 8), w=(-1, L, 3), e=(-1, L * F), rgb=(-1, 3), C=(-1, 3), drgb=(-1, 3),
+                     hidden_density=(-1, self.fc.density_hidden), hidden_color1=(-1, self.fc.color_hidden),
+                     hidden_color2=(-1, self.fc.color_hidden))
         return a.reshape(shape[name]) if name in shape else a
 
     def nsm_total_samples(self):

@@ -1,8 +1,8 @@
 // adam.cu — S13 of DESIGN.md "Algorithm": Adam with bias correction (the paper names no
 // optimiser, PAPER.md:133 only says L_M is minimised; reading R16).  Tables: only the entries
 // of the structural touched set U are updated when sparse_table_adam = 1 — untouched entries
-// keep theta, m, v bit-unchanged.  The gradients of the touched entries are zeroed and the touched bits
-// cleared in the same pass, so the next step's scatter starts clean without a separate memset.
+// keep theta, m, v bit-unchanged.  The gradient words are reset to "untouched" in the same pass,
+// so the next step's scatter starts clean without a separate memset.
 #include "nsm_internal.cuh"
 #include "table_ops.cuh"
 
@@ -10,20 +10,28 @@ namespace {
 
 using namespace tableops;
 
-// One block per ADAM_ENTRIES consecutive table entries (body: tableops::adam_block).  The touched set arrives as a bitmap
-// written by the scatter; the block walks its 512 bytes of it and then touches only what the touched entries need: their
-// gradient, their theta, their moment record.  Nothing is scanned densely (round 1's kernel read all of the gradient
-// array to find the touched 25 %: 48.8 MB at config 2, 719 MB at config 4).
+// One block per chunk of ADAM_CHUNK_FLOATS / F consecutive entries, two phases.
+//  1. The chunk's gradient words are read densely (coalesced 16-byte loads, four independent ones
+//     per thread; the array is L2-hot, the scatter has just written it).  Entries whose first word
+//     is not -0.0f (FieldParams: "referenced this step") are compacted into shared memory
+//     (index + gradient), warp-aggregated.
+//  2. The block walks the compact list: every thread has a touched entry, loads its theta (compact
+//     array) and its moment record (m | v; 16 bytes for F = 2; two entries in flight per thread),
+//     updates and stores them.  The 16-byte gradient words that held a touched entry are then reset to
+//     -0.0f, so the next step's scatter starts from "untouched" without a separate pass.
+// sparse = 0 (dense Adam, textbook): every entry goes through phase 2.
 template <int F>
 __global__ void __launch_bounds__(ADAM_THREADS) adam_table_kernel(float *__restrict__ theta, float *__restrict__ mv, float *__restrict__ grad,
-                                                                  uint32_t *__restrict__ touched, uint64_t n_entries, int sparse,
-                                                                  AdamConst c, unsigned long long *tl) {
-  __shared__ uint16_t list_e[ADAM_ENTRIES];            // local indices of the block's touched entries, ascending
-  __shared__ uint32_t warp_tot[ADAM_WORDS / 32];
+                                                                  uint64_t first_entry, uint64_t n_entries, int sparse, AdamConst c,
+                                                                  unsigned long long *tl) {
+  constexpr int CH = ADAM_CHUNK_FLOATS / F;
+  __shared__ float list_g[ADAM_CHUNK_FLOATS];          // compacted gradients, F floats per touched entry
+  __shared__ uint16_t list_e[CH];                      // compacted local entry indices
+  __shared__ uint32_t cnt;
   pdl_wait();
   pdl_trigger();
   tl_mark(tl, K_ADAM_TABLE, 0);
-  adam_block<F>(theta, mv, grad, touched, (uint64_t)blockIdx.x * ADAM_ENTRIES, n_entries, sparse, c, list_e, warp_tot);
+  adam_chunk<F>(theta, mv, grad, first_entry + (uint64_t)blockIdx.x * CH, n_entries, sparse, c, list_g, list_e, &cnt);
   tl_mark(tl, K_ADAM_TABLE, 1);
 }
 
@@ -43,12 +51,13 @@ __global__ void adam_dense_kernel(float *__restrict__ theta, float *__restrict__
 int launch_adam_table(const FieldParams &fp, uint32_t F, int sparse, float lr, float beta1, float beta2, float eps,
                       float inv_bc1, float inv_bc2, cudaStream_t st, unsigned long long *tl) {
   AdamConst c{lr, beta1, beta2, eps, inv_bc1, inv_bc2};
-  dim3 grid((unsigned)((fp.n_entries + ADAM_ENTRIES - 1) / ADAM_ENTRIES)), block(ADAM_THREADS);
+  const uint64_t chunk = ADAM_CHUNK_FLOATS / F, first_entry = 0, end_entry = fp.n_entries;
+  dim3 grid((unsigned)((end_entry - first_entry + chunk - 1) / chunk)), block(ADAM_THREADS);
   switch (F) {
-    case 1: launch_pdl(adam_table_kernel<1>, grid, block, 0, st, fp.theta, fp.mv, fp.grad, fp.touched, fp.n_entries, sparse, c, tl); break;
-    case 2: launch_pdl(adam_table_kernel<2>, grid, block, 0, st, fp.theta, fp.mv, fp.grad, fp.touched, fp.n_entries, sparse, c, tl); break;
-    case 4: launch_pdl(adam_table_kernel<4>, grid, block, 0, st, fp.theta, fp.mv, fp.grad, fp.touched, fp.n_entries, sparse, c, tl); break;
-    default: launch_pdl(adam_table_kernel<8>, grid, block, 0, st, fp.theta, fp.mv, fp.grad, fp.touched, fp.n_entries, sparse, c, tl); break;
+    case 1: launch_pdl(adam_table_kernel<1>, grid, block, 0, st, fp.theta, fp.mv, fp.grad, first_entry, end_entry, sparse, c, tl); break;
+    case 2: launch_pdl(adam_table_kernel<2>, grid, block, 0, st, fp.theta, fp.mv, fp.grad, first_entry, end_entry, sparse, c, tl); break;
+    case 4: launch_pdl(adam_table_kernel<4>, grid, block, 0, st, fp.theta, fp.mv, fp.grad, first_entry, end_entry, sparse, c, tl); break;
+    default: launch_pdl(adam_table_kernel<8>, grid, block, 0, st, fp.theta, fp.mv, fp.grad, first_entry, end_entry, sparse, c, tl); break;
   }
   return 1;
 }

@@ -133,8 +133,8 @@ __global__ void __launch_bounds__(256) encode_forward_kernel(LevelTable lv, cons
 // with a segmented warp scan and only the run's first lane issues the reductions -- the L2 reduction rate is what bounds
 // this kernel (profiles/r1p), so fewer reductions is the only way to make it faster.
 template <int F>
-__global__ void __launch_bounds__(256) scatter_backward_kernel(LevelTable lv, float *__restrict__ grad, uint32_t *__restrict__ touched,
-                                                               Workspace ws, const uint32_t *__restrict__ d_S, uint32_t l0, uint32_t l1) {
+__global__ void __launch_bounds__(256) scatter_backward_kernel(LevelTable lv, float *__restrict__ grad, Workspace ws,
+                                                               const uint32_t *__restrict__ d_S, uint32_t l0, uint32_t l1) {
   pdl_wait();
   pdl_trigger();
   tl_mark(ws.timeline, K_SCATTER, 0);
@@ -151,7 +151,7 @@ __global__ void __launch_bounds__(256) scatter_backward_kernel(LevelTable lv, fl
     const uint32_t l_first = __shfl_sync(0xffffffffu, l, 0);
     const bool one_dense_level = __all_sync(0xffffffffu, l == l_first) && lv.dense[l_first];
     if (!one_dense_level) {
-      if (valid) scatter_sample_level<F>(lv, grad, touched, ws, l, s, pol_last);
+      if (valid) scatter_sample_level<F>(lv, grad, ws, l, s, pol_last);
       continue;
     }
     uint32_t slot[8];
@@ -173,32 +173,26 @@ __global__ void __launch_bounds__(256) scatter_backward_kernel(LevelTable lv, fl
           if (lane + d < run_end) val[k][f] += o;
         }
     }
-    if (valid && ((heads >> lane) & 1u)) issue_corner_reds<F>(lv, grad, touched, l, slot, val, pol_last);
+    if (valid && ((heads >> lane) & 1u)) issue_corner_reds<F>(lv, grad, l, slot, val, pol_last);
   }
   tl_mark(ws.timeline, K_SCATTER, 1);
 }
 
-// gradient array and touched bitmap <- canonical gradient and flags (debug / test entry point; also the reset).
-// One thread per bitmap word: its 32 entries' flags and gradients.  src == nullptr: all zero, nothing touched.
-__global__ void set_grad_kernel(float *__restrict__ grad, uint32_t *__restrict__ bitmap, uint32_t F, uint64_t n_entries,
-                                const float *__restrict__ src, const uint8_t *__restrict__ touched) {
-  const uint64_t n_words = (n_entries + 31) / 32;
-  for (uint64_t w = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; w < n_words; w += (uint64_t)gridDim.x * blockDim.x) {
-    uint32_t bits = 0;
-    for (uint32_t b = 0; b < 32; ++b) {
-      const uint64_t e = w * 32 + b;
-      if (e >= n_entries) break;
-      const bool t = src && (!touched || touched[e]);
-      if (t) bits |= 1u << b;
-      for (uint32_t f = 0; f < F; ++f) grad[e * F + f] = t ? src[e * F + f] : 0.f;
-    }
-    bitmap[w] = bits;
+// gradient array <- canonical gradient and flags (debug / test entry point)
+__global__ void set_grad_kernel(float *__restrict__ grad, uint32_t F, uint64_t n_entries, const float *__restrict__ src,
+                                const uint8_t *__restrict__ touched) {
+  const uint64_t total = n_entries * F;
+  for (uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; i < total; i += (uint64_t)gridDim.x * blockDim.x) {
+    const uint64_t e = i / F;
+    const bool t = src && (!touched || touched[e]);
+    const float v = t ? src[i] : 0.f;
+    grad[i] = t ? (fabsf(v) < NSM_GRAD_MIN_ADDEND ? 0.0f : v) : __uint_as_float(NSM_GRAD_UNTOUCHED);
   }
 }
 
-__global__ void get_touched_kernel(const uint32_t *__restrict__ bitmap, uint64_t n_entries, uint8_t *__restrict__ dst) {
+__global__ void get_touched_kernel(const float *__restrict__ grad, uint32_t F, uint64_t n_entries, uint8_t *__restrict__ dst) {
   for (uint64_t e = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; e < n_entries; e += (uint64_t)gridDim.x * blockDim.x)
-    dst[e] = (bitmap[e >> 5] >> (e & 31)) & 1u;
+    dst[e] = __float_as_uint(grad[e * F]) != NSM_GRAD_UNTOUCHED;
 }
 
 __global__ void debug_slots_kernel(LevelTable lv, Workspace ws, const uint32_t *__restrict__ d_S,
@@ -286,24 +280,23 @@ int launch_encode(const LevelTable &lv, const float *theta, const Workspace &ws,
 }
 
 int launch_set_grad(const FieldParams &fp, const float *src, const uint8_t *touched, cudaStream_t st) {
-  set_grad_kernel<<<2048, 256, 0, st>>>(fp.grad, fp.touched, fp.F, fp.n_entries, src, touched);
+  set_grad_kernel<<<2048, 256, 0, st>>>(fp.grad, fp.F, fp.n_entries, src, touched);
   return 1;
 }
 
 int launch_get_touched(const FieldParams &fp, uint8_t *dst, cudaStream_t st) {
-  get_touched_kernel<<<2048, 256, 0, st>>>(fp.touched, fp.n_entries, dst);
+  get_touched_kernel<<<2048, 256, 0, st>>>(fp.grad, fp.F, fp.n_entries, dst);
   return 1;
 }
 
-int launch_scatter(const LevelTable &lv, float *grad, uint32_t *touched, const Workspace &ws,
-                   const uint32_t *d_S, int n_sms, cudaStream_t st) {
+int launch_scatter(const LevelTable &lv, float *grad, const Workspace &ws, const uint32_t *d_S, int n_sms, cudaStream_t st) {
   dim3 grid(n_sms * 8), block(256);
   const uint32_t l0 = 0, l1 = lv.n_levels;
   switch (lv.n_features) {
-    case 1: launch_pdl(scatter_backward_kernel<1>, grid, block, 0, st, lv, grad, touched, ws, d_S, l0, l1); break;
-    case 2: launch_pdl(scatter_backward_kernel<2>, grid, block, 0, st, lv, grad, touched, ws, d_S, l0, l1); break;
-    case 4: launch_pdl(scatter_backward_kernel<4>, grid, block, 0, st, lv, grad, touched, ws, d_S, l0, l1); break;
-    default: launch_pdl(scatter_backward_kernel<8>, grid, block, 0, st, lv, grad, touched, ws, d_S, l0, l1); break;
+    case 1: launch_pdl(scatter_backward_kernel<1>, grid, block, 0, st, lv, grad, ws, d_S, l0, l1); break;
+    case 2: launch_pdl(scatter_backward_kernel<2>, grid, block, 0, st, lv, grad, ws, d_S, l0, l1); break;
+    case 4: launch_pdl(scatter_backward_kernel<4>, grid, block, 0, st, lv, grad, ws, d_S, l0, l1); break;
+    default: launch_pdl(scatter_backward_kernel<8>, grid, block, 0, st, lv, grad, ws, d_S, l0, l1); break;
   }
   return 1;
 }

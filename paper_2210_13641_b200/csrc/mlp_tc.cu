@@ -234,6 +234,12 @@ __device__ __forceinline__ void emit16s(float *v, uint8_t *smem_tile, uint32_t l
 #pragma unroll
   for (int j = 0; j < 8; ++j) {
     hi[j] = pack2<T>(v[2 * j], v[2 * j + 1]);
+    if (RELU && Fmt<T>::id == 0) {
+      // fp16 flushes 0 < h < 2^-25 to zero; the backward pass reads its ReLU mask off this stored value (h > 0), so a
+      // positive activation is stored as at least the smallest subnormal: the mask is then exactly [pre-activation > 0]
+      if (v[2 * j] > 0.f && (hi[j] & 0xffffu) == 0u) hi[j] |= 1u;
+      if (v[2 * j + 1] > 0.f && (hi[j] >> 16) == 0u) hi[j] |= 0x10000u;
+    }
     const float2 h = unpack2<T>(hi[j]);
     lo[j] = pack2<T>(v[2 * j] - h.x, v[2 * j + 1] - h.y);
   }

@@ -366,7 +366,7 @@ nsm_status enqueue_backward(nsm_field *f, const nsm_ray_batch *b, float lambda_d
   }
   // train step: the scatter is issued by enqueue_adam, behind the MLP Adam's hand-off to the side stream
   f->scatter_pending = defer_scatter;
-  if (!defer_scatter) RUN(f, K_SCATTER, launch_scatter(f->lv, f->fp.grad, f->fp.touched, f->ws, d_S, f->n_sms, f->stream));
+  if (!defer_scatter) RUN(f, K_SCATTER, launch_scatter(f->lv, f->fp.grad, f->ws, d_S, f->n_sms, f->stream));
   f->grads_dirty = true;
   f->last_R = R;
   f->last_K = b->n_candidates;
@@ -399,7 +399,7 @@ nsm_status enqueue_adam(nsm_field *f) {
   // gradient array stays in L2 between its uses, was measured in round 1 -- profiles/r1j: every extra pair of launches
   // costs ~19 us of ramp and tail, more than the DRAM traffic it saves.)
   if (f->scatter_pending)
-    RUN(f, K_SCATTER, launch_scatter(f->lv, f->fp.grad, f->fp.touched, f->ws, f->ws.offsets + f->last_R, f->n_sms, f->stream));
+    RUN(f, K_SCATTER, launch_scatter(f->lv, f->fp.grad, f->ws, f->ws.offsets + f->last_R, f->n_sms, f->stream));
   f->scatter_pending = false;
   if (use_side) {   // the scatter is in: the side stream (next step's marcher) may overwrite the samples
     CUDA_TRY(cudaEventRecord(f->ev_main, f->stream));
@@ -533,7 +533,7 @@ nsm_status nsm_create_field(const nsm_field_config *cfg, void *cuda_stream, nsm_
   auto A = [&](cudaError_t r) { if (e == cudaSuccess) e = r; };
   A(f->alloc(&fp.theta, fp.n_table)); A(f->alloc(&fp.mv, 2 * fp.n_table));
   A(f->alloc(&fp.mlp_theta, fp.n_mlp)); A(f->alloc(&fp.mlp_m, fp.n_mlp)); A(f->alloc(&fp.mlp_v, fp.n_mlp)); A(f->alloc(&fp.mlp_grad, fp.n_mlp));
-  A(f->alloc(&fp.grad, fp.n_table)); A(f->alloc(&fp.touched, (fp.n_entries + 31) / 32 + 1)); A(f->alloc(&fp.occ_bits, (G3 + 7) / 8 + 4));
+  A(f->alloc(&fp.grad, fp.n_table, false)); A(f->alloc(&fp.occ_bits, (G3 + 7) / 8 + 4));
   A(f->alloc(&fp.occ_grid, G3));
   A(f->alloc(&ws.counts, R)); A(f->alloc(&ws.offsets, R + 1)); A(f->alloc(&ws.scan_state, march_scan_state_entries(R) + 1)); A(f->alloc(&ws.scan_ctr, 2));
   A(f->alloc(&ws.C, 3 * (size_t)R)); A(f->alloc(&ws.D_hat, R)); A(f->alloc(&ws.O, R));
@@ -574,7 +574,8 @@ nsm_status nsm_create_field(const nsm_field_config *cfg, void *cuda_stream, nsm_
     cudaGetLastError();
     return fail(e == cudaErrorMemoryAllocation ? NSM_ERR_OOM : NSM_ERR_CUDA, "allocation failed: %s", cudaGetErrorString(e));
   }
-  repack_weights(f);   // gradient array and touched bitmap start zeroed (alloc)
+  RUN(f, K_DEBUG, launch_set_grad(f->fp, nullptr, nullptr, f->stream));   // every gradient word = "untouched"
+  repack_weights(f);
   *out = f;
   return NSM_OK;
 }
@@ -1077,6 +1078,9 @@ nsm_status nsm_debug_last_step(nsm_field *f, int item, void *d_out, uint64_t cap
     case NSM_DBG_E: bytes = 4ull * S * f->ms.LF; break;
     case NSM_DBG_SLOTS: bytes = 4ull * S * L * 8; break;
     case NSM_DBG_W: bytes = 4ull * S * L * 3; break;
+    case NSM_DBG_HIDDEN_DENSITY: bytes = 4ull * S * f->ms.Hd; break;
+    case NSM_DBG_HIDDEN_COLOR1: bytes = 4ull * S * f->ms.Hc; break;
+    case NSM_DBG_HIDDEN_COLOR2: bytes = f->ms.n_color_layers == 2 ? 4ull * S * f->ms.Hc : 0; break;
     default: return fail(NSM_ERR_INVALID_ARG, "unknown debug item %d", item);
   }
   if (n_bytes_out) *n_bytes_out = bytes;
@@ -1099,6 +1103,15 @@ nsm_status nsm_debug_last_step(nsm_field *f, int item, void *d_out, uint64_t cap
       RUN(f, K_DEBUG, launch_blob_to_rows(f->cfg.mlp_precision == NSM_MLP_BF16, ws.blob_e, f->ms.LF, 1, d_S, (float *)d_out, f->stream));
     else
       RUN(f, K_DEBUG, launch_planes_to_rows(ws.e, ws.cap, f->ms.LF, d_S, (float *)d_out, f->stream));
+  } else if (item == NSM_DBG_HIDDEN_DENSITY || item == NSM_DBG_HIDDEN_COLOR1 || item == NSM_DBG_HIDDEN_COLOR2) {
+    const uint32_t n_cols = item == NSM_DBG_HIDDEN_DENSITY ? f->ms.Hd : f->ms.Hc;
+    if (f->use_tc) {
+      const uint8_t *blob = item == NSM_DBG_HIDDEN_DENSITY ? ws.blob_hd : (item == NSM_DBG_HIDDEN_COLOR1 ? ws.blob_h1 : ws.blob_h2);
+      RUN(f, K_DEBUG, launch_blob_to_rows(f->cfg.mlp_precision == NSM_MLP_BF16, blob, n_cols, 0, d_S, (float *)d_out, f->stream));
+    } else {
+      const float *planes = item == NSM_DBG_HIDDEN_DENSITY ? ws.hd : (item == NSM_DBG_HIDDEN_COLOR1 ? ws.h1 : ws.h2);
+      RUN(f, K_DEBUG, launch_planes_to_rows(planes, ws.cap, n_cols, d_S, (float *)d_out, f->stream));
+    }
   } else if (item == NSM_DBG_SLOTS) {
     RUN(f, K_DEBUG, launch_debug_slots(f->lv, ws, d_S, (uint32_t *)d_out, nullptr, f->stream));
   } else {

@@ -126,19 +126,26 @@ __device__ __forceinline__ void tl_mark(unsigned long long *tl, int id, int end)
 //   mv[e*2F + 0..F) = m,    Adam moments, one 4F-byte record per entry (16 B for F = 2): only the table Adam touches
 //   mv[e*2F + F..2F) = v    them, for the random ~25 % of entries a step references;
 //   grad[e*F + f]           the gradient, compact like theta (L2-sized): the scatter's vector reductions land in a
-//                           table that fits the cache; Adam reads (and zeroes) the touched entries only.
+//                           table that fits the cache, and Adam reads it as a dense coalesced stream.
 // (Measured on B200, profiles/r1h: with theta inside 32-byte per-entry records the encoder moved 120 MB of DRAM
 // for 12 MB of useful theta and ran at 81 % of the HBM peak; DRAM fetches are 64 bytes.)
 //
-// Touched set (S12's structural U): one bit per entry in `touched`, set by the scatter (test, then atomicOr), walked
-// and cleared by the table Adam, which also zeroes the gradients it consumes: between steps the gradient array is all
-// zeros and the bitmap all clear.
+// Touched set without flags: between steps every gradient word holds -0.0f (bits 0x80000000).
+// The scatter never adds -0.0 or a magnitude below 2^-96 (those addends become +0.0), and under
+// round-to-nearest a sum of such addends is +0.0, or a multiple of 2^-119 >= FLT_MIN in magnitude;
+// it is never -0.0 (x + (-x) = +0.0) and never a subnormal that the reduction unit could flush to
+// -0.0.  Hence "entry e was referenced this step"  <=>  bits(grad[e*F]) != 0x80000000, whatever the
+// gradient's value (the touched set is structural, S12); Adam writes -0.0f back.
+// (Round 2 measured the alternative -- a one-bit-per-entry touched bitmap set by atomicOr in the scatter or in the
+// training forward's encoder, walked by Adam instead of the dense gradient scan: the marking costs as much as the scan
+// saves, profiles/r2a_touched_bitmap.md.)
 // The canonical flat layout of include/nsm.h exists only at the boundary (pack/unpack kernels).
+#define NSM_GRAD_UNTOUCHED 0x80000000u
+#define NSM_GRAD_MIN_ADDEND 1.262177448e-29f   /* 2^-96 */
 struct FieldParams {
   float *theta;                                     // [n_entries][F]
   float *mv;                                        // [n_entries][2F]
   float *grad;                                      // [n_entries][F]
-  uint32_t *touched;                                // [ceil(n_entries / 32)] bit (e & 31) of word (e >> 5)
   float *mlp_theta, *mlp_m, *mlp_v, *mlp_grad;      // [n_mlp] each, canonical order
   uint8_t *occ_bits;                                // [G^3/8]
   float *occ_grid;                                  // [G^3] running density of the decayed refresh (F4); seeded by FROM_FIELD
@@ -254,10 +261,9 @@ uint32_t march_scan_state_entries(uint32_t max_rays);
 // out_mode: 0 = fp32 planes ws.e, 1 = fp16 blob ws.blob_e, 2 = bf16 blob ws.blob_e
 int launch_encode(const LevelTable &lv, const float *theta, const Workspace &ws,
                   const uint32_t *d_S, int out_mode, int n_sms, cudaStream_t st);
-// S12 over all levels: vector reductions into grad, touched bits into the bitmap
-int launch_scatter(const LevelTable &lv, float *grad, uint32_t *touched, const Workspace &ws,
-                   const uint32_t *d_S, int n_sms, cudaStream_t st);
-// gradient array + touched bitmap <- canonical gradient + flags (NULL: every entry touched); src == nullptr: zero, none touched
+// S12 over all levels: vector reductions into grad
+int launch_scatter(const LevelTable &lv, float *grad, const Workspace &ws, const uint32_t *d_S, int n_sms, cudaStream_t st);
+// gradient array <- canonical gradient + touched flags (NULL: every entry touched); src == nullptr: all untouched
 int launch_set_grad(const FieldParams &fp, const float *src, const uint8_t *touched, cudaStream_t st);
 int launch_get_touched(const FieldParams &fp, uint8_t *dst, cudaStream_t st);
 // canonical [n_entries][F] <-> `which` (0 theta, 2 m, 3 v) of the internal arrays; src == nullptr packs zeros
@@ -290,7 +296,7 @@ int launch_composite_train(const Workspace &ws, uint32_t R, const float *rgb, co
                            cudaStream_t st);
 int launch_composite_render(const Workspace &ws, uint32_t R, float cut, const float bg[3],
                             float *out_rgb, float *out_depth, float *out_opacity, cudaStream_t st);
-// S13 on the touched table entries (sparse) or on all of them; consumes the gradients and the touched bits
+// S13 on the touched table entries (sparse) or on all of them; consumes the gradients (every word back to "untouched")
 int launch_adam_table(const FieldParams &fp, uint32_t F, int sparse, float lr, float beta1, float beta2,
                       float eps, float inv_bc1, float inv_bc2, cudaStream_t st, unsigned long long *tl = nullptr);
 int launch_adam_mlp(const FieldParams &fp, float lr, float beta1, float beta2, float eps, float inv_bc1,

@@ -103,46 +103,38 @@ __device__ __forceinline__ void red_add_entry(float *p, const float g[F], uint64
   }
 }
 
-// The touched set U (S12: every entry referenced this step, whatever its gradient's value) is one bit per table entry,
-// bit (e & 31) of word (e >> 5), e = offset_l + slot.  Test first, set only if clear: the test is an ordinary load that
-// may be served by a stale L1 line (then the atomic is merely redundant -- bits are only ever SET while the scatter
-// runs), so an entry costs one L2 atomic per step instead of one per reference.  The 0.76 MB (config 2) / 5.6 MB
-// (config 4) bitmap stays cache-resident; the table Adam walks it instead of the gradient array.
-__device__ __forceinline__ void mark_touched(uint32_t *__restrict__ touched, uint64_t e, uint32_t bits) {
-  uint32_t *w = touched + (e >> 5);
-  bits <<= (uint32_t)(e & 31u);
-  if ((*w & bits) != bits) atomicOr(w, bits);
-}
-
-// S12 for one cell of one level: the eight corner reductions d theta[(offset_l + slot) F + f] += val[corner][f], and the
-// eight touched bits.
+// S12 for one cell of one level: the eight corner reductions d theta[(offset_l + slot) F + f] += val[corner][f].
+// Addends are canonicalised here (never -0.0, never near-subnormal; NaN stays NaN): the touched set U is structural
+// (every referenced entry, independent of the gradient's value) and is carried by the gradient words themselves, see
+// FieldParams in nsm_internal.cuh.
 template <int F>
-__device__ __forceinline__ void issue_corner_reds(const LevelTable &lv, float *__restrict__ grad, uint32_t *__restrict__ touched,
-                                                  uint32_t l, const uint32_t slot[8], float val[8][F], uint64_t pol_last) {
-  const uint64_t e_l = lv.offset[l];
-  float *tab = grad + e_l * F;
+__device__ __forceinline__ void issue_corner_reds(const LevelTable &lv, float *__restrict__ grad, uint32_t l, const uint32_t slot[8],
+                                                  float val[8][F], uint64_t pol_last) {
 #pragma unroll
-  for (int k = 0; k < 8; k += 2) {
+  for (int k = 0; k < 8; ++k)
+#pragma unroll
+    for (int f = 0; f < F; ++f) val[k][f] = fabsf(val[k][f]) < NSM_GRAD_MIN_ADDEND ? 0.0f : val[k][f];
+  float *tab = grad + lv.offset[l] * F;
+  if constexpr (F == 2) {
     // The two x-neighbour corners (k, k+1) are adjacent entries whenever their slots differ in bit 0 only (always on
-    // a dense level, for even cell x on a hashed one: the hash XORs x in unmultiplied): one bitmap word, and for
-    // F = 2, if the pair is also 16-byte aligned in the array, one red.v4 covers both entries (~25 % fewer
-    // reductions at the L2).
-    const uint64_t a0 = e_l + slot[k], a1 = e_l + slot[k + 1];
-    const bool pair = (a0 ^ a1) == 1ull;
-    if (pair) {
-      mark_touched(touched, a0 & ~1ull, 3u);
-    } else {
-      mark_touched(touched, a0, 1u);
-      mark_touched(touched, a1, 1u);
+    // a dense level, for even cell x on a hashed one: the hash XORs x in unmultiplied).  If the pair is also
+    // 16-byte aligned in the array, one red.v4 covers both entries: ~25 % fewer reductions at the L2.
+    const uint64_t e_l = lv.offset[l];
+#pragma unroll
+    for (int k = 0; k < 8; k += 2) {
+      const uint64_t a0 = e_l + slot[k], a1 = e_l + slot[k + 1];
+      if ((a0 ^ a1) == 1ull) {
+        float *p = grad + (a0 & ~1ull) * 2;
+        if (a0 & 1ull) red_hint_f4(p, make_float4(val[k + 1][0], val[k + 1][1], val[k][0], val[k][1]), pol_last);
+        else red_hint_f4(p, make_float4(val[k][0], val[k][1], val[k + 1][0], val[k + 1][1]), pol_last);
+      } else {
+        red_add_entry<2>(tab + (size_t)slot[k] * 2, val[k], pol_last);
+        red_add_entry<2>(tab + (size_t)slot[k + 1] * 2, val[k + 1], pol_last);
+      }
     }
-    if (F == 2 && pair) {
-      float *p = grad + (a0 & ~1ull) * 2;
-      if (a0 & 1ull) red_hint_f4(p, make_float4(val[k + 1][0], val[k + 1][1], val[k][0], val[k][1]), pol_last);
-      else red_hint_f4(p, make_float4(val[k][0], val[k][1], val[k + 1][0], val[k + 1][1]), pol_last);
-    } else {
-      red_add_entry<F>(tab + (size_t)slot[k] * F, val[k], pol_last);
-      red_add_entry<F>(tab + (size_t)slot[k + 1] * F, val[k + 1], pol_last);
-    }
+  } else {
+#pragma unroll
+    for (int k = 0; k < 8; ++k) red_add_entry<F>(tab + (size_t)slot[k] * F, val[k], pol_last);
   }
 }
 
@@ -164,137 +156,142 @@ __device__ __forceinline__ void corner_contributions(const LevelTable &lv, const
 }
 
 template <int F>
-__device__ __forceinline__ void scatter_sample_level(const LevelTable &lv, float *__restrict__ grad, uint32_t *__restrict__ touched,
-                                                     const Workspace &ws, uint32_t l, uint64_t s, uint64_t pol_last) {
+__device__ __forceinline__ void scatter_sample_level(const LevelTable &lv, float *__restrict__ grad, const Workspace &ws,
+                                                     uint32_t l, uint64_t s, uint64_t pol_last) {
   uint32_t slot[8];
   float val[8][F];
   corner_contributions<F>(lv, ws, l, s, slot, val);
-  issue_corner_reds<F>(lv, grad, touched, l, slot, val, pol_last);
+  issue_corner_reds<F>(lv, grad, l, slot, val, pol_last);
 }
 
-constexpr int ADAM_WORDS = 128;                    // bitmap words per block
-constexpr int ADAM_ENTRIES = ADAM_WORDS * 32;      // = 4096 table entries per block
+constexpr int ADAM_CHUNK_FLOATS = 4096;
 constexpr int ADAM_THREADS = 256;
 
+// one touched entry: theta (F floats of the compact array) and its moment record (m | v, 2F floats)
 template <int F>
-__device__ __forceinline__ void store_entry_hint(float *p, const float v[F], uint64_t pol) {
-  if constexpr (F == 8) {
-    st_hint_f4(p, make_float4(v[0], v[1], v[2], v[3]), pol);
-    st_hint_f4(p + 4, make_float4(v[4], v[5], v[6], v[7]), pol);
-  } else if constexpr (F == 4) {
-    st_hint_f4(p, make_float4(v[0], v[1], v[2], v[3]), pol);
+__device__ __forceinline__ void adam_entry(float *__restrict__ th_p, float *__restrict__ mv_p, const float *g, const AdamConst &c,
+                                           uint64_t pol_ld, uint64_t pol_st) {
+  float th[F], m[F], v[F];
+  if constexpr (F == 1) {
+    th[0] = ld_hint_f1(th_p, pol_ld);
+    const float2 t = ld_hint_f2(mv_p, pol_ld);
+    m[0] = t.x; v[0] = t.y;
   } else if constexpr (F == 2) {
-    st_hint_f2(p, make_float2(v[0], v[1]), pol);
+    const float2 a = ld_hint_f2(th_p, pol_ld);
+    const float4 b = ld_hint_f4(mv_p, pol_ld);
+    th[0] = a.x; th[1] = a.y; m[0] = b.x; m[1] = b.y; v[0] = b.z; v[1] = b.w;
   } else {
-    st_hint_f1(p, v[0], pol);
+#pragma unroll
+    for (int i = 0; i < F / 4; ++i) {
+      const float4 a = ld_hint_f4(th_p + 4 * i, pol_ld), b = ld_hint_f4(mv_p + 4 * i, pol_ld), d = ld_hint_f4(mv_p + F + 4 * i, pol_ld);
+      th[4 * i] = a.x; th[4 * i + 1] = a.y; th[4 * i + 2] = a.z; th[4 * i + 3] = a.w;
+      m[4 * i] = b.x; m[4 * i + 1] = b.y; m[4 * i + 2] = b.z; m[4 * i + 3] = b.w;
+      v[4 * i] = d.x; v[4 * i + 1] = d.y; v[4 * i + 2] = d.z; v[4 * i + 3] = d.w;
+    }
+  }
+#pragma unroll
+  for (int f = 0; f < F; ++f) adam_one(th[f], m[f], v[f], g[f], c);
+  if constexpr (F == 1) {
+    st_hint_f1(th_p, th[0], pol_st);
+    st_hint_f2(mv_p, make_float2(m[0], v[0]), pol_st);
+  } else if constexpr (F == 2) {
+    st_hint_f2(th_p, make_float2(th[0], th[1]), pol_st);
+    st_hint_f4(mv_p, make_float4(m[0], m[1], v[0], v[1]), pol_st);
+  } else {
+#pragma unroll
+    for (int i = 0; i < F / 4; ++i) {
+      st_hint_f4(th_p + 4 * i, make_float4(th[4 * i], th[4 * i + 1], th[4 * i + 2], th[4 * i + 3]), pol_st);
+      st_hint_f4(mv_p + 4 * i, make_float4(m[4 * i], m[4 * i + 1], m[4 * i + 2], m[4 * i + 3]), pol_st);
+      st_hint_f4(mv_p + F + 4 * i, make_float4(v[4 * i], v[4 * i + 1], v[4 * i + 2], v[4 * i + 3]), pol_st);
+    }
   }
 }
 
-// One touched entry in flight: its gradient and theta (F floats of the compact arrays each) and its moment record
-// (m | v, 2F floats).  load() issues the four accesses, step() updates and stores and zeroes the gradient.
+// S13 for one chunk of ADAM_CHUNK_FLOATS / F consecutive entries starting at e_base (e_base * F a multiple of 4),
+// by a whole block of ADAM_THREADS threads.  Shared memory: list_g [ADAM_CHUNK_FLOATS], list_e [CH], cnt_p.  The caller
+// must __syncthreads() before reusing the shared arrays.
 template <int F>
-struct AdamRec {
-  float g[F], th[F], m[F], v[F];
-  __device__ __forceinline__ void load(const float *g_p, const float *th_p, const float *mv_p, uint64_t pol_g, uint64_t pol_th,
-                                       uint64_t pol_mv) {
-    load_entry_hint<F>(g_p, g, pol_g);
-    load_entry_hint<F>(th_p, th, pol_th);
-    if constexpr (F == 1) {
-      const float2 t = ld_hint_f2(mv_p, pol_mv);
-      m[0] = t.x; v[0] = t.y;
-    } else if constexpr (F == 2) {
-      const float4 t = ld_hint_f4(mv_p, pol_mv);
-      m[0] = t.x; m[1] = t.y; v[0] = t.z; v[1] = t.w;
-    } else {
-      load_entry_hint<F>(mv_p, m, pol_mv);
-      load_entry_hint<F>(mv_p + F, v, pol_mv);
-    }
-  }
-  __device__ __forceinline__ void step(float *g_p, float *th_p, float *mv_p, const AdamConst &c, uint64_t pol_g, uint64_t pol_th,
-                                       uint64_t pol_mv) {
+__device__ __forceinline__ void adam_chunk(float *__restrict__ theta, float *__restrict__ mv, float *__restrict__ grad,
+                                           uint64_t e_base, uint64_t n_entries, int sparse, const AdamConst &c, float *list_g,
+                                           uint16_t *list_e, uint32_t *cnt_p) {
+  constexpr int CH = ADAM_CHUNK_FLOATS / F;            // entries per chunk
+  constexpr int NV = ADAM_CHUNK_FLOATS / 4 / ADAM_THREADS;   // float4 loads per thread
+  const uint32_t tid = threadIdx.x, lane = tid & 31;
+  const uint64_t n_float = n_entries * F;
+  const float *g4 = grad + e_base * F;
+  // L2 policies, swept on B200 (profiles/r1k): theta / moment stores evict_first, everything else default.  Marking
+  // Adam's own gradient reads and resets evict_last (as the scatter's reductions are) costs 4 us per step.
+  const uint64_t pol_ld = l2_evict_normal(), pol_first = l2_evict_first(), pol_last = pol_ld;
+  if (tid == 0) *cnt_p = 0;
+  float4 gv[NV];
+  uint32_t dirty = 0;                                  // bit j: the thread's j-th 16-byte word holds a touched entry
 #pragma unroll
-    for (int f = 0; f < F; ++f) adam_one(th[f], m[f], v[f], g[f], c);
-    store_entry_hint<F>(th_p, th, pol_th);
-    if constexpr (F == 1) {
-      st_hint_f2(mv_p, make_float2(m[0], v[0]), pol_mv);
-    } else if constexpr (F == 2) {
-      st_hint_f4(mv_p, make_float4(m[0], m[1], v[0], v[1]), pol_mv);
-    } else {
-      store_entry_hint<F>(mv_p, m, pol_mv);
-      store_entry_hint<F>(mv_p + F, v, pol_mv);
-    }
-#pragma unroll
-    for (int f = 0; f < F; ++f) g[f] = 0.f;
-    store_entry_hint<F>(g_p, g, pol_g);
+  for (int j = 0; j < NV; ++j) {
+    const uint32_t q = j * ADAM_THREADS + tid;         // float4 index inside the chunk
+    gv[j] = (e_base * F + 4ull * q < n_float) ? ld_hint_f4(g4 + 4 * q, pol_last) : make_float4(0.f, 0.f, 0.f, 0.f);   // the array is padded to 256 B
   }
-};
-
-// S13 for the ADAM_ENTRIES consecutive entries starting at e_base (a multiple of 32), by a block of ADAM_THREADS threads.
-// The block reads its ADAM_WORDS words of the touched bitmap (512 contiguous bytes; the scatter set the bits), clears
-// them, and expands the set bits into a list of local entry indices in shared memory -- ascending, so the threads of a
-// warp update neighbouring touched entries and share sectors.  Every thread then takes UNROLL list entries at a time:
-// all their loads (gradient, theta, moment record) are issued before the first update, so a thread keeps 3 x UNROLL
-// independent DRAM / L2 accesses in flight.  Neither the gradient array nor theta / m|v of untouched entries is read:
-// the traffic is what the touched set needs and nothing else.  sparse = 0 (dense Adam, textbook): every entry.
-template <int F>
-__device__ __forceinline__ void adam_block(float *__restrict__ theta, float *__restrict__ mv, float *__restrict__ grad,
-                                           uint32_t *__restrict__ touched, uint64_t e_base, uint64_t n_entries, int sparse,
-                                           const AdamConst &c, uint16_t *list_e, uint32_t *warp_tot) {
-  constexpr int UNROLL = F <= 2 ? 4 : (F == 4 ? 2 : 1);
-  const uint32_t tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-  uint32_t wv = 0;
-  if (tid < ADAM_WORDS) {
-    const uint64_t e0 = e_base + 32ull * tid;
-    if (e0 < n_entries) {
-      uint32_t *wp = touched + (e0 >> 5);
-      const uint32_t t = *wp;
-      if (t) *wp = 0u;
-      wv = sparse ? t : 0xffffffffu;
-      const uint64_t rem = n_entries - e0;
-      if (rem < 32) wv &= (1u << (uint32_t)rem) - 1u;
-    }
-  }
-  // exclusive scan of the per-word counts over the ADAM_WORDS / 32 loading warps
-  const uint32_t cnt = __popc(wv);
-  uint32_t incl = cnt;
-#pragma unroll
-  for (int d = 1; d < 32; d <<= 1) {
-    const uint32_t y = __shfl_up_sync(0xffffffffu, incl, d);
-    if (lane >= (uint32_t)d) incl += y;
-  }
-  if (lane == 31 && warp < ADAM_WORDS / 32) warp_tot[warp] = incl;
   __syncthreads();
-  uint32_t n = 0, pos = incl - cnt;
 #pragma unroll
-  for (uint32_t w = 0; w < ADAM_WORDS / 32; ++w) {
-    const uint32_t t = warp_tot[w];
-    if (w < warp) pos += t;
-    n += t;
+  for (int j = 0; j < NV; ++j) {
+    const uint32_t q = j * ADAM_THREADS + tid;
+    const float w[4] = {gv[j].x, gv[j].y, gv[j].z, gv[j].w};
+    if constexpr (F <= 4) {
+      constexpr int EPV = 4 / F;                       // entries per float4
+#pragma unroll
+      for (int i = 0; i < EPV; ++i) {
+        const uint32_t le = q * EPV + i;               // local entry index
+        const bool t = (e_base + le < n_entries) && (!sparse || __float_as_uint(w[i * F]) != NSM_GRAD_UNTOUCHED);
+        if (t) dirty |= 1u << j;
+        const uint32_t mk = __ballot_sync(0xffffffffu, t);
+        uint32_t base = 0;
+        if (lane == 0 && mk) base = atomicAdd(cnt_p, (uint32_t)__popc(mk));
+        base = __shfl_sync(0xffffffffu, base, 0);
+        if (t) {
+          const uint32_t pos = base + __popc(mk & ((1u << lane) - 1u));
+          list_e[pos] = (uint16_t)le;
+#pragma unroll
+          for (int f = 0; f < F; ++f) list_g[pos * F + f] = w[i * F + f];
+        }
+      }
+    } else {                                           // F = 8: an entry spans two float4 (q even: first half)
+      const uint32_t le = q >> 1;
+      const uint32_t first_word = __float_as_uint(__shfl_sync(0xffffffffu, w[0], lane & ~1u));
+      const bool t = (e_base + le < n_entries) && (!sparse || first_word != NSM_GRAD_UNTOUCHED);
+      if (t) dirty |= 1u << j;
+      const uint32_t mk = __ballot_sync(0xffffffffu, t && !(lane & 1u));
+      uint32_t base = 0;
+      if (lane == 0 && mk) base = atomicAdd(cnt_p, (uint32_t)__popc(mk));
+      base = __shfl_sync(0xffffffffu, base, 0);
+      if (t) {
+        const uint32_t pos = base + __popc(mk & ((1u << (lane & ~1u)) - 1u));
+        if (!(lane & 1u)) list_e[pos] = (uint16_t)le;
+#pragma unroll
+        for (int f = 0; f < 4; ++f) list_g[pos * F + (lane & 1u) * 4 + f] = w[f];
+      }
+    }
   }
+  __syncthreads();
+  const uint32_t n = *cnt_p;
   if (n == 0) return;
-  while (wv) {
-    const uint32_t b = (uint32_t)__ffs(wv) - 1u;
-    wv &= wv - 1u;
-    list_e[pos++] = (uint16_t)(tid * 32u + b);
+  // phase 2: two records in flight per thread
+  for (uint32_t i0 = tid; i0 < n; i0 += 2 * ADAM_THREADS) {
+    const uint32_t i1 = i0 + ADAM_THREADS;
+    const uint64_t e0 = e_base + list_e[i0], e1 = e_base + list_e[i1 < n ? i1 : i0];
+    if constexpr (F == 2) {   // touch the second entry's moment record early
+      asm volatile("prefetch.global.L2 [%0];" ::"l"(mv + e1 * 2 * F));
+    }
+    adam_entry<F>(theta + e0 * F, mv + e0 * 2 * F, list_g + i0 * F, c, pol_ld, pol_first);
+    if (i1 < n) adam_entry<F>(theta + e1 * F, mv + e1 * 2 * F, list_g + i1 * F, c, pol_ld, pol_first);
   }
-  __syncthreads();
-  // L2 policies: the moment records are a pure stream (read once, written once per step): evict_first both ways.  The
-  // gradient words were just written by the scatter (evict_last there) and theta is re-read by the next step's encoder.
-  const uint64_t pol_n = l2_evict_normal(), pol_first = l2_evict_first();
-  for (uint32_t i0 = tid; i0 < n; i0 += UNROLL * ADAM_THREADS) {
-    AdamRec<F> r[UNROLL];
-    uint64_t e[UNROLL];
+  // reset the chunk's gradient words
+  float *o4 = grad + e_base * F;
+  const float nz = __uint_as_float(NSM_GRAD_UNTOUCHED);
 #pragma unroll
-    for (int u = 0; u < UNROLL; ++u) {
-      const uint32_t i = i0 + u * ADAM_THREADS;
-      e[u] = e_base + list_e[i < n ? i : i0];
-      if (i < n) r[u].load(grad + e[u] * F, theta + e[u] * F, mv + e[u] * 2 * F, pol_n, pol_n, pol_first);
-    }
-#pragma unroll
-    for (int u = 0; u < UNROLL; ++u) {
-      const uint32_t i = i0 + u * ADAM_THREADS;
-      if (i < n) r[u].step(grad + e[u] * F, theta + e[u] * F, mv + e[u] * 2 * F, c, pol_n, pol_first, pol_first);
-    }
+  for (int j = 0; j < NV; ++j) {
+    const uint32_t q = j * ADAM_THREADS + tid;
+    // only the words that held a touched entry: the others are -0.0 already (with tables far larger than the L2 the
+    // dense rewrite was half of this kernel's DRAM traffic)
+    if (((dirty >> j) & 1u) && e_base * F + 4ull * q < n_float) st_hint_f4(o4 + 4 * q, make_float4(nz, nz, nz, nz), pol_last);
   }
 }
 

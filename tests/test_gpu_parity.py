@@ -471,15 +471,53 @@ def test_config5_full_frame_render_on_sampled_rays(nsm):
 
 # ---------------------------------------------------------------------------- row f2: pose gradients
 
+def _relu_mask_disagreements(f, O, b, tr):
+    """Samples at which the hidden-layer ReLU masks the GPU's backward pass used (activation > 0, from the saved
+    activations) differ from the float64 oracle's (pre-activation > 0).  The oracle's pre-activations are rebuilt here
+    from its traced encoder output, its weights and orc.sh; a disagreement needs a pre-activation within the forward
+    pass's rounding of zero (two-term 16-bit operands: ~1e-5; fp16 storage of the activation flushes h < 3e-8)."""
+    fc = f.fc
+    W = {}
+    o = O.n_table
+    for name, n_out, n_in in f.mlp_shapes():
+        W[name] = O.theta[o:o + n_out * n_in].reshape(n_out, n_in)
+        o += n_out * n_in
+    e = tr["e"]
+    z_d = e @ W["W_d1"].T
+    g = np.maximum(z_d, 0.0) @ W["W_d2"].T
+    Y = orc.sh(fc.sh_degree, b.dirs.astype(np.float64))[tr["s_ray"]]
+    ci = np.concatenate([g[:, fc.geo_offset:fc.geo_offset + fc.geo_count], Y], axis=1)
+    z_1 = ci @ W["W_c1"].T
+    bad = ((z_d > 0) != (f.nsm_debug_last_step("hidden_density") > 0)).any(axis=1)
+    bad |= ((z_1 > 0) != (f.nsm_debug_last_step("hidden_color1") > 0)).any(axis=1)
+    zmin = np.minimum(np.abs(z_d).min(axis=1), np.abs(z_1).min(axis=1))
+    if fc.color_hidden_layers == 2:
+        z_2 = np.maximum(z_1, 0.0) @ W["W_c2"].T
+        bad |= ((z_2 > 0) != (f.nsm_debug_last_step("hidden_color2") > 0)).any(axis=1)
+        zmin = np.minimum(zmin, np.abs(z_2).min(axis=1))
+    return bad, zmin
+
+
 def _check_pose(nsm, f, O, b, lam, tol):
+    """Per-ray dL/do and rotation gradient against the oracle: relative L2 over the batch, and element-wise P4 on every ray.
+    A ray's gradient is a sum over a few dozen samples and is DISCONTINUOUS where a hidden pre-activation crosses zero, so
+    on the 16-bit paths the rays that contain a sample whose ReLU mask the GPU took differently from the oracle are set
+    apart -- identified exactly, from the saved activations -- counted, and held to their number, not to the tolerance."""
     f.nsm_backward(nsm.DeviceBatch(b), lam)
     go, tau = (t.cpu().numpy().astype(np.float64) for t in f.nsm_pose_gradients(b.n_rays))
-    _, tr = O.train_step(b, lam, apply_adam=False, trace=("g_o", "tau"))
+    _, tr = O.train_step(b, lam, apply_adam=False, trace=("g_o", "tau", "e", "s_ray"))
+    flip_rays = np.zeros(b.n_rays, bool)
+    if f.nsm_mlp_path() != "simt_fp32":
+        bad, zmin = _relu_mask_disagreements(f, O, b, tr)
+        flip_rays[np.unique(tr["s_ray"][bad])] = True
+        print(f"pose parity: {bad.sum()} of {bad.size} samples ({flip_rays.sum()} of {b.n_rays} rays) with a ReLU mask taken differently "
+              f"from the oracle; their smallest |pre-activation| <= {zmin[bad].max() if bad.any() else 0.0:.1e}")
+        assert bad.sum() <= 2e-4 * bad.size and (not bad.any() or zmin[bad].max() <= 1e-4)
     for name, got, ref in (("g_o", go, tr["g_o"]), ("tau", tau, tr["tau"])):
         assert np.abs(ref).max() > 0, name
         assert np.linalg.norm(got - ref) <= tol * np.linalg.norm(ref), (name, np.linalg.norm(got - ref) / np.linalg.norm(ref))
-        err = np.abs(got - ref) / np.abs(ref).max()
-        assert err.max() <= tol, (name, err.max())                  # P4, element-wise, every path
+        err = np.abs(got - ref).max(axis=1) / np.abs(ref).max()
+        assert err[~flip_rays].max() <= tol, (name, err[~flip_rays].max(), int(np.argmax(np.where(flip_rays, 0, err))))
     return go, tau, tr
 
 

@@ -50,14 +50,24 @@ def check_step_parameters(f, O, before, gref, touched_ref, tol, tag):
             s = np.abs(ref[a:b]).max()
             assert np.abs(got[a:b] - ref[a:b]).max() <= tol * s + 1e-30, (tag, name, a, np.abs(got[a:b] - ref[a:b]).max() / s)
         bound[a:b] = np.abs(g_gpu[a:b] - gref[a:b])[touched[a:b]].max() if touched[a:b].any() else 0.0
+    # With 16-bit MLP operands a tensor's worst gradient error is ~1e-3 of its largest entry, so "10^3 x the error" leaves
+    # only the few largest entries of each tensor in the strong class (fp32, config 1: > 25 % of the touched set).
     strong = touched & (np.abs(gref) >= 1e3 * bound) & (np.abs(gref) >= 1e-15)
-    assert strong.sum() > 0.2 * touched.sum(), (tag, strong.sum(), touched.sum())
     d = np.abs(th.astype(np.float64) - O.theta)
-    assert d[strong].max() <= 5e-3 * LR + 1e-7, (tag, d[strong].max())
+    if strong.any():
+        assert d[strong].max() <= 5e-3 * LR + 1e-7, (tag, d[strong].max())
+    # the graded version of the same statement over ALL touched parameters: an update differs from the oracle's by at
+    # most lr x (the parameter's own relative gradient error, through m-hat and sqrt(v-hat)) -- checked in three classes
+    rel = np.abs(g_gpu - gref) / np.maximum(np.abs(gref), 1e-300)
+    for lo, hi, allow in ((0.0, 1e-3, 5e-3), (1e-3, 1e-2, 5e-2), (1e-2, 1e-1, 5e-1)):
+        cls = touched & (rel >= lo) & (rel < hi) & (np.abs(gref) >= 1e-15)
+        if cls.any():
+            assert d[cls].max() <= allow * LR + 1e-7, (tag, lo, hi, d[cls].max())
     weak = touched & ~strong
     flips = int((d[weak] > 0.5 * LR).sum())
-    print(f"{tag}: touched {touched.sum()}, strong {strong.sum()}, sign flips among the weak {flips}, "
-          f"max |dtheta| on strong {d[strong].max():.2e}")
+    assert flips <= 1e-3 * touched.sum(), (tag, flips)
+    print(f"{tag}: touched {touched.sum()}, strong {strong.sum()}, updates off by more than lr/2 (noise-level gradients) {flips}, "
+          f"share with relative gradient error < 1e-2: {np.mean(rel[touched] < 1e-2):.4f}")
     return th, m, v
 
 
@@ -103,15 +113,22 @@ def test_pipelined_steps_without_getters_track_the_oracle(nsm):
     tol = tol_for(w.field, f.nsm_mlp_path())
     f.nsm_set_option(nsm.NSM_OPT_BATCH_READY, 1)
     db = [nsm.DeviceBatch(b) for b in w.batches]
+    F = w.field.n_features
+    edges = _tensor_edges(O, F)
+    b1, b2 = float(np.float32(w.field.beta1)), float(np.float32(w.field.beta2))
+    m_scale, v_scale = np.zeros(len(edges) - 1), np.zeros(len(edges) - 1)
     for i in range(4):
         f.nsm_train_step(db[i], w.lambda_d, want_stats=False)
-        O.train_step(w.batches[i], w.lambda_d)
+        _, tr = O.train_step(w.batches[i], w.lambda_d, trace=("grad",))
+        for t, (a, b) in enumerate(zip(edges[:-1], edges[1:])):          # m = sum_k (1-b1) b1^(4-k) g_k, v likewise in g_k^2
+            gmax = np.abs(tr["grad"][a:b]).max()
+            m_scale[t] += (1 - b1) * b1 ** (3 - i) * gmax
+            v_scale[t] += (1 - b2) * b2 ** (3 - i) * gmax ** 2
     th, m, v, step = f.nsm_get_params()
     assert step == O.step == 4
-    F = w.field.n_features
-    for a, b in zip(_tensor_edges(O, F)[:-1], _tensor_edges(O, F)[1:]):
-        assert np.abs(m[a:b] - O.m[a:b]).max() <= tol * np.abs(O.m[a:b]).max(), a
-        assert np.abs(v[a:b] - O.v[a:b]).max() <= tol * np.abs(O.v[a:b]).max(), a
+    for t, (a, b) in enumerate(zip(edges[:-1], edges[1:])):
+        assert np.abs(m[a:b] - O.m[a:b]).max() <= tol * m_scale[t], (a, np.abs(m[a:b] - O.m[a:b]).max() / m_scale[t])
+        assert np.abs(v[a:b] - O.v[a:b]).max() <= 2 * tol * v_scale[t], (a, np.abs(v[a:b] - O.v[a:b]).max() / v_scale[t])
     changed = O.m != 0
     assert np.array_equal(m != 0, changed)                                   # the same entries were ever touched
     d = np.abs(th - O.theta)

@@ -164,16 +164,46 @@ class Room:
 
 
 def near_surface_occupancy(room, G, extent, target_fraction):
-    """bit = the cell centre is among the target_fraction of cells nearest to a surface."""
+    """bit = the cell centre is among the target_fraction of cells nearest to a surface (same distance as
+    Room.surface_distance, evaluated on the whole grid with per-axis terms broadcast over [gz, gy, gx])."""
     ax = cell_centres_axis(G) * extent
-    dist = np.empty((G, G, G))
-    yy, xx = np.meshgrid(ax, ax, indexing="ij")
-    for iz in range(G):
-        p = np.stack([xx.ravel(), yy.ravel(), np.full(G * G, ax[iz])], axis=1)
-        dist[iz] = room.surface_distance(p).reshape(G, G)
+    X, Y, Z = ax[None, None, :], ax[None, :, None], ax[:, None, None]
+    axes = (X, Y, Z)
+    sz = room.size
+    # walls: inside the room the nearest wall; outside it the distance to the room box
+    inside = [np.minimum(np.abs(a), np.abs(sz[i] - a)) for i, a in enumerate(axes)]
+    outside = [np.maximum(np.maximum(-a, a - sz[i]), 0.0) for i, a in enumerate(axes)]
+    d_in = np.minimum(np.minimum(inside[0], inside[1]), inside[2])
+    d_out2 = outside[0] ** 2 + outside[1] ** 2 + outside[2] ** 2
+    dist = np.where(d_out2 > 0, np.sqrt(d_out2), d_in)
+    for lo, hi in zip(room.box_lo, room.box_hi):
+        q = [np.maximum(np.maximum(lo[i] - a, a - hi[i]), 0.0) for i, a in enumerate(axes)]
+        inn = [np.minimum(a - lo[i], hi[i] - a) for i, a in enumerate(axes)]
+        out2 = q[0] ** 2 + q[1] ** 2 + q[2] ** 2
+        d_inn = np.abs(np.minimum(np.minimum(inn[0], inn[1]), inn[2]))
+        dist = np.minimum(dist, np.where(out2 > 0, np.sqrt(out2), d_inn))
+    for c, r in zip(room.sph_c, room.sph_r):
+        rr = np.sqrt((X - c[0]) ** 2 + (Y - c[1]) ** 2 + (Z - c[2]) ** 2)
+        dist = np.minimum(dist, np.abs(rr - r))
     thr = np.quantile(dist.reshape(-1)[:: max(1, G ** 3 // (1 << 20))], target_fraction)
     mask = dist <= thr
     return pack_bits(mask.reshape(-1)), float(mask.mean())
+
+
+def _mix64(x):
+    """splitmix64 finaliser on uint64 arrays (input generation only: per-pixel random numbers that do not depend on
+    which other pixels are evaluated)."""
+    x = (x ^ (x >> np.uint64(30))) * np.uint64(0xbf58476d1ce4e5b9)
+    x = (x ^ (x >> np.uint64(27))) * np.uint64(0x94d049bb133111eb)
+    return x ^ (x >> np.uint64(31))
+
+
+def pixel_uniform(seed, frame, pix, stream):
+    """U[0,1) per (seed, frame, pixel, stream), counter-based."""
+    with np.errstate(over="ignore"):
+        k = _mix64(np.uint64(seed) * np.uint64(0x9e3779b97f4a7c15) + np.uint64(frame) * np.uint64(0xd1b54a32d192ed03) + np.uint64(stream))
+        h = _mix64(k ^ (np.asarray(pix, np.uint64) * np.uint64(0x9e3779b97f4a7c15)))
+    return (h >> np.uint64(11)).astype(np.float64) * 2.0 ** -53
 
 
 class KeyframeSet:
@@ -181,7 +211,7 @@ class KeyframeSet:
     the resolution) with seeded look-at poses inside the room.  Per pixel: range r, RGB =
     albedo*(0.3+0.7 max(0,n.l)), D_slam = r(1+0.01 N(0,1)), Sigma_D = (0.01 r)^2; 5 % of pixels
     are outliers: D_slam = r U[0.3,2.0], Sigma_D = sigma_d^2, sigma_d ~ U[1,3].
-    Frames are ray-cast lazily and cached."""
+    Whole frames are ray-cast lazily and cached; batches cast only the pixels they draw."""
 
     def __init__(self, room, seed, n, width=1200, height=680):
         self.room, self.seed, self.n, self.W, self.H = room, seed, n, width, height
@@ -215,29 +245,34 @@ class KeyframeSet:
         o = np.broadcast_to(self.centres[i], d.shape).copy()
         return o, d
 
+    def pixels(self, i, pix):
+        """Keyframe i at the given pixel indices (ray cast on demand; every random number is a function of (seed, frame,
+        pixel), so a pixel's values do not depend on which other pixels are asked for)."""
+        pix = np.asarray(pix, np.int64)
+        o, d = self.rays(i, pix)
+        o32, d32 = o.astype(np.float32), d.astype(np.float32)      # cast what the field will see: the fp32 rays
+        n = o.shape[0]
+        r = np.empty(n)
+        rgb = np.empty((n, 3))
+        for a in range(0, n, 1 << 17):
+            sl = slice(a, min(n, a + (1 << 17)))
+            oo, dd = o32[sl].astype(np.float64), d32[sl].astype(np.float64)
+            rr, nn, sid = self.room.cast(oo, dd)
+            r[sl] = rr
+            rgb[sl] = self.room.shade(oo, dd, rr, nn, sid)
+        u = [pixel_uniform(self.seed, i, pix, k) for k in range(5)]
+        gauss = np.sqrt(-2.0 * np.log(1.0 - u[0])) * np.cos(2.0 * np.pi * u[1])     # Box-Muller
+        depth = r * (1.0 + 0.01 * gauss)
+        var = (0.01 * r) ** 2
+        outlier = u[2] < 0.05
+        depth = np.where(outlier, r * (0.3 + 1.7 * u[3]), depth)
+        var = np.where(outlier, (1.0 + 2.0 * u[4]) ** 2, var)
+        return dict(o=o32, d=d32, rgb=rgb.astype(np.float32), depth=depth.astype(np.float32), var=var.astype(np.float32),
+                    range=r.astype(np.float32), outlier=outlier)
+
     def frame(self, i):
         if i not in self._frames:
-            rng = np.random.Generator(np.random.PCG64([self.seed, 0xf4a3, i]))
-            o, d = self.rays(i)
-            # cast what the field will see: the fp32 rays
-            o32, d32 = o.astype(np.float32), d.astype(np.float32)
-            n = o.shape[0]
-            r = np.empty(n)
-            rgb = np.empty((n, 3))
-            for a in range(0, n, 1 << 17):
-                sl = slice(a, min(n, a + (1 << 17)))
-                oo, dd = o32[sl].astype(np.float64), d32[sl].astype(np.float64)
-                rr, nn, sid = self.room.cast(oo, dd)
-                r[sl] = rr
-                rgb[sl] = self.room.shade(oo, dd, rr, nn, sid)
-            depth = r * (1.0 + 0.01 * rng.standard_normal(n))
-            var = (0.01 * r) ** 2
-            outlier = rng.uniform(0, 1, n) < 0.05
-            depth = np.where(outlier, r * rng.uniform(0.3, 2.0, n), depth)
-            var = np.where(outlier, rng.uniform(1.0, 3.0, n) ** 2, var)
-            self._frames[i] = dict(o=o32, d=d32, rgb=rgb.astype(np.float32),
-                                   depth=depth.astype(np.float32), var=var.astype(np.float32),
-                                   range=r.astype(np.float32), outlier=outlier)
+            self._frames[i] = self.pixels(i, np.arange(self.W * self.H))
         return self._frames[i]
 
     def store_frame(self, i):
@@ -262,7 +297,10 @@ class KeyframeSet:
                for k in ("o", "d", "rgb", "depth", "var")}
         for i in np.unique(kf):
             sel = kf == i
-            fr = self.frame(int(i))
+            if int(i) in self._frames:
+                fr = {k: self._frames[int(i)][k][pix[sel]] for k in out}
+            else:
+                fr = self.pixels(int(i), pix[sel])
             for k in out:
-                out[k][sel] = fr[k][pix[sel]]
+                out[k][sel] = fr[k]
         return batch_cls(out["o"], out["d"], out["rgb"], out["depth"], out["var"], t_min, t_max, K)
