@@ -21,7 +21,8 @@ using namespace tableops;
 // the last tile beyond S are zero-filled so the MMA never reads stale data.
 template <int F, int MODE>
 __global__ void __launch_bounds__(256) encode_forward_kernel(LevelTable lv, const float *__restrict__ theta,
-                                                             Workspace ws, const uint32_t *__restrict__ d_S) {
+                                                             Workspace ws, const uint32_t *__restrict__ d_S, uint32_t seq) {
+  __shared__ uint32_t chunk_s;
   pdl_wait();
   pdl_trigger();
   tl_mark(ws.timeline, K_ENCODE, 0);
@@ -31,8 +32,12 @@ __global__ void __launch_bounds__(256) encode_forward_kernel(LevelTable lv, cons
   const uint32_t LF = lv.n_levels * F;
   const uint64_t pol_first = l2_evict_first(), pol_normal = l2_evict_normal();
   const uint32_t lane = threadIdx.x & 31;
-  for (uint64_t wb = (uint64_t)blockIdx.x * blockDim.x + (threadIdx.x & ~31u); wb < total;
-       wb += (uint64_t)gridDim.x * blockDim.x) {   // warp-uniform trip count: the dense-level path below uses warp collectives
+  ChunkQueue q(ws.work_ctr, seq);
+  for (;;) {   // 256 consecutive (level, sample) items at a time, handed out in order (see ChunkQueue); warp-uniform
+    const uint64_t cb = q.next(&chunk_s);
+    if (cb >= total) break;                        // block-uniform
+    const uint64_t wb = cb + (threadIdx.x & ~31u);
+    if (wb >= total) continue;                     // warp-uniform (the last, partial chunk)
     const uint64_t wi = wb + lane;
     const bool in_range = wi < total;
     const uint32_t l = (uint32_t)((in_range ? wi : wb) / S_it);
@@ -134,7 +139,9 @@ __global__ void __launch_bounds__(256) encode_forward_kernel(LevelTable lv, cons
 // this kernel (profiles/r1p), so fewer reductions is the only way to make it faster.
 template <int F>
 __global__ void __launch_bounds__(256) scatter_backward_kernel(LevelTable lv, float *__restrict__ grad, Workspace ws,
-                                                               const uint32_t *__restrict__ d_S, uint32_t l0, uint32_t l1) {
+                                                               const uint32_t *__restrict__ d_S, uint32_t l0, uint32_t l1, int prefetch,
+                                                               uint32_t seq) {
+  __shared__ uint32_t chunk_s;
   pdl_wait();
   pdl_trigger();
   tl_mark(ws.timeline, K_SCATTER, 0);
@@ -142,14 +149,52 @@ __global__ void __launch_bounds__(256) scatter_backward_kernel(LevelTable lv, fl
   const uint64_t total = S * (l1 - l0);
   const uint64_t pol_last = l2_evict_last();
   const uint32_t lane = threadIdx.x & 31;
-  const uint64_t stride = (uint64_t)gridDim.x * blockDim.x;
-  for (uint64_t wb = (uint64_t)blockIdx.x * blockDim.x + (threadIdx.x & ~31u); wb < total; wb += stride) {   // warp-uniform
-    const uint64_t wi = wb + lane;
+  const uint32_t nl = l1 - l0;
+  const uint64_t n_sc = (S + 255) / 256;              // 256-sample chunks per level
+  const uint64_t n_chunks = prefetch ? (total + 255) / 256 : n_sc * nl;
+  const uint64_t stride = (uint64_t)prefetch * 256;   // prefetch distance: that many chunks ahead of the one in hand
+  ChunkQueue q(ws.work_ctr, seq);
+  for (;;) {   // 256 (level, sample) items at a time, handed out in order; warp-uniform
+    const uint64_t c = q.next(&chunk_s) / 256;
+    if (c >= n_chunks) break;                          // block-uniform
+    // Two chunk orders.  Tables beyond the L2 (prefetch != 0): level-major, chunk c = items [256 c, 256 c + 256) of the
+    // level-major item list, so the chip stays inside one level's slice (ChunkQueue).  L2-resident tables: chunk c =
+    // samples [256 (c / nl), ...) of level c % nl, so the chunks in flight cover all levels evenly -- with every block
+    // on the same coarse level at once, its few thousand entries serialise the whole chip's reductions (measured at
+    // config 3: 285 us level-major, 269 us with the levels spread).
+    uint64_t wi, wb;                                   // this lane's item and its warp's first item (level-major indices)
+    if (prefetch) {
+      wb = c * 256 + (threadIdx.x & ~31u);
+      wi = wb + lane;
+    } else {
+      const uint64_t s0 = (c / nl) * 256 + (threadIdx.x & ~31u);
+      wb = (uint64_t)(c % nl) * S + s0;
+      wi = s0 + lane < S ? wb + lane : total;
+      if (s0 >= S) wb = total;
+    }
+    if (wb >= total) continue;                         // warp-uniform (partial chunks)
     const bool valid = wi < total;
     const uint32_t l = l0 + (uint32_t)((valid ? wi : wb) / S);
     const uint64_t s = (valid ? wi : wb) - (uint64_t)(l - l0) * S;
     const uint32_t l_first = __shfl_sync(0xffffffffu, l, 0);
     const bool one_dense_level = __all_sync(0xffffffffu, l == l_first) && lv.dense[l_first];
+    if (prefetch) {
+      // Tables far larger than the L2 (config 4): a reduction that misses waits in the L2's atomic unit for its DRAM fill,
+      // and that unit tracks far fewer misses than the read path (in situ: 0.98 GB of DRAM traffic in 349 us = 2.8 TB/s,
+      // while the encoder's plain loads reach 5.1 TB/s).  So the sectors a LATER chunk's item will reduce into are
+      // requested now, as L2 prefetches: by the time the reductions arrive (`prefetch` chunks later) they hit.
+      const uint64_t wn = wi + stride;
+      if (wn < total) {
+        const uint32_t ln = l0 + (uint32_t)(wn / S);
+        const uint64_t sn = wn - (uint64_t)(ln - l0) * S;
+        if (!lv.dense[ln]) {
+          const CornerIndex cn = corner_index(lv, ln, ws.s_x[sn], ws.s_x[ws.cap + sn], ws.s_x[2 * ws.cap + sn]);
+          const float *tab = grad + lv.offset[ln] * F;
+#pragma unroll
+          for (int k = 0; k < 8; ++k) asm volatile("prefetch.global.L2::evict_last [%0];" ::"l"(tab + (size_t)cn.slot[k] * F));
+        }
+      }
+    }
     if (!one_dense_level) {
       if (valid) scatter_sample_level<F>(lv, grad, ws, l, s, pol_last);
       continue;
@@ -261,20 +306,20 @@ int launch_unpack_records(const FieldParams &fp, int which, float *dst, cudaStre
 
 template <int F>
 static void launch_encode_f(const LevelTable &lv, const float *theta, const Workspace &ws, const uint32_t *d_S, int out_mode,
-                            dim3 grid, dim3 block, cudaStream_t st) {
-  if (out_mode == 0) launch_pdl(encode_forward_kernel<F, 0>, grid, block, 0, st, lv, theta, ws, d_S);
-  else if (out_mode == 1) launch_pdl(encode_forward_kernel<F, 1>, grid, block, 0, st, lv, theta, ws, d_S);
-  else launch_pdl(encode_forward_kernel<F, 2>, grid, block, 0, st, lv, theta, ws, d_S);
+                            dim3 grid, dim3 block, cudaStream_t st, uint32_t seq) {
+  if (out_mode == 0) launch_pdl(encode_forward_kernel<F, 0>, grid, block, 0, st, lv, theta, ws, d_S, seq);
+  else if (out_mode == 1) launch_pdl(encode_forward_kernel<F, 1>, grid, block, 0, st, lv, theta, ws, d_S, seq);
+  else launch_pdl(encode_forward_kernel<F, 2>, grid, block, 0, st, lv, theta, ws, d_S, seq);
 }
 
 int launch_encode(const LevelTable &lv, const float *theta, const Workspace &ws, const uint32_t *d_S, int out_mode,
-                  int n_sms, cudaStream_t st) {
+                  int n_sms, cudaStream_t st, uint32_t seq) {
   dim3 grid(n_sms * 8), block(256);
   switch (lv.n_features) {
-    case 1: launch_encode_f<1>(lv, theta, ws, d_S, out_mode, grid, block, st); break;
-    case 2: launch_encode_f<2>(lv, theta, ws, d_S, out_mode, grid, block, st); break;
-    case 4: launch_encode_f<4>(lv, theta, ws, d_S, out_mode, grid, block, st); break;
-    default: launch_encode_f<8>(lv, theta, ws, d_S, out_mode, grid, block, st); break;
+    case 1: launch_encode_f<1>(lv, theta, ws, d_S, out_mode, grid, block, st, seq); break;
+    case 2: launch_encode_f<2>(lv, theta, ws, d_S, out_mode, grid, block, st, seq); break;
+    case 4: launch_encode_f<4>(lv, theta, ws, d_S, out_mode, grid, block, st, seq); break;
+    default: launch_encode_f<8>(lv, theta, ws, d_S, out_mode, grid, block, st, seq); break;
   }
   return 1;
 }
@@ -289,14 +334,17 @@ int launch_get_touched(const FieldParams &fp, uint8_t *dst, cudaStream_t st) {
   return 1;
 }
 
-int launch_scatter(const LevelTable &lv, float *grad, const Workspace &ws, const uint32_t *d_S, int n_sms, cudaStream_t st) {
+int launch_scatter(const LevelTable &lv, float *grad, const Workspace &ws, const uint32_t *d_S, int n_sms, cudaStream_t st,
+                   uint32_t seq) {
+  // gradient array beyond what the L2 keeps (~64 MB, profiles/r1p): prefetch NSM_SCATTER_PF_CHUNKS chunks ahead
+  const int prefetch = lv.offset[lv.n_levels] * lv.n_features * sizeof(float) > (96ull << 20) ? NSM_SCATTER_PF_CHUNKS : 0;
   dim3 grid(n_sms * 8), block(256);
   const uint32_t l0 = 0, l1 = lv.n_levels;
   switch (lv.n_features) {
-    case 1: launch_pdl(scatter_backward_kernel<1>, grid, block, 0, st, lv, grad, ws, d_S, l0, l1); break;
-    case 2: launch_pdl(scatter_backward_kernel<2>, grid, block, 0, st, lv, grad, ws, d_S, l0, l1); break;
-    case 4: launch_pdl(scatter_backward_kernel<4>, grid, block, 0, st, lv, grad, ws, d_S, l0, l1); break;
-    default: launch_pdl(scatter_backward_kernel<8>, grid, block, 0, st, lv, grad, ws, d_S, l0, l1); break;
+    case 1: launch_pdl(scatter_backward_kernel<1>, grid, block, 0, st, lv, grad, ws, d_S, l0, l1, prefetch, seq); break;
+    case 2: launch_pdl(scatter_backward_kernel<2>, grid, block, 0, st, lv, grad, ws, d_S, l0, l1, prefetch, seq); break;
+    case 4: launch_pdl(scatter_backward_kernel<4>, grid, block, 0, st, lv, grad, ws, d_S, l0, l1, prefetch, seq); break;
+    default: launch_pdl(scatter_backward_kernel<8>, grid, block, 0, st, lv, grad, ws, d_S, l0, l1, prefetch, seq); break;
   }
   return 1;
 }

@@ -88,6 +88,7 @@ struct nsm_field {
   std::vector<void *> allocs;
   uint32_t step = 0;
   uint64_t launches = 0;
+  uint32_t work_seq = 0;      // launch sequence number of the table kernels (ChunkQueue counter ring)
   bool occ_full = true;
   uint32_t occ_updates = 0;   // F4: decayed partial refreshes since the last full one
   bool grid_seeded = false;   // F4: the running density grid holds a full FROM_FIELD pass (SET / FULL invalidate it)
@@ -298,7 +299,7 @@ nsm_status enqueue_forward(nsm_field *f, const nsm_ray_batch *b, uint32_t R, boo
     RUN(f, K_MARCH, launch_march(mp, f->occ_full ? nullptr : f->fp.occ_bits, b->origins, b->dirs, f->ws, train ? 1 : 0, f->stream, dirs_copy));
   }
   const int bf16 = f->cfg.mlp_precision == NSM_MLP_BF16;
-  RUN(f, K_ENCODE, launch_encode(f->lv, f->fp.theta, f->ws, d_S, f->use_tc ? 1 + bf16 : 0, f->n_sms, f->stream));
+  RUN(f, K_ENCODE, launch_encode(f->lv, f->fp.theta, f->ws, d_S, f->use_tc ? 1 + bf16 : 0, f->n_sms, f->stream, f->work_seq++));
   if (f->use_tc)
     RUN(f, K_MLP_FWD, launch_mlp_forward_tc(f->ms, bf16, mlp_dirs, f->ws, d_S, 0, train ? 1 : 0, f->n_sms, f->stream));
   else
@@ -366,7 +367,7 @@ nsm_status enqueue_backward(nsm_field *f, const nsm_ray_batch *b, float lambda_d
   }
   // train step: the scatter is issued by enqueue_adam, behind the MLP Adam's hand-off to the side stream
   f->scatter_pending = defer_scatter;
-  if (!defer_scatter) RUN(f, K_SCATTER, launch_scatter(f->lv, f->fp.grad, f->ws, d_S, f->n_sms, f->stream));
+  if (!defer_scatter) RUN(f, K_SCATTER, launch_scatter(f->lv, f->fp.grad, f->ws, d_S, f->n_sms, f->stream, f->work_seq++));
   f->grads_dirty = true;
   f->last_R = R;
   f->last_K = b->n_candidates;
@@ -399,7 +400,7 @@ nsm_status enqueue_adam(nsm_field *f) {
   // gradient array stays in L2 between its uses, was measured in round 1 -- profiles/r1j: every extra pair of launches
   // costs ~19 us of ramp and tail, more than the DRAM traffic it saves.)
   if (f->scatter_pending)
-    RUN(f, K_SCATTER, launch_scatter(f->lv, f->fp.grad, f->ws, f->ws.offsets + f->last_R, f->n_sms, f->stream));
+    RUN(f, K_SCATTER, launch_scatter(f->lv, f->fp.grad, f->ws, f->ws.offsets + f->last_R, f->n_sms, f->stream, f->work_seq++));
   f->scatter_pending = false;
   if (use_side) {   // the scatter is in: the side stream (next step's marcher) may overwrite the samples
     CUDA_TRY(cudaEventRecord(f->ev_main, f->stream));
@@ -535,7 +536,7 @@ nsm_status nsm_create_field(const nsm_field_config *cfg, void *cuda_stream, nsm_
   A(f->alloc(&fp.mlp_theta, fp.n_mlp)); A(f->alloc(&fp.mlp_m, fp.n_mlp)); A(f->alloc(&fp.mlp_v, fp.n_mlp)); A(f->alloc(&fp.mlp_grad, fp.n_mlp));
   A(f->alloc(&fp.grad, fp.n_table, false)); A(f->alloc(&fp.occ_bits, (G3 + 7) / 8 + 4));
   A(f->alloc(&fp.occ_grid, G3));
-  A(f->alloc(&ws.counts, R)); A(f->alloc(&ws.offsets, R + 1)); A(f->alloc(&ws.scan_state, march_scan_state_entries(R) + 1)); A(f->alloc(&ws.scan_ctr, 2));
+  A(f->alloc(&ws.counts, R)); A(f->alloc(&ws.offsets, R + 1)); A(f->alloc(&ws.scan_state, march_scan_state_entries(R) + 1)); A(f->alloc(&ws.scan_ctr, 2)); A(f->alloc(&ws.work_ctr, 8));
   A(f->alloc(&ws.C, 3 * (size_t)R)); A(f->alloc(&ws.D_hat, R)); A(f->alloc(&ws.O, R));
   A(f->alloc(&ws.s_ray, cap)); A(f->alloc(&ws.s_k, cap)); A(f->alloc(&ws.s_t, cap)); A(f->alloc(&ws.s_delta, cap));
   A(f->alloc(&ws.s_x, 3 * cap));
@@ -714,7 +715,7 @@ nsm_status nsm_update_occupancy(nsm_field *f, nsm_occ_mode mode, const uint8_t *
         const uint64_t n = (G3 - first < chunk) ? G3 - first : chunk;
         RUN(f, K_OCC, launch_occ_cells(f->cfg.occ_res, first, n, f->ws, d_S, f->stream));
         RUN(f, K_ENCODE, launch_encode(f->lv, f->fp.theta, f->ws, d_S, f->use_tc ? 1 + (f->cfg.mlp_precision == NSM_MLP_BF16) : 0,
-                                       f->n_sms, f->stream));
+                                       f->n_sms, f->stream, f->work_seq++));
         if (f->use_tc)
           RUN(f, K_MLP_FWD, launch_mlp_forward_tc(f->ms, f->cfg.mlp_precision == NSM_MLP_BF16, nullptr, f->ws, d_S, 1, 0, f->n_sms,
                                                   f->stream));
@@ -752,7 +753,7 @@ nsm_status nsm_update_occupancy_decay(nsm_field *f, uint32_t n_subsets, float de
     const uint64_t n = (n_vis - j0 < chunk) ? n_vis - j0 : chunk;
     const uint64_t first = c0 + j0 * n_subsets;
     RUN(f, K_OCC, launch_occ_cells_strided(f->cfg.occ_res, first, n_subsets, n, f->ws, d_S, f->stream));
-    RUN(f, K_ENCODE, launch_encode(f->lv, f->fp.theta, f->ws, d_S, f->use_tc ? 1 + bf16 : 0, f->n_sms, f->stream));
+    RUN(f, K_ENCODE, launch_encode(f->lv, f->fp.theta, f->ws, d_S, f->use_tc ? 1 + bf16 : 0, f->n_sms, f->stream, f->work_seq++));
     if (f->use_tc)
       RUN(f, K_MLP_FWD, launch_mlp_forward_tc(f->ms, bf16, nullptr, f->ws, d_S, 1, 0, f->n_sms, f->stream));
     else
