@@ -105,36 +105,48 @@ def test_config4_full_size_train_step_parameters(nsm):
 
 def test_pipelined_steps_without_getters_track_the_oracle(nsm):
     """Four nsm_train_step calls back to back with no getter, no statistics and NSM_OPT_BATCH_READY set -- so the marcher
-    of step i+1 really runs beside the table Adam of step i and the MLP Adam on the side stream -- against the oracle
-    free-running the same four steps from the same theta_0 (steps 1-4 are still comparable).  m after four
-    steps is a fixed linear combination of the four gradients, each held to P4's tolerance."""
+    of step i+1 really runs beside the table Adam of step i and the MLP Adam on the side stream -- against (a) the same four
+    steps issued one at a time (statistics read back after every step, NSM_OPT_BATCH_READY off: nothing overlaps) and (b) the
+    oracle free-running them from the same theta_0.  The iteration is chaotic (P6): from step 2 on the two sides of
+    (b) evaluate their gradients at parameters that already differ by up to 2 lr on entries whose step-1 gradient was
+    noise-level for 16-bit MLP operands, so (b) is held to 2.5 x P4's relative-L2 tolerance (measured 3.1e-2 / 3.7e-2 for
+    m / v on the worst tensor) and a fifth step's loss to 1e-3; the two GPU runs of (a) differ by the order of their atomics
+    only and must agree an order of magnitude tighter -- a stream-ordering bug of the pipelined route would show there."""
     w = configs.config2(n_batches=4)
-    f, O, _ = make_pair(nsm, w, seed=21, table_scale=0.05, omp=True)
+    f, O, theta0 = make_pair(nsm, w, seed=21, table_scale=0.05, omp=True)
+    f2 = nsm.Field(w.field, "cuda:0")
+    f2.nsm_set_params(theta0)
+    f2.nsm_update_occupancy(nsm.NSM_OCC_SET, w.bits)
     tol = tol_for(w.field, f.nsm_mlp_path())
     f.nsm_set_option(nsm.NSM_OPT_BATCH_READY, 1)
     db = [nsm.DeviceBatch(b) for b in w.batches]
     F = w.field.n_features
     edges = _tensor_edges(O, F)
-    b1, b2 = float(np.float32(w.field.beta1)), float(np.float32(w.field.beta2))
-    m_scale, v_scale = np.zeros(len(edges) - 1), np.zeros(len(edges) - 1)
     for i in range(4):
         f.nsm_train_step(db[i], w.lambda_d, want_stats=False)
-        _, tr = O.train_step(w.batches[i], w.lambda_d, trace=("grad",))
-        for t, (a, b) in enumerate(zip(edges[:-1], edges[1:])):          # m = sum_k (1-b1) b1^(4-k) g_k, v likewise in g_k^2
-            gmax = np.abs(tr["grad"][a:b]).max()
-            m_scale[t] += (1 - b1) * b1 ** (3 - i) * gmax
-            v_scale[t] += (1 - b2) * b2 ** (3 - i) * gmax ** 2
+    for i in range(4):
+        f2.nsm_train_step(db[i], w.lambda_d, want_stats=True)
+        f2.nsm_get_params()
+        O.train_step(w.batches[i], w.lambda_d)
     th, m, v, step = f.nsm_get_params()
-    assert step == O.step == 4
-    for t, (a, b) in enumerate(zip(edges[:-1], edges[1:])):
-        assert np.abs(m[a:b] - O.m[a:b]).max() <= tol * m_scale[t], (a, np.abs(m[a:b] - O.m[a:b]).max() / m_scale[t])
-        assert np.abs(v[a:b] - O.v[a:b]).max() <= 2 * tol * v_scale[t], (a, np.abs(v[a:b] - O.v[a:b]).max() / v_scale[t])
+    th2, m2, v2, step2 = f2.nsm_get_params()
+    assert step == step2 == O.step == 4
+    pairs = list(zip(edges[:-1], edges[1:]))
+    rel = lambda x, y: max(np.linalg.norm(x[a:b] - y[a:b]) / np.linalg.norm(y[a:b]) for a, b in pairs)
+    gg_m, gg_v, go_m, go_v = rel(m, m2), rel(v, v2), rel(m, O.m), rel(v, O.v)
+    print(f"pipelined 4 steps, worst per-tensor relative L2 error: m {gg_m:.2e}, v {gg_v:.2e} against the unpipelined GPU run; "
+          f"m {go_m:.2e}, v {go_v:.2e} against the oracle")
+    assert gg_m <= 1e-4 and gg_v <= 1e-4
+    assert go_m <= 2.5 * tol and go_v <= 2.5 * tol
     changed = O.m != 0
-    assert np.array_equal(m != 0, changed)                                   # the same entries were ever touched
+    assert np.array_equal(m != 0, changed) and np.array_equal(m2 != 0, changed)      # the same entries were ever touched
     d = np.abs(th - O.theta)
     print(f"pipelined 4 steps: theta differs by more than lr/2 on {(d > 0.5 * LR).sum()} of {changed.sum()} updated parameters")
     assert (d > 0.5 * LR).mean() < 2e-3
-    f.close()
+    st = f.nsm_train_step(db[0], w.lambda_d)                                 # a fifth step, each side from its own state
+    so, _ = O.train_step(w.batches[0], w.lambda_d)
+    assert st["n_samples"] == so["n_samples"] and abs(st["loss"] - so["loss"]) <= 1e-3 * abs(so["loss"]), (st["loss"], so["loss"])
+    f.close(); f2.close()
 
 
 def test_config3_free_running_loss_curve(nsm):
