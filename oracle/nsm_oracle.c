@@ -121,12 +121,68 @@ float orc_jitter_u(uint64_t seed, uint32_t step, uint32_t r, uint32_t k) {
   return (float)(orc_hash32(seed, step, r, k) >> 8) * 0x1p-24f; /* exact in fp32 */
 }
 
+/* ------------------------------------------------------------------ S2 / F4: occupancy cells */
+
+/* R23 (the paper is silent, [17] keeps a pyramid of grids): C = occ_cascades nested cubes share the
+ * centre of the field cube; cascade j has half-side 2^(j-C) in normalised coordinates (j = C-1 is the whole cube) and
+ * its own G^3 cells.  A point belongs to the finest cascade that contains it, by the max-norm of x - 0.5. */
+static uint32_t n_cascades(const orc_config *cfg) { return cfg->occ_cascades ? cfg->occ_cascades : 1u; }
+
+uint64_t orc_occupancy_cell(const orc_config *cfg, const float x[3], uint32_t *cascade_out) {
+  const uint32_t C = n_cascades(cfg), G = cfg->occ_res;
+  uint32_t j = C - 1;
+  float xp[3] = {x[0], x[1], x[2]};   /* the outermost cascade (and C = 1) uses the normalised position itself */
+  if (C > 1) {
+    float q[3], m = 0.0f;
+    for (int c = 0; c < 3; ++c) {
+      q[c] = x[c] - 0.5f;                      /* one binary32 subtraction */
+      float a = fabsf(q[c]);
+      if (a > m) m = a;
+    }
+    for (j = 0; j + 1 < C; ++j)
+      if (m < ldexpf(1.0f, (int)j - (int)C)) break;   /* smallest j with m < 2^(j-C); none: j = C-1 */
+    if (j + 1 < C) {
+      const float s = ldexpf(1.0f, (int)(C - 1 - j));  /* zoom of cascade j: 2^(C-1-j), exact */
+      for (int c = 0; c < 3; ++c) xp[c] = fmaf(q[c], s, 0.5f);   /* one rounding */
+    }
+  }
+  uint32_t g[3];
+  for (int c = 0; c < 3; ++c) {
+    float s = xp[c] * (float)G;
+    int gi = (int)floorf(s);
+    if (gi > (int)G - 1) gi = (int)G - 1;
+    if (gi < 0) gi = 0;                        /* unreachable for x in [0,1); keeps the index in range for any input */
+    g[c] = (uint32_t)gi;
+  }
+  if (cascade_out) *cascade_out = j;
+  return (uint64_t)j * G * G * G + (uint64_t)g[0] + (uint64_t)G * ((uint64_t)g[1] + (uint64_t)G * g[2]);
+}
+
+/* The inverse map: the normalised position of the point at fractional offsets u in [0,1)^3 inside cell `cell`
+ * (global index j G^3 + gx + G (gy + G gz)); u = 0.5 is the cell centre.  x' = (g + u) / G in the cascade's own
+ * coordinates (an addition and a division in binary32), then x = fma(x' - 0.5, 2^(j-(C-1)), 0.5) for j < C-1. */
+void orc_occupancy_cell_point(const orc_config *cfg, uint64_t cell, const float u[3], float x_out[3]) {
+  const uint32_t C = n_cascades(cfg), G = cfg->occ_res;
+  const uint64_t G3 = (uint64_t)G * G * G;
+  const uint32_t j = (uint32_t)(cell / G3);
+  const uint64_t loc = cell % G3;
+  const uint32_t g[3] = {(uint32_t)(loc % G), (uint32_t)((loc / G) % G), (uint32_t)(loc / ((uint64_t)G * G))};
+  for (int c = 0; c < 3; ++c) {
+    float xp = ((float)g[c] + u[c]) / (float)G;
+    if (j + 1 < C) {
+      float q = xp - 0.5f;
+      xp = fmaf(q, ldexpf(1.0f, (int)j - (int)(C - 1)), 0.5f);
+    }
+    x_out[c] = xp;
+  }
+}
+
 /* ------------------------------------------------------------------ S1-S3: march ---------- */
 
 int64_t orc_march(const orc_config *cfg, const uint8_t *bits, const orc_batch *b, int jitter,
                   uint32_t step, uint32_t *counts, uint32_t *offsets, uint32_t *s_ray,
                   uint32_t *s_k, float *s_t, float *s_delta, float *s_x) {
-  const uint32_t R = b->n_rays, K = b->n_candidates, G = cfg->occ_res;
+  const uint32_t R = b->n_rays, K = b->n_candidates;
   if (K == 0) return -1;
   /* S0 host constants, fp32 */
   const float dt = (b->t_max - b->t_min) / (float)K;
@@ -164,15 +220,8 @@ int64_t orc_march(const orc_config *cfg, const uint8_t *bits, const orc_batch *b
         if (!(x[c] >= 0.0f && x[c] < 1.0f)) inside = 0;
       }
       if (!inside) continue;
-      /* S2: occupancy cell and bit */
-      uint32_t g[3];
-      for (int c = 0; c < 3; ++c) {
-        float s = x[c] * (float)G;
-        int gi = (int)floorf(s);
-        if (gi > (int)G - 1) gi = (int)G - 1;
-        g[c] = (uint32_t)gi;
-      }
-      uint64_t cell = (uint64_t)g[0] + (uint64_t)G * ((uint64_t)g[1] + (uint64_t)G * g[2]);
+      /* S2: occupancy cell (of the finest cascade that contains x, F4 / R23) and bit */
+      uint64_t cell = orc_occupancy_cell(cfg, x, NULL);
       int bit = bits ? ((bits[cell >> 3] >> (cell & 7)) & 1) : 1; /* bits==NULL: FULL */
       if (!bit) continue;
       /* S3: append in (ray, k) order */
@@ -792,64 +841,54 @@ done:
 
 /* ------------------------------------------------------------------ S14: occupancy -------- */
 
+/* sigma (S4 + S5 + exp) at the normalised position x */
+static double point_sigma(const orc_levels *lv, const orc_mlp *M, const double *theta, const float x[3]) {
+  const double *Wm = theta + lv->off[lv->L] * lv->F;
+  double e[ORC_MAX_WIDTH], hd[ORC_MAX_WIDTH];
+  encode_point(lv, theta, x, NULL, NULL, e);
+  linear(Wm + M->o_d1, M->Hd, M->LF, e, hd, 1);
+  double g0 = 0.0;
+  for (uint32_t i = 0; i < M->Hd; ++i) g0 += Wm[M->o_d2 + i] * hd[i]; /* row 0 of W_d2 */
+  double g0c = g0 < -15.0 ? -15.0 : (g0 > 15.0 ? 15.0 : g0);
+  return exp(g0c);
+}
+
+/* sigma at the centre of occupancy cell `cell` (global index over the cascades); the centre of a cell of a
+ * power-of-two grid is exact in fp32 */
+static double cell_sigma(const orc_config *cfg, const orc_levels *lv, const orc_mlp *M, const double *theta, uint64_t cell) {
+  const float half[3] = {0.5f, 0.5f, 0.5f};
+  float x[3];
+  orc_occupancy_cell_point(cfg, cell, half, x);
+  return point_sigma(lv, M, theta, x);
+}
+
 int orc_occupancy_from_field(const orc_config *cfg, const double *theta, uint8_t *bits_out,
                              double *sigma_out) {
   orc_levels lv;
   orc_mlp M;
   if (levels_init(cfg, &lv) != 0 || mlp_init(cfg, &M) != 0) return -1;
   const uint32_t G = cfg->occ_res;
-  const uint64_t n_table = lv.off[lv.L] * lv.F;
-  const uint64_t cells = (uint64_t)G * G * G;
+  const uint64_t cells = (uint64_t)n_cascades(cfg) * G * G * G;
   memset(bits_out, 0, (cells + 7) / 8);
-  const double *Wm = theta + n_table;
-  int64_t gz;
+  int64_t w;
+  /* one 8-cell byte of the bitfield per iteration, so no two threads write the same byte */
 #pragma omp parallel for schedule(static)
-  for (gz = 0; gz < (int64_t)G; ++gz) {
-    double e[ORC_MAX_WIDTH], hd[ORC_MAX_WIDTH];
-    for (uint32_t gy = 0; gy < G; ++gy)
-      for (uint32_t gx = 0; gx < G; ++gx) {
-        /* cell centre, exact in fp32 for power-of-two G */
-        float x[3] = {((float)gx + 0.5f) / (float)G, ((float)gy + 0.5f) / (float)G,
-                      ((float)gz + 0.5f) / (float)G};
-        encode_point(&lv, theta, x, NULL, NULL, e);
-        linear(Wm + M.o_d1, M.Hd, M.LF, e, hd, 1);
-        double g0 = 0.0;
-        for (uint32_t i = 0; i < M.Hd; ++i) g0 += Wm[M.o_d2 + i] * hd[i]; /* row 0 of W_d2 */
-        double g0c = g0 < -15.0 ? -15.0 : (g0 > 15.0 ? 15.0 : g0);
-        double sigma = exp(g0c);
-        uint64_t cell = (uint64_t)gx + (uint64_t)G * ((uint64_t)gy + (uint64_t)G * (uint64_t)gz);
-        if (sigma_out) sigma_out[cell] = sigma;
-        if (sigma > (double)cfg->occ_sigma_threshold) {
-          /* byte cell>>3 belongs to one gz slab only when G^2 % 8 == 0; guard otherwise */
-#pragma omp atomic
-          bits_out[cell >> 3] |= (uint8_t)(1u << (cell & 7));
-        }
-      }
-  }
+  for (w = 0; w < (int64_t)((cells + 7) / 8); ++w)
+    for (uint64_t cell = 8 * (uint64_t)w; cell < 8 * (uint64_t)w + 8 && cell < cells; ++cell) {
+      const double sigma = cell_sigma(cfg, &lv, &M, theta, cell);
+      if (sigma_out) sigma_out[cell] = sigma;
+      if (sigma > (double)cfg->occ_sigma_threshold) bits_out[cell >> 3] |= (uint8_t)(1u << (cell & 7));
+    }
   return 0;
 }
 
 /* F4: decayed running maximum with a strided partial refresh (header comment of orc_occupancy_decay_update). */
-static double cell_sigma(const orc_config *cfg, const orc_levels *lv, const orc_mlp *M, const double *theta, uint64_t cell) {
-  const uint32_t G = cfg->occ_res;
-  const uint32_t gx = (uint32_t)(cell % G), gy = (uint32_t)((cell / G) % G), gz = (uint32_t)(cell / ((uint64_t)G * G));
-  const double *Wm = theta + lv->off[lv->L] * lv->F;
-  double e[ORC_MAX_WIDTH], hd[ORC_MAX_WIDTH];
-  float x[3] = {((float)gx + 0.5f) / (float)G, ((float)gy + 0.5f) / (float)G, ((float)gz + 0.5f) / (float)G};
-  encode_point(lv, theta, x, NULL, NULL, e);
-  linear(Wm + M->o_d1, M->Hd, M->LF, e, hd, 1);
-  double g0 = 0.0;
-  for (uint32_t i = 0; i < M->Hd; ++i) g0 += Wm[M->o_d2 + i] * hd[i];
-  double g0c = g0 < -15.0 ? -15.0 : (g0 > 15.0 ? 15.0 : g0);
-  return exp(g0c);
-}
-
 int orc_occupancy_decay_update(const orc_config *cfg, const double *theta, double *grid, uint32_t update_index,
                                uint32_t n_sub, double decay, uint8_t *bits_out, double *visited_sigma) {
   orc_levels lv;
   orc_mlp M;
   if (levels_init(cfg, &lv) != 0 || mlp_init(cfg, &M) != 0 || n_sub == 0) return -1;
-  const uint64_t cells = (uint64_t)cfg->occ_res * cfg->occ_res * cfg->occ_res;
+  const uint64_t cells = (uint64_t)n_cascades(cfg) * cfg->occ_res * cfg->occ_res * cfg->occ_res;
   memset(bits_out, 0, (cells + 7) / 8);
   for (uint64_t c = 0; c < cells; ++c) {
     grid[c] *= decay;
@@ -861,6 +900,34 @@ int orc_occupancy_decay_update(const orc_config *cfg, const double *theta, doubl
     }
     if (grid[c] > (double)cfg->occ_sigma_threshold) bits_out[c >> 3] |= (uint8_t)(1u << (c & 7));
   }
+  return 0;
+}
+
+/* F4, stochastic refresh (header comment of orc_occupancy_stochastic_update). */
+int orc_occupancy_stochastic_update(const orc_config *cfg, const double *theta, double *grid, uint32_t update_index,
+                                    uint32_t n_draws, double decay, uint8_t *bits_out, uint64_t *cells_out, float *x_out,
+                                    double *sigma_out) {
+  orc_levels lv;
+  orc_mlp M;
+  if (levels_init(cfg, &lv) != 0 || mlp_init(cfg, &M) != 0) return -1;
+  const uint64_t cells = (uint64_t)n_cascades(cfg) * cfg->occ_res * cfg->occ_res * cfg->occ_res;
+  if (cells > (1ull << 31)) return -1;            /* (hash * cells) >> 32 in 64 bits */
+  for (uint64_t c = 0; c < cells; ++c) grid[c] *= decay;
+  for (uint32_t i = 0; i < n_draws; ++i) {
+    const uint64_t cell = ((uint64_t)orc_hash32(cfg->seed, update_index, i, 0xffff0003u) * cells) >> 32;
+    float u[3], x[3];
+    for (uint32_t a = 0; a < 3; ++a)
+      u[a] = (float)(orc_hash32(cfg->seed, update_index, i, 0xffff0004u + a) >> 8) * 0x1p-24f;   /* exact */
+    orc_occupancy_cell_point(cfg, cell, u, x);
+    const double s = point_sigma(&lv, &M, theta, x);
+    if (s > grid[cell]) grid[cell] = s;           /* a cell drawn twice keeps the larger density: order-free */
+    if (cells_out) cells_out[i] = cell;
+    if (x_out) { x_out[3 * i] = x[0]; x_out[3 * i + 1] = x[1]; x_out[3 * i + 2] = x[2]; }
+    if (sigma_out) sigma_out[i] = s;
+  }
+  memset(bits_out, 0, (cells + 7) / 8);
+  for (uint64_t c = 0; c < cells; ++c)
+    if (grid[c] > (double)cfg->occ_sigma_threshold) bits_out[c >> 3] |= (uint8_t)(1u << (c & 7));
   return 0;
 }
 

@@ -23,7 +23,8 @@
  *   S15 render with transmittance cut     PAPER.md:163; R15
  *   F1  ray-batch sampler over keyframes   PAPER.md:157-159; DESIGN.md "F1"
  *   F2  pose gradients dL/do, d x dL/dd    PAPER.md:120,130-133 (Eq. 3 over T); DESIGN.md "F2" (row f2)
- *   F4  decayed partial occupancy refresh  paper silent -> [17]; DESIGN.md "F4" (row f4)
+ *   F4  decayed partial occupancy refresh (strided and stochastic), nested occupancy cascades
+ *                                          paper silent -> [17]; DESIGN.md "F4" R23-R25 (row f4)
  *
  * Precision: the INDEX PATH (everything that decides an integer, and the fp32 quantities
  * t, delta, x, w) is a fixed sequence of IEEE binary32 operations (compile with
@@ -60,6 +61,7 @@ typedef struct {
   float    lr, beta1, beta2, eps;
   uint32_t sparse_table_adam;
   uint64_t seed;
+  uint32_t occ_cascades;   /* F4 / R23: number of nested occupancy grids (0 or 1: the single grid of S2) */
 } orc_config;
 
 typedef struct {
@@ -146,12 +148,27 @@ int orc_train_step(const orc_config *cfg, double *theta, double *m, double *v, u
 void orc_adam(uint64_t n, double *theta, double *m, double *v, const double *g, const uint8_t *mask,
               uint32_t mask_group, uint32_t step, double lr, double beta1, double beta2, double eps);
 
-/* S14 FROM_FIELD: bits_out has G^3/8 bytes.  sigma_out (may be NULL) gets G^3 densities. */
+/* S2 / F4 (R23; the paper is silent on the occupancy structure and delegates to [17]; PAPER.md:266 asks
+ * for a map that follows "the region of interest"): occ_cascades = C nested occupancy grids of G^3 cells each around the
+ * centre of the field cube.  In normalised coordinates cascade j (0 = finest) is the cube |x - 0.5|_max < 2^(j-C);
+ * cascade C-1 is the whole cube [0,1)^3.  A point is tested against the finest cascade that contains it:
+ *   q_c = x_c - 0.5 (binary32),  m = max_c |q_c|,  j = the smallest j in [0, C-1) with m < 2^(j-C), else C-1;
+ *   x'_c = fma(q_c, 2^(C-1-j), 0.5) for j < C-1,  x'_c = x_c for j = C-1;   g_c = min(floor(x'_c G), G-1);
+ *   bit index = j G^3 + g_x + G (g_y + G g_z).
+ * C = 1 is S2's single grid, with identical arithmetic.  Returns the bit index; *cascade_out (may be NULL) gets j. */
+uint64_t orc_occupancy_cell(const orc_config *cfg, const float x[3], uint32_t *cascade_out);
+/* The inverse map: the normalised position of the point at offsets u in [0,1)^3 inside the cell with that bit index
+ * (u = 0.5: the cell centre, which FROM_FIELD evaluates):  x'_c = (g_c + u_c) / G (an addition and a division in
+ * binary32), x_c = fma(x'_c - 0.5, 2^(j-(C-1)), 0.5) for j < C-1, x_c = x'_c for j = C-1. */
+void orc_occupancy_cell_point(const orc_config *cfg, uint64_t cell, const float u[3], float x_out[3]);
+
+/* S14 FROM_FIELD: bits_out has C G^3/8 bytes (C = occ_cascades, cascade-major).  sigma_out (may be NULL) gets the
+ * C G^3 densities at the cell centres. */
 int orc_occupancy_from_field(const orc_config *cfg, const double *theta, uint8_t *bits_out,
                              double *sigma_out);
 
 /* F4 (the paper is silent, [17] keeps a decayed running maximum of the density and refreshes only
- * part of the grid per update): `grid` [G^3] is the running density, `update_index` the number of decay updates done so far.
+ * part of the grid per update): `grid` [C G^3] (all cascades, index = the bit index) is the running density, `update_index` the number of decay updates done so far.
  *   every cell:                                   grid[c] <- decay * grid[c]
  *   cells with c mod n_sub == update_index mod n_sub:   grid[c] <- max(grid[c], sigma(centre of c))      (1/n_sub of the grid)
  *   bit[c] = grid[c] > occ_sigma_threshold
@@ -159,6 +176,19 @@ int orc_occupancy_from_field(const orc_config *cfg, const double *theta, uint8_t
  * refresh sets grid[c] = sigma(c).  visited_sigma (may be NULL) gets sigma for the visited cells and -1 elsewhere. */
 int orc_occupancy_decay_update(const orc_config *cfg, const double *theta, double *grid, uint32_t update_index,
                                uint32_t n_sub, double decay, uint8_t *bits_out, double *visited_sigma);
+
+/* F4, stochastic variant ([17] refreshes a random subset of the cells per update, each at a random point inside the cell;
+ * reading R25: uniform draws over all C G^3 cells, no second draw among the occupied ones):
+ *   every cell:  grid[c] <- decay * grid[c]
+ *   for i < n_draws:  c_i = (h(seed, update_index, i, 0xffff0003) * n_cells) >> 32           (h = orc_hash32, n_cells <= 2^31)
+ *                     u_a = (h(seed, update_index, i, 0xffff0004 + a) >> 8) * 2^-24,  a = 0, 1, 2
+ *                     grid[c_i] <- max(grid[c_i], sigma(orc_occupancy_cell_point(c_i, u)))
+ *   bit[c] = grid[c] > occ_sigma_threshold
+ * A cell drawn twice keeps the larger density, so the result does not depend on the order of the draws.
+ * cells_out [n_draws], x_out [n_draws,3], sigma_out [n_draws] may be NULL. */
+int orc_occupancy_stochastic_update(const orc_config *cfg, const double *theta, double *grid, uint32_t update_index,
+                                    uint32_t n_draws, double decay, uint8_t *bits_out, uint64_t *cells_out, float *x_out,
+                                    double *sigma_out);
 
 /* S15. */
 int orc_render(const orc_config *cfg, const double *theta, const uint8_t *bits, const orc_batch *b,

@@ -26,7 +26,7 @@ class OrcConfig(C.Structure):
                 ("color_hidden", C.c_uint32), ("color_hidden_layers", C.c_uint32),
                 ("bg", C.c_float * 3), ("occ_sigma_threshold", C.c_float),
                 ("lr", C.c_float), ("beta1", C.c_float), ("beta2", C.c_float), ("eps", C.c_float),
-                ("sparse_table_adam", C.c_uint32), ("seed", C.c_uint64)]
+                ("sparse_table_adam", C.c_uint32), ("seed", C.c_uint64), ("occ_cascades", C.c_uint32)]
 
 
 class OrcBatch(C.Structure):
@@ -94,6 +94,12 @@ def lib(omp=False):
         L.orc_sample_batch.restype = None
         L.orc_occupancy_decay_update.argtypes = [C.POINTER(OrcConfig), _f64p, _f64p, C.c_uint32, C.c_uint32, C.c_double,
                                                  _u8p, _f64p]
+        L.orc_occupancy_stochastic_update.argtypes = [C.POINTER(OrcConfig), _f64p, _f64p, C.c_uint32, C.c_uint32, C.c_double,
+                                                      _u8p, _u64p, _f32p, _f64p]
+        L.orc_occupancy_cell.argtypes = [C.POINTER(OrcConfig), _f32p, _u32p]
+        L.orc_occupancy_cell.restype = C.c_uint64
+        L.orc_occupancy_cell_point.argtypes = [C.POINTER(OrcConfig), C.c_uint64, _f32p, _f32p]
+        L.orc_occupancy_cell_point.restype = None
         L.orc_pose_step.argtypes = [_f64p, _f64p, _f64p, _f64p, _u32p, _f64p, C.c_double, C.c_double, C.c_double,
                                     C.c_double, C.c_double]
         L.orc_pose_step.restype = None
@@ -118,7 +124,38 @@ def make_config(fc):
     c.bg[:] = [float(x) for x in fc.bg]
     for k in ("occ_sigma_threshold", "lr", "beta1", "beta2", "eps"):
         setattr(c, k, float(getattr(fc, k)))
+    c.occ_cascades = int(getattr(fc, "occ_cascades", 1))
     return c
+
+
+def n_occ_cells(fc):
+    """Cells of the occupancy structure: occ_cascades grids of occ_res^3 (F4 / R23)."""
+    return max(int(getattr(fc, "occ_cascades", 1)), 1) * int(fc.occ_res) ** 3
+
+
+def occupancy_cell(fc, x):
+    """R23: (bit index, cascade) of the occupancy cell that tests the normalised positions x [n,3]."""
+    c = make_config(fc)
+    x = np.ascontiguousarray(x, np.float32).reshape(-1, 3)
+    cell = np.empty(len(x), np.uint64)
+    casc = np.empty(len(x), np.uint32)
+    L, j = lib(), C.c_uint32()
+    for i in range(len(x)):
+        cell[i] = L.orc_occupancy_cell(C.byref(c), _p(x[i], _f32p), C.byref(j))
+        casc[i] = j.value
+    return cell, casc
+
+
+def occupancy_cell_point(fc, cells, u=None):
+    """The normalised positions of the points at offsets u [n,3] (default: the centres) inside the given cells."""
+    c = make_config(fc)
+    cells = np.asarray(cells, np.uint64).reshape(-1)
+    u = np.full((len(cells), 3), 0.5, np.float32) if u is None else np.ascontiguousarray(u, np.float32).reshape(-1, 3)
+    out = np.empty((len(cells), 3), np.float32)
+    L = lib()
+    for i in range(len(cells)):
+        L.orc_occupancy_cell_point(C.byref(c), int(cells[i]), _p(u[i], _f32p), _p(out[i], _f32p))
+    return out
 
 
 class _BatchHolder:
@@ -322,9 +359,9 @@ class Oracle:
         self.bits = None if bits is None else np.ascontiguousarray(bits, np.uint8).copy()
 
     def occupancy_from_field(self, want_sigma=False):
-        G = self.fc.occ_res
-        bits = np.zeros((G ** 3 + 7) // 8, np.uint8)
-        sig = np.zeros(G ** 3, np.float64) if want_sigma else None
+        n = n_occ_cells(self.fc)
+        bits = np.zeros((n + 7) // 8, np.uint8)
+        sig = np.zeros(n, np.float64) if want_sigma else None
         if self.lib.orc_occupancy_from_field(C.byref(self.cfg), _p(self.theta, _f64p),
                                              _p(bits, _u8p), _p(sig, _f64p)) != 0:
             raise ValueError("orc_occupancy_from_field failed")
@@ -335,17 +372,36 @@ class Oracle:
 
     def occupancy_decay_update(self, n_sub, decay, want_sigma=False):
         """F4: decayed running-maximum grid with a strided 1/n_sub refresh; keeps self.occ_grid and self.occ_updates."""
-        G = self.fc.occ_res
+        n = n_occ_cells(self.fc)
         if getattr(self, "occ_grid", None) is None:
-            self.occ_grid, self.occ_updates = np.zeros(G ** 3, np.float64), 0
-        bits = np.zeros((G ** 3 + 7) // 8, np.uint8)
-        vis = np.zeros(G ** 3, np.float64) if want_sigma else None
+            self.occ_grid, self.occ_updates = np.zeros(n, np.float64), 0
+        bits = np.zeros((n + 7) // 8, np.uint8)
+        vis = np.zeros(n, np.float64) if want_sigma else None
         if self.lib.orc_occupancy_decay_update(C.byref(self.cfg), _p(self.theta, _f64p), _p(self.occ_grid, _f64p),
                                                self.occ_updates, int(n_sub), float(decay), _p(bits, _u8p), _p(vis, _f64p)) != 0:
             raise ValueError("orc_occupancy_decay_update failed")
         self.occ_updates += 1
         self.bits = bits
         return (bits, vis) if want_sigma else bits
+
+    def occupancy_stochastic_update(self, n_draws, decay, want_draws=False):
+        """F4 (R25): decayed running-maximum grid refreshed at n_draws random points; self.occ_draws counts these updates
+        (it keys the draws and is never reset)."""
+        n = n_occ_cells(self.fc)
+        if getattr(self, "occ_grid", None) is None:
+            self.occ_grid, self.occ_updates = np.zeros(n, np.float64), 0
+        self.occ_draws = getattr(self, "occ_draws", 0)
+        bits = np.zeros((n + 7) // 8, np.uint8)
+        cells = np.zeros(n_draws, np.uint64) if want_draws else None
+        x = np.zeros((n_draws, 3), np.float32) if want_draws else None
+        sig = np.zeros(n_draws, np.float64) if want_draws else None
+        if self.lib.orc_occupancy_stochastic_update(C.byref(self.cfg), _p(self.theta, _f64p), _p(self.occ_grid, _f64p),
+                                                    self.occ_draws, int(n_draws), float(decay), _p(bits, _u8p),
+                                                    _p(cells, _u64p), _p(x, _f32p), _p(sig, _f64p)) != 0:
+            raise ValueError("orc_occupancy_stochastic_update failed")
+        self.occ_draws += 1
+        self.bits = bits
+        return (bits, cells, x, sig) if want_draws else bits
 
     def train_step(self, batch, lambda_d, jitter=True, apply_adam=True, trace=(), ):
         """trace: iterable of OrcTrace field names to return.  Returns (stats dict, trace dict)."""

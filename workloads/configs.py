@@ -45,6 +45,7 @@ class FieldConfig:
     seed: int = 0
     max_rays: int = 4096
     max_candidates: int = 128
+    occ_cascades: int = 1             # F4: nested occupancy grids (1 = the single grid of S2)
 
 
 @dataclass
