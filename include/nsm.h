@@ -36,7 +36,7 @@
  *       table parameter   theta[(offset_l + slot) * F + f]
  *       MLP matrices      row-major [out][in], in the order W_d1, W_d2, W_c1, (W_c2,) W_c3,
  *                         appended after the tables
- *       occupancy bit     i = gx + G*(gy + G*gz) is bit (i & 7) of byte (i >> 3)
+ *       occupancy bit     i = j*G^3 + gx + G*(gy + G*gz) is bit (i & 7) of byte (i >> 3); j = cascade (0 with one grid)
  *       samples           ordered by (ray, candidate k)
  */
 #ifndef NSM_H
@@ -84,6 +84,7 @@ typedef struct {
   uint32_t jitter;                   /* 1: per-(ray,bin) stratified jitter in training (S1) */
   uint64_t seed;                     /* jitter stream */
   uint32_t max_rays, max_candidates; /* workspace capacity per call / per render chunk */
+  uint32_t occ_cascades;             /* row f4: C nested occupancy grids of G^3 cells (0 or 1: one grid), C <= 8 */
 } nsm_field_config;
 
 typedef struct {
@@ -137,10 +138,10 @@ typedef enum {
 nsm_status nsm_create_field(const nsm_field_config *cfg, void *cuda_stream, nsm_field **out);
 void       nsm_destroy_field(nsm_field *f);
 
-/* S14.  SET: d_bits = G^3/8 bytes (device) in the canonical layout.  FULL: all ones.
+/* S14.  SET: d_bits = C*G^3/8 bytes (device) in the canonical layout (C = occ_cascades, 1 by default).  FULL: all ones.
  * FROM_FIELD: bit = sigma(cell centre) > occ_sigma_threshold from the current parameters. */
 nsm_status nsm_update_occupancy(nsm_field *f, nsm_occ_mode mode, const uint8_t *d_bits);
-/* Copy the current G^3/8 occupancy bytes to d_bits (device). */
+/* Copy the current C*G^3/8 occupancy bytes to d_bits (device). */
 nsm_status nsm_get_occupancy(nsm_field *f, uint8_t *d_bits);
 
 /* S1-S13: one training step of L_M (Eq. 3) on a ray batch: march, encode, MLPs, composite
@@ -168,7 +169,18 @@ nsm_status nsm_debug_timeline(nsm_field *f, uint64_t *h_out, uint64_t capacity_w
  * NSM_OCC_SET and NSM_OCC_FULL discard the running grid: until the next FROM_FIELD pass has seeded it again this call
  * fails with NSM_ERR_INVALID_ARG (a partial pass would cull every cell it does not visit). */
 nsm_status nsm_update_occupancy_decay(nsm_field *f, uint32_t n_subsets, float decay);
-/* The running density grid [G^3] (DEVICE output), for inspection and parity. */
+/* Stochastic variant ([17] refreshes a random subset of cells per update, each at a random point inside the cell;
+ * DESIGN.md 8e reading R25): every cell grid <- decay * grid; then for draw i < n_draws of update number u (u counts these
+ * calls since creation)   cell = (h(seed, u, i, 0xffff0003) * n_cells) >> 32,   offsets u_a = (h(seed, u, i, 0xffff0004 + a)
+ * >> 8) * 2^-24 inside the cell (h = the jitter hash of DESIGN.md S1),   grid[cell] <- max(grid[cell], sigma(point));
+ * bit = grid > occ_sigma_threshold.  A cell drawn twice keeps the larger density.  Needs a seeded grid like the call above. */
+nsm_status nsm_update_occupancy_stochastic(nsm_field *f, uint32_t n_draws, float decay);
+/* Nested occupancy cascades (config occ_cascades = C > 1; DESIGN.md 8e reading R23; the paper is silent, PAPER.md:266 asks
+ * for a map around "the region of interest"): C grids of G^3 cells share the centre of the field cube; in normalised
+ * coordinates cascade j (0 = finest) is the cube |x - 0.5|_max < 2^(j-C) and cascade C-1 the whole cube.  The marcher (S2)
+ * tests a candidate against the finest cascade that contains it; SET / nsm_get_occupancy move C*G^3/8 bytes (cascade-
+ * major), FROM_FIELD and the two partial refreshes evaluate the cells of all cascades. */
+/* The running density grid [C*G^3] (DEVICE output), for inspection and parity. */
 nsm_status nsm_get_occupancy_grid(nsm_field *f, float *d_grid);
 
 /* ---- Row F1: keyframe store and ray-batch sampler (the mapping thread optimises over all

@@ -31,7 +31,7 @@ EXPORTS = ["nsm_create_field", "nsm_destroy_field", "nsm_update_occupancy", "nsm
            "nsm_get_level_table", "nsm_debug_last_step", "nsm_total_samples", "nsm_profile", "nsm_set_option", "nsm_debug_timeline",
            "nsm_add_keyframe", "nsm_keyframe_count", "nsm_sample_batch", "nsm_train_step_sampled",
            "nsm_pose_gradients", "nsm_keyframe_pose_gradients", "nsm_apply_pose_step", "nsm_get_keyframe_pose",
-           "nsm_update_occupancy_decay", "nsm_get_occupancy_grid",
+           "nsm_update_occupancy_decay", "nsm_update_occupancy_stochastic", "nsm_get_occupancy_grid",
            "nsm_profile_read", "nsm_launch_count", "nsm_mlp_path",
            "nsm_last_error", "nsm_version"]
 
@@ -46,7 +46,7 @@ class NsmFieldConfig(C.Structure):
                 ("occ_sigma_threshold", C.c_float), ("lr", C.c_float), ("beta1", C.c_float),
                 ("beta2", C.c_float), ("eps", C.c_float), ("sparse_table_adam", C.c_uint32),
                 ("jitter", C.c_uint32), ("seed", C.c_uint64), ("max_rays", C.c_uint32),
-                ("max_candidates", C.c_uint32)]
+                ("max_candidates", C.c_uint32), ("occ_cascades", C.c_uint32)]
 
 
 class NsmRayBatch(C.Structure):
@@ -105,6 +105,7 @@ def load_library():
         L.nsm_pose_gradients.argtypes = [vp, vp, vp]
         L.nsm_keyframe_pose_gradients.argtypes = [vp, vp]
         L.nsm_update_occupancy_decay.argtypes = [vp, C.c_uint32, C.c_float]
+        L.nsm_update_occupancy_stochastic.argtypes = [vp, C.c_uint32, C.c_float]
         L.nsm_get_occupancy_grid.argtypes = [vp, vp]
         L.nsm_apply_pose_step.argtypes = [vp, C.c_float, C.c_float]
         L.nsm_get_keyframe_pose.argtypes = [vp, C.c_uint32, C.POINTER(C.c_float), C.POINTER(C.c_float)]
@@ -139,6 +140,7 @@ def make_config(fc):
               "mlp_precision", "sparse_table_adam", "seed", "max_rays", "max_candidates"):
         setattr(c, k, int(getattr(fc, k)))
     c.jitter = int(getattr(fc, "jitter", 1))
+    c.occ_cascades = int(getattr(fc, "occ_cascades", 1))
     c.bg[:] = [float(x) for x in fc.bg]
     for k in ("occ_sigma_threshold", "lr", "beta1", "beta2", "eps"):
         setattr(c, k, float(getattr(fc, k)))
@@ -275,18 +277,23 @@ class Field:
         return th.cpu().numpy(), m.cpu().numpy(), v.cpu().numpy(), step.value
 
     # ---- occupancy
+    @property
+    def n_occ_cells(self):
+        """occ_cascades nested grids of occ_res^3 cells (marshalling: buffer sizes only)"""
+        return max(int(getattr(self.fc, "occ_cascades", 1)), 1) * int(self.fc.occ_res) ** 3
+
     def nsm_update_occupancy(self, mode, bits=None, sync=True):
         d = None
         if bits is not None:
             d = torch.as_tensor(np.ascontiguousarray(bits, np.uint8)).to(self.device)
-            assert d.numel() == (self.fc.occ_res ** 3 + 7) // 8
+            assert d.numel() == (self.n_occ_cells + 7) // 8
             sync = True     # the staging tensor must outlive the copy
         _check(self.lib.nsm_update_occupancy(self.h, int(mode), _dev_ptr(d, torch.uint8)))
         if sync:
             torch.cuda.synchronize(self.device)
 
     def nsm_get_occupancy(self):
-        d = torch.empty((self.fc.occ_res ** 3 + 7) // 8, dtype=torch.uint8, device=self.device)
+        d = torch.empty((self.n_occ_cells + 7) // 8, dtype=torch.uint8, device=self.device)
         _check(self.lib.nsm_get_occupancy(self.h, _dev_ptr(d, torch.uint8)))
         torch.cuda.synchronize(self.device)
         return d.cpu().numpy()
@@ -362,9 +369,13 @@ class Field:
         if sync:
             torch.cuda.synchronize(self.device)
 
+    def nsm_update_occupancy_stochastic(self, n_draws, decay, sync=True):
+        _check(self.lib.nsm_update_occupancy_stochastic(self.h, int(n_draws), float(decay)))
+        if sync:
+            torch.cuda.synchronize(self.device)
+
     def nsm_get_occupancy_grid(self):
-        G = self.fc.occ_res
-        out = torch.empty(G ** 3, device=self.device)
+        out = torch.empty(self.n_occ_cells, device=self.device)
         _check(self.lib.nsm_get_occupancy_grid(self.h, out.data_ptr()))
         return out.cpu().numpy()
 

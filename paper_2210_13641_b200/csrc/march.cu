@@ -15,6 +15,55 @@ __device__ __forceinline__ float jitter_u(uint32_t h_seed_step_ray, uint32_t k, 
   return __uint2float_rn(h >> 8) * 0x1p-24f;  // 24-bit integer, exact
 }
 
+// 2^e as a float, e in [-126, 127] (exact)
+__device__ __forceinline__ float pow2f(int e) { return __int_as_float((127 + e) << 23); }
+
+// S2 / F4 (reading R23): bit index of the occupancy cell that tests the normalised position x in [0,1)^3.
+// C nested grids of G^3 cells share the cube's centre; cascade j (0 = finest) is the cube |x - 0.5|_max < 2^(j-C),
+// cascade C-1 the whole cube; a point belongs to the finest cascade that contains it.  Index path: explicit fp32 ops.
+__device__ __forceinline__ uint64_t occ_cell(uint32_t G, uint32_t C, const float x[3]) {
+  uint32_t j = C - 1;
+  float xp[3] = {x[0], x[1], x[2]};
+  if (C > 1) {
+    float q[3], m = 0.0f;
+#pragma unroll
+    for (int a = 0; a < 3; ++a) {
+      q[a] = __fsub_rn(x[a], 0.5f);
+      m = fmaxf(m, fabsf(q[a]));
+    }
+    for (j = 0; j + 1 < C; ++j)
+      if (m < pow2f((int)j - (int)C)) break;
+    if (j + 1 < C) {
+      const float s = pow2f((int)(C - 1 - j));
+#pragma unroll
+      for (int a = 0; a < 3; ++a) xp[a] = __fmaf_rn(q[a], s, 0.5f);
+    }
+  }
+  uint32_t g[3];
+  const float Gf = __uint2float_rn(G);
+#pragma unroll
+  for (int a = 0; a < 3; ++a) {
+    int gi = __float2int_rd(__fmul_rn(xp[a], Gf));
+    g[a] = (uint32_t)max(min(gi, (int)G - 1), 0);
+  }
+  return (uint64_t)j * G * G * G + (uint64_t)g[0] + (uint64_t)G * ((uint64_t)g[1] + (uint64_t)G * g[2]);
+}
+
+// the inverse: the point at offsets u in [0,1)^3 inside cell `cell` (u = 0.5: the centre, exact for power-of-two G)
+__device__ __forceinline__ void occ_cell_point(uint32_t G, uint32_t C, uint64_t cell, const float u[3], float x[3]) {
+  const uint64_t G3 = (uint64_t)G * G * G;
+  const uint32_t j = (uint32_t)(cell / G3);
+  const uint64_t loc = cell - (uint64_t)j * G3;
+  const uint32_t g[3] = {(uint32_t)(loc % G), (uint32_t)((loc / G) % G), (uint32_t)(loc / ((uint64_t)G * G))};
+  const float Gf = __uint2float_rn(G);
+#pragma unroll
+  for (int a = 0; a < 3; ++a) {
+    float xp = __fdiv_rn(__fadd_rn(__uint2float_rn(g[a]), u[a]), Gf);
+    if (j + 1 < C) xp = __fmaf_rn(__fsub_rn(xp, 0.5f), pow2f((int)j - (int)(C - 1)), 0.5f);
+    x[a] = xp;
+  }
+}
+
 struct Candidate {
   float t, delta, x[3];
   bool live;
@@ -43,14 +92,7 @@ __device__ __forceinline__ Candidate make_candidate(const MarchParams &mp, const
   }
   c.live = false;
   if (inside) {
-    uint32_t g[3];
-    const float Gf = __uint2float_rn(mp.G);
-#pragma unroll
-    for (int a = 0; a < 3; ++a) {
-      int gi = __float2int_rd(__fmul_rn(c.x[a], Gf));
-      g[a] = (uint32_t)min(gi, (int)mp.G - 1);
-    }
-    uint64_t cell = (uint64_t)g[0] + (uint64_t)mp.G * ((uint64_t)g[1] + (uint64_t)mp.G * g[2]);
+    const uint64_t cell = occ_cell(mp.G, mp.C, c.x);
     c.live = bits ? ((__ldg(bits + (cell >> 3)) >> (cell & 7)) & 1u) : true;
   }
   return c;
@@ -204,19 +246,50 @@ __global__ void __launch_bounds__(MARCH_WARPS * 32) march_fused_kernel(MarchPara
   tl_mark(ws.timeline, K_MARCH, 1);
 }
 
-// S14 FROM_FIELD: the cell centres of a chunk of the occupancy grid as "samples".
-__global__ void occ_cells_kernel(uint32_t G, uint64_t first_cell, uint64_t n_cells, Workspace ws,
+// S14 FROM_FIELD / F4: the centres of the cells first_cell + i * stride (i < n_cells) of the occupancy structure (all
+// cascades, global cell index) as "samples".
+__global__ void occ_cells_kernel(uint32_t G, uint32_t C, uint64_t first_cell, uint32_t stride, uint64_t n_cells, Workspace ws,
                                  uint32_t *d_S) {
   uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (i == 0) *d_S = (uint32_t)n_cells;
   if (i >= n_cells) return;
-  uint64_t cell = first_cell + i;
-  uint32_t gx = (uint32_t)(cell % G), gy = (uint32_t)((cell / G) % G), gz = (uint32_t)(cell / ((uint64_t)G * G));
-  const float Gf = __uint2float_rn(G);
-  ws.s_x[i] = __fdiv_rn(__fadd_rn(__uint2float_rn(gx), 0.5f), Gf);  // exact for power-of-two G
-  ws.s_x[ws.cap + i] = __fdiv_rn(__fadd_rn(__uint2float_rn(gy), 0.5f), Gf);
-  ws.s_x[2 * ws.cap + i] = __fdiv_rn(__fadd_rn(__uint2float_rn(gz), 0.5f), Gf);
+  const float half[3] = {0.5f, 0.5f, 0.5f};
+  float x[3];
+  occ_cell_point(G, C, first_cell + i * stride, half, x);
+  ws.s_x[i] = x[0];
+  ws.s_x[ws.cap + i] = x[1];
+  ws.s_x[2 * ws.cap + i] = x[2];
   ws.s_ray[i] = 0;
+}
+
+// F4, stochastic refresh (reading R25): draw i of update `upd` picks cell (h(seed, upd, i, 0xffff0003) * n_total) >> 32 and
+// the point at offsets u_a = (h(seed, upd, i, 0xffff0004 + a) >> 8) 2^-24 inside it; the cell index is kept in ws.s_k.
+__global__ void occ_cells_stochastic_kernel(uint32_t G, uint32_t C, uint64_t seed, uint32_t upd, uint32_t first_draw,
+                                            uint32_t n_draws, Workspace ws, uint32_t *d_S) {
+  uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i == 0) *d_S = n_draws;
+  if (i >= n_draws) return;
+  const uint64_t n_total = (uint64_t)C * G * G * G;
+  const uint32_t hpre = nsm_hash_prefix(seed, upd, first_draw + i);
+  const uint64_t cell = ((uint64_t)nsm_mix32(hpre ^ 0xffff0003u) * n_total) >> 32;
+  float u[3], x[3];
+#pragma unroll
+  for (uint32_t a = 0; a < 3; ++a) u[a] = __uint2float_rn(nsm_mix32(hpre ^ (0xffff0004u + a)) >> 8) * 0x1p-24f;
+  occ_cell_point(G, C, cell, u, x);
+  ws.s_x[i] = x[0];
+  ws.s_x[ws.cap + i] = x[1];
+  ws.s_x[2 * ws.cap + i] = x[2];
+  ws.s_ray[i] = 0;
+  ws.s_k[i] = (uint32_t)cell;
+}
+
+// grid[cell_i] <- max(grid[cell_i], sigma_i); a cell drawn twice keeps the larger density (order-free): densities and
+// grid values are non-negative, so the integer maximum of their bit patterns is the float maximum
+__global__ void occ_max_cells_kernel(float *__restrict__ grid, const uint32_t *__restrict__ cells, uint32_t n,
+                                     const float *__restrict__ sigma) {
+  uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  atomicMax(reinterpret_cast<int *>(grid + cells[i]), __float_as_int(fmaxf(sigma[i], 0.0f)));
 }
 
 // bit = sigma > thr; one warp packs 32 cells into one word (first_cell is a multiple of 32).  The densities also
@@ -233,20 +306,6 @@ __global__ void occ_threshold_kernel(uint64_t first_cell, uint64_t n_cells,
 // ---- F4 (row f4; paper silent, after [17]): decayed running maximum of the density with a strided partial refresh ----
 //   every cell: grid <- decay * grid;   cells c = c0 + j * n_sub (c0 = update index mod n_sub): grid <- max(grid, sigma(c));
 //   bit = grid > thr.   n_sub consecutive updates visit every cell exactly once.
-__global__ void occ_cells_strided_kernel(uint32_t G, uint64_t first_cell, uint32_t stride, uint64_t n_cells, Workspace ws,
-                                         uint32_t *d_S) {
-  uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
-  if (i == 0) *d_S = (uint32_t)n_cells;
-  if (i >= n_cells) return;
-  uint64_t cell = first_cell + i * stride;
-  uint32_t gx = (uint32_t)(cell % G), gy = (uint32_t)((cell / G) % G), gz = (uint32_t)(cell / ((uint64_t)G * G));
-  const float Gf = __uint2float_rn(G);
-  ws.s_x[i] = __fdiv_rn(__fadd_rn(__uint2float_rn(gx), 0.5f), Gf);
-  ws.s_x[ws.cap + i] = __fdiv_rn(__fadd_rn(__uint2float_rn(gy), 0.5f), Gf);
-  ws.s_x[2 * ws.cap + i] = __fdiv_rn(__fadd_rn(__uint2float_rn(gz), 0.5f), Gf);
-  ws.s_ray[i] = 0;
-}
-
 __global__ void occ_decay_kernel(float *__restrict__ grid, uint64_t n_cells, float decay) {
   for (uint64_t c = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; c < n_cells; c += (uint64_t)gridDim.x * blockDim.x)
     grid[c] *= decay;
@@ -278,9 +337,20 @@ int launch_march(const MarchParams &mp, const uint8_t *bits, const float *origin
 
 uint32_t march_scan_state_entries(uint32_t max_rays) { return (max_rays + MARCH_WARPS - 1) / MARCH_WARPS; }
 
-int launch_occ_cells(uint32_t G, uint64_t first_cell, uint64_t n_cells, const Workspace &ws,
+int launch_occ_cells(uint32_t G, uint32_t C, uint64_t first_cell, uint32_t stride, uint64_t n_cells, const Workspace &ws,
                      uint32_t *d_S, cudaStream_t st) {
-  occ_cells_kernel<<<(unsigned)((n_cells + 255) / 256), 256, 0, st>>>(G, first_cell, n_cells, ws, d_S);
+  occ_cells_kernel<<<(unsigned)((n_cells + 255) / 256), 256, 0, st>>>(G, C, first_cell, stride, n_cells, ws, d_S);
+  return 1;
+}
+
+int launch_occ_cells_stochastic(uint32_t G, uint32_t C, uint64_t seed, uint32_t upd, uint32_t first_draw, uint32_t n_draws,
+                                const Workspace &ws, uint32_t *d_S, cudaStream_t st) {
+  occ_cells_stochastic_kernel<<<(n_draws + 255) / 256, 256, 0, st>>>(G, C, seed, upd, first_draw, n_draws, ws, d_S);
+  return 1;
+}
+
+int launch_occ_max_cells(float *grid, const uint32_t *cells, uint32_t n, const float *sigma, cudaStream_t st) {
+  occ_max_cells_kernel<<<(n + 255) / 256, 256, 0, st>>>(grid, cells, n, sigma);
   return 1;
 }
 
@@ -289,12 +359,6 @@ int launch_occ_threshold(uint32_t G, uint64_t first_cell, uint64_t n_cells, cons
   (void)G;
   occ_threshold_kernel<<<(unsigned)((n_cells + 255) / 256), 256, 0, st>>>(first_cell, n_cells, sigma, thr,
                                                                          (uint32_t *)bits, grid);
-  return 1;
-}
-
-int launch_occ_cells_strided(uint32_t G, uint64_t first_cell, uint32_t stride, uint64_t n_cells, const Workspace &ws, uint32_t *d_S,
-                             cudaStream_t st) {
-  occ_cells_strided_kernel<<<(unsigned)((n_cells + 255) / 256), 256, 0, st>>>(G, first_cell, stride, n_cells, ws, d_S);
   return 1;
 }
 

@@ -91,6 +91,7 @@ struct nsm_field {
   uint32_t work_seq = 0;      // launch sequence number of the table kernels (ChunkQueue counter ring)
   bool occ_full = true;
   uint32_t occ_updates = 0;   // F4: decayed partial refreshes since the last full one
+  uint32_t occ_draws = 0;     // F4: stochastic refreshes since creation (keys their draws; never reset)
   bool grid_seeded = false;   // F4: the running density grid holds a full FROM_FIELD pass (SET / FULL invalidate it)
   bool grads_dirty = false;
   // state of the last step, for the debug getter
@@ -180,6 +181,9 @@ nsm_status validate_config(const nsm_field_config *c) {
   if (c->n_min < 1 || c->n_max < c->n_min || c->n_max > (1u << 20)) return fail(NSM_ERR_INVALID_ARG, "bad n_min/n_max");
   if (c->occ_res < 1 || (c->occ_res & (c->occ_res - 1)) || c->occ_res > 1024)
     return fail(NSM_ERR_INVALID_ARG, "occ_res must be a power of two <= 1024");
+  if (c->occ_cascades > 8) return fail(NSM_ERR_INVALID_ARG, "occ_cascades must be <= 8");
+  if ((uint64_t)(c->occ_cascades ? c->occ_cascades : 1) * c->occ_res * c->occ_res * c->occ_res > (1ull << 31))
+    return fail(NSM_ERR_INVALID_ARG, "occ_cascades * occ_res^3 exceeds 2^31 cells");
   if (c->density_hidden < 1 || c->density_hidden > 128 || c->density_out < 1 || c->density_out > 16)
     return fail(NSM_ERR_INVALID_ARG, "density MLP widths out of range");
   if (c->geo_offset + c->geo_count > c->density_out) return fail(NSM_ERR_INVALID_ARG, "geo slice exceeds density_out");
@@ -251,6 +255,10 @@ cudaError_t leave_fast_path(nsm_field *f) {
 }
 #define LEAVE_FAST_PATH(f) CUDA_TRY(leave_fast_path(f))
 
+// cells of the occupancy structure: occ_cascades nested grids of occ_res^3 (F4, reading R23)
+uint32_t occ_cascades(const nsm_field *f) { return f->cfg.occ_cascades ? f->cfg.occ_cascades : 1u; }
+uint64_t occ_cells(const nsm_field *f) { return (uint64_t)occ_cascades(f) * f->cfg.occ_res * f->cfg.occ_res * f->cfg.occ_res; }
+
 MarchParams make_march(const nsm_field *f, const nsm_ray_batch *b, uint32_t R, bool jitter, uint32_t step) {
   MarchParams mp;
   for (int a = 0; a < 3; ++a) mp.aabb_min[a] = f->cfg.aabb_min[a];
@@ -259,6 +267,7 @@ MarchParams make_march(const nsm_field *f, const nsm_ray_batch *b, uint32_t R, b
   mp.dt = (b->t_max - b->t_min) / (float)b->n_candidates;        // one fp32 subtract, one fp32 divide
   mp.K = b->n_candidates;
   mp.G = f->cfg.occ_res;
+  mp.C = f->cfg.occ_cascades ? f->cfg.occ_cascades : 1u;
   mp.jitter = jitter ? 1u : 0u;
   mp.step = step;
   mp.seed = f->cfg.seed;
@@ -528,7 +537,7 @@ nsm_status nsm_create_field(const nsm_field_config *cfg, void *cuda_stream, nsm_
   const uint64_t cap = (((uint64_t)cfg->max_rays * cfg->max_candidates + NSM_TILE - 1) / NSM_TILE) * NSM_TILE;
   ws.cap = cap;
   ws.max_rays = cfg->max_rays;
-  const uint64_t G3 = (uint64_t)cfg->occ_res * cfg->occ_res * cfg->occ_res;
+  const uint64_t G3 = (uint64_t)(cfg->occ_cascades ? cfg->occ_cascades : 1) * cfg->occ_res * cfg->occ_res * cfg->occ_res;   // all cascades
   const uint32_t R = cfg->max_rays;
   cudaError_t e = cudaSuccess;
   auto A = [&](cudaError_t r) { if (e == cudaSuccess) e = r; };
@@ -684,7 +693,7 @@ nsm_status nsm_set_params(nsm_field *f, const float *d_theta, const float *d_m, 
 nsm_status nsm_get_occupancy(nsm_field *f, uint8_t *d_bits) {
   if (!f || !d_bits) return fail(NSM_ERR_INVALID_ARG, "NULL argument");
   LEAVE_FAST_PATH(f);
-  const uint64_t G3 = (uint64_t)f->cfg.occ_res * f->cfg.occ_res * f->cfg.occ_res;
+  const uint64_t G3 = occ_cells(f);
   if (f->occ_full) CUDA_TRY(cudaMemsetAsync(d_bits, 0xff, (G3 + 7) / 8, f->stream));
   else CUDA_TRY(cudaMemcpyAsync(d_bits, f->fp.occ_bits, (G3 + 7) / 8, cudaMemcpyDeviceToDevice, f->stream));
   return NSM_OK;
@@ -693,7 +702,7 @@ nsm_status nsm_get_occupancy(nsm_field *f, uint8_t *d_bits) {
 nsm_status nsm_update_occupancy(nsm_field *f, nsm_occ_mode mode, const uint8_t *d_bits) {
   if (!f) return fail(NSM_ERR_INVALID_ARG, "field is NULL");
   LEAVE_FAST_PATH(f);
-  const uint64_t G3 = (uint64_t)f->cfg.occ_res * f->cfg.occ_res * f->cfg.occ_res;
+  const uint64_t G3 = occ_cells(f);
   switch (mode) {
     case NSM_OCC_FULL:
       f->occ_full = true;
@@ -713,7 +722,7 @@ nsm_status nsm_update_occupancy(nsm_field *f, nsm_occ_mode mode, const uint8_t *
       uint32_t *d_S = f->ws.offsets;  // offsets[0] doubles as the chunk's sample count
       for (uint64_t first = 0; first < G3; first += chunk) {
         const uint64_t n = (G3 - first < chunk) ? G3 - first : chunk;
-        RUN(f, K_OCC, launch_occ_cells(f->cfg.occ_res, first, n, f->ws, d_S, f->stream));
+        RUN(f, K_OCC, launch_occ_cells(f->cfg.occ_res, occ_cascades(f), first, 1, n, f->ws, d_S, f->stream));
         RUN(f, K_ENCODE, launch_encode(f->lv, f->fp.theta, f->ws, d_S, f->use_tc ? 1 + (f->cfg.mlp_precision == NSM_MLP_BF16) : 0,
                                        f->n_sms, f->stream, f->work_seq++));
         if (f->use_tc)
@@ -742,7 +751,7 @@ nsm_status nsm_update_occupancy_decay(nsm_field *f, uint32_t n_subsets, float de
   if (!f->grid_seeded)   // after SET / FULL the running grid says nothing about the cells a partial pass does not visit
     return fail(NSM_ERR_INVALID_ARG, "the running density grid is not seeded: call nsm_update_occupancy(NSM_OCC_FROM_FIELD) first");
   LEAVE_FAST_PATH(f);
-  const uint64_t G3 = (uint64_t)f->cfg.occ_res * f->cfg.occ_res * f->cfg.occ_res;
+  const uint64_t G3 = occ_cells(f);
   const uint64_t c0 = f->occ_updates % n_subsets;
   const uint64_t n_vis = c0 < G3 ? (G3 - c0 + n_subsets - 1) / n_subsets : 0;
   const uint64_t chunk = f->ws.cap & ~uint64_t(31);
@@ -752,7 +761,7 @@ nsm_status nsm_update_occupancy_decay(nsm_field *f, uint32_t n_subsets, float de
   for (uint64_t j0 = 0; j0 < n_vis; j0 += chunk) {
     const uint64_t n = (n_vis - j0 < chunk) ? n_vis - j0 : chunk;
     const uint64_t first = c0 + j0 * n_subsets;
-    RUN(f, K_OCC, launch_occ_cells_strided(f->cfg.occ_res, first, n_subsets, n, f->ws, d_S, f->stream));
+    RUN(f, K_OCC, launch_occ_cells(f->cfg.occ_res, occ_cascades(f), first, n_subsets, n, f->ws, d_S, f->stream));
     RUN(f, K_ENCODE, launch_encode(f->lv, f->fp.theta, f->ws, d_S, f->use_tc ? 1 + bf16 : 0, f->n_sms, f->stream, f->work_seq++));
     if (f->use_tc)
       RUN(f, K_MLP_FWD, launch_mlp_forward_tc(f->ms, bf16, nullptr, f->ws, d_S, 1, 0, f->n_sms, f->stream));
@@ -767,10 +776,39 @@ nsm_status nsm_update_occupancy_decay(nsm_field *f, uint32_t n_subsets, float de
   return NSM_OK;
 }
 
+// F4, stochastic variant (reading R25): decayed running maximum refreshed at n_draws hashed random points
+nsm_status nsm_update_occupancy_stochastic(nsm_field *f, uint32_t n_draws, float decay) {
+  if (!f) return fail(NSM_ERR_INVALID_ARG, "field is NULL");
+  if (!(decay >= 0.f && decay <= 1.f)) return fail(NSM_ERR_INVALID_ARG, "decay must be in [0, 1]");
+  if (!f->grid_seeded)
+    return fail(NSM_ERR_INVALID_ARG, "the running density grid is not seeded: call nsm_update_occupancy(NSM_OCC_FROM_FIELD) first");
+  LEAVE_FAST_PATH(f);
+  const uint64_t G3 = occ_cells(f);
+  const uint32_t chunk = (uint32_t)std::min<uint64_t>(f->ws.cap & ~uint64_t(31), 1u << 30);
+  const int bf16 = f->cfg.mlp_precision == NSM_MLP_BF16;
+  uint32_t *d_S = f->ws.offsets;
+  RUN(f, K_OCC, launch_occ_decay(f->fp.occ_grid, G3, decay, f->stream));
+  for (uint32_t i0 = 0; i0 < n_draws; i0 += chunk) {
+    const uint32_t n = n_draws - i0 < chunk ? n_draws - i0 : chunk;
+    RUN(f, K_OCC, launch_occ_cells_stochastic(f->cfg.occ_res, occ_cascades(f), f->cfg.seed, f->occ_draws, i0, n, f->ws, d_S, f->stream));
+    RUN(f, K_ENCODE, launch_encode(f->lv, f->fp.theta, f->ws, d_S, f->use_tc ? 1 + bf16 : 0, f->n_sms, f->stream, f->work_seq++));
+    if (f->use_tc)
+      RUN(f, K_MLP_FWD, launch_mlp_forward_tc(f->ms, bf16, nullptr, f->ws, d_S, 1, 0, f->n_sms, f->stream));
+    else
+      RUN(f, K_MLP_FWD, launch_mlp_forward_simt(f->ms, f->fp.mlp_theta, nullptr, f->ws, d_S, 1, f->n_sms, f->stream));
+    RUN(f, K_OCC, launch_occ_max_cells(f->fp.occ_grid, f->ws.s_k, n, f->ws.sigma, f->stream));
+  }
+  RUN(f, K_OCC, launch_occ_bits_from_grid(f->fp.occ_grid, G3, f->cfg.occ_sigma_threshold, f->fp.occ_bits, f->stream));
+  f->occ_full = false;
+  f->occ_draws += 1;
+  CUDA_TRY(cudaGetLastError());
+  return NSM_OK;
+}
+
 nsm_status nsm_get_occupancy_grid(nsm_field *f, float *d_grid) {
   if (!f || !d_grid) return fail(NSM_ERR_INVALID_ARG, "NULL argument");
   LEAVE_FAST_PATH(f);
-  const uint64_t G3 = (uint64_t)f->cfg.occ_res * f->cfg.occ_res * f->cfg.occ_res;
+  const uint64_t G3 = occ_cells(f);
   CUDA_TRY(cudaMemcpyAsync(d_grid, f->fp.occ_grid, sizeof(float) * G3, cudaMemcpyDeviceToDevice, f->stream));
   return NSM_OK;
 }

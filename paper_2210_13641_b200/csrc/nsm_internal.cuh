@@ -28,7 +28,7 @@ struct MlpShape {
 struct MarchParams {
   float aabb_min[3], inv_extent;
   float t_min, dt;
-  uint32_t K, G, jitter, step;
+  uint32_t K, G, C, jitter, step;   // C: occupancy cascades (F4)
   uint64_t seed;
   uint32_t R;
 };
@@ -344,13 +344,16 @@ int launch_pose_gradients(const LevelTable &lv, const float *theta, const Worksp
 // f2, the update: Adam + exponential map on the keyframes that received rays (kf_grad: [n_kf][NSM_KF_GRAD_STRIDE])
 int launch_pose_step(KeyframeDev *kfs, uint32_t n_kf, const float *kf_grad, float *pm, float *pv, uint32_t *pcnt, float lr_t,
                      float lr_r, float beta1, float beta2, float eps, cudaStream_t st);
-int launch_occ_cells(uint32_t G, uint64_t first_cell, uint64_t n_cells, const Workspace &ws,
+// the centres of cells first_cell + i * stride, i < n_cells (global cell index over the C cascades), as samples
+int launch_occ_cells(uint32_t G, uint32_t C, uint64_t first_cell, uint32_t stride, uint64_t n_cells, const Workspace &ws,
                      uint32_t *d_S, cudaStream_t st);
+// F4 stochastic refresh: draws first_draw .. first_draw + n_draws of update `upd` as samples; their cells in ws.s_k
+int launch_occ_cells_stochastic(uint32_t G, uint32_t C, uint64_t seed, uint32_t upd, uint32_t first_draw, uint32_t n_draws,
+                                const Workspace &ws, uint32_t *d_S, cudaStream_t st);
+int launch_occ_max_cells(float *grid, const uint32_t *cells, uint32_t n, const float *sigma, cudaStream_t st);
 int launch_occ_threshold(uint32_t G, uint64_t first_cell, uint64_t n_cells, const float *sigma,
                          float thr, uint8_t *bits, float *grid, cudaStream_t st);
 // F4: decayed running-maximum density grid with a strided partial refresh
-int launch_occ_cells_strided(uint32_t G, uint64_t first_cell, uint32_t stride, uint64_t n_cells, const Workspace &ws, uint32_t *d_S,
-                             cudaStream_t st);
 int launch_occ_decay(float *grid, uint64_t n_cells, float decay, cudaStream_t st);
 int launch_occ_max_visited(float *grid, uint64_t first_cell, uint32_t stride, uint64_t n_visited, const float *sigma, cudaStream_t st);
 int launch_occ_bits_from_grid(const float *grid, uint64_t n_cells, float thr, uint8_t *bits, cudaStream_t st);
