@@ -156,14 +156,16 @@ __global__ void __launch_bounds__(128) adam_pack_kernel(MlpShape ms, float *__re
   tl_mark(tl, K_ADAM_MLP, 1);
 }
 
-// issue the k-steps of one layer: D[128 x N] = A[128 x K] * B[N x K]^T, both K-major
+// issue the k-steps of one layer: D[128 x N] = A[128 x K] * B[N x K]^T, both K-major.  The descriptors of consecutive
+// k-steps differ in their 14-bit address field only (two 8-column panels further): one add per operand and MMA.
 __device__ __forceinline__ void issue_layer(uint32_t tmem_d, uint32_t a_saddr, uint32_t b_saddr, uint32_t K, uint32_t N,
                                             uint32_t NP, uint32_t fmt, uint32_t bar_saddr) {
   const uint32_t idesc = make_idesc(fmt, 128, N, 0, 0);
+  uint64_t da = make_desc(a_saddr, PANEL, 128), db = make_desc(b_saddr, NP * 16, 128);
+  const uint64_t sa = (2 * PANEL) >> 4, sb = (2 * NP * 16) >> 4;
   for (uint32_t k = 0; k < K / 16; ++k) {
-    const uint64_t da = make_desc(a_saddr + k * 2 * PANEL, PANEL, 128);
-    const uint64_t db = make_desc(b_saddr + k * 2 * NP * 16, NP * 16, 128);
     mma_ss(tmem_d, da, db, idesc, k > 0);
+    da += sa; db += sb;
   }
   mma_commit(bar_saddr);
 }
@@ -173,13 +175,14 @@ __device__ __forceinline__ void issue_layer_split(uint32_t tmem_d, uint32_t a_sa
                                                   uint32_t b_lo, uint32_t K, uint32_t N, uint32_t NP, uint32_t fmt,
                                                   uint32_t bar_saddr) {
   const uint32_t idesc = make_idesc(fmt, 128, N, 0, 0);
-#pragma unroll 1
+  const uint64_t da0 = make_desc(a_saddr, PANEL, 128), db0 = make_desc(b_saddr, NP * 16, 128);
+  const uint64_t sa = (2 * PANEL) >> 4, sb = (2 * NP * 16) >> 4;
+#pragma unroll
   for (uint32_t term = 0; term < 3; ++term) {
-    const uint32_t a = a_saddr + (term == 1 ? a_lo : 0u), b = b_saddr + (term == 2 ? b_lo : 0u);
+    uint64_t da = da0 + (term == 1 ? (uint64_t)(a_lo >> 4) : 0ull), db = db0 + (term == 2 ? (uint64_t)(b_lo >> 4) : 0ull);
     for (uint32_t k = 0; k < K / 16; ++k) {
-      const uint64_t da = make_desc(a + k * 2 * PANEL, PANEL, 128);
-      const uint64_t db = make_desc(b + k * 2 * NP * 16, NP * 16, 128);
       mma_ss(tmem_d, da, db, idesc, (term | k) > 0);
+      da += sa; db += sb;
     }
   }
   mma_commit(bar_saddr);
@@ -227,19 +230,16 @@ template <typename T, bool RELU>
 __device__ __forceinline__ void emit16s(float *v, uint8_t *smem_tile, uint32_t lo_off, uint8_t *blob_tile, uint32_t row,
                                         uint32_t c0, bool valid) {
   if (RELU) {
+    // fp16 rounds 0 < h < 2^-25 to zero; the backward pass reads its ReLU mask off the stored value (h > 0), so a positive
+    // activation is raised to at least the smallest fp16 subnormal, 2^-24: the mask is then exactly [pre-activation > 0]
+    constexpr float tiny = Fmt<T>::id == 0 ? 5.9604644775390625e-08f : 0.f;
 #pragma unroll
-    for (int j = 0; j < 16; ++j) v[j] = fmaxf(v[j], 0.f);
+    for (int j = 0; j < 16; ++j) v[j] = v[j] > 0.f ? fmaxf(v[j], tiny) : 0.f;
   }
   uint32_t hi[8], lo[8];
 #pragma unroll
   for (int j = 0; j < 8; ++j) {
     hi[j] = pack2<T>(v[2 * j], v[2 * j + 1]);
-    if (RELU && Fmt<T>::id == 0) {
-      // fp16 flushes 0 < h < 2^-25 to zero; the backward pass reads its ReLU mask off this stored value (h > 0), so a
-      // positive activation is stored as at least the smallest subnormal: the mask is then exactly [pre-activation > 0]
-      if (v[2 * j] > 0.f && (hi[j] & 0xffffu) == 0u) hi[j] |= 1u;
-      if (v[2 * j + 1] > 0.f && (hi[j] >> 16) == 0u) hi[j] |= 0x10000u;
-    }
     const float2 h = unpack2<T>(hi[j]);
     lo[j] = pack2<T>(v[2 * j] - h.x, v[2 * j + 1] - h.y);
   }
@@ -256,28 +256,34 @@ __device__ __forceinline__ void emit16s(float *v, uint8_t *smem_tile, uint32_t l
 }
 
 // ------------------------------------------------------------------------------------- forward
-constexpr uint32_t COL_D1 = 0, COL_D2 = 64, COL_C1 = 96, COL_C2 = 160, COL_C3 = 224, FWD_COLS = 256;
-
 constexpr uint32_t TILE_BYTES = ROWS * H * 2;   // one [128][64] 16-bit tile
-constexpr uint32_t FWD_THREADS = 256;
-// Two activation buffers (each hi | lo) ping-pong through the layer chain; the encoder tile arrives
-// by TMA into buffer A, which is dead again by the time the colour input is built.  With the
-// two-term weight images that is 48 + 64 KB, so TWO CTAs fit an SM (and 2 x 256 TMEM columns).
+
+// One CTA per SM runs FOUR independent tile pipelines ("groups" of 128 threads = 4 warps, one TMEM lane quarter each) that
+// share one copy of the weight images.  Per tile a group walks the five layers as a chain  MMA -> accumulator read-back ->
+// activation -> 16-bit operand tile in shared memory -> next MMA; each link waits on the tensor core or on shared memory,
+// so what keeps the SM busy is the number of chains in flight (round 1 ran two per SM, one per CTA, each CTA with its own
+// 48 KB of weights: tensor pipe 12 % active, a third of all warp samples waiting on the MMA barrier, profiles/r2d).
+//  - ONE activation buffer per group: a layer's output tile is written over its input tile, which is dead once the
+//    layer's MMAs have completed (the group waits on their mbarrier before it reads the accumulator back).
+//  - ONE 64-column accumulator per group, reused by every layer (its previous contents have been read back before
+//    the next layer's MMAs are issued): 4 x 64 = 256 TMEM columns per CTA.
+//  - groups synchronise on their own named barrier and mbarriers and drift apart, so one group's read-back and packing
+//    overlap another's MMAs and TMA fetch.
+constexpr uint32_t FWD_GROUPS = 4, FWD_GROUP_THREADS = 128, FWD_THREADS = FWD_GROUPS * FWD_GROUP_THREADS;
+constexpr uint32_t FWD_COLS = 64 * FWD_GROUPS;
+template <bool SPLIT>
 struct FwdSmem {
-  static constexpr uint32_t w = 0;                                // weight images: hi (WImg forward region) then lo
-  static constexpr uint32_t bufA = w + 2 * WImg::f_total;         // hi | lo; also the TMA destination of the encoder tile
-  static constexpr uint32_t bufB = bufA + 2 * TILE_BYTES;         // hi | lo
-  static constexpr uint32_t bar_mma = bufB + 2 * TILE_BYTES;
-  static constexpr uint32_t bar_w = bar_mma + 8;
-  static constexpr uint32_t bar_e = bar_w + 8;
-  static constexpr uint32_t tmem = bar_e + 8;
+  static constexpr uint32_t w = 0;                                          // weight images: hi (WImg forward region), then lo
+  static constexpr uint32_t w_bytes = SPLIT ? 2 * WImg::f_total : WImg::f_total;
+  static constexpr uint32_t buf_bytes = SPLIT ? 2 * TILE_BYTES : TILE_BYTES; // hi | lo; also the TMA destination of the encoder tile
+  static constexpr uint32_t buf = w + w_bytes;
+  static constexpr uint32_t bar_w = buf + FWD_GROUPS * buf_bytes;
+  static constexpr uint32_t bar_mma = bar_w + 8;                            // [FWD_GROUPS]
+  static constexpr uint32_t bar_e = bar_mma + 8 * FWD_GROUPS;               // [FWD_GROUPS]
+  static constexpr uint32_t tmem = bar_e + 8 * FWD_GROUPS;
   static constexpr uint32_t total = tmem + 8;
 };
 
-// 8 warps per 128-sample tile: warp w owns TMEM lanes (= sample rows) 32 (w & 3) .. +31 -- the
-// hardware's lane-quarter rule -- and the column half (w >> 2) of every 64-wide layer, so the
-// accumulator read-back / two-term split / store of a layer is shared by two warps per SM
-// sub-partition (four with the second resident CTA).
 // SPLIT = true: two-term (hi + lo) operands, three MMA groups per layer -- the training forward, whose ReLU masks the
 // backward pass reuses and must agree with the float64 oracle.  SPLIT = false: plain 16-bit operands (one MMA group, half
 // the read-back work and half the operand bytes) for the forward-only uses: render (S15) and the occupancy refresh.
@@ -292,140 +298,145 @@ __device__ __forceinline__ void emit_fwd(float *v, uint8_t *tile, uint32_t lo_of
   if constexpr (SPLIT) emit16s<T, RELU>(v, tile, lo_off, blob, row, c0, valid);
   else emit16<T, RELU>(v, tile, blob, row, c0, valid);
 }
+// barrier of one 128-thread group (barrier 0 is __syncthreads)
+__device__ __forceinline__ void group_bar(uint32_t grp) { asm volatile("bar.sync %0, 128;" ::"r"(grp + 1u) : "memory"); }
+
+// a 64-wide hidden layer's accumulator -> ReLU -> the group's operand tile (in place) and, when saved, its blob tile
+template <typename T, bool SPLIT>
+__device__ __forceinline__ void hidden_epilogue(uint32_t tlane, uint8_t *buf, uint8_t *blob, uint32_t row, bool valid) {
+  float v[32];
+#pragma unroll
+  for (uint32_t c0 = 0; c0 < H; c0 += 32) {   // two accumulator loads in flight
+    tmem_ld16(tlane + c0, v);
+    tmem_ld16(tlane + c0 + 16, v + 16);
+    tmem_ld_wait();
+    emit_fwd<T, true, SPLIT>(v, buf, TILE_BYTES, blob, row, c0, valid);
+    emit_fwd<T, true, SPLIT>(v + 16, buf, TILE_BYTES, blob, row, c0 + 16, valid);
+  }
+}
 
 template <typename T, bool SPLIT>
-__global__ void __launch_bounds__(FWD_THREADS, 2) mlp_forward_tc_kernel(MlpShape ms, const float *__restrict__ dirs, Workspace ws,
+__global__ void __launch_bounds__(FWD_THREADS, 1) mlp_forward_tc_kernel(MlpShape ms, const float *__restrict__ dirs, Workspace ws,
                                                                        const uint32_t *__restrict__ d_S, int density_only,
                                                                        int save_blobs) {
+  using SM = FwdSmem<SPLIT>;
   extern __shared__ __align__(1024) uint8_t smem[];
   const uint32_t tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
-  const uint32_t row = (warp & 3u) * 32u + lane, half = warp >> 2;
+  const uint32_t grp = tid >> 7, row = tid & 127u;          // warp & 3 = the TMEM lane quarter of rows 32 (warp & 3) .. +31
+  const bool lead_warp = row < 32;                          // the group's first warp: one lane of it issues the MMAs and the TMA
   const uint32_t sbase = smem_u32(smem);
-  const uint32_t bar_mma = sbase + FwdSmem::bar_mma, bar_w = sbase + FwdSmem::bar_w, bar_e = sbase + FwdSmem::bar_e;
+  const uint32_t bar_w = sbase + SM::bar_w, bar_mma = sbase + SM::bar_mma + 8 * grp, bar_e = sbase + SM::bar_e + 8 * grp;
   const uint32_t LF = ms.LF;
   const uint32_t e_half = LF * ROWS * 2, e_stride = 2 * e_half;   // the encoder writes hi | lo per tile
-  const uint32_t e_bytes = SPLIT ? e_stride : e_half, w_bytes = SPLIT ? 2 * WImg::f_total : WImg::f_total;
+  const uint32_t e_bytes = SPLIT ? e_stride : e_half;
   // Before pdl_wait(): only data produced at least two kernels back (S from the marcher, the weight images).
   const uint64_t S = *d_S;
-  const bool has_tiles = (uint64_t)blockIdx.x * ROWS < S;
+  const uint64_t n_tiles = (S + ROWS - 1) / ROWS;
+  const bool has_tiles = blockIdx.x < n_tiles;
   if (has_tiles) {
     if (tid == 0) {
-      mbar_init(bar_mma, 1); mbar_init(bar_w, 1); mbar_init(bar_e, 1);
+      mbar_init(bar_w, 1);
+#pragma unroll
+      for (uint32_t g = 0; g < FWD_GROUPS; ++g) { mbar_init(sbase + SM::bar_mma + 8 * g, 1); mbar_init(sbase + SM::bar_e + 8 * g, 1); }
       fence_async_smem();
-      mbar_expect_tx(bar_w, w_bytes);
-      bulk_g2s(sbase + FwdSmem::w, ws.wimg_fwd, w_bytes, bar_w);
+      mbar_expect_tx(bar_w, SM::w_bytes);
+      bulk_g2s(sbase + SM::w, ws.wimg_fwd, SM::w_bytes, bar_w);
     }
-    if (warp == 0) tmem_alloc<FWD_COLS>(sbase + FwdSmem::tmem);
+    if (warp == 0) tmem_alloc<FWD_COLS>(sbase + SM::tmem);
   }
   pdl_wait();
   pdl_trigger();
   if (!has_tiles) return;
   tl_mark(ws.timeline, K_MLP_FWD, 0);
-  if (tid == 0) {   // the encoder's output: after the wait
-    mbar_expect_tx(bar_e, e_bytes);
-    bulk_g2s(sbase + FwdSmem::bufA, ws.blob_e + (size_t)blockIdx.x * e_stride, e_bytes, bar_e);
-  }
   fence_before();
   __syncthreads();
   fence_after();
-  const uint32_t tmem_base = *reinterpret_cast<volatile uint32_t *>(smem + FwdSmem::tmem);
-  const uint32_t tlane = tmem_base + (((warp & 3u) * 32u) << 16);
+  const uint32_t tmem_base = *reinterpret_cast<volatile uint32_t *>(smem + SM::tmem);
+  const uint32_t tcol = tmem_base + 64u * grp;                        // the group's accumulator columns
+  const uint32_t tlane = tcol + (((warp & 3u) * 32u) << 16);
   uint32_t ph_mma = 0, ph_e = 0;
   const uint32_t fmt = Fmt<T>::id;
-  uint8_t *bufA = smem + FwdSmem::bufA, *bufB = smem + FwdSmem::bufB;
-  const uint32_t sA = sbase + FwdSmem::bufA, sB = sbase + FwdSmem::bufB, sW = sbase + FwdSmem::w;
-  const uint32_t cb = half * 32u;    // this thread's column half of a 64-wide layer
-  if (tid == 0) mbar_wait(bar_w, 0);
+  uint8_t *buf = smem + SM::buf + grp * SM::buf_bytes;
+  const uint32_t sBuf = sbase + SM::buf + grp * SM::buf_bytes, sW = sbase + SM::w;
+  // group g of CTA b takes tiles b + g * gridDim.x, then every 4 * gridDim.x: with few tiles every SM gets one first
+  const uint64_t first_tile = blockIdx.x + (uint64_t)grp * gridDim.x, tile_stride = (uint64_t)FWD_GROUPS * gridDim.x;
+  if (lead_warp) {
+    if (first_tile < n_tiles && elect_one()) {   // the encoder's output: after the wait
+      mbar_expect_tx(bar_e, e_bytes);
+      bulk_g2s(sBuf, ws.blob_e + (size_t)first_tile * e_stride, e_bytes, bar_e);
+    }
+    mbar_wait(bar_w, 0);
+  }
 
-  for (uint64_t tile = blockIdx.x; tile * ROWS < S; tile += gridDim.x) {
+  for (uint64_t tile = first_tile; tile < n_tiles; tile += tile_stride) {
     const uint64_t s = tile * ROWS + row;
     const bool valid = s < S;
-    float v[16];
-    // ---- density hidden layer: A = encoder tile (in buffer A via TMA)
-    if (tid == 0) {
+    // ---- density hidden layer: A = encoder tile (in the buffer via TMA)
+    if (lead_warp) {
       mbar_wait(bar_e, ph_e);
       fence_after();
-      issue_fwd<SPLIT>(tmem_base + COL_D1, sA, e_half, sW + WImg::f_d1, WImg::f_total, LF, H, H, fmt, bar_mma);
+      if (elect_one()) issue_fwd<SPLIT>(tcol, sBuf, e_half, sW + WImg::f_d1, WImg::f_total, LF, H, H, fmt, bar_mma);
     }
     ph_e ^= 1;
+    // the ray direction of this row's sample (two dependent global loads): in flight under the first MMAs
+    float dx = 0.f, dy = 0.f, dz = 1.f;
+    if (!density_only && valid) {
+      const uint32_t ray = ws.s_ray[s];
+      dx = __ldg(dirs + 3 * (size_t)ray); dy = __ldg(dirs + 3 * (size_t)ray + 1); dz = __ldg(dirs + 3 * (size_t)ray + 2);
+    }
     mbar_wait(bar_mma, ph_mma); ph_mma ^= 1; fence_after();
-    if (density_only && tid == 0) {   // the density layers never write buffer A again: fetch the CTA's next encoder tile now
-      const uint64_t nxt = tile + gridDim.x;
-      if (nxt * ROWS < S) { mbar_expect_tx(bar_e, e_bytes); bulk_g2s(sA, ws.blob_e + (size_t)nxt * e_stride, e_bytes, bar_e); }
-    }
-    uint8_t *blob_hd = (save_blobs && !density_only) ? ws.blob_hd + (size_t)tile * (H * ROWS * 2) : nullptr;
-#pragma unroll
-    for (uint32_t c0 = 0; c0 < 32; c0 += 16) {
-      tmem_ld16(tlane + COL_D1 + cb + c0, v);
-      tmem_ld_wait();
-      emit_fwd<T, true, SPLIT>(v, bufB, TILE_BYTES, blob_hd, row, cb + c0, valid);
-    }
-    fence_async_smem(); fence_before(); __syncthreads();
-    if (tid == 0) { fence_after(); issue_fwd<SPLIT>(tmem_base + COL_D2, sB, TILE_BYTES, sW + WImg::f_d2, WImg::f_total, H, DO, DO, fmt, bar_mma); }
+    hidden_epilogue<T, SPLIT>(tlane, buf, (save_blobs && !density_only) ? ws.blob_hd + (size_t)tile * (H * ROWS * 2) : nullptr, row, valid);
+    fence_async_smem(); fence_before(); group_bar(grp);
+    if (lead_warp) { fence_after(); if (elect_one()) issue_fwd<SPLIT>(tcol, sBuf, TILE_BYTES, sW + WImg::f_d2, WImg::f_total, H, DO, DO, fmt, bar_mma); }
     mbar_wait(bar_mma, ph_mma); ph_mma ^= 1; fence_after();
     float g[16];
-    tmem_ld16(tlane + COL_D2, g);
+    tmem_ld16(tlane, g);
     tmem_ld_wait();
-    if (valid && half == 0) ws.sigma[s] = expf(fminf(fmaxf(g[0], -15.f), 15.f));
+    if (valid) ws.sigma[s] = expf(fminf(fmaxf(g[0], -15.f), 15.f));
     if (density_only) {
-      fence_before(); __syncthreads();   // all reads of COL_D2 are done before the next tile's MMAs
+      if (lead_warp) {   // the buffer is free: the group's next encoder tile
+        const uint64_t nxt = tile + tile_stride;
+        if (nxt < n_tiles && elect_one()) { mbar_expect_tx(bar_e, e_bytes); bulk_g2s(sBuf, ws.blob_e + (size_t)nxt * e_stride, e_bytes, bar_e); }
+      }
+      fence_before(); group_bar(grp);   // every read of the accumulator is done before the next tile's MMAs
       continue;
     }
-    // ---- colour input [g slice, Y(d), 0 pad] -> buffer A (K = 32); each column half emits its 16 columns
+    // ---- colour input [g slice, Y(d), 0 pad] -> the buffer (K = 32)
     {
       float ci[CIP];
-#pragma unroll
-      for (int j = 0; j < (int)CIP; ++j) ci[j] = 0.f;
       // mlp_tc_supported() admits only the slice (geo_offset, geo_count) = (1, 15) with 16 SH terms (configs 2-5):
       // static register indexing, no local memory
 #pragma unroll
       for (int j = 0; j < 15; ++j) ci[j] = g[1 + j];
-      float dx = 0.f, dy = 0.f, dz = 1.f;
-      if (valid) {
-        const uint32_t ray = ws.s_ray[s];
-        dx = __ldg(dirs + 3 * (size_t)ray); dy = __ldg(dirs + 3 * (size_t)ray + 1); dz = __ldg(dirs + 3 * (size_t)ray + 2);
-      }
       float Y[16];
       sh_row(4, dx, dy, dz, Y);
 #pragma unroll
       for (int j = 0; j < 16; ++j) ci[15 + j] = Y[j];
+      ci[31] = 0.f;
       uint8_t *blob_ci = save_blobs ? ws.blob_ci + (size_t)tile * (CIP * ROWS * 2) : nullptr;
-      if (half == 0) emit_fwd<T, false, SPLIT>(ci, bufA, TILE_BYTES, blob_ci, row, 0, valid);
-      else emit_fwd<T, false, SPLIT>(ci + 16, bufA, TILE_BYTES, blob_ci, row, 16, valid);
+      emit_fwd<T, false, SPLIT>(ci, buf, TILE_BYTES, blob_ci, row, 0, valid);
+      emit_fwd<T, false, SPLIT>(ci + 16, buf, TILE_BYTES, blob_ci, row, 16, valid);
     }
-    fence_async_smem(); fence_before(); __syncthreads();
-    if (tid == 0) { fence_after(); issue_fwd<SPLIT>(tmem_base + COL_C1, sA, TILE_BYTES, sW + WImg::f_c1, WImg::f_total, CIP, H, H, fmt, bar_mma); }
+    fence_async_smem(); fence_before(); group_bar(grp);
+    if (lead_warp) { fence_after(); if (elect_one()) issue_fwd<SPLIT>(tcol, sBuf, TILE_BYTES, sW + WImg::f_c1, WImg::f_total, CIP, H, H, fmt, bar_mma); }
     mbar_wait(bar_mma, ph_mma); ph_mma ^= 1; fence_after();
-    uint8_t *blob_h1 = save_blobs ? ws.blob_h1 + (size_t)tile * (H * ROWS * 2) : nullptr;
-#pragma unroll
-    for (uint32_t c0 = 0; c0 < 32; c0 += 16) {
-      tmem_ld16(tlane + COL_C1 + cb + c0, v);
-      tmem_ld_wait();
-      emit_fwd<T, true, SPLIT>(v, bufB, TILE_BYTES, blob_h1, row, cb + c0, valid);
-    }
-    uint32_t sLast = sB;
+    hidden_epilogue<T, SPLIT>(tlane, buf, save_blobs ? ws.blob_h1 + (size_t)tile * (H * ROWS * 2) : nullptr, row, valid);
     if (ms.n_color_layers == 2) {
-      fence_async_smem(); fence_before(); __syncthreads();
-      if (tid == 0) { fence_after(); issue_fwd<SPLIT>(tmem_base + COL_C2, sB, TILE_BYTES, sW + WImg::f_c2, WImg::f_total, H, H, H, fmt, bar_mma); }
+      fence_async_smem(); fence_before(); group_bar(grp);
+      if (lead_warp) { fence_after(); if (elect_one()) issue_fwd<SPLIT>(tcol, sBuf, TILE_BYTES, sW + WImg::f_c2, WImg::f_total, H, H, H, fmt, bar_mma); }
       mbar_wait(bar_mma, ph_mma); ph_mma ^= 1; fence_after();
-      uint8_t *blob_h2 = save_blobs ? ws.blob_h2 + (size_t)tile * (H * ROWS * 2) : nullptr;
-#pragma unroll
-      for (uint32_t c0 = 0; c0 < 32; c0 += 16) {
-        tmem_ld16(tlane + COL_C2 + cb + c0, v);
-        tmem_ld_wait();
-        emit_fwd<T, true, SPLIT>(v, bufA, TILE_BYTES, blob_h2, row, cb + c0, valid);
-      }
-      sLast = sA;
+      hidden_epilogue<T, SPLIT>(tlane, buf, save_blobs ? ws.blob_h2 + (size_t)tile * (H * ROWS * 2) : nullptr, row, valid);
     }
-    fence_async_smem(); fence_before(); __syncthreads();
-    if (tid == 0) { fence_after(); issue_fwd<SPLIT>(tmem_base + COL_C3, sLast, TILE_BYTES, sW + WImg::f_c3, WImg::f_total, H, 16, 16, fmt, bar_mma); }
+    fence_async_smem(); fence_before(); group_bar(grp);
+    if (lead_warp) { fence_after(); if (elect_one()) issue_fwd<SPLIT>(tcol, sBuf, TILE_BYTES, sW + WImg::f_c3, WImg::f_total, H, 16, 16, fmt, bar_mma); }
     mbar_wait(bar_mma, ph_mma); ph_mma ^= 1; fence_after();
-    if (tid == 0) {   // every buffer is free: the CTA's next encoder tile
-      const uint64_t nxt = tile + gridDim.x;
-      if (nxt * ROWS < S) { mbar_expect_tx(bar_e, e_bytes); bulk_g2s(sA, ws.blob_e + (size_t)nxt * e_stride, e_bytes, bar_e); }
+    if (lead_warp) {   // the buffer is free: the group's next encoder tile
+      const uint64_t nxt = tile + tile_stride;
+      if (nxt < n_tiles && elect_one()) { mbar_expect_tx(bar_e, e_bytes); bulk_g2s(sBuf, ws.blob_e + (size_t)nxt * e_stride, e_bytes, bar_e); }
     }
-    if (half == 0) {
-      tmem_ld16(tlane + COL_C3, v);
+    {
+      float v[16];
+      tmem_ld16(tlane, v);
       tmem_ld_wait();
       if (valid) {
 #pragma unroll
@@ -433,7 +444,7 @@ __global__ void __launch_bounds__(FWD_THREADS, 2) mlp_forward_tc_kernel(MlpShape
       }
     }
     fence_before();
-    __syncthreads();   // nobody may still be reading TMEM / writing buffers when the next tile's first MMA is issued
+    group_bar(grp);   // nobody of the group may still be reading the accumulator when the next tile's first MMA is issued
   }
   fence_before();
   __syncthreads();
@@ -472,10 +483,11 @@ struct BwdSmem {
 __device__ __forceinline__ void issue_wgrad(uint32_t tmem_d, uint32_t x_saddr, uint32_t y_saddr, uint32_t N, uint32_t fmt,
                                             uint32_t accumulate) {
   const uint32_t idesc = make_idesc(fmt, 128, N, 1, 1);
+  uint64_t da = make_desc(x_saddr, 128, PANEL), db = make_desc(y_saddr, 128, PANEL);   // MN-major: LBO = next 8 samples, SBO = next 8 features
+#pragma unroll
   for (uint32_t k = 0; k < ROWS / 16; ++k) {
-    const uint64_t da = make_desc(x_saddr + k * 256, 128, PANEL);   // MN-major: LBO = next 8 samples, SBO = next 8 features
-    const uint64_t db = make_desc(y_saddr + k * 256, 128, PANEL);
     mma_ss(tmem_d, da, db, idesc, accumulate | (k > 0));
+    da += 256 >> 4; db += 256 >> 4;
   }
 }
 
@@ -586,7 +598,7 @@ __global__ void __launch_bounds__(BWD_THREADS, 2) mlp_backward_tc_kernel(MlpShap
   }
   const float inv_scale = 1.f / scale;
   uint32_t acc = 0;   // wgrad accumulate flag (0 on the CTA's first tile)
-  if (tid == 0) mbar_wait(bar_w, 0);
+  if (warp == 0) mbar_wait(bar_w, 0);
 
   for (uint64_t tile = blockIdx.x; tile * ROWS < S; tile += gridDim.x) {
     const uint64_t s = tile * ROWS + row;
@@ -614,13 +626,15 @@ __global__ void __launch_bounds__(BWD_THREADS, 2) mlp_backward_tc_kernel(MlpShap
     wait_x(cur);
     uint32_t mask = row_mask32<T>(bufX(cur), row, cb);
     fence_async_smem(); fence_before(); __syncthreads();
-    if (tid == 0) {
+    if (warp == 0) {
       fence_after();
-      issue_wgrad(tmem_base + GW_C3, sX(cur), sY, 16, fmt, acc);
-      issue_layer(tmem_base + COL_G, sY, sW + WImg::b_c3, 16, H, H, fmt, bar_mma);
+      if (elect_one()) {
+        issue_wgrad(tmem_base + GW_C3, sX(cur), sY, 16, fmt, acc);
+        issue_layer(tmem_base + COL_G, sY, sW + WImg::b_c3, 16, H, H, fmt, bar_mma);
+      }
     }
     mbar_wait(bar_mma, ph_mma); ph_mma ^= 1; fence_after();
-    if (tid == 0) load_x(two ? 2 : 3, cur, tile);    // buffer free: fetch the layer after next
+    if (warp == 0 && elect_one()) load_x(two ? 2 : 3, cur, tile);    // buffer free: fetch the layer after next
     cur ^= 1;
     // ---- second colour hidden layer
     if (two) {
@@ -628,26 +642,30 @@ __global__ void __launch_bounds__(BWD_THREADS, 2) mlp_backward_tc_kernel(MlpShap
       wait_x(cur);
       mask = row_mask32<T>(bufX(cur), row, cb);
       fence_async_smem(); fence_before(); __syncthreads();
-      if (tid == 0) {
+      if (warp == 0) {
         fence_after();
-        issue_wgrad(tmem_base + GW_C2, sX(cur), sY, H, fmt, acc);
-        issue_layer(tmem_base + COL_G, sY, sW + WImg::b_c2, H, H, H, fmt, bar_mma);
+        if (elect_one()) {
+          issue_wgrad(tmem_base + GW_C2, sX(cur), sY, H, fmt, acc);
+          issue_layer(tmem_base + COL_G, sY, sW + WImg::b_c2, H, H, H, fmt, bar_mma);
+        }
       }
       mbar_wait(bar_mma, ph_mma); ph_mma ^= 1; fence_after();
-      if (tid == 0) load_x(3, cur, tile);
+      if (warp == 0 && elect_one()) load_x(3, cur, tile);
       cur ^= 1;
     }
     // ---- first colour layer: dY = d h1 (masked); X = [g slice, Y(d), 0]; wgrad transposed: G^T = dY^T X
     masked_to_Y<T>(tlane, mask, bufY, row, cb);
     wait_x(cur);
     fence_async_smem(); fence_before(); __syncthreads();
-    if (tid == 0) {
+    if (warp == 0) {
       fence_after();
-      issue_wgrad(tmem_base + GW_C1T, sY, sX(cur), CIP, fmt, acc);
-      issue_layer(tmem_base + COL_G, sY, sW + WImg::b_c1, H, CIP, CIP, fmt, bar_mma);
+      if (elect_one()) {
+        issue_wgrad(tmem_base + GW_C1T, sY, sX(cur), CIP, fmt, acc);
+        issue_layer(tmem_base + COL_G, sY, sW + WImg::b_c1, H, CIP, CIP, fmt, bar_mma);
+      }
     }
     mbar_wait(bar_mma, ph_mma); ph_mma ^= 1; fence_after();
-    if (tid == 0) load_x(4, cur, tile);
+    if (warp == 0 && elect_one()) load_x(4, cur, tile);
     cur ^= 1;
     // ---- density output layer: dg = [geo slice of d ci] + e_0 * dL/dsigma * sigma (0 where clamped)
     if (half == 0) {
@@ -670,10 +688,12 @@ __global__ void __launch_bounds__(BWD_THREADS, 2) mlp_backward_tc_kernel(MlpShap
     wait_x(cur);
     mask = row_mask32<T>(bufX(cur), row, cb);
     fence_async_smem(); fence_before(); __syncthreads();
-    if (tid == 0) {
+    if (warp == 0) {
       fence_after();
-      issue_wgrad(tmem_base + GW_D2, sX(cur), sY, 16, fmt, acc);
-      issue_layer(tmem_base + COL_G, sY, sW + WImg::b_d2, 16, H, H, fmt, bar_mma);
+      if (elect_one()) {
+        issue_wgrad(tmem_base + GW_D2, sX(cur), sY, 16, fmt, acc);
+        issue_layer(tmem_base + COL_G, sY, sW + WImg::b_d2, 16, H, H, fmt, bar_mma);
+      }
     }
     mbar_wait(bar_mma, ph_mma); ph_mma ^= 1; fence_after();
     cur ^= 1;
@@ -681,14 +701,16 @@ __global__ void __launch_bounds__(BWD_THREADS, 2) mlp_backward_tc_kernel(MlpShap
     masked_to_Y<T>(tlane, mask, bufY, row, cb);
     wait_x(cur);
     fence_async_smem(); fence_before(); __syncthreads();
-    if (tid == 0) {
+    if (warp == 0) {
       fence_after();
-      issue_wgrad(tmem_base + GW_D1, sX(cur), sY, H, fmt, acc);
-      issue_layer(tmem_base + COL_G, sY, sW + WImg::b_d1, H, LF, LF, fmt, bar_mma);
+      if (elect_one()) {
+        issue_wgrad(tmem_base + GW_D1, sX(cur), sY, H, fmt, acc);
+        issue_layer(tmem_base + COL_G, sY, sW + WImg::b_d1, H, LF, LF, fmt, bar_mma);
+      }
     }
     mbar_wait(bar_mma, ph_mma); ph_mma ^= 1; fence_after();
     // both X buffers are free: the next tile's first two layers (tiles always start at buffer 0)
-    if (tid == 0 && has_next) {
+    if (warp == 0 && has_next && elect_one()) {
       load_x(0, 0, next_tile);
       load_x(two ? 1 : 2, 1, next_tile);
     }
@@ -798,10 +820,10 @@ uint32_t mlp_tc_backward_ctas(int n_sms) { return 2u * (uint32_t)n_sms; }
 // The kernels need more than 48 KB of dynamic shared memory: an opt-in that CUDA keeps per device.
 cudaError_t mlp_tc_prepare_device() {
   const auto attr = cudaFuncAttributeMaxDynamicSharedMemorySize;
-  cudaError_t e = cudaFuncSetAttribute(mlp_forward_tc_kernel<__half, true>, attr, (int)FwdSmem::total);
-  if (e == cudaSuccess) e = cudaFuncSetAttribute(mlp_forward_tc_kernel<__half, false>, attr, (int)FwdSmem::total);
-  if (e == cudaSuccess) e = cudaFuncSetAttribute(mlp_forward_tc_kernel<__nv_bfloat16, true>, attr, (int)FwdSmem::total);
-  if (e == cudaSuccess) e = cudaFuncSetAttribute(mlp_forward_tc_kernel<__nv_bfloat16, false>, attr, (int)FwdSmem::total);
+  cudaError_t e = cudaFuncSetAttribute(mlp_forward_tc_kernel<__half, true>, attr, (int)FwdSmem<true>::total);
+  if (e == cudaSuccess) e = cudaFuncSetAttribute(mlp_forward_tc_kernel<__half, false>, attr, (int)FwdSmem<false>::total);
+  if (e == cudaSuccess) e = cudaFuncSetAttribute(mlp_forward_tc_kernel<__nv_bfloat16, true>, attr, (int)FwdSmem<true>::total);
+  if (e == cudaSuccess) e = cudaFuncSetAttribute(mlp_forward_tc_kernel<__nv_bfloat16, false>, attr, (int)FwdSmem<false>::total);
   if (e == cudaSuccess) e = cudaFuncSetAttribute(mlp_backward_tc_kernel<__half>, attr, (int)BwdSmem::total);
   if (e == cudaSuccess) e = cudaFuncSetAttribute(mlp_backward_tc_kernel<__nv_bfloat16>, attr, (int)BwdSmem::total);
   return e;
@@ -810,7 +832,7 @@ cudaError_t mlp_tc_prepare_device() {
 template <typename T, bool SPLIT>
 static void launch_fwd_variant(const MlpShape &ms, const float *dirs, const Workspace &ws, const uint32_t *d_S, int density_only,
                                int save_blobs, int n_sms, cudaStream_t st) {
-  launch_pdl(mlp_forward_tc_kernel<T, SPLIT>, dim3(2 * n_sms), dim3(FWD_THREADS), (size_t)FwdSmem::total, st, ms, dirs, ws, d_S,
+  launch_pdl(mlp_forward_tc_kernel<T, SPLIT>, dim3(n_sms), dim3(FWD_THREADS), (size_t)FwdSmem<SPLIT>::total, st, ms, dirs, ws, d_S,
              density_only, save_blobs);
 }
 

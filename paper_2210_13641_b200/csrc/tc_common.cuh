@@ -58,6 +58,21 @@ __device__ __forceinline__ void mma_ss(uint32_t tmem_d, uint64_t desc_a, uint64_
       : "memory");
 }
 
+// One lane of a converged warp (elect.sync).  The single-thread instructions (tcgen05.mma / commit, TMA issue) sit in
+// `if (warp-uniform condition) { if (elect_one()) ... }`: with a thread-divergent condition such as `tid == 0` the compiler
+// wraps every instruction that takes uniform-register operands (UTCHMMA's descriptors) in a loop over the active lanes.
+__device__ __forceinline__ bool elect_one() {
+  uint32_t p;
+  asm volatile(
+      "{\n\t"
+      ".reg .pred p;\n\t"
+      "elect.sync _|p, 0xffffffff;\n\t"
+      "selp.u32 %0, 1, 0, p;\n\t"
+      "}\n"
+      : "=r"(p));
+  return p != 0;
+}
+
 // all prior tcgen05.mma of this thread arrive on the mbarrier when complete
 __device__ __forceinline__ void mma_commit(uint32_t bar_saddr) {
   asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(bar_saddr)
