@@ -149,11 +149,11 @@ def config2(seed=2, R=4096, K=128, n_batches=1, occ_res=128, field_overrides=Non
 # --------------------------------------------------------------------------- configs 3, 4, 5
 
 def config3(seed=3, R=1 << 14, K=128, n_keyframes=10, n_batches=4, width=1200, height=680,
-            first_batch=0, field_overrides=None):
+            first_batch=0, field_overrides=None, outlier_fraction=0.05):
     """Keyframe-window mapping in the synthetic room (BASELINE.json configs[2]).  Batches are
     drawn uniformly over all (keyframe, pixel) pairs, seeded per step."""
     room = scenes.Room(seed)
-    kfs = scenes.KeyframeSet(room, seed, n_keyframes, width, height)
+    kfs = scenes.KeyframeSet(room, seed, n_keyframes, width, height, outlier_fraction)
     fc = FieldConfig(aabb_min=(0.0, 0.0, 0.0), aabb_extent=8.0, seed=seed, max_rays=R,
                      max_candidates=K, mlp_precision=1)
     t_min, t_max = 0.05, 10.5

@@ -213,8 +213,9 @@ class KeyframeSet:
     are outliers: D_slam = r U[0.3,2.0], Sigma_D = sigma_d^2, sigma_d ~ U[1,3].
     Whole frames are ray-cast lazily and cached; batches cast only the pixels they draw."""
 
-    def __init__(self, room, seed, n, width=1200, height=680):
+    def __init__(self, room, seed, n, width=1200, height=680, outlier_fraction=0.05):
         self.room, self.seed, self.n, self.W, self.H = room, seed, n, width, height
+        self.outlier_fraction = outlier_fraction      # BASELINE.json: 5 %; the ablation also runs heavier contamination
         s = width / 1200.0
         self.fx = self.fy = 600.0 * s
         self.cx, self.cy = (width - 1) / 2.0, (height - 1) / 2.0
@@ -264,7 +265,7 @@ class KeyframeSet:
         gauss = np.sqrt(-2.0 * np.log(1.0 - u[0])) * np.cos(2.0 * np.pi * u[1])     # Box-Muller
         depth = r * (1.0 + 0.01 * gauss)
         var = (0.01 * r) ** 2
-        outlier = u[2] < 0.05
+        outlier = u[2] < self.outlier_fraction
         depth = np.where(outlier, r * (0.3 + 1.7 * u[3]), depth)
         var = np.where(outlier, (1.0 + 2.0 * u[4]) ** 2, var)
         return dict(o=o32, d=d32, rgb=rgb.astype(np.float32), depth=depth.astype(np.float32), var=var.astype(np.float32),
