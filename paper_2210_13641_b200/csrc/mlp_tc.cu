@@ -466,18 +466,19 @@ constexpr uint32_t GW_C3 = 64, GW_C2 = 80, GW_C1T = 144, GW_D2 = 176, GW_D1 = 19
 constexpr uint32_t BWD_THREADS = 256;
 
 struct BwdSmem {
-  static constexpr uint32_t w = 0;                                // weight image (WImg backward region)
-  static constexpr uint32_t bufX0 = w + WImg::b_total;            // [128][64]; the M=128 wgrad also reads the 16 KB after it
-  static constexpr uint32_t bufX1 = bufX0 + ROWS * H * 2;         // [128][64]
-  static constexpr uint32_t bufY = bufX1 + ROWS * H * 2;          // [128][64]
-  static constexpr uint32_t pad = bufY + ROWS * H * 2;            // 16 KB readable slack behind bufY (M=128 reads of a 64-column tile)
-  static constexpr uint32_t bar_mma = pad + ROWS * H * 2;
+  // [X0][X1][X2][Y0][Y1][W], 16 KB tiles.  An M = 128 MMA that reads a 64-column tile MN-major also reads the 16 KB behind
+  // it (rows 64..127 of its result are never used): behind every tile sits another tile, behind Y1 the weight image.
+  static constexpr uint32_t tile = ROWS * H * 2;
+  static constexpr uint32_t bufX = 0;                              // ring of three saved-activation tiles (TMA destinations)
+  static constexpr uint32_t bufY = bufX + 3 * tile;                // two dY tiles, alternating per layer
+  static constexpr uint32_t w = bufY + 2 * tile;                   // weight image (WImg backward region)
+  static constexpr uint32_t bar_mma = w + WImg::b_total;
   static constexpr uint32_t bar_w = bar_mma + 8;
-  static constexpr uint32_t bar_x0 = bar_w + 8;
-  static constexpr uint32_t bar_x1 = bar_x0 + 8;
-  static constexpr uint32_t tmem = bar_x1 + 8;
+  static constexpr uint32_t bar_x = bar_w + 8;                     // [3]
+  static constexpr uint32_t tmem = bar_x + 24;
   static constexpr uint32_t total = tmem + 8;
 };
+static_assert(WImg::b_total >= BwdSmem::tile, "the slack behind Y1 must be covered by the weight image");
 
 // wgrad k-steps over the 128 samples: G[128 (columns of tile A) x N (columns of tile B)] (+)= A^T B
 __device__ __forceinline__ void issue_wgrad(uint32_t tmem_d, uint32_t x_saddr, uint32_t y_saddr, uint32_t N, uint32_t fmt,
@@ -523,8 +524,16 @@ __device__ __forceinline__ void masked_to_Y(uint32_t tlane, uint32_t mask, uint8
   }
 }
 
-// 8 warps per tile as in the forward kernel: warp w owns sample rows 32 (w & 3) .. +31 (TMEM lane quarter) and the
-// column half (w >> 2) of every 64-wide dgrad.
+// 8 warps per tile: warp w owns sample rows 32 (w & 3) .. +31 (TMEM lane quarter) and the column half (w >> 2) of every
+// 64-wide dgrad.  Two CTAs per SM.
+//
+// The layers of the CTA's tiles form one sequence of items n = 0, 1, 2, ...  Item n reads its saved activation from
+// X[n % 3] and its dY from Y[n % 2].  Only the item's dgrad is on the critical path (the next item's dY is computed from
+// it): the elected lane issues the dgrad MMAs, commits them onto the barrier the CTA waits on, and THEN issues the item's
+// wgrad MMAs, which run under the CTA's read-back and packing of the next item (round 1 waited for both: 8 of an item's
+// ~12 MMAs are wgrad).  A tcgen05.commit covers every MMA the thread issued before it, so when item n+1's dgrad has
+// completed, item n's wgrad has too: X[n % 3] is then refilled by TMA with the activation of item n+3, and Y[n % 2] is
+// free for item n+2.
 template <typename T>
 __global__ void __launch_bounds__(BWD_THREADS, 2) mlp_backward_tc_kernel(MlpShape ms, Workspace ws,
                                                                         const uint32_t *__restrict__ d_S) {
@@ -533,49 +542,55 @@ __global__ void __launch_bounds__(BWD_THREADS, 2) mlp_backward_tc_kernel(MlpShap
   const uint32_t row = (warp & 3u) * 32u + lane, half = warp >> 2, cb = half * 32u;
   const uint32_t sbase = smem_u32(smem);
   const uint32_t bar_mma = sbase + BwdSmem::bar_mma, bar_w = sbase + BwdSmem::bar_w;
-  // the two X buffers, selected arithmetically (indexing a two-element array by a runtime value goes to local memory)
-  auto bar_x = [&](uint32_t b) { return sbase + BwdSmem::bar_x0 + 8u * b; };
-  auto sX = [&](uint32_t b) { return sbase + BwdSmem::bufX0 + (ROWS * H * 2) * b; };
-  auto bufX = [&](uint32_t b) { return smem + BwdSmem::bufX0 + (ROWS * H * 2) * b; };
-  uint32_t ph_x0 = 0, ph_x1 = 0;
-  auto wait_x = [&](uint32_t b) {
-    if (b) { mbar_wait(bar_x(1), ph_x1); ph_x1 ^= 1; } else { mbar_wait(bar_x(0), ph_x0); ph_x0 ^= 1; }
-  };
-  uint8_t *bufY = smem + BwdSmem::bufY;
-  const uint32_t sY = sbase + BwdSmem::bufY, sW = sbase + BwdSmem::w;
+  const uint32_t sW = sbase + BwdSmem::w;
   const uint32_t LF = ms.LF;
   const uint64_t S = *d_S;                         // from the marcher, several kernels back: safe before pdl_wait()
   const bool has_tiles = (uint64_t)blockIdx.x * ROWS < S;
   const bool two = ms.n_color_layers == 2;
   const uint32_t hbytes = H * ROWS * 2, cbytes = CIP * ROWS * 2, ebytes = LF * ROWS * 2;
 
-  // the activation tiles of one 128-sample tile, in the order the layers consume them
-  auto load_x = [&](uint32_t which, uint32_t buf, uint64_t tile) {   // one thread
-    const uint8_t *src; uint32_t bytes;
-    switch (which) {
-      case 0: src = (two ? ws.blob_h2 : ws.blob_h1) + tile * hbytes; bytes = hbytes; break;
-      case 1: src = ws.blob_h1 + tile * hbytes; bytes = hbytes; break;
-      case 2: src = ws.blob_ci + tile * cbytes; bytes = cbytes; break;
-      case 3: src = ws.blob_hd + tile * hbytes; bytes = hbytes; break;
-      default: src = ws.blob_e + tile * (2 * (size_t)ebytes); bytes = ebytes; break;   // the hi half of the two-term tile
+  // ---- the X ring.  Loader state (identical in every lane of warp 0; the elected lane issues): the next item to fetch.
+  uint64_t ld_tile = blockIdx.x;
+  uint32_t ld_layer = 0, ld_slot = 0;              // layer 0..4 (1 is skipped with one hidden colour layer); ring slot
+  auto load_next = [&]() {                         // warp 0, converged
+    if (ld_tile * ROWS < S && elect_one()) {
+      const uint8_t *src; uint32_t bytes;
+      switch (ld_layer) {                          // the activation the layer's wgrad needs
+        case 0: src = (two ? ws.blob_h2 : ws.blob_h1) + ld_tile * hbytes; bytes = hbytes; break;
+        case 1: src = ws.blob_h1 + ld_tile * hbytes; bytes = hbytes; break;
+        case 2: src = ws.blob_ci + ld_tile * cbytes; bytes = cbytes; break;
+        case 3: src = ws.blob_hd + ld_tile * hbytes; bytes = hbytes; break;
+        default: src = ws.blob_e + ld_tile * (2 * (size_t)ebytes); bytes = ebytes; break;   // the hi half of the two-term tile
+      }
+      const uint32_t bar = sbase + BwdSmem::bar_x + 8 * ld_slot;
+      mbar_expect_tx(bar, bytes);
+      bulk_g2s(sbase + BwdSmem::bufX + ld_slot * BwdSmem::tile, src, bytes, bar);
     }
-    mbar_expect_tx(bar_x(buf), bytes);
-    bulk_g2s(sX(buf), src, bytes, bar_x(buf));
+    ld_layer = ld_layer == 4 ? 0u : (ld_layer == 0 && !two ? 2u : ld_layer + 1u);
+    if (ld_layer == 0) ld_tile += gridDim.x;
+    ld_slot = ld_slot == 2 ? 0u : ld_slot + 1u;
   };
+  // consumer state: ring slot and dY buffer of the current item, barrier phases of the three slots (bit i = slot i)
+  uint32_t xs = 0, ys = 0, ph_x = 0, items = 0;
+  auto wait_x = [&]() { mbar_wait(sbase + BwdSmem::bar_x + 8 * xs, (ph_x >> xs) & 1u); ph_x ^= 1u << xs; };
+  auto bufX = [&]() { return smem + BwdSmem::bufX + xs * BwdSmem::tile; };
+  auto sX = [&]() { return sbase + BwdSmem::bufX + xs * BwdSmem::tile; };
+  auto bufY = [&]() { return smem + BwdSmem::bufY + ys * BwdSmem::tile; };
+  auto sY = [&]() { return sbase + BwdSmem::bufY + ys * BwdSmem::tile; };
 
   if (has_tiles) {   // prologue on data that is at least two kernels old (weight image, the forward pass's saved activations)
     if (tid == 0) {
-      mbar_init(bar_mma, 1); mbar_init(bar_w, 1); mbar_init(bar_x(0), 1); mbar_init(bar_x(1), 1);
+      mbar_init(bar_mma, 1); mbar_init(bar_w, 1);
+      mbar_init(sbase + BwdSmem::bar_x, 1); mbar_init(sbase + BwdSmem::bar_x + 8, 1); mbar_init(sbase + BwdSmem::bar_x + 16, 1);
       fence_async_smem();
       mbar_expect_tx(bar_w, WImg::b_total);
       bulk_g2s(sW, ws.wimg_bwd, WImg::b_total, bar_w);
-      load_x(0, 0, blockIdx.x);
-      load_x(two ? 1 : 2, 1, blockIdx.x);
     }
-    // the slack behind bufY is read as rows 64..127 of an M = 128 operand: keep it finite
-    for (uint32_t i = tid; i < ROWS * H * 2 / 16; i += BWD_THREADS)
-      reinterpret_cast<uint4 *>(smem + BwdSmem::pad)[i] = make_uint4(0, 0, 0, 0);
-    if (warp == 0) tmem_alloc<BWD_COLS>(sbase + BwdSmem::tmem);
+    if (warp == 0) {
+      __syncwarp();
+      load_next(); load_next(); load_next();
+      tmem_alloc<BWD_COLS>(sbase + BwdSmem::tmem);
+    }
   }
   pdl_wait();     // the compositor's dL/dsigma, dL/dc and gradient maximum
   pdl_trigger();
@@ -600,13 +615,25 @@ __global__ void __launch_bounds__(BWD_THREADS, 2) mlp_backward_tc_kernel(MlpShap
   uint32_t acc = 0;   // wgrad accumulate flag (0 on the CTA's first tile)
   if (warp == 0) mbar_wait(bar_w, 0);
 
+  // one item: dY is in Y[ys] and X[xs] has landed (the caller waited).  Issue dgrad (committed: the CTA waits for it) and
+  // wgrad (not waited for), wait for the dgrad, refill the ring slot that the PREVIOUS item's wgrad has released, advance.
+#define BWD_ITEM(WGRAD_STMT, DGRAD_STMT)                                                     \
+  do {                                                                                       \
+    fence_async_smem(); fence_before(); __syncthreads();                                     \
+    if (warp == 0) {                                                                         \
+      fence_after();                                                                         \
+      if (elect_one()) { DGRAD_STMT; WGRAD_STMT; }                                           \
+    }                                                                                        \
+    mbar_wait(bar_mma, ph_mma); ph_mma ^= 1; fence_after();                                  \
+    if (warp == 0 && items > 0) load_next();                                                 \
+    items += 1;                                                                              \
+    xs = xs == 2 ? 0u : xs + 1u; ys ^= 1u;                                                   \
+  } while (0)
+
   for (uint64_t tile = blockIdx.x; tile * ROWS < S; tile += gridDim.x) {
     const uint64_t s = tile * ROWS + row;
     const bool valid = s < S;
-    const uint64_t next_tile = tile + gridDim.x;
-    const bool has_next = next_tile * ROWS < S;
     float v[16];
-    uint32_t cur = 0;   // X buffer of the current layer; tiles always start with buffer 0
     // ---- colour output layer: dY = dL/dc * c (1 - c); X = last hidden activations
     float sig = 0.f, dsig = 0.f;
     if (half == 0) {
@@ -621,52 +648,25 @@ __global__ void __launch_bounds__(BWD_THREADS, 2) mlp_backward_tc_kernel(MlpShap
         sig = ws.sigma[s];
         dsig = ws.dsigma[s];
       }
-      emit16<T, false>(v, bufY, nullptr, row, 0, true);
+      emit16<T, false>(v, bufY(), nullptr, row, 0, true);
     }
-    wait_x(cur);
-    uint32_t mask = row_mask32<T>(bufX(cur), row, cb);
-    fence_async_smem(); fence_before(); __syncthreads();
-    if (warp == 0) {
-      fence_after();
-      if (elect_one()) {
-        issue_wgrad(tmem_base + GW_C3, sX(cur), sY, 16, fmt, acc);
-        issue_layer(tmem_base + COL_G, sY, sW + WImg::b_c3, 16, H, H, fmt, bar_mma);
-      }
-    }
-    mbar_wait(bar_mma, ph_mma); ph_mma ^= 1; fence_after();
-    if (warp == 0 && elect_one()) load_x(two ? 2 : 3, cur, tile);    // buffer free: fetch the layer after next
-    cur ^= 1;
+    wait_x();
+    uint32_t mask = row_mask32<T>(bufX(), row, cb);
+    BWD_ITEM(issue_wgrad(tmem_base + GW_C3, sX(), sY(), 16, fmt, acc),
+             issue_layer(tmem_base + COL_G, sY(), sW + WImg::b_c3, 16, H, H, fmt, bar_mma));
     // ---- second colour hidden layer
     if (two) {
-      masked_to_Y<T>(tlane, mask, bufY, row, cb);
-      wait_x(cur);
-      mask = row_mask32<T>(bufX(cur), row, cb);
-      fence_async_smem(); fence_before(); __syncthreads();
-      if (warp == 0) {
-        fence_after();
-        if (elect_one()) {
-          issue_wgrad(tmem_base + GW_C2, sX(cur), sY, H, fmt, acc);
-          issue_layer(tmem_base + COL_G, sY, sW + WImg::b_c2, H, H, H, fmt, bar_mma);
-        }
-      }
-      mbar_wait(bar_mma, ph_mma); ph_mma ^= 1; fence_after();
-      if (warp == 0 && elect_one()) load_x(3, cur, tile);
-      cur ^= 1;
+      masked_to_Y<T>(tlane, mask, bufY(), row, cb);
+      wait_x();
+      mask = row_mask32<T>(bufX(), row, cb);
+      BWD_ITEM(issue_wgrad(tmem_base + GW_C2, sX(), sY(), H, fmt, acc),
+               issue_layer(tmem_base + COL_G, sY(), sW + WImg::b_c2, H, H, H, fmt, bar_mma));
     }
     // ---- first colour layer: dY = d h1 (masked); X = [g slice, Y(d), 0]; wgrad transposed: G^T = dY^T X
-    masked_to_Y<T>(tlane, mask, bufY, row, cb);
-    wait_x(cur);
-    fence_async_smem(); fence_before(); __syncthreads();
-    if (warp == 0) {
-      fence_after();
-      if (elect_one()) {
-        issue_wgrad(tmem_base + GW_C1T, sY, sX(cur), CIP, fmt, acc);
-        issue_layer(tmem_base + COL_G, sY, sW + WImg::b_c1, H, CIP, CIP, fmt, bar_mma);
-      }
-    }
-    mbar_wait(bar_mma, ph_mma); ph_mma ^= 1; fence_after();
-    if (warp == 0 && elect_one()) load_x(4, cur, tile);
-    cur ^= 1;
+    masked_to_Y<T>(tlane, mask, bufY(), row, cb);
+    wait_x();
+    BWD_ITEM(issue_wgrad(tmem_base + GW_C1T, sY(), sX(), CIP, fmt, acc),
+             issue_layer(tmem_base + COL_G, sY(), sW + WImg::b_c1, H, CIP, CIP, fmt, bar_mma));
     // ---- density output layer: dg = [geo slice of d ci] + e_0 * dL/dsigma * sigma (0 where clamped)
     if (half == 0) {
       float dci[CIP], dg[16];
@@ -683,37 +683,17 @@ __global__ void __launch_bounds__(BWD_THREADS, 2) mlp_backward_tc_kernel(MlpShap
       }
       // sigma = exp(clamp(g0, -15, 15)): the clamp is active iff sigma sits on a bound
       if (valid && sig > 3.0590232e-07f * 1.0001f && sig < 3269017.4f * 0.9999f) dg[0] += dsig * sig * scale;
-      emit16<T, false>(dg, bufY, nullptr, row, 0, true);
+      emit16<T, false>(dg, bufY(), nullptr, row, 0, true);
     }
-    wait_x(cur);
-    mask = row_mask32<T>(bufX(cur), row, cb);
-    fence_async_smem(); fence_before(); __syncthreads();
-    if (warp == 0) {
-      fence_after();
-      if (elect_one()) {
-        issue_wgrad(tmem_base + GW_D2, sX(cur), sY, 16, fmt, acc);
-        issue_layer(tmem_base + COL_G, sY, sW + WImg::b_d2, 16, H, H, fmt, bar_mma);
-      }
-    }
-    mbar_wait(bar_mma, ph_mma); ph_mma ^= 1; fence_after();
-    cur ^= 1;
+    wait_x();
+    mask = row_mask32<T>(bufX(), row, cb);
+    BWD_ITEM(issue_wgrad(tmem_base + GW_D2, sX(), sY(), 16, fmt, acc),
+             issue_layer(tmem_base + COL_G, sY(), sW + WImg::b_d2, 16, H, H, fmt, bar_mma));
     // ---- density hidden layer: dY = d hd (masked); X = e
-    masked_to_Y<T>(tlane, mask, bufY, row, cb);
-    wait_x(cur);
-    fence_async_smem(); fence_before(); __syncthreads();
-    if (warp == 0) {
-      fence_after();
-      if (elect_one()) {
-        issue_wgrad(tmem_base + GW_D1, sX(cur), sY, H, fmt, acc);
-        issue_layer(tmem_base + COL_G, sY, sW + WImg::b_d1, H, LF, LF, fmt, bar_mma);
-      }
-    }
-    mbar_wait(bar_mma, ph_mma); ph_mma ^= 1; fence_after();
-    // both X buffers are free: the next tile's first two layers (tiles always start at buffer 0)
-    if (warp == 0 && has_next && elect_one()) {
-      load_x(0, 0, next_tile);
-      load_x(two ? 1 : 2, 1, next_tile);
-    }
+    masked_to_Y<T>(tlane, mask, bufY(), row, cb);
+    wait_x();
+    BWD_ITEM(issue_wgrad(tmem_base + GW_D1, sX(), sY(), H, fmt, acc),
+             issue_layer(tmem_base + COL_G, sY(), sW + WImg::b_d1, H, LF, LF, fmt, bar_mma));
     // ---- dL/de -> planes; each column half writes its LF/2 columns
     const uint32_t ncol = LF / 2;
     for (uint32_t c0 = half * ncol; c0 < (half + 1) * ncol; c0 += 16) {
@@ -723,13 +703,17 @@ __global__ void __launch_bounds__(BWD_THREADS, 2) mlp_backward_tc_kernel(MlpShap
 #pragma unroll
         for (int j = 0; j < 16; ++j) ws.de[(size_t)(c0 + j) * ws.cap + s] = v[j] * inv_scale;
     }
-    fence_before();
-    __syncthreads();   // all reads of COL_G and writes of bufY are done before the next tile reuses them
-    acc = 1;
+    acc = 1;   // (the next item's __syncthreads follows these reads of COL_G, before its dgrad overwrites it)
   }
-  // ---- flush the CTA's weight gradients: thread (row i, column half) holds row i of every G
+#undef BWD_ITEM
+  // ---- the last item's wgrad is still in flight: one more commit, then flush the CTA's weight gradients
   fence_before();
   __syncthreads();
+  if (warp == 0) {
+    fence_after();
+    if (elect_one()) mma_commit(bar_mma);
+  }
+  mbar_wait(bar_mma, ph_mma); ph_mma ^= 1;
   fence_after();
   // Each CTA stores its sums into its own slice of ws.wgrad_part with plain, lane-coalesced stores; the slices are
   // summed by the consumer (the MLP Adam kernel, or reduce_wgrad_kernel).  Atomics onto the 9-11 K shared addresses
