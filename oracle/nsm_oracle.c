@@ -724,7 +724,9 @@ int orc_train_step(const orc_config *cfg, double *theta, double *m, double *v, u
         if (want_pose) {
           /* dL/dx_c = sum_l N_l sum_corners (d omega / d w_c) (theta[corner] . dL/de_l): w_c = x_c N_l - c0_c */
           double dxs[3] = {0.0, 0.0, 0.0};
-          for (uint32_t l = 0; l < L; ++l) {
+          /* R26 (coarse-to-fine pose gradients): only the levels l < pose_levels carry the position's derivative */
+          const uint32_t L_pose = (cfg->pose_levels == 0 || cfg->pose_levels > L) ? L : cfg->pose_levels;
+          for (uint32_t l = 0; l < L_pose; ++l) {
             const uint32_t *slot = slots + ((size_t)s * L + l) * 8;
             const float *w = wfr + ((size_t)s * L + l) * 3;
             for (uint32_t corner = 0; corner < 8; ++corner) {

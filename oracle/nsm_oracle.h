@@ -62,6 +62,12 @@ typedef struct {
   uint32_t sparse_table_adam;
   uint64_t seed;
   uint32_t occ_cascades;   /* F4 / R23: number of nested occupancy grids (0 or 1: the single grid of S2) */
+  uint32_t pose_levels;    /* F2 / R26: the pose gradients differentiate the sample position through the encoding levels
+                            * l < pose_levels only (0 or >= L: all levels).  The field itself is always evaluated with all
+                            * levels; only dL/dx -- hence g_o and the geometric part of tau -- is restricted.  The paper is
+                            * silent (PAPER.md:120, 130-133 only name T among the variables of Eq. 3); the fine levels of a
+                            * hash grid vary on a scale far below a pose error and their spatial derivative misleads a
+                            * first-order pose step, so a refinement runs coarse to fine. */
 } orc_config;
 
 typedef struct {

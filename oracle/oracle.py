@@ -26,7 +26,8 @@ class OrcConfig(C.Structure):
                 ("color_hidden", C.c_uint32), ("color_hidden_layers", C.c_uint32),
                 ("bg", C.c_float * 3), ("occ_sigma_threshold", C.c_float),
                 ("lr", C.c_float), ("beta1", C.c_float), ("beta2", C.c_float), ("eps", C.c_float),
-                ("sparse_table_adam", C.c_uint32), ("seed", C.c_uint64), ("occ_cascades", C.c_uint32)]
+                ("sparse_table_adam", C.c_uint32), ("seed", C.c_uint64), ("occ_cascades", C.c_uint32),
+                ("pose_levels", C.c_uint32)]
 
 
 class OrcBatch(C.Structure):
@@ -125,6 +126,7 @@ def make_config(fc):
     for k in ("occ_sigma_threshold", "lr", "beta1", "beta2", "eps"):
         setattr(c, k, float(getattr(fc, k)))
     c.occ_cascades = int(getattr(fc, "occ_cascades", 1))
+    c.pose_levels = int(getattr(fc, "pose_levels", 0))
     return c
 
 

@@ -172,3 +172,78 @@ def test_pose_step_descends_the_loss():
     predicted = -eps * (G ** 2).sum()
     assert l2 < st["loss"]
     assert abs((l2 - st["loss"]) - predicted) <= 0.15 * abs(predicted), (l2 - st["loss"], predicted)
+
+
+# ---------------------------------------------------------------- coarse-to-fine pose gradients (reading R26)
+
+def _ray_loss(fc, theta, b, r, xs_coarse, xs_fine, n_coarse, d_sh, t, delta, lam):
+    """Ray r's term of L (Eqs. 3, 4, 7 with R rays in the batch) restated through the oracle's public stage functions, with
+    the encoding levels l < n_coarse evaluated at xs_coarse and the others at xs_fine, and the SH encoding at d_sh."""
+    F = fc.n_features
+    n_table, _ = orc.param_count(fc)
+    e_c, _, _ = orc.encode(fc, theta, xs_coarse, want_index=False)
+    e_f, _, _ = orc.encode(fc, theta, xs_fine, want_index=False)
+    e = np.concatenate([e_c[:, :n_coarse * F], e_f[:, n_coarse * F:]], axis=1)
+    Y = orc.sh(fc.sh_degree, d_sh[None])[0]
+    sig, rgb = [], []
+    for i in range(len(e)):
+        s_, c_ = orc.field_eval(fc, theta[n_table:], e[i], Y)
+        sig.append(s_); rgb.append(c_)
+    C, D, _ = orc.composite(np.array(sig), np.array(rgb), t, delta, fc.bg)
+    R = b.n_rays
+    L_rgb = ((C - b.rgb[r].astype(np.float64)) ** 2).sum() / R
+    L_d = (D - float(b.depth[r])) ** 2 / float(b.depth_var[r]) / R
+    return L_rgb + lam * L_d
+
+
+@pytest.mark.parametrize("n_coarse", [1, 2, 3])
+def test_masked_pose_gradients_differentiate_the_coarse_levels_only(n_coarse):
+    """pose_levels = n: g_o and tau must be the derivative of the loss when ONLY the levels l < n see the moved ray, the
+    finer levels keeping the unmoved positions (and the SH encoding seeing the rotated direction in full).  Checked by
+    central differences of a per-ray loss rebuilt from orc.encode / field_eval / sh / composite with spliced encodings."""
+    lam = 0.3
+    fc, b, theta = tiny(3, seed=1)
+    fc_m = replace(fc, pose_levels=n_coarse)
+    assert n_coarse < fc.n_levels
+    O = orc.Oracle(fc_m, theta.copy())
+    _, tr = O.train_step(b, lam, apply_adam=False, trace=("g_o", "tau", "s_ray", "s_x", "s_t", "s_delta"))
+    _, tr_all = orc.Oracle(fc, theta.copy()).train_step(b, lam, apply_adam=False, trace=("g_o", "tau"))
+    assert np.abs(tr["g_o"] - tr_all["g_o"]).max() > 1e-3 * np.abs(tr_all["g_o"]).max()      # the mask does something
+    ext = float(np.float32(fc.aabb_extent))
+    amin = np.asarray(fc.aabb_min, np.float64)
+    h = 2.0 ** -11
+    ok = 0
+    scale_o, scale_t = np.abs(tr["g_o"]).max(), np.abs(tr["tau"]).max()
+    for r in range(b.n_rays):
+        sel = tr["s_ray"] == r
+        if sel.sum() == 0:
+            continue
+        x0, t, delta = tr["s_x"][sel].astype(np.float64), tr["s_t"][sel], tr["s_delta"][sel]
+        o, d = b.origins[r].astype(np.float64), b.dirs[r].astype(np.float64)
+        f = lambda xc, dsh: _ray_loss(fc, theta, b, r, xc.astype(np.float32), x0.astype(np.float32), n_coarse, dsh, t, delta, lam)
+        for c in range(3):
+            step = np.eye(3)[c] * h / ext
+            lp, l0, lm = f(x0 + step, d), f(x0, d), f(x0 - step, d)
+            if abs(lp - 2 * l0 + lm) / h > 0.02 * scale_o:          # a cell boundary inside the stencil
+                continue
+            assert abs((lp - lm) / (2 * h) - tr["g_o"][r, c]) <= 2e-2 * scale_o, (r, c)
+            ok += 1
+        for k in range(3):
+            xs = lambda s_: ((o + t[:, None].astype(np.float64) * (rot(k, s_ * h) @ d) - amin) / ext)
+            lp, l0, lm = f(xs(+1), rot(k, h) @ d), f(x0, d), f(xs(-1), rot(k, -h) @ d)
+            if abs(lp - 2 * l0 + lm) / h > 0.02 * scale_t:
+                continue
+            assert abs((lp - lm) / (2 * h) - tr["tau"][r, k]) <= 2e-2 * scale_t, (r, k)
+            ok += 1
+    assert ok >= 3 * b.n_rays                                          # at least half of the 6 R derivatives were testable
+
+
+def test_pose_levels_zero_and_all_levels_are_the_unmasked_gradients():
+    fc, b, theta = tiny(3)
+    ref = orc.Oracle(fc, theta.copy()).train_step(b, 0.3, apply_adam=False, trace=("g_o", "tau", "grad"))[1]
+    for n in (0, fc.n_levels, fc.n_levels + 5):
+        tr = orc.Oracle(replace(fc, pose_levels=n), theta.copy()).train_step(b, 0.3, apply_adam=False, trace=("g_o", "tau", "grad"))[1]
+        assert np.array_equal(tr["g_o"], ref["g_o"]) and np.array_equal(tr["tau"], ref["tau"])
+    # the mask never touches the parameter gradients
+    tr = orc.Oracle(replace(fc, pose_levels=1), theta.copy()).train_step(b, 0.3, apply_adam=False, trace=("grad",))[1]
+    assert np.array_equal(tr["grad"], ref["grad"])

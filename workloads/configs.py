@@ -46,6 +46,7 @@ class FieldConfig:
     max_rays: int = 4096
     max_candidates: int = 128
     occ_cascades: int = 1             # F4: nested occupancy grids (1 = the single grid of S2)
+    pose_levels: int = 0              # F2: levels that carry the pose gradient (0 = all); oracle config / GPU option
 
 
 @dataclass
