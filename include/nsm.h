@@ -237,7 +237,10 @@ nsm_status nsm_get_keyframe_pose(nsm_field *f, uint32_t index, float *h_R, float
  * of workspace. */
 /* NSM_OPT_DEBUG_TIMELINE (default 0).  With 1 the kernels of every training step record the in-kernel timeline that
  * nsm_debug_timeline reads. */
-typedef enum { NSM_OPT_BATCH_READY = 0, NSM_OPT_POSE_GRADIENTS = 1, NSM_OPT_DEBUG_TIMELINE = 2 } nsm_option;
+/* NSM_OPT_POSE_LEVELS (default 0 = all).  Coarse-to-fine pose refinement (reading R26): the pose gradients
+ * differentiate the sample positions through the encoding levels l < value only; the field itself is always evaluated
+ * with all levels and the parameter gradients do not change.  May be changed between steps (a schedule). */
+typedef enum { NSM_OPT_BATCH_READY = 0, NSM_OPT_POSE_GRADIENTS = 1, NSM_OPT_DEBUG_TIMELINE = 2, NSM_OPT_POSE_LEVELS = 3 } nsm_option;
 nsm_status nsm_set_option(nsm_field *f, nsm_option opt, uint32_t value);
 
 /* S1-S12 only: forward + backward, gradients left in place for nsm_debug_last_step; and S13

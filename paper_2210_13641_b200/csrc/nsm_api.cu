@@ -114,6 +114,7 @@ struct nsm_field {
   KeyframeDev *kf_dev = nullptr;
   // row f2: pose gradients (NSM_OPT_POSE_GRADIENTS)
   bool pose_grads = false, last_sampled = false;
+  uint32_t pose_levels = 0;   // row f2, reading R26: encoding levels that carry the pose gradient (0 = all)
   float *pose_go = nullptr, *pose_tau = nullptr, *kf_grad = nullptr;   // [max_rays,3] x2, [NSM_MAX_KEYFRAMES,NSM_KF_GRAD_STRIDE]
   float *kf_pose_m = nullptr, *kf_pose_v = nullptr;                    // Adam moments of the keyframe poses [NSM_MAX_KEYFRAMES,6]
   uint32_t *kf_pose_cnt = nullptr;                                     // updates received per keyframe
@@ -372,7 +373,7 @@ nsm_status enqueue_backward(nsm_field *f, const nsm_ray_batch *b, float lambda_d
     f->last_sampled = sample_draw >= 0;
     RUN(f, K_POSE, launch_pose_gradients(f->lv, f->fp.theta, f->ws, d_S, R, dirs_copy ? dirs_copy : b->dirs, 1.0f / f->cfg.aabb_extent,
                                          f->cfg.sh_degree, f->pose_go, f->pose_tau, f->last_sampled ? f->ray_kf : nullptr, f->kf_grad,
-                                         (uint32_t)f->kf_host.size(), f->n_sms, f->stream));
+                                         (uint32_t)f->kf_host.size(), f->n_sms, f->stream, f->pose_levels));
   }
   // train step: the scatter is issued by enqueue_adam, behind the MLP Adam's hand-off to the side stream
   f->scatter_pending = defer_scatter;
@@ -1010,6 +1011,7 @@ nsm_status nsm_set_option(nsm_field *f, nsm_option opt, uint32_t value) {
       f->pose_grads = value != 0;
       return NSM_OK;
     }
+    case NSM_OPT_POSE_LEVELS: f->pose_levels = value; return NSM_OK;
     case NSM_OPT_DEBUG_TIMELINE: {
       LEAVE_FAST_PATH(f);
       if (value && !f->timeline_base) {

@@ -340,7 +340,7 @@ int launch_sample_batch(const KeyframeDev *kfs, uint32_t n_kf, uint64_t seed, ui
 // (optional): the per-keyframe vectors [n_kf][NSM_KF_GRAD_STRIDE], written (not accumulated) by a block per keyframe
 int launch_pose_gradients(const LevelTable &lv, const float *theta, const Workspace &ws, const uint32_t *d_S, uint32_t R,
                           const float *dirs, float inv_extent, uint32_t sh_degree, float *g_o, float *tau, const uint32_t *ray_kf,
-                          float *kf_grad, uint32_t n_kf, int n_sms, cudaStream_t st);
+                          float *kf_grad, uint32_t n_kf, int n_sms, cudaStream_t st, uint32_t pose_levels = 0);
 // f2, the update: Adam + exponential map on the keyframes that received rays (kf_grad: [n_kf][NSM_KF_GRAD_STRIDE])
 int launch_pose_step(KeyframeDev *kfs, uint32_t n_kf, const float *kf_grad, float *pm, float *pv, uint32_t *pcnt, float lr_t,
                      float lr_r, float beta1, float beta2, float eps, cudaStream_t st);

@@ -25,16 +25,17 @@ __device__ __forceinline__ float warp_sum(float v) {
 }
 
 // LPS lanes per sample (16 when L <= 16: two samples per warp; else 32), lane = level.
+// n_pose: the levels l < n_pose carry the position's derivative (coarse-to-fine pose refinement, DESIGN.md 8d reading R26)
 template <int F, int LPS>
 __global__ void __launch_bounds__(256) pose_dx_kernel(LevelTable lv, const float *__restrict__ theta, Workspace ws,
-                                                      const uint32_t *__restrict__ d_S) {
+                                                      const uint32_t *__restrict__ d_S, uint32_t n_pose) {
   const uint64_t S = *d_S;
   const uint32_t lane = threadIdx.x & (LPS - 1);
   const uint64_t group0 = ((uint64_t)blockIdx.x * blockDim.x + threadIdx.x) / LPS, n_groups = ((uint64_t)gridDim.x * blockDim.x) / LPS;
   const uint64_t S_pad = (S + (32 / LPS) - 1) / (32 / LPS) * (32 / LPS);   // whole warps stay converged for the shuffles
   for (uint64_t s = group0; s < S_pad; s += n_groups) {
     float acc[3] = {0.f, 0.f, 0.f};
-    if (s < S && lane < lv.n_levels) {
+    if (s < S && lane < n_pose) {
       const uint32_t l = lane;
       const CornerIndex ci = corner_index(lv, l, ws.s_x[s], ws.s_x[ws.cap + s], ws.s_x[2 * ws.cap + s]);
       float de[F];
@@ -219,14 +220,15 @@ int launch_pose_step(KeyframeDev *kfs, uint32_t n_kf, const float *kf_grad, floa
 
 int launch_pose_gradients(const LevelTable &lv, const float *theta, const Workspace &ws, const uint32_t *d_S, uint32_t R,
                           const float *dirs, float inv_extent, uint32_t sh_degree, float *g_o, float *tau, const uint32_t *ray_kf,
-                          float *kf_grad, uint32_t n_kf, int n_sms, cudaStream_t st) {
+                          float *kf_grad, uint32_t n_kf, int n_sms, cudaStream_t st, uint32_t pose_levels) {
   dim3 grid(n_sms * 8), block(256);
+  const uint32_t n_pose = (pose_levels == 0 || pose_levels > lv.n_levels) ? lv.n_levels : pose_levels;
   const bool half = lv.n_levels <= 16;
   switch (lv.n_features) {
-    case 1: if (half) pose_dx_kernel<1, 16><<<grid, block, 0, st>>>(lv, theta, ws, d_S); else pose_dx_kernel<1, 32><<<grid, block, 0, st>>>(lv, theta, ws, d_S); break;
-    case 2: if (half) pose_dx_kernel<2, 16><<<grid, block, 0, st>>>(lv, theta, ws, d_S); else pose_dx_kernel<2, 32><<<grid, block, 0, st>>>(lv, theta, ws, d_S); break;
-    case 4: if (half) pose_dx_kernel<4, 16><<<grid, block, 0, st>>>(lv, theta, ws, d_S); else pose_dx_kernel<4, 32><<<grid, block, 0, st>>>(lv, theta, ws, d_S); break;
-    default: if (half) pose_dx_kernel<8, 16><<<grid, block, 0, st>>>(lv, theta, ws, d_S); else pose_dx_kernel<8, 32><<<grid, block, 0, st>>>(lv, theta, ws, d_S); break;
+    case 1: if (half) pose_dx_kernel<1, 16><<<grid, block, 0, st>>>(lv, theta, ws, d_S, n_pose); else pose_dx_kernel<1, 32><<<grid, block, 0, st>>>(lv, theta, ws, d_S, n_pose); break;
+    case 2: if (half) pose_dx_kernel<2, 16><<<grid, block, 0, st>>>(lv, theta, ws, d_S, n_pose); else pose_dx_kernel<2, 32><<<grid, block, 0, st>>>(lv, theta, ws, d_S, n_pose); break;
+    case 4: if (half) pose_dx_kernel<4, 16><<<grid, block, 0, st>>>(lv, theta, ws, d_S, n_pose); else pose_dx_kernel<4, 32><<<grid, block, 0, st>>>(lv, theta, ws, d_S, n_pose); break;
+    default: if (half) pose_dx_kernel<8, 16><<<grid, block, 0, st>>>(lv, theta, ws, d_S, n_pose); else pose_dx_kernel<8, 32><<<grid, block, 0, st>>>(lv, theta, ws, d_S, n_pose); break;
   }
   pose_ray_kernel<<<(R + 7) / 8, 256, 0, st>>>(ws, R, dirs, inv_extent, sh_degree, g_o, tau);
   if (ray_kf && n_kf) pose_kf_reduce_kernel<<<n_kf, 256, 0, st>>>(R, ray_kf, g_o, tau, kf_grad);

@@ -533,6 +533,39 @@ def test_pose_gradients_fp32_path(nsm):
         f.close()
 
 
+def test_pose_gradients_restricted_to_coarse_levels(nsm):
+    """NSM_OPT_POSE_LEVELS (reading R26) against the oracle's pose_levels: the same per-ray criterion with the position's
+    derivative taken through the levels l < n only, on the fp32 path (n = 1, 3 of 4 levels) and on the tensor-core path
+    (n = 5 of 16); n = 0 and n >= L give the unrestricted gradients back, and the parameter gradients never change."""
+    w = configs.config1(variant_b=True)
+    w = replace(w, field=replace(w.field, sh_degree=4))
+    f, O, _ = make_pair(nsm, w, seed=13, table_scale=0.3, mlp_scale=1.5)
+    f.nsm_set_option(nsm.NSM_OPT_POSE_GRADIENTS, 1)
+    full, _, _ = _check_pose(nsm, f, O, w.batches[0], 0.4, 1e-3)
+    g_full = f.nsm_debug_last_step("grad")
+    for n in (1, 3):
+        f.nsm_set_option(nsm.NSM_OPT_POSE_LEVELS, n)
+        O.cfg.pose_levels = n
+        go, _, _ = _check_pose(nsm, f, O, w.batches[0], 0.4, 1e-3)
+        assert np.abs(go - full).max() > 1e-3 * np.abs(full).max()                     # the restriction does something
+        g_n = f.nsm_debug_last_step("grad")                                            # the parameter gradients do not change
+        assert np.abs(g_n - g_full).max() <= 1e-5 * np.abs(g_full).max()
+    for n in (0, 4, 9):
+        f.nsm_set_option(nsm.NSM_OPT_POSE_LEVELS, n)
+        O.cfg.pose_levels = n
+        go, _, _ = _check_pose(nsm, f, O, w.batches[0], 0.4, 1e-3)
+        assert np.abs(go - full).max() <= 1e-5 * np.abs(full).max()
+    f.close()
+    w = configs.config3(R=512, K=128, n_keyframes=3, n_batches=1, width=300, height=170)
+    f, O, _ = make_pair(nsm, w, seed=19, table_scale=0.5)
+    assert f.nsm_mlp_path().startswith("tcgen05")
+    f.nsm_set_option(nsm.NSM_OPT_POSE_GRADIENTS, 1)
+    f.nsm_set_option(nsm.NSM_OPT_POSE_LEVELS, 5)
+    O.cfg.pose_levels = 5
+    _check_pose(nsm, f, O, w.batches[0], w.lambda_d, tol_for(w.field, f.nsm_mlp_path()))
+    f.close()
+
+
 def test_pose_gradients_tensor_core_path_and_keyframe_sums(nsm):
     """The 16-bit tensor-core configuration (SH degree 4), through nsm_train_step_sampled: per-ray gradients against the
     oracle on the oracle-drawn batch, and the per-keyframe se(3) sums against numpy sums of the oracle's per-ray values."""
