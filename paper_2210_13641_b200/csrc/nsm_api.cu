@@ -52,6 +52,7 @@ static const char *kKernelNames[K_COUNT] = {"march", "encode", "mlp_fwd", "compo
 // bracketed by two events on the field's stream and each step ends with a synchronise.
 struct Profiler {
   bool on = false;
+  bool failed = false;   // an event of the timing pass could not be recorded or read: its numbers are not to be trusted
   double ms[K_COUNT] = {0};
   uint64_t n[K_COUNT] = {0};
   struct Rec { int id; cudaEvent_t a, b; };
@@ -64,8 +65,7 @@ struct Profiler {
   void collect() {
     for (auto &r : pending) {
       float t = 0.f;
-      cudaEventSynchronize(r.b);
-      cudaEventElapsedTime(&t, r.a, r.b);
+      if (cudaEventSynchronize(r.b) != cudaSuccess || cudaEventElapsedTime(&t, r.a, r.b) != cudaSuccess) failed = true;
       ms[r.id] += t; n[r.id] += 1;
       pool.push_back(r.a); pool.push_back(r.b);
     }
@@ -224,9 +224,11 @@ nsm_status validate_batch(const nsm_field *f, const nsm_ray_batch *b, bool train
     g_cur_kernel = (id);                                                    \
     if ((f)->prof.on) {                                                     \
       Profiler::Rec r_{id, (f)->prof.get(), (f)->prof.get()};               \
-      cudaEventRecord(r_.a, (st_));                                         \
+      const cudaError_t ea_ = cudaEventRecord(r_.a, (st_));                 \
       int n_ = (call);                                                      \
-      cudaEventRecord(r_.b, (st_));                                         \
+      const cudaError_t eb_ = cudaEventRecord(r_.b, (st_));                 \
+      if (ea_ != cudaSuccess || eb_ != cudaSuccess)                         \
+        (f)->prof.failed = true;   /* reported by nsm_profile_read */       \
       (f)->prof.pending.push_back(r_);                                      \
       (f)->launches += n_; (f)->launches_by[id] += n_;                      \
     } else {                                                                \
@@ -630,6 +632,10 @@ nsm_status nsm_profile_read(nsm_field *f, uint32_t capacity, const char **names,
                             uint32_t *n_out) {
   if (!f || !n_out) return fail(NSM_ERR_INVALID_ARG, "NULL argument");
   f->prof.collect();
+  if (f->prof.failed) {
+    f->prof.failed = false;
+    return fail(NSM_ERR_CUDA, "a timing event of the per-kernel pass could not be recorded or read");
+  }
   *n_out = K_COUNT;
   for (uint32_t i = 0; i < capacity && i < K_COUNT; ++i) {
     if (names) names[i] = kKernelNames[i];
