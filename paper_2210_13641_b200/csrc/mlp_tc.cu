@@ -694,9 +694,8 @@ __global__ void __launch_bounds__(BWD_THREADS, 2) mlp_backward_tc_kernel(MlpShap
     wait_x();
     BWD_ITEM(issue_wgrad(tmem_base + GW_D1, sX(), sY(), H, fmt, acc),
              issue_layer(tmem_base + COL_G, sY(), sW + WImg::b_d1, H, LF, LF, fmt, bar_mma));
-    // ---- dL/de -> planes; each column half writes its LF/2 columns
-    const uint32_t ncol = LF / 2;
-    for (uint32_t c0 = half * ncol; c0 < (half + 1) * ncol; c0 += 16) {
+    // ---- dL/de -> planes; the two column halves take the 16-column chunks of the LF columns alternately
+    for (uint32_t c0 = half * 16; c0 < LF; c0 += 32) {
       tmem_ld16(tlane + COL_G + c0, v);
       tmem_ld_wait();
       if (valid)
