@@ -256,14 +256,18 @@ def test_occupancy_set_get_roundtrip(nsm):
     f.close()
 
 
-@pytest.mark.parametrize("precision", [1, 2])
-def test_render_parity(nsm, precision):
+@pytest.mark.parametrize("precision,shape", [(1, None), (2, None), (1, (12, 4, 1)), (2, (8, 2, 1))])
+def test_render_parity(nsm, precision, shape):
     """P8: nsm_render vs the oracle's S15 on a pixel-strided view of the room, field = a few GPU
-    training steps on config-3-style data (parameters copied to the oracle); fp16 and bf16 tensor-core MLPs."""
+    training steps on config-3-style data (parameters copied to the oracle); fp16 and bf16 tensor-core MLPs; shape =
+    (L, F, hidden colour layers) also runs the forward-only tensor-core kernels on encoder widths 48 and 16 with one layer."""
     w = configs.config3(R=2048, K=128, n_keyframes=3, n_batches=6, width=300, height=170)
     fc = replace(w.field, bg=(0.1, 0.2, 0.3), max_candidates=256, mlp_precision=precision)
+    if shape:
+        fc = replace(fc, n_levels=shape[0], n_features=shape[1], color_hidden_layers=shape[2], n_max=512, log2_table_size=16)
     w = replace(w, field=fc)
     f, O, theta0 = make_pair(nsm, w, seed=6, table_scale=0.05)
+    assert f.nsm_mlp_path().startswith("tcgen05")
     for b in w.batches:
         f.nsm_train_step(nsm.DeviceBatch(b), w.lambda_d, want_stats=False)
     th, m, v, step = f.nsm_get_params()
