@@ -617,56 +617,68 @@ __global__ void __launch_bounds__(BWD_THREADS, 2) mlp_backward_tc_kernel(MlpShap
 
   // one item: dY is in Y[ys] and X[xs] has landed (the caller waited).  Issue dgrad (committed: the CTA waits for it) and
   // wgrad (not waited for), wait for the dgrad, refill the ring slot that the PREVIOUS item's wgrad has released, advance.
-#define BWD_ITEM(WGRAD_STMT, DGRAD_STMT)                                                     \
+#define BWD_ITEM(WGRAD_STMT, DGRAD_STMT, UNDER_MMA_STMT)                                     \
   do {                                                                                       \
     fence_async_smem(); fence_before(); __syncthreads();                                     \
     if (warp == 0) {                                                                         \
       fence_after();                                                                         \
       if (elect_one()) { DGRAD_STMT; WGRAD_STMT; }                                           \
     }                                                                                        \
+    UNDER_MMA_STMT;   /* work that does not need the dgrad: runs under the MMAs' latency */  \
     mbar_wait(bar_mma, ph_mma); ph_mma ^= 1; fence_after();                                  \
     if (warp == 0 && items > 0) load_next();                                                 \
     items += 1;                                                                              \
     xs = xs == 2 ? 0u : xs + 1u; ys ^= 1u;                                                   \
   } while (0)
 
+  // the first item's inputs (dL/dc * c (1 - c), sigma, dL/dsigma of this thread's sample): global loads, fetched for the
+  // NEXT tile under the last item's MMAs
+  float in_dc[3] = {0.f, 0.f, 0.f}, in_sig = 0.f, in_dsig = 0.f;
+  auto fetch_inputs = [&](uint64_t tile) {
+    const uint64_t s = tile * ROWS + row;
+    in_dc[0] = in_dc[1] = in_dc[2] = 0.f; in_sig = 0.f; in_dsig = 0.f;
+    if (half == 0 && s < S) {
+#pragma unroll
+      for (int c = 0; c < 3; ++c) {
+        const float col = ws.rgb[3 * s + c];
+        in_dc[c] = ws.drgb[3 * s + c] * col * (1.f - col) * scale;
+      }
+      in_sig = ws.sigma[s];
+      in_dsig = ws.dsigma[s];
+    }
+  };
+  fetch_inputs(blockIdx.x);
+
   for (uint64_t tile = blockIdx.x; tile * ROWS < S; tile += gridDim.x) {
     const uint64_t s = tile * ROWS + row;
     const bool valid = s < S;
     float v[16];
     // ---- colour output layer: dY = dL/dc * c (1 - c); X = last hidden activations
-    float sig = 0.f, dsig = 0.f;
+    const float sig = in_sig, dsig = in_dsig;
     if (half == 0) {
 #pragma unroll
       for (int j = 0; j < 16; ++j) v[j] = 0.f;
-      if (valid) {
-#pragma unroll
-        for (int c = 0; c < 3; ++c) {
-          const float col = ws.rgb[3 * s + c];
-          v[c] = ws.drgb[3 * s + c] * col * (1.f - col) * scale;
-        }
-        sig = ws.sigma[s];
-        dsig = ws.dsigma[s];
-      }
+      v[0] = in_dc[0]; v[1] = in_dc[1]; v[2] = in_dc[2];
       emit16<T, false>(v, bufY(), nullptr, row, 0, true);
     }
     wait_x();
-    uint32_t mask = row_mask32<T>(bufX(), row, cb);
+    uint32_t mask = 0;   // ReLU mask of the item's saved activation: needed by the NEXT item's dY, read under this item's MMAs
     BWD_ITEM(issue_wgrad(tmem_base + GW_C3, sX(), sY(), 16, fmt, acc),
-             issue_layer(tmem_base + COL_G, sY(), sW + WImg::b_c3, 16, H, H, fmt, bar_mma));
+             issue_layer(tmem_base + COL_G, sY(), sW + WImg::b_c3, 16, H, H, fmt, bar_mma),
+             mask = row_mask32<T>(bufX(), row, cb));
     // ---- second colour hidden layer
     if (two) {
       masked_to_Y<T>(tlane, mask, bufY(), row, cb);
       wait_x();
-      mask = row_mask32<T>(bufX(), row, cb);
       BWD_ITEM(issue_wgrad(tmem_base + GW_C2, sX(), sY(), H, fmt, acc),
-               issue_layer(tmem_base + COL_G, sY(), sW + WImg::b_c2, H, H, H, fmt, bar_mma));
+               issue_layer(tmem_base + COL_G, sY(), sW + WImg::b_c2, H, H, H, fmt, bar_mma),
+               mask = row_mask32<T>(bufX(), row, cb));
     }
     // ---- first colour layer: dY = d h1 (masked); X = [g slice, Y(d), 0]; wgrad transposed: G^T = dY^T X
     masked_to_Y<T>(tlane, mask, bufY(), row, cb);
     wait_x();
     BWD_ITEM(issue_wgrad(tmem_base + GW_C1T, sY(), sX(), CIP, fmt, acc),
-             issue_layer(tmem_base + COL_G, sY(), sW + WImg::b_c1, H, CIP, CIP, fmt, bar_mma));
+             issue_layer(tmem_base + COL_G, sY(), sW + WImg::b_c1, H, CIP, CIP, fmt, bar_mma), (void)0);
     // ---- density output layer: dg = [geo slice of d ci] + e_0 * dL/dsigma * sigma (0 where clamped)
     if (half == 0) {
       float dci[CIP], dg[16];
@@ -686,14 +698,14 @@ __global__ void __launch_bounds__(BWD_THREADS, 2) mlp_backward_tc_kernel(MlpShap
       emit16<T, false>(dg, bufY(), nullptr, row, 0, true);
     }
     wait_x();
-    mask = row_mask32<T>(bufX(), row, cb);
     BWD_ITEM(issue_wgrad(tmem_base + GW_D2, sX(), sY(), 16, fmt, acc),
-             issue_layer(tmem_base + COL_G, sY(), sW + WImg::b_d2, 16, H, H, fmt, bar_mma));
+             issue_layer(tmem_base + COL_G, sY(), sW + WImg::b_d2, 16, H, H, fmt, bar_mma),
+             mask = row_mask32<T>(bufX(), row, cb));
     // ---- density hidden layer: dY = d hd (masked); X = e
     masked_to_Y<T>(tlane, mask, bufY(), row, cb);
     wait_x();
     BWD_ITEM(issue_wgrad(tmem_base + GW_D1, sX(), sY(), H, fmt, acc),
-             issue_layer(tmem_base + COL_G, sY(), sW + WImg::b_d1, H, LF, LF, fmt, bar_mma));
+             issue_layer(tmem_base + COL_G, sY(), sW + WImg::b_d1, H, LF, LF, fmt, bar_mma), fetch_inputs(tile + gridDim.x));
     // ---- dL/de -> planes; the two column halves take the 16-column chunks of the LF columns alternately
     for (uint32_t c0 = half * 16; c0 < LF; c0 += 32) {
       tmem_ld16(tlane + COL_G + c0, v);
