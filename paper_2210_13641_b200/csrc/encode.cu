@@ -115,16 +115,39 @@ __global__ void __launch_bounds__(256) encode_forward_kernel(LevelTable lv, cons
       // two-term tile: [hi: LF*256 bytes][lo: LF*256 bytes] per 128-sample tile (e = hi + lo)
       const size_t half = (size_t)LF * NSM_TILE * 2;
       uint8_t *dst = ws.blob_e + (s >> 7) * (2 * half) + (c >> 3) * (NSM_TILE * 16) + (s & 127) * 16 + (c & 7) * 2;
+      // the F columns of the level are adjacent 16-bit elements of one panel row: one store per term (F = 2: 4 bytes)
+      uint16_t hi16[F], lo16[F];
 #pragma unroll
       for (int f = 0; f < F; ++f) {
         if (MODE == 1) {
           const __half hi = __float2half_rn(acc[f]);
-          reinterpret_cast<__half *>(dst)[f] = hi;
-          reinterpret_cast<__half *>(dst + half)[f] = __float2half_rn(acc[f] - __half2float(hi));
+          hi16[f] = __half_as_ushort(hi);
+          lo16[f] = __half_as_ushort(__float2half_rn(acc[f] - __half2float(hi)));
         } else {
           const __nv_bfloat16 hi = __float2bfloat16_rn(acc[f]);
-          reinterpret_cast<__nv_bfloat16 *>(dst)[f] = hi;
-          reinterpret_cast<__nv_bfloat16 *>(dst + half)[f] = __float2bfloat16_rn(acc[f] - __bfloat162float(hi));
+          hi16[f] = __bfloat16_as_ushort(hi);
+          lo16[f] = __bfloat16_as_ushort(__float2bfloat16_rn(acc[f] - __bfloat162float(hi)));
+        }
+      }
+      if constexpr (F == 1) {
+        *reinterpret_cast<uint16_t *>(dst) = hi16[0];
+        *reinterpret_cast<uint16_t *>(dst + half) = lo16[0];
+      } else {
+        uint32_t hw[F / 2], lw[F / 2];
+#pragma unroll
+        for (int i = 0; i < F / 2; ++i) {
+          hw[i] = (uint32_t)hi16[2 * i] | ((uint32_t)hi16[2 * i + 1] << 16);
+          lw[i] = (uint32_t)lo16[2 * i] | ((uint32_t)lo16[2 * i + 1] << 16);
+        }
+        if constexpr (F == 2) {
+          *reinterpret_cast<uint32_t *>(dst) = hw[0];
+          *reinterpret_cast<uint32_t *>(dst + half) = lw[0];
+        } else if constexpr (F == 4) {
+          *reinterpret_cast<uint2 *>(dst) = make_uint2(hw[0], hw[1]);
+          *reinterpret_cast<uint2 *>(dst + half) = make_uint2(lw[0], lw[1]);
+        } else {
+          *reinterpret_cast<uint4 *>(dst) = make_uint4(hw[0], hw[1], hw[2], hw[3]);
+          *reinterpret_cast<uint4 *>(dst + half) = make_uint4(lw[0], lw[1], lw[2], lw[3]);
         }
       }
     }
