@@ -155,6 +155,125 @@ __global__ void __launch_bounds__(256) encode_forward_kernel(LevelTable lv, cons
   tl_mark(ws.timeline, K_ENCODE, 1);
 }
 
+// The same for the tensor-core path, one thread per (PANEL of 8 columns, sample): the 8 / F levels whose features fill one
+// 8-column panel of the operand tile.  The thread then owns a whole 16-byte panel row chunk of the hi and of the lo tile:
+// a warp writes 512 contiguous bytes per store instead of 4-byte pieces at a 16-byte stride (partial-sector writes were
+// what the L2 spent its time on: one store per term and level took config 3's encoder from 200.8 to 175.1 us, this
+// mapping to 155.4 us), and the sample position is loaded once per panel.  Items are panel-major, 256 per chunk, in
+// order.  launch_encode picks between the two mappings.
+template <int F, int MODE>
+__global__ void __launch_bounds__(256) encode_forward_panel_kernel(LevelTable lv, const float *__restrict__ theta, Workspace ws,
+                                                                   const uint32_t *__restrict__ d_S, uint32_t seq) {
+  static_assert(MODE == 1 || MODE == 2, "operand-tile output only");
+  constexpr int LPG = 8 / F;                       // levels per panel
+  __shared__ uint32_t chunk_s;
+  pdl_wait();
+  pdl_trigger();
+  tl_mark(ws.timeline, K_ENCODE, 0);
+  const uint64_t S = *d_S;
+  const uint64_t S_it = ((S + NSM_TILE - 1) / NSM_TILE) * NSM_TILE;     // whole tiles: rows beyond S are zero-filled
+  const uint32_t LF = lv.n_levels * F, n_panels = LF / 8;               // LF is a multiple of 16 on this path
+  const uint64_t total = S_it * n_panels;
+  const uint64_t pol_first = l2_evict_first(), pol_normal = l2_evict_normal();
+  const uint32_t lane = threadIdx.x & 31;
+  const size_t half = (size_t)LF * NSM_TILE * 2;   // two-term tile: [hi: LF*256 bytes][lo: LF*256 bytes] per 128-sample tile
+  ChunkQueue q(ws.work_ctr, seq);
+  for (;;) {
+    const uint64_t cb = q.next(&chunk_s);
+    if (cb >= total) break;                        // block-uniform
+    const uint64_t wi = cb + threadIdx.x;          // S_it is a multiple of 128: a warp never straddles two panels
+    if (wi >= total) continue;                     // (total is a multiple of 128 too: warp-uniform)
+    const uint32_t g = (uint32_t)(wi / S_it);
+    const uint64_t s = wi - (uint64_t)g * S_it;
+    const bool live = s < S;
+    float x0 = 0.f, x1 = 0.f, x2 = 0.f;
+    if (live) { x0 = ws.s_x[s]; x1 = ws.s_x[ws.cap + s]; x2 = ws.s_x[2 * ws.cap + s]; }
+    uint32_t hw[4] = {0u, 0u, 0u, 0u}, lw[4] = {0u, 0u, 0u, 0u};        // the 8 columns of the panel row, hi and lo terms
+#pragma unroll
+    for (int j = 0; j < LPG; ++j) {
+      const uint32_t l = g * LPG + j;              // warp-uniform
+      float acc[F];
+#pragma unroll
+      for (int f = 0; f < F; ++f) acc[f] = 0.0f;
+      const bool dense = lv.dense[l];
+      CornerIndex ci;
+      if (live) ci = corner_index(lv, l, x0, x1, x2);
+      // dense (coarse) level: only the first lane of each run of equal cells gathers, the run takes the corners by shuffle
+      uint32_t head_lane = lane;
+      bool gathers = live;
+      if (dense) {
+        const uint32_t key = live ? ci.slot[0] : 0xffffffffu - lane;
+        const uint32_t prev = __shfl_up_sync(0xffffffffu, key, 1);
+        const uint32_t heads = __ballot_sync(0xffffffffu, lane == 0 || key != prev);
+        head_lane = 31u - (uint32_t)__clz(heads & (0xffffffffu >> (31u - lane)));
+        gathers = live && head_lane == lane;
+      }
+      float v[8][F];
+#pragma unroll
+      for (int k = 0; k < 8; ++k)
+#pragma unroll
+        for (int f = 0; f < F; ++f) v[k][f] = 0.f;
+      if (gathers) {
+        const float *tab = theta + lv.offset[l] * F;
+        const uint64_t pol = dense ? pol_normal : pol_first;
+        if constexpr (F == 2) {
+          const uint64_t e_l = lv.offset[l];
+#pragma unroll
+          for (int k = 0; k < 8; k += 2) {
+            const uint64_t a0 = e_l + ci.slot[k], a1 = e_l + ci.slot[k + 1];
+            if ((a0 ^ a1) == 1ull) {
+              const float4 qv = ld_hint_f4(theta + (a0 & ~1ull) * 2, pol);
+              const bool odd = a0 & 1ull;
+              v[k][0] = odd ? qv.z : qv.x; v[k][1] = odd ? qv.w : qv.y;
+              v[k + 1][0] = odd ? qv.x : qv.z; v[k + 1][1] = odd ? qv.y : qv.w;
+            } else {
+              load_entry_hint<2>(tab + (size_t)ci.slot[k] * 2, v[k], pol);
+              load_entry_hint<2>(tab + (size_t)ci.slot[k + 1] * 2, v[k + 1], pol);
+            }
+          }
+        } else {
+#pragma unroll
+          for (int k = 0; k < 8; ++k) load_entry_hint<F>(tab + (size_t)ci.slot[k] * F, v[k], pol);
+        }
+      }
+      if (dense) {
+#pragma unroll
+        for (int k = 0; k < 8; ++k)
+#pragma unroll
+          for (int f = 0; f < F; ++f) v[k][f] = __shfl_sync(0xffffffffu, v[k][f], head_lane);
+      }
+      if (live) {
+#pragma unroll
+        for (int k = 0; k < 8; ++k) {
+          const float om = corner_weight(k, ci.w);
+#pragma unroll
+          for (int f = 0; f < F; ++f) acc[f] = fmaf(om, v[k][f], acc[f]);
+        }
+      }
+#pragma unroll
+      for (int f = 0; f < F; ++f) {
+        uint32_t h16, l16;
+        if (MODE == 1) {
+          const __half hi = __float2half_rn(acc[f]);
+          h16 = __half_as_ushort(hi);
+          l16 = __half_as_ushort(__float2half_rn(acc[f] - __half2float(hi)));
+        } else {
+          const __nv_bfloat16 hi = __float2bfloat16_rn(acc[f]);
+          h16 = __bfloat16_as_ushort(hi);
+          l16 = __bfloat16_as_ushort(__float2bfloat16_rn(acc[f] - __bfloat162float(hi)));
+        }
+        const int col = j * F + f;                 // column inside the panel, compile-time
+        hw[col >> 1] |= h16 << ((col & 1) * 16);
+        lw[col >> 1] |= l16 << ((col & 1) * 16);
+      }
+    }
+    uint8_t *dst = ws.blob_e + (s >> 7) * (2 * half) + (size_t)g * (NSM_TILE * 16) + (s & 127) * 16;
+    *reinterpret_cast<uint4 *>(dst) = make_uint4(hw[0], hw[1], hw[2], hw[3]);
+    *reinterpret_cast<uint4 *>(dst + half) = make_uint4(lw[0], lw[1], lw[2], lw[3]);
+  }
+  tl_mark(ws.timeline, K_ENCODE, 1);
+}
+
 // S12, thread per (level, sample), level-major (see table_ops.cuh).  On DENSE (coarse) levels consecutive samples of a
 // ray sit in the same cell for several steps (level 0: ~6 samples per cell at config 3), and every sample of a cell adds
 // to the same eight entries: when a warp holds one dense level, the contributions of each run of equal cells are summed
@@ -329,20 +448,33 @@ int launch_unpack_records(const FieldParams &fp, int which, float *dst, cudaStre
 
 template <int F>
 static void launch_encode_f(const LevelTable &lv, const float *theta, const Workspace &ws, const uint32_t *d_S, int out_mode,
-                            dim3 grid, dim3 block, cudaStream_t st, uint32_t seq) {
+                            dim3 grid, dim3 block, cudaStream_t st, uint32_t seq, bool per_panel) {
   if (out_mode == 0) launch_pdl(encode_forward_kernel<F, 0>, grid, block, 0, st, lv, theta, ws, d_S, seq);
-  else if (out_mode == 1) launch_pdl(encode_forward_kernel<F, 1>, grid, block, 0, st, lv, theta, ws, d_S, seq);
-  else launch_pdl(encode_forward_kernel<F, 2>, grid, block, 0, st, lv, theta, ws, d_S, seq);
+  else if (out_mode == 1) {
+    if (per_panel) launch_pdl(encode_forward_panel_kernel<F, 1>, grid, block, 0, st, lv, theta, ws, d_S, seq);
+    else launch_pdl(encode_forward_kernel<F, 1>, grid, block, 0, st, lv, theta, ws, d_S, seq);
+  } else {
+    if (per_panel) launch_pdl(encode_forward_panel_kernel<F, 2>, grid, block, 0, st, lv, theta, ws, d_S, seq);
+    else launch_pdl(encode_forward_kernel<F, 2>, grid, block, 0, st, lv, theta, ws, d_S, seq);
+  }
 }
 
 int launch_encode(const LevelTable &lv, const float *theta, const Workspace &ws, const uint32_t *d_S, int out_mode,
-                  int n_sms, cudaStream_t st, uint32_t seq) {
+                  int n_sms, cudaStream_t st, uint32_t seq, uint64_t max_samples) {
   dim3 grid(n_sms * 8), block(256);
+  // Which mapping (measured on B200, profiles/r2g): a thread per (panel, sample) writes whole 16-byte rows of the operand
+  // tile and wins when the tables fit the L2 and there is enough work to fill the chip with a quarter of the threads
+  // (config 3: 175 -> 155 us, config 5: 12.4 -> 10.4 ms per two views); a thread per (level, sample) keeps the chip inside
+  // one level's slice of tables beyond the L2 (config 4: 159 against 167 us) and has four times the threads when a step
+  // has few samples (config 2, 22 K samples: 19.4 against 22.5 us).  S itself is only known on the device: the switch
+  // uses the step's upper bound, rays x candidates.
+  const bool l2_resident = lv.offset[lv.n_levels] * lv.n_features * sizeof(float) <= (96ull << 20);
+  const bool per_panel = out_mode != 0 && l2_resident && max_samples >= (1ull << 20);
   switch (lv.n_features) {
-    case 1: launch_encode_f<1>(lv, theta, ws, d_S, out_mode, grid, block, st, seq); break;
-    case 2: launch_encode_f<2>(lv, theta, ws, d_S, out_mode, grid, block, st, seq); break;
-    case 4: launch_encode_f<4>(lv, theta, ws, d_S, out_mode, grid, block, st, seq); break;
-    default: launch_encode_f<8>(lv, theta, ws, d_S, out_mode, grid, block, st, seq); break;
+    case 1: launch_encode_f<1>(lv, theta, ws, d_S, out_mode, grid, block, st, seq, per_panel); break;
+    case 2: launch_encode_f<2>(lv, theta, ws, d_S, out_mode, grid, block, st, seq, per_panel); break;
+    case 4: launch_encode_f<4>(lv, theta, ws, d_S, out_mode, grid, block, st, seq, per_panel); break;
+    default: launch_encode_f<8>(lv, theta, ws, d_S, out_mode, grid, block, st, seq, per_panel); break;
   }
   return 1;
 }

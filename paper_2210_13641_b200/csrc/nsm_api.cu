@@ -311,7 +311,8 @@ nsm_status enqueue_forward(nsm_field *f, const nsm_ray_batch *b, uint32_t R, boo
     RUN(f, K_MARCH, launch_march(mp, f->occ_full ? nullptr : f->fp.occ_bits, b->origins, b->dirs, f->ws, train ? 1 : 0, f->stream, dirs_copy));
   }
   const int bf16 = f->cfg.mlp_precision == NSM_MLP_BF16;
-  RUN(f, K_ENCODE, launch_encode(f->lv, f->fp.theta, f->ws, d_S, f->use_tc ? 1 + bf16 : 0, f->n_sms, f->stream, f->work_seq++));
+  RUN(f, K_ENCODE, launch_encode(f->lv, f->fp.theta, f->ws, d_S, f->use_tc ? 1 + bf16 : 0, f->n_sms, f->stream, f->work_seq++,
+                                 (uint64_t)R * b->n_candidates));
   if (f->use_tc)
     RUN(f, K_MLP_FWD, launch_mlp_forward_tc(f->ms, bf16, mlp_dirs, f->ws, d_S, 0, train ? 1 : 0, f->n_sms, f->stream));
   else
@@ -731,7 +732,7 @@ nsm_status nsm_update_occupancy(nsm_field *f, nsm_occ_mode mode, const uint8_t *
         const uint64_t n = (G3 - first < chunk) ? G3 - first : chunk;
         RUN(f, K_OCC, launch_occ_cells(f->cfg.occ_res, occ_cascades(f), first, 1, n, f->ws, d_S, f->stream));
         RUN(f, K_ENCODE, launch_encode(f->lv, f->fp.theta, f->ws, d_S, f->use_tc ? 1 + (f->cfg.mlp_precision == NSM_MLP_BF16) : 0,
-                                       f->n_sms, f->stream, f->work_seq++));
+                                       f->n_sms, f->stream, f->work_seq++, n));
         if (f->use_tc)
           RUN(f, K_MLP_FWD, launch_mlp_forward_tc(f->ms, f->cfg.mlp_precision == NSM_MLP_BF16, nullptr, f->ws, d_S, 1, 0, f->n_sms,
                                                   f->stream));
@@ -769,7 +770,7 @@ nsm_status nsm_update_occupancy_decay(nsm_field *f, uint32_t n_subsets, float de
     const uint64_t n = (n_vis - j0 < chunk) ? n_vis - j0 : chunk;
     const uint64_t first = c0 + j0 * n_subsets;
     RUN(f, K_OCC, launch_occ_cells(f->cfg.occ_res, occ_cascades(f), first, n_subsets, n, f->ws, d_S, f->stream));
-    RUN(f, K_ENCODE, launch_encode(f->lv, f->fp.theta, f->ws, d_S, f->use_tc ? 1 + bf16 : 0, f->n_sms, f->stream, f->work_seq++));
+    RUN(f, K_ENCODE, launch_encode(f->lv, f->fp.theta, f->ws, d_S, f->use_tc ? 1 + bf16 : 0, f->n_sms, f->stream, f->work_seq++, n));
     if (f->use_tc)
       RUN(f, K_MLP_FWD, launch_mlp_forward_tc(f->ms, bf16, nullptr, f->ws, d_S, 1, 0, f->n_sms, f->stream));
     else
@@ -798,7 +799,7 @@ nsm_status nsm_update_occupancy_stochastic(nsm_field *f, uint32_t n_draws, float
   for (uint32_t i0 = 0; i0 < n_draws; i0 += chunk) {
     const uint32_t n = n_draws - i0 < chunk ? n_draws - i0 : chunk;
     RUN(f, K_OCC, launch_occ_cells_stochastic(f->cfg.occ_res, occ_cascades(f), f->cfg.seed, f->occ_draws, i0, n, f->ws, d_S, f->stream));
-    RUN(f, K_ENCODE, launch_encode(f->lv, f->fp.theta, f->ws, d_S, f->use_tc ? 1 + bf16 : 0, f->n_sms, f->stream, f->work_seq++));
+    RUN(f, K_ENCODE, launch_encode(f->lv, f->fp.theta, f->ws, d_S, f->use_tc ? 1 + bf16 : 0, f->n_sms, f->stream, f->work_seq++, n));
     if (f->use_tc)
       RUN(f, K_MLP_FWD, launch_mlp_forward_tc(f->ms, bf16, nullptr, f->ws, d_S, 1, 0, f->n_sms, f->stream));
     else

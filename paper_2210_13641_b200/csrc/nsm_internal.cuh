@@ -285,8 +285,9 @@ int launch_march(const MarchParams &mp, const uint8_t *bits, const float *origin
 uint32_t march_scan_state_entries(uint32_t max_rays);
 // out_mode: 0 = fp32 planes ws.e, 1 = fp16 blob ws.blob_e, 2 = bf16 blob ws.blob_e
 // seq: launch sequence number of the field's table kernels (selects the ChunkQueue counter)
+// max_samples: an upper bound on S known to the host (rays x candidates, cells of a refresh chunk): picks the work mapping
 int launch_encode(const LevelTable &lv, const float *theta, const Workspace &ws,
-                  const uint32_t *d_S, int out_mode, int n_sms, cudaStream_t st, uint32_t seq);
+                  const uint32_t *d_S, int out_mode, int n_sms, cudaStream_t st, uint32_t seq, uint64_t max_samples);
 // S12 over all levels: vector reductions into grad
 int launch_scatter(const LevelTable &lv, float *grad, const Workspace &ws, const uint32_t *d_S, int n_sms, cudaStream_t st,
                    uint32_t seq);

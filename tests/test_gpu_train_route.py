@@ -184,19 +184,22 @@ def test_config3_free_running_loss_curve(nsm):
     f.close()
 
 
-@pytest.mark.parametrize("L,F,layers,precision,R", [(8, 2, 2, 1, 700), (12, 4, 1, 2, 300), (16, 4, 1, 1, 2100), (16, 2, 1, 1, 1)])
-def test_tensor_core_mlp_shapes_outside_the_configurations(nsm, L, F, layers, precision, R):
+@pytest.mark.parametrize("L,F,layers,precision,R,K", [(8, 2, 2, 1, 700, 128), (12, 4, 1, 2, 300, 128), (16, 4, 1, 1, 2100, 128),
+                                                       (16, 2, 1, 1, 1, 128), (16, 1, 2, 1, 4096, 256), (2, 8, 2, 2, 4096, 256),
+                                                       (12, 4, 1, 1, 4096, 256), (8, 2, 1, 2, 4096, 256)])
+def test_tensor_core_mlp_shapes_outside_the_configurations(nsm, L, F, layers, precision, R, K):
     """The tcgen05 kernels accept encoder widths L F = 16 .. 64 in steps of 16 and one or two hidden colour layers; the five
     configurations only exercise (32, two layers, fp16) and (64, two layers, bf16).  Backward parity (P1-P4) and one
     nsm_train_step (m, v against the oracle) for L F = 16, 48 and 64, ONE hidden colour layer (the backward kernel then
     skips an item of its activation ring), both 16-bit formats, and sample counts that leave tiles ragged, groups of
-    the forward kernel idle (fewer tiles than pipelines), or nearly empty (a single ray)."""
+    the forward kernel idle (fewer tiles than pipelines), or nearly empty (a single ray).  The cases with 4096 rays x 256
+    candidates (>= 2^20) take the encoder's thread-per-panel mapping, for every feature width F = 1, 2, 4, 8."""
     from tests.test_gpu_parity import check_backward
     w = configs.config2(n_batches=2)
     fc = replace(w.field, n_levels=L, n_features=F, color_hidden_layers=layers, mlp_precision=precision, n_max=512,
-                 log2_table_size=14)
+                 log2_table_size=14, max_candidates=K)
     bs = [replace(b, origins=b.origins[:R].copy(), dirs=b.dirs[:R].copy(), rgb=b.rgb[:R].copy(), depth=b.depth[:R].copy(),
-                  depth_var=b.depth_var[:R].copy()) for b in w.batches]
+                  depth_var=b.depth_var[:R].copy(), n_candidates=K) for b in w.batches]
     w = replace(w, field=fc, batches=bs)
     f, O, _ = make_pair(nsm, w, seed=40 + L, table_scale=0.05, omp=True)
     assert f.nsm_mlp_path() == ("tcgen05_f16" if precision == 1 else "tcgen05_bf16")
@@ -209,5 +212,5 @@ def test_tensor_core_mlp_shapes_outside_the_configurations(nsm, L, F, layers, pr
     f.nsm_train_step(nsm.DeviceBatch(bs[1]), w.lambda_d, want_stats=False)
     _, tr = O.train_step(bs[1], w.lambda_d, trace=("grad", "touched"))
     if so["n_samples"] > 64:
-        check_step_parameters(f, O, before, tr["grad"], tr["touched"], tol, f"L{L} F{F} layers{layers} prec{precision} R{R}")
+        check_step_parameters(f, O, before, tr["grad"], tr["touched"], tol, f"L{L} F{F} layers{layers} prec{precision} R{R} K{K}")
     f.close()
