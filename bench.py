@@ -478,7 +478,10 @@ def measure_training(cfg, K, W, env, want_sampled=False, want_pose=False):
                 # what bounds S4 / S12 while the tables fit the L2: its random-access rate (8 corners per sample and level)
                 acc = 8 * L * S_avg / avg_s
                 pk = l2["gathers_per_s"] if name == "encode" else l2["reductions_per_s"]
-                k["l2_random"] = dict(achieved_accesses_per_s=acc, peak_accesses_per_s=pk, frac=acc / pk)
+                k["l2_random"] = dict(achieved_accesses_per_s=acc, peak_accesses_per_s=pk, frac=acc / pk,
+                                      note="corner REFERENCES per second (8 per sample and level) against the probe's rate of physical "
+                                           "L2 accesses: x-neighbour pairs share one access and runs of samples in one coarse cell are "
+                                           "merged, so the ratio can exceed 1")
             kernels.append(k)
         kernels.sort(key=lambda k: -k["share_of_serialised_pass"])
         top = kernels[0]
