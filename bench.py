@@ -274,6 +274,47 @@ def probe_l2(dev_index):
         return dict(error=repr(e))
 
 
+def probe_mma():
+    """Cycles per small tcgen05.mma (M = 128, K = 16) in a stream of 48 at N = 16 / 32 / 48 / 64, and the issue-to-completion
+    latency of a single one, measured now by libnsm_bench_probe.so: the MLP kernels' bound (profiles/r2d)."""
+    path = os.path.join(ROOT, "paper_2210_13641_b200", "libnsm_bench_probe.so")
+    try:
+        lib = ctypes.CDLL(path)
+        lib.nsm_bench_probe_mma.argtypes = [ctypes.c_uint32, ctypes.c_uint32, ctypes.POINTER(ctypes.c_longlong)]
+        cyc = ctypes.c_longlong()
+        out = dict(cycles_per_mma={})
+        for N in (16, 32, 48, 64):
+            if lib.nsm_bench_probe_mma(N, 48, ctypes.byref(cyc)) != 0:
+                return dict(error="nsm_bench_probe_mma failed")
+            out["cycles_per_mma"][N] = cyc.value / 48.0
+        if lib.nsm_bench_probe_mma(64, 1, ctypes.byref(cyc)) != 0:
+            return dict(error="nsm_bench_probe_mma failed")
+        out["single_mma_cycles"] = int(cyc.value)
+        out["how"] = ("libnsm_bench_probe.so: one CTA, an elected lane issues 48 (1) tcgen05.mma.cta_group::1.kind::f16 M=128 K=16 and one "
+                      "commit; SM cycles from the first issue to the mbarrier flip, best of 4, this run")
+        return out
+    except (OSError, AttributeError) as e:
+        return dict(error=repr(e))
+
+
+def mma_dispatch_floor(name, mma, fc, S, n_sms, sm_hz, two_term):
+    """MMA instructions per 128-sample tile of the tcgen05 MLP kernels and the time their dispatch alone takes at the
+    measured rate (one tensor core per SM, tiles spread over n_sms SMs)."""
+    c = lambda N: mma["cycles_per_mma"][min((16, 32, 48, 64), key=lambda n: abs(n - N))]
+    LF = fc.n_levels * fc.n_features
+    two = fc.color_hidden_layers == 2
+    if name == "mlp_fwd":
+        t = 3 if two_term else 1
+        groups = [(t * LF // 16, 64), (t * 4, 16), (t * 2, 64)] + ([(t * 4, 64)] if two else []) + [(t * 4, 16)]
+    else:   # per layer: 8 wgrad k-steps over the 128 samples + the dgrad's K / 16
+        groups = [(8, 16), (1, 64)] + ([(8, 64), (4, 64)] if two else []) + [(8, 32), (4, 32), (8, 16), (1, 64), (8, 64), (4, LF)]
+    n = sum(g[0] for g in groups)
+    cycles = sum(g[0] * c(g[1]) for g in groups)
+    tiles = -(-int(S) // 128)
+    floor_s = -(-tiles // n_sms) * cycles / sm_hz
+    return dict(mmas_per_tile=n, dispatch_cycles_per_tile=cycles, tiles=tiles, floor_us=1e6 * floor_s)
+
+
 class Timer:
     def __init__(self, torch, dev, replicas):
         self.torch, self.dev, self.replicas = torch, dev, replicas
@@ -474,6 +515,12 @@ def measure_training(cfg, K, W, env, want_sampled=False, want_pose=False):
                 k.update(achieved=model["flops"] / avg_s / 1e12 if avg_s > 0 else 0.0, unit="TFLOP/s", peak=peak,
                          algorithmic_flops=model["flops"])
             k["frac"] = k["achieved"] / k["peak"]
+            if name in ("mlp_fwd", "mlp_bwd") and k["bound"] == "tensor" and "error" not in env["mma"] and avg_s > 0:
+                # what bounds these kernels: the dispatch rate of their small MMAs (measured in this run), not tensor math
+                d = mma_dispatch_floor(name, env["mma"], fc, S_avg, torch.cuda.get_device_properties(dev).multi_processor_count,
+                                       1e6 * ((clocks or {}).get("sm_mhz") or 1965.0), two_term=True)
+                d["frac_of_floor"] = d["floor_us"] / (1e6 * avg_s)
+                k["mma_dispatch"] = d
             if name in ("encode", "scatter") and avg_s > 0 and "error" not in l2:
                 # what bounds S4 / S12 while the tables fit the L2: its random-access rate (8 corners per sample and level)
                 acc = 8 * L * S_avg / avg_s
@@ -587,7 +634,8 @@ def run_cuda(args):
     dev = torch.device("cuda", local_rank if world > 1 else 0)
     torch.cuda.set_device(dev)
     env = dict(torch=torch, nsm=nsm, replicas=replicas, dev=dev, rank=rank, world=world, peaks=measured_peaks(),
-               l2=probe_l2(dev.index) if rank == 0 else dict(error="rank != 0"))
+               l2=probe_l2(dev.index) if rank == 0 else dict(error="rank != 0"),
+               mma=probe_mma() if rank == 0 else dict(error="rank != 0"))
     t_all = time.perf_counter()
     head_cfg = args.config or HEADLINE
     K, W = args.steps, max(args.warmup, 3)
@@ -613,6 +661,7 @@ def run_cuda(args):
             if k in head:
                 line[k] = head[k]
         line["l2_probe"] = env["l2"]
+        line["mma_probe"] = env["mma"]
         line["peaks"] = env["peaks"]
         if subs:
             line["configs"] = subs

@@ -10,6 +10,7 @@ CSRC = os.path.join(HERE, "csrc")
 OUT = os.path.join(HERE, "libnsm.so")
 # bench-only micro-benchmark (csrc/bench_probe/): its own shared object, loaded by bench.py only; not in include/nsm.h
 PROBE_SRC = os.path.join(CSRC, "bench_probe", "l2_probe.cu")
+PROBE_SRCS = [PROBE_SRC, os.path.join(CSRC, "bench_probe", "mma_probe.cu")]
 PROBE_OUT = os.path.join(HERE, "libnsm_bench_probe.so")
 BUILD = os.path.join(HERE, "build")
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
@@ -27,10 +28,11 @@ def _deps_mtime():
 
 
 def build_probe(force=False):
-    if not force and os.path.exists(PROBE_OUT) and os.path.getmtime(PROBE_OUT) >= os.path.getmtime(PROBE_SRC):
+    newest = max(os.path.getmtime(p) for p in PROBE_SRCS + [os.path.join(CSRC, "tc_common.cuh")])
+    if not force and os.path.exists(PROBE_OUT) and os.path.getmtime(PROBE_OUT) >= newest:
         return PROBE_OUT
     cmd = [NVCC, "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-std=c++17", "-lineinfo", "-Xcompiler", "-fPIC", "-shared",
-           PROBE_SRC, "-o", PROBE_OUT + ".tmp", "-lcudart"]
+           *PROBE_SRCS, "-o", PROBE_OUT + ".tmp", "-lcudart"]
     r = subprocess.run(cmd, capture_output=True, text=True)
     if r.returncode != 0:
         raise RuntimeError(f"nvcc failed on {PROBE_SRC}:\n{r.stdout}\n{r.stderr}")
