@@ -606,8 +606,52 @@ def measure_render(K, W, env):
         prof = f.nsm_profile_read()
         f.nsm_profile(False)
         total_ms = sum(ms for ms, n in prof.values())
-        kernels = sorted([dict(kernel=k, total_ms=ms, launches=n, share_of_serialised_pass=ms / total_ms) for k, (ms, n) in prof.items() if n],
-                         key=lambda k: -k["share_of_serialised_pass"])
+        n_prof_views = min(K, 2)
+        # live samples of one view (S is a device-side count per ray chunk): view 0 rendered chunk by chunk, counts read back
+        M = fc.max_rays
+        S_view = 0
+        for a in range(0, n_rays, M):
+            part = configs.RayBatch(hv[0].origins[a:a + M], hv[0].dirs[a:a + M], None, None, None, hv[0].t_min, hv[0].t_max, hv[0].n_candidates)
+            f.nsm_render(nsm.DeviceBatch(part, dev), 1e-4)
+            S_view += int(f.nsm_debug_last_step("counts").sum())
+        L, F, mac = fc.n_levels, fc.n_features, f.n_mlp
+        kernels = []
+        for kname, (ms, n) in prof.items():
+            if n == 0:
+                continue
+            per_view_s = ms * 1e-3 / n_prof_views
+            k = dict(kernel=kname, total_ms=ms, launches=n, us_per_view=1e6 * per_view_s, share_of_serialised_pass=ms / total_ms)
+            if kname == "encode":
+                nbytes = 8 * L * F * 4 * S_view + 12 * S_view + 4 * L * F * S_view
+                k.update(bound="hbm", algorithmic_bytes=nbytes, achieved=nbytes / per_view_s / 1e9, unit="GB/s", peak=peaks["hbm_gbs"])
+                k["frac"] = k["achieved"] / k["peak"]
+                if "error" not in l2:
+                    acc = 8 * L * S_view / per_view_s
+                    k["l2_random"] = dict(achieved_accesses_per_s=acc, peak_accesses_per_s=l2["gathers_per_s"], frac=acc / l2["gathers_per_s"],
+                                          note="corner references per second against the probe's rate of physical L2 accesses (pairs and "
+                                               "runs of equal coarse cells are merged: the ratio can exceed 1)")
+            elif kname == "mlp_fwd":
+                flops = 2 * mac * S_view
+                k.update(bound="tensor", algorithmic_flops=flops, achieved=flops / per_view_s / 1e12, unit="TFLOP/s", peak=peaks["bf16_tflops"])
+                k["frac"] = k["achieved"] / k["peak"]
+                if "error" not in env["mma"]:
+                    # 13 launches per view, each spreading its own tiles over the SMs: the floor is summed per launch
+                    d = mma_dispatch_floor("mlp_fwd", env["mma"], fc, S_view / max(n / n_prof_views, 1),
+                                           torch.cuda.get_device_properties(dev).multi_processor_count,
+                                           1e6 * ((clocks or {}).get("sm_mhz") or 1965.0), two_term=False)
+                    d["floor_us"] *= n / n_prof_views
+                    d["frac_of_floor"] = d["floor_us"] / (1e6 * per_view_s)
+                    k["mma_dispatch"] = d
+            kernels.append(k)
+        kernels.sort(key=lambda k: -k["share_of_serialised_pass"])
+        top = kernels[0]
+        roofline = None
+        if "achieved" in top:
+            roofline = dict(kernel=top["kernel"], bound=top["bound"], achieved=top["achieved"], peak=top["peak"], unit=top["unit"],
+                            frac=top["frac"], traffic=None, us_per_view=top["us_per_view"],
+                            share_of_serialised_pass=top["share_of_serialised_pass"], samples_per_view=S_view,
+                            algorithmic=f"SURVEY.md 8(d) gather bytes x S = {S_view} live samples of one view (all evaluated: the "
+                                        "transmittance cut is applied in the compositor)", peak_source=peaks["source"])
         theta = f.nsm_get_params()[0]
         cpu = oracle_render_baseline(fc, theta, bits, hv[0])
         out = dict(config=dict(workload=WORKLOADS[5], config=5, rays_per_view=n_rays, candidates_per_ray=256, train_steps=train_steps,
@@ -616,7 +660,8 @@ def measure_render(K, W, env):
                    ms_per_step=1e3 * t_max / K, dtype="f16", clocks=clocks,
                    e2e=dict(value=e2e_v, unit="rays/s", h2d_bytes_per_step=hviews[0].bytes_in(), d2h_bytes_per_step=n_rays * 20,
                             ms_per_step=1e3 * t_e2e_max / K, api="nsm_render_host, pinned host rays in, pinned host image out"),
-                   gpu_launches=launches, kernels=kernels, cpu_baseline=cpu)
+                   gpu_launches=launches, samples_per_view=S_view, samples_per_s=rays_s * S_view / n_rays, roofline=roofline,
+                   kernels=kernels, cpu_baseline=cpu)
     f.close()
     replicas.barrier()
     return out
@@ -656,7 +701,8 @@ def run_cuda(args):
         line = dict(metric=head["metric"], value=head["value"], unit=head["unit"], n_gpus=world, steps=head["steps"], warmup=head["warmup"],
                     ms_per_step=head["ms_per_step"], higher_is_better=True, scaling="weak", vs_baseline=None, dtype=head["dtype"],
                     data="synthetic", config=head["config"])
-        for k in ("samples_per_step", "touched_entries", "rays_per_s", "candidates_per_s", "clocks", "e2e", "gpu_launches", "roofline",
+        for k in ("samples_per_step", "touched_entries", "rays_per_s", "candidates_per_s", "samples_per_view", "samples_per_s", "clocks", "e2e",
+                  "gpu_launches", "roofline",
                   "kernels", "cpu_baseline", "occupancy_refresh", "sampled"):
             if k in head:
                 line[k] = head[k]
