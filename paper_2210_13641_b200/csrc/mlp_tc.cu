@@ -260,22 +260,26 @@ constexpr uint32_t TILE_BYTES = ROWS * H * 2;   // one [128][64] 16-bit tile
 
 // One CTA per SM runs FOUR independent tile pipelines ("groups" of 128 threads = 4 warps, one TMEM lane quarter each) that
 // share one copy of the weight images.  Per tile a group walks the five layers as a chain  MMA -> accumulator read-back ->
-// activation -> 16-bit operand tile in shared memory -> next MMA; each link waits on the tensor core or on shared memory,
-// so what keeps the SM busy is the number of chains in flight (round 1 ran two per SM, one per CTA, each CTA with its own
-// 48 KB of weights: tensor pipe 12 % active, a third of all warp samples waiting on the MMA barrier, profiles/r2d).
-//  - ONE activation buffer per group: a layer's output tile is written over its input tile, which is dead once the
-//    layer's MMAs have completed (the group waits on their mbarrier before it reads the accumulator back).
-//  - ONE 64-column accumulator per group, reused by every layer (its previous contents have been read back before
-//    the next layer's MMAs are issued): 4 x 64 = 256 TMEM columns per CTA.
+// activation -> next layer's A operand -> next MMA; each link waits on the tensor core, so what keeps the SM busy is the
+// number of chains in flight (round 1 ran two per SM, one per CTA, each CTA with its own 48 KB of weights: tensor pipe
+// 12 % active, a third of all warp samples waiting on the MMA barrier, profiles/r2d).
+//  - Two-term (training) forward: the activations never touch shared memory: thread r owns sample row r = TMEM lane r, and a K-major A operand in tensor
+//    memory is exactly "lane = row, two 16-bit K elements per 32-bit column" -- so the thread that read its accumulator row
+//    back writes its row of the next layer's A operand (hi and lo terms) straight into TMEM with tcgen05.st, and the
+//    next layer's MMAs take A from TMEM (no st.shared, no proxy fence, no shared-memory read of A by the tensor core).
+//    Only the first layer's A, the encoder tile, comes from shared memory, where TMA puts it.  (Config 3: 66.7 -> 54.3 us.)
+//    The plain forward keeps one in-place shared-memory buffer per group (see emit32).
+//  - 128 TMEM columns per group: a 64-column accumulator reused by every layer (read back before the next layer's MMAs are
+//    issued), 32 columns of A_hi and 32 of A_lo: 4 x 128 = 512 columns per CTA.
 //  - groups synchronise on their own named barrier and mbarriers and drift apart, so one group's read-back and packing
 //    overlap another's MMAs and TMA fetch.
 constexpr uint32_t FWD_GROUPS = 4, FWD_GROUP_THREADS = 128, FWD_THREADS = FWD_GROUPS * FWD_GROUP_THREADS;
-constexpr uint32_t FWD_COLS = 64 * FWD_GROUPS;
+constexpr uint32_t FWD_COLS = 128 * FWD_GROUPS, FWD_COL_AHI = 64, FWD_COL_ALO = 96;
 template <bool SPLIT>
 struct FwdSmem {
   static constexpr uint32_t w = 0;                                          // weight images: hi (WImg forward region), then lo
   static constexpr uint32_t w_bytes = SPLIT ? 2 * WImg::f_total : WImg::f_total;
-  static constexpr uint32_t buf_bytes = SPLIT ? 2 * TILE_BYTES : TILE_BYTES; // hi | lo; also the TMA destination of the encoder tile
+  static constexpr uint32_t buf_bytes = SPLIT ? 2 * TILE_BYTES : TILE_BYTES; // the TMA destination of the encoder tile (hi | lo)
   static constexpr uint32_t buf = w + w_bytes;
   static constexpr uint32_t bar_w = buf + FWD_GROUPS * buf_bytes;
   static constexpr uint32_t bar_mma = bar_w + 8;                            // [FWD_GROUPS]
@@ -293,15 +297,78 @@ __device__ __forceinline__ void issue_fwd(uint32_t tmem_d, uint32_t a, uint32_t 
   if constexpr (SPLIT) issue_layer_split(tmem_d, a, a_lo, b, b_lo, K, N, NP, fmt, bar);
   else issue_layer(tmem_d, a, b, K, N, NP, fmt, bar);
 }
-template <typename T, bool RELU, bool SPLIT>
-__device__ __forceinline__ void emit_fwd(float *v, uint8_t *tile, uint32_t lo_off, uint8_t *blob, uint32_t row, uint32_t c0, bool valid) {
-  if constexpr (SPLIT) emit16s<T, RELU>(v, tile, lo_off, blob, row, c0, valid);
-  else emit16<T, RELU>(v, tile, blob, row, c0, valid);
+// the same with A in tensor memory: D[128 x N] = A[128 x K] * B[N x K]^T, A_hi at ta_hi, A_lo at ta_lo (8 columns per k-step)
+template <bool SPLIT>
+__device__ __forceinline__ void issue_fwd_ts(uint32_t tmem_d, uint32_t ta_hi, uint32_t ta_lo, uint32_t b_saddr, uint32_t b_lo, uint32_t K,
+                                             uint32_t N, uint32_t NP, uint32_t fmt, uint32_t bar) {
+  const uint32_t idesc = make_idesc(fmt, 128, N, 0, 0);
+  const uint64_t db0 = make_desc(b_saddr, NP * 16, 128), sb = (2 * NP * 16) >> 4;
+#pragma unroll
+  for (uint32_t term = 0; term < (SPLIT ? 3u : 1u); ++term) {
+    uint32_t ta = term == 1 ? ta_lo : ta_hi;
+    uint64_t db = db0 + (term == 2 ? (uint64_t)(b_lo >> 4) : 0ull);
+    for (uint32_t k = 0; k < K / 16; ++k) {
+      mma_ts(tmem_d, ta, db, idesc, (term | k) > 0);
+      ta += 8; db += sb;
+    }
+  }
+  mma_commit(bar);
 }
 // barrier of one 128-thread group (barrier 0 is __syncthreads)
 __device__ __forceinline__ void group_bar(uint32_t grp) { asm volatile("bar.sync %0, 128;" ::"r"(grp + 1u) : "memory"); }
 
-// a 64-wide hidden layer's accumulator -> ReLU -> the group's operand tile (in place) and, when saved, its blob tile
+// 32 values of this thread's row (columns c0 .. c0+31 of a layer's output) -> (optional ReLU) -> the next layer's A operand in
+// tensor memory (16 packed columns of A_hi, and of A_lo when SPLIT) and, when saved, the global blob tile (hi term)
+template <typename T, bool RELU, bool SPLIT>
+__device__ __forceinline__ void emit32_tmem(float *v, uint32_t ta_hi, uint32_t ta_lo, uint8_t *blob_tile, uint32_t row, uint32_t c0,
+                                            bool valid) {
+  if (RELU) {
+    // fp16 rounds 0 < h < 2^-25 to zero; the backward pass reads its ReLU mask off the stored value (h > 0), so a positive
+    // activation is raised to at least the smallest fp16 subnormal, 2^-24: the mask is then exactly [pre-activation > 0]
+    constexpr float tiny = (SPLIT && Fmt<T>::id == 0) ? 5.9604644775390625e-08f : 0.f;
+#pragma unroll
+    for (int j = 0; j < 32; ++j) v[j] = v[j] > 0.f ? fmaxf(v[j], tiny) : 0.f;
+  }
+  uint32_t hi[16];
+#pragma unroll
+  for (int j = 0; j < 16; ++j) hi[j] = pack2<T>(v[2 * j], v[2 * j + 1]);
+  tmem_st16(ta_hi + c0 / 2, hi);
+  if constexpr (SPLIT) {
+    uint32_t lo[16];
+#pragma unroll
+    for (int j = 0; j < 16; ++j) {
+      const float2 h = unpack2<T>(hi[j]);
+      lo[j] = pack2<T>(v[2 * j] - h.x, v[2 * j + 1] - h.y);
+    }
+    tmem_st16(ta_lo + c0 / 2, lo);
+  }
+  if (blob_tile) {   // rows of invalid samples are stored as zeros so the backward wgrad never sees garbage
+    const uint4 z = make_uint4(0, 0, 0, 0);
+#pragma unroll
+    for (int p = 0; p < 4; ++p)
+      *reinterpret_cast<uint4 *>(blob_tile + tile_off(ROWS, row, c0 + 8 * p)) =
+          valid ? make_uint4(hi[4 * p], hi[4 * p + 1], hi[4 * p + 2], hi[4 * p + 3]) : z;
+  }
+}
+
+// the plain 16-bit forward keeps its operands in shared memory (one in-place buffer per group): with one MMA group per
+// layer the chain is short and the A-from-TMEM MMAs' longer latency costs more than the shared-memory traffic they save
+// (render: 2.39 ms against 2.81 ms per two views with A in TMEM)
+template <typename T, bool RELU, bool SPLIT>
+__device__ __forceinline__ void emit32(float *v, uint32_t tlane, uint8_t *buf, uint8_t *blob_tile, uint32_t row, uint32_t c0, bool valid) {
+  if constexpr (SPLIT) emit32_tmem<T, RELU, true>(v, tlane + FWD_COL_AHI, tlane + FWD_COL_ALO, blob_tile, row, c0, valid);
+  else {
+    emit16<T, RELU>(v, buf, blob_tile, row, c0, valid);
+    emit16<T, RELU>(v + 16, buf, blob_tile, row, c0 + 16, valid);
+  }
+}
+// what a group does between writing an operand and the barrier before its MMAs
+template <bool SPLIT>
+__device__ __forceinline__ void operand_written() {
+  if constexpr (SPLIT) tmem_st_wait(); else fence_async_smem();
+}
+
+// a 64-wide hidden layer's accumulator -> ReLU -> the next layer's A operand (TMEM) and, when saved, its blob tile
 template <typename T, bool SPLIT>
 __device__ __forceinline__ void hidden_epilogue(uint32_t tlane, uint8_t *buf, uint8_t *blob, uint32_t row, bool valid) {
   float v[32];
@@ -310,9 +377,17 @@ __device__ __forceinline__ void hidden_epilogue(uint32_t tlane, uint8_t *buf, ui
     tmem_ld16(tlane + c0, v);
     tmem_ld16(tlane + c0 + 16, v + 16);
     tmem_ld_wait();
-    emit_fwd<T, true, SPLIT>(v, buf, TILE_BYTES, blob, row, c0, valid);
-    emit_fwd<T, true, SPLIT>(v + 16, buf, TILE_BYTES, blob, row, c0 + 16, valid);
+    emit32<T, true, SPLIT>(v, tlane, buf, blob, row, c0, valid);
   }
+  operand_written<SPLIT>();
+}
+
+// a layer after the first: A from tensor memory (two-term forward) or from the group's shared-memory buffer (plain forward)
+template <bool SPLIT>
+__device__ __forceinline__ void issue_next(uint32_t tcol, uint32_t sBuf, uint32_t b_saddr, uint32_t K, uint32_t N, uint32_t NP,
+                                           uint32_t fmt, uint32_t bar) {
+  if constexpr (SPLIT) issue_fwd_ts<true>(tcol, tcol + FWD_COL_AHI, tcol + FWD_COL_ALO, b_saddr, WImg::f_total, K, N, NP, fmt, bar);
+  else issue_layer(tcol, sBuf, b_saddr, K, N, NP, fmt, bar);
 }
 
 template <typename T, bool SPLIT>
@@ -321,7 +396,7 @@ __global__ void __launch_bounds__(FWD_THREADS, 1) mlp_forward_tc_kernel(MlpShape
                                                                        int save_blobs) {
   using SM = FwdSmem<SPLIT>;
   extern __shared__ __align__(1024) uint8_t smem[];
-  const uint32_t tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+  const uint32_t tid = threadIdx.x, warp = tid >> 5;
   const uint32_t grp = tid >> 7, row = tid & 127u;          // warp & 3 = the TMEM lane quarter of rows 32 (warp & 3) .. +31
   const bool lead_warp = row < 32;                          // the group's first warp: one lane of it issues the MMAs and the TMA
   const uint32_t sbase = smem_u32(smem);
@@ -352,7 +427,7 @@ __global__ void __launch_bounds__(FWD_THREADS, 1) mlp_forward_tc_kernel(MlpShape
   __syncthreads();
   fence_after();
   const uint32_t tmem_base = *reinterpret_cast<volatile uint32_t *>(smem + SM::tmem);
-  const uint32_t tcol = tmem_base + 64u * grp;                        // the group's accumulator columns
+  const uint32_t tcol = tmem_base + 128u * grp;                       // the group's columns: accumulator | A_hi | A_lo
   const uint32_t tlane = tcol + (((warp & 3u) * 32u) << 16);
   uint32_t ph_mma = 0, ph_e = 0;
   const uint32_t fmt = Fmt<T>::id;
@@ -371,7 +446,7 @@ __global__ void __launch_bounds__(FWD_THREADS, 1) mlp_forward_tc_kernel(MlpShape
   for (uint64_t tile = first_tile; tile < n_tiles; tile += tile_stride) {
     const uint64_t s = tile * ROWS + row;
     const bool valid = s < S;
-    // ---- density hidden layer: A = encoder tile (in the buffer via TMA)
+    // ---- density hidden layer: A = encoder tile (in shared memory via TMA)
     if (lead_warp) {
       mbar_wait(bar_e, ph_e);
       fence_after();
@@ -385,23 +460,25 @@ __global__ void __launch_bounds__(FWD_THREADS, 1) mlp_forward_tc_kernel(MlpShape
       dx = __ldg(dirs + 3 * (size_t)ray); dy = __ldg(dirs + 3 * (size_t)ray + 1); dz = __ldg(dirs + 3 * (size_t)ray + 2);
     }
     mbar_wait(bar_mma, ph_mma); ph_mma ^= 1; fence_after();
+    auto fetch_next_e = [&]() {   // the group's next encoder tile
+      const uint64_t nxt = tile + tile_stride;
+      if (lead_warp && nxt < n_tiles && elect_one()) { mbar_expect_tx(bar_e, e_bytes); bulk_g2s(sBuf, ws.blob_e + (size_t)nxt * e_stride, e_bytes, bar_e); }
+    };
+    if constexpr (SPLIT) fetch_next_e();   // only the first layer reads the buffer: it is free as soon as that layer's MMAs are done
     hidden_epilogue<T, SPLIT>(tlane, buf, (save_blobs && !density_only) ? ws.blob_hd + (size_t)tile * (H * ROWS * 2) : nullptr, row, valid);
-    fence_async_smem(); fence_before(); group_bar(grp);
-    if (lead_warp) { fence_after(); if (elect_one()) issue_fwd<SPLIT>(tcol, sBuf, TILE_BYTES, sW + WImg::f_d2, WImg::f_total, H, DO, DO, fmt, bar_mma); }
+    fence_before(); group_bar(grp);
+    if (lead_warp) { fence_after(); if (elect_one()) issue_next<SPLIT>(tcol, sBuf, sW + WImg::f_d2, H, DO, DO, fmt, bar_mma); }
     mbar_wait(bar_mma, ph_mma); ph_mma ^= 1; fence_after();
     float g[16];
     tmem_ld16(tlane, g);
     tmem_ld_wait();
     if (valid) ws.sigma[s] = expf(fminf(fmaxf(g[0], -15.f), 15.f));
     if (density_only) {
-      if (lead_warp) {   // the buffer is free: the group's next encoder tile
-        const uint64_t nxt = tile + tile_stride;
-        if (nxt < n_tiles && elect_one()) { mbar_expect_tx(bar_e, e_bytes); bulk_g2s(sBuf, ws.blob_e + (size_t)nxt * e_stride, e_bytes, bar_e); }
-      }
+      if constexpr (!SPLIT) fetch_next_e();   // (plain forward: the buffer held the hidden activations until now)
       fence_before(); group_bar(grp);   // every read of the accumulator is done before the next tile's MMAs
       continue;
     }
-    // ---- colour input [g slice, Y(d), 0 pad] -> the buffer (K = 32)
+    // ---- colour input [g slice, Y(d), 0 pad] -> A operand (K = 32)
     {
       float ci[CIP];
       // mlp_tc_supported() admits only the slice (geo_offset, geo_count) = (1, 15) with 16 SH terms (configs 2-5):
@@ -413,27 +490,23 @@ __global__ void __launch_bounds__(FWD_THREADS, 1) mlp_forward_tc_kernel(MlpShape
 #pragma unroll
       for (int j = 0; j < 16; ++j) ci[15 + j] = Y[j];
       ci[31] = 0.f;
-      uint8_t *blob_ci = save_blobs ? ws.blob_ci + (size_t)tile * (CIP * ROWS * 2) : nullptr;
-      emit_fwd<T, false, SPLIT>(ci, buf, TILE_BYTES, blob_ci, row, 0, valid);
-      emit_fwd<T, false, SPLIT>(ci + 16, buf, TILE_BYTES, blob_ci, row, 16, valid);
+      emit32<T, false, SPLIT>(ci, tlane, buf, save_blobs ? ws.blob_ci + (size_t)tile * (CIP * ROWS * 2) : nullptr, row, 0, valid);
+      operand_written<SPLIT>();
     }
-    fence_async_smem(); fence_before(); group_bar(grp);
-    if (lead_warp) { fence_after(); if (elect_one()) issue_fwd<SPLIT>(tcol, sBuf, TILE_BYTES, sW + WImg::f_c1, WImg::f_total, CIP, H, H, fmt, bar_mma); }
+    fence_before(); group_bar(grp);
+    if (lead_warp) { fence_after(); if (elect_one()) issue_next<SPLIT>(tcol, sBuf, sW + WImg::f_c1, CIP, H, H, fmt, bar_mma); }
     mbar_wait(bar_mma, ph_mma); ph_mma ^= 1; fence_after();
     hidden_epilogue<T, SPLIT>(tlane, buf, save_blobs ? ws.blob_h1 + (size_t)tile * (H * ROWS * 2) : nullptr, row, valid);
     if (ms.n_color_layers == 2) {
-      fence_async_smem(); fence_before(); group_bar(grp);
-      if (lead_warp) { fence_after(); if (elect_one()) issue_fwd<SPLIT>(tcol, sBuf, TILE_BYTES, sW + WImg::f_c2, WImg::f_total, H, H, H, fmt, bar_mma); }
+      fence_before(); group_bar(grp);
+      if (lead_warp) { fence_after(); if (elect_one()) issue_next<SPLIT>(tcol, sBuf, sW + WImg::f_c2, H, H, H, fmt, bar_mma); }
       mbar_wait(bar_mma, ph_mma); ph_mma ^= 1; fence_after();
       hidden_epilogue<T, SPLIT>(tlane, buf, save_blobs ? ws.blob_h2 + (size_t)tile * (H * ROWS * 2) : nullptr, row, valid);
     }
-    fence_async_smem(); fence_before(); group_bar(grp);
-    if (lead_warp) { fence_after(); if (elect_one()) issue_fwd<SPLIT>(tcol, sBuf, TILE_BYTES, sW + WImg::f_c3, WImg::f_total, H, 16, 16, fmt, bar_mma); }
+    fence_before(); group_bar(grp);
+    if (lead_warp) { fence_after(); if (elect_one()) issue_next<SPLIT>(tcol, sBuf, sW + WImg::f_c3, H, 16, 16, fmt, bar_mma); }
     mbar_wait(bar_mma, ph_mma); ph_mma ^= 1; fence_after();
-    if (lead_warp) {   // the buffer is free: the group's next encoder tile
-      const uint64_t nxt = tile + tile_stride;
-      if (nxt < n_tiles && elect_one()) { mbar_expect_tx(bar_e, e_bytes); bulk_g2s(sBuf, ws.blob_e + (size_t)nxt * e_stride, e_bytes, bar_e); }
-    }
+    if constexpr (!SPLIT) fetch_next_e();
     {
       float v[16];
       tmem_ld16(tlane, v);
