@@ -1,12 +1,26 @@
 // mlp_tc.cu — S5/S6/S7 and S11 on the 5th-generation tensor cores: the density and colour MLPs of
 // PAPER.md:143,151 as 128-sample tcgen05.mma tiles (M = 128 samples, N = layer width, K = input
-// width; 16-bit operands in shared memory, fp32 accumulators in TMEM).
+// width; 16-bit operands, fp32 accumulators in TMEM).
 //
-// One CTA (4 warps) owns a 128-sample tile; thread r owns sample row r: it writes its row of the
-// next layer's input into shared memory (UMMA canonical no-swizzle layout: 16-byte chunks at a 16 B
-// stride across threads, conflict-free), ONE thread issues the layer's tcgen05.mma k-steps and a
-// tcgen05.commit onto an mbarrier, everyone waits on it and reads its accumulator row back with
-// tcgen05.ld (TMEM lane = sample row).  Activations never leave the SM between layers.
+// A group of 4 warps owns a 128-sample tile; thread r owns sample row r (TMEM lane = sample row): it
+// reads its accumulator row back with tcgen05.ld, applies the activation and writes its row of the
+// next layer's A operand; ONE elected thread issues the layer's tcgen05.mma k-steps and a
+// tcgen05.commit onto an mbarrier the group waits on.  Activations never leave the SM between layers.
+//
+// Forward (mlp_forward_tc_kernel): one persistent CTA per SM holding FWD_GROUPS = 4 such groups,
+// each a pipeline of its own (own tiles, own 128 TMEM columns, own mbarriers, bar.sync on a named
+// barrier of 128 threads), so four dependent layer chains hide each other's MMA issue-to-commit
+// latency.  On the two-term training path the next layer's A operand goes straight into tensor
+// memory (tcgen05.st by the thread that owns the row: hi at +64, lo at +96 of the group's columns)
+// and the MMAs take A from TMEM (.ts form); only the first layer's A (the encoder's blob, by TMA)
+// and the weights sit in shared memory.  The plain 16-bit forward (render, occupancy refresh) keeps
+// its A operand in shared memory (UMMA canonical no-swizzle layout: 16-byte chunks at a 16 B stride
+// across threads, conflict-free), which measured faster there.
+//
+// Backward (mlp_backward_tc_kernel): 256 threads, 2 CTAs per SM (TMEM bounds it), a three-slot ring
+// of TMA-loaded saved activations X and two buffers for the gradients Y; per layer the data
+// gradient's MMAs are issued and committed BEFORE the weight gradient's, so the next layer's
+// epilogue starts while the weight-gradient MMAs still run.
 //
 // Everything that crosses HBM is stored as the exact byte image of the shared-memory operand tile
 // ("blob": [tile][8-column panel][128 rows][8 x 16 bit]), so it comes back with ONE TMA bulk copy
