@@ -286,6 +286,58 @@ nsm_status nsm_profile(nsm_field *f, int enable);
 nsm_status nsm_profile_read(nsm_field *f, uint32_t capacity, const char **names, double *total_ms,
                             uint64_t *launches, uint32_t *n_out);
 
+/* ---- S1-S3 alone, allocating nothing -----------------------------------------------------------
+ * For callers that cannot call cudaMalloc (code under CUDA graph capture, tight serving loops): the marcher of
+ * S1-S3 ("sampling 3D positions along the pixel's ray", delta_i = d_{i+1} - d_i; the occupancy
+ * test of DESIGN.md S2 with the cascades of reading R23; compaction in (ray, k) order) as ONE call that takes every
+ * input and output from the caller and needs no nsm_field.  It is the same kernel the training step launches; the only
+ * scratch memory it needs, the chained scan's ticket counters and per-block status words, lives in a file-scope
+ * `static __device__` array inside the library sized for NSM_MARCH_STATIC_MAX_RAYS rays (512 KiB + 256 B, held by
+ * every GPU that loads the library until the process exits).  The call makes no cudaMalloc / cudaFree and calls no
+ * allocating routine: it enqueues one memset of the scratch words it uses and one kernel on `cuda_stream`, and
+ * returns without synchronising.
+ *
+ * cfg: the cube, the occupancy structure's shape and the jitter stream (the values an nsm_field_config carries;
+ * step = the jitter stream's step index, which nsm_train_step sets to the Adam step count + 1).  rays: origins, dirs,
+ * t_min, t_max, n_candidates as for nsm_train_step (DEVICE pointers; rgb / depth / depth_var are ignored).
+ * d_occ_bits: the bit i = j*G^3 + gx + G*(gy + G*gz) layout of nsm_update_occupancy, ceil(C*G^3 / 8) bytes, or
+ * NULL = every cell live.  out: caller-owned DEVICE arrays; capacity = samples each per-sample array can hold and
+ * must be >= n_rays * n_candidates (the kernel is unchanged and does not bounds-check its writes against less).
+ * On return (stream order): counts[r] = n_r, offsets = exclusive scan with offsets[n_rays] = S, and the first S
+ * entries of s_ray, s_k, s_t, s_delta and of each of the three planes s_x[a * capacity + s] are the live samples
+ * in (ray, k) order, bit-identical to what the field's own step computes for the same inputs.
+ *
+ * The current CUDA device must be the one that owns the pointers and the stream (the scratch address is looked up
+ * once per device, with that device current).  Every call on a device shares the one scratch array: calls in one
+ * stream are ordered and safe, calls that OVERLAP on the GPU (two streams, two host threads) race on it and give
+ * wrong offsets or hang the look-back -- serialise them.  nsm_field calls use the field's own scratch and do not
+ * interfere.  Errors: NSM_ERR_INVALID_ARG (NULL / malformed arguments, pointers of another device),
+ * NSM_ERR_CAPACITY (n_rays > NSM_MARCH_STATIC_MAX_RAYS, n_candidates > 4096, out->capacity too small),
+ * NSM_ERR_CUDA; nothing is enqueued on a failed call. */
+#define NSM_MARCH_STATIC_MAX_RAYS (1u << 20)
+
+typedef struct {
+  uint32_t struct_size;              /* sizeof(nsm_march_config), ABI check */
+  float    aabb_min[3], aabb_extent; /* cube: x = (p - aabb_min) / aabb_extent in [0,1)^3 */
+  uint32_t occ_res;                  /* G, power of two <= 1024 */
+  uint32_t occ_cascades;             /* C <= 8 (0 or 1: one grid) */
+  uint32_t jitter;                   /* 0: interval midpoints; else the stratified jitter u(seed, step, ray, k) of S1 */
+  uint32_t step;                     /* step index of the jitter stream */
+  uint64_t seed;                     /* jitter stream */
+} nsm_march_config;
+
+typedef struct {
+  uint64_t  capacity;                /* samples per per-sample array, >= n_rays * n_candidates */
+  uint32_t *counts;                  /* [n_rays] */
+  uint32_t *offsets;                 /* [n_rays + 1] */
+  uint32_t *s_ray, *s_k;             /* [capacity] */
+  float    *s_t, *s_delta;           /* [capacity] */
+  float    *s_x;                     /* [3][capacity] planes */
+} nsm_march_result;
+
+nsm_status nsm_march_static(const nsm_march_config *cfg, const nsm_ray_batch *rays, const uint8_t *d_occ_bits,
+                            const nsm_march_result *out, void *cuda_stream);
+
 /* Number of this library's kernels launched by this field so far (bench.py's gpu_launches). */
 uint64_t    nsm_launch_count(const nsm_field *f);
 /* Which MLP path the field runs: "simt_fp32", "tcgen05_f16", "tcgen05_bf16". */

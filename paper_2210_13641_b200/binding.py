@@ -17,6 +17,7 @@ NSM_OK, NSM_ERR_INVALID_ARG, NSM_ERR_OOM, NSM_ERR_CUDA, NSM_ERR_CAPACITY, NSM_ER
 NSM_MLP_FP32, NSM_MLP_FP16, NSM_MLP_BF16 = 0, 1, 2
 NSM_OCC_FULL, NSM_OCC_SET, NSM_OCC_FROM_FIELD = 0, 1, 2
 NSM_OPT_BATCH_READY, NSM_OPT_POSE_GRADIENTS, NSM_OPT_DEBUG_TIMELINE, NSM_OPT_POSE_LEVELS = 0, 1, 2, 3
+NSM_MARCH_STATIC_MAX_RAYS = 1 << 20
 
 DEBUG_ITEMS = dict(counts=(0, np.uint32), offsets=(1, np.uint32), s_ray=(2, np.uint32), s_k=(3, np.uint32),
                    s_t=(4, np.float32), s_delta=(5, np.float32), s_x=(6, np.float32), slots=(7, np.uint32),
@@ -32,7 +33,7 @@ EXPORTS = ["nsm_create_field", "nsm_destroy_field", "nsm_update_occupancy", "nsm
            "nsm_add_keyframe", "nsm_keyframe_count", "nsm_sample_batch", "nsm_train_step_sampled",
            "nsm_pose_gradients", "nsm_keyframe_pose_gradients", "nsm_apply_pose_step", "nsm_get_keyframe_pose",
            "nsm_update_occupancy_decay", "nsm_update_occupancy_stochastic", "nsm_get_occupancy_grid",
-           "nsm_profile_read", "nsm_launch_count", "nsm_mlp_path",
+           "nsm_profile_read", "nsm_launch_count", "nsm_mlp_path", "nsm_march_static",
            "nsm_last_error", "nsm_version"]
 
 
@@ -63,6 +64,17 @@ class NsmKeyframeInfo(C.Structure):
 class NsmStepStats(C.Structure):
     _fields_ = [("loss", C.c_double), ("loss_rgb", C.c_double), ("loss_depth", C.c_double),
                 ("n_samples", C.c_uint64), ("n_rays", C.c_uint32), ("step", C.c_uint32)]
+
+
+class NsmMarchConfig(C.Structure):
+    _fields_ = [("struct_size", C.c_uint32), ("aabb_min", C.c_float * 3), ("aabb_extent", C.c_float),
+                ("occ_res", C.c_uint32), ("occ_cascades", C.c_uint32), ("jitter", C.c_uint32), ("step", C.c_uint32),
+                ("seed", C.c_uint64)]
+
+
+class NsmMarchResult(C.Structure):
+    _fields_ = [("capacity", C.c_uint64), ("counts", C.c_void_p), ("offsets", C.c_void_p), ("s_ray", C.c_void_p),
+                ("s_k", C.c_void_p), ("s_t", C.c_void_p), ("s_delta", C.c_void_p), ("s_x", C.c_void_p)]
 
 
 class NsmError(RuntimeError):
@@ -116,6 +128,7 @@ def load_library():
         L.nsm_debug_timeline.argtypes = [vp, u64p, C.c_uint64, u32p]
         L.nsm_profile_read.argtypes = [vp, C.c_uint32, C.POINTER(C.c_char_p), C.POINTER(C.c_double), u64p, u32p]
         L.nsm_launch_count.argtypes = [vp]
+        L.nsm_march_static.argtypes = [C.POINTER(NsmMarchConfig), C.POINTER(NsmRayBatch), vp, C.POINTER(NsmMarchResult), vp]
         L.nsm_launch_count.restype = C.c_uint64
         for name in ("nsm_mlp_path", "nsm_last_error", "nsm_version"):
             getattr(L, name).restype = C.c_char_p
@@ -181,6 +194,56 @@ class DeviceBatch:
         b.rgb, b.depth, b.depth_var = _dev_ptr(self.rgb), _dev_ptr(self.depth), _dev_ptr(self.depth_var)
         b.t_min, b.t_max, b.n_candidates = self.t_min, self.t_max, self.n_candidates
         return b
+
+
+class MarchBuffers:
+    """Caller-owned device arrays nsm_march_static writes (include/nsm.h nsm_march_result): allocated once, by torch,
+    outside the call; capacity = samples per per-sample array."""
+
+    def __init__(self, max_rays, capacity, device="cuda"):
+        z = lambda n, dt: torch.zeros(n, dtype=dt, device=device)
+        self.max_rays, self.capacity = int(max_rays), int(capacity)
+        self.counts, self.offsets = z(self.max_rays, torch.int32), z(self.max_rays + 1, torch.int32)
+        self.s_ray, self.s_k = z(self.capacity, torch.int32), z(self.capacity, torch.int32)
+        self.s_t, self.s_delta = z(self.capacity, torch.float32), z(self.capacity, torch.float32)
+        self.s_x = z(3 * self.capacity, torch.float32)
+
+    def c_struct(self):
+        r = NsmMarchResult()
+        r.capacity = self.capacity
+        for k in ("counts", "offsets", "s_ray", "s_k"):
+            setattr(r, k, _dev_ptr(getattr(self, k), torch.int32))
+        for k in ("s_t", "s_delta", "s_x"):
+            setattr(r, k, _dev_ptr(getattr(self, k)))
+        return r
+
+    def read(self, n_rays):
+        """The result of the last call as numpy arrays named like nsm_debug_last_step's items (synchronises)."""
+        torch.cuda.synchronize(self.counts.device)
+        u32 = lambda t, n: t[:n].cpu().numpy().view(np.uint32)
+        offsets = u32(self.offsets, n_rays + 1)
+        S = int(offsets[n_rays])
+        return dict(counts=u32(self.counts, n_rays), offsets=offsets, s_ray=u32(self.s_ray, S), s_k=u32(self.s_k, S),
+                    s_t=self.s_t[:S].cpu().numpy(), s_delta=self.s_delta[:S].cpu().numpy(),
+                    s_x=self.s_x.view(3, self.capacity)[:, :S].t().contiguous().cpu().numpy())
+
+
+def nsm_march_static(fc, batch, bits, out, step, stream=None):
+    """S1-S3 alone through the entry point that allocates nothing (include/nsm.h).  fc: FieldConfig attribute names
+    (aabb_min, aabb_extent, occ_res, occ_cascades, jitter, seed); batch: DeviceBatch; bits: uint8 device tensor or
+    None (every cell live); out: MarchBuffers; step: the jitter stream's step index.  Enqueues and returns."""
+    if not torch.cuda.is_available():
+        raise RuntimeError("nsm needs a CUDA device (B200); there is no CPU fallback")
+    lib = load_library()
+    c = NsmMarchConfig()
+    c.struct_size = C.sizeof(NsmMarchConfig)
+    c.aabb_min[:] = [float(x) for x in fc.aabb_min]
+    c.aabb_extent = float(fc.aabb_extent)
+    c.occ_res, c.occ_cascades = int(fc.occ_res), int(getattr(fc, "occ_cascades", 1))
+    c.jitter, c.step, c.seed = int(getattr(fc, "jitter", 1)), int(step), int(fc.seed)
+    b, r = batch.c_struct(), out.c_struct()
+    s = stream if stream is not None else torch.cuda.current_stream(out.counts.device)
+    _check(lib.nsm_march_static(C.byref(c), C.byref(b), _dev_ptr(bits, torch.uint8), C.byref(r), C.c_void_p(s.cuda_stream)))
 
 
 class HostBatch:

@@ -5,6 +5,9 @@
 // Index path: every fp32 operation below is an explicit round-to-nearest intrinsic so that the
 // compiler cannot contract or reorder it; the integers it decides (live bits, counts) must be
 // bit-exact against the oracle, and so must t, delta, x.
+#include <cstdio>
+#include <mutex>
+
 #include "nsm_internal.cuh"
 
 namespace {
@@ -375,4 +378,142 @@ int launch_occ_max_visited(float *grid, uint64_t first_cell, uint32_t stride, ui
 int launch_occ_bits_from_grid(const float *grid, uint64_t n_cells, float thr, uint8_t *bits, cudaStream_t st) {
   occ_bits_from_grid_kernel<<<(unsigned)((n_cells + 255) / 256), 256, 0, st>>>(grid, n_cells, thr, (uint32_t *)bits);
   return 1;
+}
+
+// ---- nsm_march_static (include/nsm.h "S1-S3 alone, allocating nothing") ---------------------------------------------
+// The scratch memory of march_fused_kernel -- the ticket / finished-block counters and the chained scan's per-block
+// status words, plus the few words the kernel writes beside the loss sums for the field's step -- in a file-scope
+// device array instead of the field's arena, so that the entry point below never allocates.  Layout (bytes):
+//   [0, 8)     scan_ctr[2]          [8, 12)  grad_absmax        [16, 40)  loss_acc[3]        [40, 48)  total_samples
+//   [256, ...) scan_state[NSM_MARCH_STATIC_MAX_RAYS / MARCH_WARPS]
+// In HOST code the name below is a host-side stand-in, not a device address: the kernel gets the address that
+// cudaGetSymbolAddress returns for the current device (looked up once per device, cached).
+namespace {
+
+constexpr uint32_t STATIC_ENTRIES = NSM_MARCH_STATIC_MAX_RAYS / MARCH_WARPS;
+constexpr size_t STATIC_HEADER = 256, STATIC_BYTES = STATIC_HEADER + sizeof(unsigned long long) * STATIC_ENTRIES;
+static_assert(NSM_MARCH_STATIC_MAX_RAYS % MARCH_WARPS == 0, "whole blocks");
+
+static __device__ __align__(256) unsigned char march_static_scratch[STATIC_BYTES];
+
+constexpr int STATIC_MAX_DEVICES = 64;
+std::mutex g_static_mu;
+unsigned char *g_static_ptr[STATIC_MAX_DEVICES] = {};
+
+// device address of march_static_scratch on the CURRENT device
+nsm_status static_scratch(unsigned char **out, int *dev_out) {
+  char msg[256];
+  int dev = -1;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e != cudaSuccess) {
+    snprintf(msg, sizeof msg, "cudaGetDevice: %s (there is no CPU fallback)", cudaGetErrorString(e));
+    cudaGetLastError();
+    return nsm_set_error(NSM_ERR_CUDA, msg);
+  }
+  if (dev < 0 || dev >= STATIC_MAX_DEVICES) return nsm_set_error(NSM_ERR_CUDA, "nsm_march_static: device ordinal out of range");
+  std::lock_guard<std::mutex> lock(g_static_mu);
+  if (!g_static_ptr[dev]) {
+    void *p = nullptr;
+    e = cudaGetSymbolAddress(&p, march_static_scratch);
+    if (e != cudaSuccess || !p) {
+      snprintf(msg, sizeof msg, "cudaGetSymbolAddress(march_static_scratch) on device %d: %s", dev, cudaGetErrorString(e));
+      cudaGetLastError();
+      return nsm_set_error(NSM_ERR_CUDA, msg);
+    }
+    g_static_ptr[dev] = (unsigned char *)p;
+  }
+  *out = g_static_ptr[dev];
+  *dev_out = dev;
+  return NSM_OK;
+}
+
+// a device pointer that belongs to another device than `dev`?  (host-mapped and unregistered pointers pass)
+bool on_other_device(const void *p, int dev) {
+  cudaPointerAttributes a;
+  if (cudaPointerGetAttributes(&a, p) != cudaSuccess) { cudaGetLastError(); return false; }
+  return a.type == cudaMemoryTypeDevice && a.device != dev;
+}
+
+}  // namespace
+
+extern "C" nsm_status nsm_march_static(const nsm_march_config *cfg, const nsm_ray_batch *rays, const uint8_t *d_occ_bits,
+                                       const nsm_march_result *out, void *cuda_stream) {
+  char msg[256];
+  if (!cfg || !rays || !out) return nsm_set_error(NSM_ERR_INVALID_ARG, "nsm_march_static: cfg, rays or out is NULL");
+  if (cfg->struct_size != sizeof(nsm_march_config)) {
+    snprintf(msg, sizeof msg, "nsm_march_static: struct_size %u != %zu (ABI mismatch)", cfg->struct_size, sizeof(nsm_march_config));
+    return nsm_set_error(NSM_ERR_INVALID_ARG, msg);
+  }
+  if (!(cfg->aabb_extent > 0.f) || !isfinite(cfg->aabb_extent)) return nsm_set_error(NSM_ERR_INVALID_ARG, "nsm_march_static: aabb_extent must be > 0");
+  const uint32_t G = cfg->occ_res, C = cfg->occ_cascades ? cfg->occ_cascades : 1u;
+  if (G < 1 || G > 1024 || (G & (G - 1))) return nsm_set_error(NSM_ERR_INVALID_ARG, "nsm_march_static: occ_res must be a power of two <= 1024");
+  if (C > 8) return nsm_set_error(NSM_ERR_INVALID_ARG, "nsm_march_static: occ_cascades must be <= 8");
+  if ((uint64_t)C * G * G * G > (1ull << 31)) return nsm_set_error(NSM_ERR_INVALID_ARG, "nsm_march_static: occ_cascades * occ_res^3 exceeds 2^31 cells");
+  if (!rays->origins || !rays->dirs) return nsm_set_error(NSM_ERR_INVALID_ARG, "nsm_march_static: origins/dirs are NULL");
+  const uint32_t R = rays->n_rays, K = rays->n_candidates;
+  if (R == 0 || K == 0) return nsm_set_error(NSM_ERR_INVALID_ARG, "nsm_march_static: n_rays or n_candidates is 0");
+  if (!(rays->t_min < rays->t_max) || !isfinite(rays->t_min) || !isfinite(rays->t_max))
+    return nsm_set_error(NSM_ERR_INVALID_ARG, "nsm_march_static: need finite t_min < t_max");
+  if (R > NSM_MARCH_STATIC_MAX_RAYS) {
+    snprintf(msg, sizeof msg, "nsm_march_static: n_rays %u exceeds the static scratch array's maximum of %u rays per call", R,
+             NSM_MARCH_STATIC_MAX_RAYS);
+    return nsm_set_error(NSM_ERR_CAPACITY, msg);
+  }
+  if (K > MARCH_MAX_WORDS * 32) {
+    snprintf(msg, sizeof msg, "nsm_march_static: n_candidates %u exceeds the maximum of %u", K, MARCH_MAX_WORDS * 32);
+    return nsm_set_error(NSM_ERR_CAPACITY, msg);
+  }
+  if ((uint64_t)R * K > (1ull << 31)) return nsm_set_error(NSM_ERR_CAPACITY, "nsm_march_static: n_rays * n_candidates exceeds 2^31");
+  if (!out->counts || !out->offsets || !out->s_ray || !out->s_k || !out->s_t || !out->s_delta || !out->s_x)
+    return nsm_set_error(NSM_ERR_INVALID_ARG, "nsm_march_static: an output pointer is NULL");
+  if (out->capacity < (uint64_t)R * K) {
+    snprintf(msg, sizeof msg, "nsm_march_static: out->capacity %llu < n_rays * n_candidates = %llu", (unsigned long long)out->capacity,
+             (unsigned long long)R * K);
+    return nsm_set_error(NSM_ERR_CAPACITY, msg);
+  }
+  unsigned char *scratch = nullptr;
+  int dev = -1;
+  nsm_status st = static_scratch(&scratch, &dev);
+  if (st != NSM_OK) return st;
+  if (on_other_device(rays->origins, dev) || on_other_device(out->counts, dev) || on_other_device(out->s_x, dev)) {
+    snprintf(msg, sizeof msg, "nsm_march_static: the pointers belong to another device than the current one (%d)", dev);
+    return nsm_set_error(NSM_ERR_INVALID_ARG, msg);
+  }
+  cudaStream_t stream = (cudaStream_t)cuda_stream;
+
+  MarchParams mp;
+  for (int a = 0; a < 3; ++a) mp.aabb_min[a] = cfg->aabb_min[a];
+  mp.inv_extent = 1.0f / cfg->aabb_extent;                        // as make_march (nsm_api.cu): one fp32 divide
+  mp.t_min = rays->t_min;
+  mp.dt = (rays->t_max - rays->t_min) / (float)K;                 // one fp32 subtract, one fp32 divide
+  mp.K = K; mp.G = G; mp.C = C;
+  mp.jitter = cfg->jitter ? 1u : 0u;
+  mp.step = cfg->step;
+  mp.seed = cfg->seed;
+  mp.R = R;
+
+  Workspace ws = {};                                              // everything the marcher does not touch stays NULL
+  ws.cap = out->capacity;
+  ws.max_rays = NSM_MARCH_STATIC_MAX_RAYS;
+  ws.counts = out->counts; ws.offsets = out->offsets;
+  ws.s_ray = out->s_ray; ws.s_k = out->s_k; ws.s_t = out->s_t; ws.s_delta = out->s_delta; ws.s_x = out->s_x;
+  ws.scan_ctr = (uint32_t *)scratch;
+  ws.grad_absmax = (uint32_t *)(scratch + 8);
+  ws.loss_acc = (double *)(scratch + 16);
+  ws.total_samples = (unsigned long long *)(scratch + 40);
+  ws.scan_state = (unsigned long long *)(scratch + STATIC_HEADER);
+
+  // The array keeps the last call's contents.  The kernel's last block zeroes the words it used, but a call that was
+  // cut short (a fault, a reset stream) would leave them set: clear what this launch reads before it starts.
+  const uint32_t n_blocks = (R + MARCH_WARPS - 1) / MARCH_WARPS;
+  cudaError_t e = cudaMemsetAsync(scratch, 0, STATIC_HEADER + sizeof(unsigned long long) * n_blocks, stream);
+  if (e == cudaSuccess) {
+    march_fused_kernel<<<n_blocks, MARCH_WARPS * 32, 0, stream>>>(mp, d_occ_bits, rays->origins, rays->dirs, ws, 0, nullptr);
+    e = cudaGetLastError();
+  }
+  if (e != cudaSuccess) {
+    snprintf(msg, sizeof msg, "nsm_march_static: %s", cudaGetErrorString(e));
+    return nsm_set_error(NSM_ERR_CUDA, msg);
+  }
+  return NSM_OK;
 }

@@ -38,6 +38,12 @@ nsm_status fail(nsm_status st, const char *fmt, ...) {
 
 }  // namespace
 
+// the thread-local message behind nsm_last_error(), for entry points defined in other files (march.cu)
+nsm_status nsm_set_error(nsm_status st, const char *msg) {
+  g_err = msg;
+  return st;
+}
+
 // Default: every hot-path kernel except the marcher (bit 0) and the scatter (bit 5).  Measured on B200 at
 // config 2 (profiles/r1g_pdl_sweep.md): 148.7 us/step without PDL, 135.5 us with this mask; letting the
 // table Adam's blocks become resident under the scatter, or the marcher's under the MLP Adam, costs

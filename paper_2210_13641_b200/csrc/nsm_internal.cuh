@@ -166,6 +166,8 @@ __device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;"
 __device__ __forceinline__ void pdl_trigger() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
 
 // Which kernel classes (bit = KernelId) are launched with the PDL attribute (swept on the GPU, profiles/r1g).
+nsm_status nsm_set_error(nsm_status st, const char *msg);   // nsm_api.cu: sets nsm_last_error()'s message, returns st
+
 extern const uint32_t g_pdl_mask;
 extern thread_local int g_cur_kernel;
 

@@ -41,7 +41,10 @@ def test_struct_layouts_match_c(lib, tmp_path):
     fields_b = [n for n, _ in B.NsmRayBatch._fields_]
     fields_s = [n for n, _ in B.NsmStepStats._fields_]
     lines = ['#include <stdio.h>', '#include <stddef.h>', '#include "nsm.h"', 'int main(void){']
-    for typ, fs in (("nsm_field_config", fields_cfg), ("nsm_ray_batch", fields_b), ("nsm_step_stats", fields_s)):
+    fields_mc = [n for n, _ in B.NsmMarchConfig._fields_]
+    fields_mr = [n for n, _ in B.NsmMarchResult._fields_]
+    for typ, fs in (("nsm_field_config", fields_cfg), ("nsm_ray_batch", fields_b), ("nsm_step_stats", fields_s),
+                    ("nsm_march_config", fields_mc), ("nsm_march_result", fields_mr)):
         lines.append(f'printf("%zu\\n", sizeof({typ}));')
         for f in fs:
             lines.append(f'printf("%zu\\n", offsetof({typ}, {f}));')
@@ -51,7 +54,7 @@ def test_struct_layouts_match_c(lib, tmp_path):
     subprocess.run(["gcc", "-I", os.path.join(ROOT, "include"), str(prog), "-o", str(exe)], check=True)
     vals = [int(x) for x in subprocess.run([str(exe)], capture_output=True, text=True, check=True).stdout.split()]
     want = []
-    for cls in (B.NsmFieldConfig, B.NsmRayBatch, B.NsmStepStats):
+    for cls in (B.NsmFieldConfig, B.NsmRayBatch, B.NsmStepStats, B.NsmMarchConfig, B.NsmMarchResult):
         want.append(C.sizeof(cls))
         want += [getattr(cls, n).offset for n, _ in cls._fields_]
     assert vals == want
