@@ -315,6 +315,18 @@ def mma_dispatch_floor(name, mma, fc, S, n_sms, sm_hz, two_term):
     return dict(mmas_per_tile=n, dispatch_cycles_per_tile=cycles, tiles=tiles, floor_us=1e6 * floor_s)
 
 
+def mlp_activation_bytes(name, fc, S):
+    """HBM bytes one launch of a tcgen05 TRAINING MLP kernel has to move ("blobs"): the forward reads
+    the two-term 16-bit encoder tile and writes the 16-bit activations the backward pass needs (hidden density layer,
+    colour-MLP input padded to 32, one or two hidden colour layers) plus sigma and rgb; the backward reads those, the hi
+    term of the encoder tile and dL/dsigma, dL/drgb, and writes dL/de in fp32 for the scatter."""
+    LF = fc.n_levels * fc.n_features
+    saved = 2 * (fc.density_hidden + 32 + fc.color_hidden * (2 if fc.color_hidden_layers == 2 else 1))
+    if name == "mlp_fwd":
+        return S * (4 * LF + saved + 16 + 4)
+    return S * (2 * LF + saved + 16 + 4 + 4 * LF)
+
+
 class Timer:
     def __init__(self, torch, dev, replicas):
         self.torch, self.dev, self.replicas = torch, dev, replicas
@@ -521,6 +533,12 @@ def measure_training(cfg, K, W, env, want_sampled=False, want_pose=False):
                                        1e6 * ((clocks or {}).get("sm_mhz") or 1965.0), two_term=True)
                 d["frac_of_floor"] = d["floor_us"] / (1e6 * avg_s)
                 k["mma_dispatch"] = d
+                # ... and the activations that cross HBM between the forward and the backward kernel
+                nb = mlp_activation_bytes(name, fc, S_avg)
+                k["hbm"] = dict(algorithmic_bytes=nb, achieved=nb / avg_s / 1e9, unit="GB/s", peak=peaks["hbm_gbs"],
+                                frac=nb / avg_s / 1e9 / peaks["hbm_gbs"],
+                                note="operand-tile images read and written by this launch (encoder tile, saved activations, "
+                                     "dL/de): the second bound of this kernel beside MMA dispatch")
             if name in ("encode", "scatter") and avg_s > 0 and "error" not in l2:
                 # what bounds S4 / S12 while the tables fit the L2: its random-access rate (8 corners per sample and level)
                 acc = 8 * L * S_avg / avg_s

@@ -17,10 +17,10 @@
 // its A operand in shared memory (UMMA canonical no-swizzle layout: 16-byte chunks at a 16 B stride
 // across threads, conflict-free), which measured faster there.
 //
-// Backward (mlp_backward_tc_kernel): 256 threads, 2 CTAs per SM (TMEM bounds it), a three-slot ring
-// of TMA-loaded saved activations X and two buffers for the gradients Y; per layer the data
-// gradient's MMAs are issued and committed BEFORE the weight gradient's, so the next layer's
-// epilogue starts while the weight-gradient MMAs still run.
+// Backward (mlp_backward_tc_kernel): 2 CTAs per SM (TMEM bounds it) of 8 epilogue warps, one MMA-
+// issuing warp and one TMA warp; a three-slot ring of TMA-loaded saved activations X and two buffers
+// for the gradients Y; per layer the data gradient's MMAs are issued and committed BEFORE the weight
+// gradient's, so the next layer's epilogue starts while the weight-gradient MMAs still run.
 //
 // Everything that crosses HBM is stored as the exact byte image of the shared-memory operand tile
 // ("blob": [tile][8-column panel][128 rows][8 x 16 bit]), so it comes back with ONE TMA bulk copy
@@ -550,7 +550,9 @@ constexpr uint32_t COL_G = 0;                                   // dgrad result,
 // wgrad accumulators.  The first colour layer's is kept TRANSPOSED (rows = 64 outputs, 32 input columns), which
 // brings the total to 256 columns: two CTAs per SM.
 constexpr uint32_t GW_C3 = 64, GW_C2 = 80, GW_C1T = 144, GW_D2 = 176, GW_D1 = 192, BWD_COLS = 256;
-constexpr uint32_t BWD_THREADS = 256;
+// 8 epilogue warps (TMEM lane quarter x column half) + one warp whose elected lane issues every MMA of the CTA + one warp
+// whose elected lane issues every TMA load of the saved activations
+constexpr uint32_t BWD_EPI_WARPS = 8, BWD_MMA_WARP = 8, BWD_TMA_WARP = 9, BWD_THREADS = 32 * (BWD_EPI_WARPS + 2);
 
 struct BwdSmem {
   // [X0][X1][X2][Y0][Y1][W], 16 KB tiles.  An M = 128 MMA that reads a 64-column tile MN-major also reads the 16 KB behind
@@ -562,7 +564,10 @@ struct BwdSmem {
   static constexpr uint32_t bar_mma = w + WImg::b_total;
   static constexpr uint32_t bar_w = bar_mma + 8;
   static constexpr uint32_t bar_x = bar_w + 8;                     // [3]
-  static constexpr uint32_t tmem = bar_x + 24;
+  static constexpr uint32_t bar_y = bar_x + 24;                    // dY of the next item written (one arrival per epilogue warp)
+  static constexpr uint32_t bar_fin = bar_y + 8;                   // every MMA of the CTA done
+  static constexpr uint32_t bar_free = bar_fin + 8;                // [3] ring slot released (its item's wgrad done, its mask read)
+  static constexpr uint32_t tmem = bar_free + 24;
   static constexpr uint32_t total = tmem + 8;
 };
 static_assert(WImg::b_total >= BwdSmem::tile, "the slack behind Y1 must be covered by the weight image");
@@ -611,24 +616,36 @@ __device__ __forceinline__ void masked_to_Y(uint32_t tlane, uint32_t mask, uint8
   }
 }
 
-// 8 warps per tile: warp w owns sample rows 32 (w & 3) .. +31 (TMEM lane quarter) and the column half (w >> 2) of every
-// 64-wide dgrad.  Two CTAs per SM.
+// 8 epilogue warps per tile: warp w owns sample rows 32 (w & 3) .. +31 (TMEM lane quarter) and the column half (w >> 2) of
+// every 64-wide dgrad; a ninth warp does nothing but issue the CTA's MMAs, a tenth nothing but the TMA loads of the saved
+// activations.  Two CTAs per SM.
 //
 // The layers of the CTA's tiles form one sequence of items n = 0, 1, 2, ...  Item n reads its saved activation from
 // X[n % 3] and its dY from Y[n % 2].  Only the item's dgrad is on the critical path (the next item's dY is computed from
-// it): the elected lane issues the dgrad MMAs, commits them onto the barrier the CTA waits on, and THEN issues the item's
-// wgrad MMAs, which run under the CTA's read-back and packing of the next item (round 1 waited for both: 8 of an item's
-// ~12 MMAs are wgrad).  A tcgen05.commit covers every MMA the thread issued before it, so when item n+1's dgrad has
-// completed, item n's wgrad has too: X[n % 3] is then refilled by TMA with the activation of item n+3, and Y[n % 2] is
-// free for item n+2.
+// it): the MMA warp's elected lane issues the dgrad MMAs, commits them onto the barrier the epilogue warps wait on, and
+// THEN issues the item's wgrad MMAs, which run under the read-back and packing of the next item.  A tcgen05.commit
+// covers every MMA the thread issued before it, so when item n+1's dgrad has completed, item n's wgrad has too and
+// Y[n % 2] is free for item n+2.  The ring slot X[n % 3] is released to the TMA warp (bar_free) by a commit the MMA warp
+// issues once the epilogue warps have handed over item n+1, i.e. have read item n's ReLU mask; the TMA warp then
+// fetches item n+3 into it.
+//
+// Why a warp of its own: a tcgen05.mma takes ~50 cycles to issue and an item has ~12 of them, so the issuing thread is
+// busy for ~600 cycles per item; while it also owned a sample row, its share of the read-back started that much later
+// than everyone else's and the whole CTA waited for it at the next barrier (measured with clock64 per phase: 2100
+// cycles per item of which the issuing thread spent 600 issuing, 500 on its row mask behind the queued MMAs and 460
+// on the TMA request; the request alone still cost the warp that issued it ~500 cycles per item, hence the TMA warp).
+// The epilogue warps hand an item over with one mbarrier arrival per warp (bar_y) and never __syncthreads inside the
+// tile loop.
 template <typename T>
 __global__ void __launch_bounds__(BWD_THREADS, 2) mlp_backward_tc_kernel(MlpShape ms, Workspace ws,
                                                                         const uint32_t *__restrict__ d_S) {
   extern __shared__ __align__(1024) uint8_t smem[];
   const uint32_t tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
-  const uint32_t row = (warp & 3u) * 32u + lane, half = warp >> 2, cb = half * 32u;
+  const uint32_t row = (warp & 3u) * 32u + lane, half = warp >> 2, cb = half * 32u;   // epilogue warps (half < 2)
+  const bool mma_warp = warp == BWD_MMA_WARP, tma_warp = warp == BWD_TMA_WARP;
   const uint32_t sbase = smem_u32(smem);
   const uint32_t bar_mma = sbase + BwdSmem::bar_mma, bar_w = sbase + BwdSmem::bar_w;
+  const uint32_t bar_y = sbase + BwdSmem::bar_y, bar_fin = sbase + BwdSmem::bar_fin;
   const uint32_t sW = sbase + BwdSmem::w;
   const uint32_t LF = ms.LF;
   const uint64_t S = *d_S;                         // from the marcher, several kernels back: safe before pdl_wait()
@@ -639,7 +656,7 @@ __global__ void __launch_bounds__(BWD_THREADS, 2) mlp_backward_tc_kernel(MlpShap
   // ---- the X ring.  Loader state (identical in every lane of warp 0; the elected lane issues): the next item to fetch.
   uint64_t ld_tile = blockIdx.x;
   uint32_t ld_layer = 0, ld_slot = 0;              // layer 0..4 (1 is skipped with one hidden colour layer); ring slot
-  auto load_next = [&]() {                         // warp 0, converged
+  auto load_next = [&]() {                         // the TMA warp, converged
     if (ld_tile * ROWS < S && elect_one()) {
       const uint8_t *src; uint32_t bytes;
       switch (ld_layer) {                          // the activation the layer's wgrad needs
@@ -668,15 +685,22 @@ __global__ void __launch_bounds__(BWD_THREADS, 2) mlp_backward_tc_kernel(MlpShap
   if (has_tiles) {   // prologue on data that is at least two kernels old (weight image, the forward pass's saved activations)
     if (tid == 0) {
       mbar_init(bar_mma, 1); mbar_init(bar_w, 1);
-      mbar_init(sbase + BwdSmem::bar_x, 1); mbar_init(sbase + BwdSmem::bar_x + 8, 1); mbar_init(sbase + BwdSmem::bar_x + 16, 1);
+      mbar_init(bar_y, BWD_EPI_WARPS); mbar_init(bar_fin, 1);
       fence_async_smem();
       mbar_expect_tx(bar_w, WImg::b_total);
       bulk_g2s(sW, ws.wimg_bwd, WImg::b_total, bar_w);
     }
     if (warp == 0) {
       __syncwarp();
-      load_next(); load_next(); load_next();
       tmem_alloc<BWD_COLS>(sbase + BwdSmem::tmem);
+    }
+    if (tma_warp) {   // the ring's barriers are this warp's own: initialise them and request the first three items
+      if (lane == 0) {
+        for (uint32_t i = 0; i < 3; ++i) { mbar_init(sbase + BwdSmem::bar_x + 8 * i, 1); mbar_init(sbase + BwdSmem::bar_free + 8 * i, 1); }
+        fence_async_smem();
+      }
+      __syncwarp();
+      load_next(); load_next(); load_next();
     }
   }
   pdl_wait();     // the compositor's dL/dsigma, dL/dc and gradient maximum
@@ -699,36 +723,75 @@ __global__ void __launch_bounds__(BWD_THREADS, 2) mlp_backward_tc_kernel(MlpShap
     if (mx > 0.f && isfinite(mx)) scale = exp2f(fminf(fmaxf(floorf(8.f - log2f(mx)), -24.f), 30.f));
   }
   const float inv_scale = 1.f / scale;
-  uint32_t acc = 0;   // wgrad accumulate flag (0 on the CTA's first tile)
-  if (warp == 0) mbar_wait(bar_w, 0);
-
-  // one item: dY is in Y[ys] and X[xs] has landed (the caller waited).  Issue dgrad (committed: the CTA waits for it) and
-  // wgrad (not waited for), wait for the dgrad, refill the ring slot that the PREVIOUS item's wgrad has released, advance.
-#define BWD_ITEM(WGRAD_STMT, DGRAD_STMT, UNDER_MMA_STMT)                                     \
+  if (mma_warp) {
+    // ---- the MMA warp: per item, wait for the item's dY (bar_y) and saved activation (its ring slot), issue
+    // Behind bar_y of item n+1 the epilogue warps have read item n's ring slot for the last time (its ReLU mask), so a
+    // commit issued there -- it also covers item n's wgrad MMAs -- releases the slot to the TMA warp.
+    uint32_t ph_y = 0, acc = 0, issued = 0;   // acc: wgrad accumulate flag (0 on the CTA's first tile)
+    mbar_wait(bar_w, 0);
+#define BWD_ISSUE(WGRAD_STMT, DGRAD_STMT)                                                    \
   do {                                                                                       \
-    fence_async_smem(); fence_before(); __syncthreads();                                     \
-    if (warp == 0) {                                                                         \
-      fence_after();                                                                         \
-      if (elect_one()) { DGRAD_STMT; WGRAD_STMT; }                                           \
-    }                                                                                        \
-    UNDER_MMA_STMT;   /* work that does not need the dgrad: runs under the MMAs' latency */  \
+    mbar_wait(bar_y, ph_y); ph_y ^= 1;                                                       \
+    if (issued && elect_one()) mma_commit(sbase + BwdSmem::bar_free + 8 * (xs == 0 ? 2u : xs - 1u)); \
+    __syncwarp();                                                                            \
+    wait_x();                                                                                \
+    fence_after();                                                                           \
+    if (elect_one()) { DGRAD_STMT; WGRAD_STMT; }                                             \
+    __syncwarp();                                                                            \
+    issued = 1;                                                                              \
+    xs = xs == 2 ? 0u : xs + 1u; ys ^= 1u;                                                   \
+  } while (0)
+    for (uint64_t tile = blockIdx.x; tile * ROWS < S; tile += gridDim.x) {
+      BWD_ISSUE(issue_wgrad(tmem_base + GW_C3, sX(), sY(), 16, fmt, acc),
+                issue_layer(tmem_base + COL_G, sY(), sW + WImg::b_c3, 16, H, H, fmt, bar_mma));
+      if (two)
+        BWD_ISSUE(issue_wgrad(tmem_base + GW_C2, sX(), sY(), H, fmt, acc),
+                  issue_layer(tmem_base + COL_G, sY(), sW + WImg::b_c2, H, H, H, fmt, bar_mma));
+      BWD_ISSUE(issue_wgrad(tmem_base + GW_C1T, sY(), sX(), CIP, fmt, acc),                 // transposed: G^T = dY^T X
+                issue_layer(tmem_base + COL_G, sY(), sW + WImg::b_c1, H, CIP, CIP, fmt, bar_mma));
+      BWD_ISSUE(issue_wgrad(tmem_base + GW_D2, sX(), sY(), 16, fmt, acc),
+                issue_layer(tmem_base + COL_G, sY(), sW + WImg::b_d2, 16, H, H, fmt, bar_mma));
+      BWD_ISSUE(issue_wgrad(tmem_base + GW_D1, sX(), sY(), H, fmt, acc),
+                issue_layer(tmem_base + COL_G, sY(), sW + WImg::b_d1, H, LF, LF, fmt, bar_mma));
+      acc = 1;
+    }
+#undef BWD_ISSUE
+    if (elect_one()) mma_commit(bar_fin);   // the last item's wgrad is still in flight
+    __syncwarp();
+  } else if (tma_warp) {
+    // ---- the TMA warp: item j goes into ring slot j % 3 once item j - 3 has released it
+    uint32_t ph_f = 0;
+    while (ld_tile * ROWS < S) {
+      mbar_wait(sbase + BwdSmem::bar_free + 8 * ld_slot, (ph_f >> ld_slot) & 1u);
+      ph_f ^= 1u << ld_slot;
+      load_next();
+    }
+  } else {
+  // ---- the epilogue warps.  One item: this thread's part of dY is in Y[ys]; hand the item to the MMA warp, do what does
+  // not need the dgrad under the MMAs' latency, wait for the dgrad, advance.
+#define BWD_ITEM(UNDER_MMA_STMT)                                                             \
+  do {                                                                                       \
+    fence_async_smem(); fence_before(); __syncwarp();                                        \
+    if (lane == 0) mbar_arrive(bar_y);                                                       \
+    wait_x();                                                                                \
+    UNDER_MMA_STMT;                                                                          \
     mbar_wait(bar_mma, ph_mma); ph_mma ^= 1; fence_after();                                  \
-    if (warp == 0 && items > 0) load_next();                                                 \
     items += 1;                                                                              \
     xs = xs == 2 ? 0u : xs + 1u; ys ^= 1u;                                                   \
   } while (0)
 
   // the first item's inputs (dL/dc * c (1 - c), sigma, dL/dsigma of this thread's sample): global loads, fetched for the
   // NEXT tile under the last item's MMAs
-  float in_dc[3] = {0.f, 0.f, 0.f}, in_sig = 0.f, in_dsig = 0.f;
+  // (raw values only: the arithmetic on them waits until the top of that tile, so nothing here stalls on the loads)
+  float in_col[3] = {0.f, 0.f, 0.f}, in_dc[3] = {0.f, 0.f, 0.f}, in_sig = 0.f, in_dsig = 0.f;
   auto fetch_inputs = [&](uint64_t tile) {
     const uint64_t s = tile * ROWS + row;
-    in_dc[0] = in_dc[1] = in_dc[2] = 0.f; in_sig = 0.f; in_dsig = 0.f;
+    in_col[0] = in_col[1] = in_col[2] = 0.f; in_dc[0] = in_dc[1] = in_dc[2] = 0.f; in_sig = 0.f; in_dsig = 0.f;
     if (half == 0 && s < S) {
 #pragma unroll
       for (int c = 0; c < 3; ++c) {
-        const float col = ws.rgb[3 * s + c];
-        in_dc[c] = ws.drgb[3 * s + c] * col * (1.f - col) * scale;
+        in_col[c] = ws.rgb[3 * s + c];
+        in_dc[c] = ws.drgb[3 * s + c];
       }
       in_sig = ws.sigma[s];
       in_dsig = ws.dsigma[s];
@@ -745,27 +808,20 @@ __global__ void __launch_bounds__(BWD_THREADS, 2) mlp_backward_tc_kernel(MlpShap
     if (half == 0) {
 #pragma unroll
       for (int j = 0; j < 16; ++j) v[j] = 0.f;
-      v[0] = in_dc[0]; v[1] = in_dc[1]; v[2] = in_dc[2];
+#pragma unroll
+      for (int c = 0; c < 3; ++c) v[c] = in_dc[c] * in_col[c] * (1.f - in_col[c]) * scale;
       emit16<T, false>(v, bufY(), nullptr, row, 0, true);
     }
-    wait_x();
     uint32_t mask = 0;   // ReLU mask of the item's saved activation: needed by the NEXT item's dY, read under this item's MMAs
-    BWD_ITEM(issue_wgrad(tmem_base + GW_C3, sX(), sY(), 16, fmt, acc),
-             issue_layer(tmem_base + COL_G, sY(), sW + WImg::b_c3, 16, H, H, fmt, bar_mma),
-             mask = row_mask32<T>(bufX(), row, cb));
+    BWD_ITEM(mask = row_mask32<T>(bufX(), row, cb));
     // ---- second colour hidden layer
     if (two) {
       masked_to_Y<T>(tlane, mask, bufY(), row, cb);
-      wait_x();
-      BWD_ITEM(issue_wgrad(tmem_base + GW_C2, sX(), sY(), H, fmt, acc),
-               issue_layer(tmem_base + COL_G, sY(), sW + WImg::b_c2, H, H, H, fmt, bar_mma),
-               mask = row_mask32<T>(bufX(), row, cb));
+      BWD_ITEM(mask = row_mask32<T>(bufX(), row, cb));
     }
-    // ---- first colour layer: dY = d h1 (masked); X = [g slice, Y(d), 0]; wgrad transposed: G^T = dY^T X
+    // ---- first colour layer: dY = d h1 (masked); X = [g slice, Y(d), 0]
     masked_to_Y<T>(tlane, mask, bufY(), row, cb);
-    wait_x();
-    BWD_ITEM(issue_wgrad(tmem_base + GW_C1T, sY(), sX(), CIP, fmt, acc),
-             issue_layer(tmem_base + COL_G, sY(), sW + WImg::b_c1, H, CIP, CIP, fmt, bar_mma), (void)0);
+    BWD_ITEM((void)0);
     // ---- density output layer: dg = [geo slice of d ci] + e_0 * dL/dsigma * sigma (0 where clamped)
     if (half == 0) {
       float dci[CIP], dg[16];
@@ -784,15 +840,10 @@ __global__ void __launch_bounds__(BWD_THREADS, 2) mlp_backward_tc_kernel(MlpShap
       if (valid && sig > 3.0590232e-07f * 1.0001f && sig < 3269017.4f * 0.9999f) dg[0] += dsig * sig * scale;
       emit16<T, false>(dg, bufY(), nullptr, row, 0, true);
     }
-    wait_x();
-    BWD_ITEM(issue_wgrad(tmem_base + GW_D2, sX(), sY(), 16, fmt, acc),
-             issue_layer(tmem_base + COL_G, sY(), sW + WImg::b_d2, 16, H, H, fmt, bar_mma),
-             mask = row_mask32<T>(bufX(), row, cb));
+    BWD_ITEM(mask = row_mask32<T>(bufX(), row, cb));
     // ---- density hidden layer: dY = d hd (masked); X = e
     masked_to_Y<T>(tlane, mask, bufY(), row, cb);
-    wait_x();
-    BWD_ITEM(issue_wgrad(tmem_base + GW_D1, sX(), sY(), H, fmt, acc),
-             issue_layer(tmem_base + COL_G, sY(), sW + WImg::b_d1, H, LF, LF, fmt, bar_mma), fetch_inputs(tile + gridDim.x));
+    BWD_ITEM(fetch_inputs(tile + gridDim.x));
     // ---- dL/de -> planes; the two column halves take the 16-column chunks of the LF columns alternately
     for (uint32_t c0 = half * 16; c0 < LF; c0 += 32) {
       tmem_ld16(tlane + COL_G + c0, v);
@@ -801,17 +852,12 @@ __global__ void __launch_bounds__(BWD_THREADS, 2) mlp_backward_tc_kernel(MlpShap
 #pragma unroll
         for (int j = 0; j < 16; ++j) ws.de[(size_t)(c0 + j) * ws.cap + s] = v[j] * inv_scale;
     }
-    acc = 1;   // (the next item's __syncthreads follows these reads of COL_G, before its dgrad overwrites it)
+    // (the next item's arrival on bar_y follows these reads of COL_G, before the MMA warp's next dgrad overwrites it)
   }
 #undef BWD_ITEM
-  // ---- the last item's wgrad is still in flight: one more commit, then flush the CTA's weight gradients
-  fence_before();
-  __syncthreads();
-  if (warp == 0) {
-    fence_after();
-    if (elect_one()) mma_commit(bar_mma);
   }
-  mbar_wait(bar_mma, ph_mma); ph_mma ^= 1;
+  // ---- every MMA of the CTA done (the MMA warp's last commit), then flush the CTA's weight gradients
+  mbar_wait(bar_fin, 0);
   fence_after();
   // Each CTA stores its sums into its own slice of ws.wgrad_part with plain, lane-coalesced stores; the slices are
   // summed by the consumer (the MLP Adam kernel, or reduce_wgrad_kernel).  Atomics onto the 9-11 K shared addresses
@@ -831,6 +877,7 @@ __global__ void __launch_bounds__(BWD_THREADS, 2) mlp_backward_tc_kernel(MlpShap
         }
     }
   };
+  if (!mma_warp) {
   flush(GW_C3, ms.o_c3, 3, H, 16);
   if (two) flush(GW_C2, ms.o_c2, H, H, H);
   {   // transposed accumulator: rows = outputs, columns = inputs
@@ -846,6 +893,7 @@ __global__ void __launch_bounds__(BWD_THREADS, 2) mlp_backward_tc_kernel(MlpShap
   }
   flush(GW_D2, ms.o_d2, DO, H, 16);
   flush(GW_D1, ms.o_d1, H, LF, H);
+  }
   fence_before();
   __syncthreads();
   if (warp == 0) tmem_free<BWD_COLS>(tmem_base);

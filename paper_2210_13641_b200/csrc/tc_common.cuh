@@ -118,6 +118,10 @@ __device__ __forceinline__ void mbar_wait(uint32_t bar_saddr, uint32_t parity) {
   }
 }
 
+__device__ __forceinline__ void mbar_arrive(uint32_t bar_saddr) {   // release at CTA scope
+  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar_saddr) : "memory");
+}
+
 // ---- TMA 1-D bulk copies (cp.async.bulk, SASS UBLKCP): global -> shared, completion on an mbarrier ----
 __device__ __forceinline__ void mbar_expect_tx(uint32_t bar_saddr, uint32_t bytes) {
   asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar_saddr), "r"(bytes) : "memory");
