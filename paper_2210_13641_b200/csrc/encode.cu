@@ -365,21 +365,36 @@ __global__ void __launch_bounds__(256) scatter_backward_kernel(LevelTable lv, fl
   tl_mark(ws.timeline, K_SCATTER, 1);
 }
 
-// gradient array <- canonical gradient and flags (debug / test entry point)
-__global__ void set_grad_kernel(float *__restrict__ grad, uint32_t F, uint64_t n_entries, const float *__restrict__ src,
+// canonical entry -> storage entry (EntryMap, nsm_internal.cuh)
+__device__ __forceinline__ uint64_t storage_entry(const EntryMap &m, uint64_t e_canon) {
+  uint32_t l = 0;
+  while (l + 1 < m.n_levels && e_canon >= m.canon[l + 1]) ++l;
+  return m.storage[l] + (e_canon - m.canon[l]);
+}
+// storage entry -> canonical entry, or ~0 for a padding entry
+__device__ __forceinline__ uint64_t canonical_entry(const EntryMap &m, uint64_t e_storage) {
+  uint32_t l = 0;
+  while (l + 1 < m.n_levels && e_storage >= m.storage[l + 1]) ++l;
+  const uint64_t i = e_storage - m.storage[l];
+  return i < m.canon[l + 1] - m.canon[l] ? m.canon[l] + i : ~0ull;
+}
+
+// gradient array <- canonical gradient and flags (debug / test entry point); walks the STORAGE array, padding included
+__global__ void set_grad_kernel(float *__restrict__ grad, uint32_t F, uint64_t n_entries, EntryMap map, const float *__restrict__ src,
                                 const uint8_t *__restrict__ touched) {
   const uint64_t total = n_entries * F;
   for (uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; i < total; i += (uint64_t)gridDim.x * blockDim.x) {
-    const uint64_t e = i / F;
-    const bool t = src && (!touched || touched[e]);
-    const float v = t ? src[i] : 0.f;
+    const uint64_t es = i / F;
+    const uint64_t e = src ? canonical_entry(map, es) : ~0ull;
+    const bool t = e != ~0ull && (!touched || touched[e]);
+    const float v = t ? src[e * F + (i - es * F)] : 0.f;
     grad[i] = t ? (fabsf(v) < NSM_GRAD_MIN_ADDEND ? 0.0f : v) : __uint_as_float(NSM_GRAD_UNTOUCHED);
   }
 }
 
-__global__ void get_touched_kernel(const float *__restrict__ grad, uint32_t F, uint64_t n_entries, uint8_t *__restrict__ dst) {
-  for (uint64_t e = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; e < n_entries; e += (uint64_t)gridDim.x * blockDim.x)
-    dst[e] = __float_as_uint(grad[e * F]) != NSM_GRAD_UNTOUCHED;
+__global__ void get_touched_kernel(const float *__restrict__ grad, uint32_t F, uint64_t n_canon, EntryMap map, uint8_t *__restrict__ dst) {
+  for (uint64_t e = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; e < n_canon; e += (uint64_t)gridDim.x * blockDim.x)
+    dst[e] = __float_as_uint(grad[storage_entry(map, e) * F]) != NSM_GRAD_UNTOUCHED;
 }
 
 __global__ void debug_slots_kernel(LevelTable lv, Workspace ws, const uint32_t *__restrict__ d_S,
@@ -411,38 +426,42 @@ __global__ void planes_to_rows_kernel(const float *__restrict__ planes, uint64_t
 }
 
 __device__ __forceinline__ uint64_t param_index(uint32_t F, uint64_t e, uint32_t f, int which) {
-  return which == 0 ? e * F + f : e * 2 * F + (which == 3 ? F : 0) + f;
+  return which <= 1 ? e * F + f : e * 2 * F + (which == 3 ? F : 0) + f;
 }
 
-__global__ void pack_records_kernel(float *__restrict__ theta, float *__restrict__ mv, uint32_t F, uint64_t n_entries, int which,
-                                    const float *__restrict__ src) {
+// walks the STORAGE arrays: padding entries become zeros
+__global__ void pack_records_kernel(float *__restrict__ theta, float *__restrict__ mv, uint32_t F, uint64_t n_entries, EntryMap map,
+                                    int which, const float *__restrict__ src) {
   const uint64_t total = n_entries * F;
   float *dst = which == 0 ? theta : mv;
   for (uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; i < total; i += (uint64_t)gridDim.x * blockDim.x) {
-    const uint64_t e = i / F;
-    dst[param_index(F, e, (uint32_t)(i - e * F), which)] = src ? src[i] : 0.f;
+    const uint64_t es = i / F;
+    const uint32_t f = (uint32_t)(i - es * F);
+    const uint64_t e = src ? canonical_entry(map, es) : ~0ull;
+    dst[param_index(F, es, f, which)] = e != ~0ull ? src[e * F + f] : 0.f;
   }
 }
 
-__global__ void unpack_records_kernel(const float *__restrict__ theta, const float *__restrict__ mv, uint32_t F, uint64_t n_entries,
-                                      int which, float *__restrict__ dst) {
-  const uint64_t total = n_entries * F;
-  const float *src = which == 0 ? theta : mv;
+// walks the canonical array; which == 1: the gradient array ("untouched" words read as -0.0)
+__global__ void unpack_records_kernel(const float *__restrict__ theta, const float *__restrict__ mv, const float *__restrict__ grad,
+                                      uint32_t F, uint64_t n_canon, EntryMap map, int which, float *__restrict__ dst) {
+  const uint64_t total = n_canon * F;
+  const float *src = which == 0 ? theta : (which == 1 ? grad : mv);
   for (uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; i < total; i += (uint64_t)gridDim.x * blockDim.x) {
     const uint64_t e = i / F;
-    dst[i] = src[param_index(F, e, (uint32_t)(i - e * F), which)];
+    dst[i] = src[param_index(F, storage_entry(map, e), (uint32_t)(i - e * F), which)];
   }
 }
 
 }  // namespace
 
 int launch_pack_records(const FieldParams &fp, int which, const float *src, cudaStream_t st) {
-  pack_records_kernel<<<2048, 256, 0, st>>>(fp.theta, fp.mv, fp.F, fp.n_entries, which, src);
+  pack_records_kernel<<<2048, 256, 0, st>>>(fp.theta, fp.mv, fp.F, fp.n_entries, fp.map, which, src);
   return 1;
 }
 
 int launch_unpack_records(const FieldParams &fp, int which, float *dst, cudaStream_t st) {
-  unpack_records_kernel<<<2048, 256, 0, st>>>(fp.theta, fp.mv, fp.F, fp.n_entries, which, dst);
+  unpack_records_kernel<<<2048, 256, 0, st>>>(fp.theta, fp.mv, fp.grad, fp.F, fp.n_canon, fp.map, which, dst);
   return 1;
 }
 
@@ -480,12 +499,12 @@ int launch_encode(const LevelTable &lv, const float *theta, const Workspace &ws,
 }
 
 int launch_set_grad(const FieldParams &fp, const float *src, const uint8_t *touched, cudaStream_t st) {
-  set_grad_kernel<<<2048, 256, 0, st>>>(fp.grad, fp.F, fp.n_entries, src, touched);
+  set_grad_kernel<<<2048, 256, 0, st>>>(fp.grad, fp.F, fp.n_entries, fp.map, src, touched);
   return 1;
 }
 
 int launch_get_touched(const FieldParams &fp, uint8_t *dst, cudaStream_t st) {
-  get_touched_kernel<<<2048, 256, 0, st>>>(fp.grad, fp.F, fp.n_entries, dst);
+  get_touched_kernel<<<2048, 256, 0, st>>>(fp.grad, fp.F, fp.n_canon, fp.map, dst);
   return 1;
 }
 

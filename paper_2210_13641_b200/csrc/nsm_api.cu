@@ -132,6 +132,7 @@ struct nsm_field {
   bool scatter_pending = false;   // the backward pass stopped before S12: enqueue_adam issues the scatter right before the table Adam
   uint32_t wgrad_parts = 0;   // > 0: the MLP weight gradient of the last backward is still in that many per-CTA slices
   bool batch_ready = false;   // NSM_OPT_BATCH_READY
+  bool render_interleave = true;   // NSM_OPT_RENDER_INTERLEAVE
   bool side_ok = false;       // nothing but a train step's Adam has been enqueued on `stream` since ev_pre_adam
   const char *mlp_path = "simt_fp32";
   bool use_tc = false;   // tcgen05 MLP kernels (16-bit configurations with supported shapes)
@@ -153,13 +154,17 @@ namespace {
 
 // S0 — integer level table: N_l = floor(N_min * exp(l ln(N_max/N_min)/(L-1)) + 1e-6) in float64,
 // ends forced; E_l = min((N_l+1)^3, T); dense iff (N_l+1)^3 <= T.
-nsm_status build_levels(const nsm_field_config &c, LevelTable &lv) {
+// lv.offset: storage offsets, each level on a 16-byte boundary; map: canonical <-> storage (EntryMap, nsm_internal.cuh)
+nsm_status build_levels(const nsm_field_config &c, LevelTable &lv, EntryMap &map) {
   const uint32_t L = c.n_levels;
   const uint64_t T = 1ull << c.log2_table_size;
+  const uint64_t align = c.n_features >= 4 ? 1 : 4 / c.n_features;   // entries per 16 bytes
   lv.n_levels = L;
   lv.n_features = c.n_features;
   lv.t_mask = (uint32_t)(T - 1);
   lv.offset[0] = 0;
+  map.n_levels = L;
+  map.canon[0] = map.storage[0] = 0;
   for (uint32_t l = 0; l < L; ++l) {
     uint32_t N;
     if (l == 0) N = c.n_min;
@@ -171,7 +176,10 @@ nsm_status build_levels(const nsm_field_config &c, LevelTable &lv) {
     lv.res[l] = N;
     const uint64_t side = (uint64_t)N + 1, cube = side * side * side;
     lv.dense[l] = cube <= T;
-    lv.offset[l + 1] = lv.offset[l] + (cube <= T ? cube : T);
+    const uint64_t n_l = cube <= T ? cube : T;
+    map.canon[l + 1] = map.canon[l] + n_l;
+    lv.offset[l + 1] = (lv.offset[l] + n_l + align - 1) / align * align;
+    map.storage[l + 1] = lv.offset[l + 1];
   }
   return NSM_OK;
 }
@@ -291,10 +299,12 @@ MarchParams make_march(const nsm_field *f, const nsm_ray_batch *b, uint32_t R, b
 // sample_draw >= 0: the batch is first drawn from the keyframe store (F1) into b's buffers (the field's staging area),
 // on the stream the marcher runs on.
 nsm_status enqueue_forward(nsm_field *f, const nsm_ray_batch *b, uint32_t R, bool jitter, uint32_t step, bool train,
-                           bool march_on_side = false, float *dirs_copy = nullptr, int64_t sample_draw = -1) {
+                           bool march_on_side = false, float *dirs_copy = nullptr, int64_t sample_draw = -1,
+                           bool interleave = false) {
   const uint32_t *d_S = f->ws.offsets + R;
   const float *mlp_dirs = dirs_copy ? dirs_copy : b->dirs;
   MarchParams mp = make_march(f, b, R, jitter, step);
+  mp.interleave = interleave ? 1u : 0u;
   if (march_on_side && !f->prof.on) {
     if (!f->side_ok) {   // other work has been enqueued on the main stream since the last Adam: order behind all of it
       CUDA_TRY(cudaEventRecord(f->ev_main, f->stream));
@@ -505,7 +515,7 @@ nsm_status nsm_create_field(const nsm_field_config *cfg, void *cuda_stream, nsm_
   f->device = dev;
   f->stream = (cudaStream_t)cuda_stream;
   f->n_sms = prop.multiProcessorCount;
-  build_levels(*cfg, f->lv);
+  build_levels(*cfg, f->lv, f->fp.map);
   MlpShape &ms = f->ms;
   ms.LF = cfg->n_levels * cfg->n_features;
   ms.Hd = cfg->density_hidden; ms.Do = cfg->density_out;
@@ -540,7 +550,8 @@ nsm_status nsm_create_field(const nsm_field_config *cfg, void *cuda_stream, nsm_
   }
   FieldParams &fp = f->fp;
   fp.n_entries = f->lv.offset[cfg->n_levels];
-  fp.n_table = fp.n_entries * cfg->n_features;
+  fp.n_canon = fp.map.canon[cfg->n_levels];
+  fp.n_table = fp.n_canon * cfg->n_features;
   fp.n_mlp = ms.n_mlp;
   fp.F = cfg->n_features;
   Workspace &ws = f->ws;
@@ -551,14 +562,15 @@ nsm_status nsm_create_field(const nsm_field_config *cfg, void *cuda_stream, nsm_
   const uint32_t R = cfg->max_rays;
   cudaError_t e = cudaSuccess;
   auto A = [&](cudaError_t r) { if (e == cudaSuccess) e = r; };
-  A(f->alloc(&fp.theta, fp.n_table)); A(f->alloc(&fp.mv, 2 * fp.n_table));
+  const uint64_t n_store = fp.n_entries * cfg->n_features;   // floats of a storage array (padding included)
+  A(f->alloc(&fp.theta, n_store)); A(f->alloc(&fp.mv, 2 * n_store));
   A(f->alloc(&fp.mlp_theta, fp.n_mlp)); A(f->alloc(&fp.mlp_m, fp.n_mlp)); A(f->alloc(&fp.mlp_v, fp.n_mlp)); A(f->alloc(&fp.mlp_grad, fp.n_mlp));
-  A(f->alloc(&fp.grad, fp.n_table, false)); A(f->alloc(&fp.occ_bits, (G3 + 7) / 8 + 4));
+  A(f->alloc(&fp.grad, n_store, false)); A(f->alloc(&fp.occ_bits, (G3 + 7) / 8 + 4));
   A(f->alloc(&fp.occ_grid, G3));
   A(f->alloc(&ws.counts, R)); A(f->alloc(&ws.offsets, R + 1)); A(f->alloc(&ws.scan_state, march_scan_state_entries(R) + 1)); A(f->alloc(&ws.scan_ctr, 2)); A(f->alloc(&ws.work_ctr, 8));
   A(f->alloc(&ws.C, 3 * (size_t)R)); A(f->alloc(&ws.D_hat, R)); A(f->alloc(&ws.O, R));
   A(f->alloc(&ws.s_ray, cap)); A(f->alloc(&ws.s_k, cap)); A(f->alloc(&ws.s_t, cap)); A(f->alloc(&ws.s_delta, cap));
-  A(f->alloc(&ws.s_x, 3 * cap));
+  A(f->alloc(&ws.s_x, 3 * cap)); A(f->alloc(&ws.s_idx, cap));
   ws.e = ws.hd = ws.g = ws.h1 = ws.h2 = nullptr;
   ws.blob_e = ws.blob_hd = ws.blob_ci = ws.blob_h1 = ws.blob_h2 = ws.wimg_fwd = ws.wimg_bwd = nullptr;
   ws.wgrad_part = nullptr;
@@ -663,9 +675,9 @@ nsm_status nsm_get_level_table(const nsm_field *f, uint32_t *res, uint64_t *offs
   if (!f) return fail(NSM_ERR_INVALID_ARG, "field is NULL");
   for (uint32_t l = 0; l < f->lv.n_levels; ++l) {
     if (res) res[l] = f->lv.res[l];
-    if (offset) offset[l] = f->lv.offset[l];
+    if (offset) offset[l] = f->fp.map.canon[l];
   }
-  if (offset) offset[f->lv.n_levels] = f->lv.offset[f->lv.n_levels];
+  if (offset) offset[f->lv.n_levels] = f->fp.map.canon[f->lv.n_levels];
   return NSM_OK;
 }
 
@@ -1025,6 +1037,7 @@ nsm_status nsm_set_option(nsm_field *f, nsm_option opt, uint32_t value) {
       return NSM_OK;
     }
     case NSM_OPT_POSE_LEVELS: f->pose_levels = value; return NSM_OK;
+    case NSM_OPT_RENDER_INTERLEAVE: f->render_interleave = value != 0; return NSM_OK;
     case NSM_OPT_DEBUG_TIMELINE: {
       LEAVE_FAST_PATH(f);
       if (value && !f->timeline_base) {
@@ -1072,9 +1085,9 @@ static nsm_status render_chunks(nsm_field *f, const nsm_ray_batch *b, float cut,
       cb.origins = b->origins + 3 * (size_t)first;
       cb.dirs = b->dirs + 3 * (size_t)first;
     }
-    st = enqueue_forward(f, &cb, R, false, 0, false);
+    st = enqueue_forward(f, &cb, R, false, 0, false, false, nullptr, -1, f->render_interleave);
     if (st != NSM_OK) return st;
-    RUN(f, K_COMPOSITE, launch_composite_render(f->ws, R, cut, f->cfg.bg, o_rgb, o_d, o_op, f->stream));
+    RUN(f, K_COMPOSITE, launch_composite_render(f->ws, R, cut, f->cfg.bg, o_rgb, o_d, o_op, f->stream, f->render_interleave));
     if (f->prof.on) f->prof.collect();
     if (host) {
       CUDA_TRY(cudaMemcpyAsync(rgb + 3 * (size_t)first, o_rgb, sizeof(float) * 3 * R, cudaMemcpyDeviceToHost, f->stream));
@@ -1127,7 +1140,7 @@ nsm_status nsm_debug_last_step(nsm_field *f, int item, void *d_out, uint64_t cap
     case NSM_DBG_DSIGMA: src = ws.dsigma; bytes = 4ull * S; break;
     case NSM_DBG_DRGB: src = ws.drgb; bytes = 12ull * S; break;
     case NSM_DBG_GRAD: bytes = 4ull * (f->fp.n_table + f->fp.n_mlp); break;
-    case NSM_DBG_TOUCHED: bytes = f->fp.n_entries; break;
+    case NSM_DBG_TOUCHED: bytes = f->fp.n_canon; break;
     case NSM_DBG_SAMPLE_X: bytes = 12ull * S; break;
     case NSM_DBG_E: bytes = 4ull * S * f->ms.LF; break;
     case NSM_DBG_SLOTS: bytes = 4ull * S * L * 8; break;
@@ -1148,7 +1161,7 @@ nsm_status nsm_debug_last_step(nsm_field *f, int item, void *d_out, uint64_t cap
   } else if (item == NSM_DBG_TOUCHED) {
     RUN(f, K_DEBUG, launch_get_touched(f->fp, (uint8_t *)d_out, f->stream));
   } else if (item == NSM_DBG_GRAD) {
-    CUDA_TRY(cudaMemcpyAsync(d_out, f->fp.grad, sizeof(float) * f->fp.n_table, cudaMemcpyDeviceToDevice, f->stream));
+    RUN(f, K_DEBUG, launch_unpack_records(f->fp, 1, (float *)d_out, f->stream));
     CUDA_TRY(cudaMemcpyAsync((float *)d_out + f->fp.n_table, f->fp.mlp_grad, sizeof(float) * f->fp.n_mlp, cudaMemcpyDeviceToDevice, f->stream));
   } else if (item == NSM_DBG_SAMPLE_X) {
     RUN(f, K_DEBUG, launch_planes_to_rows(ws.s_x, ws.cap, 3, d_S, (float *)d_out, f->stream));

@@ -15,7 +15,19 @@ struct LevelTable {
   uint32_t n_levels, n_features, t_mask;
   uint32_t res[NSM_MAX_LEVELS];
   uint32_t dense[NSM_MAX_LEVELS];      // 1: slot = vx + (N+1)(vy + (N+1) vz); 0: hashed
-  uint64_t offset[NSM_MAX_LEVELS + 1]; // in entries
+  uint64_t offset[NSM_MAX_LEVELS + 1]; // in entries, of the STORAGE arrays (theta, m|v, grad): every level starts on a 16-byte
+                                       // boundary (see EntryMap); the canonical offsets of include/nsm.h are EntryMap::canon
+};
+
+// Canonical entry index (include/nsm.h: levels back to back) <-> storage entry index.  A level's slice of the storage
+// arrays starts at a multiple of 16 bytes (4 / F entries for F < 4), so that the x-neighbour corners (x, x + 1) of an even
+// cell x -- adjacent slots on a dense level and, the hash XORing x in unmultiplied, on a hashed level too -- form an
+// ALIGNED 16-byte pair for F = 2 whatever the sizes of the levels before (config 2: the five dense levels hold an odd
+// number of entries, which left every hashed level's pairs straddling a boundary).  The padding entries are never
+// referenced: theta 0, gradient "untouched" for ever.  Used by the boundary kernels only (pack / unpack / debug).
+struct EntryMap {
+  uint32_t n_levels;
+  uint64_t canon[NSM_MAX_LEVELS + 1], storage[NSM_MAX_LEVELS + 1];
 };
 
 // Offsets (floats) of the MLP matrices inside the MLP block (canonical order) and their shapes.
@@ -31,6 +43,7 @@ struct MarchParams {
   uint32_t K, G, C, jitter, step;   // C: occupancy cascades (F4)
   uint64_t seed;
   uint32_t R;
+  uint32_t interleave = 0;          // forward-only rendering: (k, ray) sample order inside each block of rays (march.cu)
 };
 
 // Per-step device workspace.  All per-sample arrays are planes of `cap` floats (cap = capacity,
@@ -47,6 +60,7 @@ struct Workspace {
   float *C, *D_hat, *O;  // [R,3], [R], [R]
   // samples
   uint32_t *s_ray, *s_k; // [cap]
+  uint32_t *s_idx;       // [cap] interleaved rendering only: position of ray r's i-th live sample at [offsets[r] + i]
   float *s_t, *s_delta;  // [cap]
   float *s_x;            // [3][cap] planes
   float *e;              // [LF][cap]
@@ -150,8 +164,10 @@ struct FieldParams {
   float *mlp_theta, *mlp_m, *mlp_v, *mlp_grad;      // [n_mlp] each, canonical order
   uint8_t *occ_bits;                                // [G^3/8]
   float *occ_grid;                                  // [G^3] running density of the decayed refresh (F4); seeded by FROM_FIELD
-  uint64_t n_entries, n_table, n_mlp;
+  uint64_t n_entries;                               // STORAGE entries (padding included): array sizes, the table Adam's range
+  uint64_t n_canon, n_table, n_mlp;                 // canonical entries, n_table = n_canon * F parameters (the boundary's count)
   uint32_t F;
+  EntryMap map;
 };
 
 // ---- programmatic dependent launch (PDL) ---------------------------------------------------------
@@ -296,7 +312,7 @@ int launch_scatter(const LevelTable &lv, float *grad, const Workspace &ws, const
 // gradient array <- canonical gradient + touched flags (NULL: every entry touched); src == nullptr: all untouched
 int launch_set_grad(const FieldParams &fp, const float *src, const uint8_t *touched, cudaStream_t st);
 int launch_get_touched(const FieldParams &fp, uint8_t *dst, cudaStream_t st);
-// canonical [n_entries][F] <-> `which` (0 theta, 2 m, 3 v) of the internal arrays; src == nullptr packs zeros
+// canonical [n_canon][F] <-> `which` (0 theta, 1 gradient (unpack only), 2 m, 3 v) of the internal arrays; src == nullptr packs zeros
 int launch_pack_records(const FieldParams &fp, int which, const float *src, cudaStream_t st);
 int launch_unpack_records(const FieldParams &fp, int which, float *dst, cudaStream_t st);
 int launch_mlp_forward_simt(const MlpShape &ms, const float *theta_mlp, const float *dirs,
@@ -324,8 +340,9 @@ int launch_blob_to_rows(int bf16, const uint8_t *blob, uint32_t n_cols, int two_
 int launch_composite_train(const Workspace &ws, uint32_t R, const float *rgb, const float *depth,
                            const float *depth_var, float lambda_d, const float bg[3],
                            cudaStream_t st);
+// interleaved: the samples are in the rendering marcher's (k, ray) order (MarchParams::interleave), reached through ws.s_idx
 int launch_composite_render(const Workspace &ws, uint32_t R, float cut, const float bg[3],
-                            float *out_rgb, float *out_depth, float *out_opacity, cudaStream_t st);
+                            float *out_rgb, float *out_depth, float *out_opacity, cudaStream_t st, bool interleaved);
 // S13 on the touched table entries (sparse) or on all of them; consumes the gradients (every word back to "untouched")
 int launch_adam_table(const FieldParams &fp, uint32_t F, int sparse, float lr, float beta1, float beta2,
                       float eps, float inv_bc1, float inv_bc2, cudaStream_t st, unsigned long long *tl = nullptr);
