@@ -30,7 +30,6 @@ __global__ void __launch_bounds__(256) encode_forward_kernel(LevelTable lv, cons
   const uint64_t S_it = MODE == 0 ? S : ((S + NSM_TILE - 1) / NSM_TILE) * NSM_TILE;
   const uint64_t total = S_it * lv.n_levels;
   const uint32_t LF = lv.n_levels * F;
-  const uint64_t pol_first = l2_evict_first(), pol_normal = l2_evict_normal();
   const uint32_t lane = threadIdx.x & 31;
   ChunkQueue q(ws.work_ctr, seq);
   for (;;) {   // 256 consecutive (level, sample) items at a time, handed out in order (see ChunkQueue); warp-uniform
@@ -70,27 +69,8 @@ __global__ void __launch_bounds__(256) encode_forward_kernel(LevelTable lv, cons
     if (gathers) {
       const float *tab = theta + lv.offset[l] * F;
       // coarse (dense) levels are re-read every step: default policy; hashed levels stream through L2
-      const uint64_t pol = lv.dense[l] ? pol_normal : pol_first;
-      if constexpr (F == 2) {
-        // x-neighbour corners that form an aligned pair of entries come in with one 16-byte load (see issue_corner_reds)
-        const uint64_t e_l = lv.offset[l];
-#pragma unroll
-        for (int k = 0; k < 8; k += 2) {
-          const uint64_t a0 = e_l + ci.slot[k], a1 = e_l + ci.slot[k + 1];
-          if ((a0 ^ a1) == 1ull) {
-            const float4 q = ld_hint_f4(theta + (a0 & ~1ull) * 2, pol);
-            const bool odd = a0 & 1ull;
-            v[k][0] = odd ? q.z : q.x; v[k][1] = odd ? q.w : q.y;
-            v[k + 1][0] = odd ? q.x : q.z; v[k + 1][1] = odd ? q.y : q.w;
-          } else {
-            load_entry_hint<2>(tab + (size_t)ci.slot[k] * 2, v[k], pol);
-            load_entry_hint<2>(tab + (size_t)ci.slot[k + 1] * 2, v[k + 1], pol);
-          }
-        }
-      } else {
-#pragma unroll
-        for (int k = 0; k < 8; ++k) load_entry_hint<F>(tab + (size_t)ci.slot[k] * F, v[k], pol);  // 8 gathers in flight
-      }
+      if (lv.dense[l]) gather_corners<F, NSM_L2_EVICT_NORMAL>(tab, ci.slot, v);
+      else gather_corners<F, NSM_L2_EVICT_FIRST>(tab, ci.slot, v);
     }
     if (one_dense_level) {
 #pragma unroll
@@ -174,7 +154,6 @@ __global__ void __launch_bounds__(256) encode_forward_panel_kernel(LevelTable lv
   const uint64_t S_it = ((S + NSM_TILE - 1) / NSM_TILE) * NSM_TILE;     // whole tiles: rows beyond S are zero-filled
   const uint32_t LF = lv.n_levels * F, n_panels = LF / 8;               // LF is a multiple of 16 on this path
   const uint64_t total = S_it * n_panels;
-  const uint64_t pol_first = l2_evict_first(), pol_normal = l2_evict_normal();
   const uint32_t lane = threadIdx.x & 31;
   const size_t half = (size_t)LF * NSM_TILE * 2;   // two-term tile: [hi: LF*256 bytes][lo: LF*256 bytes] per 128-sample tile
   ChunkQueue q(ws.work_ctr, seq);
@@ -215,26 +194,8 @@ __global__ void __launch_bounds__(256) encode_forward_panel_kernel(LevelTable lv
         for (int f = 0; f < F; ++f) v[k][f] = 0.f;
       if (gathers) {
         const float *tab = theta + lv.offset[l] * F;
-        const uint64_t pol = dense ? pol_normal : pol_first;
-        if constexpr (F == 2) {
-          const uint64_t e_l = lv.offset[l];
-#pragma unroll
-          for (int k = 0; k < 8; k += 2) {
-            const uint64_t a0 = e_l + ci.slot[k], a1 = e_l + ci.slot[k + 1];
-            if ((a0 ^ a1) == 1ull) {
-              const float4 qv = ld_hint_f4(theta + (a0 & ~1ull) * 2, pol);
-              const bool odd = a0 & 1ull;
-              v[k][0] = odd ? qv.z : qv.x; v[k][1] = odd ? qv.w : qv.y;
-              v[k + 1][0] = odd ? qv.x : qv.z; v[k + 1][1] = odd ? qv.y : qv.w;
-            } else {
-              load_entry_hint<2>(tab + (size_t)ci.slot[k] * 2, v[k], pol);
-              load_entry_hint<2>(tab + (size_t)ci.slot[k + 1] * 2, v[k + 1], pol);
-            }
-          }
-        } else {
-#pragma unroll
-          for (int k = 0; k < 8; ++k) load_entry_hint<F>(tab + (size_t)ci.slot[k] * F, v[k], pol);
-        }
+        if (dense) gather_corners<F, NSM_L2_EVICT_NORMAL>(tab, ci.slot, v);
+        else gather_corners<F, NSM_L2_EVICT_FIRST>(tab, ci.slot, v);
       }
       if (dense) {
 #pragma unroll

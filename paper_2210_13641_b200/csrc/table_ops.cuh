@@ -103,6 +103,51 @@ __device__ __forceinline__ void red_add_entry(float *p, const float g[F], uint64
   }
 }
 
+// L2 cache-policy words as compile-time constants (the values createpolicy.fractional.L2::evict_*.b64 ..., 1.0 returns;
+// published in CUTLASS as CacheHintSm90).  A policy that is an immediate lives in a uniform register: with a policy held in
+// a per-thread variable every hinted load paid two R2UR moves (the encoder's instruction stream, not its memory traffic,
+// was what bounded it: profiles/r2k).
+constexpr uint64_t NSM_L2_EVICT_NORMAL = 0x1000000000000000ull, NSM_L2_EVICT_FIRST = 0x12F0000000000000ull;
+template <uint64_t POL>
+__device__ __forceinline__ float4 ld_pol_f4(const float *p) {
+  float4 v;
+  asm volatile("ld.global.L2::cache_hint.v4.f32 {%0, %1, %2, %3}, [%4], %5;"
+               : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "l"(p), "l"(POL) : "memory");
+  return v;
+}
+template <uint64_t POL>
+__device__ __forceinline__ float2 ld_pol_f2(const float *p) {
+  float2 v;
+  asm volatile("ld.global.L2::cache_hint.v2.f32 {%0, %1}, [%2], %3;" : "=f"(v.x), "=f"(v.y) : "l"(p), "l"(POL) : "memory");
+  return v;
+}
+
+// S4's gather for one (sample, level): the eight corner entries of the level slice `tab` (= theta + offset_l F, 16-byte
+// aligned: EntryMap).  F = 2: the x-neighbour corners (k, k + 1) are one aligned 16-byte pair of entries whenever their
+// slots differ in bit 0 only -- on a dense level for every even slot, on a hashed level for every even cell x (the hash
+// XORs x in unmultiplied) -- and then come in with one load.  All index arithmetic is 32-bit.
+template <int F, uint64_t POL>
+__device__ __forceinline__ void gather_corners(const float *__restrict__ tab, const uint32_t slot[8], float v[8][F]) {
+  if constexpr (F == 2) {
+#pragma unroll
+    for (int k = 0; k < 8; k += 2) {
+      const uint32_t s0 = slot[k], s1 = slot[k + 1];
+      if ((s0 ^ s1) == 1u) {
+        const float4 q = ld_pol_f4<POL>(tab + 2 * (size_t)(s0 & ~1u));
+        const bool odd = s0 & 1u;
+        v[k][0] = odd ? q.z : q.x; v[k][1] = odd ? q.w : q.y;
+        v[k + 1][0] = odd ? q.x : q.z; v[k + 1][1] = odd ? q.y : q.w;
+      } else {
+        const float2 a = ld_pol_f2<POL>(tab + 2 * (size_t)s0), b = ld_pol_f2<POL>(tab + 2 * (size_t)s1);
+        v[k][0] = a.x; v[k][1] = a.y; v[k + 1][0] = b.x; v[k + 1][1] = b.y;
+      }
+    }
+  } else {
+#pragma unroll
+    for (int k = 0; k < 8; ++k) load_entry_hint<F>(tab + (size_t)slot[k] * F, v[k], POL);   // 8 gathers in flight
+  }
+}
+
 // S12 for one cell of one level: the eight corner reductions d theta[(offset_l + slot) F + f] += val[corner][f].
 // Addends are canonicalised here (never -0.0, never near-subnormal; NaN stays NaN): the touched set U is structural
 // (every referenced entry, independent of the gradient's value) and is carried by the gradient words themselves, see
@@ -119,13 +164,13 @@ __device__ __forceinline__ void issue_corner_reds(const LevelTable &lv, float *_
     // The two x-neighbour corners (k, k+1) are adjacent entries whenever their slots differ in bit 0 only (always on
     // a dense level, for even cell x on a hashed one: the hash XORs x in unmultiplied).  If the pair is also
     // 16-byte aligned in the array, one red.v4 covers both entries: ~25 % fewer reductions at the L2.
-    const uint64_t e_l = lv.offset[l];
+    // (the level slice starts on a 16-byte boundary, EntryMap: the pair test needs the slots only)
 #pragma unroll
     for (int k = 0; k < 8; k += 2) {
-      const uint64_t a0 = e_l + slot[k], a1 = e_l + slot[k + 1];
-      if ((a0 ^ a1) == 1ull) {
-        float *p = grad + (a0 & ~1ull) * 2;
-        if (a0 & 1ull) red_hint_f4(p, make_float4(val[k + 1][0], val[k + 1][1], val[k][0], val[k][1]), pol_last);
+      const uint32_t s0 = slot[k], s1 = slot[k + 1];
+      if ((s0 ^ s1) == 1u) {
+        float *p = tab + 2 * (size_t)(s0 & ~1u);
+        if (s0 & 1u) red_hint_f4(p, make_float4(val[k + 1][0], val[k + 1][1], val[k][0], val[k][1]), pol_last);
         else red_hint_f4(p, make_float4(val[k][0], val[k][1], val[k + 1][0], val[k + 1][1]), pol_last);
       } else {
         red_add_entry<2>(tab + (size_t)slot[k] * 2, val[k], pol_last);
