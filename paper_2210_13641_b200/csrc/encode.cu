@@ -16,6 +16,10 @@ namespace {
 
 using namespace tableops;
 
+#ifndef NSM_PANEL_HASHED_POL
+#define NSM_PANEL_HASHED_POL NSM_L2_EVICT_LAST
+#endif
+
 // MODE 0: e -> fp32 planes [l*F+f][cap].  MODE 1 / 2: e -> fp16 / bf16 operand-tile blob of the
 // tensor-core MLP kernels ([tile][8-column panel][128 rows][8 x 16 bit], mlp_tc.cu); the rows of
 // the last tile beyond S are zero-filled so the MMA never reads stale data.
@@ -195,7 +199,7 @@ __global__ void __launch_bounds__(256) encode_forward_panel_kernel(LevelTable lv
       if (gathers) {
         const float *tab = theta + lv.offset[l] * F;
         if (dense) gather_corners<F, NSM_L2_EVICT_NORMAL>(tab, ci.slot, v);
-        else gather_corners<F, NSM_L2_EVICT_FIRST>(tab, ci.slot, v);
+        else gather_corners<F, NSM_PANEL_HASHED_POL>(tab, ci.slot, v);
       }
       if (dense) {
 #pragma unroll
@@ -229,8 +233,8 @@ __global__ void __launch_bounds__(256) encode_forward_panel_kernel(LevelTable lv
       }
     }
     uint8_t *dst = ws.blob_e + (s >> 7) * (2 * half) + (size_t)g * (NSM_TILE * 16) + (s & 127) * 16;
-    *reinterpret_cast<uint4 *>(dst) = make_uint4(hw[0], hw[1], hw[2], hw[3]);
-    *reinterpret_cast<uint4 *>(dst + half) = make_uint4(lw[0], lw[1], lw[2], lw[3]);
+    st_pol_u4<NSM_L2_EVICT_FIRST>(dst, make_uint4(hw[0], hw[1], hw[2], hw[3]));
+    st_pol_u4<NSM_L2_EVICT_FIRST>(dst + half, make_uint4(lw[0], lw[1], lw[2], lw[3]));
   }
   tl_mark(ws.timeline, K_ENCODE, 1);
 }

@@ -107,7 +107,12 @@ __device__ __forceinline__ void red_add_entry(float *p, const float g[F], uint64
 // published in CUTLASS as CacheHintSm90).  A policy that is an immediate lives in a uniform register: with a policy held in
 // a per-thread variable every hinted load paid two R2UR moves (the encoder's instruction stream, not its memory traffic,
 // was what bounded it: profiles/r2k).
-constexpr uint64_t NSM_L2_EVICT_NORMAL = 0x1000000000000000ull, NSM_L2_EVICT_FIRST = 0x12F0000000000000ull;
+constexpr uint64_t NSM_L2_EVICT_NORMAL = 0x1000000000000000ull, NSM_L2_EVICT_FIRST = 0x12F0000000000000ull,
+                   NSM_L2_EVICT_LAST = 0x14F0000000000000ull;
+template <uint64_t POL>
+__device__ __forceinline__ void st_pol_u4(void *p, uint4 v) {
+  asm volatile("st.global.L2::cache_hint.v4.b32 [%0], {%1, %2, %3, %4}, %5;" ::"l"(p), "r"(v.x), "r"(v.y), "r"(v.z), "r"(v.w), "l"(POL) : "memory");
+}
 template <uint64_t POL>
 __device__ __forceinline__ float4 ld_pol_f4(const float *p) {
   float4 v;
