@@ -23,7 +23,9 @@ using namespace tableops;
 // MODE 0: e -> fp32 planes [l*F+f][cap].  MODE 1 / 2: e -> fp16 / bf16 operand-tile blob of the
 // tensor-core MLP kernels ([tile][8-column panel][128 rows][8 x 16 bit], mlp_tc.cu); the rows of
 // the last tile beyond S are zero-filled so the MMA never reads stale data.
-template <int F, int MODE>
+// TWO_TERM = false (forward-only uses: render, occupancy refresh -- their MLP kernel reads the hi tile only): the lo term is
+// neither computed nor stored.
+template <int F, int MODE, bool TWO_TERM = true>
 __global__ void __launch_bounds__(256) encode_forward_kernel(LevelTable lv, const float *__restrict__ theta,
                                                              Workspace ws, const uint32_t *__restrict__ d_S, uint32_t seq) {
   __shared__ uint32_t chunk_s;
@@ -106,16 +108,16 @@ __global__ void __launch_bounds__(256) encode_forward_kernel(LevelTable lv, cons
         if (MODE == 1) {
           const __half hi = __float2half_rn(acc[f]);
           hi16[f] = __half_as_ushort(hi);
-          lo16[f] = __half_as_ushort(__float2half_rn(acc[f] - __half2float(hi)));
+          lo16[f] = TWO_TERM ? __half_as_ushort(__float2half_rn(acc[f] - __half2float(hi))) : (uint16_t)0;
         } else {
           const __nv_bfloat16 hi = __float2bfloat16_rn(acc[f]);
           hi16[f] = __bfloat16_as_ushort(hi);
-          lo16[f] = __bfloat16_as_ushort(__float2bfloat16_rn(acc[f] - __bfloat162float(hi)));
+          lo16[f] = TWO_TERM ? __bfloat16_as_ushort(__float2bfloat16_rn(acc[f] - __bfloat162float(hi))) : (uint16_t)0;
         }
       }
       if constexpr (F == 1) {
         *reinterpret_cast<uint16_t *>(dst) = hi16[0];
-        *reinterpret_cast<uint16_t *>(dst + half) = lo16[0];
+        if (TWO_TERM) *reinterpret_cast<uint16_t *>(dst + half) = lo16[0];
       } else {
         uint32_t hw[F / 2], lw[F / 2];
 #pragma unroll
@@ -125,13 +127,13 @@ __global__ void __launch_bounds__(256) encode_forward_kernel(LevelTable lv, cons
         }
         if constexpr (F == 2) {
           *reinterpret_cast<uint32_t *>(dst) = hw[0];
-          *reinterpret_cast<uint32_t *>(dst + half) = lw[0];
+          if (TWO_TERM) *reinterpret_cast<uint32_t *>(dst + half) = lw[0];
         } else if constexpr (F == 4) {
           *reinterpret_cast<uint2 *>(dst) = make_uint2(hw[0], hw[1]);
-          *reinterpret_cast<uint2 *>(dst + half) = make_uint2(lw[0], lw[1]);
+          if (TWO_TERM) *reinterpret_cast<uint2 *>(dst + half) = make_uint2(lw[0], lw[1]);
         } else {
           *reinterpret_cast<uint4 *>(dst) = make_uint4(hw[0], hw[1], hw[2], hw[3]);
-          *reinterpret_cast<uint4 *>(dst + half) = make_uint4(lw[0], lw[1], lw[2], lw[3]);
+          if (TWO_TERM) *reinterpret_cast<uint4 *>(dst + half) = make_uint4(lw[0], lw[1], lw[2], lw[3]);
         }
       }
     }
@@ -145,7 +147,7 @@ __global__ void __launch_bounds__(256) encode_forward_kernel(LevelTable lv, cons
 // what the L2 spent its time on: one store per term and level took config 3's encoder from 200.8 to 175.1 us, this
 // mapping to 155.4 us), and the sample position is loaded once per panel.  Items are panel-major, 256 per chunk, in
 // order.  launch_encode picks between the two mappings.
-template <int F, int MODE>
+template <int F, int MODE, bool TWO_TERM = true>
 __global__ void __launch_bounds__(256) encode_forward_panel_kernel(LevelTable lv, const float *__restrict__ theta, Workspace ws,
                                                                    const uint32_t *__restrict__ d_S, uint32_t seq) {
   static_assert(MODE == 1 || MODE == 2, "operand-tile output only");
@@ -221,11 +223,11 @@ __global__ void __launch_bounds__(256) encode_forward_panel_kernel(LevelTable lv
         if (MODE == 1) {
           const __half hi = __float2half_rn(acc[f]);
           h16 = __half_as_ushort(hi);
-          l16 = __half_as_ushort(__float2half_rn(acc[f] - __half2float(hi)));
+          l16 = TWO_TERM ? __half_as_ushort(__float2half_rn(acc[f] - __half2float(hi))) : 0u;
         } else {
           const __nv_bfloat16 hi = __float2bfloat16_rn(acc[f]);
           h16 = __bfloat16_as_ushort(hi);
-          l16 = __bfloat16_as_ushort(__float2bfloat16_rn(acc[f] - __bfloat162float(hi)));
+          l16 = TWO_TERM ? __bfloat16_as_ushort(__float2bfloat16_rn(acc[f] - __bfloat162float(hi))) : 0u;
         }
         const int col = j * F + f;                 // column inside the panel, compile-time
         hw[col >> 1] |= h16 << ((col & 1) * 16);
@@ -234,7 +236,7 @@ __global__ void __launch_bounds__(256) encode_forward_panel_kernel(LevelTable lv
     }
     uint8_t *dst = ws.blob_e + (s >> 7) * (2 * half) + (size_t)g * (NSM_TILE * 16) + (s & 127) * 16;
     st_pol_u4<NSM_L2_EVICT_FIRST>(dst, make_uint4(hw[0], hw[1], hw[2], hw[3]));
-    st_pol_u4<NSM_L2_EVICT_FIRST>(dst + half, make_uint4(lw[0], lw[1], lw[2], lw[3]));
+    if (TWO_TERM) st_pol_u4<NSM_L2_EVICT_FIRST>(dst + half, make_uint4(lw[0], lw[1], lw[2], lw[3]));
   }
   tl_mark(ws.timeline, K_ENCODE, 1);
 }
@@ -430,21 +432,28 @@ int launch_unpack_records(const FieldParams &fp, int which, float *dst, cudaStre
   return 1;
 }
 
-template <int F>
-static void launch_encode_f(const LevelTable &lv, const float *theta, const Workspace &ws, const uint32_t *d_S, int out_mode,
-                            dim3 grid, dim3 block, cudaStream_t st, uint32_t seq, bool per_panel) {
-  if (out_mode == 0) launch_pdl(encode_forward_kernel<F, 0>, grid, block, 0, st, lv, theta, ws, d_S, seq);
-  else if (out_mode == 1) {
-    if (per_panel) launch_pdl(encode_forward_panel_kernel<F, 1>, grid, block, 0, st, lv, theta, ws, d_S, seq);
-    else launch_pdl(encode_forward_kernel<F, 1>, grid, block, 0, st, lv, theta, ws, d_S, seq);
+template <int F, bool TT>
+static void launch_encode_ft(const LevelTable &lv, const float *theta, const Workspace &ws, const uint32_t *d_S, int out_mode,
+                             dim3 grid, dim3 block, cudaStream_t st, uint32_t seq, bool per_panel) {
+  if (out_mode == 1) {
+    if (per_panel) launch_pdl(encode_forward_panel_kernel<F, 1, TT>, grid, block, 0, st, lv, theta, ws, d_S, seq);
+    else launch_pdl(encode_forward_kernel<F, 1, TT>, grid, block, 0, st, lv, theta, ws, d_S, seq);
   } else {
-    if (per_panel) launch_pdl(encode_forward_panel_kernel<F, 2>, grid, block, 0, st, lv, theta, ws, d_S, seq);
-    else launch_pdl(encode_forward_kernel<F, 2>, grid, block, 0, st, lv, theta, ws, d_S, seq);
+    if (per_panel) launch_pdl(encode_forward_panel_kernel<F, 2, TT>, grid, block, 0, st, lv, theta, ws, d_S, seq);
+    else launch_pdl(encode_forward_kernel<F, 2, TT>, grid, block, 0, st, lv, theta, ws, d_S, seq);
   }
 }
 
+template <int F>
+static void launch_encode_f(const LevelTable &lv, const float *theta, const Workspace &ws, const uint32_t *d_S, int out_mode,
+                            dim3 grid, dim3 block, cudaStream_t st, uint32_t seq, bool per_panel, bool two_term) {
+  if (out_mode == 0) launch_pdl(encode_forward_kernel<F, 0>, grid, block, 0, st, lv, theta, ws, d_S, seq);
+  else if (two_term) launch_encode_ft<F, true>(lv, theta, ws, d_S, out_mode, grid, block, st, seq, per_panel);
+  else launch_encode_ft<F, false>(lv, theta, ws, d_S, out_mode, grid, block, st, seq, per_panel);
+}
+
 int launch_encode(const LevelTable &lv, const float *theta, const Workspace &ws, const uint32_t *d_S, int out_mode,
-                  int n_sms, cudaStream_t st, uint32_t seq, uint64_t max_samples) {
+                  int n_sms, cudaStream_t st, uint32_t seq, uint64_t max_samples, bool two_term) {
   dim3 grid(n_sms * 8), block(256);
   // Which mapping (measured on B200, profiles/r2g): a thread per (panel, sample) writes whole 16-byte rows of the operand
   // tile and wins when the tables fit the L2 and there is enough work to fill the chip with a quarter of the threads
@@ -455,10 +464,10 @@ int launch_encode(const LevelTable &lv, const float *theta, const Workspace &ws,
   const bool l2_resident = lv.offset[lv.n_levels] * lv.n_features * sizeof(float) <= (96ull << 20);
   const bool per_panel = out_mode != 0 && l2_resident && max_samples >= (1ull << 20);
   switch (lv.n_features) {
-    case 1: launch_encode_f<1>(lv, theta, ws, d_S, out_mode, grid, block, st, seq, per_panel); break;
-    case 2: launch_encode_f<2>(lv, theta, ws, d_S, out_mode, grid, block, st, seq, per_panel); break;
-    case 4: launch_encode_f<4>(lv, theta, ws, d_S, out_mode, grid, block, st, seq, per_panel); break;
-    default: launch_encode_f<8>(lv, theta, ws, d_S, out_mode, grid, block, st, seq, per_panel); break;
+    case 1: launch_encode_f<1>(lv, theta, ws, d_S, out_mode, grid, block, st, seq, per_panel, two_term); break;
+    case 2: launch_encode_f<2>(lv, theta, ws, d_S, out_mode, grid, block, st, seq, per_panel, two_term); break;
+    case 4: launch_encode_f<4>(lv, theta, ws, d_S, out_mode, grid, block, st, seq, per_panel, two_term); break;
+    default: launch_encode_f<8>(lv, theta, ws, d_S, out_mode, grid, block, st, seq, per_panel, two_term); break;
   }
   return 1;
 }

@@ -911,7 +911,7 @@ __global__ void blob_to_rows_kernel(const uint8_t *__restrict__ blob, uint32_t n
     const size_t half = (size_t)n_cols * ROWS * 2;
     const uint8_t *p = blob + (s >> 7) * (two_term ? 2 * half : half) + tile_off(ROWS, (uint32_t)(s & 127), c);
     float v = (float)(*reinterpret_cast<const T *>(p));
-    if (two_term) v += (float)(*reinterpret_cast<const T *>(p + half));
+    if (two_term == 1) v += (float)(*reinterpret_cast<const T *>(p + half));   // 2: hi | lo layout whose lo tile was not written
     rows[i] = v;
   }
 }

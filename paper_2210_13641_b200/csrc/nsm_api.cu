@@ -133,6 +133,7 @@ struct nsm_field {
   uint32_t wgrad_parts = 0;   // > 0: the MLP weight gradient of the last backward is still in that many per-CTA slices
   bool batch_ready = false;   // NSM_OPT_BATCH_READY
   bool render_interleave = true;   // NSM_OPT_RENDER_INTERLEAVE
+  bool e_two_term = true;     // the last encoder launch wrote hi + lo operand tiles (training) or hi alone (forward-only uses)
   bool side_ok = false;       // nothing but a train step's Adam has been enqueued on `stream` since ev_pre_adam
   const char *mlp_path = "simt_fp32";
   bool use_tc = false;   // tcgen05 MLP kernels (16-bit configurations with supported shapes)
@@ -328,7 +329,8 @@ nsm_status enqueue_forward(nsm_field *f, const nsm_ray_batch *b, uint32_t R, boo
   }
   const int bf16 = f->cfg.mlp_precision == NSM_MLP_BF16;
   RUN(f, K_ENCODE, launch_encode(f->lv, f->fp.theta, f->ws, d_S, f->use_tc ? 1 + bf16 : 0, f->n_sms, f->stream, f->work_seq++,
-                                 (uint64_t)R * b->n_candidates));
+                                 (uint64_t)R * b->n_candidates, train));
+  f->e_two_term = train;
   if (f->use_tc)
     RUN(f, K_MLP_FWD, launch_mlp_forward_tc(f->ms, bf16, mlp_dirs, f->ws, d_S, 0, train ? 1 : 0, f->n_sms, f->stream));
   else
@@ -750,7 +752,8 @@ nsm_status nsm_update_occupancy(nsm_field *f, nsm_occ_mode mode, const uint8_t *
         const uint64_t n = (G3 - first < chunk) ? G3 - first : chunk;
         RUN(f, K_OCC, launch_occ_cells(f->cfg.occ_res, occ_cascades(f), first, 1, n, f->ws, d_S, f->stream));
         RUN(f, K_ENCODE, launch_encode(f->lv, f->fp.theta, f->ws, d_S, f->use_tc ? 1 + (f->cfg.mlp_precision == NSM_MLP_BF16) : 0,
-                                       f->n_sms, f->stream, f->work_seq++, n));
+                                       f->n_sms, f->stream, f->work_seq++, n, false));
+        f->e_two_term = false;
         if (f->use_tc)
           RUN(f, K_MLP_FWD, launch_mlp_forward_tc(f->ms, f->cfg.mlp_precision == NSM_MLP_BF16, nullptr, f->ws, d_S, 1, 0, f->n_sms,
                                                   f->stream));
@@ -788,7 +791,8 @@ nsm_status nsm_update_occupancy_decay(nsm_field *f, uint32_t n_subsets, float de
     const uint64_t n = (n_vis - j0 < chunk) ? n_vis - j0 : chunk;
     const uint64_t first = c0 + j0 * n_subsets;
     RUN(f, K_OCC, launch_occ_cells(f->cfg.occ_res, occ_cascades(f), first, n_subsets, n, f->ws, d_S, f->stream));
-    RUN(f, K_ENCODE, launch_encode(f->lv, f->fp.theta, f->ws, d_S, f->use_tc ? 1 + bf16 : 0, f->n_sms, f->stream, f->work_seq++, n));
+    RUN(f, K_ENCODE, launch_encode(f->lv, f->fp.theta, f->ws, d_S, f->use_tc ? 1 + bf16 : 0, f->n_sms, f->stream, f->work_seq++, n, false));
+    f->e_two_term = false;
     if (f->use_tc)
       RUN(f, K_MLP_FWD, launch_mlp_forward_tc(f->ms, bf16, nullptr, f->ws, d_S, 1, 0, f->n_sms, f->stream));
     else
@@ -817,7 +821,8 @@ nsm_status nsm_update_occupancy_stochastic(nsm_field *f, uint32_t n_draws, float
   for (uint32_t i0 = 0; i0 < n_draws; i0 += chunk) {
     const uint32_t n = n_draws - i0 < chunk ? n_draws - i0 : chunk;
     RUN(f, K_OCC, launch_occ_cells_stochastic(f->cfg.occ_res, occ_cascades(f), f->cfg.seed, f->occ_draws, i0, n, f->ws, d_S, f->stream));
-    RUN(f, K_ENCODE, launch_encode(f->lv, f->fp.theta, f->ws, d_S, f->use_tc ? 1 + bf16 : 0, f->n_sms, f->stream, f->work_seq++, n));
+    RUN(f, K_ENCODE, launch_encode(f->lv, f->fp.theta, f->ws, d_S, f->use_tc ? 1 + bf16 : 0, f->n_sms, f->stream, f->work_seq++, n, false));
+    f->e_two_term = false;
     if (f->use_tc)
       RUN(f, K_MLP_FWD, launch_mlp_forward_tc(f->ms, bf16, nullptr, f->ws, d_S, 1, 0, f->n_sms, f->stream));
     else
@@ -1167,7 +1172,7 @@ nsm_status nsm_debug_last_step(nsm_field *f, int item, void *d_out, uint64_t cap
     RUN(f, K_DEBUG, launch_planes_to_rows(ws.s_x, ws.cap, 3, d_S, (float *)d_out, f->stream));
   } else if (item == NSM_DBG_E) {
     if (f->use_tc)
-      RUN(f, K_DEBUG, launch_blob_to_rows(f->cfg.mlp_precision == NSM_MLP_BF16, ws.blob_e, f->ms.LF, 1, d_S, (float *)d_out, f->stream));
+      RUN(f, K_DEBUG, launch_blob_to_rows(f->cfg.mlp_precision == NSM_MLP_BF16, ws.blob_e, f->ms.LF, f->e_two_term ? 1 : 2, d_S, (float *)d_out, f->stream));
     else
       RUN(f, K_DEBUG, launch_planes_to_rows(ws.e, ws.cap, f->ms.LF, d_S, (float *)d_out, f->stream));
   } else if (item == NSM_DBG_HIDDEN_DENSITY || item == NSM_DBG_HIDDEN_COLOR1 || item == NSM_DBG_HIDDEN_COLOR2) {

@@ -304,8 +304,10 @@ uint32_t march_scan_state_entries(uint32_t max_rays);
 // out_mode: 0 = fp32 planes ws.e, 1 = fp16 blob ws.blob_e, 2 = bf16 blob ws.blob_e
 // seq: launch sequence number of the field's table kernels (selects the ChunkQueue counter)
 // max_samples: an upper bound on S known to the host (rays x candidates, cells of a refresh chunk): picks the work mapping
+// two_term: blob modes only -- write the hi AND the lo tile (training: the two-term forward) or the hi tile alone
+// (forward-only uses, whose MLP kernel reads nothing else)
 int launch_encode(const LevelTable &lv, const float *theta, const Workspace &ws,
-                  const uint32_t *d_S, int out_mode, int n_sms, cudaStream_t st, uint32_t seq, uint64_t max_samples);
+                  const uint32_t *d_S, int out_mode, int n_sms, cudaStream_t st, uint32_t seq, uint64_t max_samples, bool two_term);
 // S12 over all levels: vector reductions into grad
 int launch_scatter(const LevelTable &lv, float *grad, const Workspace &ws, const uint32_t *d_S, int n_sms, cudaStream_t st,
                    uint32_t seq);
