@@ -240,14 +240,7 @@ nsm_status nsm_get_keyframe_pose(nsm_field *f, uint32_t index, float *h_R, float
 /* NSM_OPT_POSE_LEVELS (default 0 = all).  Coarse-to-fine pose refinement (reading R26): the pose gradients
  * differentiate the sample positions through the encoding levels l < value only; the field itself is always evaluated
  * with all levels and the parameter gradients do not change.  May be changed between steps (a schedule). */
-/* NSM_OPT_RENDER_INTERLEAVE (default 1).  nsm_render / nsm_render_host keep the live samples of every 16 consecutive rays
- * of a call in (candidate k, ray) order instead of (ray, k): neighbouring pixels of a frame reach the same depth at the
- * same k, so consecutive samples then fall into the same cells of the encoding and are fetched together (hand the rays of
- * a frame over in small pixel tiles, e.g. 4 x 4, for the most of it; any order is correct).  The image is the same up to
- * the rounding of one sum per ray; only the order of the per-SAMPLE debug items after a render changes (NSM_DBG_SAMPLE_RAY /
- * NSM_DBG_SAMPLE_K still name each sample).  0 restores the (ray, k) order. */
-typedef enum { NSM_OPT_BATCH_READY = 0, NSM_OPT_POSE_GRADIENTS = 1, NSM_OPT_DEBUG_TIMELINE = 2, NSM_OPT_POSE_LEVELS = 3,
-               NSM_OPT_RENDER_INTERLEAVE = 4 } nsm_option;
+typedef enum { NSM_OPT_BATCH_READY = 0, NSM_OPT_POSE_GRADIENTS = 1, NSM_OPT_DEBUG_TIMELINE = 2, NSM_OPT_POSE_LEVELS = 3 } nsm_option;
 nsm_status nsm_set_option(nsm_field *f, nsm_option opt, uint32_t value);
 
 /* S1-S12 only: forward + backward, gradients left in place for nsm_debug_last_step; and S13

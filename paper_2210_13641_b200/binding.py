@@ -16,7 +16,7 @@ LIB_PATH = os.path.join(_HERE, "libnsm.so")
 NSM_OK, NSM_ERR_INVALID_ARG, NSM_ERR_OOM, NSM_ERR_CUDA, NSM_ERR_CAPACITY, NSM_ERR_UNIMPLEMENTED = range(6)
 NSM_MLP_FP32, NSM_MLP_FP16, NSM_MLP_BF16 = 0, 1, 2
 NSM_OCC_FULL, NSM_OCC_SET, NSM_OCC_FROM_FIELD = 0, 1, 2
-NSM_OPT_BATCH_READY, NSM_OPT_POSE_GRADIENTS, NSM_OPT_DEBUG_TIMELINE, NSM_OPT_POSE_LEVELS, NSM_OPT_RENDER_INTERLEAVE = 0, 1, 2, 3, 4
+NSM_OPT_BATCH_READY, NSM_OPT_POSE_GRADIENTS, NSM_OPT_DEBUG_TIMELINE, NSM_OPT_POSE_LEVELS = 0, 1, 2, 3
 NSM_MARCH_STATIC_MAX_RAYS = 1 << 20
 
 DEBUG_ITEMS = dict(counts=(0, np.uint32), offsets=(1, np.uint32), s_ray=(2, np.uint32), s_k=(3, np.uint32),

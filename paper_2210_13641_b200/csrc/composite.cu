@@ -154,39 +154,6 @@ __global__ void __launch_bounds__(256) composite_kernel(Workspace ws, uint32_t R
   tl_mark(ws.timeline, K_COMPOSITE, 1);
 }
 
-// S15 for the interleaved sample order of the rendering marcher (march.cu): a THREAD per ray walks its samples through
-// ws.s_idx.  The lanes of a warp are neighbouring rays, whose i-th samples sit next to each other in the (k, ray)-ordered
-// list, so their loads share sectors; a ray that has fallen below the cut simply stops.  Same arithmetic as
-// composite_kernel<false>, the sum of sigma_j delta_j taken sequentially instead of by a warp scan.
-__global__ void __launch_bounds__(128) composite_render_interleaved_kernel(Workspace ws, uint32_t R, float bg0, float bg1, float bg2,
-                                                                          float cut, float *__restrict__ out_rgb,
-                                                                          float *__restrict__ out_depth,
-                                                                          float *__restrict__ out_opacity) {
-  pdl_wait();
-  pdl_trigger();
-  tl_mark(ws.timeline, K_COMPOSITE, 0);
-  const uint32_t r = blockIdx.x * blockDim.x + threadIdx.x;
-  if (r < R) {
-    const uint32_t off = ws.offsets[r], n = ws.offsets[r + 1] - off;
-    float A = 0.f, C0 = 0.f, C1 = 0.f, C2 = 0.f, D = 0.f, O = 0.f;
-    for (uint32_t i = 0; i < n; ++i) {
-      const uint64_t s = ws.s_idx[off + i];
-      const float a = ws.sigma[s] * ws.s_delta[s];
-      const float w = expf(-A) * (-expm1f(-a));   // T_i (1 - exp(-sigma_i delta_i)), Eqs. 5, 6
-      C0 += w * ws.rgb[3 * s]; C1 += w * ws.rgb[3 * s + 1]; C2 += w * ws.rgb[3 * s + 2];
-      D += w * ws.s_t[s];
-      O += w;
-      A += a;
-      if (cut > 0.f && expf(-A) < cut) break;     // the ray stops after the first sample whose T_{i+1} < cut
-    }
-    const float T_end = expf(-A);
-    out_rgb[3 * (size_t)r] = C0 + T_end * bg0; out_rgb[3 * (size_t)r + 1] = C1 + T_end * bg1; out_rgb[3 * (size_t)r + 2] = C2 + T_end * bg2;
-    out_depth[r] = D;
-    if (out_opacity) out_opacity[r] = O;
-  }
-  tl_mark(ws.timeline, K_COMPOSITE, 1);
-}
-
 }  // namespace
 
 int launch_composite_train(const Workspace &ws, uint32_t R, const float *rgb, const float *depth,
@@ -198,12 +165,7 @@ int launch_composite_train(const Workspace &ws, uint32_t R, const float *rgb, co
 }
 
 int launch_composite_render(const Workspace &ws, uint32_t R, float cut, const float bg[3], float *out_rgb,
-                            float *out_depth, float *out_opacity, cudaStream_t st, bool interleaved) {
-  if (interleaved) {
-    launch_pdl(composite_render_interleaved_kernel, dim3((R + 127) / 128), dim3(128), 0, st, ws, R, bg[0], bg[1], bg[2], cut, out_rgb,
-               out_depth, out_opacity);
-    return 1;
-  }
+                            float *out_depth, float *out_opacity, cudaStream_t st) {
   dim3 grid((R + 7) / 8), block(256);
   launch_pdl(composite_kernel<false>, grid, block, 0, st, ws, R, (const float *)nullptr, (const float *)nullptr,
              (const float *)nullptr, 0.f, bg[0], bg[1], bg[2], cut, out_rgb, out_depth, out_opacity);

@@ -109,29 +109,15 @@ __device__ __forceinline__ Candidate make_candidate(const MarchParams &mp, const
 // Pass 2: each live candidate is written at offsets[r] + its rank among the ray's live ones, so the
 // compacted list is in (ray, k) order and bit-identical from run to run.  The last block to finish
 // resets the scan state for the next launch.
-//
-// INTERLEAVE (forward-only rendering, S15): the samples of a block's MARCH_WARPS consecutive rays are written in
-// (k, ray) order instead -- candidate k of all the block's rays, then candidate k + 1 -- inside the same range of the
-// compacted list (the block's rays still own offsets[r0] .. offsets[r0 + MARCH_WARPS)).  Neighbouring pixels of a
-// frame reach the same depth at the same k, so 32 consecutive samples then lie within a few centimetres of each other
-// and the encoder's gathers of a warp fall into the same cells on all but the finest levels (profiles/r2k).  Which
-// samples exist, and every value stored for them, is unchanged; ws.s_idx[offsets[r] + i] gives the position of ray r's
-// i-th live sample for the compositor.
 constexpr uint32_t MARCH_WARPS = 16;
 constexpr uint32_t MARCH_MAX_WORDS = 128;        // K <= 4096 (validate_config)
 constexpr uint64_t SCAN_AGG = 1ull << 32, SCAN_INCL = 2ull << 32;
 
-template <bool INTERLEAVE>
 __global__ void __launch_bounds__(MARCH_WARPS * 32) march_fused_kernel(MarchParams mp, const uint8_t *bits,
                                                                        const float *__restrict__ origins,
                                                                        const float *__restrict__ dirs, Workspace ws,
                                                                        int count_total, float *__restrict__ dirs_copy) {
   __shared__ uint32_t masks[MARCH_WARPS][MARCH_MAX_WORDS];
-  // INTERLEAVE: per candidate k, the block's rays that are live there (bit w = ray w) and the number of live
-  // (k', ray) pairs before row k inside k's 32-candidate word; per word, the number before the word
-  __shared__ uint16_t col_bits[INTERLEAVE ? MARCH_MAX_WORDS * 32 : 1], col_pre[INTERLEAVE ? MARCH_MAX_WORDS * 32 : 1];
-  __shared__ uint32_t word_pre[INTERLEAVE ? MARCH_MAX_WORDS : 1];
-  static_assert(MARCH_WARPS <= 16, "col_bits holds one bit per ray of the block");
   __shared__ uint32_t warp_n[MARCH_WARPS];
   __shared__ uint32_t look_first[MARCH_WARPS], look_sum[MARCH_WARPS];
   __shared__ uint32_t ticket_s, block_base_s, total_s;
@@ -170,42 +156,8 @@ __global__ void __launch_bounds__(MARCH_WARPS * 32) march_fused_kernel(MarchPara
       }
     }
   }
-  if (INTERLEAVE && r >= mp.R)
-    for (uint32_t wd = lane; wd < words; wd += 32) masks[wid][wd] = 0u;
   if (lane == 0) warp_n[wid] = n;
   __syncthreads();
-  if (INTERLEAVE) {
-    for (uint32_t wd = wid; wd < words; wd += MARCH_WARPS) {   // transpose the live masks of word wd: lane = candidate
-      uint32_t cb = 0;
-#pragma unroll
-      for (uint32_t w = 0; w < MARCH_WARPS; ++w) cb |= ((masks[w][wd] >> lane) & 1u) << w;
-      const uint32_t c = __popc(cb);
-      uint32_t incl = c;
-#pragma unroll
-      for (int s = 1; s < 32; s <<= 1) {
-        const uint32_t y = __shfl_up_sync(0xffffffffu, incl, s);
-        if (lane >= (uint32_t)s) incl += y;
-      }
-      col_bits[wd * 32 + lane] = (uint16_t)cb;
-      col_pre[wd * 32 + lane] = (uint16_t)(incl - c);          // < 16 * 32
-      if (lane == 31) word_pre[wd] = incl;                     // the word's total, scanned below
-    }
-    __syncthreads();
-    if (wid == 1) {   // exclusive scan of the word totals (warp 0 publishes the block's aggregate meanwhile)
-      uint32_t carry = 0;
-      for (uint32_t w0 = 0; w0 < words; w0 += 32) {
-        const uint32_t v = w0 + lane < words ? word_pre[w0 + lane] : 0u;
-        uint32_t incl = v;
-#pragma unroll
-        for (int s = 1; s < 32; s <<= 1) {
-          const uint32_t y = __shfl_up_sync(0xffffffffu, incl, s);
-          if (lane >= (uint32_t)s) incl += y;
-        }
-        if (w0 + lane < words) word_pre[w0 + lane] = carry + incl - v;
-        carry += __shfl_sync(0xffffffffu, incl, 31);
-      }
-    }
-  }
   uint32_t total = 0;
   if (wid == 0) {
     // block-local exclusive scan of the MARCH_WARPS counts, then publish the block's aggregate
@@ -271,12 +223,7 @@ __global__ void __launch_bounds__(MARCH_WARPS * 32) march_fused_kernel(MarchPara
       if ((m >> lane) & 1u) {
         const uint32_t k = wd * 32 + lane;
         const Candidate c = make_candidate(mp, nullptr, hpre, o, d, k);
-        uint64_t s = (uint64_t)base + __popc(m & ((1u << lane) - 1u));
-        if (INTERLEAVE) {   // (k, ray) order inside the block's range; the ray-major slot keeps the position
-          const uint64_t si = (uint64_t)block_base_s + word_pre[wd] + col_pre[k] + __popc(col_bits[k] & ((1u << wid) - 1u));
-          ws.s_idx[s] = (uint32_t)si;
-          s = si;
-        }
+        const uint64_t s = (uint64_t)base + __popc(m & ((1u << lane) - 1u));
         ws.s_ray[s] = r;
         ws.s_k[s] = k;
         ws.s_t[s] = c.t;
@@ -387,12 +334,9 @@ __global__ void occ_bits_from_grid_kernel(const float *__restrict__ grid, uint64
 int launch_march(const MarchParams &mp, const uint8_t *bits, const float *origins, const float *dirs,
                  const Workspace &ws, int count_total, cudaStream_t st, float *dirs_copy) {
   dim3 grid((mp.R + MARCH_WARPS - 1) / MARCH_WARPS), block(MARCH_WARPS * 32);
-  if (mp.interleave) launch_pdl(march_fused_kernel<true>, grid, block, 0, st, mp, bits, origins, dirs, ws, count_total, dirs_copy);
-  else launch_pdl(march_fused_kernel<false>, grid, block, 0, st, mp, bits, origins, dirs, ws, count_total, dirs_copy);
+  launch_pdl(march_fused_kernel, grid, block, 0, st, mp, bits, origins, dirs, ws, count_total, dirs_copy);
   return 1;
 }
-
-uint32_t march_interleave_group() { return MARCH_WARPS; }
 
 uint32_t march_scan_state_entries(uint32_t max_rays) { return (max_rays + MARCH_WARPS - 1) / MARCH_WARPS; }
 
@@ -564,7 +508,7 @@ extern "C" nsm_status nsm_march_static(const nsm_march_config *cfg, const nsm_ra
   const uint32_t n_blocks = (R + MARCH_WARPS - 1) / MARCH_WARPS;
   cudaError_t e = cudaMemsetAsync(scratch, 0, STATIC_HEADER + sizeof(unsigned long long) * n_blocks, stream);
   if (e == cudaSuccess) {
-    march_fused_kernel<false><<<n_blocks, MARCH_WARPS * 32, 0, stream>>>(mp, d_occ_bits, rays->origins, rays->dirs, ws, 0, nullptr);
+    march_fused_kernel<<<n_blocks, MARCH_WARPS * 32, 0, stream>>>(mp, d_occ_bits, rays->origins, rays->dirs, ws, 0, nullptr);
     e = cudaGetLastError();
   }
   if (e != cudaSuccess) {

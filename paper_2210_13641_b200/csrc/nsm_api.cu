@@ -132,7 +132,6 @@ struct nsm_field {
   bool scatter_pending = false;   // the backward pass stopped before S12: enqueue_adam issues the scatter right before the table Adam
   uint32_t wgrad_parts = 0;   // > 0: the MLP weight gradient of the last backward is still in that many per-CTA slices
   bool batch_ready = false;   // NSM_OPT_BATCH_READY
-  bool render_interleave = true;   // NSM_OPT_RENDER_INTERLEAVE
   bool e_two_term = true;     // the last encoder launch wrote hi + lo operand tiles (training) or hi alone (forward-only uses)
   bool side_ok = false;       // nothing but a train step's Adam has been enqueued on `stream` since ev_pre_adam
   const char *mlp_path = "simt_fp32";
@@ -300,12 +299,10 @@ MarchParams make_march(const nsm_field *f, const nsm_ray_batch *b, uint32_t R, b
 // sample_draw >= 0: the batch is first drawn from the keyframe store (F1) into b's buffers (the field's staging area),
 // on the stream the marcher runs on.
 nsm_status enqueue_forward(nsm_field *f, const nsm_ray_batch *b, uint32_t R, bool jitter, uint32_t step, bool train,
-                           bool march_on_side = false, float *dirs_copy = nullptr, int64_t sample_draw = -1,
-                           bool interleave = false) {
+                           bool march_on_side = false, float *dirs_copy = nullptr, int64_t sample_draw = -1) {
   const uint32_t *d_S = f->ws.offsets + R;
   const float *mlp_dirs = dirs_copy ? dirs_copy : b->dirs;
   MarchParams mp = make_march(f, b, R, jitter, step);
-  mp.interleave = interleave ? 1u : 0u;
   if (march_on_side && !f->prof.on) {
     if (!f->side_ok) {   // other work has been enqueued on the main stream since the last Adam: order behind all of it
       CUDA_TRY(cudaEventRecord(f->ev_main, f->stream));
@@ -572,7 +569,7 @@ nsm_status nsm_create_field(const nsm_field_config *cfg, void *cuda_stream, nsm_
   A(f->alloc(&ws.counts, R)); A(f->alloc(&ws.offsets, R + 1)); A(f->alloc(&ws.scan_state, march_scan_state_entries(R) + 1)); A(f->alloc(&ws.scan_ctr, 2)); A(f->alloc(&ws.work_ctr, 8));
   A(f->alloc(&ws.C, 3 * (size_t)R)); A(f->alloc(&ws.D_hat, R)); A(f->alloc(&ws.O, R));
   A(f->alloc(&ws.s_ray, cap)); A(f->alloc(&ws.s_k, cap)); A(f->alloc(&ws.s_t, cap)); A(f->alloc(&ws.s_delta, cap));
-  A(f->alloc(&ws.s_x, 3 * cap)); A(f->alloc(&ws.s_idx, cap));
+  A(f->alloc(&ws.s_x, 3 * cap));
   ws.e = ws.hd = ws.g = ws.h1 = ws.h2 = nullptr;
   ws.blob_e = ws.blob_hd = ws.blob_ci = ws.blob_h1 = ws.blob_h2 = ws.wimg_fwd = ws.wimg_bwd = nullptr;
   ws.wgrad_part = nullptr;
@@ -1042,7 +1039,6 @@ nsm_status nsm_set_option(nsm_field *f, nsm_option opt, uint32_t value) {
       return NSM_OK;
     }
     case NSM_OPT_POSE_LEVELS: f->pose_levels = value; return NSM_OK;
-    case NSM_OPT_RENDER_INTERLEAVE: f->render_interleave = value != 0; return NSM_OK;
     case NSM_OPT_DEBUG_TIMELINE: {
       LEAVE_FAST_PATH(f);
       if (value && !f->timeline_base) {
@@ -1090,9 +1086,9 @@ static nsm_status render_chunks(nsm_field *f, const nsm_ray_batch *b, float cut,
       cb.origins = b->origins + 3 * (size_t)first;
       cb.dirs = b->dirs + 3 * (size_t)first;
     }
-    st = enqueue_forward(f, &cb, R, false, 0, false, false, nullptr, -1, f->render_interleave);
+    st = enqueue_forward(f, &cb, R, false, 0, false);
     if (st != NSM_OK) return st;
-    RUN(f, K_COMPOSITE, launch_composite_render(f->ws, R, cut, f->cfg.bg, o_rgb, o_d, o_op, f->stream, f->render_interleave));
+    RUN(f, K_COMPOSITE, launch_composite_render(f->ws, R, cut, f->cfg.bg, o_rgb, o_d, o_op, f->stream));
     if (f->prof.on) f->prof.collect();
     if (host) {
       CUDA_TRY(cudaMemcpyAsync(rgb + 3 * (size_t)first, o_rgb, sizeof(float) * 3 * R, cudaMemcpyDeviceToHost, f->stream));

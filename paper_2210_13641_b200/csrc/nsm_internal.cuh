@@ -43,7 +43,6 @@ struct MarchParams {
   uint32_t K, G, C, jitter, step;   // C: occupancy cascades (F4)
   uint64_t seed;
   uint32_t R;
-  uint32_t interleave = 0;          // forward-only rendering: (k, ray) sample order inside each block of rays (march.cu)
 };
 
 // Per-step device workspace.  All per-sample arrays are planes of `cap` floats (cap = capacity,
@@ -60,7 +59,6 @@ struct Workspace {
   float *C, *D_hat, *O;  // [R,3], [R], [R]
   // samples
   uint32_t *s_ray, *s_k; // [cap]
-  uint32_t *s_idx;       // [cap] interleaved rendering only: position of ray r's i-th live sample at [offsets[r] + i]
   float *s_t, *s_delta;  // [cap]
   float *s_x;            // [3][cap] planes
   float *e;              // [LF][cap]
@@ -342,9 +340,8 @@ int launch_blob_to_rows(int bf16, const uint8_t *blob, uint32_t n_cols, int two_
 int launch_composite_train(const Workspace &ws, uint32_t R, const float *rgb, const float *depth,
                            const float *depth_var, float lambda_d, const float bg[3],
                            cudaStream_t st);
-// interleaved: the samples are in the rendering marcher's (k, ray) order (MarchParams::interleave), reached through ws.s_idx
 int launch_composite_render(const Workspace &ws, uint32_t R, float cut, const float bg[3],
-                            float *out_rgb, float *out_depth, float *out_opacity, cudaStream_t st, bool interleaved);
+                            float *out_rgb, float *out_depth, float *out_opacity, cudaStream_t st);
 // S13 on the touched table entries (sparse) or on all of them; consumes the gradients (every word back to "untouched")
 int launch_adam_table(const FieldParams &fp, uint32_t F, int sparse, float lr, float beta1, float beta2,
                       float eps, float inv_bc1, float inv_bc2, cudaStream_t st, unsigned long long *tl = nullptr);

@@ -290,48 +290,6 @@ def test_render_parity(nsm, precision, shape):
     f.close()
 
 
-@pytest.mark.parametrize("R,K", [(1000, 256), (1, 33), (17, 32), (16, 4096)])
-def test_render_interleaved_sample_order(nsm, R, K):
-    """NSM_OPT_RENDER_INTERLEAVE (default on): the rendering marcher keeps the live samples of each block of 16 rays in
-    (k, ray) order.  Against the (ray, k) order of the same call with the option off: the same set of samples with
-    bit-identical t, delta, x (P1 / P2 hold for both), counts and offsets unchanged, every block's samples inside the
-    block's range and sorted by (k, ray), and the same image up to the rounding of the per-ray sums.  Ragged ray counts,
-    a single ray, one and 128 mask words per ray."""
-    w = configs.config3(R=1024, K=128, n_keyframes=2, n_batches=3, width=300, height=170)
-    fc = replace(w.field, bg=(0.1, 0.2, 0.3), max_candidates=max(K, 128), max_rays=1024)
-    w = replace(w, field=fc)
-    f, O, _ = make_pair(nsm, w, seed=21, table_scale=0.05)
-    for b in w.batches:
-        f.nsm_train_step(nsm.DeviceBatch(b), w.lambda_d, want_stats=False)
-    f.nsm_update_occupancy(nsm.NSM_OCC_FROM_FIELD)
-    view = configs.config5_views(seed=4, n_views=1, width=300, height=170, K=K, stride=5)[0]
-    view = _first_rays(view, R)
-    got = {}
-    for on in (0, 1):
-        f.nsm_set_option(nsm.NSM_OPT_RENDER_INTERLEAVE, on)
-        img = [t.cpu().numpy() for t in f.nsm_render(nsm.DeviceBatch(view), 1e-4)]
-        got[on] = (img, {k: f.nsm_debug_last_step(k) for k in ("counts", "offsets", "s_ray", "s_k", "s_t", "s_delta", "s_x", "sigma")})
-    (img0, d0), (img1, d1) = got[0], got[1]
-    assert np.array_equal(d0["counts"], d1["counts"]) and np.array_equal(d0["offsets"], d1["offsets"])
-    S = int(d0["offsets"][R])
-    assert S > 0 and len(d1["s_ray"]) == S
-    ray, k = d1["s_ray"].astype(np.int64), d1["s_k"].astype(np.int64)
-    order = np.lexsort((k, ray))                              # back to (ray, k)
-    for name in ("s_ray", "s_k", "s_t", "s_delta", "s_x"):
-        assert np.array_equal(d1[name][order].view(np.uint32), d0[name].view(np.uint32)), name
-    assert np.allclose(d1["sigma"][order], d0["sigma"], rtol=1e-6, atol=0)    # the field does not care where a sample sits
-    pos = np.arange(S)
-    blk = ray // 16
-    lo = d0["offsets"][np.minimum(blk * 16, R)].astype(np.int64)
-    hi = d0["offsets"][np.minimum(blk * 16 + 16, R)].astype(np.int64)
-    assert np.all((pos >= lo) & (pos < hi))                   # a block's samples stay inside the block's range
-    key = (blk * K + k) * 16 + ray % 16
-    assert np.all(np.diff(key) > 0)                           # ... in (k, ray) order, blocks in ray order
-    for a, b in zip(img0, img1):
-        assert np.abs(a - b).max() <= 2e-5 * max(np.abs(a).max(), 1e-3)
-    f.close()
-
-
 @pytest.mark.parametrize("pinned", [True, False])
 def test_host_entry_point_matches_device_entry_point(nsm, pinned):
     """pinned: the kernels read the host batch in place; pageable: staged by host-to-device copies."""

@@ -183,30 +183,15 @@ def config4(seed=4, R=1 << 12, K=512, n_keyframes=25, n_batches=1, occ_res=256, 
                     dict(room=room, keyframes=kfs, occupancy_fraction=frac))
 
 
-def pixel_tile_order(width, height, tile_w=4, tile_h=4):
-    """Raster pixel indices (y * width + x) in the order that walks the frame tile by tile (tile_w x tile_h pixels, tiles in
-    raster order, raster order inside a tile; ragged tiles at the right and bottom edges).  A caller that hands the rays of
-    a frame to nsm_render in this order gives every run of tile_w * tile_h consecutive rays a compact footprint in the
-    scene; out[order] = image undoes it.  No arithmetic of the method: an index permutation."""
-    y, x = np.divmod(np.arange(width * height, dtype=np.int64), width)
-    return np.lexsort((x % tile_w, y % tile_h, x // tile_w, y // tile_h))
-
-
-def config5_views(seed=3, n_views=4, width=1200, height=680, K=256, stride=1, tile=None):
+def config5_views(seed=3, n_views=4, width=1200, height=680, K=256, stride=1):
     """Held-out full-frame views of config 3's room for nsm_render (BASELINE.json configs[4]).
-    stride>1 gives the pixel-strided subset the oracle renders; tile=(w, h) hands the rays over in pixel tiles
-    (pixel_tile_order) instead of raster order."""
+    stride>1 gives the pixel-strided subset the oracle renders."""
     room = scenes.Room(seed)
     kfs = scenes.KeyframeSet(room, seed + 5000, n_views, width, height)
     views = []
     for i in range(n_views):
         o, d = kfs.rays(i)
-        o = o.reshape(height, width, 3)[::stride, ::stride]
-        d = d.reshape(height, width, 3)[::stride, ::stride]
-        h, w = o.shape[:2]
-        o, d = o.reshape(-1, 3), d.reshape(-1, 3)
-        if tile:
-            order = pixel_tile_order(w, h, *tile)
-            o, d = o[order], d[order]
+        o = o.reshape(height, width, 3)[::stride, ::stride].reshape(-1, 3)
+        d = d.reshape(height, width, 3)[::stride, ::stride].reshape(-1, 3)
         views.append(RayBatch(_f32(o), _f32(d), None, None, None, 0.05, 10.5, K))
     return views
