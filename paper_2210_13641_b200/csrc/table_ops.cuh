@@ -133,12 +133,15 @@ __device__ __forceinline__ float2 ld_pol_f2(const float *p) {
 // XORs x in unmultiplied) -- and then come in with one load.  All index arithmetic is 32-bit.
 template <int F, uint64_t POL>
 __device__ __forceinline__ void gather_corners(const float *__restrict__ tab, const uint32_t slot[8], float v[8][F]) {
+  // the slice pointer as one opaque 64-bit register pair: every address below is then a single IMAD.WIDE (left to itself
+  // the compiler re-adds table base, level offset and slot with carries for each of the twelve loads)
+  asm volatile("" : "+l"(tab));
   if constexpr (F == 2) {
 #pragma unroll
     for (int k = 0; k < 8; k += 2) {
       const uint32_t s0 = slot[k], s1 = slot[k + 1];
       if ((s0 ^ s1) == 1u) {
-        const float4 q = ld_pol_f4<POL>(tab + 2 * (size_t)(s0 & ~1u));
+        const float4 q = ld_pol_f4<POL>(tab + 4 * (size_t)(s0 >> 1));
         const bool odd = s0 & 1u;
         v[k][0] = odd ? q.z : q.x; v[k][1] = odd ? q.w : q.y;
         v[k + 1][0] = odd ? q.x : q.z; v[k + 1][1] = odd ? q.y : q.w;
