@@ -154,11 +154,13 @@ namespace {
 
 // S0 — integer level table: N_l = floor(N_min * exp(l ln(N_max/N_min)/(L-1)) + 1e-6) in float64,
 // ends forced; E_l = min((N_l+1)^3, T); dense iff (N_l+1)^3 <= T.
-// lv.offset: storage offsets, each level on a 16-byte boundary; map: canonical <-> storage (EntryMap, nsm_internal.cuh)
+// lv.offset: storage offsets, each level on a 64-byte boundary; map: canonical <-> storage (EntryMap, nsm_internal.cuh)
 nsm_status build_levels(const nsm_field_config &c, LevelTable &lv, EntryMap &map) {
   const uint32_t L = c.n_levels;
   const uint64_t T = 1ull << c.log2_table_size;
-  const uint64_t align = c.n_features >= 4 ? 1 : 4 / c.n_features;   // entries per 16 bytes
+  // entries per 64 bytes: the x-neighbour pair (slot, slot ^ 1) of an even cell x then shares one 16-byte (F = 2) or one
+  // 32-byte sector (F = 4) in theta, in the gradient array and in the moment records' neighbourhood
+  const uint64_t align = c.n_features >= 16 ? 1 : 16 / c.n_features;
   lv.n_levels = L;
   lv.n_features = c.n_features;
   lv.t_mask = (uint32_t)(T - 1);

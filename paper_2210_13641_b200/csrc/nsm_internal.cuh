@@ -15,16 +15,17 @@ struct LevelTable {
   uint32_t n_levels, n_features, t_mask;
   uint32_t res[NSM_MAX_LEVELS];
   uint32_t dense[NSM_MAX_LEVELS];      // 1: slot = vx + (N+1)(vy + (N+1) vz); 0: hashed
-  uint64_t offset[NSM_MAX_LEVELS + 1]; // in entries, of the STORAGE arrays (theta, m|v, grad): every level starts on a 16-byte
+  uint64_t offset[NSM_MAX_LEVELS + 1]; // in entries, of the STORAGE arrays (theta, m|v, grad): every level starts on a 64-byte
                                        // boundary (see EntryMap); the canonical offsets of include/nsm.h are EntryMap::canon
 };
 
 // Canonical entry index (include/nsm.h: levels back to back) <-> storage entry index.  A level's slice of the storage
-// arrays starts at a multiple of 16 bytes (4 / F entries for F < 4), so that the x-neighbour corners (x, x + 1) of an even
+// arrays starts at a multiple of 64 bytes of theta (16 / F entries), so that the x-neighbour corners (x, x + 1) of an even
 // cell x -- adjacent slots on a dense level and, the hash XORing x in unmultiplied, on a hashed level too -- form an
-// ALIGNED 16-byte pair for F = 2 whatever the sizes of the levels before (config 2: the five dense levels hold an odd
-// number of entries, which left every hashed level's pairs straddling a boundary).  The padding entries are never
-// referenced: theta 0, gradient "untouched" for ever.  Used by the boundary kernels only (pack / unpack / debug).
+// ALIGNED pair whatever the sizes of the levels before: one 16-byte load / reduction at F = 2, one 32-byte sector at
+// F = 4 (configs 2 and 4: the dense levels hold an odd number of entries, which left every hashed level's pairs
+// straddling a boundary).  The padding entries are never referenced: theta 0, gradient "untouched" for ever.  Used by
+// the boundary kernels only (pack / unpack / debug).
 struct EntryMap {
   uint32_t n_levels;
   uint64_t canon[NSM_MAX_LEVELS + 1], storage[NSM_MAX_LEVELS + 1];
