@@ -23,7 +23,7 @@ using namespace tableops;
 template <int F>
 __global__ void __launch_bounds__(ADAM_THREADS) adam_table_kernel(float *__restrict__ theta, float *__restrict__ mv, float *__restrict__ grad,
                                                                   uint64_t first_entry, uint64_t n_entries, int sparse, AdamConst c,
-                                                                  unsigned long long *tl) {
+                                                                  unsigned long long *tl, int theta_resident) {
   constexpr int CH = ADAM_CHUNK_FLOATS / F;
   __shared__ float list_g[ADAM_CHUNK_FLOATS];          // compacted gradients, F floats per touched entry
   __shared__ uint16_t list_e[CH];                      // compacted local entry indices
@@ -31,7 +31,7 @@ __global__ void __launch_bounds__(ADAM_THREADS) adam_table_kernel(float *__restr
   pdl_wait();
   pdl_trigger();
   tl_mark(tl, K_ADAM_TABLE, 0);
-  adam_chunk<F>(theta, mv, grad, first_entry + (uint64_t)blockIdx.x * CH, n_entries, sparse, c, list_g, list_e, &cnt);
+  adam_chunk<F>(theta, mv, grad, first_entry + (uint64_t)blockIdx.x * CH, n_entries, sparse, c, list_g, list_e, &cnt, theta_resident);
   tl_mark(tl, K_ADAM_TABLE, 1);
 }
 
@@ -49,15 +49,19 @@ __global__ void adam_dense_kernel(float *__restrict__ theta, float *__restrict__
 }  // namespace
 
 int launch_adam_table(const FieldParams &fp, uint32_t F, int sparse, float lr, float beta1, float beta2, float eps,
-                      float inv_bc1, float inv_bc2, cudaStream_t st, unsigned long long *tl) {
+                      float inv_bc1, float inv_bc2, cudaStream_t st, unsigned long long *tl, uint64_t max_samples) {
   AdamConst c{lr, beta1, beta2, eps, inv_bc1, inv_bc2};
   const uint64_t chunk = ADAM_CHUNK_FLOATS / F, first_entry = 0, end_entry = fp.n_entries;
   dim3 grid((unsigned)((end_entry - first_entry + chunk - 1) / chunk)), block(ADAM_THREADS);
+  // the panel encoder's case (launch_encode): tables that fit the L2 and a large step, whose encoder re-reads every table
+  // line many times -- the updated theta then stays in the L2 for it (config 3: encode 128.7 -> 119.7 us against +3 us
+  // here); with small steps (config 2) the same costs 2.7 us per step, so it is tied to the step's size
+  const int theta_resident = fp.n_entries * F * sizeof(float) <= (96ull << 20) && max_samples >= (1ull << 20);
   switch (F) {
-    case 1: launch_pdl(adam_table_kernel<1>, grid, block, 0, st, fp.theta, fp.mv, fp.grad, first_entry, end_entry, sparse, c, tl); break;
-    case 2: launch_pdl(adam_table_kernel<2>, grid, block, 0, st, fp.theta, fp.mv, fp.grad, first_entry, end_entry, sparse, c, tl); break;
-    case 4: launch_pdl(adam_table_kernel<4>, grid, block, 0, st, fp.theta, fp.mv, fp.grad, first_entry, end_entry, sparse, c, tl); break;
-    default: launch_pdl(adam_table_kernel<8>, grid, block, 0, st, fp.theta, fp.mv, fp.grad, first_entry, end_entry, sparse, c, tl); break;
+    case 1: launch_pdl(adam_table_kernel<1>, grid, block, 0, st, fp.theta, fp.mv, fp.grad, first_entry, end_entry, sparse, c, tl, theta_resident); break;
+    case 2: launch_pdl(adam_table_kernel<2>, grid, block, 0, st, fp.theta, fp.mv, fp.grad, first_entry, end_entry, sparse, c, tl, theta_resident); break;
+    case 4: launch_pdl(adam_table_kernel<4>, grid, block, 0, st, fp.theta, fp.mv, fp.grad, first_entry, end_entry, sparse, c, tl, theta_resident); break;
+    default: launch_pdl(adam_table_kernel<8>, grid, block, 0, st, fp.theta, fp.mv, fp.grad, first_entry, end_entry, sparse, c, tl, theta_resident); break;
   }
   return 1;
 }

@@ -437,7 +437,8 @@ nsm_status enqueue_adam(nsm_field *f) {
     CUDA_TRY(cudaStreamWaitEvent(f->side, f->ev_main, 0));
   }
   RUN(f, K_ADAM_TABLE, launch_adam_table(f->fp, f->cfg.n_features, f->cfg.sparse_table_adam != 0, f->cfg.lr, f->cfg.beta1, f->cfg.beta2,
-                                         f->cfg.eps, (float)(1.0 / bc1), (float)(1.0 / bc2), f->stream, f->ws.timeline));
+                                         f->cfg.eps, (float)(1.0 / bc1), (float)(1.0 / bc2), f->stream, f->ws.timeline,
+                                         (uint64_t)f->last_R * f->last_K));
   if (use_side) {   // to be joined (lazily, join_side): everything later on the main stream must see the new MLP weights
     CUDA_TRY(cudaEventRecord(f->ev_side, f->side));
     f->join_pending = true;

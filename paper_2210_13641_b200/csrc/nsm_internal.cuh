@@ -345,7 +345,7 @@ int launch_composite_render(const Workspace &ws, uint32_t R, float cut, const fl
                             float *out_rgb, float *out_depth, float *out_opacity, cudaStream_t st);
 // S13 on the touched table entries (sparse) or on all of them; consumes the gradients (every word back to "untouched")
 int launch_adam_table(const FieldParams &fp, uint32_t F, int sparse, float lr, float beta1, float beta2,
-                      float eps, float inv_bc1, float inv_bc2, cudaStream_t st, unsigned long long *tl = nullptr);
+                      float eps, float inv_bc1, float inv_bc2, cudaStream_t st, unsigned long long *tl, uint64_t max_samples);
 int launch_adam_mlp(const FieldParams &fp, float lr, float beta1, float beta2, float eps, float inv_bc1,
                     float inv_bc2, cudaStream_t st);
 // tensor-core path: Adam on the MLP weights and, in the same launch, the refreshed 16-bit weight images
