@@ -247,9 +247,9 @@ def kernel_model(name, S, R, K, L, F, U, mac):
 
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, RECORDED from the committed
 # `ncu --set full` capture of this command (bench.py cannot run ncu on itself; refreshed with every committed profile)
-NCU_TRAFFIC = {(4, "adam_table"): 2.746e9}
+NCU_TRAFFIC = {(4, "adam_table"): 2.539e9}
 NCU_TRAFFIC_SOURCE = ("recorded, not measured by this run: dram__bytes_read.sum + dram__bytes_write.sum of one adam_table_kernel<4> launch in the "
-                      "`ncu --set full` capture of `python bench.py --config 4 --only-headline --steps 10 --warmup 3` (profiles/r2b_config4_baseline.md)")
+                      "`ncu --set full` capture of `python bench.py --config 4 --only-headline --steps 10 --warmup 3` (profiles/r2k_table_alignment_and_encoder.md)")
 
 
 def probe_l2(dev_index):
