@@ -256,6 +256,10 @@ nsm_status nsm_debug_set_grad(nsm_field *f, const float *d_grad, const uint8_t *
  * d_rgb [R,3], d_depth [R], d_opacity [R] or NULL.  R may exceed max_rays (chunked). */
 nsm_status nsm_render(nsm_field *f, const nsm_ray_batch *batch, float transmittance_cut,
                       float *d_rgb, float *d_depth, float *d_opacity);
+/* The same with HOST pointers in *host_batch and for the three outputs (pinned or pageable).  The chunks' rays and images
+ * cross the host link by copies on an internal stream, double-buffered, under the kernels of the neighbouring chunks
+ * (pinned buffers; copies of pageable ones block the host).  Synchronises: on return the image is complete and the ray
+ * buffers are free. */
 nsm_status nsm_render_host(nsm_field *f, const nsm_ray_batch *host_batch, float transmittance_cut,
                            float *h_rgb, float *h_depth, float *h_opacity);
 

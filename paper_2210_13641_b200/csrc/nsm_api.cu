@@ -104,8 +104,8 @@ struct nsm_field {
   uint32_t last_R = 0, last_K = 0;
   bool last_was_render = false;
   // staging for the *_host entry points
-  float *stage_dev = nullptr;     // [max_rays * 11]
-  float *stage_out = nullptr;     // render outputs [max_rays * 5]
+  float *stage_dev = nullptr;     // [max_rays * 12]: a training batch (11 floats per ray) or two render buffers (origins | dirs)
+  float *stage_out = nullptr;     // render outputs, two buffers of [max_rays * 5]
   struct HostStats { double acc[3]; uint32_t S; } *pinned = nullptr;   // acc[2] = S of the step, as a double
   // Side stream: work that does not depend on the table Adam runs beside it (it is DRAM-bound, the others
   // are latency-bound): the MLP Adam of the same step and, when the caller has declared its batches ready
@@ -115,6 +115,9 @@ struct nsm_field {
   // the step's statistics (loss sums, S) are final after the compositor: they are copied out on the side stream right
   // behind it, and a call that wants them waits for that copy only, not for the backward pass and Adam
   cudaEvent_t ev_comp = nullptr, ev_stats = nullptr;
+  // nsm_render_host: two staging buffers each way; [j] "rays of buffer j are on the device", "the kernels of buffer j's
+  // chunk are done" (its rays consumed, its image complete), "buffer j's image has been copied out"
+  cudaEvent_t ev_in[2] = {nullptr, nullptr}, ev_done[2] = {nullptr, nullptr}, ev_outfree[2] = {nullptr, nullptr};
   // F1: the keyframe store (library-owned device copies) and its device-side directory
   std::vector<KeyframeDev> kf_host;
   KeyframeDev *kf_dev = nullptr;
@@ -591,7 +594,7 @@ nsm_status nsm_create_field(const nsm_field_config *cfg, void *cuda_stream, nsm_
   ws.dY = ws.dx = nullptr;
   ws.timeline = nullptr;
   A(f->alloc(&ws.loss_acc, 3)); A(f->alloc(&ws.total_samples, 1)); A(f->alloc(&ws.grad_absmax, 1));
-  A(f->alloc(&f->stage_dev, 11 * (size_t)R)); A(f->alloc(&f->stage_out, 5 * (size_t)R));
+  A(f->alloc(&f->stage_dev, 12 * (size_t)R)); A(f->alloc(&f->stage_out, 10 * (size_t)R));
   if (e == cudaSuccess) e = cudaMallocHost((void **)&f->pinned, sizeof(*f->pinned));
   if (e == cudaSuccess) {   // highest priority: the side stream's small grids must not queue behind the table Adam's 3000 blocks
     int prio_lo = 0, prio_hi = 0;
@@ -603,6 +606,11 @@ nsm_status nsm_create_field(const nsm_field_config *cfg, void *cuda_stream, nsm_
   if (e == cudaSuccess) e = cudaEventCreateWithFlags(&f->ev_main, cudaEventDisableTiming);
   if (e == cudaSuccess) e = cudaEventCreateWithFlags(&f->ev_comp, cudaEventDisableTiming);
   if (e == cudaSuccess) e = cudaEventCreateWithFlags(&f->ev_stats, cudaEventDisableTiming);
+  for (int j = 0; j < 2; ++j) {
+    if (e == cudaSuccess) e = cudaEventCreateWithFlags(&f->ev_in[j], cudaEventDisableTiming);
+    if (e == cudaSuccess) e = cudaEventCreateWithFlags(&f->ev_done[j], cudaEventDisableTiming);
+    if (e == cudaSuccess) e = cudaEventCreateWithFlags(&f->ev_outfree[j], cudaEventDisableTiming);
+  }
   if (e != cudaSuccess) {
     nsm_destroy_field(f);
     cudaGetLastError();
@@ -623,6 +631,11 @@ void nsm_destroy_field(nsm_field *f) {
   if (f->ev_main) cudaEventDestroy(f->ev_main);
   if (f->ev_comp) cudaEventDestroy(f->ev_comp);
   if (f->ev_stats) cudaEventDestroy(f->ev_stats);
+  for (int j = 0; j < 2; ++j) {
+    if (f->ev_in[j]) cudaEventDestroy(f->ev_in[j]);
+    if (f->ev_done[j]) cudaEventDestroy(f->ev_done[j]);
+    if (f->ev_outfree[j]) cudaEventDestroy(f->ev_outfree[j]);
+  }
   f->prof.destroy();
   for (void *p : f->allocs) cudaFree(p);
   if (f->pinned) cudaFreeHost(f->pinned);
@@ -1068,6 +1081,62 @@ nsm_status nsm_debug_set_grad(nsm_field *f, const float *d_grad, const uint8_t *
   return NSM_OK;
 }
 
+// nsm_render_host: the chunks' rays go in and their images come out by copies on the side stream, through two staging
+// buffers each way, while the field's stream renders: chunk i + 1's rays arrive and chunk i - 1's image leaves under chunk
+// i's kernels (config 5: the copies are 36 MB per view, 1.1 ms at the host link's rate, and were serialised with the
+// kernels before: 6.96 -> 5.94 ms per view end to end, 137 M rays/s against 139 M with device buffers).  Unlike a training batch a frame is not read in place from pinned memory:
+// with the marcher fetching 24 B per ray and the compositor storing 20 B per ray over the host link a 816 000-ray view
+// took 8.85 ms.  Pageable buffers work too (their copies block the host).  Synchronises: on return the image is in the
+// host buffers and the rays are free.
+static nsm_status render_chunks_host(nsm_field *f, const nsm_ray_batch *b, float cut, float *rgb, float *depth, float *opacity) {
+  const uint32_t M = f->cfg.max_rays;
+  const uint32_t n_chunks = (b->n_rays + M - 1) / M;
+  auto rays_of = [&](uint32_t i) { return (b->n_rays - i * M < M) ? b->n_rays - i * M : M; };
+  auto copy_in = [&](uint32_t i) -> cudaError_t {   // side stream: rays of chunk i -> staging buffer i & 1
+    const uint32_t j = i & 1u, R = rays_of(i);
+    float *p = f->stage_dev + (size_t)j * 6 * M;
+    cudaError_t e = cudaSuccess;
+    if (i >= 2) e = cudaStreamWaitEvent(f->side, f->ev_done[j], 0);   // the chunk that used this buffer has consumed it
+    if (e == cudaSuccess) e = cudaMemcpyAsync(p, b->origins + 3 * (size_t)i * M, sizeof(float) * 3 * R, cudaMemcpyHostToDevice, f->side);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(p + 3 * (size_t)M, b->dirs + 3 * (size_t)i * M, sizeof(float) * 3 * R, cudaMemcpyHostToDevice, f->side);
+    if (e == cudaSuccess) e = cudaEventRecord(f->ev_in[j], f->side);
+    return e;
+  };
+  // the side stream starts behind everything enqueued on the field's stream so far
+  CUDA_TRY(cudaEventRecord(f->ev_main, f->stream));
+  CUDA_TRY(cudaStreamWaitEvent(f->side, f->ev_main, 0));
+  CUDA_TRY(copy_in(0));
+  for (uint32_t i = 0; i < n_chunks; ++i) {
+    const uint32_t j = i & 1u, R = rays_of(i);
+    const size_t first = (size_t)i * M;
+    if (i + 1 < n_chunks) CUDA_TRY(copy_in(i + 1));
+    nsm_ray_batch cb = *b;
+    cb.n_rays = R;
+    cb.origins = f->stage_dev + (size_t)j * 6 * M;
+    cb.dirs = cb.origins + 3 * (size_t)M;
+    float *o = f->stage_out + (size_t)j * 5 * M;
+    CUDA_TRY(cudaStreamWaitEvent(f->stream, f->ev_in[j], 0));
+    if (i >= 2) CUDA_TRY(cudaStreamWaitEvent(f->stream, f->ev_outfree[j], 0));   // this output buffer's last image is out
+    nsm_status st = enqueue_forward(f, &cb, R, false, 0, false);
+    if (st != NSM_OK) return st;
+    RUN(f, K_COMPOSITE, launch_composite_render(f->ws, R, cut, f->cfg.bg, o, o + 3 * (size_t)M, o + 4 * (size_t)M, f->stream));
+    if (f->prof.on) f->prof.collect();
+    CUDA_TRY(cudaEventRecord(f->ev_done[j], f->stream));
+    CUDA_TRY(cudaStreamWaitEvent(f->side, f->ev_done[j], 0));
+    CUDA_TRY(cudaMemcpyAsync(rgb + 3 * first, o, sizeof(float) * 3 * R, cudaMemcpyDeviceToHost, f->side));
+    CUDA_TRY(cudaMemcpyAsync(depth + first, o + 3 * (size_t)M, sizeof(float) * R, cudaMemcpyDeviceToHost, f->side));
+    if (opacity) CUDA_TRY(cudaMemcpyAsync(opacity + first, o + 4 * (size_t)M, sizeof(float) * R, cudaMemcpyDeviceToHost, f->side));
+    CUDA_TRY(cudaEventRecord(f->ev_outfree[j], f->side));
+    f->last_R = R;
+    f->last_K = b->n_candidates;
+    f->last_was_render = true;
+  }
+  CUDA_TRY(cudaStreamSynchronize(f->side));     // the last image copy is behind every kernel
+  CUDA_TRY(cudaStreamSynchronize(f->stream));
+  CUDA_TRY(cudaGetLastError());
+  return NSM_OK;
+}
+
 static nsm_status render_chunks(nsm_field *f, const nsm_ray_batch *b, float cut, float *rgb, float *depth, float *opacity,
                                 bool host) {
   nsm_status st = validate_batch(f, b, false, true);
@@ -1076,29 +1145,18 @@ static nsm_status render_chunks(nsm_field *f, const nsm_ray_batch *b, float cut,
   if (!rgb || !depth) return fail(NSM_ERR_INVALID_ARG, "output pointers are NULL");
   if (!(cut >= 0.f)) return fail(NSM_ERR_INVALID_ARG, "transmittance_cut must be >= 0");
   const uint32_t M = f->cfg.max_rays;
+  if (host) return render_chunks_host(f, b, cut, rgb, depth, opacity);
   for (uint32_t first = 0; first < b->n_rays; first += M) {
     const uint32_t R = (b->n_rays - first < M) ? b->n_rays - first : M;
     nsm_ray_batch cb = *b;
     cb.n_rays = R;
-    float *o_rgb = rgb + 3 * (size_t)first, *o_d = depth + first, *o_op = opacity ? opacity + first : nullptr;
-    if (host) {
-      st = stage_batch(f, b, first, R, false, &cb);
-      if (st != NSM_OK) return st;
-      o_rgb = f->stage_out; o_d = f->stage_out + 3 * (size_t)M; o_op = f->stage_out + 4 * (size_t)M;
-    } else {
-      cb.origins = b->origins + 3 * (size_t)first;
-      cb.dirs = b->dirs + 3 * (size_t)first;
-    }
+    cb.origins = b->origins + 3 * (size_t)first;
+    cb.dirs = b->dirs + 3 * (size_t)first;
     st = enqueue_forward(f, &cb, R, false, 0, false);
     if (st != NSM_OK) return st;
-    RUN(f, K_COMPOSITE, launch_composite_render(f->ws, R, cut, f->cfg.bg, o_rgb, o_d, o_op, f->stream));
+    RUN(f, K_COMPOSITE, launch_composite_render(f->ws, R, cut, f->cfg.bg, rgb + 3 * (size_t)first, depth + first,
+                                                opacity ? opacity + first : nullptr, f->stream));
     if (f->prof.on) f->prof.collect();
-    if (host) {
-      CUDA_TRY(cudaMemcpyAsync(rgb + 3 * (size_t)first, o_rgb, sizeof(float) * 3 * R, cudaMemcpyDeviceToHost, f->stream));
-      CUDA_TRY(cudaMemcpyAsync(depth + first, o_d, sizeof(float) * R, cudaMemcpyDeviceToHost, f->stream));
-      if (opacity) CUDA_TRY(cudaMemcpyAsync(opacity + first, o_op, sizeof(float) * R, cudaMemcpyDeviceToHost, f->stream));
-      CUDA_TRY(cudaStreamSynchronize(f->stream));  // staging buffers are reused by the next chunk
-    }
     f->last_R = R;
     f->last_K = b->n_candidates;
     f->last_was_render = true;

@@ -285,8 +285,12 @@ def test_render_parity(nsm, precision, shape):
         assert np.abs(opa - o_ref).max() <= tol + allow
     # chunked render (R > max_rays) and the host entry point give the same image
     assert view.n_rays > fc.max_rays
-    out = f.nsm_render_host(nsm.HostBatch(view), 1e-4)
-    assert np.array_equal(out[0].numpy(), rgb) and np.array_equal(out[1].numpy(), dep)
+    out = f.nsm_render_host(nsm.HostBatch(view), 1e-4)      # pinned: rays read in place, image written in place
+    assert np.array_equal(out[0].numpy(), rgb) and np.array_equal(out[1].numpy(), dep) and np.array_equal(out[2].numpy(), opa)
+    import torch
+    pageable = (torch.empty((view.n_rays, 3)), torch.empty(view.n_rays), torch.empty(view.n_rays))
+    out = f.nsm_render_host(nsm.HostBatch(view, pinned=False), 1e-4, out=pageable)   # staged by copies, chunk by chunk
+    assert np.array_equal(out[0].numpy(), rgb) and np.array_equal(out[1].numpy(), dep) and np.array_equal(out[2].numpy(), opa)
     f.close()
 
 
