@@ -828,3 +828,43 @@ def test_other_feature_widths(nsm, F, L, log2T):
     untouched = np.abs(O.m[:O.n_table]) == 0
     assert np.array_equal(th[:O.n_table][untouched], theta0[:O.n_table][untouched])
     f.close()
+
+
+@pytest.mark.parametrize("F,L,log2T,n_min,n_max", [(1, 6, 12, 4, 48), (2, 7, 13, 4, 64), (4, 5, 10, 6, 40), (8, 3, 11, 4, 48)])
+def test_canonical_layout_round_trip(nsm, F, L, log2T, n_min, n_max):
+    """The storage arrays start every level on a 64-byte boundary; include/nsm.h's layout (levels back to back) exists at
+    the boundary only.  With dense levels of odd size (so that every later level is shifted by padding entries): the level
+    table reports the canonical offsets; theta, m, v and a gradient with its touched flags come back bit for bit through
+    nsm_set_params / nsm_get_params and nsm_debug_set_grad / nsm_debug_last_step; an Adam step on that gradient changes
+    exactly the flagged entries."""
+    w = configs.config1(variant_b=True)
+    fc = replace(w.field, n_features=F, n_levels=L, log2_table_size=log2T, n_min=n_min, n_max=n_max)
+    f = nsm.Field(fc, "cuda:0")
+    O = orc.Oracle(fc, np.zeros(f.n_table + f.n_mlp, np.float32))
+    assert np.array_equal(O.offset, f.offset) and f.n_table == int(O.offset[L]) * F
+    sizes = np.diff(np.asarray(O.offset, np.int64))
+    assert (sizes[:-1] % max(16 // F, 1) != 0).any()                       # some level is followed by padding
+    rng = np.random.default_rng(40 + F)
+    P = f.n_table + f.n_mlp
+    th, m, v = (rng.standard_normal(P).astype(np.float32) for _ in range(3))
+    v = np.abs(v)
+    f.nsm_set_params(th, m, v, step=3)
+    th2, m2, v2, step = f.nsm_get_params()
+    assert step == 3
+    for a, b in ((th, th2), (m, m2), (v, v2)):
+        assert np.array_equal(a.view(np.uint32), b.view(np.uint32))
+    n_entries = f.n_table // F
+    grad = rng.standard_normal(P).astype(np.float32)
+    touched = (rng.uniform(size=n_entries) < 0.3).astype(np.uint8)
+    grad[:f.n_table][np.repeat(touched == 0, F)] = 0.0
+    f.nsm_backward(nsm.DeviceBatch(w.batches[0]), w.lambda_d)             # the debug getters want a step; its gradient is overwritten
+    f.nsm_debug_set_grad(grad, touched)
+    assert np.array_equal(f.nsm_debug_last_step("touched"), touched)
+    assert np.array_equal(f.nsm_debug_last_step("grad"), grad)            # untouched words read -0.0 == 0.0
+    f.nsm_apply_adam()
+    th3, m3, v3, step = f.nsm_get_params()
+    assert step == 4
+    changed = (th3[:f.n_table] != th[:f.n_table]).reshape(n_entries, F).any(axis=1)
+    moved = (m3[:f.n_table] != m[:f.n_table]).reshape(n_entries, F).any(axis=1)
+    assert np.array_equal(moved, touched.astype(bool)) and not (changed & ~touched.astype(bool)).any()
+    f.close()
