@@ -25,10 +25,11 @@ using namespace tableops;
 // the last tile beyond S are zero-filled so the MMA never reads stale data.
 // TWO_TERM = false (forward-only uses: render, occupancy refresh -- their MLP kernel reads the hi tile only): the lo term is
 // neither computed nor stored.
-// F >= 4: capped at 64 registers (80 otherwise) for four blocks per SM: with tables beyond the L2 the kernel waits for
-// DRAM and a fourth block's gathers in flight are worth 2 % (config 4: 148.8 -> 146.2 us; five blocks spill: 151.8 us)
+// F = 4: capped at 64 registers (80 otherwise) for four blocks per SM: with tables beyond the L2 the kernel waits for
+// DRAM and a fourth block's gathers in flight are worth 2 % (config 4: 148.8 -> 146.2 us; five blocks spill: 151.8 us).
+// (0 = no minimum, the compiler's own choice: 47 registers at F = 2; a minimum of 1 lets it take 72.)
 template <int F, int MODE, bool TWO_TERM = true>
-__global__ void __launch_bounds__(256, F >= 4 ? 4 : 1) encode_forward_kernel(LevelTable lv, const float *__restrict__ theta,
+__global__ void __launch_bounds__(256, F == 4 ? 4 : 0) encode_forward_kernel(LevelTable lv, const float *__restrict__ theta,
                                                              Workspace ws, const uint32_t *__restrict__ d_S, uint32_t seq) {
   __shared__ uint32_t chunk_s;
   pdl_wait();
