@@ -35,8 +35,10 @@ __global__ void __launch_bounds__(ADAM_THREADS) adam_table_kernel(float *__restr
   // kernel walks the levels upwards there, so the gradient lines it wrote last -- the finest levels' -- are the ones
   // still (dirty) in the L2, and the coarse levels this kernel then ends with are what the next encoder starts with
   // (config 4: adam_table 509 -> 494 us, encode 146 -> 142 us).  With tables inside the L2 it costs (config 2: +2.3 us).
+  // In that order the theta stores also take the default policy instead of evict_first (486 us; the moment records'
+  // stores stay evict_first: 494 us with both default).
   const uint32_t chunk = reverse ? gridDim.x - 1 - blockIdx.x : blockIdx.x;
-  adam_chunk<F>(theta, mv, grad, first_entry + (uint64_t)chunk * CH, n_entries, sparse, c, list_g, list_e, &cnt, theta_resident);
+  adam_chunk<F>(theta, mv, grad, first_entry + (uint64_t)chunk * CH, n_entries, sparse, c, list_g, list_e, &cnt, theta_resident || reverse);
   tl_mark(tl, K_ADAM_TABLE, 1);
 }
 
