@@ -30,7 +30,8 @@ using namespace tableops;
 // (0 = no minimum, the compiler's own choice: 47 registers at F = 2; a minimum of 1 lets it take 72.)
 template <int F, int MODE, bool TWO_TERM = true>
 __global__ void __launch_bounds__(256, F == 4 ? 4 : 0) encode_forward_kernel(LevelTable lv, const float *__restrict__ theta,
-                                                             Workspace ws, const uint32_t *__restrict__ d_S, uint32_t seq) {
+                                                             Workspace ws, const uint32_t *__restrict__ d_S, uint32_t seq,
+                                                             uint32_t stream_hashed) {
   __shared__ uint32_t chunk_s;
   pdl_wait();
   pdl_trigger();
@@ -77,8 +78,12 @@ __global__ void __launch_bounds__(256, F == 4 ? 4 : 0) encode_forward_kernel(Lev
       for (int f = 0; f < F; ++f) v[k][f] = 0.f;
     if (gathers) {
       const float *tab = theta + lv.offset[l] * F;
-      // coarse (dense) levels are re-read every step: default policy; hashed levels stream through L2
-      if (lv.dense[l]) gather_corners<F, NSM_L2_EVICT_NORMAL>(tab, ci.slot, v);
+      // coarse (dense) levels are re-read every step: default policy.  Hashed levels: evict_first where the tables are
+      // L2-sized and a small step references an entry less than once (stream_hashed, config 2: the lines would only push the
+      // gradient array out, scatter 19 -> 24 us with the default policy); default where the tables dwarf the L2 (config 4:
+      // a fetched sector is met again by the next samples of the ray within microseconds, and "evict first" lines do not
+      // live that long under 0.5 GB of misses: encode 142 -> 117 us)
+      if (lv.dense[l] || !stream_hashed) gather_corners<F, NSM_L2_EVICT_NORMAL>(tab, ci.slot, v);
       else gather_corners<F, NSM_L2_EVICT_FIRST>(tab, ci.slot, v);
     }
     if (one_dense_level) {
@@ -437,22 +442,23 @@ int launch_unpack_records(const FieldParams &fp, int which, float *dst, cudaStre
 
 template <int F, bool TT>
 static void launch_encode_ft(const LevelTable &lv, const float *theta, const Workspace &ws, const uint32_t *d_S, int out_mode,
-                             dim3 grid, dim3 block, cudaStream_t st, uint32_t seq, bool per_panel) {
+                             dim3 grid, dim3 block, cudaStream_t st, uint32_t seq, bool per_panel, uint32_t stream_hashed) {
   if (out_mode == 1) {
     if (per_panel) launch_pdl(encode_forward_panel_kernel<F, 1, TT>, grid, block, 0, st, lv, theta, ws, d_S, seq);
-    else launch_pdl(encode_forward_kernel<F, 1, TT>, grid, block, 0, st, lv, theta, ws, d_S, seq);
+    else launch_pdl(encode_forward_kernel<F, 1, TT>, grid, block, 0, st, lv, theta, ws, d_S, seq, stream_hashed);
   } else {
     if (per_panel) launch_pdl(encode_forward_panel_kernel<F, 2, TT>, grid, block, 0, st, lv, theta, ws, d_S, seq);
-    else launch_pdl(encode_forward_kernel<F, 2, TT>, grid, block, 0, st, lv, theta, ws, d_S, seq);
+    else launch_pdl(encode_forward_kernel<F, 2, TT>, grid, block, 0, st, lv, theta, ws, d_S, seq, stream_hashed);
   }
 }
 
 template <int F>
 static void launch_encode_f(const LevelTable &lv, const float *theta, const Workspace &ws, const uint32_t *d_S, int out_mode,
-                            dim3 grid, dim3 block, cudaStream_t st, uint32_t seq, bool per_panel, bool two_term) {
-  if (out_mode == 0) launch_pdl(encode_forward_kernel<F, 0>, grid, block, 0, st, lv, theta, ws, d_S, seq);
-  else if (two_term) launch_encode_ft<F, true>(lv, theta, ws, d_S, out_mode, grid, block, st, seq, per_panel);
-  else launch_encode_ft<F, false>(lv, theta, ws, d_S, out_mode, grid, block, st, seq, per_panel);
+                            dim3 grid, dim3 block, cudaStream_t st, uint32_t seq, bool per_panel, bool two_term,
+                            uint32_t stream_hashed) {
+  if (out_mode == 0) launch_pdl(encode_forward_kernel<F, 0>, grid, block, 0, st, lv, theta, ws, d_S, seq, stream_hashed);
+  else if (two_term) launch_encode_ft<F, true>(lv, theta, ws, d_S, out_mode, grid, block, st, seq, per_panel, stream_hashed);
+  else launch_encode_ft<F, false>(lv, theta, ws, d_S, out_mode, grid, block, st, seq, per_panel, stream_hashed);
 }
 
 int launch_encode(const LevelTable &lv, const float *theta, const Workspace &ws, const uint32_t *d_S, int out_mode,
@@ -466,11 +472,12 @@ int launch_encode(const LevelTable &lv, const float *theta, const Workspace &ws,
   // uses the step's upper bound, rays x candidates.
   const bool l2_resident = lv.offset[lv.n_levels] * lv.n_features * sizeof(float) <= (96ull << 20);
   const bool per_panel = out_mode != 0 && l2_resident && max_samples >= (1ull << 20);
+  const uint32_t stream_hashed = l2_resident ? 1u : 0u;   // the thread-per-(level, sample) kernel's hashed-level gather policy
   switch (lv.n_features) {
-    case 1: launch_encode_f<1>(lv, theta, ws, d_S, out_mode, grid, block, st, seq, per_panel, two_term); break;
-    case 2: launch_encode_f<2>(lv, theta, ws, d_S, out_mode, grid, block, st, seq, per_panel, two_term); break;
-    case 4: launch_encode_f<4>(lv, theta, ws, d_S, out_mode, grid, block, st, seq, per_panel, two_term); break;
-    default: launch_encode_f<8>(lv, theta, ws, d_S, out_mode, grid, block, st, seq, per_panel, two_term); break;
+    case 1: launch_encode_f<1>(lv, theta, ws, d_S, out_mode, grid, block, st, seq, per_panel, two_term, stream_hashed); break;
+    case 2: launch_encode_f<2>(lv, theta, ws, d_S, out_mode, grid, block, st, seq, per_panel, two_term, stream_hashed); break;
+    case 4: launch_encode_f<4>(lv, theta, ws, d_S, out_mode, grid, block, st, seq, per_panel, two_term, stream_hashed); break;
+    default: launch_encode_f<8>(lv, theta, ws, d_S, out_mode, grid, block, st, seq, per_panel, two_term, stream_hashed); break;
   }
   return 1;
 }
