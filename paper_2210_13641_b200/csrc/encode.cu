@@ -307,8 +307,13 @@ __global__ void __launch_bounds__(256) scatter_backward_kernel(LevelTable lv, fl
         if (!lv.dense[ln]) {
           const CornerIndex cn = corner_index(lv, ln, ws.s_x[sn], ws.s_x[ws.cap + sn], ws.s_x[2 * ws.cap + sn]);
           const float *tab = grad + lv.offset[ln] * F;
+          // one request per sector: an x-neighbour pair (slots s, s ^ 1) lies in one 32-byte sector for F <= 4 (EntryMap)
 #pragma unroll
-          for (int k = 0; k < 8; ++k) asm volatile("prefetch.global.L2::evict_last [%0];" ::"l"(tab + (size_t)cn.slot[k] * F));
+          for (int k = 0; k < 8; k += 2) {
+            asm volatile("prefetch.global.L2::evict_last [%0];" ::"l"(tab + (size_t)cn.slot[k] * F));
+            if (F > 4 || (cn.slot[k] ^ cn.slot[k + 1]) != 1u)
+              asm volatile("prefetch.global.L2::evict_last [%0];" ::"l"(tab + (size_t)cn.slot[k + 1] * F));
+          }
         }
       }
     }
