@@ -113,7 +113,9 @@ constexpr uint32_t MARCH_WARPS = 16;
 constexpr uint32_t MARCH_MAX_WORDS = 128;        // K <= 4096 (validate_config)
 constexpr uint64_t SCAN_AGG = 1ull << 32, SCAN_INCL = 2ull << 32;
 
-__global__ void __launch_bounds__(MARCH_WARPS * 32) march_fused_kernel(MarchParams mp, const uint8_t *bits,
+// Four blocks per SM (32 registers instead of 38, 16 bytes of spill): the kernel is issue- and barrier-bound, and a
+// fourth block's warps fill the chained scan's waits (config 5: 1240 -> 1164 us per 816 000-ray view).
+__global__ void __launch_bounds__(MARCH_WARPS * 32, 4) march_fused_kernel(MarchParams mp, const uint8_t *bits,
                                                                        const float *__restrict__ origins,
                                                                        const float *__restrict__ dirs, Workspace ws,
                                                                        int count_total, float *__restrict__ dirs_copy) {
