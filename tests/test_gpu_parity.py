@@ -474,6 +474,9 @@ def test_config5_full_frame_render_on_sampled_rays(nsm):
     assert np.abs(opa[:n] - o_ref).max() <= tol + allow
     assert np.isfinite(rgb).all() and rgb.min() >= -1e-6 and rgb.max() <= 1 + 1e-5
     assert opa.min() >= -1e-6 and opa.max() <= 1 + 1e-5 and dep.min() >= 0 and dep.max() <= view.t_max * (1 + 1e-5)
+    # the host entry point: 13 chunks through the two staging buffers each way, copies under the neighbouring chunks' kernels
+    out = f.nsm_render_host(nsm.HostBatch(view), 1e-4)
+    assert np.array_equal(out[0].numpy(), rgb) and np.array_equal(out[1].numpy(), dep) and np.array_equal(out[2].numpy(), opa)
     f.close()
 
 
